@@ -1,0 +1,536 @@
+/*
+ * oracle/vmg_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU implementation (fp64, triple loops) of the path the CUDA library
+ * computes: cell-centred geometric multigrid for
+ *
+ *        alpha * a * phi  -  beta * div( b grad phi )  =  f        (uniform Cartesian box)
+ *
+ * the "Helmholtz equation form" every governing equation is cast into (sec. 4): Poisson
+ * Eq. 3, implicit diffusion of Eq. 17, photoionisation Eq. 9
+ * (PAPER.md:83).  Discretisation: finite volume on Cartesian cells, second-order central diffusive flux,
+ * implicit (sec. 3).  The paper names "multigrid" and nothing else; the
+ * components are those BASELINE.json:north_star lists, read as SURVEY.md sec. 8(c) C1-C5 / DESIGN.md
+ * "Readings".  Nothing here is blocked, fused or reordered beyond those statements.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may load this.
+ * It shares no code with paper_2507_08200_b200/csrc and neither includes the other.
+ *
+ * Parity pins (tests/test_oracle_pins.py): dense LAPACK solve on 8^3 / 16x8x8, manufactured solutions at
+ * second order (configs 1, 2), the paper's printed closed form phi = (x^4 - x)/12 (PAPER.md:186-194,
+ * Eq. 24-27), exactness for linear phi, symmetry / positive definiteness, constant-vector row sums,
+ * axis-permutation invariance, per-cycle contraction < 0.2.  No function here is "parity unpinned".
+ *
+ * Layout (x fastest): cell arrays idx = i + nx*(j + ny*k); bx (nx+1)*ny*nz, idx = i + (nx+1)*(j + ny*k),
+ * face i lies between cells i-1 and i; by nx*(ny+1)*nz, idx = i + nx*(j + (ny+1)*k); bz nx*ny*(nz+1).
+ * BC value planes: x faces j + ny*k, y faces i + nx*k, z faces i + nx*j.  nz == 1 selects the 2-D operator.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+enum { XLO = 0, XHI = 1, YLO = 2, YHI = 3, ZLO = 4, ZHI = 5 };
+enum { BC_DIRICHLET = 0, BC_NEUMANN = 1 };
+enum { O_OK = 0, O_MAXCYCLES = 1, O_STALLED = 2, O_ERR_ARG = -1, O_ERR_SIZE = -2, O_ERR_STATE = -3,
+       O_ERR_SINGULAR = -4, O_ERR_DIVERGED = -5 };
+
+typedef struct {
+    int nx, ny, nz;
+    double hx, hy, hz;
+    double *a, *bx, *by, *bz;   /* coefficients of this level (owned) */
+    double *phi, *rhs, *res;    /* work arrays of this level (owned) */
+} olevel;
+
+typedef struct ovmg {
+    int nlev, three_d;
+    olevel *lev;
+    double alpha, beta;
+    int bctype[6];
+    double *bcval[6];           /* level-0 value planes (owned copies; NULL = homogeneous) */
+    int have_coeffs, have_bc;
+    int nu1, nu2, nbottom;
+    int cycles, status;
+    double relres;
+    double *hist;
+    int hist_len;
+} ovmg;
+
+static size_t ncell(const olevel *L) { return (size_t)L->nx * L->ny * L->nz; }
+static size_t CI(const olevel *L, int i, int j, int k) { return i + (size_t)L->nx * (j + (size_t)L->ny * k); }
+static size_t XI(const olevel *L, int i, int j, int k) { return i + (size_t)(L->nx + 1) * (j + (size_t)L->ny * k); }
+static size_t YI(const olevel *L, int i, int j, int k) { return i + (size_t)L->nx * (j + (size_t)(L->ny + 1) * k); }
+static size_t ZI(const olevel *L, int i, int j, int k) { return i + (size_t)L->nx * (j + (size_t)L->ny * k); }
+
+/* ---------------------------------------------------------------------------------------------
+ * C1. The stencil of cell (i,j,k): neighbour weights w[6] (order XLO..ZHI; 0 where the face is a
+ * domain boundary) and the diagonal D.  Interior face: w = beta*b_face/h^2 on the diagonal and as
+ * the coupling.  Dirichlet boundary face: 2w on the diagonal (value half a cell away), no coupling.
+ * Neumann boundary face: nothing.
+ * --------------------------------------------------------------------------------------------- */
+static void stencil(const ovmg *h, const olevel *L, int i, int j, int k, double w[6], double *D)
+{
+    double b[6], hh[6];
+    int nd = h->three_d ? 6 : 4, f;
+    int at_bnd[6];
+    b[XLO] = L->bx[XI(L, i, j, k)];     b[XHI] = L->bx[XI(L, i + 1, j, k)];
+    b[YLO] = L->by[YI(L, i, j, k)];     b[YHI] = L->by[YI(L, i, j + 1, k)];
+    at_bnd[XLO] = (i == 0);             at_bnd[XHI] = (i == L->nx - 1);
+    at_bnd[YLO] = (j == 0);             at_bnd[YHI] = (j == L->ny - 1);
+    hh[XLO] = hh[XHI] = L->hx;          hh[YLO] = hh[YHI] = L->hy;
+    if (h->three_d) {
+        b[ZLO] = L->bz[ZI(L, i, j, k)]; b[ZHI] = L->bz[ZI(L, i, j, k + 1)];
+        at_bnd[ZLO] = (k == 0);         at_bnd[ZHI] = (k == L->nz - 1);
+        hh[ZLO] = hh[ZHI] = L->hz;
+    }
+    *D = h->alpha * (L->a ? L->a[CI(L, i, j, k)] : 0.0);
+    for (f = 0; f < 6; ++f) w[f] = 0.0;
+    for (f = 0; f < nd; ++f) {
+        double wf = h->beta * b[f] / (hh[f] * hh[f]);
+        if (!at_bnd[f]) { w[f] = wf; *D += wf; }
+        else if (h->bctype[f] == BC_DIRICHLET) { *D += 2.0 * wf; }
+    }
+}
+
+static double nbsum(const olevel *L, const double *phi, int i, int j, int k, const double w[6])
+{
+    double s = 0.0;
+    if (w[XLO] != 0.0) s += w[XLO] * phi[CI(L, i - 1, j, k)];
+    if (w[XHI] != 0.0) s += w[XHI] * phi[CI(L, i + 1, j, k)];
+    if (w[YLO] != 0.0) s += w[YLO] * phi[CI(L, i, j - 1, k)];
+    if (w[YHI] != 0.0) s += w[YHI] * phi[CI(L, i, j + 1, k)];
+    if (w[ZLO] != 0.0) s += w[ZLO] * phi[CI(L, i, j, k - 1)];
+    if (w[ZHI] != 0.0) s += w[ZHI] * phi[CI(L, i, j, k + 1)];
+    return s;
+}
+
+/* (A phi)_c = D_c phi_c - sum_interior w phi_nb   (homogeneous-BC operator of level lev) */
+static void apply_level(const ovmg *h, int lev, const double *phi, double *out)
+{
+    const olevel *L = &h->lev[lev];
+    int i, j, k;
+#pragma omp parallel for collapse(2) private(i)
+    for (k = 0; k < L->nz; ++k)
+        for (j = 0; j < L->ny; ++j)
+            for (i = 0; i < L->nx; ++i) {
+                double w[6], D;
+                stencil(h, L, i, j, k, w, &D);
+                out[CI(L, i, j, k)] = D * phi[CI(L, i, j, k)] - nbsum(L, phi, i, j, k, w);
+            }
+}
+
+/* r = rhs - A phi */
+static void residual_level(const ovmg *h, int lev, const double *phi, const double *rhs, double *r)
+{
+    const olevel *L = &h->lev[lev];
+    int i, j, k;
+#pragma omp parallel for collapse(2) private(i)
+    for (k = 0; k < L->nz; ++k)
+        for (j = 0; j < L->ny; ++j)
+            for (i = 0; i < L->nx; ++i) {
+                double w[6], D;
+                stencil(h, L, i, j, k, w, &D);
+                r[CI(L, i, j, k)] = rhs[CI(L, i, j, k)] - (D * phi[CI(L, i, j, k)] - nbsum(L, phi, i, j, k, w));
+            }
+}
+
+/* C2. One red-black Gauss-Seidel sweep: red = (i+j+k) even first, then black; no over-relaxation. */
+static void smooth_level(const ovmg *h, int lev, double *phi, const double *rhs, int nsweeps)
+{
+    const olevel *L = &h->lev[lev];
+    int s, colour, i, j, k;
+    for (s = 0; s < nsweeps; ++s)
+        for (colour = 0; colour < 2; ++colour) {
+#pragma omp parallel for collapse(2) private(i)
+            for (k = 0; k < L->nz; ++k)
+                for (j = 0; j < L->ny; ++j)
+                    for (i = 0; i < L->nx; ++i) {
+                        double w[6], D;
+                        if (((i + j + k) & 1) != colour) continue;
+                        stencil(h, L, i, j, k, w, &D);
+                        phi[CI(L, i, j, k)] = (rhs[CI(L, i, j, k)] + nbsum(L, phi, i, j, k, w)) / D;
+                    }
+        }
+}
+
+/* C3. Restriction: coarse rhs = mean of the 8 (4 in 2-D) children of the fine residual. */
+static void restrict_level(const ovmg *h, int lev, const double *rfine, double *rcoarse)
+{
+    const olevel *F = &h->lev[lev], *C = &h->lev[lev + 1];
+    int sz = h->three_d ? 2 : 1, I, J, K, p, q, s;
+    for (K = 0; K < C->nz; ++K)
+        for (J = 0; J < C->ny; ++J)
+            for (I = 0; I < C->nx; ++I) {
+                double sum = 0.0;
+                for (s = 0; s < sz; ++s)
+                    for (q = 0; q < 2; ++q)
+                        for (p = 0; p < 2; ++p)
+                            sum += rfine[CI(F, 2 * I + p, 2 * J + q, sz * K + s)];
+                rcoarse[CI(C, I, J, K)] = sum / (4.0 * sz);
+            }
+}
+
+/* C3. Prolongation + correction: piecewise constant, phi_f[i,j,k] += e_c[i/2, j/2, k/2]. */
+static void prolong_add_level(const ovmg *h, int lev, double *phifine, const double *ecoarse)
+{
+    const olevel *F = &h->lev[lev], *C = &h->lev[lev + 1];
+    int i, j, k;
+    for (k = 0; k < F->nz; ++k)
+        for (j = 0; j < F->ny; ++j)
+            for (i = 0; i < F->nx; ++i)
+                phifine[CI(F, i, j, k)] += ecoarse[CI(C, i / 2, j / 2, h->three_d ? k / 2 : k)];
+}
+
+/* C3 / R10. Coarse coefficients: a = mean of the children; b on a coarse face = mean of the fine
+ * faces lying on it (4 in 3-D, 2 in 2-D).  The coarse operator is the re-discretisation C1 with 2h. */
+static void average_coeffs(const ovmg *h, int lev)
+{
+    const olevel *F = &h->lev[lev];
+    olevel *C = &h->lev[lev + 1];
+    int sz = h->three_d ? 2 : 1, I, J, K, p, q, s;
+    for (K = 0; K < C->nz; ++K)
+        for (J = 0; J < C->ny; ++J)
+            for (I = 0; I < C->nx; ++I) {
+                double sum = 0.0;
+                for (s = 0; s < sz; ++s) for (q = 0; q < 2; ++q) for (p = 0; p < 2; ++p)
+                    sum += F->a[CI(F, 2 * I + p, 2 * J + q, sz * K + s)];
+                C->a[CI(C, I, J, K)] = sum / (4.0 * sz);
+            }
+    for (K = 0; K < C->nz; ++K)
+        for (J = 0; J < C->ny; ++J)
+            for (I = 0; I <= C->nx; ++I) {
+                double sum = 0.0;
+                for (s = 0; s < sz; ++s) for (q = 0; q < 2; ++q)
+                    sum += F->bx[XI(F, 2 * I, 2 * J + q, sz * K + s)];
+                C->bx[XI(C, I, J, K)] = sum / (2.0 * sz);
+            }
+    for (K = 0; K < C->nz; ++K)
+        for (J = 0; J <= C->ny; ++J)
+            for (I = 0; I < C->nx; ++I) {
+                double sum = 0.0;
+                for (s = 0; s < sz; ++s) for (p = 0; p < 2; ++p)
+                    sum += F->by[YI(F, 2 * I + p, 2 * J, sz * K + s)];
+                C->by[YI(C, I, J, K)] = sum / (2.0 * sz);
+            }
+    if (h->three_d)
+        for (K = 0; K <= C->nz; ++K)
+            for (J = 0; J < C->ny; ++J)
+                for (I = 0; I < C->nx; ++I) {
+                    double sum = 0.0;
+                    for (q = 0; q < 2; ++q) for (p = 0; p < 2; ++p)
+                        sum += F->bz[ZI(F, 2 * I + p, 2 * J + q, 2 * K)];
+                    C->bz[ZI(C, I, J, K)] = sum / 4.0;
+                }
+}
+
+/* C1. btilde = f + boundary terms: Dirichlet face with value g adds 2*beta*b*g/h^2; Neumann face with
+ * outward-normal derivative q adds beta*b*q/h (R5).  Level 0 only; coarse levels are homogeneous (R4). */
+static void fold_bc(const ovmg *h, const double *rhs, double *bt)
+{
+    const olevel *L = &h->lev[0];
+    int i, j, k, f, nd = h->three_d ? 6 : 4;
+    for (k = 0; k < L->nz; ++k)
+        for (j = 0; j < L->ny; ++j)
+            for (i = 0; i < L->nx; ++i) {
+                double v = rhs[CI(L, i, j, k)];
+                for (f = 0; f < nd; ++f) {
+                    double b, hd, g;
+                    int on;
+                    size_t pl;
+                    switch (f) {
+                    case XLO: on = (i == 0);          b = L->bx[XI(L, 0, j, k)];      hd = L->hx; pl = j + (size_t)L->ny * k; break;
+                    case XHI: on = (i == L->nx - 1);  b = L->bx[XI(L, L->nx, j, k)];  hd = L->hx; pl = j + (size_t)L->ny * k; break;
+                    case YLO: on = (j == 0);          b = L->by[YI(L, i, 0, k)];      hd = L->hy; pl = i + (size_t)L->nx * k; break;
+                    case YHI: on = (j == L->ny - 1);  b = L->by[YI(L, i, L->ny, k)];  hd = L->hy; pl = i + (size_t)L->nx * k; break;
+                    case ZLO: on = (k == 0);          b = L->bz[ZI(L, i, j, 0)];      hd = L->hz; pl = i + (size_t)L->nx * j; break;
+                    default:  on = (k == L->nz - 1);  b = L->bz[ZI(L, i, j, L->nz)];  hd = L->hz; pl = i + (size_t)L->nx * j; break;
+                    }
+                    if (!on || !h->bcval[f]) continue;
+                    g = h->bcval[f][pl];
+                    if (h->bctype[f] == BC_DIRICHLET) v += 2.0 * h->beta * b * g / (hd * hd);
+                    else                              v += h->beta * b * g / hd;
+                }
+                bt[CI(L, i, j, k)] = v;
+            }
+}
+
+/* C4. V-cycle on level lev: phi (in/out), rhs. */
+static void vcycle(ovmg *h, int lev, double *phi, const double *rhs)
+{
+    olevel *L = &h->lev[lev];
+    if (lev == h->nlev - 1) {                       /* bottom: fixed sweeps from zero (R11) */
+        memset(phi, 0, ncell(L) * sizeof(double));
+        smooth_level(h, lev, phi, rhs, h->nbottom);
+        return;
+    }
+    smooth_level(h, lev, phi, rhs, h->nu1);
+    residual_level(h, lev, phi, rhs, L->res);
+    restrict_level(h, lev, L->res, h->lev[lev + 1].rhs);
+    memset(h->lev[lev + 1].phi, 0, ncell(&h->lev[lev + 1]) * sizeof(double));
+    vcycle(h, lev + 1, h->lev[lev + 1].phi, h->lev[lev + 1].rhs);
+    prolong_add_level(h, lev, phi, h->lev[lev + 1].phi);
+    smooth_level(h, lev, phi, rhs, h->nu2);
+}
+
+static double norm_inf(const double *v, size_t n)
+{
+    double m = 0.0;
+    size_t q;
+    for (q = 0; q < n; ++q) {
+        double t = fabs(v[q]);
+        if (t != t) return t;      /* NaN propagates */
+        if (t > m) m = t;
+    }
+    return m;
+}
+
+/* =============================================================================================
+ * Exported interface (host pointers).  Mirrors the vmg_* boundary of include/vmg.h in meaning, with an
+ * ovmg_ prefix, plus per-step entry points so that tests can compare single kernels.
+ * ============================================================================================= */
+static void free_level(olevel *L)
+{
+    free(L->a); free(L->bx); free(L->by); free(L->bz); free(L->phi); free(L->rhs); free(L->res);
+}
+
+int ovmg_create(ovmg **out, int nx, int ny, int nz, double dx, double dy, double dz)
+{
+    ovmg *h;
+    int n[3], l, nlev = 1, three_d = nz > 1;
+    if (!out) return O_ERR_ARG;
+    *out = NULL;
+    if (nx < 2 || ny < 2 || nz < 1 || !(dx > 0) || !(dy > 0) || (three_d && !(dz > 0))) return O_ERR_SIZE;
+    if (three_d && nz < 2) return O_ERR_SIZE;
+    /* R11: halve while every active dimension is even and stays >= 2 */
+    n[0] = nx; n[1] = ny; n[2] = nz;
+    for (;;) {
+        int ok = (n[0] % 2 == 0 && n[0] / 2 >= 2 && n[1] % 2 == 0 && n[1] / 2 >= 2);
+        if (three_d) ok = ok && (n[2] % 2 == 0 && n[2] / 2 >= 2);
+        if (!ok) break;
+        n[0] /= 2; n[1] /= 2; if (three_d) n[2] /= 2;
+        ++nlev;
+    }
+    if ((long)n[0] * n[1] * n[2] > 512) return O_ERR_SIZE;   /* fixed-sweep bottom needs a small grid */
+    h = (ovmg *)calloc(1, sizeof(ovmg));
+    h->lev = (olevel *)calloc(nlev, sizeof(olevel));
+    h->nlev = nlev; h->three_d = three_d;
+    h->nu1 = 3; h->nu2 = 3; h->nbottom = 32;                 /* R8, R11 */
+    for (l = 0; l < nlev; ++l) {
+        olevel *L = &h->lev[l];
+        size_t nc;
+        L->nx = nx >> l; L->ny = ny >> l; L->nz = three_d ? nz >> l : 1;
+        L->hx = dx * (1 << l); L->hy = dy * (1 << l); L->hz = three_d ? dz * (1 << l) : 1.0;
+        nc = ncell(L);
+        L->a = (double *)calloc(nc, sizeof(double));
+        L->bx = (double *)calloc((size_t)(L->nx + 1) * L->ny * L->nz, sizeof(double));
+        L->by = (double *)calloc((size_t)L->nx * (L->ny + 1) * L->nz, sizeof(double));
+        L->bz = (double *)calloc((size_t)L->nx * L->ny * (L->nz + 1), sizeof(double));
+        L->phi = (double *)calloc(nc, sizeof(double));
+        L->rhs = (double *)calloc(nc, sizeof(double));
+        L->res = (double *)calloc(nc, sizeof(double));
+    }
+    for (l = 0; l < 6; ++l) h->bctype[l] = BC_NEUMANN;
+    *out = h;
+    return O_OK;
+}
+
+int ovmg_destroy(ovmg *h)
+{
+    int l;
+    if (!h) return O_ERR_ARG;
+    for (l = 0; l < h->nlev; ++l) free_level(&h->lev[l]);
+    for (l = 0; l < 6; ++l) free(h->bcval[l]);
+    free(h->lev); free(h->hist); free(h);
+    return O_OK;
+}
+
+/* a == NULL means a = 0; bx,by,bz all NULL means b = 1 (bz ignored in 2-D). */
+int ovmg_set_coeffs(ovmg *h, const double *a, const double *bx, const double *by, const double *bz,
+                    double alpha, double beta)
+{
+    olevel *L;
+    size_t q, nbx, nby, nbz;
+    int l;
+    if (!h) return O_ERR_ARG;
+    L = &h->lev[0];
+    nbx = (size_t)(L->nx + 1) * L->ny * L->nz; nby = (size_t)L->nx * (L->ny + 1) * L->nz;
+    nbz = (size_t)L->nx * L->ny * (L->nz + 1);
+    if (!bx != !by) return O_ERR_ARG;
+    if (h->three_d && (!bx != !bz)) return O_ERR_ARG;
+    if (a) memcpy(L->a, a, ncell(L) * sizeof(double)); else memset(L->a, 0, ncell(L) * sizeof(double));
+    if (bx) {
+        memcpy(L->bx, bx, nbx * sizeof(double));
+        memcpy(L->by, by, nby * sizeof(double));
+        if (h->three_d) memcpy(L->bz, bz, nbz * sizeof(double));
+    } else {
+        for (q = 0; q < nbx; ++q) L->bx[q] = 1.0;
+        for (q = 0; q < nby; ++q) L->by[q] = 1.0;
+        for (q = 0; q < nbz; ++q) L->bz[q] = 1.0;
+    }
+    h->alpha = a ? alpha : 0.0;
+    h->beta = beta;
+    for (l = 0; l + 1 < h->nlev; ++l) average_coeffs(h, l);
+    h->have_coeffs = 1;
+    return O_OK;
+}
+
+int ovmg_set_bc(ovmg *h, const int *type, const double *const *value)
+{
+    const olevel *L;
+    size_t sizes[6];
+    int f;
+    if (!h || !type) return O_ERR_ARG;
+    L = &h->lev[0];
+    sizes[XLO] = sizes[XHI] = (size_t)L->ny * L->nz;
+    sizes[YLO] = sizes[YHI] = (size_t)L->nx * L->nz;
+    sizes[ZLO] = sizes[ZHI] = (size_t)L->nx * L->ny;
+    for (f = 0; f < 6; ++f)
+        if (type[f] != BC_DIRICHLET && type[f] != BC_NEUMANN) return O_ERR_ARG;
+    for (f = 0; f < 6; ++f) {
+        h->bctype[f] = type[f];
+        free(h->bcval[f]); h->bcval[f] = NULL;
+        if (value && value[f] && (f < 4 || h->three_d)) {
+            h->bcval[f] = (double *)malloc(sizes[f] * sizeof(double));
+            memcpy(h->bcval[f], value[f], sizes[f] * sizeof(double));
+        }
+    }
+    h->have_bc = 1;
+    return O_OK;
+}
+
+int ovmg_set_option(ovmg *h, const char *key, double v)
+{
+    if (!h || !key) return O_ERR_ARG;
+    if (!strcmp(key, "nu1")) { if (v < 0) return O_ERR_ARG; h->nu1 = (int)v; return O_OK; }
+    if (!strcmp(key, "nu2")) { if (v < 0) return O_ERR_ARG; h->nu2 = (int)v; return O_OK; }
+    if (!strcmp(key, "bottom_sweeps")) { if (v < 1) return O_ERR_ARG; h->nbottom = (int)v; return O_OK; }
+    return O_ERR_ARG;
+}
+
+static int singular(const ovmg *h)
+{
+    int f, nd = h->three_d ? 6 : 4;
+    for (f = 0; f < nd; ++f) if (h->bctype[f] == BC_DIRICHLET) return 0;
+    return h->alpha == 0.0;
+}
+
+/* C5. Solve: relres = ||btilde - A phi||_inf / ||btilde||_inf (R12), stall rule, status codes. */
+int ovmg_solve(ovmg *h, const double *rhs, double *phi, double rtol, int max_vcycles)
+{
+    olevel *L;
+    double nb, *bt;
+    int c, slow = 0;
+    if (!h || !rhs || !phi || max_vcycles < 0) return O_ERR_ARG;
+    if (!h->have_coeffs || !h->have_bc) return O_ERR_STATE;
+    if (singular(h)) return O_ERR_SINGULAR;
+    L = &h->lev[0];
+    bt = L->rhs;
+    free(h->hist);
+    h->hist = (double *)calloc((size_t)max_vcycles + 1, sizeof(double));
+    h->hist_len = 0; h->cycles = 0; h->relres = 0.0;
+    fold_bc(h, rhs, bt);
+    nb = norm_inf(bt, ncell(L));
+    if (nb == 0.0) {
+        memset(phi, 0, ncell(L) * sizeof(double));
+        h->hist[0] = 0.0; h->hist_len = 1;
+        return h->status = O_OK;
+    }
+    residual_level(h, 0, phi, bt, L->res);
+    h->hist[0] = h->relres = norm_inf(L->res, ncell(L)) / nb;
+    h->hist_len = 1;
+    if (!(h->relres == h->relres) || isinf(h->relres)) return h->status = O_ERR_DIVERGED;
+    if (rtol > 0.0 && h->relres <= rtol) return h->status = O_OK;
+    for (c = 1; c <= max_vcycles; ++c) {
+        vcycle(h, 0, phi, bt);
+        residual_level(h, 0, phi, bt, L->res);
+        h->hist[c] = h->relres = norm_inf(L->res, ncell(L)) / nb;
+        h->hist_len = c + 1; h->cycles = c;
+        if (!(h->relres == h->relres) || isinf(h->relres)) return h->status = O_ERR_DIVERGED;
+        if (rtol > 0.0) {
+            if (h->relres <= rtol) return h->status = O_OK;
+            slow = (h->hist[c] >= 0.9 * h->hist[c - 1]) ? slow + 1 : 0;
+            if (slow >= 3) return h->status = O_STALLED;
+        }
+    }
+    return h->status = O_MAXCYCLES;
+}
+
+int ovmg_get_info(const ovmg *h, int *cycles, double *relres, double *history)
+{
+    if (!h) return O_ERR_ARG;
+    if (cycles) *cycles = h->cycles;
+    if (relres) *relres = h->relres;
+    if (history && h->hist) memcpy(history, h->hist, (size_t)h->hist_len * sizeof(double));
+    return O_OK;
+}
+
+/* ---- per-step entry points for tests (all arrays are caller-owned host arrays of the level's size) ---- */
+int ovmg_num_levels(const ovmg *h) { return h ? h->nlev : O_ERR_ARG; }
+
+int ovmg_level_dims(const ovmg *h, int lev, int *dims)
+{
+    if (!h || lev < 0 || lev >= h->nlev) return O_ERR_ARG;
+    dims[0] = h->lev[lev].nx; dims[1] = h->lev[lev].ny; dims[2] = h->lev[lev].nz;
+    return O_OK;
+}
+
+int ovmg_get_level_coeffs(const ovmg *h, int lev, double *a, double *bx, double *by, double *bz)
+{
+    const olevel *L;
+    if (!h || lev < 0 || lev >= h->nlev) return O_ERR_ARG;
+    L = &h->lev[lev];
+    if (a) memcpy(a, L->a, ncell(L) * sizeof(double));
+    if (bx) memcpy(bx, L->bx, (size_t)(L->nx + 1) * L->ny * L->nz * sizeof(double));
+    if (by) memcpy(by, L->by, (size_t)L->nx * (L->ny + 1) * L->nz * sizeof(double));
+    if (bz) memcpy(bz, L->bz, (size_t)L->nx * L->ny * (L->nz + 1) * sizeof(double));
+    return O_OK;
+}
+
+int ovmg_apply(const ovmg *h, int lev, const double *phi, double *out)
+{
+    if (!h || lev < 0 || lev >= h->nlev || !h->have_coeffs || !h->have_bc) return O_ERR_ARG;
+    apply_level(h, lev, phi, out);
+    return O_OK;
+}
+
+int ovmg_fold_bc(const ovmg *h, const double *rhs, double *btilde)
+{
+    if (!h || !h->have_coeffs || !h->have_bc) return O_ERR_ARG;
+    fold_bc(h, rhs, btilde);
+    return O_OK;
+}
+
+int ovmg_smooth(const ovmg *h, int lev, double *phi, const double *rhs, int nsweeps)
+{
+    if (!h || lev < 0 || lev >= h->nlev) return O_ERR_ARG;
+    smooth_level(h, lev, phi, rhs, nsweeps);
+    return O_OK;
+}
+
+int ovmg_residual(const ovmg *h, int lev, const double *phi, const double *rhs, double *r)
+{
+    if (!h || lev < 0 || lev >= h->nlev) return O_ERR_ARG;
+    residual_level(h, lev, phi, rhs, r);
+    return O_OK;
+}
+
+int ovmg_restrict(const ovmg *h, int lev, const double *rfine, double *rcoarse)
+{
+    if (!h || lev < 0 || lev + 1 >= h->nlev) return O_ERR_ARG;
+    restrict_level(h, lev, rfine, rcoarse);
+    return O_OK;
+}
+
+int ovmg_prolong_add(const ovmg *h, int lev, double *phifine, const double *ecoarse)
+{
+    if (!h || lev < 0 || lev + 1 >= h->nlev) return O_ERR_ARG;
+    prolong_add_level(h, lev, phifine, ecoarse);
+    return O_OK;
+}
+
+/* one V-cycle on level 0 with a caller-supplied (already BC-folded) right-hand side */
+int ovmg_vcycle(ovmg *h, double *phi, const double *btilde)
+{
+    if (!h || !h->have_coeffs || !h->have_bc) return O_ERR_ARG;
+    vcycle(h, 0, phi, btilde);
+    return O_OK;
+}
