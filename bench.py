@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the vmg hot path (BASELINE.json metric: multigrid cell-updates/s and
+solves/s at 4.19M cells fp64; % of B200 HBM BW).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3|4|2|5]
+
+A step = one pass of the whole hot path over one batch of synthetic input: vmg_set_coeffs (S0 coefficient
+averaging + stencil build) + vmg_set_bc + vmg_solve from a zero guess to relative residual 1e-12 (S1 fold_bc,
+S6 norms, ~10 V-cycles of S2-S5, S7 sequencing).  Workload at N = 1: BASELINE.json configs[2], the 256x128x128
+(4 194 304-cell) electrostatic Poisson solve the metric is quoted on.  N > 1: independent replicas, one per
+GPU, no collective on the data path (replicas only).
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+# algorithmic bytes per cell: fp64, 6 input arrays + 1 output
+B_SMOOTH_PASS = 56.0        # one blocked pass of nu sweeps: read phi,btilde,dinv,wx,wy,wz, write phi
+B_RESID_RESTRICT = 49.0
+B_PROLONG_CORRECT = 17.0
+B_FOLD = 16.0
+B_NORM = 8.0
+B_SETCOEFFS = 24.0
+
+
+def level_cells(nx, ny, nz):
+    """cells per level, finest first (R11: halve while all active dims are even and stay >= 2)."""
+    three_d = nz > 1
+    out = [nx * ny * nz]
+    while nx % 2 == 0 and ny % 2 == 0 and nx // 2 >= 2 and ny // 2 >= 2 and (not three_d or (nz % 2 == 0 and nz // 2 >= 2)):
+        nx, ny, nz = nx // 2, ny // 2, (nz // 2 if three_d else 1)
+        out.append(nx * ny * nz)
+    return out
+
+
+def work_model(p, nu1=3, nu2=3, nbottom=32):
+    cells = level_cells(p.nx, p.ny, p.nz)
+    upper = sum(cells[:-1])
+    return {
+        "updates_per_cycle": (nu1 + nu2) * upper + nbottom * cells[-1],
+        "bytes_per_cycle": (2 * B_SMOOTH_PASS + B_RESID_RESTRICT + B_PROLONG_CORRECT) * upper,
+        "bytes_solve_fixed": (B_FOLD + B_NORM) * cells[0],
+        "bytes_set_coeffs": B_SETCOEFFS * sum(cells),
+        "cells": cells,
+    }
+
+
+def measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.1):
+        super().__init__(daemon=True)
+        self.index, self.period, self.samples, self.reasons, self.max_mhz = index, period, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop_evt.wait(self.period)
+
+    def finish(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2.0)
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def make_problem(config: int):
+    from paper_2507_08200_b200 import inputs
+    return inputs.CONFIGS[config]()
+
+
+# ----------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on the box's host cores
+# ----------------------------------------------------------------------------------------------------
+def oracle_sample(p, cycles_per_step: int):
+    """A bounded sample of the workload: set_coeffs + set_bc + `cycles_per_step` V-cycles (rtol = 0)."""
+    from oracle import Oracle
+    t0 = time.perf_counter()
+    o = Oracle.from_problem(p)
+    o.solve(p.rhs, rtol=0.0, max_vcycles=cycles_per_step)
+    dt = time.perf_counter() - t0
+    o.close()
+    return dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    p = make_problem(args.config)
+    wm = work_model(p)
+    cyc = 2
+    for _ in range(args.warmup):
+        oracle_sample(p, cyc)
+    times = [oracle_sample(p, cyc) for _ in range(args.steps)]
+    dt = float(np.mean(times))
+    value = cyc * wm["updates_per_cycle"] / dt
+    cores = os.cpu_count()
+    sample = (f"set_coeffs + set_bc + {cyc} V(3,3)-cycles (rtol=0) of {p.name} per step, "
+              f"OpenMP over all {cores} host threads, gcc -O2 -ffp-contract=off")
+    line = {
+        "impl": "reference", "metric": "multigrid_cell_updates_per_s", "value": value, "unit": "cell-updates/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": p.name, "cells": p.ncells, "sample": sample},
+        "vcycles_per_s": cyc / dt,
+        "cpu_baseline": {"value": value, "unit": "cell-updates/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ----------------------------------------------------------------------------------------------------
+def run_vmg(args):
+    import torch
+    from paper_2507_08200_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; --impl reference times the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    p = make_problem(args.config)
+    wm = work_model(p)
+    peak, peak_src = measured_peak_gbs()
+    stream = torch.cuda.Stream()
+    dev = torch.device("cuda", local)
+
+    # host copies in pinned memory (for the e2e leg), device-resident copies (for the headline leg)
+    host = {k: (None if v is None else torch.from_numpy(np.ascontiguousarray(v)).pin_memory())
+            for k, v in dict(a=p.a, bx=p.bx, by=p.by, bz=p.bz, rhs=p.rhs).items()}
+    host_bc = [None if v is None else torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for v in p.bc_value]
+    host_phi = torch.zeros(p.rhs.shape, dtype=torch.float64).pin_memory()
+    with torch.cuda.stream(stream):
+        d = {k: (None if v is None else v.to(dev, non_blocking=True)) for k, v in host.items()}
+        d_bc = [None if v is None else v.to(dev, non_blocking=True) for v in host_bc]
+        phi = torch.zeros(p.rhs.shape, dtype=torch.float64, device=dev)
+        flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # 256 MiB > 126 MB L2
+        s = binding.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, stream=stream)
+    stream.synchronize()
+
+    def step_resident():
+        """inputs already resident in HBM"""
+        phi.zero_()
+        s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+        s.set_bc(p.bc_type, d_bc)
+        return s.solve(d["rhs"], phi, rtol=p.rtol, max_vcycles=p.max_vcycles)
+
+    def step_e2e():
+        """host buffers in, host buffer out: H2D of every input and D2H of phi inside the timed region"""
+        dd = {k: (None if v is None else v.to(dev, non_blocking=True)) for k, v in host.items()}
+        dbc = [None if v is None else v.to(dev, non_blocking=True) for v in host_bc]
+        ph = host_phi.to(dev, non_blocking=True)                       # zero initial guess from the host
+        s.set_coeffs(dd["a"], dd["bx"], dd["by"], dd["bz"], p.alpha, p.beta)
+        s.set_bc(p.bc_type, dbc)
+        st = s.solve(dd["rhs"], ph, rtol=p.rtol, max_vcycles=p.max_vcycles)
+        out_host.copy_(ph, non_blocking=True)
+        return st
+
+    out_host = torch.empty(p.rhs.shape, dtype=torch.float64).pin_memory()
+    h2d = sum(v.numel() * 8 for v in host.values() if v is not None) + sum(v.numel() * 8 for v in host_bc if v is not None) \
+        + host_phi.numel() * 8
+    d2h = out_host.numel() * 8
+
+    def timed(fn, steps, warmup, sampler=None):
+        times, cycles, launches = [], [], 0
+        with torch.cuda.stream(stream):
+            for _ in range(warmup):
+                fn()
+            stream.synchronize()
+            if dist is not None:
+                dist.barrier()
+            torch.cuda.synchronize()
+            if sampler is not None:
+                sampler.start()
+            for _ in range(steps):
+                flush.fill_(1.0)                                   # evict L2 between timed iterations
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                l0 = s.total_launch_count()
+                e0.record(stream)
+                st = fn()
+                e1.record(stream)
+                e1.synchronize()
+                assert st in (0, 1), f"solve status {st}"
+                times.append(e0.elapsed_time(e1) * 1e-3)
+                cycles.append(s.get_info()[0])
+                launches += s.total_launch_count() - l0
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+        return np.array(times), np.array(cycles), launches
+
+    sampler = ClockSampler(local)
+    times, cycles, launches = timed(step_resident, args.steps, args.warmup, sampler)
+    clocks = sampler.finish()
+    total = float(times.sum())
+    if dist is not None:
+        t = torch.tensor([total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total = float(t.item())
+    updates_per_step = float(np.mean(cycles)) * wm["updates_per_cycle"]
+    value = world * args.steps * updates_per_step / total
+
+    # solve-only and per-kernel-class numbers (plain launches with event pairs; same workload)
+    s.set_option("profile", 1)
+    ptimes, pcycles, _ = timed(step_resident, max(2, min(args.steps, 5)), 1)
+    prof = s.get_profile()
+    s.set_option("profile", 0)
+    n_prof_cycles = float(pcycles.sum())
+    sm_ms, sm_launches = prof["smooth_l0"]
+    n0 = wm["cells"][0]
+    achieved = (2 * B_SMOOTH_PASS * n0 * n_prof_cycles) / (sm_ms * 1e-3) / 1e9 if sm_ms > 0 else 0.0
+    klass = {k: {"ms_per_cycle": v[0] / max(n_prof_cycles, 1), "launches_per_cycle": v[1] / max(n_prof_cycles, 1)}
+             for k, v in prof.items()}
+
+    # solve only (coefficients already set): the SURVEY's solves/s definition
+    def solve_only():
+        phi.zero_()
+        return s.solve(d["rhs"], phi, rtol=p.rtol, max_vcycles=p.max_vcycles)
+    stimes, scycles, _ = timed(solve_only, args.steps, 1)
+    solve_s = float(np.mean(stimes))
+    ncyc = float(np.mean(scycles))
+    bytes_solve = ncyc * wm["bytes_per_cycle"] + wm["bytes_solve_fixed"]
+
+    # end to end through the C-ABI with host buffers
+    etimes, ecycles, _ = timed(step_e2e, args.steps, max(1, min(args.warmup, 2)))
+    etotal = float(etimes.sum())
+    if dist is not None:
+        t = torch.tensor([etotal], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        etotal = float(t.item())
+    e2e_value = world * args.steps * float(np.mean(ecycles)) * wm["updates_per_cycle"] / etotal
+
+    line = {
+        "metric": "multigrid_cell_updates_per_s", "value": value, "unit": "cell-updates/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": p.name, "cells": p.ncells, "levels": len(wm["cells"]), "smoother": "V(3,3) red-black GS",
+                   "rtol": p.rtol, "cycles_per_solve": ncyc, "step": "vmg_set_coeffs + vmg_set_bc + vmg_solve",
+                   "l2": "256 MiB flush write between timed steps; level-0 working set 201 MB > 126 MB L2",
+                   "multi_gpu": "replicas only"},
+        "solves_per_s": world / solve_s, "vcycles_per_s": world * ncyc / solve_s,
+        "solve_ms": solve_s * 1e3,
+        "hbm_frac_solve": bytes_solve / solve_s / 1e9 / peak,
+        "hbm_frac_note": f"algorithmic bytes (203.4 B/cell/V-cycle model) / solve time / {peak} GB/s {peak_src}",
+        "roofline": {"bound": "hbm", "kernel": "level-0 red-black smoother (all launches of a nu-sweep pass)",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "peak_source": peak_src,
+                     "launches_per_pass": sm_launches / max(2 * n_prof_cycles, 1)},
+        "kernel_classes": klass,
+        "e2e": {"value": e2e_value, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": etotal / args.steps * 1e3},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cyc = 2
+        oracle_sample(p, 1)
+        t_or = [oracle_sample(p, cyc) for _ in range(2)]
+        dt = float(np.mean(t_or))
+        line["cpu_baseline"] = {"value": cyc * wm["updates_per_cycle"] / dt, "unit": "cell-updates/s",
+                                "cores": os.cpu_count(), "kind": "oracle",
+                                "sample": f"set_coeffs + set_bc + {cyc} V(3,3)-cycles of {p.name}, mean of 2 runs"}
+    s.destroy()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="vmg", choices=["vmg", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4, 5])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "vmg" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_vmg(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,137 @@
+/*
+ * vmg.h -- C-ABI boundary of the B200-native variable-coefficient geometric multigrid library (libvmg.so).
+ *
+ * Solves, in fp64 on one GPU (sm_100a), the cell-centred finite-volume discretisation of
+ *
+ *        alpha * a * phi  -  beta * div( b grad phi )  =  f          on a uniform Cartesian box,
+ *
+ * the "Helmholtz equation form" into which the paper casts every governing equation before handing it to
+ * its multigrid solver (sec. 4): the electrostatic Poisson equation Eq. 3, the
+ * implicit diffusion part of the species / electron-energy equations Eq. 17 and the
+ * photoionisation Helmholtz equations Eq. 9.  Discretisation: second-order central diffusive
+ * flux on Cartesian finite-volume cells, implicit in time (sec. 3).  Boundary kinds: fixed
+ * potential (Dirichlet) electrodes and homogeneous Neumann walls.  The multigrid
+ * components (red-black Gauss-Seidel with face coefficients, residual+restriction, prolongation+correction,
+ * coefficient averaging, fixed-sweep bottom solve, V-cycle) are those named by BASELINE.json:north_star; the
+ * paper itself only names "multigrid".  All readings are listed in DESIGN.md.
+ *
+ * All array arguments are DEVICE pointers (fp64, 16-byte aligned) on the device that was current at
+ * vmg_create, unless a parameter says "host".  Nothing here takes or returns a torch type.
+ *
+ * Layout (x fastest).  Cell arrays (a, rhs, phi): idx = i + nx*(j + ny*k).
+ *   bx: (nx+1)*ny*nz, bx[i,j,k] is the face at x = i*dx between cells i-1 and i, idx = i + (nx+1)*(j + ny*k);
+ *   by: nx*(ny+1)*nz, idx = i + nx*(j + (ny+1)*k);     bz: nx*ny*(nz+1), idx = i + nx*(j + ny*k).
+ *   Boundary value planes: x faces idx = j + ny*k; y faces idx = i + nx*k; z faces idx = i + nx*j.
+ * nz == 1 selects the 2-D operator: no z coupling; bz, dz and the z-face boundary entries are ignored.
+ *
+ * Every function returns a status code (below); there are no exceptions, no output on stderr, no abort.
+ * After a negative code from vmg_solve the contents of phi are unspecified but the handle stays usable.
+ * Calls on one handle must not overlap in time (no internal locking).
+ */
+#ifndef VMG_H
+#define VMG_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vmg_s* vmg_handle;
+
+enum { VMG_XLO = 0, VMG_XHI = 1, VMG_YLO = 2, VMG_YHI = 3, VMG_ZLO = 4, VMG_ZHI = 5 };
+enum { VMG_BC_DIRICHLET = 0, VMG_BC_NEUMANN = 1 };
+enum {
+    VMG_OK = 0,              /* converged to rtol                                                       */
+    VMG_MAXCYCLES = 1,       /* ran max_vcycles cycles without reaching rtol (always, when rtol <= 0)   */
+    VMG_STALLED = 2,         /* residual reduced by less than 10 % in 3 consecutive cycles (fp64 floor) */
+    VMG_ERR_ARG = -1,        /* NULL / out-of-range argument, unknown option key                        */
+    VMG_ERR_SIZE = -2,       /* grid cannot be coarsened to a bottom grid of <= 512 cells               */
+    VMG_ERR_STATE = -3,      /* vmg_solve before both vmg_set_coeffs and vmg_set_bc                     */
+    VMG_ERR_SINGULAR = -4,   /* all active faces Neumann and (a == NULL or alpha == 0)                  */
+    VMG_ERR_DIVERGED = -5,   /* residual became NaN or Inf                                              */
+    VMG_ERR_CUDA = -6,       /* a CUDA runtime call failed (vmg_last_cuda_error gives the code)         */
+    VMG_ERR_ALLOC = -7       /* device or host allocation failed                                        */
+};
+
+/* Create a solver for an nx x ny x nz box with cell sizes dx, dy, dz.  The level hierarchy halves every
+ * active dimension while all stay even and >= 2 afterwards (256x128x128 -> ... -> 4x2x2); the coarsest grid
+ * must have <= 512 cells (VMG_ERR_SIZE otherwise).  cuda_stream is a cudaStream_t (NULL = legacy default
+ * stream); every kernel, copy and graph of this handle is enqueued on it.  All device memory the handle
+ * needs (about 6.9 fp64 arrays of nx*ny*nz) is allocated here; vmg_solve allocates nothing on the device. */
+int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream);
+
+/* Coefficients.  a: cell array or NULL (a == 0, alpha ignored).  bx, by, bz: face arrays, or all NULL for
+ * b == 1.  a must be >= 0 with alpha >= 0 and b > 0, beta > 0 (not checked; otherwise undefined behaviour).
+ * The arrays are read during this call only (enqueued on the stream, then synchronised): the library
+ * averages them to all coarse levels (a: mean of the 8 children, 4 in 2-D; b: mean of the fine faces lying
+ * on the coarse face) and converts each level to its internal stencil form.  The caller may free or modify
+ * them afterwards; call again when coefficients change. */
+int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double* by, const double* bz,
+                   double alpha, double beta);
+
+/* Boundary conditions.  type: HOST array of 6 entries (VMG_BC_DIRICHLET / VMG_BC_NEUMANN), order XLO..ZHI.
+ * value: HOST array of 6 DEVICE pointers to value planes, or NULL; a NULL entry (or value == NULL) means
+ * homogeneous.  Dirichlet value = phi on the face; Neumann value = outward-normal derivative d(phi)/dn on
+ * the face (not the flux b*d(phi)/dn).  The planes are copied.  May be called before or after
+ * vmg_set_coeffs, and again at any time. */
+int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6]);
+
+/* Solve.  rhs: f at cell centres (never written).  phi: initial guess in, solution out.
+ * Iterates V(nu1,nu2) cycles until ||btilde - A phi||_inf <= rtol * ||btilde||_inf, where btilde is f with
+ * the boundary data folded in, or until max_vcycles cycles (rtol <= 0: run exactly max_vcycles cycles).
+ * Returns VMG_OK / VMG_MAXCYCLES / VMG_STALLED or a negative error.  Synchronises the stream before
+ * returning. */
+int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max_vcycles);
+
+/* Result of the last vmg_solve.  cycles, relres: HOST scalars (may be NULL).  history: HOST array of at
+ * least cycles+1 doubles (relative residual before the first cycle and after each cycle) or NULL. */
+int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
+
+/* Options (key is a HOST C string): "nu1", "nu2" (pre/post red-black sweeps, default 3, 0..8),
+ * "bottom_sweeps" (default 32), "graph" (1: replay the V-cycle as a CUDA graph, default; 0: plain launches),
+ * "blocked" (1: temporally blocked smoother where available, default; 0: one kernel per colour),
+ * "profile" (1: per-kernel-class event timing, see vmg_get_profile; implies plain launches; default 0). */
+int vmg_set_option(vmg_handle h, const char* key, double v);
+
+int vmg_destroy(vmg_handle h);
+
+const char* vmg_strerror(int code);       /* static string */
+int vmg_last_cuda_error(vmg_handle h);    /* cudaError_t of the last failed runtime call, 0 if none */
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Introspection and single-step entry points.  They run the very kernels vmg_solve runs, one step at a
+ * time, on caller-owned DEVICE arrays of the level's size, so that tests can compare each kernel with the
+ * oracle.  Each synchronises the stream before returning.  Level 0 is the finest.
+ * --------------------------------------------------------------------------------------------------------- */
+int vmg_num_levels(vmg_handle h);
+int vmg_level_dims(vmg_handle h, int level, int dims[3]);                       /* dims: HOST */
+/* averaged coefficients of a level in the public layout (any pointer may be NULL) */
+int vmg_get_level_coeffs(vmg_handle h, int level, double* a, double* bx, double* by, double* bz);
+/* btilde = rhs + boundary terms (level 0) */
+int vmg_step_fold_bc(vmg_handle h, const double* rhs, double* btilde);
+/* nsweeps red-black Gauss-Seidel sweeps on a level: phi in/out */
+int vmg_step_smooth(vmg_handle h, int level, double* phi, const double* rhs, int nsweeps);
+/* r = rhs - A phi on a level */
+int vmg_step_residual(vmg_handle h, int level, const double* phi, const double* rhs, double* r);
+/* rhs_coarse = mean over children of (rhs - A phi) on `level`; coarse array has the size of level+1 */
+int vmg_step_residual_restrict(vmg_handle h, int level, const double* phi, const double* rhs, double* rhs_coarse);
+/* phi += P e_coarse */
+int vmg_step_prolong_correct(vmg_handle h, int level, double* phi, const double* e_coarse);
+/* one V-cycle from level 0 with an already folded right-hand side: phi in/out */
+int vmg_step_vcycle(vmg_handle h, double* phi, const double* btilde);
+/* ||v||_inf of a device array of n doubles -> HOST scalar */
+int vmg_step_norm_inf(vmg_handle h, const double* v, long long n, double* out);
+/* number of kernel launches (graph nodes count individually) issued by the last vmg_solve, and by every
+ * vmg_set_coeffs / vmg_solve since vmg_create */
+long long vmg_last_launch_count(vmg_handle h);
+long long vmg_total_launch_count(vmg_handle h);
+/* Per-kernel-class device times.  With option "profile" = 1 the library issues plain launches (no graph)
+ * and brackets each group of launches of one class with a CUDA event pair on the handle's stream; the
+ * totals accumulate until the option is set again.  ms, launches: HOST arrays of 8 entries, classes:
+ * 0 level-0 smoother, 1 level-0 residual+restriction, 2 level-0 prolongation+correction, 3 all coarser
+ * levels (incl. bottom), 4 norms, 5 fold_bc, 6 phi copies in/out, 7 vmg_set_coeffs kernels. */
+int vmg_get_profile(vmg_handle h, double ms[8], long long launches[8]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VMG_H */

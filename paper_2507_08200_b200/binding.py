@@ -1,0 +1,233 @@
+"""Thin Python binding of libvmg.so (include/vmg.h): argument marshalling only.
+
+torch is used for device memory (tensors' data_ptr) and streams; every step of the path runs in the CUDA
+kernels of libvmg.so.  There is NO CPU fallback: if the library is missing or no CUDA device is present the
+calls raise.  Arrays are torch fp64 CUDA tensors indexed [k, j, i] (x fastest), see paper_2507_08200_b200.inputs.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import List, Optional, Sequence
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libvmg.so")
+
+STATUS = {0: "OK", 1: "MAXCYCLES", 2: "STALLED", -1: "ERR_ARG", -2: "ERR_SIZE", -3: "ERR_STATE",
+          -4: "ERR_SINGULAR", -5: "ERR_DIVERGED", -6: "ERR_CUDA", -7: "ERR_ALLOC"}
+
+# every symbol include/vmg.h declares (checked by tests/test_abi.py)
+SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_solve", "vmg_get_info", "vmg_set_option",
+           "vmg_destroy", "vmg_strerror", "vmg_last_cuda_error", "vmg_num_levels", "vmg_level_dims",
+           "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
+           "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_vcycle", "vmg_step_norm_inf",
+           "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile"]
+
+_lib = None
+_vp = C.c_void_p
+
+
+def load():
+    """dlopen libvmg.so; raises if it has not been built (python -m paper_2507_08200_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2507_08200_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    lib.vmg_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _vp]
+    lib.vmg_set_coeffs.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_double, C.c_double]
+    lib.vmg_set_bc.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(_vp)]
+    lib.vmg_solve.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int]
+    lib.vmg_get_info.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.vmg_set_option.argtypes = [_vp, C.c_char_p, C.c_double]
+    lib.vmg_destroy.argtypes = [_vp]
+    lib.vmg_strerror.argtypes = [C.c_int]
+    lib.vmg_strerror.restype = C.c_char_p
+    lib.vmg_last_cuda_error.argtypes = [_vp]
+    lib.vmg_num_levels.argtypes = [_vp]
+    lib.vmg_level_dims.argtypes = [_vp, C.c_int, C.POINTER(C.c_int)]
+    lib.vmg_get_level_coeffs.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp]
+    lib.vmg_step_fold_bc.argtypes = [_vp, _vp, _vp]
+    lib.vmg_step_smooth.argtypes = [_vp, C.c_int, _vp, _vp, C.c_int]
+    lib.vmg_step_residual.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
+    lib.vmg_step_residual_restrict.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
+    lib.vmg_step_prolong_correct.argtypes = [_vp, C.c_int, _vp, _vp]
+    lib.vmg_step_vcycle.argtypes = [_vp, _vp, _vp]
+    lib.vmg_step_norm_inf.argtypes = [_vp, _vp, C.c_longlong, C.POINTER(C.c_double)]
+    lib.vmg_last_launch_count.argtypes = [_vp]
+    lib.vmg_last_launch_count.restype = C.c_longlong
+    lib.vmg_total_launch_count.argtypes = [_vp]
+    lib.vmg_total_launch_count.restype = C.c_longlong
+    lib.vmg_get_profile.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    _lib = lib
+    return lib
+
+
+class VmgError(RuntimeError):
+    def __init__(self, code: int, where: str, cuda: int = 0):
+        msg = load().vmg_strerror(code).decode()
+        super().__init__(f"{where}: {STATUS.get(code, code)} ({msg})" + (f" [cudaError {cuda}]" if cuda else ""))
+        self.code = code
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2507_08200_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _ptr(t) -> Optional[int]:
+    if t is None:
+        return None
+    torch = _torch()
+    assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous(), "need contiguous fp64 CUDA tensors"
+    return t.data_ptr()
+
+
+class Vmg:
+    """One solver handle (vmg_create ... vmg_destroy). Method names follow include/vmg.h."""
+
+    def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, stream=None):
+        torch = _torch()
+        self._lib = load()
+        self._h = _vp()
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        sptr = self.stream.cuda_stream
+        rc = self._lib.vmg_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, _vp(sptr) if sptr else None)
+        if rc != 0:
+            self._h = None
+            raise VmgError(rc, "vmg_create")
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.device = torch.device("cuda", torch.cuda.current_device())
+
+    def _chk(self, rc: int, where: str) -> int:
+        if rc < 0:
+            raise VmgError(rc, where, self._lib.vmg_last_cuda_error(self._h))
+        return rc
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.vmg_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    # ---- the boundary ---------------------------------------------------------------------------------
+    def set_coeffs(self, a, bx, by, bz, alpha: float, beta: float):
+        self._chk(self._lib.vmg_set_coeffs(self._h, _ptr(a), _ptr(bx), _ptr(by), _ptr(bz), alpha, beta), "vmg_set_coeffs")
+
+    def set_bc(self, types: Sequence[int], values: Optional[List] = None):
+        t = (C.c_int * 6)(*[int(v) for v in types])
+        vals = list(values) if values is not None else [None] * 6
+        arr = (_vp * 6)(*[_ptr(v) for v in vals])
+        self._chk(self._lib.vmg_set_bc(self._h, t, arr), "vmg_set_bc")
+
+    def set_option(self, key: str, v: float):
+        self._chk(self._lib.vmg_set_option(self._h, key.encode(), float(v)), "vmg_set_option")
+
+    def solve(self, rhs, phi, rtol: float = 1e-12, max_vcycles: int = 50) -> int:
+        """phi: initial guess in, solution out (in place). Returns the status code (>= 0)."""
+        return self._chk(self._lib.vmg_solve(self._h, _ptr(rhs), _ptr(phi), rtol, max_vcycles), "vmg_solve")
+
+    def get_info(self):
+        cyc, rr = C.c_int(), C.c_double()
+        self._lib.vmg_get_info(self._h, C.byref(cyc), C.byref(rr), None)
+        hist = (C.c_double * (cyc.value + 1))()
+        self._lib.vmg_get_info(self._h, None, None, hist)
+        return cyc.value, rr.value, list(hist)
+
+    def last_launch_count(self) -> int:
+        return int(self._lib.vmg_last_launch_count(self._h))
+
+    def total_launch_count(self) -> int:
+        return int(self._lib.vmg_total_launch_count(self._h))
+
+    PROFILE_CLASSES = ["smooth_l0", "residual_restrict_l0", "prolong_correct_l0", "coarse_levels", "norms",
+                       "fold_bc", "phi_copies", "set_coeffs"]
+
+    def get_profile(self):
+        """{class: (ms, launches)} accumulated since set_option("profile", 1)."""
+        ms, ln = (C.c_double * 8)(), (C.c_longlong * 8)()
+        self._chk(self._lib.vmg_get_profile(self._h, ms, ln), "vmg_get_profile")
+        return {k: (ms[i], ln[i]) for i, k in enumerate(self.PROFILE_CLASSES)}
+
+    # ---- introspection / single steps ---------------------------------------------------------------------
+    @property
+    def num_levels(self) -> int:
+        return self._lib.vmg_num_levels(self._h)
+
+    def level_dims(self, level: int):
+        d = (C.c_int * 3)()
+        self._chk(self._lib.vmg_level_dims(self._h, level, d), "vmg_level_dims")
+        return d[0], d[1], d[2]
+
+    def _empty(self, level: int):
+        nx, ny, nz = self.level_dims(level)
+        return _torch().empty((nz, ny, nx), dtype=_torch().float64, device=self.device)
+
+    def get_level_coeffs(self, level: int):
+        torch = _torch()
+        nx, ny, nz = self.level_dims(level)
+        mk = lambda *s: torch.zeros(s, dtype=torch.float64, device=self.device)
+        a, bx, by, bz = mk(nz, ny, nx), mk(nz, ny, nx + 1), mk(nz, ny + 1, nx), mk(nz + 1, ny, nx)
+        self._chk(self._lib.vmg_get_level_coeffs(self._h, level, _ptr(a), _ptr(bx), _ptr(by), _ptr(bz)),
+                  "vmg_get_level_coeffs")
+        return a, bx, by, bz
+
+    def step_fold_bc(self, rhs):
+        out = _torch().empty_like(rhs)
+        self._chk(self._lib.vmg_step_fold_bc(self._h, _ptr(rhs), _ptr(out)), "vmg_step_fold_bc")
+        return out
+
+    def step_smooth(self, level: int, phi, rhs, nsweeps: int):
+        phi = phi.clone()
+        self._chk(self._lib.vmg_step_smooth(self._h, level, _ptr(phi), _ptr(rhs), nsweeps), "vmg_step_smooth")
+        return phi
+
+    def step_residual(self, level: int, phi, rhs):
+        out = _torch().empty_like(phi)
+        self._chk(self._lib.vmg_step_residual(self._h, level, _ptr(phi), _ptr(rhs), _ptr(out)), "vmg_step_residual")
+        return out
+
+    def step_residual_restrict(self, level: int, phi, rhs):
+        out = self._empty(level + 1)
+        self._chk(self._lib.vmg_step_residual_restrict(self._h, level, _ptr(phi), _ptr(rhs), _ptr(out)),
+                  "vmg_step_residual_restrict")
+        return out
+
+    def step_prolong_correct(self, level: int, phi, e_coarse):
+        phi = phi.clone()
+        self._chk(self._lib.vmg_step_prolong_correct(self._h, level, _ptr(phi), _ptr(e_coarse)),
+                  "vmg_step_prolong_correct")
+        return phi
+
+    def step_vcycle(self, phi, btilde):
+        phi = phi.clone()
+        self._chk(self._lib.vmg_step_vcycle(self._h, _ptr(phi), _ptr(btilde)), "vmg_step_vcycle")
+        return phi
+
+    def step_norm_inf(self, v) -> float:
+        out = C.c_double()
+        self._chk(self._lib.vmg_step_norm_inf(self._h, _ptr(v), v.numel(), C.byref(out)), "vmg_step_norm_inf")
+        return out.value
+
+
+def upload(p, device=None):
+    """Problem (numpy, paper_2507_08200_b200.inputs) -> dict of fp64 CUDA tensors."""
+    torch = _torch()
+    dev = device or torch.device("cuda", torch.cuda.current_device())
+    t = lambda x: None if x is None else torch.from_numpy(x).to(dev)
+    return {"a": t(p.a), "bx": t(p.bx), "by": t(p.by), "bz": t(p.bz), "rhs": t(p.rhs),
+            "bc_value": [t(v) for v in p.bc_value]}
+
+
+def from_problem(p, stream=None):
+    """Create a handle for a Problem and load its coefficients and boundary data. Returns (Vmg, tensors)."""
+    d = upload(p)
+    s = Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, stream=stream)
+    s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+    s.set_bc(p.bc_type, d["bc_value"])
+    return s, d

@@ -1,0 +1,380 @@
+// vmg_api.cu -- C-ABI boundary of libvmg (see include/vmg.h for the contract and the paper citations).
+#include "../../include/vmg.h"
+#include "vmg_internal.h"
+#include "vmg_kernels.cuh"
+#include "vmg_sched.cuh"
+
+#include <cmath>
+#include <cstring>
+#include <new>
+
+using namespace vmg;
+
+#define CUDA_TRY(h, expr)                                                      \
+    do {                                                                       \
+        cudaError_t e__ = (expr);                                              \
+        if (e__ != cudaSuccess) {                                              \
+            if (h) (h)->last_cuda_error = (int)e__;                            \
+            (void)cudaGetLastError();                                          \
+            return VMG_ERR_CUDA;                                               \
+        }                                                                      \
+    } while (0)
+
+static inline size_t round_up(size_t v, size_t m) { return (v + m - 1) / m * m; }
+
+namespace {
+
+struct ArenaPlan {
+    size_t off = 0;
+    size_t take(size_t doubles) { size_t o = off; off += round_up(doubles, 32); return o; }
+};
+
+size_t face_count(const VmgLevel& L, int dir)
+{
+    return (size_t)(L.nx + (dir == 0)) * (L.ny + (dir == 1)) * (L.nz + (dir == 2));
+}
+
+size_t plane_count(const VmgLevel& L, int f)
+{
+    return f < 2 ? (size_t)L.ny * L.nz : f < 4 ? (size_t)L.nx * L.nz : (size_t)L.nx * L.ny;
+}
+
+// lays the arena out; with base == nullptr only measures
+size_t layout(vmg_s* h, double* base)
+{
+    ArenaPlan p;
+    for (int l = 0; l < h->nlev; ++l) {
+        VmgLevel& L = h->lev[l];
+        double** padded[7] = {&L.wx, &L.wy, &L.wz, &L.dinv, &L.dbase, &L.phi, &L.rhs};
+        for (auto pp : padded) {
+            size_t o = p.take((size_t)L.pad + (size_t)L.n + (size_t)L.pad);
+            if (base) *pp = base + o + L.pad;
+        }
+        for (int f = 0; f < 6; ++f) {
+            size_t o = p.take(plane_count(L, f));
+            if (base) L.wb[f] = base + o;
+        }
+        if (l > 0) {
+            size_t o = p.take((size_t)L.n);          if (base) L.a = base + o;
+            o = p.take(face_count(L, 0));            if (base) L.bx = base + o;
+            o = p.take(face_count(L, 1));            if (base) L.by = base + o;
+            o = p.take(face_count(L, 2));            if (base) L.bz = base + o;
+        }
+    }
+    for (int f = 0; f < 6; ++f) {
+        size_t o = p.take(plane_count(h->lev[0], f));
+        if (base) h->bcval[f] = base + o;
+    }
+    size_t o = p.take(32);
+    if (base) h->d_scal = base + o;
+    return p.off;
+}
+
+int finalize_dinv(vmg_s* h)
+{
+    for (int l = 0; l < h->nlev; ++l) {
+        VmgLevel& L = h->lev[l];
+        DinvArgs g;
+        g.dbase = L.dbase; g.dinv = L.dinv;
+        for (int f = 0; f < 6; ++f) { g.wb[f] = L.wb[f]; g.dirichlet[f] = h->bctype[f] == VMG_BC_DIRICHLET; }
+        g.nx = L.nx; g.ny = L.ny; g.nz = L.nz; g.three_d = h->three_d;
+        finalize_dinv_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(g);
+    }
+    CUDA_TRY(h, cudaGetLastError());
+    h->dinv_dirty = false;
+    h->graph_valid = false;
+    return VMG_OK;
+}
+
+bool singular(const vmg_s* h)
+{
+    int nd = h->three_d ? 6 : 4;
+    for (int f = 0; f < nd; ++f) if (h->bctype[f] == VMG_BC_DIRICHLET) return false;
+    return h->alpha == 0.0;
+}
+
+int ready(vmg_s* h)
+{
+    if (!h) return VMG_ERR_ARG;
+    if (!h->have_coeffs || !h->have_bc) return VMG_ERR_STATE;
+    if (h->dinv_dirty) return finalize_dinv(h);
+    return VMG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* vmg_strerror(int code)
+{
+    switch (code) {
+    case VMG_OK: return "ok";
+    case VMG_MAXCYCLES: return "max_vcycles reached before rtol";
+    case VMG_STALLED: return "residual stalled (fp64 floor)";
+    case VMG_ERR_ARG: return "invalid argument";
+    case VMG_ERR_SIZE: return "grid size not supported (bottom grid > 512 cells or a dimension < 2)";
+    case VMG_ERR_STATE: return "vmg_solve needs vmg_set_coeffs and vmg_set_bc first";
+    case VMG_ERR_SINGULAR: return "singular problem: all faces Neumann and no absorption term";
+    case VMG_ERR_DIVERGED: return "residual is NaN or Inf";
+    case VMG_ERR_CUDA: return "CUDA runtime error";
+    case VMG_ERR_ALLOC: return "allocation failed";
+    default: return "unknown status";
+    }
+}
+
+int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream)
+{
+    if (!out) return VMG_ERR_ARG;
+    *out = nullptr;
+    bool three_d = nz > 1;
+    if (nx < 2 || ny < 2 || nz < 1 || !(dx > 0) || !(dy > 0) || (three_d && !(dz > 0))) return VMG_ERR_SIZE;
+    int n[3] = {nx, ny, nz}, nlev = 1;
+    for (;;) {   // R11: halve while every active dimension is even and stays >= 2
+        bool ok = n[0] % 2 == 0 && n[0] / 2 >= 2 && n[1] % 2 == 0 && n[1] / 2 >= 2;
+        if (three_d) ok = ok && n[2] % 2 == 0 && n[2] / 2 >= 2;
+        if (!ok) break;
+        n[0] /= 2; n[1] /= 2; if (three_d) n[2] /= 2;
+        ++nlev;
+    }
+    if ((long long)n[0] * n[1] * n[2] > 512) return VMG_ERR_SIZE;
+    vmg_s* h = new (std::nothrow) vmg_s();
+    if (!h) return VMG_ERR_ALLOC;
+    h->nlev = nlev; h->three_d = three_d;
+    h->lev.resize(nlev);
+    for (int l = 0; l < nlev; ++l) {
+        VmgLevel& L = h->lev[l];
+        L.nx = nx >> l; L.ny = ny >> l; L.nz = three_d ? nz >> l : 1;
+        L.n = (long long)L.nx * L.ny * L.nz;
+        L.pad = (long long)round_up((size_t)L.nx * L.ny + L.nx + 2, 32);
+        L.hx = dx * (1 << l); L.hy = dy * (1 << l); L.hz = three_d ? dz * (1 << l) : 1.0;
+    }
+    cudaError_t e = cudaGetDevice(&h->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); delete h; return VMG_ERR_CUDA; }
+    if (cuda_stream) { h->stream = (cudaStream_t)cuda_stream; h->own_stream = false; }
+    else {
+        // a blocking stream: ordered with the legacy default stream, and capturable into a graph
+        if (cudaStreamCreate(&h->stream) != cudaSuccess) { (void)cudaGetLastError(); delete h; return VMG_ERR_CUDA; }
+        h->own_stream = true;
+    }
+    h->arena_bytes = layout(h, nullptr) * sizeof(double);
+    if (cudaMalloc(&h->arena, h->arena_bytes) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (h->own_stream) cudaStreamDestroy(h->stream);
+        delete h;
+        return VMG_ERR_ALLOC;
+    }
+    layout(h, (double*)h->arena);
+    if (cudaMemsetAsync(h->arena, 0, h->arena_bytes, h->stream) != cudaSuccess ||
+        cudaMallocHost((void**)&h->h_scal, 32 * sizeof(double)) != cudaSuccess ||
+        cudaStreamSynchronize(h->stream) != cudaSuccess) {
+        (void)cudaGetLastError();
+        cudaFree(h->arena);
+        if (h->own_stream) cudaStreamDestroy(h->stream);
+        delete h;
+        return VMG_ERR_CUDA;
+    }
+    plan_schedule(h);
+    *out = h;
+    return VMG_OK;
+}
+
+int vmg_destroy(vmg_handle h)
+{
+    if (!h) return VMG_ERR_ARG;
+    cudaStreamSynchronize(h->stream);
+    prof_collect(h);
+    for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
+    if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+    if (h->graph) cudaGraphDestroy(h->graph);
+    if (h->h_scal) cudaFreeHost(h->h_scal);
+    if (h->arena) cudaFree(h->arena);
+    if (h->own_stream) cudaStreamDestroy(h->stream);
+    (void)cudaGetLastError();
+    delete h;
+    return VMG_OK;
+}
+
+int vmg_last_cuda_error(vmg_handle h) { return h ? h->last_cuda_error : 0; }
+
+int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double* by, const double* bz,
+                   double alpha, double beta)
+{
+    if (!h) return VMG_ERR_ARG;
+    if (!bx != !by) return VMG_ERR_ARG;
+    if (h->three_d && (!bx != !bz)) return VMG_ERR_ARG;
+    if (!(beta > 0.0) || alpha < 0.0) return VMG_ERR_ARG;
+    h->alpha = a ? alpha : 0.0;
+    h->beta = beta;
+    int sz = h->three_d ? 2 : 1;
+    const double *fa = a, *fbx = bx, *fby = by, *fbz = h->three_d ? bz : nullptr;
+    long long setup_launches = 0;
+    ProfScope* ps = new ProfScope(h, VMG_PC_SETUP, &setup_launches);
+    for (int l = 0; l < h->nlev; ++l) {
+        VmgLevel& L = h->lev[l];
+        if (l > 0) {   // S0: average the previous level's raw coefficients
+            coarsen_a_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(fa, L.a, L.nx, L.ny, L.nz, sz);
+            coarsen_b_kernel<<<grid_for((long long)face_count(L, 0)), kThreads, 0, h->stream>>>(fbx, L.bx, L.nx, L.ny, L.nz, sz, 0);
+            coarsen_b_kernel<<<grid_for((long long)face_count(L, 1)), kThreads, 0, h->stream>>>(fby, L.by, L.nx, L.ny, L.nz, sz, 1);
+            if (h->three_d)
+                coarsen_b_kernel<<<grid_for((long long)face_count(L, 2)), kThreads, 0, h->stream>>>(fbz, L.bz, L.nx, L.ny, L.nz, sz, 2);
+            fa = L.a; fbx = L.bx; fby = L.by; fbz = h->three_d ? L.bz : nullptr;
+            setup_launches += h->three_d ? 4 : 3;
+        }
+        StencilBuildArgs g;
+        g.a = (l == 0 && !a) ? nullptr : fa;
+        g.bx = fbx; g.by = fby; g.bz = fbz;
+        g.wx = L.wx; g.wy = L.wy; g.wz = L.wz; g.dbase = L.dbase;
+        for (int f = 0; f < 6; ++f) g.wb[f] = L.wb[f];
+        g.nx = L.nx; g.ny = L.ny; g.nz = L.nz; g.three_d = h->three_d;
+        g.alpha = h->alpha; g.cx = beta / (L.hx * L.hx); g.cy = beta / (L.hy * L.hy);
+        g.cz = h->three_d ? beta / (L.hz * L.hz) : 0.0;
+        build_stencil_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(g);
+        ++setup_launches;
+    }
+    delete ps;
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    h->total_launches += setup_launches;
+    if (h->profile) prof_collect(h);
+    h->have_coeffs = true;
+    h->dinv_dirty = true;
+    return VMG_OK;
+}
+
+int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
+{
+    if (!h || !type) return VMG_ERR_ARG;
+    for (int f = 0; f < 6; ++f)
+        if (type[f] != VMG_BC_DIRICHLET && type[f] != VMG_BC_NEUMANN) return VMG_ERR_ARG;
+    for (int f = 0; f < 6; ++f) {
+        h->bctype[f] = type[f];
+        bool active = f < 4 || h->three_d;
+        h->bc_has_value[f] = active && value && value[f];
+        if (h->bc_has_value[f])
+            CUDA_TRY(h, cudaMemcpyAsync(h->bcval[f], value[f], plane_count(h->lev[0], f) * sizeof(double),
+                                        cudaMemcpyDeviceToDevice, h->stream));
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    h->have_bc = true;
+    h->dinv_dirty = true;
+    return VMG_OK;
+}
+
+int vmg_set_option(vmg_handle h, const char* key, double v)
+{
+    if (!h || !key) return VMG_ERR_ARG;
+    int iv = (int)v;
+    if (!strcmp(key, "nu1")) { if (iv < 0 || iv > 8) return VMG_ERR_ARG; h->nu1 = iv; }
+    else if (!strcmp(key, "nu2")) { if (iv < 0 || iv > 8) return VMG_ERR_ARG; h->nu2 = iv; }
+    else if (!strcmp(key, "bottom_sweeps")) { if (iv < 1) return VMG_ERR_ARG; h->nbottom = iv; }
+    else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
+    else if (!strcmp(key, "blocked")) { h->use_blocked = iv != 0; }
+    else if (!strcmp(key, "profile")) {
+        h->profile = iv != 0;
+        for (int c = 0; c < VMG_PC_COUNT; ++c) { h->prof_ms[c] = 0.0; h->prof_launches[c] = 0; }
+    }
+    else return VMG_ERR_ARG;
+    h->graph_valid = false;
+    plan_schedule(h);
+    return VMG_OK;
+}
+
+int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history)
+{
+    if (!h) return VMG_ERR_ARG;
+    if (cycles) *cycles = h->cycles;
+    if (relres) *relres = h->relres;
+    if (history) memcpy(history, h->hist.data(), h->hist.size() * sizeof(double));
+    return VMG_OK;
+}
+
+long long vmg_last_launch_count(vmg_handle h) { return h ? h->launches : 0; }
+long long vmg_total_launch_count(vmg_handle h) { return h ? h->total_launches : 0; }
+
+int vmg_get_profile(vmg_handle h, double ms[8], long long launches[8])
+{
+    if (!h) return VMG_ERR_ARG;
+    for (int c = 0; c < VMG_PC_COUNT; ++c) {
+        if (ms) ms[c] = h->prof_ms[c];
+        if (launches) launches[c] = h->prof_launches[c];
+    }
+    return VMG_OK;
+}
+
+// C5 of DESIGN.md: relres = ||btilde - A phi||_inf / ||btilde||_inf; stall rule; status codes.
+static int solve_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int max_vcycles)
+{
+    VmgLevel& L0 = h->lev[0];
+    unsigned long long* scal = (unsigned long long*)h->d_scal;
+
+    int rc = enqueue_fold_bc(h, rhs, L0.rhs);
+    if (rc != VMG_OK) return rc;
+    {
+        ProfScope ps(h, VMG_PC_COPY, nullptr);
+        CUDA_TRY(h, cudaMemcpyAsync(L0.phi, phi, L0.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    }
+    CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
+    {
+        ProfScope ps(h, VMG_PC_NORM, nullptr);
+        norm_inf_kernel<<<std::min<unsigned>(grid_for(L0.n), 4u * h->num_sms), kThreads, 0, h->stream>>>(L0.rhs, L0.n, scal + 0);
+    }
+    enqueue_residual_norm(h, scal + 1);
+    h->launches += 2;
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaMemcpyAsync(h->h_scal, scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    double nb = h->h_scal[0], r = h->h_scal[1];
+    int status = VMG_MAXCYCLES;
+    if (nb == 0.0) {
+        CUDA_TRY(h, cudaMemsetAsync(phi, 0, L0.n * sizeof(double), h->stream));
+        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+        h->hist.push_back(0.0);
+        return VMG_OK;
+    }
+    h->relres = r / nb;
+    h->hist.push_back(h->relres);
+    if (std::isnan(h->relres) || std::isinf(h->relres)) return VMG_ERR_DIVERGED;
+    if (rtol > 0.0 && h->relres <= rtol) status = VMG_OK;
+    else {
+        int slow = 0;
+        for (int c = 1; c <= max_vcycles; ++c) {
+            rc = run_vcycle_with_norm(h, scal + 1);       // graph replay or plain launches
+            if (rc != VMG_OK) return rc;
+            CUDA_TRY(h, cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+            CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+            h->relres = h->h_scal[1] / nb;
+            h->hist.push_back(h->relres);
+            h->cycles = c;
+            if (std::isnan(h->relres) || std::isinf(h->relres)) { status = VMG_ERR_DIVERGED; break; }
+            if (rtol > 0.0) {
+                if (h->relres <= rtol) { status = VMG_OK; break; }
+                slow = (h->hist[c] >= 0.9 * h->hist[c - 1]) ? slow + 1 : 0;
+                if (slow >= 3) { status = VMG_STALLED; break; }
+            }
+        }
+    }
+    {
+        ProfScope ps(h, VMG_PC_COPY, nullptr);
+        CUDA_TRY(h, cudaMemcpyAsync(phi, L0.phi, L0.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return status;
+}
+
+int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max_vcycles)
+{
+    if (!h || !rhs || !phi || max_vcycles < 0) return VMG_ERR_ARG;
+    int rc = ready(h);
+    if (rc != VMG_OK) return rc;
+    if (singular(h)) return VMG_ERR_SINGULAR;
+    h->hist.clear(); h->cycles = 0; h->relres = 0.0; h->launches = 0;
+    rc = solve_impl(h, rhs, phi, rtol, max_vcycles);
+    if (h->profile) { cudaStreamSynchronize(h->stream); prof_collect(h); }
+    h->total_launches += h->launches;
+    return rc;
+}
+
+}  // extern "C"
+
+#include "vmg_steps.inl"

@@ -1,0 +1,78 @@
+// vmg_internal.h -- data structures of libvmg (CUDA side only; shares nothing with oracle/).
+//
+// Internal stencil form of a level (built by vmg_set_coeffs / vmg_set_bc):
+//   wx[c] = beta*bx/hx^2 of the LOW-x face of cell c, stored per cell and 0 where that face is a domain
+//           boundary; the HIGH-x face weight of cell c is wx[c+1], which is the next row's (zero) low
+//           boundary entry when c is the last cell of a row.  Same for wy (stride nx) and wz (stride nx*ny).
+//   dinv[c] = 1 / D_c,  D_c = alpha*a_c + sum(interior face weights) + 2*sum(Dirichlet boundary face weights)
+//   dbase[c] = alpha*a_c + sum(interior face weights)          (boundary-type independent part of D_c)
+//   wb[f]    = boundary-face weights beta*b/h^2 on domain face f (a plane), used to finish dinv and by fold_bc
+// Every cell array is allocated with `pad` zeroed doubles before and after, so that c-1, c+1, c-nx, c+nx,
+// c-nx*ny, c+nx*ny are always readable and every out-of-domain neighbour is multiplied by a zero weight:
+// the kernels carry no boundary branches (PAPER.md:230,266,284 boundary kinds live in the coefficients).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <vector>
+
+// kernel classes for the optional per-kernel event profile (vmg_get_profile)
+enum { VMG_PC_SMOOTH0 = 0, VMG_PC_RESREST0 = 1, VMG_PC_PROLONG0 = 2, VMG_PC_COARSE = 3, VMG_PC_NORM = 4,
+       VMG_PC_FOLD = 5, VMG_PC_COPY = 6, VMG_PC_SETUP = 7, VMG_PC_COUNT = 8 };
+
+struct VmgProfEvent { int cls; long long launches; cudaEvent_t start, stop; };
+
+struct VmgLevel {
+    int nx = 0, ny = 0, nz = 0;
+    long long n = 0;          // cells
+    long long pad = 0;        // zeroed doubles before and after each padded array
+    double hx = 0, hy = 0, hz = 0;
+    // padded cell arrays (pointer to cell 0)
+    double *wx = nullptr, *wy = nullptr, *wz = nullptr, *dinv = nullptr, *dbase = nullptr;
+    double *phi = nullptr, *rhs = nullptr;
+    // boundary-face weight planes, order XLO..ZHI (unpadded)
+    double* wb[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    // averaged raw coefficients in the public layout (levels >= 1 only; level 0 reads the caller's arrays)
+    double *a = nullptr, *bx = nullptr, *by = nullptr, *bz = nullptr;
+};
+
+struct vmg_s {
+    int nlev = 0;
+    bool three_d = true;
+    std::vector<VmgLevel> lev;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    int device = 0;
+    int num_sms = 0;
+    double alpha = 0.0, beta = 1.0;
+    int bctype[6] = {1, 1, 1, 1, 1, 1};
+    double* bcval[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // device copies of value planes
+    bool bc_has_value[6] = {false, false, false, false, false, false};
+    bool have_coeffs = false, have_bc = false, dinv_dirty = true;
+    int nu1 = 3, nu2 = 3, nbottom = 32;
+    int use_graph = 1, use_blocked = 1;
+    int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
+    // device scalars
+    double* d_scal = nullptr;     // [0] = ||btilde||_inf bits, [1] = residual norm bits, ...
+    double* h_scal = nullptr;     // pinned host mirror
+    // arena
+    void* arena = nullptr;
+    size_t arena_bytes = 0;
+    // graph of one V-cycle (+ residual norm)
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
+    bool graph_valid = false;
+    // result of the last solve
+    int cycles = 0;
+    double relres = 0.0;
+    std::vector<double> hist;
+    int last_cuda_error = 0;
+    long long launches = 0;            // launches of the last solve
+    long long launches_per_cycle = 0;  // kernel nodes in one V-cycle
+    long long total_launches = 0;      // since vmg_create
+    // optional per-kernel-class event timing (option "profile"): plain launches, one event pair per group
+    bool profile = false;
+    std::vector<VmgProfEvent> prof_pending;
+    std::vector<cudaEvent_t> prof_pool;
+    double prof_ms[VMG_PC_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long prof_launches[VMG_PC_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0};
+};

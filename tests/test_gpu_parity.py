@@ -1,0 +1,230 @@
+"""GPU parity: the CUDA path (through the C-ABI of libvmg.so) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json:north_star): relative L-inf difference of phi <= 1e-10 after both reach relative
+residual 1e-12, V-cycle counts equal within 1.  Single steps: <= 1e-13 relative (rounding-order only:
+the GPU uses pre-multiplied face weights, a reciprocal diagonal and FMAs).
+"""
+import os
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import Oracle, OracleError
+from paper_2507_08200_b200 import inputs
+from paper_2507_08200_b200.inputs import DIRICHLET as D, NEUMANN as N
+
+pytestmark = pytest.mark.gpu
+
+STEP_TOL = 1e-13
+PHI_TOL = 1e-10
+
+
+def _binding():
+    from paper_2507_08200_b200 import binding
+    return binding
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def rel(a, b):
+    return np.abs(a - b).max() / max(np.abs(b).max(), 1e-300)
+
+
+# sizes span several 256-thread blocks / tiles with ragged tails, odd coarse grids and the 2-D path
+SIZES = [(40, 24, 16), (72, 40, 24), (16, 8, 8), (48, 40, 1), (88, 56, 24), (5, 3, 4), (144, 80, 48)]
+MIXED = [D, N, N, D, D, N]
+
+
+@pytest.mark.parametrize("dims", SIZES)
+def test_single_steps_match_oracle(dims):
+    b = _binding()
+    p = inputs.random_problem(*dims, seed=sum(dims), bc_type=MIXED, sigma=1.0)
+    o = Oracle.from_problem(p)
+    s, d = b.from_problem(p)
+    assert s.num_levels == o.num_levels
+    rng = np.random.default_rng(7)
+    for lev in range(o.num_levels):
+        assert s.level_dims(lev) == o.level_dims(lev)
+        nx, ny, nz = o.level_dims(lev)
+        if lev > 0:   # S0 coefficient averaging
+            ca = o.level_coeffs(lev)
+            ga = s.get_level_coeffs(lev)
+            for name, x, y in zip("a bx by bz".split(), ga, ca):
+                if name == "bz" and nz == 1 and p.nz == 1:
+                    continue
+                assert rel(x.cpu().numpy(), y) <= 1e-15, (lev, name)
+        phi = rng.standard_normal((nz, ny, nx))
+        rhs = rng.standard_normal((nz, ny, nx)) * 50.0
+        # S2 smoother, 1 and 3 sweeps
+        for ns in (1, 3):
+            assert rel(s.step_smooth(lev, dev(phi), dev(rhs), ns).cpu().numpy(), o.smooth(phi, rhs, ns, lev)) <= STEP_TOL
+        # residual
+        r_o = o.residual(phi, rhs, lev)
+        assert rel(s.step_residual(lev, dev(phi), dev(rhs)).cpu().numpy(), r_o) <= STEP_TOL
+        if lev + 1 < o.num_levels:
+            # S3 fused residual + restriction; S4 fused prolongation + correction
+            assert np.abs(s.step_residual_restrict(lev, dev(phi), dev(rhs)).cpu().numpy() - o.restrict(r_o, lev)).max() \
+                <= STEP_TOL * np.abs(r_o).max()
+            cnx, cny, cnz = o.level_dims(lev + 1)
+            e = rng.standard_normal((cnz, cny, cnx))
+            assert np.array_equal(s.step_prolong_correct(lev, dev(phi), dev(e)).cpu().numpy(), o.prolong_add(phi, e, lev))
+    # S1 fold_bc, S6 norm, one whole V-cycle (S7)
+    bt_o = o.fold_bc(p.rhs)
+    bt_g = s.step_fold_bc(d["rhs"]).cpu().numpy()
+    assert rel(bt_g, bt_o) <= STEP_TOL
+    assert s.step_norm_inf(dev(bt_o)) == np.abs(bt_o).max()
+    phi0 = rng.standard_normal(p.rhs.shape)
+    for graph in (0, 1):
+        s.set_option("graph", graph)
+        assert rel(s.step_vcycle(dev(phi0), dev(bt_o)).cpu().numpy(), o.vcycle(phi0, bt_o)) <= 1e-12
+    s.destroy()
+
+
+def solve_both(p, **opts):
+    b = _binding()
+    o = Oracle.from_problem(p)
+    s, d = b.from_problem(p)
+    for k, v in opts.items():
+        o.set_option(k, v) if k in ("nu1", "nu2", "bottom_sweeps") else None
+        s.set_option(k, v)
+    phi_o, st_o, cyc_o, rr_o, hist_o = o.solve(p.rhs, rtol=p.rtol, max_vcycles=p.max_vcycles)
+    phi_g = torch.zeros_like(d["rhs"])
+    st_g = s.solve(d["rhs"], phi_g, rtol=p.rtol, max_vcycles=p.max_vcycles)
+    cyc_g, rr_g, hist_g = s.get_info()
+    s.destroy()
+    return (phi_o, st_o, cyc_o, rr_o, hist_o), (phi_g.cpu().numpy(), st_g, cyc_g, rr_g, np.array(hist_g))
+
+
+def check_parity(p, **opts):
+    (phi_o, st_o, cyc_o, rr_o, hist_o), (phi_g, st_g, cyc_g, rr_g, hist_g) = solve_both(p, **opts)
+    assert st_o == st_g, (st_o, st_g)
+    assert abs(cyc_o - cyc_g) <= 1, (cyc_o, cyc_g)
+    if p.rtol > 0:
+        assert rr_o <= p.rtol and rr_g <= p.rtol
+    assert rel(phi_g, phi_o) <= PHI_TOL, rel(phi_g, phi_o)
+    # residual histories agree while above the rounding floor
+    m = min(len(hist_o), len(hist_g))
+    live = hist_o[:m] > 1e-11
+    assert np.all(np.abs(hist_g[:m][live] / hist_o[:m][live] - 1.0) < 1e-3)
+    return cyc_o, cyc_g, rel(phi_g, phi_o)
+
+
+@pytest.mark.parametrize("make", [lambda: inputs.config1(64), lambda: inputs.config2(32), lambda: inputs.config3(32),
+                                  lambda: inputs.config4(32), lambda: inputs.config4(32, sheath=True),
+                                  lambda: inputs.config5(64, cycles=20)],
+                         ids=["config1", "config2_32", "config3_64x32x32", "config4_64x32x32", "config4b", "config5_64"])
+def test_configs_reduced_size_parity(make):
+    check_parity(make())
+
+
+@pytest.mark.parametrize("make", [lambda: inputs.config2(128), lambda: inputs.config3(128), lambda: inputs.config4(128)],
+                         ids=["config2_128^3", "config3_256x128x128", "config4_256x128x128"])
+def test_configs_full_size_parity(make):
+    """BASELINE.json configs[1..3] at full size, in the launch configuration bench.py times (defaults)."""
+    p = make()
+    cyc_o, cyc_g, err = check_parity(p)
+    assert 8 <= cyc_g <= 12
+
+
+@pytest.mark.skipif(os.environ.get("VMG_FULL_CONFIG5", "0") != "1", reason="512^3 oracle run takes minutes; VMG_FULL_CONFIG5=1")
+def test_config5_full_size_parity():
+    check_parity(inputs.config5(512))
+
+
+@pytest.mark.parametrize("opts", [dict(nu1=2, nu2=2), dict(nu1=1, nu2=3, bottom_sweeps=8), dict(graph=0), dict(blocked=0)])
+def test_options_parity(opts):
+    check_parity(inputs.random_problem(48, 24, 24, seed=3, bc_type=[D, D, N, N, N, D]), **opts)
+
+
+def test_edge_cases_and_status_codes():
+    b = _binding()
+    p = inputs.random_problem(32, 16, 16, seed=5, bc_type=[D, D, N, N, N, N])
+    o = Oracle.from_problem(p)
+    s, d = b.from_problem(p)
+    phi = torch.zeros_like(d["rhs"])
+    assert s.solve(d["rhs"], phi, rtol=1e-9) == 0
+    cyc, rr, hist = s.get_info()
+    phi_o, st_o, cyc_o, rr_o, hist_o = o.solve(p.rhs, rtol=1e-9)
+    assert cyc == cyc_o and len(hist) == cyc + 1 and abs(hist[0] - 1.0) < 1e-15
+    assert s.last_launch_count() > 0
+    # warm start from the converged field: 0 cycles, phi untouched
+    keep = phi.clone()
+    assert s.solve(d["rhs"], phi, rtol=1e-9) == 0 and s.get_info()[0] == 0 and torch.equal(phi, keep)
+    # rtol <= 0: exactly max_vcycles cycles
+    phi.zero_()
+    assert s.solve(d["rhs"], phi, rtol=0.0, max_vcycles=3) == 1 and s.get_info()[0] == 3
+    phi3_o, *_ = o.solve(p.rhs, rtol=0.0, max_vcycles=3)
+    assert rel(phi.cpu().numpy(), phi3_o) <= 1e-12
+    # unreachable tolerance stalls on the rounding floor, like the oracle
+    phi.zero_()
+    assert s.solve(d["rhs"], phi, rtol=1e-30, max_vcycles=60) == 2
+    # zero rhs with homogeneous data: phi = 0 after 0 cycles
+    s.set_bc(p.bc_type, None)
+    phi.fill_(1.0)
+    assert s.solve(torch.zeros_like(phi), phi) == 0 and s.get_info()[0] == 0 and not phi.any()
+    # NaN in the right-hand side: DIVERGED, handle stays usable
+    bad = d["rhs"].clone()
+    bad[3, 3, 3] = float("nan")
+    with pytest.raises(b.VmgError) as e:
+        s.solve(bad, phi)
+    assert e.value.code == -5
+    phi.zero_()
+    assert s.solve(d["rhs"], phi, rtol=1e-9) == 0
+    # pure Neumann without absorption: SINGULAR
+    s.set_coeffs(None, d["bx"], d["by"], d["bz"], 0.0, 1.0)
+    s.set_bc([N] * 6, None)
+    with pytest.raises(b.VmgError) as e:
+        s.solve(d["rhs"], phi)
+    assert e.value.code == -4
+    s.destroy()
+    # solve before set_coeffs / set_bc: STATE
+    s2 = b.Vmg(16, 8, 8, 1.0, 1.0, 1.0)
+    with pytest.raises(b.VmgError) as e:
+        s2.solve(phi[:8, :8, :16].contiguous(), phi[:8, :8, :16].contiguous())
+    assert e.value.code == -3
+    s2.destroy()
+    with pytest.raises(b.VmgError) as e:
+        b.Vmg(1030, 1030, 1030, 1.0, 1.0, 1.0)
+    assert e.value.code == -2
+
+
+def test_null_coefficients_mean_a_zero_b_one_and_bc_order_is_free():
+    b = _binding()
+    p = inputs.config3(16)
+    o = Oracle.from_problem(p)
+    phi_o, st_o, cyc_o, *_ = o.solve(p.rhs)
+    d = b.upload(p)
+    s = b.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz)
+    s.set_bc(p.bc_type, d["bc_value"])                   # bc before coeffs is legal
+    s.set_coeffs(None, None, None, None, 0.0, 1.0)       # NULL a, NULL b
+    phi = torch.zeros_like(d["rhs"])
+    assert s.solve(d["rhs"], phi) == 0 and abs(s.get_info()[0] - cyc_o) <= 1
+    assert rel(phi.cpu().numpy(), phi_o) <= PHI_TOL
+    # changing BC types afterwards re-finalises the diagonal
+    types = [D, N, N, N, N, N]
+    s.set_bc(types, d["bc_value"])
+    o.set_bc(types, p.bc_value)
+    phi.zero_()
+    phi_o2, st2, cyc2, *_ = o.solve(p.rhs)
+    assert s.solve(d["rhs"], phi) == st2
+    assert rel(phi.cpu().numpy(), phi_o2) <= PHI_TOL
+    s.destroy()
+
+
+def test_user_stream_and_repeatability():
+    b = _binding()
+    p = inputs.config4(16)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        s, d = b.from_problem(p, stream=st)
+        phi1 = torch.zeros_like(d["rhs"])
+        phi2 = torch.zeros_like(d["rhs"])
+        assert s.solve(d["rhs"], phi1) == 0
+        assert s.solve(d["rhs"], phi2) == 0
+    st.synchronize()
+    assert torch.equal(phi1, phi2)          # red-black updates are order independent: bitwise repeatable
+    s.destroy()
