@@ -197,6 +197,9 @@ def run_vmg(args):
         phi = torch.zeros(p.rhs.shape, dtype=torch.float64, device=dev)
         flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # 256 MiB > 126 MB L2
         s = binding.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, stream=stream)
+        for kv in args.opt:
+            key, val = kv.split("=")
+            s.set_option(key, float(val))
     stream.synchronize()
 
     def step_resident():
@@ -298,7 +301,7 @@ def run_vmg(args):
         "config": {"workload": p.name, "cells": p.ncells, "levels": len(wm["cells"]), "smoother": "V(3,3) red-black GS",
                    "rtol": p.rtol, "cycles_per_solve": ncyc, "step": "vmg_set_coeffs + vmg_set_bc + vmg_solve",
                    "l2": "256 MiB flush write between timed steps; level-0 working set 201 MB > 126 MB L2",
-                   "multi_gpu": "replicas only"},
+                   "multi_gpu": "replicas only", "options": args.opt},
         "solves_per_s": world / solve_s, "vcycles_per_s": world * ncyc / solve_s,
         "solve_ms": solve_s * 1e3,
         "hbm_frac_solve": bytes_solve / solve_s / 1e9 / peak,
@@ -336,6 +339,7 @@ def main():
     ap.add_argument("--impl", default="vmg", choices=["vmg", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], help="vmg_set_option key=value (experiments)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "vmg" else args.warmup
     if args.impl == "reference":

@@ -50,6 +50,13 @@ struct vmg_s {
     bool have_coeffs = false, have_bc = false, dinv_dirty = true;
     int nu1 = 3, nu2 = 3, nbottom = 32;
     int use_graph = 1, use_blocked = 1;
+    // L2 wavefront schedule (vmg_sched.cuh): slab thickness in planes (0 = off) and the smallest level it is used on
+    int wf_planes = 4;
+    long long wf_min_cells = 1 << 20;
+    static constexpr int kMaxStages = 20;
+    cudaStream_t side[kMaxStages] = {};
+    bool side_ready = false;
+    std::vector<cudaEvent_t> wf_events;
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
     // device scalars
     double* d_scal = nullptr;     // [0] = ||btilde||_inf bits, [1] = residual norm bits, ...

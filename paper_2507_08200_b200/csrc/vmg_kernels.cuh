@@ -179,13 +179,15 @@ __device__ __forceinline__ double nb_sum(const LevelView& L, const double* __res
 }
 
 // S2 (baseline). One colour half-sweep: phi_c <- (rhs_c + sum w phi_nb) / D_c for (i+j+k)%2 == colour.
-__global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour)
+// Planes [k0, k1) only (the L2 wavefront schedule launches it slab by slab).
+__global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour,
+                                     int k0, int k1)
 {
     int hx = (L.nx + 1) >> 1;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long nt = (long long)hx * L.ny * L.nz;
+    long long nt = (long long)hx * L.ny * (k1 - k0);
     if (t >= nt) return;
-    int m = (int)(t % hx), j = (int)((t / hx) % L.ny), k = (int)(t / ((long long)hx * L.ny));
+    int m = (int)(t % hx), j = (int)((t / hx) % L.ny), k = k0 + (int)(t / ((long long)hx * L.ny));
     int i = 2 * m + ((colour + j + k) & 1);
     if (i >= L.nx) return;
     long long c = i + (long long)L.nx * j + L.nxy * k;
@@ -208,14 +210,16 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 }
 
 // S3 (baseline). Fused residual + restriction: one thread per coarse cell; also zeroes the coarse phi.
+// Coarse planes [K0, K1) only.
 __global__ void residual_restrict_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz)
+                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz, int K0, int K1)
 {
-    int cnx = L.nx >> 1, cny = L.ny >> 1, cnz = (sz == 2) ? (L.nz >> 1) : L.nz;
+    int cnx = L.nx >> 1, cny = L.ny >> 1;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long n = (long long)cnx * cny * cnz;
+    long long n = (long long)cnx * cny * (K1 - K0);
     if (t >= n) return;
-    int I = (int)(t % cnx), J = (int)((t / cnx) % cny), K = (int)(t / ((long long)cnx * cny));
+    int I = (int)(t % cnx), J = (int)((t / cnx) % cny), K = K0 + (int)(t / ((long long)cnx * cny));
+    t = I + (long long)cnx * (J + (long long)cny * K);
     double s = 0.0;
     for (int r = 0; r < sz; ++r)
         for (int q = 0; q < 2; ++q)
@@ -228,12 +232,14 @@ __global__ void residual_restrict_kernel(LevelView L, const double* __restrict__
 }
 
 // S4 (baseline). Fused prolongation + correction (piecewise constant, R9): phi_f += e_c[i/2, j/2, k/2].
+// Fine planes [k0, k1) only.
 __global__ void prolong_correct_kernel(double* __restrict__ phi, const double* __restrict__ e,
-                                       int nx, int ny, int nz, int sz)
+                                       int nx, int ny, int sz, int k0, int k1)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long n = (long long)nx * ny * nz;
+    long long n = (long long)nx * ny * (k1 - k0);
     if (t >= n) return;
+    t += (long long)nx * ny * k0;
     int i = (int)(t % nx), j = (int)((t / nx) % ny), k = (int)(t / ((long long)nx * ny));
     int cnx = nx >> 1, cny = ny >> 1;
     phi[t] += e[(i >> 1) + (long long)cnx * ((j >> 1) + (long long)cny * (sz == 2 ? (k >> 1) : k))];
@@ -279,12 +285,14 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
     block_max_to_global(m, out);
 }
 
+// planes [k0, k1) only; accumulates into *out with atomicMax (the caller zeroes it)
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                     unsigned long long* out)
+                                     unsigned long long* out, int k0, int k1)
 {
     double m = 0.0;
     bool nan = false;
-    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < L.n; t += (long long)gridDim.x * blockDim.x) {
+    long long t1 = L.nxy * k1;
+    for (long long t = L.nxy * k0 + blockIdx.x * (long long)blockDim.x + threadIdx.x; t < t1; t += (long long)gridDim.x * blockDim.x) {
         double x = fabs(residual_at(L, phi, rhs, t));
         nan |= (x != x);
         m = fmax(m, x);

@@ -90,6 +90,7 @@ def solve_both(p, **opts):
     s, d = b.from_problem(p)
     for k, v in opts.items():
         o.set_option(k, v) if k in ("nu1", "nu2", "bottom_sweeps") else None
+    for k, v in opts.items():
         s.set_option(k, v)
     phi_o, st_o, cyc_o, rr_o, hist_o = o.solve(p.rhs, rtol=p.rtol, max_vcycles=p.max_vcycles)
     phi_g = torch.zeros_like(d["rhs"])
@@ -135,9 +136,13 @@ def test_config5_full_size_parity():
     check_parity(inputs.config5(512))
 
 
-@pytest.mark.parametrize("opts", [dict(nu1=2, nu2=2), dict(nu1=1, nu2=3, bottom_sweeps=8), dict(graph=0), dict(blocked=0)])
+@pytest.mark.parametrize("opts", [dict(nu1=2, nu2=2), dict(nu1=1, nu2=3, bottom_sweeps=8), dict(graph=0), dict(blocked=0),
+                                  dict(wavefront_min_cells=0, wavefront_planes=2),
+                                  dict(wavefront_min_cells=0, wavefront_planes=4, graph=0),
+                                  dict(wavefront_min_cells=0, wavefront_planes=6, nu1=2, nu2=4),
+                                  dict(wavefront_min_cells=0, wavefront_planes=4, nu1=0, nu2=1)])
 def test_options_parity(opts):
-    check_parity(inputs.random_problem(48, 24, 24, seed=3, bc_type=[D, D, N, N, N, D]), **opts)
+    check_parity(inputs.random_problem(48, 24, 48, seed=3, bc_type=[D, D, N, N, N, D]), **opts)
 
 
 def test_edge_cases_and_status_codes():
