@@ -56,7 +56,7 @@ enum {
  * active dimension while all stay even and >= 2 afterwards (256x128x128 -> ... -> 4x2x2); the coarsest grid
  * must have <= 512 cells (VMG_ERR_SIZE otherwise).  cuda_stream is a cudaStream_t (NULL = legacy default
  * stream); every kernel, copy and graph of this handle is enqueued on it.  All device memory the handle
- * needs (about 6.9 fp64 arrays of nx*ny*nz) is allocated here; vmg_solve allocates nothing on the device. */
+ * needs (about 9.2 fp64 arrays of nx*ny*nz) is allocated here; vmg_solve allocates nothing on the device. */
 int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream);
 
 /* Coefficients.  a: cell array or NULL (a == 0, alpha ignored).  bx, by, bz: face arrays, or all NULL for
@@ -88,7 +88,9 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
 
 /* Options (key is a HOST C string): "nu1", "nu2" (pre/post red-black sweeps, default 3, 0..8),
  * "bottom_sweeps" (default 32), "graph" (1: replay the V-cycle as a CUDA graph, default; 0: plain launches),
- * "blocked" (1: temporally blocked smoother where available, default; 0: one kernel per colour),
+ * "blocked" (1: temporally blocked smoother passes with fused transfers, default; 0: one kernel per step),
+ * "block_min_cells" (smallest level the blocked smoother is used on, default 4096),
+ * "tail" (1: the coarsest levels run in one single-CTA launch, default; 0: one kernel per step),
  * "profile" (1: per-kernel-class event timing, see vmg_get_profile; implies plain launches; default 0). */
 int vmg_set_option(vmg_handle h, const char* key, double v);
 
@@ -116,6 +118,11 @@ int vmg_step_residual(vmg_handle h, int level, const double* phi, const double* 
 int vmg_step_residual_restrict(vmg_handle h, int level, const double* phi, const double* rhs, double* rhs_coarse);
 /* phi += P e_coarse */
 int vmg_step_prolong_correct(vmg_handle h, int level, double* phi, const double* e_coarse);
+/* the down-stroke of a level as vmg_solve runs it: nu1 sweeps (phi in/out), then rhs_coarse = mean over children
+ * of (rhs - A phi); on levels the blocked smoother covers these are the fused passes */
+int vmg_step_down(vmg_handle h, int level, double* phi, const double* rhs, double* rhs_coarse);
+/* the up-stroke of a level: phi += P e_coarse, then nu2 sweeps (phi in/out) */
+int vmg_step_up(vmg_handle h, int level, double* phi, const double* rhs, const double* e_coarse);
 /* one V-cycle from level 0 with an already folded right-hand side: phi in/out */
 int vmg_step_vcycle(vmg_handle h, double* phi, const double* btilde);
 /* ||v||_inf of a device array of n doubles -> HOST scalar */

@@ -20,7 +20,7 @@ STATUS = {0: "OK", 1: "MAXCYCLES", 2: "STALLED", -1: "ERR_ARG", -2: "ERR_SIZE", 
 SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_solve", "vmg_get_info", "vmg_set_option",
            "vmg_destroy", "vmg_strerror", "vmg_last_cuda_error", "vmg_num_levels", "vmg_level_dims",
            "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
-           "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_vcycle", "vmg_step_norm_inf",
+           "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_down", "vmg_step_up", "vmg_step_vcycle", "vmg_step_norm_inf",
            "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile"]
 
 _lib = None
@@ -54,6 +54,8 @@ def load():
     lib.vmg_step_residual.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
     lib.vmg_step_residual_restrict.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
     lib.vmg_step_prolong_correct.argtypes = [_vp, C.c_int, _vp, _vp]
+    lib.vmg_step_down.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
+    lib.vmg_step_up.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
     lib.vmg_step_vcycle.argtypes = [_vp, _vp, _vp]
     lib.vmg_step_norm_inf.argtypes = [_vp, _vp, C.c_longlong, C.POINTER(C.c_double)]
     lib.vmg_last_launch_count.argtypes = [_vp]
@@ -202,6 +204,19 @@ class Vmg:
         phi = phi.clone()
         self._chk(self._lib.vmg_step_prolong_correct(self._h, level, _ptr(phi), _ptr(e_coarse)),
                   "vmg_step_prolong_correct")
+        return phi
+
+    def step_down(self, level: int, phi, rhs):
+        """nu1 sweeps, then residual + restriction: returns (phi, rhs_coarse)."""
+        phi = phi.clone()
+        out = self._empty(level + 1)
+        self._chk(self._lib.vmg_step_down(self._h, level, _ptr(phi), _ptr(rhs), _ptr(out)), "vmg_step_down")
+        return phi, out
+
+    def step_up(self, level: int, phi, rhs, e_coarse):
+        """prolongation + correction, then nu2 sweeps: returns phi."""
+        phi = phi.clone()
+        self._chk(self._lib.vmg_step_up(self._h, level, _ptr(phi), _ptr(rhs), _ptr(e_coarse)), "vmg_step_up")
         return phi
 
     def step_vcycle(self, phi, btilde):

@@ -45,7 +45,7 @@ size_t layout(vmg_s* h, double* base)
     ArenaPlan p;
     for (int l = 0; l < h->nlev; ++l) {
         VmgLevel& L = h->lev[l];
-        double** padded[7] = {&L.wx, &L.wy, &L.wz, &L.dinv, &L.dbase, &L.phi, &L.rhs};
+        double** padded[8] = {&L.wx, &L.wy, &L.wz, &L.dinv, &L.dbase, &L.phi, &L.rhs, &L.phi2};
         for (auto pp : padded) {
             size_t o = p.take((size_t)L.pad + (size_t)L.n + (size_t)L.pad);
             if (base) *pp = base + o + L.pad;
@@ -185,8 +185,6 @@ int vmg_destroy(vmg_handle h)
     cudaStreamSynchronize(h->stream);
     prof_collect(h);
     for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
-    for (cudaEvent_t e : h->wf_events) cudaEventDestroy(e);
-    if (h->side_ready) for (int s = 0; s < vmg_s::kMaxStages; ++s) cudaStreamDestroy(h->side[s]);
     if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
     if (h->graph) cudaGraphDestroy(h->graph);
     if (h->h_scal) cudaFreeHost(h->h_scal);
@@ -272,8 +270,8 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "bottom_sweeps")) { if (iv < 1) return VMG_ERR_ARG; h->nbottom = iv; }
     else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
     else if (!strcmp(key, "blocked")) { h->use_blocked = iv != 0; }
-    else if (!strcmp(key, "wavefront_planes")) { if (iv < 0 || iv > 64) return VMG_ERR_ARG; h->wf_planes = iv; }
-    else if (!strcmp(key, "wavefront_min_cells")) { if (v < 0) return VMG_ERR_ARG; h->wf_min_cells = (long long)v; }
+    else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }
+    else if (!strcmp(key, "block_min_cells")) { if (v < 0) return VMG_ERR_ARG; h->block_min_cells = (long long)v; }
     else if (!strcmp(key, "profile")) {
         h->profile = iv != 0;
         for (int c = 0; c < VMG_PC_COUNT; ++c) { h->prof_ms[c] = 0.0; h->prof_launches[c] = 0; }

@@ -29,6 +29,8 @@ struct VmgLevel {
     // padded cell arrays (pointer to cell 0)
     double *wx = nullptr, *wy = nullptr, *wz = nullptr, *dinv = nullptr, *dbase = nullptr;
     double *phi = nullptr, *rhs = nullptr;
+    double *phi2 = nullptr;   // second phi buffer: passes of the blocked smoother ping-pong (tiles overlap)
+    int cur = 0;              // which buffer holds phi while a V-cycle is being enqueued (0: phi, 1: phi2)
     // boundary-face weight planes, order XLO..ZHI (unpadded)
     double* wb[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     // averaged raw coefficients in the public layout (levels >= 1 only; level 0 reads the caller's arrays)
@@ -50,14 +52,10 @@ struct vmg_s {
     bool have_coeffs = false, have_bc = false, dinv_dirty = true;
     int nu1 = 3, nu2 = 3, nbottom = 32;
     int use_graph = 1, use_blocked = 1;
-    // L2 wavefront schedule (vmg_sched.cuh): slab thickness in planes (0 = off) and the smallest level it is used on
-    int wf_planes = 4;
-    long long wf_min_cells = 1 << 20;
-    static constexpr int kMaxStages = 20;
-    cudaStream_t side[kMaxStages] = {};
-    bool side_ready = false;
-    std::vector<cudaEvent_t> wf_events;
+    int use_tail = 1;             // run the coarsest levels in one CTA (vmg_tail.cuh)
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
+    size_t tail_smem = 0;         // dynamic shared memory of the tail kernel
+    long long block_min_cells = 4096;   // smallest level the blocked smoother is used on
     // device scalars
     double* d_scal = nullptr;     // [0] = ||btilde||_inf bits, [1] = residual norm bits, ...
     double* h_scal = nullptr;     // pinned host mirror

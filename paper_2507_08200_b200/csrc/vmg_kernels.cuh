@@ -222,11 +222,10 @@ __global__ void residual_restrict_kernel(LevelView L, const double* __restrict__
     t = I + (long long)cnx * (J + (long long)cny * K);
     double s = 0.0;
     for (int r = 0; r < sz; ++r)
-        for (int q = 0; q < 2; ++q)
-            for (int p = 0; p < 2; ++p) {
-                long long c = (2 * I + p) + (long long)L.nx * (2 * J + q) + L.nxy * (sz * K + r);
-                s += residual_at(L, phi, rhs, c);
-            }
+        for (int q = 0; q < 2; ++q) {   // the x-pair first, then accumulated (the blocked kernel sums in this order too)
+            long long c = (2 * I) + (long long)L.nx * (2 * J + q) + L.nxy * (sz * K + r);
+            s += residual_at(L, phi, rhs, c) + residual_at(L, phi, rhs, c + 1);
+        }
     crhs[t] = s / (4.0 * sz);
     if (cphi) cphi[t] = 0.0;
 }

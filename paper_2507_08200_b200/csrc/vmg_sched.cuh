@@ -1,8 +1,12 @@
 // vmg_sched.cuh -- sequencing of one V-cycle (S7): which kernel runs each step on each level, plain
 // launches or one CUDA graph replay (north_star (4)).
+//   levels 0 .. tail_level-1 : blocked passes (vmg_block.cuh) where the level qualifies, else one launch per step
+//   levels tail_level .. last: one single-CTA launch (vmg_tail.cuh)
 #pragma once
 #include "vmg_internal.h"
 #include "vmg_kernels.cuh"
+#include "vmg_tail.cuh"
+#include "vmg_block.cuh"
 #include "../../include/vmg.h"
 #include <algorithm>
 
@@ -18,7 +22,8 @@ inline LevelView view(const VmgLevel& L)
 
 inline unsigned grid_for(long long n) { return (unsigned)cdiv(n, kThreads); }
 
-inline void plan_schedule(vmg_s* h) { (void)h; }
+inline double* cur_phi(VmgLevel& L) { return L.cur ? L.phi2 : L.phi; }
+inline double* other_phi(VmgLevel& L) { return L.cur ? L.phi : L.phi2; }
 
 // RAII event pair around a group of launches of one kernel class (only when option "profile" is on).
 struct ProfScope {
@@ -81,200 +86,286 @@ inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt)
     return cudaGetLastError() == cudaSuccess ? VMG_OK : VMG_ERR_CUDA;
 }
 
-// counts launches into *count
-inline void enqueue_smooth(vmg_s* h, int l, double* phi, const double* rhs, int nsweeps, long long* count)
+// ------------------------------------------------------------------------------------------------
+// plain path: one launch per step, in place on the level's current phi buffer
+// ------------------------------------------------------------------------------------------------
+inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count)
 {
     VmgLevel& L = h->lev[l];
     LevelView v = view(L);
-    ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
     long long nt = (long long)((L.nx + 1) / 2) * L.ny * L.nz;
     for (int s = 0; s < nsweeps; ++s)
         for (int colour = 0; colour < 2; ++colour) {
-            smooth_colour_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(v, phi, rhs, colour, 0, L.nz);
+            smooth_colour_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(v, cur_phi(L), L.rhs, colour, 0, L.nz);
             ++*count;
         }
 }
 
-inline void enqueue_residual_restrict(vmg_s* h, int l, const double* phi, const double* rhs, double* crhs,
-                                      double* cphi, long long* count)
+inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
 {
     VmgLevel& L = h->lev[l];
-    ProfScope ps(h, l == 0 ? VMG_PC_RESREST0 : VMG_PC_COARSE, count);
-    residual_restrict_kernel<<<grid_for(h->lev[l + 1].n), kThreads, 0, h->stream>>>(view(L), phi, rhs, crhs, cphi,
-                                                                                    h->three_d ? 2 : 1, 0, h->lev[l + 1].nz);
+    VmgLevel& C = h->lev[l + 1];
+    C.cur = 0;
+    residual_restrict_kernel<<<grid_for(C.n), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, C.rhs, C.phi,
+                                                                       h->three_d ? 2 : 1, 0, C.nz);
     ++*count;
 }
 
-inline void enqueue_prolong_correct(vmg_s* h, int l, double* phi, const double* e, long long* count)
+inline void plain_prolong_correct(vmg_s* h, int l, long long* count)
 {
     VmgLevel& L = h->lev[l];
-    ProfScope ps(h, l == 0 ? VMG_PC_PROLONG0 : VMG_PC_COARSE, count);
-    prolong_correct_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(phi, e, L.nx, L.ny, h->three_d ? 2 : 1, 0, L.nz);
+    prolong_correct_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(cur_phi(L), cur_phi(h->lev[l + 1]), L.nx, L.ny,
+                                                                     h->three_d ? 2 : 1, 0, L.nz);
     ++*count;
 }
 
 inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out)
 {
     VmgLevel& L = h->lev[0];
-    unsigned g = std::min<unsigned>(grid_for(L.n), 8u * (unsigned)h->num_sms);
+    unsigned g = std::min<unsigned>(grid_for(L.n), 16u * (unsigned)h->num_sms);
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    residual_norm_kernel<<<g, kThreads, 0, h->stream>>>(view(L), L.phi, L.rhs, out, 0, L.nz);
+    residual_norm_kernel<<<g, kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out, 0, L.nz);
 }
 
 // ------------------------------------------------------------------------------------------------
-// L2 wavefront schedule for one stroke of a level.  A stroke is a list of stages, each a
-// whole-level operation whose value at plane k depends on the previous stage at planes k-1, k, k+1 only:
-//   down-stroke: red, black (x nu1), residual+restriction          up-stroke: prolongation+correction, red, black (x nu2)
-//   [, residual norm].  Stage s of slab j covers planes [j*T - s, (j+1)*T - s): a parallelogram tiling of (z, stage)
-// without redundant work.  Stage s runs on its own stream, in slab order; it waits for stage s-1 of the same slab.
-// Up to S launches on S consecutive slabs are in flight together and the slabs they touch (about (S+1)*T planes of
-// the six arrays) stay resident in the 126 MB L2, so HBM sees each array once per stroke instead of once per stage.
-// Under stream capture the cross-stream events become edges of the V-cycle's CUDA graph.
+// S5: the coarse tail.  plan: the longest suffix of levels whose shared-memory blocks fit one CTA.
 // ------------------------------------------------------------------------------------------------
-enum StageKind { ST_SMOOTH = 0, ST_RESREST = 1, ST_PROLONG = 2, ST_NORM = 3 };
-struct Stage { int kind; int colour; };
+constexpr size_t kTailSmemCap = 200 * 1024;
 
-inline bool use_wavefront(const vmg_s* h, int l)
+inline int tail_guard(const vmg_s* h, const VmgLevel& L) { return (h->three_d ? L.nx * L.ny : 0) + L.nx + 2; }
+
+inline void plan_schedule(vmg_s* h)
+{
+    h->tail_level = -1;
+    h->tail_smem = 0;
+    if (!h->use_tail) return;
+    size_t doubles = 0;
+    int first = h->nlev;
+    for (int l = h->nlev - 1; l >= 0 && h->nlev - l <= kTailMaxLevels; --l) {
+        const VmgLevel& L = h->lev[l];
+        if (L.n > 4096) break;
+        size_t d = (size_t)tail_level_doubles((int)L.n, tail_guard(h, L));
+        if ((doubles + d) * sizeof(double) > kTailSmemCap) break;
+        doubles += d;
+        first = l;
+    }
+    if (first == h->nlev) return;
+    h->tail_level = first;
+    h->tail_smem = doubles * sizeof(double);
+    cudaFuncSetAttribute(coarse_tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmemCap);
+    (void)cudaGetLastError();
+}
+
+inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* count)
+{
+    TailArgs g;
+    int first = h->tail_level, off = 0;
+    g.nl = h->nlev - first;
+    for (int l = first; l < h->nlev; ++l) {
+        VmgLevel& L = h->lev[l];
+        TailLevel& T = g.lev[l - first];
+        L.cur = 0;
+        T.wx = L.wx; T.wy = L.wy; T.wz = L.wz; T.dinv = L.dinv; T.phi = L.phi; T.rhs = L.rhs;
+        T.nx = L.nx; T.ny = L.ny; T.nz = L.nz; T.n = (int)L.n; T.nxy = L.nx * L.ny;
+        T.zs = h->three_d ? T.nxy : 0;
+        T.guard = tail_guard(h, L);
+        T.off = off;
+        off += tail_level_doubles(T.n, T.guard);
+    }
+    g.nu1 = h->nu1; g.nu2 = h->nu2; g.nbottom = h->nbottom; g.sz = h->three_d ? 2 : 1;
+    g.whole = first == 0;
+    g.norm_out = first == 0 ? norm_out : nullptr;
+    int threads = (int)std::min<long long>(kTailThreads, std::max<long long>(64, (h->lev[first].n / 2 + 31) / 32 * 32));
+    ProfScope ps(h, VMG_PC_COARSE, count);
+    coarse_tail_kernel<<<1, threads, h->tail_smem, h->stream>>>(g);
+    ++*count;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2-S4, S6: blocked passes.  Tile width 40 (32 interior + 2 x 4 halo); the tile height is the largest even number
+// of rows whose rings fit 227 KB of shared memory with at most 768 threads (one thread per x-pair).
+// ------------------------------------------------------------------------------------------------
+constexpr int kBlkNXT = 40;
+constexpr int kBlkMaxSmem = 232448;
+constexpr int kBlkMaxPairs = 768;
+
+constexpr int blk_pick_nyt(int S, int TAIL)
+{
+    int best = 0;
+    for (int nyt = 2 * (S + (TAIL ? 1 : 0)) + 2; nyt <= 64; nyt += 2) {
+        long long np = (long long)(kBlkNXT / 2) * nyt;
+        int rp = S + 2 + (TAIL ? 1 : 0), rc = S + (TAIL ? 1 : 0), rz = rc + 1;
+        long long smem = ((long long)(rp + 4 * rc + rz) * 2 * np + (TAIL == BT_RESTRICT ? np : 0)) * 8;
+        if (np <= kBlkMaxPairs && smem <= kBlkMaxSmem) best = nyt;
+    }
+    return best;
+}
+
+template <int S, int TAIL, bool PROLONG>
+struct BlkKernel {
+    static constexpr int NYT = blk_pick_nyt(S, TAIL);
+    using C = BlockCfg<S, TAIL, kBlkNXT, NYT>;
+    static void prepare()
+    {
+        cudaFuncSetAttribute(smooth_block_kernel<S, TAIL, PROLONG, kBlkNXT, NYT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)C::SMEM);
+    }
+    static void launch(vmg_s* h, BlockArgs g)
+    {
+        g.ntx = (int)cdiv(g.nx, C::TX); g.nty = (int)cdiv(g.ny, C::TY);
+        g.W = (long long)g.ntx * g.nty * g.nz;
+        unsigned grid = (unsigned)std::max<long long>(1, std::min<long long>(h->num_sms, g.W / 2));
+        smooth_block_kernel<S, TAIL, PROLONG, kBlkNXT, NYT><<<grid, C::NT, C::SMEM, h->stream>>>(g);
+    }
+};
+
+#define VMG_BLK_CASE(S_, T_, P_)                                             \
+    if (prepare_all) BlkKernel<S_, T_, P_>::prepare();                       \
+    else if (S == S_ && tail == T_ && prolong == P_) { BlkKernel<S_, T_, P_>::launch(h, g); return; }
+
+inline void blk_run(vmg_s* h, const BlockArgs& g, int S, int tail, bool prolong, bool prepare_all = false)
+{
+    VMG_BLK_CASE(1, 0, false) VMG_BLK_CASE(1, 0, true) VMG_BLK_CASE(1, 1, false) VMG_BLK_CASE(1, 1, true)
+    VMG_BLK_CASE(1, 2, false) VMG_BLK_CASE(1, 2, true)
+    VMG_BLK_CASE(2, 0, false) VMG_BLK_CASE(2, 0, true) VMG_BLK_CASE(2, 1, false) VMG_BLK_CASE(2, 1, true)
+    VMG_BLK_CASE(2, 2, false) VMG_BLK_CASE(2, 2, true)
+    VMG_BLK_CASE(3, 0, false) VMG_BLK_CASE(3, 0, true) VMG_BLK_CASE(3, 1, false) VMG_BLK_CASE(3, 1, true)
+    VMG_BLK_CASE(3, 2, false) VMG_BLK_CASE(3, 2, true)
+}
+#undef VMG_BLK_CASE
+
+// once per process, outside any stream capture
+inline void prepare_blocked(vmg_s* h)
+{
+    static bool done = false;
+    if (done) return;
+    BlockArgs g{};
+    blk_run(h, g, 0, 0, false, true);
+    (void)cudaGetLastError();
+    done = true;
+}
+
+inline bool blocked_ok(const vmg_s* h, int l)
 {
     const VmgLevel& L = h->lev[l];
-    return h->use_blocked && h->wf_planes >= 2 && h->three_d && L.n >= h->wf_min_cells && L.nz >= 4 * h->wf_planes &&
-           l + 1 < h->nlev;
+    return h->use_blocked && h->three_d && L.nx % 2 == 0 && L.ny % 2 == 0 && L.nz % 2 == 0 && L.n >= h->block_min_cells;
 }
 
-inline void launch_stage(vmg_s* h, int l, const Stage& st, int k0, int k1, cudaStream_t stream, unsigned long long* norm_out)
+// nhalf colour half-sweeps starting with colour `colour0` on level l, as ceil(nhalf/3) blocked passes; the first
+// pass may add the coarse correction while loading (prolong), the last may end with a residual stage (tail).
+inline void blocked_sweeps(vmg_s* h, int l, int nhalf, int colour0, bool prolong, int tail, unsigned long long* norm_out,
+                           long long* count)
 {
     VmgLevel& L = h->lev[l];
-    LevelView v = view(L);
-    int sz = h->three_d ? 2 : 1;
-    switch (st.kind) {
-    case ST_SMOOTH: {
-        long long nt = (long long)((L.nx + 1) / 2) * L.ny * (k1 - k0);
-        smooth_colour_kernel<<<grid_for(nt), kThreads, 0, stream>>>(v, L.phi, L.rhs, st.colour, k0, k1);
-        break;
-    }
-    case ST_RESREST: {
-        VmgLevel& C = h->lev[l + 1];
-        long long nt = (long long)C.nx * C.ny * ((k1 - k0) / 2);
-        residual_restrict_kernel<<<grid_for(nt), kThreads, 0, stream>>>(v, L.phi, L.rhs, C.rhs, C.phi, sz, k0 / 2, k1 / 2);
-        break;
-    }
-    case ST_PROLONG: {
-        long long nt = (long long)L.nx * L.ny * (k1 - k0);
-        prolong_correct_kernel<<<grid_for(nt), kThreads, 0, stream>>>(L.phi, h->lev[l + 1].phi, L.nx, L.ny, sz, k0, k1);
-        break;
-    }
-    case ST_NORM: {
-        long long nt = (long long)L.nx * L.ny * (k1 - k0);
-        unsigned g = std::min<unsigned>(grid_for(nt), 8u * (unsigned)h->num_sms);
-        residual_norm_kernel<<<g, kThreads, 0, stream>>>(v, L.phi, L.rhs, norm_out, k0, k1);
-        break;
-    }
-    }
-}
-
-// creates the side streams and the event pool (outside any stream capture)
-inline void prepare_wavefront(vmg_s* h)
-{
-    size_t need = 0;
-    for (int l = 0; l + 1 < h->nlev; ++l)
-        if (use_wavefront(h, l)) {
-            size_t S = 2 * (size_t)std::max(h->nu1, h->nu2) + 2;
-            size_t J = (size_t)cdiv(h->lev[l].nz + (long long)S - 1, h->wf_planes);
-            need = std::max(need, S * J + S + 1);
+    int passes = (nhalf + 2) / 3, base = nhalf / passes, rem = nhalf % passes, done = 0;
+    for (int p = 0; p < passes; ++p) {
+        int S = base + (p < rem ? 1 : 0);
+        BlockArgs g{};
+        g.wx = L.wx; g.wy = L.wy; g.wz = L.wz; g.dinv = L.dinv; g.rhs = L.rhs;
+        g.phi_in = cur_phi(L); g.phi_out = other_phi(L);
+        g.nx = L.nx; g.ny = L.ny; g.nz = L.nz; g.nxy = (long long)L.nx * L.ny;
+        g.colour0 = (colour0 + done) & 1;
+        bool first = p == 0, last = p == passes - 1;
+        int T = last ? tail : BT_NONE;
+        if ((first && prolong) || T == BT_RESTRICT) {
+            VmgLevel& C = h->lev[l + 1];
+            g.cnx = C.nx; g.cny = C.ny;
+            if (first && prolong) g.e = cur_phi(C);
+            if (T == BT_RESTRICT) { C.cur = 0; g.crhs = C.rhs; g.cphi = C.phi; }
         }
-    if (need == 0) return;
-    if (!h->side_ready) {
-        for (int s = 0; s < vmg_s::kMaxStages; ++s) cudaStreamCreateWithFlags(&h->side[s], cudaStreamNonBlocking);
-        h->side_ready = true;
-    }
-    while (h->wf_events.size() < need) {
-        cudaEvent_t e;
-        cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
-        h->wf_events.push_back(e);
+        g.norm_out = norm_out;
+        blk_run(h, g, S, T, first && prolong);
+        L.cur ^= 1;
+        done += S;
+        ++*count;
     }
 }
 
-inline void enqueue_wavefront(vmg_s* h, int l, const std::vector<Stage>& stages, unsigned long long* norm_out, long long* count)
+// leaves phi of level l in its primary buffer
+inline void settle_phi(vmg_s* h, int l)
 {
     VmgLevel& L = h->lev[l];
-    const int S = (int)stages.size(), T = h->wf_planes, nz = L.nz;
-    const int J = (int)cdiv(nz + S - 1, T);
-    if ((size_t)S * J + S + 1 > h->wf_events.size()) return;   // prepare_wavefront() sizes the pool; cannot happen
-    auto ev = [&](int s, int j) { return h->wf_events[(size_t)s * J + j]; };
-    cudaEvent_t fork = h->wf_events[(size_t)S * J + S];
-    cudaEventRecord(fork, h->stream);
-    for (int s = 0; s < S; ++s) cudaStreamWaitEvent(h->side[s], fork, 0);
-    for (int j = 0; j < J; ++j)
-        for (int s = 0; s < S; ++s) {
-            int k0 = std::max(0, j * T - s), k1 = std::min(nz, (j + 1) * T - s);
-            if (s > 0) cudaStreamWaitEvent(h->side[s], ev(s - 1, j), 0);
-            if (k1 > k0) { launch_stage(h, l, stages[s], k0, k1, h->side[s], norm_out); ++*count; }
-            cudaEventRecord(ev(s, j), h->side[s]);
-        }
-    for (int s = 0; s < S; ++s) {
-        cudaEvent_t done = h->wf_events[(size_t)S * J + s];
-        cudaEventRecord(done, h->side[s]);
-        cudaStreamWaitEvent(h->stream, done, 0);
+    if (L.cur == 0) return;
+    cudaMemcpyAsync(L.phi, L.phi2, L.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream);
+    L.cur = 0;
+}
+
+// nsweeps red-black sweeps on the level's phi (primary buffer in, primary buffer out)
+inline void enqueue_smooth(vmg_s* h, int l, int nsweeps, long long* count)
+{
+    ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
+    h->lev[l].cur = 0;
+    if (nsweeps > 0 && blocked_ok(h, l)) {
+        blocked_sweeps(h, l, 2 * nsweeps, 0, false, BT_NONE, nullptr, count);
+        settle_phi(h, l);
+    } else {
+        plain_smooth(h, l, nsweeps, count);
     }
 }
 
 // down-stroke of level l: nu1 sweeps then residual+restriction into level l+1 (which also zeroes its phi)
 inline void enqueue_down(vmg_s* h, int l, long long* count)
 {
-    VmgLevel& L = h->lev[l];
-    if (use_wavefront(h, l) && (h->wf_planes % 2 == 0)) {
+    if (h->nu1 > 0 && blocked_ok(h, l)) {
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
-        std::vector<Stage> st;
-        for (int s = 0; s < h->nu1; ++s) { st.push_back({ST_SMOOTH, 0}); st.push_back({ST_SMOOTH, 1}); }
-        st.push_back({ST_RESREST, 0});
-        enqueue_wavefront(h, l, st, nullptr, count);
+        blocked_sweeps(h, l, 2 * h->nu1, 0, false, BT_RESTRICT, nullptr, count);
         return;
     }
-    enqueue_smooth(h, l, L.phi, L.rhs, h->nu1, count);
-    enqueue_residual_restrict(h, l, L.phi, L.rhs, h->lev[l + 1].rhs, h->lev[l + 1].phi, count);
+    {
+        ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
+        plain_smooth(h, l, h->nu1, count);
+    }
+    ProfScope ps(h, l == 0 ? VMG_PC_RESREST0 : VMG_PC_COARSE, count);
+    plain_residual_restrict(h, l, count);
 }
 
-// up-stroke of level l: prolongation+correction from level l+1 then nu2 sweeps [then the residual norm (level 0)]
-// returns true if the residual norm was fused into the stroke
+// up-stroke of level l: prolongation+correction from level l+1 then nu2 sweeps [then the residual norm (level 0)].
+// Returns true if the residual norm was fused into the stroke.
 inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long* count)
 {
-    VmgLevel& L = h->lev[l];
-    if (use_wavefront(h, l)) {
+    if (h->nu2 > 0 && blocked_ok(h, l)) {
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
-        std::vector<Stage> st;
-        st.push_back({ST_PROLONG, 0});
-        for (int s = 0; s < h->nu2; ++s) { st.push_back({ST_SMOOTH, 0}); st.push_back({ST_SMOOTH, 1}); }
-        bool fuse_norm = (l == 0 && norm_out != nullptr);
-        if (fuse_norm) st.push_back({ST_NORM, 0});
-        enqueue_wavefront(h, l, st, norm_out, count);
-        return fuse_norm;
+        bool fuse = l == 0 && norm_out != nullptr;
+        blocked_sweeps(h, l, 2 * h->nu2, 0, true, fuse ? BT_NORM : BT_NONE, norm_out, count);
+        return fuse;
     }
-    enqueue_prolong_correct(h, l, L.phi, h->lev[l + 1].phi, count);
-    enqueue_smooth(h, l, L.phi, L.rhs, h->nu2, count);
+    {
+        ProfScope ps(h, l == 0 ? VMG_PC_PROLONG0 : VMG_PC_COARSE, count);
+        plain_prolong_correct(h, l, count);
+    }
+    ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
+    plain_smooth(h, l, h->nu2, count);
     return false;
 }
 
-// C4: one V-cycle on the handle's own level arrays (level-0 phi / rhs = btilde already in place).
+// C4: one V-cycle on the handle's own level arrays (level-0 phi / rhs = btilde already in place, primary buffer).
 // If norm_out is given, *norm_out (zeroed here) receives the bit pattern of ||rhs - A phi||_inf on level 0.
 inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* count)
 {
-    int last = h->nlev - 1;
+    const int last = h->nlev - 1;
+    const int tail = h->tail_level >= 0 ? h->tail_level : last;   // first level not handled stroke by stroke
     if (norm_out) cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
-    for (int l = 0; l < last; ++l) enqueue_down(h, l, count);
-    {
+    for (int l = 0; l <= last; ++l) h->lev[l].cur = 0;
+    for (int l = 0; l < tail; ++l) enqueue_down(h, l, count);
+    bool norm_done = false;
+    if (h->tail_level >= 0) {
+        enqueue_tail(h, norm_out, count);
+        norm_done = h->tail_level == 0 && norm_out;
+    } else {
         VmgLevel& B = h->lev[last];
         if (last == 0) cudaMemsetAsync(B.phi, 0, B.n * sizeof(double), h->stream);   // single level: bottom from zero
-        enqueue_smooth(h, last, B.phi, B.rhs, h->nbottom, count);
+        ProfScope ps(h, VMG_PC_COARSE, count);
+        plain_smooth(h, last, h->nbottom, count);
     }
-    bool norm_done = false;
-    for (int l = last - 1; l >= 0; --l) norm_done = enqueue_up(h, l, l == 0 ? norm_out : nullptr, count);
+    for (int l = tail - 1; l >= 0; --l) norm_done = enqueue_up(h, l, l == 0 ? norm_out : nullptr, count);
     if (norm_out && !norm_done) { enqueue_residual_norm(h, norm_out); ++*count; }
+    settle_phi(h, 0);
 }
 
 // V-cycle followed by the residual norm into *out (device), as a graph replay when enabled.
 inline int run_vcycle_with_norm(vmg_s* h, unsigned long long* out)
 {
-    prepare_wavefront(h);
+    prepare_blocked(h);
     auto body = [&](long long* count) { enqueue_vcycle(h, out, count); };
     if (!h->use_graph || h->profile) {
         long long count = 0;

@@ -62,7 +62,8 @@ int vmg_step_smooth(vmg_handle h, int level, double* phi, const double* rhs, int
     if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
     if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
     long long count = 0;
-    enqueue_smooth(h, level, L.phi, L.rhs, nsweeps, &count);
+    prepare_blocked(h);
+    enqueue_smooth(h, level, nsweeps, &count);
     if ((rc = stage_in(h, phi, L.phi, L.n)) != VMG_OK) return rc;
     return finish(h);
 }
@@ -88,7 +89,8 @@ int vmg_step_residual_restrict(vmg_handle h, int level, const double* phi, const
     if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
     if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
     long long count = 0;
-    enqueue_residual_restrict(h, level, L.phi, L.rhs, h->lev[level + 1].rhs, h->lev[level + 1].phi, &count);
+    L.cur = 0;
+    plain_residual_restrict(h, level, &count);
     if ((rc = stage_in(h, rhs_coarse, h->lev[level + 1].rhs, h->lev[level + 1].n)) != VMG_OK) return rc;
     return finish(h);
 }
@@ -101,8 +103,47 @@ int vmg_step_prolong_correct(vmg_handle h, int level, double* phi, const double*
     if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
     if ((rc = stage_in(h, h->lev[level + 1].phi, e_coarse, h->lev[level + 1].n)) != VMG_OK) return rc;
     long long count = 0;
-    enqueue_prolong_correct(h, level, L.phi, h->lev[level + 1].phi, &count);
+    L.cur = 0; h->lev[level + 1].cur = 0;
+    plain_prolong_correct(h, level, &count);
     if ((rc = stage_in(h, phi, L.phi, L.n)) != VMG_OK) return rc;
+    return finish(h);
+}
+
+int vmg_step_down(vmg_handle h, int level, double* phi, const double* rhs, double* rhs_coarse)
+{
+    if (bad_level(h, level) || level + 1 >= h->nlev || !phi || !rhs || !rhs_coarse) return VMG_ERR_ARG;
+    int rc = ready(h);
+    if (rc != VMG_OK) return rc;
+    VmgLevel& L = h->lev[level];
+    VmgLevel& C = h->lev[level + 1];
+    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
+    prepare_blocked(h);
+    long long count = 0;
+    L.cur = 0;
+    enqueue_down(h, level, &count);
+    if ((rc = stage_in(h, phi, cur_phi(L), L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, rhs_coarse, C.rhs, C.n)) != VMG_OK) return rc;
+    L.cur = 0;
+    return finish(h);
+}
+
+int vmg_step_up(vmg_handle h, int level, double* phi, const double* rhs, const double* e_coarse)
+{
+    if (bad_level(h, level) || level + 1 >= h->nlev || !phi || !rhs || !e_coarse) return VMG_ERR_ARG;
+    int rc = ready(h);
+    if (rc != VMG_OK) return rc;
+    VmgLevel& L = h->lev[level];
+    VmgLevel& C = h->lev[level + 1];
+    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, C.phi, e_coarse, C.n)) != VMG_OK) return rc;
+    prepare_blocked(h);
+    long long count = 0;
+    L.cur = 0; C.cur = 0;
+    enqueue_up(h, level, nullptr, &count);
+    if ((rc = stage_in(h, phi, cur_phi(L), L.n)) != VMG_OK) return rc;
+    L.cur = 0;
     return finish(h);
 }
 

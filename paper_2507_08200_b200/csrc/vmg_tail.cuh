@@ -1,0 +1,164 @@
+// vmg_tail.cuh -- S5: the coarse tail of the V-cycle in ONE CTA (north_star (3): "a single-CTA smoother";
+// SURVEY.md 8(a) S5).  Every level from `first` down to the bottom lives in shared memory for the whole
+// launch: pre-smoothing, residual+restriction, the fixed-sweep bottom solve (R11), prolongation+correction and
+// post-smoothing run back to back with __syncthreads() between colour half-sweeps instead of kernel launches.
+// The arithmetic of every step is the same expression, in the same order, as the per-step kernels of
+// vmg_kernels.cuh, so the tail is bitwise identical to the plain launches it replaces.
+#pragma once
+#include "vmg_kernels.cuh"
+
+namespace vmg {
+
+constexpr int kTailMaxLevels = 12;
+constexpr int kTailThreads = 1024;
+
+struct TailLevel {
+    const double *wx, *wy, *wz, *dinv;   // global, internal stencil form (cell 0)
+    double *phi, *rhs;                   // global level arrays (cell 0)
+    int nx, ny, nz, n, nxy, guard, off;  // off: offset (doubles) of this level's block in shared memory
+    int zs;                              // stride to the z neighbours: nxy in 3-D, 0 in 2-D (their weight is zero)
+};
+
+struct TailArgs {
+    TailLevel lev[kTailMaxLevels];
+    int nl;                    // levels in the tail; lev[nl-1] is the bottom
+    int nu1, nu2, nbottom, sz; // sz = 2 in 3-D, 1 in 2-D (children per coarse cell along z)
+    int whole;                 // 1: lev[0] is level 0 of the hierarchy (phi is an initial guess, not zero)
+    unsigned long long* norm_out;   // whole == 1: ||rhs - A phi||_inf bits after the cycle (may be NULL)
+};
+
+// shared-memory block of a level: six arrays (phi, rhs, dinv, wx, wy, wz), each `guard` zeroed doubles, n cells,
+// `guard` zeroed doubles; guard >= zs + nx + 2 so that every stencil neighbour of every cell is addressable
+// and every out-of-domain neighbour meets a zero weight (same convention as the global arrays).
+__host__ __device__ inline int tail_stride(int n, int guard) { return ((n + 2 * guard + 3) / 4) * 4; }
+__host__ __device__ inline int tail_level_doubles(int n, int guard) { return 6 * tail_stride(n, guard); }
+
+struct TailSmem {
+    double *phi, *rhs, *dinv, *wx, *wy, *wz;
+    __device__ TailSmem(double* base, const TailLevel& L)
+    {
+        int st = tail_stride(L.n, L.guard);
+        double* p = base + L.off + L.guard;
+        phi = p; rhs = p + st; dinv = p + 2 * st; wx = p + 3 * st; wy = p + 4 * st; wz = p + 5 * st;
+    }
+};
+
+__device__ __forceinline__ double tail_nb_sum(const TailSmem& s, const TailLevel& L, int c)
+{
+    double v = s.wx[c] * s.phi[c - 1];
+    v = fma(s.wx[c + 1], s.phi[c + 1], v);
+    v = fma(s.wy[c], s.phi[c - L.nx], v);
+    v = fma(s.wy[c + L.nx], s.phi[c + L.nx], v);
+    v = fma(s.wz[c], s.phi[c - L.zs], v);
+    v = fma(s.wz[c + L.zs], s.phi[c + L.zs], v);
+    return v;
+}
+
+__device__ __forceinline__ void tail_smooth(const TailSmem& s, const TailLevel& L, int nsweeps)
+{
+    const int hx = (L.nx + 1) >> 1;
+    const int nt = hx * L.ny * L.nz;
+    for (int sw = 0; sw < nsweeps; ++sw)
+        for (int colour = 0; colour < 2; ++colour) {
+            for (int t = threadIdx.x; t < nt; t += blockDim.x) {
+                int m = t % hx, j = (t / hx) % L.ny, k = t / (hx * L.ny);
+                int i = 2 * m + ((colour + j + k) & 1);
+                if (i < L.nx) {
+                    int c = i + L.nx * j + L.nxy * k;
+                    s.phi[c] = s.dinv[c] * (s.rhs[c] + tail_nb_sum(s, L, c));
+                }
+            }
+            __syncthreads();
+        }
+}
+
+__device__ __forceinline__ double tail_residual_at(const TailSmem& s, const TailLevel& L, int c)
+{
+    return s.rhs[c] + tail_nb_sum(s, L, c) - s.phi[c] / s.dinv[c];
+}
+
+__global__ void __launch_bounds__(kTailThreads, 1) coarse_tail_kernel(TailArgs g)
+{
+    extern __shared__ __align__(16) double tail_smem[];
+    const int tid = threadIdx.x, nth = blockDim.x;
+
+    // ---- stage in: zero everything (guards), then copy coefficients of every level, rhs (and phi) of the first ----
+    {
+        const TailLevel& B = g.lev[g.nl - 1];
+        int total = B.off + tail_level_doubles(B.n, B.guard);
+        for (int t = tid; t < total; t += nth) tail_smem[t] = 0.0;
+    }
+    __syncthreads();
+    for (int l = 0; l < g.nl; ++l) {
+        const TailLevel& L = g.lev[l];
+        TailSmem s(tail_smem, L);
+        for (int t = tid; t < L.n; t += nth) {
+            s.dinv[t] = L.dinv[t]; s.wx[t] = L.wx[t]; s.wy[t] = L.wy[t]; s.wz[t] = L.wz[t];
+            if (l == 0) { s.rhs[t] = L.rhs[t]; if (g.whole) s.phi[t] = L.phi[t]; }
+        }
+    }
+    __syncthreads();
+
+    // ---- down-stroke ----
+    for (int l = 0; l + 1 < g.nl; ++l) {
+        const TailLevel& L = g.lev[l];
+        const TailLevel& C = g.lev[l + 1];
+        TailSmem s(tail_smem, L), c(tail_smem, C);
+        tail_smooth(s, L, g.nu1);
+        for (int t = tid; t < C.n; t += nth) {     // residual + restriction (same order as residual_restrict_kernel)
+            int I = t % C.nx, J = (t / C.nx) % C.ny, K = t / (C.nx * C.ny);
+            double acc = 0.0;
+            for (int r = 0; r < g.sz; ++r)
+                for (int q = 0; q < 2; ++q) {
+                    int cc = (2 * I) + L.nx * (2 * J + q) + L.nx * L.ny * (g.sz * K + r);
+                    acc += tail_residual_at(s, L, cc) + tail_residual_at(s, L, cc + 1);
+                }
+            c.rhs[t] = acc / (4.0 * g.sz);
+            c.phi[t] = 0.0;
+        }
+        __syncthreads();
+    }
+    // ---- bottom: fixed number of sweeps from zero (R11) ----
+    {
+        const TailLevel& B = g.lev[g.nl - 1];
+        TailSmem s(tail_smem, B);
+        if (g.nl == 1 && g.whole) {                 // single-level hierarchy: the bottom solve is the cycle (C4)
+            for (int t = tid; t < B.n; t += nth) s.phi[t] = 0.0;
+            __syncthreads();
+        }
+        tail_smooth(s, B, g.nbottom);
+    }
+    // ---- up-stroke ----
+    for (int l = g.nl - 2; l >= 0; --l) {
+        const TailLevel& L = g.lev[l];
+        const TailLevel& C = g.lev[l + 1];
+        TailSmem s(tail_smem, L), c(tail_smem, C);
+        for (int t = tid; t < L.n; t += nth) {     // prolongation + correction (piecewise constant, R9)
+            int i = t % L.nx, j = (t / L.nx) % L.ny, k = t / L.nxy;
+            s.phi[t] += c.phi[(i >> 1) + C.nx * ((j >> 1) + C.ny * (g.sz == 2 ? (k >> 1) : k))];
+        }
+        __syncthreads();
+        tail_smooth(s, L, g.nu2);
+    }
+    // ---- stage out ----
+    {
+        const TailLevel& L = g.lev[0];
+        TailSmem s(tail_smem, L);
+        double m = 0.0;
+        bool nan = false;
+        for (int t = tid; t < L.n; t += nth) {
+            L.phi[t] = s.phi[t];
+            if (g.whole && g.norm_out) {
+                double x = fabs(tail_residual_at(s, L, t));
+                nan |= (x != x);
+                m = fmax(m, x);
+            }
+        }
+        if (g.whole && g.norm_out) {
+            if (nan) m = __longlong_as_double(0x7ff8000000000000ll);
+            block_max_to_global(m, g.norm_out);
+        }
+    }
+}
+
+}  // namespace vmg

@@ -72,6 +72,13 @@ def test_single_steps_match_oracle(dims):
             cnx, cny, cnz = o.level_dims(lev + 1)
             e = rng.standard_normal((cnz, cny, cnx))
             assert np.array_equal(s.step_prolong_correct(lev, dev(phi), dev(e)).cpu().numpy(), o.prolong_add(phi, e, lev))
+            # whole strokes as vmg_solve runs them (fused blocked passes where the level qualifies)
+            phi_d, rc_d = s.step_down(lev, dev(phi), dev(rhs))
+            phi_sm = o.smooth(phi, rhs, 3, lev)
+            assert rel(phi_d.cpu().numpy(), phi_sm) <= STEP_TOL
+            assert np.abs(rc_d.cpu().numpy() - o.restrict(o.residual(phi_sm, rhs, lev), lev)).max() <= STEP_TOL * np.abs(r_o).max()
+            phi_u = s.step_up(lev, dev(phi), dev(rhs), dev(e))
+            assert rel(phi_u.cpu().numpy(), o.smooth(o.prolong_add(phi, e, lev), rhs, 3, lev)) <= STEP_TOL
     # S1 fold_bc, S6 norm, one whole V-cycle (S7)
     bt_o = o.fold_bc(p.rhs)
     bt_g = s.step_fold_bc(d["rhs"]).cpu().numpy()
@@ -81,6 +88,37 @@ def test_single_steps_match_oracle(dims):
     for graph in (0, 1):
         s.set_option("graph", graph)
         assert rel(s.step_vcycle(dev(phi0), dev(bt_o)).cpu().numpy(), o.vcycle(phi0, bt_o)) <= 1e-12
+    s.destroy()
+
+
+@pytest.mark.parametrize("dims", [(40, 24, 16), (88, 56, 24), (144, 80, 48), (256, 128, 32)])
+def test_blocked_passes_equal_plain_launches_bitwise(dims):
+    """The temporally blocked passes (with fused prolongation / restriction) relax in the same order with the
+    same expression as one launch per colour: bitwise equal on every level with even dimensions, on sizes that
+    span several tiles and z-segments with ragged edges."""
+    b = _binding()
+    p = inputs.random_problem(*dims, seed=11, bc_type=MIXED, sigma=1.0)
+    s, d = b.from_problem(p)
+    s.set_option("block_min_cells", 0)
+    rng = np.random.default_rng(3)
+    for lev in range(s.num_levels - 1):
+        nx, ny, nz = s.level_dims(lev)
+        if nx % 2 or ny % 2 or nz % 2:
+            break
+        cnx, cny, cnz = s.level_dims(lev + 1)
+        phi, rhs = dev(rng.standard_normal((nz, ny, nx))), dev(rng.standard_normal((nz, ny, nx)) * 50.0)
+        e = dev(rng.standard_normal((cnz, cny, cnx)))
+        out = {}
+        for blocked in (1, 0):
+            s.set_option("blocked", blocked)
+            res = [s.step_smooth(lev, phi, rhs, ns) for ns in (1, 2, 3, 4)]
+            for nu in (1, 2, 3):
+                s.set_option("nu1", nu)
+                s.set_option("nu2", nu)
+                res += list(s.step_down(lev, phi, rhs)) + [s.step_up(lev, phi, rhs, e)]
+            out[blocked] = res
+        for x, y in zip(out[1], out[0]):
+            assert torch.equal(x, y), (lev, (x - y).abs().max().item())
     s.destroy()
 
 
@@ -137,10 +175,9 @@ def test_config5_full_size_parity():
 
 
 @pytest.mark.parametrize("opts", [dict(nu1=2, nu2=2), dict(nu1=1, nu2=3, bottom_sweeps=8), dict(graph=0), dict(blocked=0),
-                                  dict(wavefront_min_cells=0, wavefront_planes=2),
-                                  dict(wavefront_min_cells=0, wavefront_planes=4, graph=0),
-                                  dict(wavefront_min_cells=0, wavefront_planes=6, nu1=2, nu2=4),
-                                  dict(wavefront_min_cells=0, wavefront_planes=4, nu1=0, nu2=1)])
+                                  dict(tail=0), dict(blocked=0, tail=0, graph=0), dict(block_min_cells=0),
+                                  dict(block_min_cells=0, graph=0, nu1=2, nu2=4), dict(block_min_cells=0, nu1=1, nu2=2),
+                                  dict(block_min_cells=0, nu1=4, nu2=1, tail=0)])
 def test_options_parity(opts):
     check_parity(inputs.random_problem(48, 24, 48, seed=3, bc_type=[D, D, N, N, N, D]), **opts)
 
