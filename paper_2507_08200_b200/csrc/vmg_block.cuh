@@ -41,7 +41,7 @@ struct BlockArgs {
     long long nxy;
     int colour0;                   // colour of the first half-sweep of this pass (0 = red = (i+j+k) even)
     int ntx, nty;                  // tiles in x and y
-    long long W;                   // ntx * nty * nz plane-tiles, cut into gridDim.x segments
+    int nzseg;                     // z-segments per tile; gridDim.x = ntx * nty * nzseg, tile index fastest
     const double* e;               // PROLONG: coarse correction (cnx x cny x cnz)
     double *crhs, *cphi;           // BT_RESTRICT: coarse right-hand side (written), coarse phi (zeroed)
     int cnx, cny;
@@ -87,17 +87,16 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
     for (int q = t; q < (int)(C::SMEM / sizeof(double)); q += C::NT) blk_smem[q] = 0.0;
     __syncthreads();
 
-    // this CTA's segment of the (tile, z) space; cut at even z so that restriction pairs stay together
-    long long w = (g.W / 2 * blockIdx.x / gridDim.x) * 2, w1 = (g.W / 2 * (blockIdx.x + 1) / gridDim.x) * 2;
-    if (blockIdx.x == gridDim.x - 1) w1 = g.W;
-
+    // CTA -> (tile, z-segment), tile index fastest: the CTAs that run at the same time are x-y neighbours marching
+    // through the same z-range in step, so that the tile halos they share are fetched from HBM once and hit in L2
+    // for the others.  Segments are cut at even z so that restriction pairs stay together.
+    const int ntiles = g.ntx * g.nty;
     double nrm = 0.0;
     bool nrm_nan = false;
-
-    while (w < w1) {
-        const int tile = (int)(w / g.nz), za = (int)(w % g.nz);
-        const int zb = (int)min((long long)g.nz, (long long)za + (w1 - w));
-        w += zb - za;
+    {
+        const int tile = (int)(blockIdx.x % ntiles), seg = (int)(blockIdx.x / ntiles);
+        const int za = (int)((long long)(g.nz / 2) * seg / g.nzseg) * 2;
+        const int zb = seg == g.nzseg - 1 ? g.nz : (int)((long long)(g.nz / 2) * (seg + 1) / g.nzseg) * 2;
         const int tx = tile % g.ntx, ty = tile / g.ntx;
         const int gx = tx * C::TX - C::HX + 2 * m, gy = ty * C::TY - H + j;
         const bool in_xy = live && gx >= 0 && gx < g.nx && gy >= 0 && gy < g.ny;
@@ -237,7 +236,6 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
                 }
             }
         }
-        __syncthreads();   // rings are reused by the next segment
     }
 
     if (TAIL == BT_NORM) {

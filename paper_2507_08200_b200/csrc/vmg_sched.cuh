@@ -213,8 +213,17 @@ struct BlkKernel {
     static void launch(vmg_s* h, BlockArgs g)
     {
         g.ntx = (int)cdiv(g.nx, C::TX); g.nty = (int)cdiv(g.ny, C::TY);
-        g.W = (long long)g.ntx * g.nty * g.nz;
-        unsigned grid = (unsigned)std::max<long long>(1, std::min<long long>(h->num_sms, g.W / 2));
+        // z-segments per tile: minimise waves x (planes per CTA incl. the 2H halo planes each segment pays)
+        const long long ntiles = (long long)g.ntx * g.nty;
+        int best = 1;
+        double best_cost = 1e300;
+        for (int ns = 1; ns <= std::max(1, g.nz / 4); ++ns) {
+            double waves = (double)cdiv(ntiles * ns, h->num_sms);
+            double cost = waves * ((double)cdiv(g.nz / 2, ns) * 2 + 2 * C::H + 2);
+            if (cost < best_cost) { best_cost = cost; best = ns; }
+        }
+        g.nzseg = best;
+        unsigned grid = (unsigned)(ntiles * g.nzseg);
         smooth_block_kernel<S, TAIL, PROLONG, kBlkNXT, NYT><<<grid, C::NT, C::SMEM, h->stream>>>(g);
     }
 };
