@@ -6,7 +6,7 @@
 #include "vmg_internal.h"
 #include "vmg_kernels.cuh"
 #include "vmg_tail.cuh"
-#include "vmg_block.cuh"
+#include "vmg_block2.cuh"
 #include "../../include/vmg.h"
 #include <algorithm>
 
@@ -182,21 +182,21 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
 }
 
 // ------------------------------------------------------------------------------------------------
-// S2-S4, S6: blocked passes.  Tile width 40 (32 interior + 2 x 4 halo); the tile height is the largest even number
-// of rows whose rings fit 227 KB of shared memory with at most 768 threads (one thread per x-pair).
+// S2-S4, S6: blocked passes.  Tile width 40 (32 interior + 2 x 4 halo); one thread per x-pair, at most 640 threads
+// (102 registers each), the tile height is the largest even number of rows that fits threads and shared memory.
 // ------------------------------------------------------------------------------------------------
 constexpr int kBlkNXT = 40;
-constexpr int kBlkMaxSmem = 232448;
-constexpr int kBlkMaxPairs = 768;
+constexpr int kBlkMaxSmem = 232448 - 1024;
+constexpr int blk_max_pairs(int TAIL) { return TAIL ? 560 : 640; }   // residual stage needs ~112 registers
 
 constexpr int blk_pick_nyt(int S, int TAIL)
 {
     int best = 0;
     for (int nyt = 2 * (S + (TAIL ? 1 : 0)) + 2; nyt <= 64; nyt += 2) {
         long long np = (long long)(kBlkNXT / 2) * nyt;
-        int rp = S + 2 + (TAIL ? 1 : 0), rc = S + (TAIL ? 1 : 0), rz = rc + 1;
-        long long smem = ((long long)(rp + 4 * rc + rz) * 2 * np + (TAIL == BT_RESTRICT ? np : 0)) * 8;
-        if (np <= kBlkMaxPairs && smem <= kBlkMaxSmem) best = nyt;
+        int rs = S + (TAIL ? 1 : 0);
+        long long smem = ((long long)rs * 10 * np + (TAIL == BT_RESTRICT ? np : 0)) * 8;
+        if (np <= blk_max_pairs(TAIL) && smem <= kBlkMaxSmem) best = nyt;
     }
     return best;
 }
