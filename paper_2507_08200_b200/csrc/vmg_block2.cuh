@@ -18,18 +18,21 @@
 //
 // Where the data lives (what the first design got wrong: every operand of every relaxation came from shared
 // memory, 15 LDS.64 + 1 STS.64 = 32 shared-memory wavefronts per warp-update, more than the 128 B/clk port can
-// feed at the HBM rate).  Thread t owns the x-pair (2m, 2m+1) of row j, t = j*NXP + m, in every plane, and keeps
-// in REGISTERS what only it ever reads: its own phi column (planes zl .. zl-S-1: the z-neighbours and the
-// pair-mate of the cell it relaxes) and its own wz column.  Shared memory holds, for the S planes in flight, what
-// OTHER threads read: phi (x-neighbour outside the pair, y-neighbours) and rhs, 1/D, wx, wy, split by x-parity so
-// that a half-sweep (which touches one parity per row) reads and writes unit-stride fp64 vectors without bank
-// conflicts.  One relaxation = 9 LDS.64 + 1 STS.64.  Global loads are register-staged one plane ahead
-// (6 x 16-byte loads per thread per plane), so data in flight costs no shared memory.
+// feed at the HBM rate).  Thread t owns a 2 x 2 patch: the x-pair (2m, 2m+1) of rows 2jj and 2jj+1, t = jj*NXP + m,
+// in every plane, and keeps in REGISTERS what only it ever reads: its own phi columns (planes zl .. zl-S-1: the
+// z-neighbours, the pair-mate and the y-neighbour inside the patch of the cells it relaxes) and its own wz columns.
+// Shared memory holds, for the S planes in flight, what OTHER threads read: phi (x- and y-neighbour outside the
+// patch) and rhs, 1/D, wx, wy, split by x-parity and by row parity so that a half-sweep (which touches one
+// x-parity per row) reads and writes unit-stride fp64 vectors without bank conflicts.  One relaxation = 8 LDS.64 +
+// 1 STS.64.  Global loads are register-staged one plane ahead (12 x 16-byte loads per thread per plane), so data
+// in flight costs no shared memory; a 2 x 2 patch per thread halves the thread count, which leaves each thread the
+// ~170 registers that the rings, the staged loads and the residual stage need without spilling.
 //
-// Register rings are indexed by ROLE, not by x-parity: in plane q the cell relaxed at odd stages has x-parity
-// (colour0 + gy + q) & 1 ("role A"), the other is "role B".  Roles swap parity from plane to plane, so the
-// z-neighbours and the pair-mate of a role-A cell are role-B cells: every register index is a compile-time
-// constant.  In one iteration the active cell has the same x-parity sigma in all stages, sigma flips per iteration.
+// No index arithmetic at run time.  Tiles start at even x, y, z offsets plus the halo, so the x-parity of the cell
+// a thread relaxes in row r of iteration n is (colour0 + r + n + 1) & 1 for every thread of the grid: colour0 is a
+// template parameter and the z-loop is unrolled by the period R of the register rings (even), which makes every
+// register index, every parity and every shared-memory offset (relative to one base per stage) a compile-time
+// constant: no selects, no ring rotation moves.
 //
 // The arithmetic of one relaxation / residual is the same expression, in the same order, as smooth_colour_kernel /
 // residual_at: results are bitwise identical to the one-launch-per-step path.
@@ -55,40 +58,44 @@ struct BlockArgs {
     unsigned long long* norm_out;  // BT_NORM
 };
 
+
 template <int S, int TAIL, int NXT, int NYT>
 struct BlockCfg {
-    static constexpr int H = S + (TAIL ? 1 : 0);          // halo in y and z
+    // halo in y and z; with a residual stage S+1, rounded up to even so that a thread's two rows are the two
+    // y-children of one coarse cell
+    static constexpr int H = TAIL ? (S + 2) / 2 * 2 : S;
     static constexpr int HX = 4;                          // halo in x (kept 32-byte aligned)
     static constexpr int TX = NXT - 2 * HX, TY = NYT - 2 * H;
-    static constexpr int NXP = NXT / 2, NP = NXP * NYT;   // pairs per row, pairs per plane
-    static constexpr int NT = (NP + 31) / 32 * 32;        // threads
+    static constexpr int NXP = NXT / 2, NPH = NXP * (NYT / 2);   // x-pairs per row, 2x2 patches per plane (= threads)
+    static constexpr int NT = (NPH + 31) / 32 * 32;
     static constexpr int RS = S + (TAIL ? 1 : 0);         // shared-memory ring: planes zl-1 .. zl-RS
-    static constexpr int RPSI = S + 2 + (TAIL ? 1 : 0);   // register ring of phi: planes zl .. zl-RPSI+1
-    static constexpr int RWZ = S + 1 + (TAIL ? 1 : 0);    // register ring of wz:  planes zl .. zl-RWZ+1
-    static constexpr int SLOT = 10 * NP;                  // doubles per slot: phi, rhs, dinv, wx, wy, each [2][NP]
-    static constexpr size_t SMEM = (size_t)(RS * SLOT + (TAIL == BT_RESTRICT ? NP : 0)) * sizeof(double);
-    static_assert(H >= S && HX >= H && TX > 0 && TY > 0 && TX % 2 == 0 && TY % 2 == 0, "tile");
+    static constexpr int R = (S + 4) / 2 * 2;             // register rings: planes zl .. zl-S-2 (S+3 planes), period even
+    static constexpr int ARR = 4 * NPH;                   // one array of one plane: [x-parity][row parity][NPH]
+    static constexpr int SLOT = 5 * ARR;                  // phi, rhs, dinv, wx, wy
+    static constexpr size_t SMEM = (size_t)(RS * SLOT) * sizeof(double);
+    static_assert(H >= S + (TAIL ? 1 : 0) && HX >= H && TX > 0 && TY > 0 &&
+                      TX % 2 == 0 && TY % 2 == 0 && NYT % 2 == 0 && R >= S + 3 && R % 2 == 0, "tile");
 };
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
 __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 constexpr int kBlkPrefetch = 2;   // planes ahead of the register-staged loads
 
-template <int S, int TAIL, bool PROLONG, int NXT, int NYT>
+template <int S, int TAIL, bool PROLONG, int C0, int NXT, int NYT>
 __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_block_kernel(BlockArgs g)
 {
     using C = BlockCfg<S, TAIL, NXT, NYT>;
-    constexpr int H = C::H, NXP = C::NXP, NP = C::NP, RS = C::RS, RPSI = C::RPSI, RWZ = C::RWZ, SLOT = C::SLOT;
-    constexpr int A_PHI = 0, A_RHS = 2 * NP, A_DINV = 4 * NP, A_WX = 6 * NP, A_WY = 8 * NP;   // arrays inside a slot
+    constexpr int H = C::H, NXP = C::NXP, NPH = C::NPH, RS = C::RS, R = C::R, SLOT = C::SLOT;
+    constexpr int A_PHI = 0, A_RHS = C::ARR, A_DINV = 2 * C::ARR, A_WX = 3 * C::ARR, A_WY = 4 * C::ARR;
+    constexpr int XB = 2 * NPH;                     // offset of the odd-x block inside an array
     extern __shared__ __align__(16) double blk_smem[];
-    double* const s_scr = blk_smem + RS * SLOT;   // BT_RESTRICT only
 
-    const int t = threadIdx.x;
-    const bool live = t < NP;
-    const int m = t % NXP, j = t / NXP;
+    const bool live = threadIdx.x < NPH;
+    const int t = live ? threadIdx.x : 0;          // idle lanes of the last warp shadow thread 0 (and commit nothing)
+    const int m = t % NXP, jj = t / NXP;
 
     // planes before the first loaded one: zero weights and zero 1/D keep them at zero (finite)
-    for (int q = t; q < (int)(C::SMEM / sizeof(double)); q += C::NT) blk_smem[q] = 0.0;
+    for (int q = threadIdx.x; q < RS * SLOT; q += C::NT) blk_smem[q] = 0.0;
 
     // CTA -> (tile, z-segment), tile index fastest; segments are cut at even z (restriction pairs stay together)
     const int ntiles = g.ntx * g.nty;
@@ -96,188 +103,229 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
     const int za = (int)((long long)(g.nz / 2) * seg / g.nzseg) * 2;
     const int zb = seg == g.nzseg - 1 ? g.nz : (int)((long long)(g.nz / 2) * (seg + 1) / g.nzseg) * 2;
     const int tx = tile % g.ntx, ty = tile / g.ntx;
-    const int gx = tx * C::TX - C::HX + 2 * m, gy = ty * C::TY - H + j;
-    const bool in_xy = live && gx >= 0 && gx < g.nx && gy >= 0 && gy < g.ny;
-    const bool interior = in_xy && m >= C::HX / 2 && m < C::HX / 2 + C::TX / 2 && j >= H && j < H + C::TY;
-    const bool row_ok = live && j >= 1 && j <= NYT - 2;
-    const long long cbase = gx + (long long)g.nx * gy;
-    const long long ebase = PROLONG ? (gx >> 1) + (long long)g.cnx * (gy >> 1) : 0;
-    const int par0 = g.colour0 + gy;   // + plane index: x-parity of the role-A cell of that plane
+    const int gx = tx * C::TX - C::HX + 2 * m, gy0 = ty * C::TY - H + 2 * jj;      // rows gy0 and gy0 + 1
+    const bool in_x = live && gx >= 0 && gx < g.nx;
+    const bool in_r[2] = {in_x && gy0 >= 0 && gy0 < g.ny, in_x && gy0 + 1 >= 0 && gy0 + 1 < g.ny};
+    const bool int_x = m >= C::HX / 2 && m < C::HX / 2 + C::TX / 2;
+    const bool interior[2] = {in_r[0] && int_x && 2 * jj >= H && 2 * jj < H + C::TY,
+                              in_r[1] && int_x && 2 * jj + 1 >= H && 2 * jj + 1 < H + C::TY};
+    // rows 0 and NYT-1 and the first / last column of the tile are rim: never relaxed.  ok[r][sg]: row r, x-parity sg
+    const bool ok[2][2] = {{live && jj >= 1 && m > 0, live && jj >= 1 && m < NXP - 1},
+                           {live && jj <= NYT / 2 - 2 && m > 0, live && jj <= NYT / 2 - 2 && m < NXP - 1}};
+    const long long cbase = gx + (long long)g.nx * gy0;
 
-    // register rings, index k <-> plane zl - k (role A / role B values of this thread's pair)
-    double pa[RPSI], pb[RPSI], wa[RWZ], wb[RWZ];
+    // register rings [row][slot]: even-x / odd-x phi and wz of this thread's pair; plane z0 + n lives in slot n % R
+    double pe[2][R], po[2][R], we[2][R], wo[2][R];
 #pragma unroll
-    for (int k = 0; k < RPSI; ++k) pa[k] = pb[k] = 0.0;
+    for (int r = 0; r < 2; ++r)
 #pragma unroll
-    for (int k = 0; k < RWZ; ++k) wa[k] = wb[k] = 0.0;
-    int sl[RS];                                    // sl[k]: offset of the slot holding plane zl - 1 - k
+        for (int k = 0; k < R; ++k) pe[r][k] = po[r][k] = we[r][k] = wo[r][k] = 0.0;
+    int sl[RS];                                    // sl[k]: offset of the slot holding plane zl - 1 - k, + t
 #pragma unroll
-    for (int k = 0; k < RS; ++k) sl[k] = k * SLOT;
+    for (int k = 0; k < RS; ++k) sl[k] = k * SLOT + t;
 
     // loads in flight: phi, wz (and the coarse correction) of plane zq; rhs, 1/D, wx, wy of plane zq - 1
-    double2 r_phi, r_wz, r_rhs, r_dinv, r_wx, r_wy;
-    double r_e = 0.0;
+    double2 r_phi[2], r_wz[2], r_rhs[2], r_dinv[2], r_wx[2], r_wy[2];
+    double r_e[2] = {0.0, 0.0};
     auto issue = [&](int zq) {
-        // pull the planes kBlkPrefetch further on from HBM into L2 now: all CTAs march in step, so their loads come
-        // in bursts; with the DRAM latency taken early the register-staged loads below are L2 hits
-        if (in_xy && zq + kBlkPrefetch < g.nz && zq + kBlkPrefetch > 0) {
-            const long long c = cbase + g.nxy * (zq + kBlkPrefetch);
-            prefetch_l2(g.phi_in + c); prefetch_l2(g.wz + c);
-            prefetch_l2(g.rhs + c - g.nxy); prefetch_l2(g.dinv + c - g.nxy);
-            prefetch_l2(g.wx + c - g.nxy); prefetch_l2(g.wy + c - g.nxy);
+        // pull the planes kBlkPrefetch further on from HBM into L2 now (one request per 32-byte sector): all CTAs march
+        // in step, so their loads come in bursts; with the DRAM latency taken early the staged loads below hit L2
+        if (!(m & 1) && zq + kBlkPrefetch < g.nz && zq + kBlkPrefetch > 0) {
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+                if (in_r[r]) {
+                    const long long c = cbase + r * g.nx + g.nxy * (zq + kBlkPrefetch);
+                    prefetch_l2(g.phi_in + c); prefetch_l2(g.wz + c);
+                    prefetch_l2(g.rhs + c - g.nxy); prefetch_l2(g.dinv + c - g.nxy);
+                    prefetch_l2(g.wx + c - g.nxy); prefetch_l2(g.wy + c - g.nxy);
+                }
         }
         const double2 zero = make_double2(0.0, 0.0);
-        r_phi = r_wz = r_rhs = r_dinv = r_wx = r_wy = zero;
-        r_e = 0.0;
-        if (in_xy && zq >= 0 && zq < g.nz) {
-            const long long c = cbase + g.nxy * zq;
-            r_phi = ldg2(g.phi_in + c);
-            r_wz = ldg2(g.wz + c);
-            if (PROLONG) r_e = __ldg(g.e + ebase + (long long)g.cnx * g.cny * (zq >> 1));
-        }
-        if (in_xy && zq - 1 >= 0 && zq - 1 < g.nz) {
-            const long long c = cbase + g.nxy * (zq - 1);
-            r_rhs = ldg2(g.rhs + c);
-            r_dinv = ldg2(g.dinv + c);
-            r_wx = ldg2(g.wx + c);
-            r_wy = ldg2(g.wy + c);
-        }
-    };
-    // rings move one plane on; the loaded phi, wz of plane zq become index 0 (pA = x-parity of its role-A cell)
-    auto insert = [&](int pA) {
 #pragma unroll
-        for (int k = RPSI - 1; k > 0; --k) { pa[k] = pa[k - 1]; pb[k] = pb[k - 1]; }
-#pragma unroll
-        for (int k = RWZ - 1; k > 0; --k) { wa[k] = wa[k - 1]; wb[k] = wb[k - 1]; }
-        if (PROLONG) { r_phi.x += r_e; r_phi.y += r_e; }   // S4: phi += P e (piecewise constant); r_e = 0 off-domain
-        pa[0] = pA ? r_phi.y : r_phi.x; pb[0] = pA ? r_phi.x : r_phi.y;
-        wa[0] = pA ? r_wz.y : r_wz.x;   wb[0] = pA ? r_wz.x : r_wz.y;
+        for (int r = 0; r < 2; ++r) {
+            r_phi[r] = r_wz[r] = r_rhs[r] = r_dinv[r] = r_wx[r] = r_wy[r] = zero;
+            r_e[r] = 0.0;
+#ifdef VMG_ABL_NOLOAD
+            if (in_r[r] && zq == -12345) {
+#else
+            if (in_r[r] && zq >= 0 && zq < g.nz) {
+#endif
+                const long long c = cbase + r * g.nx + g.nxy * zq;
+                r_phi[r] = ldg2(g.phi_in + c);
+                r_wz[r] = ldg2(g.wz + c);
+                if (PROLONG)
+                    r_e[r] = __ldg(g.e + (gx >> 1) + (long long)g.cnx * (((gy0 + r) >> 1) + (long long)g.cny * (zq >> 1)));
+            }
+#ifdef VMG_ABL_NOLOAD
+            if (in_r[r] && zq == -12345) {
+#else
+            if (in_r[r] && zq - 1 >= 0 && zq - 1 < g.nz) {
+#endif
+                const long long c = cbase + r * g.nx + g.nxy * (zq - 1);
+                r_rhs[r] = ldg2(g.rhs + c);
+                r_dinv[r] = ldg2(g.dinv + c);
+                r_wx[r] = ldg2(g.wx + c);
+                r_wy[r] = ldg2(g.wy + c);
+            }
+        }
     };
 
     const int z0 = za - H, z1 = zb + H - 1;
     issue(z0);
-    insert((par0 + z0) & 1);
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {                  // plane z0 -> slot 0
+        if (PROLONG) { r_phi[r].x += r_e[r]; r_phi[r].y += r_e[r]; }
+        pe[r][0] = r_phi[r].x; po[r][0] = r_phi[r].y; we[r][0] = r_wz[r].x; wo[r][0] = r_wz[r].y;
+    }
     issue(z0 + 1);
     __syncthreads();
 
     double nrm = 0.0;
     bool nrm_nan = false;
-    double acc = 0.0;    // BT_RESTRICT: running sum over the children of one coarse cell (even rows, even..odd plane)
-    double pair = 0.0;
+    double acc = 0.0;    // BT_RESTRICT: running sum over the children of one coarse cell (even plane, then odd plane)
 
-    for (int zl = z0; zl <= z1; ++zl) {
-        const int sigma = (par0 + zl - 1) & 1;             // x-parity of the cells relaxed in this iteration
-        const int offA = sigma * NP + t;                   // active cell (also: its wx_lo, wy_lo, rhs, 1/D)
-        const int offX = sigma ? t + 1 : NP + t - 1;       // its x-neighbour outside the pair
-        const int offW = sigma ? t + 1 : NP + t;           // wx of its high-x face
-        const bool ok = row_ok && (sigma ? m < NXP - 1 : m > 0);
-
-        // ---- stages: half-sweep s on plane zl - s (ring index s, slot sl[s-1]) ----
+    for (int zbase = z0; zbase <= z1; zbase += R) {
 #pragma unroll
-        for (int s = 1; s <= S; ++s) {
-            if (ok) {
+        for (int u = 0; u < R; ++u) {
+            const int zl = zbase + u;              // iteration n = zl - z0, n % R == u
+            if (zl > z1) break;                    // uniform
+
+            // ---- stages: half-sweep s on plane zl - s (ring slot (u-s) % R, shared slot sl[s-1]); rim threads compute
+            // and discard.  Row r relaxes its cell of x-parity sg = (C0 + r + u + 1) & 1. ----
+#ifdef VMG_ABL_NOSTAGE
+            for (int s = 1; s <= 0; ++s) {
+#else
+#pragma unroll
+            for (int s = 1; s <= S; ++s) {
+#endif
+                const int c = ((u - s) % R + R) % R, cu = ((u - s + 1) % R + R) % R, cd = ((u - s - 1) % R + R) % R;
                 double* P = blk_smem + sl[s - 1];
-                double mate, zup, zdn, wzl, wzh;
-                if (s & 1) { mate = pb[s]; zup = pb[s - 1]; zdn = pb[s + 1]; wzl = wa[s]; wzh = wb[s - 1]; }
-                else       { mate = pa[s]; zup = pa[s - 1]; zdn = pa[s + 1]; wzl = wb[s]; wzh = wa[s - 1]; }
-                const double xo = P[A_PHI + offX];
-                const double xm = sigma ? mate : xo, xp = sigma ? xo : mate;
-                double v = P[A_WX + offA] * xm;
-                v = fma(P[A_WX + offW], xp, v);
-                v = fma(P[A_WY + offA], P[A_PHI + offA - NXP], v);
-                v = fma(P[A_WY + offA + NXP], P[A_PHI + offA + NXP], v);
-                v = fma(wzl, zdn, v);
-                v = fma(wzh, zup, v);
-                const double nv = P[A_DINV + offA] * (P[A_RHS + offA] + v);
-                if (s & 1) pa[s] = nv; else pb[s] = nv;
-                P[A_PHI + offA] = nv;
+                double nv[2];
+#pragma unroll
+                for (int r = 0; r < 2; ++r) {
+                    const int sg = (C0 + r + u + 1) & 1;
+                    const int oA = sg * XB + r * NPH;                                   // active cell
+                    const double mate = sg ? pe[r][c] : po[r][c];
+                    const double zup = sg ? po[r][cu] : pe[r][cu], zdn = sg ? po[r][cd] : pe[r][cd];
+                    const double wzl = sg ? wo[r][c] : we[r][c], wzh = sg ? wo[r][cu] : we[r][cu];
+                    const double yin = sg ? po[1 - r][c] : pe[1 - r][c];
+                    const double xo = P[A_PHI + (sg ? r * NPH + 1 : XB + r * NPH - 1)];   // x-neighbour outside the pair
+                    const double yo = P[A_PHI + sg * XB + (r ? NXP : NPH - NXP)];        // y-neighbour outside the patch
+                    const double xm = sg ? mate : xo, xp = sg ? xo : mate;
+                    const double ym = r ? yin : yo, yp = r ? yo : yin;
+                    double v = P[A_WX + oA] * xm;
+                    v = fma(P[A_WX + (sg ? r * NPH + 1 : XB + r * NPH)], xp, v);
+                    v = fma(P[A_WY + oA], ym, v);
+                    v = fma(P[A_WY + sg * XB + (r ? NXP : NPH)], yp, v);
+                    v = fma(wzl, zdn, v);
+                    v = fma(wzh, zup, v);
+                    nv[r] = P[A_DINV + oA] * (P[A_RHS + oA] + v);
+                }
+#pragma unroll
+                for (int r = 0; r < 2; ++r) {
+                    const int sg = (C0 + r + u + 1) & 1;
+                    if (ok[r][sg]) {
+                        if (sg) po[r][c] = nv[r]; else pe[r][c] = nv[r];
+                        P[A_PHI + sg * XB + r * NPH] = nv[r];
+                    }
+                }
+
+                // ---- residual stage on plane zl - S - 1 (shared slot sl[S]); all its neighbours are final: plane
+                // zl - S in this thread's registers (just relaxed), the others since the previous iteration ----
+                if (TAIL != BT_NONE && s == S) {
+                    const int pr = zl - S - 1;
+                    if (pr >= za && pr < zb && interior[0]) {     // interior rows come in pairs (H, TY, ny are even)
+                        const int k = ((u - S - 1) % R + R) % R, ku = ((u - S) % R + R) % R, kd = ((u - S - 2) % R + R) % R;
+                        const double* Q = blk_smem + sl[RS - 1];
+                        double res[2][2];                    // [row][x-parity]
+#pragma unroll
+                        for (int r = 0; r < 2; ++r)
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const int o = e * XB + r * NPH;
+                                const double ce = e ? po[r][k] : pe[r][k], mate = e ? pe[r][k] : po[r][k];
+                                const double xo = Q[A_PHI + (e ? r * NPH + 1 : XB + r * NPH - 1)];
+                                const double yo = Q[A_PHI + e * XB + (r ? NXP : NPH - NXP)];
+                                const double yin = e ? po[1 - r][k] : pe[1 - r][k];
+                                const double xm = e ? mate : xo, xp = e ? xo : mate;
+                                const double ym = r ? yin : yo, yp = r ? yo : yin;
+                                double v = Q[A_WX + o] * xm;
+                                v = fma(Q[A_WX + (e ? r * NPH + 1 : XB + r * NPH)], xp, v);
+                                v = fma(Q[A_WY + o], ym, v);
+                                v = fma(Q[A_WY + e * XB + (r ? NXP : NPH)], yp, v);
+                                v = fma(e ? wo[r][k] : we[r][k], e ? po[r][kd] : pe[r][kd], v);
+                                v = fma(e ? wo[r][ku] : we[r][ku], e ? po[r][ku] : pe[r][ku], v);
+                                res[r][e] = Q[A_RHS + o] + v - ce / Q[A_DINV + o];
+                            }
+                        if (TAIL == BT_NORM) {
+#pragma unroll
+                            for (int r = 0; r < 2; ++r)
+#pragma unroll
+                                for (int e = 0; e < 2; ++e) {
+                                    const double a = fabs(res[r][e]);
+                                    nrm_nan |= (a != a);
+                                    nrm = fmax(nrm, a);
+                                }
+                        }
+                        if (TAIL == BT_RESTRICT) {
+                            // S3: children summed as in residual_restrict_kernel: per (z, y) the x-pair first, then accumulated
+                            acc += res[0][0] + res[0][1];
+                            acc += res[1][0] + res[1][1];
+                            if (pr & 1) {
+                                const long long cc = (gx >> 1) + (long long)g.cnx * ((gy0 >> 1) + (long long)g.cny * (pr >> 1));
+                                g.crhs[cc] = acc / 8.0;
+                                g.cphi[cc] = 0.0;
+                                acc = 0.0;
+                            }
+                        }
+                    }
+                }
+#ifndef VMG_ABL_NOBAR
+                __syncthreads();
+#endif
             }
 
-            // ---- residual stage on plane zl - S - 1 (ring index S+1, slot sl[S]); all its neighbours are final:
-            // plane zl - S in this thread's registers (just relaxed), the others since the previous iteration ----
-            if (TAIL != BT_NONE && s == S) {
-                const int pr = zl - S - 1;
-                const bool on = pr >= za && pr < zb;     // uniform over the CTA
-                double res[2] = {0.0, 0.0};              // even-x cell, odd-x cell
-                if (on && interior) {
-                    constexpr int K = S + 1;             // ring index of plane pr
-                    const double* P = blk_smem + sl[RS - 1];
-                    // x-parity of the role-A cell of ring index k is sigma ^ ((k-1)&1)
-                    const int pK = sigma ^ ((K - 1) & 1);
-                    const double ce[2] = {pK ? pb[K] : pa[K], pK ? pa[K] : pb[K]};                           // plane pr
-                    const double cu[2] = {pK ? pa[K - 1] : pb[K - 1], pK ? pb[K - 1] : pa[K - 1]};           // plane pr+1
-                    const double cd[2] = {pK ? pa[K + 1] : pb[K + 1], pK ? pb[K + 1] : pa[K + 1]};           // plane pr-1
-                    const double wl[2] = {pK ? wb[K] : wa[K], pK ? wa[K] : wb[K]};                           // wz of plane pr
-                    const double wh[2] = {pK ? wa[K - 1] : wb[K - 1], pK ? wb[K - 1] : wa[K - 1]};           // wz of plane pr+1
+            // ---- plane zl - S is final: write it back from registers ----
+            {
+                const int p = zl - S, c = ((u - S) % R + R) % R;
+                if (p >= za && p < zb) {
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int oA = e * NP + t;
-                        const double xo = P[A_PHI + (e ? t + 1 : NP + t - 1)];
-                        const double xm = e ? ce[0] : xo, xp = e ? xo : ce[1];
-                        double v = P[A_WX + oA] * xm;
-                        v = fma(P[A_WX + (e ? t + 1 : NP + t)], xp, v);
-                        v = fma(P[A_WY + oA], P[A_PHI + oA - NXP], v);
-                        v = fma(P[A_WY + oA + NXP], P[A_PHI + oA + NXP], v);
-                        v = fma(wl[e], cd[e], v);
-                        v = fma(wh[e], cu[e], v);
-                        res[e] = P[A_RHS + oA] + v - ce[e] / P[A_DINV + oA];
-                    }
-                    if (TAIL == BT_NORM) {
-                        const double a = fabs(res[0]), b = fabs(res[1]);
-                        nrm_nan |= (a != a) | (b != b);
-                        nrm = fmax(nrm, fmax(a, b));
-                    }
-                }
-                if (TAIL == BT_RESTRICT) {
-                    pair = res[0] + res[1];
-                    if (on && live && (gy & 1)) s_scr[t] = pair;   // odd rows hand their x-pair sum to the row below
+                    for (int r = 0; r < 2; ++r)
+                        if (interior[r])
+                            *reinterpret_cast<double2*>(g.phi_out + cbase + r * g.nx + g.nxy * p) = make_double2(pe[r][c], po[r][c]);
                 }
             }
+            // ---- plane zl (still untouched, ring slot u) and its coefficients replace plane zl - RS in shared memory ----
+            if (live) {
+                double* F = blk_smem + sl[RS - 1];
+#pragma unroll
+                for (int r = 0; r < 2; ++r) {
+                    const int o0 = r * NPH, o1 = XB + r * NPH;
+                    F[A_PHI + o0] = pe[r][u];     F[A_PHI + o1] = po[r][u];
+#ifndef VMG_ABL_NOFILL
+                    F[A_RHS + o0] = r_rhs[r].x;   F[A_RHS + o1] = r_rhs[r].y;
+                    F[A_DINV + o0] = r_dinv[r].x; F[A_DINV + o1] = r_dinv[r].y;
+                    F[A_WX + o0] = r_wx[r].x;     F[A_WX + o1] = r_wx[r].y;
+                    F[A_WY + o0] = r_wy[r].x;     F[A_WY + o1] = r_wy[r].y;
+#endif
+                }
+            }
+            {
+                const int freed = sl[RS - 1];
+#pragma unroll
+                for (int k = RS - 1; k > 0; --k) sl[k] = sl[k - 1];
+                sl[0] = freed;
+            }
+            // ---- plane zl + 1 enters the register rings (slot (u+1) % R held plane zl + 1 - R, no longer needed) ----
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                const int n1 = (u + 1) % R;
+                if (PROLONG) { r_phi[r].x += r_e[r]; r_phi[r].y += r_e[r]; }   // S4: phi += P e; r_e = 0 off-domain
+                pe[r][n1] = r_phi[r].x; po[r][n1] = r_phi[r].y; we[r][n1] = r_wz[r].x; wo[r][n1] = r_wz[r].y;
+            }
+            if (zl < z1) issue(zl + 2);
             __syncthreads();
         }
-
-        // ---- plane zl - S is final: write it back from registers ----
-        {
-            const int p = zl - S;
-            if (interior && p >= za && p < zb) {
-                const int pS = sigma ^ ((S - 1) & 1);
-                const double2 o = make_double2(pS ? pb[S] : pa[S], pS ? pa[S] : pb[S]);
-                *reinterpret_cast<double2*>(g.phi_out + cbase + g.nxy * p) = o;
-            }
-        }
-        // ---- S3: children are summed as in residual_restrict_kernel: per (z, y) the x-pair first, then accumulated ----
-        if (TAIL == BT_RESTRICT) {
-            const int pr = zl - S - 1;
-            if (pr >= za && pr < zb && interior && !(gy & 1)) {
-                acc += pair;
-                acc += s_scr[t + NXP];
-                if (pr & 1) {
-                    const long long cc = (gx >> 1) + (long long)g.cnx * ((gy >> 1) + (long long)g.cny * (pr >> 1));
-                    g.crhs[cc] = acc / 8.0;
-                    g.cphi[cc] = 0.0;
-                    acc = 0.0;
-                }
-            }
-        }
-        // ---- plane zl (still untouched, ring index 0) and its coefficients replace plane zl - RS in shared memory ----
-        if (live) {
-            double* F = blk_smem + sl[RS - 1];
-            const int p0 = sigma ^ 1;                     // x-parity of the role-A cell of plane zl
-            F[A_PHI + t] = p0 ? pb[0] : pa[0];   F[A_PHI + NP + t] = p0 ? pa[0] : pb[0];
-            F[A_RHS + t] = r_rhs.x;              F[A_RHS + NP + t] = r_rhs.y;
-            F[A_DINV + t] = r_dinv.x;            F[A_DINV + NP + t] = r_dinv.y;
-            F[A_WX + t] = r_wx.x;                F[A_WX + NP + t] = r_wx.y;
-            F[A_WY + t] = r_wy.x;                F[A_WY + NP + t] = r_wy.y;
-        }
-        {
-            const int freed = sl[RS - 1];
-#pragma unroll
-            for (int k = RS - 1; k > 0; --k) sl[k] = sl[k - 1];
-            sl[0] = freed;
-        }
-        insert(sigma);                                    // plane zl + 1: its role-A parity is (par0 + zl + 1) & 1 = sigma
-        if (zl < z1) issue(zl + 2);
-        __syncthreads();
     }
 
     if (TAIL == BT_NORM) {

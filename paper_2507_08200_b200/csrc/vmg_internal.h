@@ -51,7 +51,7 @@ struct vmg_s {
     bool bc_has_value[6] = {false, false, false, false, false, false};
     bool have_coeffs = false, have_bc = false, dinv_dirty = true;
     int nu1 = 3, nu2 = 3, nbottom = 32;
-    int use_graph = 1, use_blocked = 1;
+    int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200
     int use_tail = 1;             // run the coarsest levels in one CTA (vmg_tail.cuh)
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
     size_t tail_smem = 0;         // dynamic shared memory of the tail kernel

@@ -194,6 +194,45 @@ __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, cons
     phi[c] = L.dinv[c] * (rhs[c] + nb_sum(L, phi, c));
 }
 
+// S4 + S2 fused (plain path).  The first colour half-sweep after a coarse-grid correction: a relaxation never reads
+// the old value of the cell it overwrites, and all six neighbours of a cell of one colour have the other colour, so
+// the correction phi += P e (piecewise constant, R9) is applied to the NEIGHBOURS on the fly and never stored: the
+// cells of the other colour keep their uncorrected values in memory until the next half-sweep overwrites them.
+// Valid when at least one full sweep follows (nu2 >= 1).  phi_nb + e is the very addition prolong_correct_kernel
+// performs, so results are bitwise those of the two separate kernels.
+__global__ void smooth_colour_prolong_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs,
+                                             const double* __restrict__ e, int colour, int sz)
+{
+    int hx = (L.nx + 1) >> 1;
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long nt = (long long)hx * L.ny * L.nz;
+    if (t >= nt) return;
+    int m = (int)(t % hx), j = (int)((t / hx) % L.ny), k = (int)(t / ((long long)hx * L.ny));
+    int i = 2 * m + ((colour + j + k) & 1);
+    if (i >= L.nx) return;
+    long long c = i + (long long)L.nx * j + L.nxy * k;
+    const int cnx = L.nx >> 1, cny = L.ny >> 1;
+    const int K = sz == 2 ? (k >> 1) : k;
+    auto ec = [&](int ii, int jj, int kk) { return e[(ii >> 1) + (long long)cnx * ((jj >> 1) + (long long)cny * kk)]; };
+    // out-of-domain neighbours carry a zero weight; their (zero-pad) value is used uncorrected
+    double xm = phi[c - 1], xp = phi[c + 1], ym = phi[c - L.nx], yp = phi[c + L.nx], zm = phi[c - L.nxy], zp = phi[c + L.nxy];
+    if (i > 0) xm += ec(i - 1, j, K);
+    if (i < L.nx - 1) xp += ec(i + 1, j, K);
+    if (j > 0) ym += ec(i, j - 1, K);
+    if (j < L.ny - 1) yp += ec(i, j + 1, K);
+    if (sz == 2) {
+        if (k > 0) zm += e[(i >> 1) + (long long)cnx * ((j >> 1) + (long long)cny * ((k - 1) >> 1))];
+        if (k < L.nz - 1) zp += e[(i >> 1) + (long long)cnx * ((j >> 1) + (long long)cny * ((k + 1) >> 1))];
+    }
+    double s = L.wx[c] * xm;
+    s = fma(L.wx[c + 1], xp, s);
+    s = fma(L.wy[c], ym, s);
+    s = fma(L.wy[c + L.nx], yp, s);
+    s = fma(L.wz[c], zm, s);
+    s = fma(L.wz[c + L.nxy], zp, s);
+    phi[c] = L.dinv[c] * (rhs[c] + s);
+}
+
 // r = rhs - A phi, A phi = D phi - sum w phi_nb, D = 1/dinv.
 __device__ __forceinline__ double residual_at(const LevelView& L, const double* __restrict__ phi,
                                               const double* __restrict__ rhs, long long c)

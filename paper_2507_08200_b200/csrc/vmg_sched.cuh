@@ -89,13 +89,15 @@ inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt)
 // ------------------------------------------------------------------------------------------------
 // plain path: one launch per step, in place on the level's current phi buffer
 // ------------------------------------------------------------------------------------------------
-inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count)
+// skip_first: number of leading half-sweeps already done by the caller
+inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int skip_first = 0)
 {
     VmgLevel& L = h->lev[l];
     LevelView v = view(L);
     long long nt = (long long)((L.nx + 1) / 2) * L.ny * L.nz;
     for (int s = 0; s < nsweeps; ++s)
         for (int colour = 0; colour < 2; ++colour) {
+            if (2 * s + colour < skip_first) continue;
             smooth_colour_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(v, cur_phi(L), L.rhs, colour, 0, L.nz);
             ++*count;
         }
@@ -122,7 +124,7 @@ inline void plain_prolong_correct(vmg_s* h, int l, long long* count)
 inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out)
 {
     VmgLevel& L = h->lev[0];
-    unsigned g = std::min<unsigned>(grid_for(L.n), 16u * (unsigned)h->num_sms);
+    unsigned g = grid_for(L.n);   // one cell per thread: a grid-stride loop serialises 13 dependent loads + a division per cell
     ProfScope ps(h, VMG_PC_NORM, nullptr);
     residual_norm_kernel<<<g, kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out, 0, L.nz);
 }
@@ -182,32 +184,32 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
 }
 
 // ------------------------------------------------------------------------------------------------
-// S2-S4, S6: blocked passes.  Tile width 40 (32 interior + 2 x 4 halo); one thread per x-pair, at most 640 threads
-// (102 registers each), the tile height is the largest even number of rows that fits threads and shared memory.
+// S2-S4, S6: blocked passes.  Tile width 40 (32 interior + 2 x 4 halo); one thread per 2 x 2 patch, at most 384
+// threads (168 registers each), the tile height is the largest even number of rows that fits threads and shared memory.
 // ------------------------------------------------------------------------------------------------
 constexpr int kBlkNXT = 40;
 constexpr int kBlkMaxSmem = 232448 - 1024;
-constexpr int blk_max_pairs(int TAIL) { return TAIL ? 560 : 640; }   // residual stage needs ~112 registers
+constexpr int kBlkMaxThreads = 384;
 
 constexpr int blk_pick_nyt(int S, int TAIL)
 {
     int best = 0;
-    for (int nyt = 2 * (S + (TAIL ? 1 : 0)) + 2; nyt <= 64; nyt += 2) {
-        long long np = (long long)(kBlkNXT / 2) * nyt;
+    for (int nyt = 2 * (S + 2) + 2; nyt <= 64; nyt += 2) {
+        long long nph = (long long)(kBlkNXT / 2) * (nyt / 2);
         int rs = S + (TAIL ? 1 : 0);
-        long long smem = ((long long)rs * 10 * np + (TAIL == BT_RESTRICT ? np : 0)) * 8;
-        if (np <= blk_max_pairs(TAIL) && smem <= kBlkMaxSmem) best = nyt;
+        long long smem = (long long)rs * 20 * nph * 8;
+        if (nph <= kBlkMaxThreads && smem <= kBlkMaxSmem) best = nyt;
     }
     return best;
 }
 
-template <int S, int TAIL, bool PROLONG>
+template <int S, int TAIL, bool PROLONG, int C0>
 struct BlkKernel {
     static constexpr int NYT = blk_pick_nyt(S, TAIL);
     using C = BlockCfg<S, TAIL, kBlkNXT, NYT>;
     static void prepare()
     {
-        cudaFuncSetAttribute(smooth_block_kernel<S, TAIL, PROLONG, kBlkNXT, NYT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaFuncSetAttribute(smooth_block_kernel<S, TAIL, PROLONG, C0, kBlkNXT, NYT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)C::SMEM);
     }
     static void launch(vmg_s* h, BlockArgs g)
@@ -224,13 +226,16 @@ struct BlkKernel {
         }
         g.nzseg = best;
         unsigned grid = (unsigned)(ntiles * g.nzseg);
-        smooth_block_kernel<S, TAIL, PROLONG, kBlkNXT, NYT><<<grid, C::NT, C::SMEM, h->stream>>>(g);
+        smooth_block_kernel<S, TAIL, PROLONG, C0, kBlkNXT, NYT><<<grid, C::NT, C::SMEM, h->stream>>>(g);
     }
 };
 
-#define VMG_BLK_CASE(S_, T_, P_)                                             \
-    if (prepare_all) BlkKernel<S_, T_, P_>::prepare();                       \
-    else if (S == S_ && tail == T_ && prolong == P_) { BlkKernel<S_, T_, P_>::launch(h, g); return; }
+#define VMG_BLK_CASE(S_, T_, P_)                                                             \
+    if (prepare_all) { BlkKernel<S_, T_, P_, 0>::prepare(); BlkKernel<S_, T_, P_, 1>::prepare(); } \
+    else if (S == S_ && tail == T_ && prolong == P_) {                                       \
+        if (g.colour0 & 1) BlkKernel<S_, T_, P_, 1>::launch(h, g); else BlkKernel<S_, T_, P_, 0>::launch(h, g); \
+        return;                                                                              \
+    }
 
 inline void blk_run(vmg_s* h, const BlockArgs& g, int S, int tail, bool prolong, bool prepare_all = false)
 {
@@ -338,12 +343,20 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         blocked_sweeps(h, l, 2 * h->nu2, 0, true, fuse ? BT_NORM : BT_NONE, norm_out, count);
         return fuse;
     }
+    if (h->nu2 >= 1) {   // the correction rides on the first half-sweep (smooth_colour_prolong_kernel)
+        ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
+        VmgLevel& L = h->lev[l];
+        long long nt = (long long)((L.nx + 1) / 2) * L.ny * L.nz;
+        smooth_colour_prolong_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, cur_phi(h->lev[l + 1]), 0,
+                                                                              h->three_d ? 2 : 1);
+        ++*count;
+        plain_smooth(h, l, h->nu2, count, 1);
+        return false;
+    }
     {
         ProfScope ps(h, l == 0 ? VMG_PC_PROLONG0 : VMG_PC_COARSE, count);
         plain_prolong_correct(h, l, count);
     }
-    ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
-    plain_smooth(h, l, h->nu2, count);
     return false;
 }
 
