@@ -47,7 +47,7 @@ size_t layout(vmg_s* h, double* base)
         VmgLevel& L = h->lev[l];
         double** padded[8] = {&L.wx, &L.wy, &L.wz, &L.dinv, &L.dbase, &L.phi, &L.rhs, &L.phi2};
         for (auto pp : padded) {
-            size_t o = p.take((size_t)L.pad + (size_t)L.n + (size_t)L.pad);
+            size_t o = p.take((size_t)L.pad + (size_t)L.nalloc + (size_t)L.pad);
             if (base) *pp = base + o + L.pad;
         }
         for (int f = 0; f < 6; ++f) {
@@ -77,7 +77,7 @@ int finalize_dinv(vmg_s* h)
         DinvArgs g;
         g.dbase = L.dbase; g.dinv = L.dinv;
         for (int f = 0; f < 6; ++f) { g.wb[f] = L.wb[f]; g.dirichlet[f] = h->bctype[f] == VMG_BC_DIRICHLET; }
-        g.nx = L.nx; g.ny = L.ny; g.nz = L.nz; g.three_d = h->three_d;
+        g.G = L.G; g.three_d = h->three_d;
         finalize_dinv_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(g);
     }
     CUDA_TRY(h, cudaGetLastError());
@@ -145,7 +145,9 @@ int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, do
         VmgLevel& L = h->lev[l];
         L.nx = nx >> l; L.ny = ny >> l; L.nz = three_d ? nz >> l : 1;
         L.n = (long long)L.nx * L.ny * L.nz;
-        L.pad = (long long)round_up((size_t)L.nx * L.ny + L.nx + 2, 32);
+        L.G = make_geom(L.nx, L.ny, L.nz);
+        L.nalloc = geom_alloc(L.G);
+        L.pad = (long long)round_up((size_t)L.G.plane + L.G.pitch + 2, 32);
         L.hx = dx * (1 << l); L.hy = dy * (1 << l); L.hz = three_d ? dz * (1 << l) : 1.0;
     }
     cudaError_t e = cudaGetDevice(&h->device);
@@ -226,7 +228,7 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
         g.bx = fbx; g.by = fby; g.bz = fbz;
         g.wx = L.wx; g.wy = L.wy; g.wz = L.wz; g.dbase = L.dbase;
         for (int f = 0; f < 6; ++f) g.wb[f] = L.wb[f];
-        g.nx = L.nx; g.ny = L.ny; g.nz = L.nz; g.three_d = h->three_d;
+        g.G = L.G; g.three_d = h->three_d;
         g.alpha = h->alpha; g.cx = beta / (L.hx * L.hx); g.cy = beta / (L.hy * L.hy);
         g.cz = h->three_d ? beta / (L.hz * L.hz) : 0.0;
         build_stencil_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(g);
@@ -314,15 +316,15 @@ static int solve_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int
     if (rc != VMG_OK) return rc;
     {
         ProfScope ps(h, VMG_PC_COPY, nullptr);
-        CUDA_TRY(h, cudaMemcpyAsync(L0.phi, phi, L0.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+        to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, L0.phi);
     }
     CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
     {
         ProfScope ps(h, VMG_PC_NORM, nullptr);
-        norm_inf_kernel<<<std::min<unsigned>(grid_for(L0.n), 4u * h->num_sms), kThreads, 0, h->stream>>>(L0.rhs, L0.n, scal + 0);
+        norm_inf_kernel<<<std::min<unsigned>(grid_for(L0.nalloc), 8u * h->num_sms), kThreads, 0, h->stream>>>(L0.rhs, L0.nalloc, scal + 0);
     }
     enqueue_residual_norm(h, scal + 1);
-    h->launches += 2;
+    h->launches += 3;   // phi copy-in, ||btilde||, first residual norm
     CUDA_TRY(h, cudaGetLastError());
     CUDA_TRY(h, cudaMemcpyAsync(h->h_scal, scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
@@ -358,7 +360,8 @@ static int solve_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int
     }
     {
         ProfScope ps(h, VMG_PC_COPY, nullptr);
-        CUDA_TRY(h, cudaMemcpyAsync(phi, L0.phi, L0.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+        to_natural_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, L0.phi, phi);
+        h->launches += 1;
     }
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     return status;

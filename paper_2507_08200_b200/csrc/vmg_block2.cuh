@@ -47,14 +47,12 @@ struct BlockArgs {
     const double *wx, *wy, *wz, *dinv, *rhs;   // level arrays, internal stencil form (cell 0)
     const double* phi_in;
     double* phi_out;
-    int nx, ny, nz;
-    long long nxy;
+    Geom G, CG;                    // layout of the level arrays and of the next coarser level's (vmg_kernels.cuh)
     int colour0;                   // colour of the first half-sweep of this pass (0 = red = (i+j+k) even)
     int ntx, nty;                  // tiles in x and y
     int nzseg;                     // z-segments per tile; gridDim.x = ntx * nty * nzseg, tile index fastest
     const double* e;               // PROLONG: coarse correction (cnx x cny x cnz)
     double *crhs, *cphi;           // BT_RESTRICT: coarse right-hand side (written), coarse phi (zeroed)
-    int cnx, cny;
     unsigned long long* norm_out;  // BT_NORM
 };
 
@@ -100,19 +98,21 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
     // CTA -> (tile, z-segment), tile index fastest; segments are cut at even z (restriction pairs stay together)
     const int ntiles = g.ntx * g.nty;
     const int tile = (int)(blockIdx.x % ntiles), seg = (int)(blockIdx.x / ntiles);
-    const int za = (int)((long long)(g.nz / 2) * seg / g.nzseg) * 2;
-    const int zb = seg == g.nzseg - 1 ? g.nz : (int)((long long)(g.nz / 2) * (seg + 1) / g.nzseg) * 2;
+    const int za = (int)((long long)(g.G.nz / 2) * seg / g.nzseg) * 2;
+    const int zb = seg == g.nzseg - 1 ? g.G.nz : (int)((long long)(g.G.nz / 2) * (seg + 1) / g.nzseg) * 2;
     const int tx = tile % g.ntx, ty = tile / g.ntx;
     const int gx = tx * C::TX - C::HX + 2 * m, gy0 = ty * C::TY - H + 2 * jj;      // rows gy0 and gy0 + 1
-    const bool in_x = live && gx >= 0 && gx < g.nx;
-    const bool in_r[2] = {in_x && gy0 >= 0 && gy0 < g.ny, in_x && gy0 + 1 >= 0 && gy0 + 1 < g.ny};
+    const bool in_x = live && gx >= 0 && gx < g.G.nx;
+    const bool in_r[2] = {in_x && gy0 >= 0 && gy0 < g.G.ny, in_x && gy0 + 1 >= 0 && gy0 + 1 < g.G.ny};
     const bool int_x = m >= C::HX / 2 && m < C::HX / 2 + C::TX / 2;
     const bool interior[2] = {in_r[0] && int_x && 2 * jj >= H && 2 * jj < H + C::TY,
                               in_r[1] && int_x && 2 * jj + 1 >= H && 2 * jj + 1 < H + C::TY};
     // rows 0 and NYT-1 and the first / last column of the tile are rim: never relaxed.  ok[r][sg]: row r, x-parity sg
     const bool ok[2][2] = {{live && jj >= 1 && m > 0, live && jj >= 1 && m < NXP - 1},
                            {live && jj <= NYT / 2 - 2 && m > 0, live && jj <= NYT / 2 - 2 && m < NXP - 1}};
-    const long long cbase = gx + (long long)g.nx * gy0;
+    // the x-pair's even cell in row gy0 of plane 0 (internal layout); its odd cell is `odd` further on
+    const long long cbase = (long long)g.G.pitch * gy0 + (gx >> 1);
+    const int odd = g.G.ne + 1;
 
     // register rings [row][slot]: even-x / odd-x phi and wz of this thread's pair; plane z0 + n lives in slot n % R
     double pe[2][R], po[2][R], we[2][R], wo[2][R];
@@ -127,17 +127,22 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
     // loads in flight: phi, wz (and the coarse correction) of plane zq; rhs, 1/D, wx, wy of plane zq - 1
     double2 r_phi[2], r_wz[2], r_rhs[2], r_dinv[2], r_wx[2], r_wy[2];
     double r_e[2] = {0.0, 0.0};
+    auto ld2 = [&](const double* p, long long c) { return make_double2(__ldg(p + c), __ldg(p + c + odd)); };
     auto issue = [&](int zq) {
         // pull the planes kBlkPrefetch further on from HBM into L2 now (one request per 32-byte sector): all CTAs march
         // in step, so their loads come in bursts; with the DRAM latency taken early the staged loads below hit L2
-        if (!(m & 1) && zq + kBlkPrefetch < g.nz && zq + kBlkPrefetch > 0) {
+        if (!(m & 3) && zq + kBlkPrefetch < g.G.nz && zq + kBlkPrefetch > 0) {
 #pragma unroll
             for (int r = 0; r < 2; ++r)
                 if (in_r[r]) {
-                    const long long c = cbase + r * g.nx + g.nxy * (zq + kBlkPrefetch);
-                    prefetch_l2(g.phi_in + c); prefetch_l2(g.wz + c);
-                    prefetch_l2(g.rhs + c - g.nxy); prefetch_l2(g.dinv + c - g.nxy);
-                    prefetch_l2(g.wx + c - g.nxy); prefetch_l2(g.wy + c - g.nxy);
+                    const long long c = cbase + r * g.G.pitch + g.G.plane * (zq + kBlkPrefetch);
+#pragma unroll
+                    for (int o = 0; o < 2; ++o) {
+                        const long long d = c + o * odd;
+                        prefetch_l2(g.phi_in + d); prefetch_l2(g.wz + d);
+                        prefetch_l2(g.rhs + d - g.G.plane); prefetch_l2(g.dinv + d - g.G.plane);
+                        prefetch_l2(g.wx + d - g.G.plane); prefetch_l2(g.wy + d - g.G.plane);
+                    }
                 }
         }
         const double2 zero = make_double2(0.0, 0.0);
@@ -148,24 +153,23 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
 #ifdef VMG_ABL_NOLOAD
             if (in_r[r] && zq == -12345) {
 #else
-            if (in_r[r] && zq >= 0 && zq < g.nz) {
+            if (in_r[r] && zq >= 0 && zq < g.G.nz) {
 #endif
-                const long long c = cbase + r * g.nx + g.nxy * zq;
-                r_phi[r] = ldg2(g.phi_in + c);
-                r_wz[r] = ldg2(g.wz + c);
-                if (PROLONG)
-                    r_e[r] = __ldg(g.e + (gx >> 1) + (long long)g.cnx * (((gy0 + r) >> 1) + (long long)g.cny * (zq >> 1)));
+                const long long c = cbase + r * g.G.pitch + g.G.plane * zq;
+                r_phi[r] = ld2(g.phi_in, c);
+                r_wz[r] = ld2(g.wz, c);
+                if (PROLONG) r_e[r] = __ldg(g.e + cell_at(g.CG, gx >> 1, (gy0 + r) >> 1, zq >> 1));
             }
 #ifdef VMG_ABL_NOLOAD
             if (in_r[r] && zq == -12345) {
 #else
-            if (in_r[r] && zq - 1 >= 0 && zq - 1 < g.nz) {
+            if (in_r[r] && zq - 1 >= 0 && zq - 1 < g.G.nz) {
 #endif
-                const long long c = cbase + r * g.nx + g.nxy * (zq - 1);
-                r_rhs[r] = ldg2(g.rhs + c);
-                r_dinv[r] = ldg2(g.dinv + c);
-                r_wx[r] = ldg2(g.wx + c);
-                r_wy[r] = ldg2(g.wy + c);
+                const long long c = cbase + r * g.G.pitch + g.G.plane * (zq - 1);
+                r_rhs[r] = ld2(g.rhs, c);
+                r_dinv[r] = ld2(g.dinv, c);
+                r_wx[r] = ld2(g.wx, c);
+                r_wy[r] = ld2(g.wy, c);
             }
         }
     };
@@ -272,7 +276,7 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
                             acc += res[0][0] + res[0][1];
                             acc += res[1][0] + res[1][1];
                             if (pr & 1) {
-                                const long long cc = (gx >> 1) + (long long)g.cnx * ((gy0 >> 1) + (long long)g.cny * (pr >> 1));
+                                const long long cc = cell_at(g.CG, gx >> 1, gy0 >> 1, pr >> 1);
                                 g.crhs[cc] = acc / 8.0;
                                 g.cphi[cc] = 0.0;
                                 acc = 0.0;
@@ -291,8 +295,10 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
                 if (p >= za && p < zb) {
 #pragma unroll
                     for (int r = 0; r < 2; ++r)
-                        if (interior[r])
-                            *reinterpret_cast<double2*>(g.phi_out + cbase + r * g.nx + g.nxy * p) = make_double2(pe[r][c], po[r][c]);
+                        if (interior[r]) {
+                            double* q = g.phi_out + cbase + r * g.G.pitch + g.G.plane * p;
+                            q[0] = pe[r][c]; q[odd] = po[r][c];
+                        }
                 }
             }
             // ---- plane zl (still untouched, ring slot u) and its coefficients replace plane zl - RS in shared memory ----

@@ -2,18 +2,21 @@
 //
 // Internal stencil form of a level (built by vmg_set_coeffs / vmg_set_bc):
 //   wx[c] = beta*bx/hx^2 of the LOW-x face of cell c, stored per cell and 0 where that face is a domain
-//           boundary; the HIGH-x face weight of cell c is wx[c+1], which is the next row's (zero) low
-//           boundary entry when c is the last cell of a row.  Same for wy (stride nx) and wz (stride nx*ny).
+//           boundary; the HIGH-x face weight of cell c is the wx of its high-x neighbour (a zero pad element
+//           after the last cell of a row).  Same for wy (one row on) and wz (one plane on).
+//   Cell arrays are stored x-parity split (struct Geom in vmg_kernels.cuh): per row the even-x cells, a zero,
+//   the odd-x cells, a zero.
 //   dinv[c] = 1 / D_c,  D_c = alpha*a_c + sum(interior face weights) + 2*sum(Dirichlet boundary face weights)
 //   dbase[c] = alpha*a_c + sum(interior face weights)          (boundary-type independent part of D_c)
 //   wb[f]    = boundary-face weights beta*b/h^2 on domain face f (a plane), used to finish dinv and by fold_bc
-// Every cell array is allocated with `pad` zeroed doubles before and after, so that c-1, c+1, c-nx, c+nx,
-// c-nx*ny, c+nx*ny are always readable and every out-of-domain neighbour is multiplied by a zero weight:
+// Every cell array is allocated with `pad` zeroed doubles before and after, so that the six neighbours of every
+// cell are always readable and every out-of-domain neighbour is multiplied by a zero weight:
 // the kernels carry no boundary branches (PAPER.md:230,266,284 boundary kinds live in the coefficients).
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <vector>
+#include "vmg_kernels.cuh"
 
 // kernel classes for the optional per-kernel event profile (vmg_get_profile)
 enum { VMG_PC_SMOOTH0 = 0, VMG_PC_RESREST0 = 1, VMG_PC_PROLONG0 = 2, VMG_PC_COARSE = 3, VMG_PC_NORM = 4,
@@ -24,6 +27,8 @@ struct VmgProfEvent { int cls; long long launches; cudaEvent_t start, stop; };
 struct VmgLevel {
     int nx = 0, ny = 0, nz = 0;
     long long n = 0;          // cells
+    vmg::Geom G;              // internal layout of the cell arrays
+    long long nalloc = 0;     // doubles of one cell array (pitch * ny * nz)
     long long pad = 0;        // zeroed doubles before and after each padded array
     double hx = 0, hy = 0, hz = 0;
     // padded cell arrays (pointer to cell 0)

@@ -12,6 +12,39 @@ constexpr int kThreads = 256;
 __host__ __device__ inline long long cdiv(long long a, long long b) { return (a + b - 1) / b; }
 
 // ------------------------------------------------------------------------------------------------
+// Internal layout of a level's cell arrays ("x-parity split").  A colour half-sweep
+// touches every other cell of a row, so in the natural layout half of every 32-byte sector of rhs, 1/D and of the
+// phi being written is fetched for nothing.  Each row therefore stores its even-x cells first, then its odd-x
+// cells, each block followed by one zero element:   [E_0 .. E_{ne-1} 0 | O_0 .. O_{no-1} 0],  pitch = nx + 2.
+// A half-sweep then reads and writes unit-stride runs and moves 5 doubles per relaxation instead of 7.  The pad
+// elements double as the zero weight / zero neighbour beyond the low and high x faces (the x-neighbours of E_m are
+// O_{m-1}, O_m, those of O_m are E_m, E_{m+1}); y- and z-neighbours are +-pitch, +-plane away, and beyond the domain
+// they land in another row / plane or in the zeroed pad before and after the array, always under a zero weight.
+// ------------------------------------------------------------------------------------------------
+struct Geom {
+    int nx, ny, nz, ne, pitch;   // ne = even-x cells per row
+    long long plane, n;          // plane = pitch * ny (doubles per z-plane), n = nx*ny*nz (cells)
+};
+
+__host__ __device__ inline Geom make_geom(int nx, int ny, int nz)
+{
+    Geom G;
+    G.nx = nx; G.ny = ny; G.nz = nz; G.ne = (nx + 1) / 2; G.pitch = nx + 2;
+    G.plane = (long long)G.pitch * ny; G.n = (long long)nx * ny * nz;
+    return G;
+}
+__host__ __device__ inline long long geom_alloc(const Geom& G) { return G.plane * G.nz; }
+__host__ __device__ __forceinline__ long long cell_at(const Geom& G, int i, int j, int k)
+{
+    return G.plane * k + (long long)G.pitch * j + (i & 1) * (G.ne + 1) + (i >> 1);
+}
+// natural cell number t = i + nx*(j + ny*k) -> (i, j, k)
+__device__ __forceinline__ void unflatten(const Geom& G, long long t, int& i, int& j, int& k)
+{
+    i = (int)(t % G.nx); j = (int)((t / G.nx) % G.ny); k = (int)(t / ((long long)G.nx * G.ny));
+}
+
+// ------------------------------------------------------------------------------------------------
 // S0. Coefficient averaging to the next coarser level (north_star (2) "coefficient averaging";
 // reading R10: a = mean of children, b = mean of the fine faces lying on the coarse face).
 // Public layouts on both sides.  NULL fine a means a == 0; NULL fine b means b == 1.
@@ -60,101 +93,130 @@ __global__ void coarsen_b_kernel(const double* __restrict__ fb, double* __restri
     }
 }
 
+
 // ------------------------------------------------------------------------------------------------
-// Internal stencil form of one level from its raw coefficients (C1 of DESIGN.md).
+// Internal stencil form of one level from its raw coefficients (C1 of DESIGN.md).  Raw arrays in the public
+// layout, internal arrays in the x-parity split layout.
 // ------------------------------------------------------------------------------------------------
 struct StencilBuildArgs {
     const double *a, *bx, *by, *bz;      // raw, public layout (may be NULL)
-    double *wx, *wy, *wz, *dbase;        // padded cell arrays
-    double* wb[6];                       // boundary planes
-    int nx, ny, nz, three_d;
+    double *wx, *wy, *wz, *dbase;        // internal cell arrays
+    double* wb[6];                       // boundary planes (natural plane layout)
+    Geom G;
+    int three_d;
     double alpha, cx, cy, cz;            // cx = beta/hx^2 ...
 };
 
 __global__ void build_stencil_kernel(StencilBuildArgs g)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long n = (long long)g.nx * g.ny * g.nz;
-    if (t >= n) return;
-    int i = (int)(t % g.nx), j = (int)((t / g.nx) % g.ny), k = (int)(t / ((long long)g.nx * g.ny));
-    long long nxy = (long long)g.nx * g.ny;
-    double bxl = g.bx ? g.bx[i + (long long)(g.nx + 1) * (j + (long long)g.ny * k)] : 1.0;
-    double bxh = g.bx ? g.bx[i + 1 + (long long)(g.nx + 1) * (j + (long long)g.ny * k)] : 1.0;
-    double byl = g.by ? g.by[i + (long long)g.nx * (j + (long long)(g.ny + 1) * k)] : 1.0;
-    double byh = g.by ? g.by[i + (long long)g.nx * (j + 1 + (long long)(g.ny + 1) * k)] : 1.0;
+    if (t >= g.G.n) return;
+    const int nx = g.G.nx, ny = g.G.ny, nz = g.G.nz;
+    int i, j, k;
+    unflatten(g.G, t, i, j, k);
+    long long nxy = (long long)nx * ny;
+    double bxl = g.bx ? g.bx[i + (long long)(nx + 1) * (j + (long long)ny * k)] : 1.0;
+    double bxh = g.bx ? g.bx[i + 1 + (long long)(nx + 1) * (j + (long long)ny * k)] : 1.0;
+    double byl = g.by ? g.by[i + (long long)nx * (j + (long long)(ny + 1) * k)] : 1.0;
+    double byh = g.by ? g.by[i + (long long)nx * (j + 1 + (long long)(ny + 1) * k)] : 1.0;
     double wxl = g.cx * bxl, wxh = g.cx * bxh, wyl = g.cy * byl, wyh = g.cy * byh, wzl = 0.0, wzh = 0.0;
     if (g.three_d) {
         double bzl = g.bz ? g.bz[t] : 1.0;
         double bzh = g.bz ? g.bz[t + nxy] : 1.0;
         wzl = g.cz * bzl; wzh = g.cz * bzh;
     }
-    if (i == 0)        { g.wb[0][j + (long long)g.ny * k] = wxl; wxl = 0.0; }
-    if (i == g.nx - 1) { g.wb[1][j + (long long)g.ny * k] = wxh; wxh = 0.0; }
-    if (j == 0)        { g.wb[2][i + (long long)g.nx * k] = wyl; wyl = 0.0; }
-    if (j == g.ny - 1) { g.wb[3][i + (long long)g.nx * k] = wyh; wyh = 0.0; }
+    if (i == 0)      { g.wb[0][j + (long long)ny * k] = wxl; wxl = 0.0; }
+    if (i == nx - 1) { g.wb[1][j + (long long)ny * k] = wxh; wxh = 0.0; }
+    if (j == 0)      { g.wb[2][i + (long long)nx * k] = wyl; wyl = 0.0; }
+    if (j == ny - 1) { g.wb[3][i + (long long)nx * k] = wyh; wyh = 0.0; }
     if (g.three_d) {
-        if (k == 0)        { g.wb[4][i + (long long)g.nx * j] = wzl; wzl = 0.0; }
-        if (k == g.nz - 1) { g.wb[5][i + (long long)g.nx * j] = wzh; wzh = 0.0; }
+        if (k == 0)      { g.wb[4][i + (long long)nx * j] = wzl; wzl = 0.0; }
+        if (k == nz - 1) { g.wb[5][i + (long long)nx * j] = wzh; wzh = 0.0; }
     }
-    g.wx[t] = wxl; g.wy[t] = wyl; g.wz[t] = wzl;
+    const long long c = cell_at(g.G, i, j, k);
+    g.wx[c] = wxl; g.wy[c] = wyl; g.wz[c] = wzl;
     double d = g.a ? g.alpha * g.a[t] : 0.0;
     d += wxl; d += wxh; d += wyl; d += wyh; d += wzl; d += wzh;
-    g.dbase[t] = d;
+    g.dbase[c] = d;
 }
 
 struct DinvArgs {
     const double* dbase; double* dinv; const double* wb[6];
-    int nx, ny, nz, three_d; int dirichlet[6];
+    Geom G;
+    int three_d; int dirichlet[6];
 };
 
 __global__ void finalize_dinv_kernel(DinvArgs g)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long n = (long long)g.nx * g.ny * g.nz;
-    if (t >= n) return;
-    int i = (int)(t % g.nx), j = (int)((t / g.nx) % g.ny), k = (int)(t / ((long long)g.nx * g.ny));
-    double d = g.dbase[t];
-    if (i == 0 && g.dirichlet[0])        d += 2.0 * g.wb[0][j + (long long)g.ny * k];
-    if (i == g.nx - 1 && g.dirichlet[1]) d += 2.0 * g.wb[1][j + (long long)g.ny * k];
-    if (j == 0 && g.dirichlet[2])        d += 2.0 * g.wb[2][i + (long long)g.nx * k];
-    if (j == g.ny - 1 && g.dirichlet[3]) d += 2.0 * g.wb[3][i + (long long)g.nx * k];
+    if (t >= g.G.n) return;
+    const int nx = g.G.nx, ny = g.G.ny, nz = g.G.nz;
+    int i, j, k;
+    unflatten(g.G, t, i, j, k);
+    const long long c = cell_at(g.G, i, j, k);
+    double d = g.dbase[c];
+    if (i == 0 && g.dirichlet[0])      d += 2.0 * g.wb[0][j + (long long)ny * k];
+    if (i == nx - 1 && g.dirichlet[1]) d += 2.0 * g.wb[1][j + (long long)ny * k];
+    if (j == 0 && g.dirichlet[2])      d += 2.0 * g.wb[2][i + (long long)nx * k];
+    if (j == ny - 1 && g.dirichlet[3]) d += 2.0 * g.wb[3][i + (long long)nx * k];
     if (g.three_d) {
-        if (k == 0 && g.dirichlet[4])        d += 2.0 * g.wb[4][i + (long long)g.nx * j];
-        if (k == g.nz - 1 && g.dirichlet[5]) d += 2.0 * g.wb[5][i + (long long)g.nx * j];
+        if (k == 0 && g.dirichlet[4])      d += 2.0 * g.wb[4][i + (long long)nx * j];
+        if (k == nz - 1 && g.dirichlet[5]) d += 2.0 * g.wb[5][i + (long long)nx * j];
     }
-    g.dinv[t] = 1.0 / d;
+    g.dinv[c] = 1.0 / d;
 }
 
 // ------------------------------------------------------------------------------------------------
 // S1. fold_bc: btilde = f + 2*w_b*g on Dirichlet-adjacent cells + w_b*h*q on Neumann-adjacent cells
-// (w_b = beta*b/h^2 of the boundary face; R3, R5).  Level 0, once per solve.
+// (w_b = beta*b/h^2 of the boundary face; R3, R5).  Level 0, once per solve.  rhs: public layout; bt: internal
+// layout, or public layout when bt_natural (the single-step entry point).
 // ------------------------------------------------------------------------------------------------
 struct FoldArgs {
     const double* rhs; double* bt; const double* wb[6]; const double* val[6];
-    int nx, ny, nz, three_d; int dirichlet[6]; double h[3];
+    Geom G;
+    int three_d, bt_natural; int dirichlet[6]; double h[3];
 };
 
 __global__ void fold_bc_kernel(FoldArgs g)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long n = (long long)g.nx * g.ny * g.nz;
-    if (t >= n) return;
-    int i = (int)(t % g.nx), j = (int)((t / g.nx) % g.ny), k = (int)(t / ((long long)g.nx * g.ny));
+    if (t >= g.G.n) return;
+    const int nx = g.G.nx, ny = g.G.ny, nz = g.G.nz;
+    int i, j, k;
+    unflatten(g.G, t, i, j, k);
     double v = g.rhs[t];
     auto add = [&](int f, long long pl, double hd) {
         if (!g.val[f]) return;
         double w = g.wb[f][pl], q = g.val[f][pl];
         v += g.dirichlet[f] ? 2.0 * w * q : w * hd * q;
     };
-    if (i == 0)        add(0, j + (long long)g.ny * k, g.h[0]);
-    if (i == g.nx - 1) add(1, j + (long long)g.ny * k, g.h[0]);
-    if (j == 0)        add(2, i + (long long)g.nx * k, g.h[1]);
-    if (j == g.ny - 1) add(3, i + (long long)g.nx * k, g.h[1]);
+    if (i == 0)      add(0, j + (long long)ny * k, g.h[0]);
+    if (i == nx - 1) add(1, j + (long long)ny * k, g.h[0]);
+    if (j == 0)      add(2, i + (long long)nx * k, g.h[1]);
+    if (j == ny - 1) add(3, i + (long long)nx * k, g.h[1]);
     if (g.three_d) {
-        if (k == 0)        add(4, i + (long long)g.nx * j, g.h[2]);
-        if (k == g.nz - 1) add(5, i + (long long)g.nx * j, g.h[2]);
+        if (k == 0)      add(4, i + (long long)nx * j, g.h[2]);
+        if (k == nz - 1) add(5, i + (long long)nx * j, g.h[2]);
     }
-    g.bt[t] = v;
+    g.bt[g.bt_natural ? t : cell_at(g.G, i, j, k)] = v;
+}
+
+// public (natural) layout <-> internal layout of one cell array
+__global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in)
+{
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= G.n) return;
+    int i, j, k;
+    unflatten(G, t, i, j, k);
+    in[cell_at(G, i, j, k)] = nat[t];
+}
+__global__ void to_natural_kernel(Geom G, const double* __restrict__ in, double* __restrict__ nat)
+{
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= G.n) return;
+    int i, j, k;
+    unflatten(G, t, i, j, k);
+    nat[t] = in[cell_at(G, i, j, k)];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -163,124 +225,133 @@ __global__ void fold_bc_kernel(FoldArgs g)
 // ------------------------------------------------------------------------------------------------
 struct LevelView {
     const double *wx, *wy, *wz, *dinv;
-    int nx, ny, nz;
-    long long nxy, n;
+    Geom G;
 };
 
-__device__ __forceinline__ double nb_sum(const LevelView& L, const double* __restrict__ phi, long long c)
+// c: the cell; xm: its low-x neighbour (the high-x neighbour is xm + 1: E_m sits between O_{m-1} and O_m, O_m between
+// E_m and E_{m+1}).  Same expression, same order, everywhere a relaxation or a residual is evaluated.
+__device__ __forceinline__ double nb_sum(const LevelView& L, const double* __restrict__ phi, long long c, long long xm)
 {
-    double s = L.wx[c] * phi[c - 1];
-    s = fma(L.wx[c + 1], phi[c + 1], s);
-    s = fma(L.wy[c], phi[c - L.nx], s);
-    s = fma(L.wy[c + L.nx], phi[c + L.nx], s);
-    s = fma(L.wz[c], phi[c - L.nxy], s);
-    s = fma(L.wz[c + L.nxy], phi[c + L.nxy], s);
+    double s = L.wx[c] * phi[xm];
+    s = fma(L.wx[xm + 1], phi[xm + 1], s);
+    s = fma(L.wy[c], phi[c - L.G.pitch], s);
+    s = fma(L.wy[c + L.G.pitch], phi[c + L.G.pitch], s);
+    s = fma(L.wz[c], phi[c - L.G.plane], s);
+    s = fma(L.wz[c + L.G.plane], phi[c + L.G.plane], s);
     return s;
 }
 
-// S2 (baseline). One colour half-sweep: phi_c <- (rhs_c + sum w phi_nb) / D_c for (i+j+k)%2 == colour.
-// Planes [k0, k1) only (the L2 wavefront schedule launches it slab by slab).
-__global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour,
-                                     int k0, int k1)
+// cell and low-x neighbour of pair m, x-parity par, in the row starting at `row`
+__device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, int par, long long& c, long long& xm)
 {
-    int hx = (L.nx + 1) >> 1;
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long nt = (long long)hx * L.ny * (k1 - k0);
-    if (t >= nt) return;
-    int m = (int)(t % hx), j = (int)((t / hx) % L.ny), k = k0 + (int)(t / ((long long)hx * L.ny));
-    int i = 2 * m + ((colour + j + k) & 1);
-    if (i >= L.nx) return;
-    long long c = i + (long long)L.nx * j + L.nxy * k;
-    phi[c] = L.dinv[c] * (rhs[c] + nb_sum(L, phi, c));
+    c = row + m + (par ? G.ne + 1 : 0);
+    xm = row + m + (par ? 0 : G.ne);
 }
 
-// S4 + S2 fused (plain path).  The first colour half-sweep after a coarse-grid correction: a relaxation never reads
-// the old value of the cell it overwrites, and all six neighbours of a cell of one colour have the other colour, so
-// the correction phi += P e (piecewise constant, R9) is applied to the NEIGHBOURS on the fly and never stored: the
-// cells of the other colour keep their uncorrected values in memory until the next half-sweep overwrites them.
-// Valid when at least one full sweep follows (nu2 >= 1).  phi_nb + e is the very addition prolong_correct_kernel
-// performs, so results are bitwise those of the two separate kernels.
-__global__ void smooth_colour_prolong_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs,
+// S2 (per-colour path). One colour half-sweep: phi_c <- (rhs_c + sum w phi_nb) / D_c for (i+j+k)%2 == colour.
+__global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour)
+{
+    const Geom& G = L.G;
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long nt = (long long)G.ne * G.ny * G.nz;
+    if (t >= nt) return;
+    int m = (int)(t % G.ne), j = (int)((t / G.ne) % G.ny), k = (int)(t / ((long long)G.ne * G.ny));
+    int par = (colour + j + k) & 1;
+    if (2 * m + par >= G.nx) return;
+    long long c, xm;
+    pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
+    phi[c] = L.dinv[c] * (rhs[c] + nb_sum(L, phi, c, xm));
+}
+
+// S4 + S2 fused (per-colour path).  The first colour half-sweep after a coarse-grid correction: a relaxation never
+// reads the old value of the cell it overwrites, and all six neighbours of a cell of one colour have the other
+// colour, so the correction phi += P e (piecewise constant, R9) is applied to the NEIGHBOURS on the fly and never
+// stored: the cells of the other colour keep their uncorrected values in memory until the next half-sweep
+// overwrites them.  Valid when at least one full sweep follows (nu2 >= 1).  phi_nb + e is the very addition
+// prolong_correct_kernel performs, so results are bitwise those of the two separate kernels.
+__global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __restrict__ phi, const double* __restrict__ rhs,
                                              const double* __restrict__ e, int colour, int sz)
 {
-    int hx = (L.nx + 1) >> 1;
+    const Geom& G = L.G;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long nt = (long long)hx * L.ny * L.nz;
+    long long nt = (long long)G.ne * G.ny * G.nz;
     if (t >= nt) return;
-    int m = (int)(t % hx), j = (int)((t / hx) % L.ny), k = (int)(t / ((long long)hx * L.ny));
-    int i = 2 * m + ((colour + j + k) & 1);
-    if (i >= L.nx) return;
-    long long c = i + (long long)L.nx * j + L.nxy * k;
-    const int cnx = L.nx >> 1, cny = L.ny >> 1;
+    int m = (int)(t % G.ne), j = (int)((t / G.ne) % G.ny), k = (int)(t / ((long long)G.ne * G.ny));
+    int par = (colour + j + k) & 1;
+    int i = 2 * m + par;
+    if (i >= G.nx) return;
+    long long c, xm;
+    pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
     const int K = sz == 2 ? (k >> 1) : k;
-    auto ec = [&](int ii, int jj, int kk) { return e[(ii >> 1) + (long long)cnx * ((jj >> 1) + (long long)cny * kk)]; };
-    // out-of-domain neighbours carry a zero weight; their (zero-pad) value is used uncorrected
-    double xm = phi[c - 1], xp = phi[c + 1], ym = phi[c - L.nx], yp = phi[c + L.nx], zm = phi[c - L.nxy], zp = phi[c + L.nxy];
-    if (i > 0) xm += ec(i - 1, j, K);
-    if (i < L.nx - 1) xp += ec(i + 1, j, K);
-    if (j > 0) ym += ec(i, j - 1, K);
-    if (j < L.ny - 1) yp += ec(i, j + 1, K);
+    // out-of-domain neighbours carry a zero weight; their (zero-pad or foreign) value is used uncorrected
+    double vxm = phi[xm], vxp = phi[xm + 1], vym = phi[c - G.pitch], vyp = phi[c + G.pitch], vzm = phi[c - G.plane], vzp = phi[c + G.plane];
+    if (i > 0) vxm += e[cell_at(CG, (i - 1) >> 1, j >> 1, K)];
+    if (i < G.nx - 1) vxp += e[cell_at(CG, (i + 1) >> 1, j >> 1, K)];
+    if (j > 0) vym += e[cell_at(CG, i >> 1, (j - 1) >> 1, K)];
+    if (j < G.ny - 1) vyp += e[cell_at(CG, i >> 1, (j + 1) >> 1, K)];
     if (sz == 2) {
-        if (k > 0) zm += e[(i >> 1) + (long long)cnx * ((j >> 1) + (long long)cny * ((k - 1) >> 1))];
-        if (k < L.nz - 1) zp += e[(i >> 1) + (long long)cnx * ((j >> 1) + (long long)cny * ((k + 1) >> 1))];
+        if (k > 0) vzm += e[cell_at(CG, i >> 1, j >> 1, (k - 1) >> 1)];
+        if (k < G.nz - 1) vzp += e[cell_at(CG, i >> 1, j >> 1, (k + 1) >> 1)];
     }
-    double s = L.wx[c] * xm;
-    s = fma(L.wx[c + 1], xp, s);
-    s = fma(L.wy[c], ym, s);
-    s = fma(L.wy[c + L.nx], yp, s);
-    s = fma(L.wz[c], zm, s);
-    s = fma(L.wz[c + L.nxy], zp, s);
+    double s = L.wx[c] * vxm;
+    s = fma(L.wx[xm + 1], vxp, s);
+    s = fma(L.wy[c], vym, s);
+    s = fma(L.wy[c + G.pitch], vyp, s);
+    s = fma(L.wz[c], vzm, s);
+    s = fma(L.wz[c + G.plane], vzp, s);
     phi[c] = L.dinv[c] * (rhs[c] + s);
 }
 
 // r = rhs - A phi, A phi = D phi - sum w phi_nb, D = 1/dinv.
 __device__ __forceinline__ double residual_at(const LevelView& L, const double* __restrict__ phi,
-                                              const double* __restrict__ rhs, long long c)
+                                              const double* __restrict__ rhs, long long c, long long xm)
 {
-    return rhs[c] + nb_sum(L, phi, c) - phi[c] / L.dinv[c];
+    return rhs[c] + nb_sum(L, phi, c, xm) - phi[c] / L.dinv[c];
 }
 
+// r in the public layout (single-step entry point)
 __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
                                 double* __restrict__ r)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (t >= L.n) return;
-    r[t] = residual_at(L, phi, rhs, t);
+    if (t >= L.G.n) return;
+    int i, j, k;
+    unflatten(L.G, t, i, j, k);
+    long long c, xm;
+    pair_addr(L.G, L.G.plane * k + (long long)L.G.pitch * j, i >> 1, i & 1, c, xm);
+    r[t] = residual_at(L, phi, rhs, c, xm);
 }
 
-// S3 (baseline). Fused residual + restriction: one thread per coarse cell; also zeroes the coarse phi.
-// Coarse planes [K0, K1) only.
-__global__ void residual_restrict_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz, int K0, int K1)
+// S3 (per-colour path). Fused residual + restriction: one thread per coarse cell; also zeroes the coarse phi.
+__global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
+                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz)
 {
-    int cnx = L.nx >> 1, cny = L.ny >> 1;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long n = (long long)cnx * cny * (K1 - K0);
-    if (t >= n) return;
-    int I = (int)(t % cnx), J = (int)((t / cnx) % cny), K = K0 + (int)(t / ((long long)cnx * cny));
-    t = I + (long long)cnx * (J + (long long)cny * K);
+    if (t >= CG.n) return;
+    int I, J, K;
+    unflatten(CG, t, I, J, K);
     double s = 0.0;
     for (int r = 0; r < sz; ++r)
         for (int q = 0; q < 2; ++q) {   // the x-pair first, then accumulated (the blocked kernel sums in this order too)
-            long long c = (2 * I) + (long long)L.nx * (2 * J + q) + L.nxy * (sz * K + r);
-            s += residual_at(L, phi, rhs, c) + residual_at(L, phi, rhs, c + 1);
+            long long row = L.G.plane * (sz * K + r) + (long long)L.G.pitch * (2 * J + q), ce, xe, co, xo;
+            pair_addr(L.G, row, I, 0, ce, xe);
+            pair_addr(L.G, row, I, 1, co, xo);
+            s += residual_at(L, phi, rhs, ce, xe) + residual_at(L, phi, rhs, co, xo);
         }
-    crhs[t] = s / (4.0 * sz);
-    if (cphi) cphi[t] = 0.0;
+    const long long cc = cell_at(CG, I, J, K);
+    crhs[cc] = s / (4.0 * sz);
+    if (cphi) cphi[cc] = 0.0;
 }
 
-// S4 (baseline). Fused prolongation + correction (piecewise constant, R9): phi_f += e_c[i/2, j/2, k/2].
-// Fine planes [k0, k1) only.
-__global__ void prolong_correct_kernel(double* __restrict__ phi, const double* __restrict__ e,
-                                       int nx, int ny, int sz, int k0, int k1)
+// S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise
+// constant, R9): phi_f += e_c[i/2, j/2, k/2].
+__global__ void prolong_correct_kernel(Geom G, Geom CG, double* __restrict__ phi, const double* __restrict__ e, int sz)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long n = (long long)nx * ny * (k1 - k0);
-    if (t >= n) return;
-    t += (long long)nx * ny * k0;
-    int i = (int)(t % nx), j = (int)((t / nx) % ny), k = (int)(t / ((long long)nx * ny));
-    int cnx = nx >> 1, cny = ny >> 1;
-    phi[t] += e[(i >> 1) + (long long)cnx * ((j >> 1) + (long long)cny * (sz == 2 ? (k >> 1) : k))];
+    if (t >= G.n) return;
+    int i, j, k;
+    unflatten(G, t, i, j, k);
+    phi[cell_at(G, i, j, k)] += e[cell_at(CG, i >> 1, j >> 1, sz == 2 ? (k >> 1) : k)];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -310,6 +381,7 @@ __device__ __forceinline__ void block_max_to_global(double v, unsigned long long
     }
 }
 
+// any array of n doubles (an internal array is passed whole: its pad elements are zero)
 __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsigned long long* out)
 {
     double m = 0.0;
@@ -323,20 +395,29 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
     block_max_to_global(m, out);
 }
 
-// planes [k0, k1) only; accumulates into *out with atomicMax (the caller zeroes it)
+// ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one thread per x-pair
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                     unsigned long long* out, int k0, int k1)
+                                     unsigned long long* out)
 {
-    double m = 0.0;
+    const Geom& G = L.G;
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long nt = (long long)G.ne * G.ny * G.nz;
+    double mx = 0.0;
     bool nan = false;
-    long long t1 = L.nxy * k1;
-    for (long long t = L.nxy * k0 + blockIdx.x * (long long)blockDim.x + threadIdx.x; t < t1; t += (long long)gridDim.x * blockDim.x) {
-        double x = fabs(residual_at(L, phi, rhs, t));
-        nan |= (x != x);
-        m = fmax(m, x);
+    if (t < nt) {
+        int m = (int)(t % G.ne), j = (int)((t / G.ne) % G.ny), k = (int)(t / ((long long)G.ne * G.ny));
+        const long long row = G.plane * k + (long long)G.pitch * j;
+        for (int par = 0; par < 2; ++par) {
+            if (2 * m + par >= G.nx) break;
+            long long c, xm;
+            pair_addr(G, row, m, par, c, xm);
+            double x = fabs(residual_at(L, phi, rhs, c, xm));
+            nan |= (x != x);
+            mx = fmax(mx, x);
+        }
     }
-    if (nan) m = __longlong_as_double(0x7ff8000000000000ll);
-    block_max_to_global(m, out);
+    if (nan) mx = __longlong_as_double(0x7ff8000000000000ll);
+    block_max_to_global(mx, out);
 }
 
 }  // namespace vmg

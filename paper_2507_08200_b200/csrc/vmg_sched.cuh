@@ -16,7 +16,7 @@ inline LevelView view(const VmgLevel& L)
 {
     LevelView v;
     v.wx = L.wx; v.wy = L.wy; v.wz = L.wz; v.dinv = L.dinv;
-    v.nx = L.nx; v.ny = L.ny; v.nz = L.nz; v.nxy = (long long)L.nx * L.ny; v.n = L.n;
+    v.G = L.G;
     return v;
 }
 
@@ -66,7 +66,8 @@ inline void prof_collect(vmg_s* h)
     (void)cudaGetLastError();
 }
 
-inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt)
+// bt: the level-0 internal array, or (bt_natural) a caller array in the public layout
+inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt, bool bt_natural = false)
 {
     VmgLevel& L = h->lev[0];
     FoldArgs g;
@@ -76,7 +77,7 @@ inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt)
         g.val[f] = h->bc_has_value[f] ? h->bcval[f] : nullptr;
         g.dirichlet[f] = h->bctype[f] == VMG_BC_DIRICHLET;
     }
-    g.nx = L.nx; g.ny = L.ny; g.nz = L.nz; g.three_d = h->three_d;
+    g.G = L.G; g.three_d = h->three_d; g.bt_natural = bt_natural;
     g.h[0] = L.hx; g.h[1] = L.hy; g.h[2] = L.hz;
     {
         ProfScope ps(h, VMG_PC_FOLD, nullptr);
@@ -94,11 +95,11 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
 {
     VmgLevel& L = h->lev[l];
     LevelView v = view(L);
-    long long nt = (long long)((L.nx + 1) / 2) * L.ny * L.nz;
+    long long nt = (long long)L.G.ne * L.ny * L.nz;
     for (int s = 0; s < nsweeps; ++s)
         for (int colour = 0; colour < 2; ++colour) {
             if (2 * s + colour < skip_first) continue;
-            smooth_colour_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(v, cur_phi(L), L.rhs, colour, 0, L.nz);
+            smooth_colour_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(v, cur_phi(L), L.rhs, colour);
             ++*count;
         }
 }
@@ -108,25 +109,25 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
     VmgLevel& L = h->lev[l];
     VmgLevel& C = h->lev[l + 1];
     C.cur = 0;
-    residual_restrict_kernel<<<grid_for(C.n), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, C.rhs, C.phi,
-                                                                       h->three_d ? 2 : 1, 0, C.nz);
+    residual_restrict_kernel<<<grid_for(C.n), kThreads, 0, h->stream>>>(view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
+                                                                       h->three_d ? 2 : 1);
     ++*count;
 }
 
 inline void plain_prolong_correct(vmg_s* h, int l, long long* count)
 {
     VmgLevel& L = h->lev[l];
-    prolong_correct_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(cur_phi(L), cur_phi(h->lev[l + 1]), L.nx, L.ny,
-                                                                     h->three_d ? 2 : 1, 0, L.nz);
+    prolong_correct_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(L.G, h->lev[l + 1].G, cur_phi(L), cur_phi(h->lev[l + 1]),
+                                                                     h->three_d ? 2 : 1);
     ++*count;
 }
 
 inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out)
 {
     VmgLevel& L = h->lev[0];
-    unsigned g = grid_for(L.n);   // one cell per thread: a grid-stride loop serialises 13 dependent loads + a division per cell
+    unsigned g = grid_for((long long)L.G.ne * L.ny * L.nz);   // one x-pair per thread
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    residual_norm_kernel<<<g, kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out, 0, L.nz);
+    residual_norm_kernel<<<g, kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -168,7 +169,7 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
         TailLevel& T = g.lev[l - first];
         L.cur = 0;
         T.wx = L.wx; T.wy = L.wy; T.wz = L.wz; T.dinv = L.dinv; T.phi = L.phi; T.rhs = L.rhs;
-        T.nx = L.nx; T.ny = L.ny; T.nz = L.nz; T.n = (int)L.n; T.nxy = L.nx * L.ny;
+        T.nx = L.nx; T.ny = L.ny; T.nz = L.nz; T.n = (int)L.n; T.nxy = L.nx * L.ny; T.G = L.G;
         T.zs = h->three_d ? T.nxy : 0;
         T.guard = tail_guard(h, L);
         T.off = off;
@@ -214,14 +215,14 @@ struct BlkKernel {
     }
     static void launch(vmg_s* h, BlockArgs g)
     {
-        g.ntx = (int)cdiv(g.nx, C::TX); g.nty = (int)cdiv(g.ny, C::TY);
+        g.ntx = (int)cdiv(g.G.nx, C::TX); g.nty = (int)cdiv(g.G.ny, C::TY);
         // z-segments per tile: minimise waves x (planes per CTA incl. the 2H halo planes each segment pays)
         const long long ntiles = (long long)g.ntx * g.nty;
         int best = 1;
         double best_cost = 1e300;
-        for (int ns = 1; ns <= std::max(1, g.nz / 4); ++ns) {
+        for (int ns = 1; ns <= std::max(1, g.G.nz / 4); ++ns) {
             double waves = (double)cdiv(ntiles * ns, h->num_sms);
-            double cost = waves * ((double)cdiv(g.nz / 2, ns) * 2 + 2 * C::H + 2);
+            double cost = waves * ((double)cdiv(g.G.nz / 2, ns) * 2 + 2 * C::H + 2);
             if (cost < best_cost) { best_cost = cost; best = ns; }
         }
         g.nzseg = best;
@@ -277,13 +278,13 @@ inline void blocked_sweeps(vmg_s* h, int l, int nhalf, int colour0, bool prolong
         BlockArgs g{};
         g.wx = L.wx; g.wy = L.wy; g.wz = L.wz; g.dinv = L.dinv; g.rhs = L.rhs;
         g.phi_in = cur_phi(L); g.phi_out = other_phi(L);
-        g.nx = L.nx; g.ny = L.ny; g.nz = L.nz; g.nxy = (long long)L.nx * L.ny;
+        g.G = L.G;
         g.colour0 = (colour0 + done) & 1;
         bool first = p == 0, last = p == passes - 1;
         int T = last ? tail : BT_NONE;
         if ((first && prolong) || T == BT_RESTRICT) {
             VmgLevel& C = h->lev[l + 1];
-            g.cnx = C.nx; g.cny = C.ny;
+            g.CG = C.G;
             if (first && prolong) g.e = cur_phi(C);
             if (T == BT_RESTRICT) { C.cur = 0; g.crhs = C.rhs; g.cphi = C.phi; }
         }
@@ -300,7 +301,7 @@ inline void settle_phi(vmg_s* h, int l)
 {
     VmgLevel& L = h->lev[l];
     if (L.cur == 0) return;
-    cudaMemcpyAsync(L.phi, L.phi2, L.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream);
+    cudaMemcpyAsync(L.phi, L.phi2, L.nalloc * sizeof(double), cudaMemcpyDeviceToDevice, h->stream);
     L.cur = 0;
 }
 
@@ -346,9 +347,9 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
     if (h->nu2 >= 1) {   // the correction rides on the first half-sweep (smooth_colour_prolong_kernel)
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         VmgLevel& L = h->lev[l];
-        long long nt = (long long)((L.nx + 1) / 2) * L.ny * L.nz;
-        smooth_colour_prolong_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, cur_phi(h->lev[l + 1]), 0,
-                                                                              h->three_d ? 2 : 1);
+        long long nt = (long long)L.G.ne * L.ny * L.nz;
+        smooth_colour_prolong_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
+                                                                              cur_phi(h->lev[l + 1]), 0, h->three_d ? 2 : 1);
         ++*count;
         plain_smooth(h, l, h->nu2, count, 1);
         return false;
@@ -375,7 +376,7 @@ inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* co
         norm_done = h->tail_level == 0 && norm_out;
     } else {
         VmgLevel& B = h->lev[last];
-        if (last == 0) cudaMemsetAsync(B.phi, 0, B.n * sizeof(double), h->stream);   // single level: bottom from zero
+        if (last == 0) cudaMemsetAsync(B.phi, 0, B.nalloc * sizeof(double), h->stream);   // single level: bottom from zero
         ProfScope ps(h, VMG_PC_COARSE, count);
         plain_smooth(h, last, h->nbottom, count);
     }

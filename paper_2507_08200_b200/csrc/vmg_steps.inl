@@ -3,9 +3,18 @@
 
 namespace {
 
-int stage_in(vmg_s* h, double* dst, const double* src, long long n)
+// caller array (public layout) -> level array (internal layout) and back
+int stage_in(vmg_s* h, const VmgLevel& L, double* dst, const double* src)
 {
-    CUDA_TRY(h, cudaMemcpyAsync(dst, src, n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    to_internal_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(L.G, src, dst);
+    CUDA_TRY(h, cudaGetLastError());
+    return VMG_OK;
+}
+
+int stage_out(vmg_s* h, const VmgLevel& L, double* dst, const double* src)
+{
+    to_natural_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(L.G, src, dst);
+    CUDA_TRY(h, cudaGetLastError());
     return VMG_OK;
 }
 
@@ -48,7 +57,7 @@ int vmg_step_fold_bc(vmg_handle h, const double* rhs, double* btilde)
     if (!rhs || !btilde) return VMG_ERR_ARG;
     int rc = ready(h);
     if (rc != VMG_OK) return rc;
-    rc = enqueue_fold_bc(h, rhs, btilde);
+    rc = enqueue_fold_bc(h, rhs, btilde, true);
     if (rc != VMG_OK) return rc;
     return finish(h);
 }
@@ -59,12 +68,12 @@ int vmg_step_smooth(vmg_handle h, int level, double* phi, const double* rhs, int
     int rc = ready(h);
     if (rc != VMG_OK) return rc;
     VmgLevel& L = h->lev[level];
-    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.phi, phi)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.rhs, rhs)) != VMG_OK) return rc;
     long long count = 0;
     prepare_blocked(h);
     enqueue_smooth(h, level, nsweeps, &count);
-    if ((rc = stage_in(h, phi, L.phi, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_out(h, L, phi, L.phi)) != VMG_OK) return rc;
     return finish(h);
 }
 
@@ -74,8 +83,8 @@ int vmg_step_residual(vmg_handle h, int level, const double* phi, const double* 
     int rc = ready(h);
     if (rc != VMG_OK) return rc;
     VmgLevel& L = h->lev[level];
-    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.phi, phi)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.rhs, rhs)) != VMG_OK) return rc;
     residual_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(view(L), L.phi, L.rhs, r);
     return finish(h);
 }
@@ -86,12 +95,12 @@ int vmg_step_residual_restrict(vmg_handle h, int level, const double* phi, const
     int rc = ready(h);
     if (rc != VMG_OK) return rc;
     VmgLevel& L = h->lev[level];
-    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.phi, phi)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.rhs, rhs)) != VMG_OK) return rc;
     long long count = 0;
     L.cur = 0;
     plain_residual_restrict(h, level, &count);
-    if ((rc = stage_in(h, rhs_coarse, h->lev[level + 1].rhs, h->lev[level + 1].n)) != VMG_OK) return rc;
+    if ((rc = stage_out(h, h->lev[level + 1], rhs_coarse, h->lev[level + 1].rhs)) != VMG_OK) return rc;
     return finish(h);
 }
 
@@ -100,12 +109,12 @@ int vmg_step_prolong_correct(vmg_handle h, int level, double* phi, const double*
     if (bad_level(h, level) || level + 1 >= h->nlev || !phi || !e_coarse) return VMG_ERR_ARG;
     VmgLevel& L = h->lev[level];
     int rc;
-    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, h->lev[level + 1].phi, e_coarse, h->lev[level + 1].n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.phi, phi)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, h->lev[level + 1], h->lev[level + 1].phi, e_coarse)) != VMG_OK) return rc;
     long long count = 0;
     L.cur = 0; h->lev[level + 1].cur = 0;
     plain_prolong_correct(h, level, &count);
-    if ((rc = stage_in(h, phi, L.phi, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_out(h, L, phi, L.phi)) != VMG_OK) return rc;
     return finish(h);
 }
 
@@ -116,14 +125,14 @@ int vmg_step_down(vmg_handle h, int level, double* phi, const double* rhs, doubl
     if (rc != VMG_OK) return rc;
     VmgLevel& L = h->lev[level];
     VmgLevel& C = h->lev[level + 1];
-    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.phi, phi)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.rhs, rhs)) != VMG_OK) return rc;
     prepare_blocked(h);
     long long count = 0;
     L.cur = 0;
     enqueue_down(h, level, &count);
-    if ((rc = stage_in(h, phi, cur_phi(L), L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, rhs_coarse, C.rhs, C.n)) != VMG_OK) return rc;
+    if ((rc = stage_out(h, L, phi, cur_phi(L))) != VMG_OK) return rc;
+    if ((rc = stage_out(h, C, rhs_coarse, C.rhs)) != VMG_OK) return rc;
     L.cur = 0;
     return finish(h);
 }
@@ -135,14 +144,14 @@ int vmg_step_up(vmg_handle h, int level, double* phi, const double* rhs, const d
     if (rc != VMG_OK) return rc;
     VmgLevel& L = h->lev[level];
     VmgLevel& C = h->lev[level + 1];
-    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, L.rhs, rhs, L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, C.phi, e_coarse, C.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.phi, phi)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.rhs, rhs)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, C, C.phi, e_coarse)) != VMG_OK) return rc;
     prepare_blocked(h);
     long long count = 0;
     L.cur = 0; C.cur = 0;
     enqueue_up(h, level, nullptr, &count);
-    if ((rc = stage_in(h, phi, cur_phi(L), L.n)) != VMG_OK) return rc;
+    if ((rc = stage_out(h, L, phi, cur_phi(L))) != VMG_OK) return rc;
     L.cur = 0;
     return finish(h);
 }
@@ -153,12 +162,12 @@ int vmg_step_vcycle(vmg_handle h, double* phi, const double* btilde)
     int rc = ready(h);
     if (rc != VMG_OK) return rc;
     VmgLevel& L = h->lev[0];
-    if ((rc = stage_in(h, L.phi, phi, L.n)) != VMG_OK) return rc;
-    if ((rc = stage_in(h, L.rhs, btilde, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.phi, phi)) != VMG_OK) return rc;
+    if ((rc = stage_in(h, L, L.rhs, btilde)) != VMG_OK) return rc;
     h->launches = 0;
     rc = run_vcycle_with_norm(h, (unsigned long long*)h->d_scal + 1);
     if (rc != VMG_OK) return rc;
-    if ((rc = stage_in(h, phi, L.phi, L.n)) != VMG_OK) return rc;
+    if ((rc = stage_out(h, L, phi, L.phi)) != VMG_OK) return rc;
     return finish(h);
 }
 

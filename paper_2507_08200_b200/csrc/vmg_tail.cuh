@@ -16,6 +16,7 @@ struct TailLevel {
     const double *wx, *wy, *wz, *dinv;   // global, internal stencil form (cell 0)
     double *phi, *rhs;                   // global level arrays (cell 0)
     int nx, ny, nz, n, nxy, guard, off;  // off: offset (doubles) of this level's block in shared memory
+    Geom G;                              // layout of the global arrays (shared memory uses the natural layout)
     int zs;                              // stride to the z neighbours: nxy in 3-D, 0 in 2-D (their weight is zero)
 };
 
@@ -93,8 +94,9 @@ __global__ void __launch_bounds__(kTailThreads, 1) coarse_tail_kernel(TailArgs g
         const TailLevel& L = g.lev[l];
         TailSmem s(tail_smem, L);
         for (int t = tid; t < L.n; t += nth) {
-            s.dinv[t] = L.dinv[t]; s.wx[t] = L.wx[t]; s.wy[t] = L.wy[t]; s.wz[t] = L.wz[t];
-            if (l == 0) { s.rhs[t] = L.rhs[t]; if (g.whole) s.phi[t] = L.phi[t]; }
+            const long long c = cell_at(L.G, t % L.nx, (t / L.nx) % L.ny, t / L.nxy);
+            s.dinv[t] = L.dinv[c]; s.wx[t] = L.wx[c]; s.wy[t] = L.wy[c]; s.wz[t] = L.wz[c];
+            if (l == 0) { s.rhs[t] = L.rhs[c]; if (g.whole) s.phi[t] = L.phi[c]; }
         }
     }
     __syncthreads();
@@ -147,7 +149,7 @@ __global__ void __launch_bounds__(kTailThreads, 1) coarse_tail_kernel(TailArgs g
         double m = 0.0;
         bool nan = false;
         for (int t = tid; t < L.n; t += nth) {
-            L.phi[t] = s.phi[t];
+            L.phi[cell_at(L.G, t % L.nx, (t / L.nx) % L.ny, t / L.nxy)] = s.phi[t];
             if (g.whole && g.norm_out) {
                 double x = fabs(tail_residual_at(s, L, t));
                 nan |= (x != x);
