@@ -59,6 +59,7 @@ struct vmg_s {
     int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200
     int use_tail = 1;             // run the coarsest levels in one CTA (vmg_tail.cuh)
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
+    int cluster_level = -1;       // unused (-1)
     size_t tail_smem = 0;         // dynamic shared memory of the tail kernel
     long long block_min_cells = 4096;   // smallest level the blocked smoother is used on
     // device scalars

@@ -38,10 +38,18 @@ __host__ __device__ __forceinline__ long long cell_at(const Geom& G, int i, int 
 {
     return G.plane * k + (long long)G.pitch * j + (i & 1) * (G.ne + 1) + (i >> 1);
 }
-// natural cell number t = i + nx*(j + ny*k) -> (i, j, k)
+// natural cell number t = i + nx*(j + ny*k) -> (i, j, k).  32-bit arithmetic: vmg_create caps n below 2^31, and a
+// 64-bit division is ~100 dependent instructions, which the latency-bound coarse levels cannot hide.
 __device__ __forceinline__ void unflatten(const Geom& G, long long t, int& i, int& j, int& k)
 {
-    i = (int)(t % G.nx); j = (int)((t / G.nx) % G.ny); k = (int)(t / ((long long)G.nx * G.ny));
+    const unsigned u = (unsigned)t, q = u / (unsigned)G.nx;
+    i = (int)(u - q * (unsigned)G.nx); k = (int)(q / (unsigned)G.ny); j = (int)(q - (unsigned)k * (unsigned)G.ny);
+}
+// pair number t = m + ne*(j + ny*k) -> (m, j, k)
+__device__ __forceinline__ void unflatten_pair(const Geom& G, long long t, int& m, int& j, int& k)
+{
+    const unsigned u = (unsigned)t, q = u / (unsigned)G.ne;
+    m = (int)(u - q * (unsigned)G.ne); k = (int)(q / (unsigned)G.ny); j = (int)(q - (unsigned)k * (unsigned)G.ny);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -230,7 +238,7 @@ struct LevelView {
 
 // c: the cell; xm: its low-x neighbour (the high-x neighbour is xm + 1: E_m sits between O_{m-1} and O_m, O_m between
 // E_m and E_{m+1}).  Same expression, same order, everywhere a relaxation or a residual is evaluated.
-__device__ __forceinline__ double nb_sum(const LevelView& L, const double* __restrict__ phi, long long c, long long xm)
+__device__ __forceinline__ double nb_sum(const LevelView& L, const double* phi, long long c, long long xm)
 {
     double s = L.wx[c] * phi[xm];
     s = fma(L.wx[xm + 1], phi[xm + 1], s);
@@ -249,18 +257,25 @@ __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, i
 }
 
 // S2 (per-colour path). One colour half-sweep: phi_c <- (rhs_c + sum w phi_nb) / D_c for (i+j+k)%2 == colour.
-__global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour)
+// t: index of the x-pair (m, j, k), t < ne*ny*nz.  The *_one functions take plain pointers: the cluster tail calls
+// them on arrays that other CTAs of the same launch have just written (no non-coherent loads there).
+__device__ __forceinline__ void relax_one(const LevelView& L, double* phi, const double* rhs, int colour,
+                                          long long t)
 {
     const Geom& G = L.G;
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long nt = (long long)G.ne * G.ny * G.nz;
-    if (t >= nt) return;
-    int m = (int)(t % G.ne), j = (int)((t / G.ne) % G.ny), k = (int)(t / ((long long)G.ne * G.ny));
+    int m, j, k;
+    unflatten_pair(G, t, m, j, k);
     int par = (colour + j + k) & 1;
     if (2 * m + par >= G.nx) return;
     long long c, xm;
     pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
     phi[c] = L.dinv[c] * (rhs[c] + nb_sum(L, phi, c, xm));
+}
+
+__global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour)
+{
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < (long long)L.G.ne * L.G.ny * L.G.nz) relax_one(L, phi, rhs, colour, t);
 }
 
 // S4 + S2 fused (per-colour path).  The first colour half-sweep after a coarse-grid correction: a relaxation never
@@ -269,14 +284,13 @@ __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, cons
 // stored: the cells of the other colour keep their uncorrected values in memory until the next half-sweep
 // overwrites them.  Valid when at least one full sweep follows (nu2 >= 1).  phi_nb + e is the very addition
 // prolong_correct_kernel performs, so results are bitwise those of the two separate kernels.
-__global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __restrict__ phi, const double* __restrict__ rhs,
-                                             const double* __restrict__ e, int colour, int sz)
+__device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom& CG, double* phi,
+                                                  const double* rhs, const double* e, int colour, int sz,
+                                                  long long t)
 {
     const Geom& G = L.G;
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long nt = (long long)G.ne * G.ny * G.nz;
-    if (t >= nt) return;
-    int m = (int)(t % G.ne), j = (int)((t / G.ne) % G.ny), k = (int)(t / ((long long)G.ne * G.ny));
+    int m, j, k;
+    unflatten_pair(G, t, m, j, k);
     int par = (colour + j + k) & 1;
     int i = 2 * m + par;
     if (i >= G.nx) return;
@@ -302,9 +316,15 @@ __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __res
     phi[c] = L.dinv[c] * (rhs[c] + s);
 }
 
+__global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __restrict__ phi, const double* __restrict__ rhs,
+                                             const double* __restrict__ e, int colour, int sz)
+{
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < (long long)L.G.ne * L.G.ny * L.G.nz) relax_prolong_one(L, CG, phi, rhs, e, colour, sz, t);
+}
+
 // r = rhs - A phi, A phi = D phi - sum w phi_nb, D = 1/dinv.
-__device__ __forceinline__ double residual_at(const LevelView& L, const double* __restrict__ phi,
-                                              const double* __restrict__ rhs, long long c, long long xm)
+__device__ __forceinline__ double residual_at(const LevelView& L, const double* phi, const double* rhs, long long c, long long xm)
 {
     return rhs[c] + nb_sum(L, phi, c, xm) - phi[c] / L.dinv[c];
 }
@@ -323,11 +343,12 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 }
 
 // S3 (per-colour path). Fused residual + restriction: one thread per coarse cell; also zeroes the coarse phi.
-__global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz)
+// (Four lanes per coarse cell with a shuffle gather was tried: 70 us instead of 49 us on 256x128x128, the 64-byte
+// runs per row coalesce worse than they gain in occupancy.)
+__device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG, const double* phi,
+                                             const double* rhs, double* crhs, double* cphi,
+                                             int sz, long long t)
 {
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (t >= CG.n) return;
     int I, J, K;
     unflatten(CG, t, I, J, K);
     double s = 0.0;
@@ -343,15 +364,27 @@ __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __r
     if (cphi) cphi[cc] = 0.0;
 }
 
-// S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise
-// constant, R9): phi_f += e_c[i/2, j/2, k/2].
-__global__ void prolong_correct_kernel(Geom G, Geom CG, double* __restrict__ phi, const double* __restrict__ e, int sz)
+__global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
+                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (t >= G.n) return;
+    if (t < CG.n) restrict_one(L, CG, phi, rhs, crhs, cphi, sz, t);
+}
+
+// S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise
+// constant, R9): phi_f += e_c[i/2, j/2, k/2].
+__device__ __forceinline__ void prolong_one(const Geom& G, const Geom& CG, double* phi, const double* e,
+                                            int sz, long long t)
+{
     int i, j, k;
     unflatten(G, t, i, j, k);
     phi[cell_at(G, i, j, k)] += e[cell_at(CG, i >> 1, j >> 1, sz == 2 ? (k >> 1) : k)];
+}
+
+__global__ void prolong_correct_kernel(Geom G, Geom CG, double* __restrict__ phi, const double* __restrict__ e, int sz)
+{
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < G.n) prolong_one(G, CG, phi, e, sz, t);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -395,7 +428,8 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
     block_max_to_global(m, out);
 }
 
-// ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one thread per x-pair
+// ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one cell per thread, blockIdx.y =
+// colour (like two colour half-sweeps in one launch: 13 loads and a division per thread at full occupancy)
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
                                      unsigned long long* out)
 {
@@ -403,20 +437,17 @@ __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     long long nt = (long long)G.ne * G.ny * G.nz;
     double mx = 0.0;
-    bool nan = false;
     if (t < nt) {
-        int m = (int)(t % G.ne), j = (int)((t / G.ne) % G.ny), k = (int)(t / ((long long)G.ne * G.ny));
-        const long long row = G.plane * k + (long long)G.pitch * j;
-        for (int par = 0; par < 2; ++par) {
-            if (2 * m + par >= G.nx) break;
+        int m, j, k;
+    unflatten_pair(G, t, m, j, k);
+        int par = ((int)blockIdx.y + j + k) & 1;
+        if (2 * m + par < G.nx) {
             long long c, xm;
-            pair_addr(G, row, m, par, c, xm);
-            double x = fabs(residual_at(L, phi, rhs, c, xm));
-            nan |= (x != x);
-            mx = fmax(mx, x);
+            pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
+            mx = fabs(residual_at(L, phi, rhs, c, xm));
+            if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
         }
     }
-    if (nan) mx = __longlong_as_double(0x7ff8000000000000ll);
     block_max_to_global(mx, out);
 }
 

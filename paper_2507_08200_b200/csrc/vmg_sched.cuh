@@ -9,6 +9,7 @@
 #include "vmg_block2.cuh"
 #include "../../include/vmg.h"
 #include <algorithm>
+#include <cstring>
 
 namespace vmg {
 
@@ -127,7 +128,7 @@ inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out)
     VmgLevel& L = h->lev[0];
     unsigned g = grid_for((long long)L.G.ne * L.ny * L.nz);   // one x-pair per thread
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    residual_norm_kernel<<<g, kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out);
+    residual_norm_kernel<<<dim3(g, 2), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -140,6 +141,7 @@ inline int tail_guard(const vmg_s* h, const VmgLevel& L) { return (h->three_d ? 
 inline void plan_schedule(vmg_s* h)
 {
     h->tail_level = -1;
+    h->cluster_level = -1;
     h->tail_smem = 0;
     if (!h->use_tail) return;
     size_t doubles = 0;
@@ -162,8 +164,10 @@ inline void plan_schedule(vmg_s* h)
 inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* count)
 {
     TailArgs g;
-    int first = h->tail_level, off = 0;
+    const int tail = h->tail_level, first = h->cluster_level >= 0 ? h->cluster_level : tail;
+    int off = 0;
     g.nl = h->nlev - first;
+    g.ns = tail - first;
     for (int l = first; l < h->nlev; ++l) {
         VmgLevel& L = h->lev[l];
         TailLevel& T = g.lev[l - first];
@@ -173,14 +177,16 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
         T.zs = h->three_d ? T.nxy : 0;
         T.guard = tail_guard(h, L);
         T.off = off;
-        off += tail_level_doubles(T.n, T.guard);
+        if (l >= tail) off += tail_level_doubles(T.n, T.guard);
     }
     g.nu1 = h->nu1; g.nu2 = h->nu2; g.nbottom = h->nbottom; g.sz = h->three_d ? 2 : 1;
     g.whole = first == 0;
     g.norm_out = first == 0 ? norm_out : nullptr;
-    int threads = (int)std::min<long long>(kTailThreads, std::max<long long>(64, (h->lev[first].n / 2 + 31) / 32 * 32));
     ProfScope ps(h, VMG_PC_COARSE, count);
-    coarse_tail_kernel<<<1, threads, h->tail_smem, h->stream>>>(g);
+    {
+        int threads = (int)std::min<long long>(kTailThreads, std::max<long long>(64, (h->lev[first].n / 2 + 31) / 32 * 32));
+        coarse_tail_kernel<<<1, threads, h->tail_smem, h->stream>>>(g);
+    }
     ++*count;
 }
 
@@ -366,7 +372,8 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
 inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* count)
 {
     const int last = h->nlev - 1;
-    const int tail = h->tail_level >= 0 ? h->tail_level : last;   // first level not handled stroke by stroke
+    // first level not handled stroke by stroke
+    const int tail = h->tail_level < 0 ? last : h->cluster_level >= 0 ? h->cluster_level : h->tail_level;
     if (norm_out) cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
     for (int l = 0; l <= last; ++l) h->lev[l].cur = 0;
     for (int l = 0; l < tail; ++l) enqueue_down(h, l, count);
