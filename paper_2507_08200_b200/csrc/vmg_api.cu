@@ -93,10 +93,43 @@ bool singular(const vmg_s* h)
     return h->alpha == 0.0;
 }
 
+// Set part of L2 aside for the level-0 face weights (wx, wy, wz: contiguous in the arena), which every half-sweep
+// re-reads: an access-policy window on the handle's stream (inherited by the captured graph nodes), hit ratio =
+// set-aside / window so that the lines kept do not thrash among themselves.  Measured on 256x128x128 (B200, 126 MB
+// L2): 24 MB is the optimum (-13 % on the level-0 smoother); larger carve-outs take more from the reuse
+// between consecutive half-sweeps than they give.  Only when the weights do not fit L2 anyway.
+int apply_l2_window(vmg_s* h)
+{
+    h->l2_applied = true;
+    VmgLevel& L = h->lev[0];
+    cudaDeviceProp prop;
+    CUDA_TRY(h, cudaGetDeviceProperties(&prop, h->device));
+    size_t bytes = 3 * ((size_t)L.nalloc + 2 * (size_t)L.pad) * sizeof(double);
+    size_t want = (size_t)(h->l2_persist_mb * 1048576.0), cap = (size_t)prop.persistingL2CacheMaxSize;
+    if (bytes < (size_t)prop.l2CacheSize / 2) want = 0;
+    if (want > cap) want = cap;
+    if (want == 0 && !h->l2_window_set) return VMG_OK;
+    if (want) CUDA_TRY(h, cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));
+    cudaStreamAttrValue a;
+    memset(&a, 0, sizeof(a));
+    if (bytes > (size_t)prop.accessPolicyMaxWindowSize) bytes = (size_t)prop.accessPolicyMaxWindowSize;
+    a.accessPolicyWindow.base_ptr = (void*)(L.wx - L.pad);
+    a.accessPolicyWindow.num_bytes = want ? bytes : 0;
+    a.accessPolicyWindow.hitRatio = want ? (float)std::min(1.0, (double)want / (double)bytes) : 0.f;
+    a.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    a.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    CUDA_TRY(h, cudaStreamSetAttribute(h->stream, cudaStreamAttributeAccessPolicyWindow, &a));
+    if (!want) CUDA_TRY(h, cudaCtxResetPersistingL2Cache());
+    h->l2_window_set = want != 0;
+    h->graph_valid = false;
+    return VMG_OK;
+}
+
 int ready(vmg_s* h)
 {
     if (!h) return VMG_ERR_ARG;
     if (!h->have_coeffs || !h->have_bc) return VMG_ERR_STATE;
+    if (!h->l2_applied) { int rc = apply_l2_window(h); if (rc != VMG_OK) return rc; }
     if (h->dinv_dirty) return finalize_dinv(h);
     return VMG_OK;
 }
@@ -274,7 +307,9 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
     else if (!strcmp(key, "blocked")) { h->use_blocked = iv != 0; }
     else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }
+    else if (!strcmp(key, "snake")) { h->snake = iv != 0; }
     else if (!strcmp(key, "block_min_cells")) { if (v < 0) return VMG_ERR_ARG; h->block_min_cells = (long long)v; }
+    else if (!strcmp(key, "l2_persist")) { if (v < 0) return VMG_ERR_ARG; h->l2_persist_mb = v; h->l2_applied = false; }
     else if (!strcmp(key, "profile")) {
         h->profile = iv != 0;
         for (int c = 0; c < VMG_PC_COUNT; ++c) { h->prof_ms[c] = 0.0; h->prof_launches[c] = 0; }

@@ -35,6 +35,7 @@ struct VmgLevel {
     double *wx = nullptr, *wy = nullptr, *wz = nullptr, *dinv = nullptr, *dbase = nullptr;
     double *phi = nullptr, *rhs = nullptr;
     double *phi2 = nullptr;   // second phi buffer: passes of the blocked smoother ping-pong (tiles overlap)
+    int dir = 0;              // direction of the next whole-level kernel (see next_dir)
     int cur = 0;              // which buffer holds phi while a V-cycle is being enqueued (0: phi, 1: phi2)
     // boundary-face weight planes, order XLO..ZHI (unpadded)
     double* wb[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -57,6 +58,9 @@ struct vmg_s {
     bool have_coeffs = false, have_bc = false, dinv_dirty = true;
     int nu1 = 3, nu2 = 3, nbottom = 32;
     int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200
+    double l2_persist_mb = 24.0;  // L2 set aside for the level-0 face weights (0: none); see apply_l2_window
+    bool l2_applied = false, l2_window_set = false;
+    int snake = 1;                // consecutive half-sweeps walk the level in opposite directions (L2 reuse)
     int use_tail = 1;             // run the coarsest levels in one CTA (vmg_tail.cuh)
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
     int cluster_level = -1;       // unused (-1)

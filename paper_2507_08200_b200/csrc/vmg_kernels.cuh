@@ -259,8 +259,10 @@ __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, i
 // S2 (per-colour path). One colour half-sweep: phi_c <- (rhs_c + sum w phi_nb) / D_c for (i+j+k)%2 == colour.
 // t: index of the x-pair (m, j, k), t < ne*ny*nz.  The *_one functions take plain pointers: the cluster tail calls
 // them on arrays that other CTAs of the same launch have just written (no non-coherent loads there).
-__device__ __forceinline__ void relax_one(const LevelView& L, double* phi, const double* rhs, int colour,
-                                          long long t)
+// L2 residency: what the NEXT half-sweep (other colour, opposite direction) needs again are the face weights and the
+// phi written here; rhs, 1/D and the neighbours' phi are dead after this read, so they are loaded with the streaming
+// (evict-first) policy and do not push the weights out of the 126 MB L2.
+__device__ __forceinline__ void relax_one(const LevelView& L, double* phi, const double* rhs, int colour, long long t)
 {
     const Geom& G = L.G;
     int m, j, k;
@@ -269,13 +271,24 @@ __device__ __forceinline__ void relax_one(const LevelView& L, double* phi, const
     if (2 * m + par >= G.nx) return;
     long long c, xm;
     pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
-    phi[c] = L.dinv[c] * (rhs[c] + nb_sum(L, phi, c, xm));
+    double s = L.wx[c] * __ldcs(phi + xm);
+    s = fma(L.wx[xm + 1], __ldcs(phi + xm + 1), s);
+    s = fma(L.wy[c], __ldcs(phi + c - G.pitch), s);
+    s = fma(L.wy[c + G.pitch], __ldcs(phi + c + G.pitch), s);
+    s = fma(L.wz[c], __ldcs(phi + c - G.plane), s);
+    s = fma(L.wz[c + G.plane], __ldcs(phi + c + G.plane), s);
+    phi[c] = __ldcs(L.dinv + c) * (__ldcs(rhs + c) + s);
 }
 
-__global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour)
+// reverse: walk the level from its last plane to its first.  Consecutive half-sweeps alternate direction, so that
+// each one starts on the planes the previous one touched last, which are still in the 126 MB L2 (face weights and
+// the phi just written are common to both colours).
+__global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour, int reverse)
 {
+    const long long nt = (long long)L.G.ne * L.G.ny * L.G.nz;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (t < (long long)L.G.ne * L.G.ny * L.G.nz) relax_one(L, phi, rhs, colour, t);
+    if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
+    if (t < nt) relax_one(L, phi, rhs, colour, t);
 }
 
 // S4 + S2 fused (per-colour path).  The first colour half-sweep after a coarse-grid correction: a relaxation never
@@ -317,9 +330,10 @@ __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom
 }
 
 __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __restrict__ phi, const double* __restrict__ rhs,
-                                             const double* __restrict__ e, int colour, int sz)
+                                             const double* __restrict__ e, int colour, int sz, int reverse)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
     if (t < (long long)L.G.ne * L.G.ny * L.G.nz) relax_prolong_one(L, CG, phi, rhs, e, colour, sz, t);
 }
 
@@ -365,9 +379,10 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
 }
 
 __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz)
+                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
     if (t < CG.n) restrict_one(L, CG, phi, rhs, crhs, cphi, sz, t);
 }
 
@@ -431,10 +446,11 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
 // ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one cell per thread, blockIdx.y =
 // colour (like two colour half-sweeps in one launch: 13 loads and a division per thread at full occupancy)
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                     unsigned long long* out)
+                                     unsigned long long* out, int reverse)
 {
     const Geom& G = L.G;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
     long long nt = (long long)G.ne * G.ny * G.nz;
     double mx = 0.0;
     if (t < nt) {

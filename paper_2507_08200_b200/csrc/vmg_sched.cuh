@@ -23,6 +23,9 @@ inline LevelView view(const VmgLevel& L)
 
 inline unsigned grid_for(long long n) { return (unsigned)cdiv(n, kThreads); }
 
+// direction of the next whole-level kernel: consecutive kernels walk the level in opposite directions (L2 reuse)
+inline int next_dir(vmg_s* h, VmgLevel& L) { int d = h->snake ? L.dir : 0; L.dir ^= 1; return d; }
+
 inline double* cur_phi(VmgLevel& L) { return L.cur ? L.phi2 : L.phi; }
 inline double* other_phi(VmgLevel& L) { return L.cur ? L.phi : L.phi2; }
 
@@ -100,7 +103,7 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
     for (int s = 0; s < nsweeps; ++s)
         for (int colour = 0; colour < 2; ++colour) {
             if (2 * s + colour < skip_first) continue;
-            smooth_colour_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(v, cur_phi(L), L.rhs, colour);
+            smooth_colour_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(v, cur_phi(L), L.rhs, colour, next_dir(h, L));
             ++*count;
         }
 }
@@ -111,7 +114,7 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
     VmgLevel& C = h->lev[l + 1];
     C.cur = 0;
     residual_restrict_kernel<<<grid_for(C.n), kThreads, 0, h->stream>>>(view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
-                                                                       h->three_d ? 2 : 1);
+                                                                       h->three_d ? 2 : 1, next_dir(h, L));
     ++*count;
 }
 
@@ -128,7 +131,7 @@ inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out)
     VmgLevel& L = h->lev[0];
     unsigned g = grid_for((long long)L.G.ne * L.ny * L.nz);   // one x-pair per thread
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    residual_norm_kernel<<<dim3(g, 2), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out);
+    residual_norm_kernel<<<dim3(g, 2), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -355,7 +358,7 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         VmgLevel& L = h->lev[l];
         long long nt = (long long)L.G.ne * L.ny * L.nz;
         smooth_colour_prolong_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
-                                                                              cur_phi(h->lev[l + 1]), 0, h->three_d ? 2 : 1);
+                                                                              cur_phi(h->lev[l + 1]), 0, h->three_d ? 2 : 1, next_dir(h, L));
         ++*count;
         plain_smooth(h, l, h->nu2, count, 1);
         return false;
@@ -375,7 +378,7 @@ inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* co
     // first level not handled stroke by stroke
     const int tail = h->tail_level < 0 ? last : h->cluster_level >= 0 ? h->cluster_level : h->tail_level;
     if (norm_out) cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
-    for (int l = 0; l <= last; ++l) h->lev[l].cur = 0;
+    for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }
     for (int l = 0; l < tail; ++l) enqueue_down(h, l, count);
     bool norm_done = false;
     if (h->tail_level >= 0) {
