@@ -44,7 +44,7 @@ enum {
     VMG_MAXCYCLES = 1,       /* ran max_vcycles cycles without reaching rtol (always, when rtol <= 0)   */
     VMG_STALLED = 2,         /* residual reduced by less than 10 % in 3 consecutive cycles (fp64 floor) */
     VMG_ERR_ARG = -1,        /* NULL / out-of-range argument, unknown option key                        */
-    VMG_ERR_SIZE = -2,       /* grid cannot be coarsened to a bottom grid of <= 512 cells               */
+    VMG_ERR_SIZE = -2,       /* grid cannot be coarsened to a bottom grid of <= 512 cells, or >= 2^31 cells */
     VMG_ERR_STATE = -3,      /* vmg_solve before both vmg_set_coeffs and vmg_set_bc                     */
     VMG_ERR_SINGULAR = -4,   /* all active faces Neumann and (a == NULL or alpha == 0)                  */
     VMG_ERR_DIVERGED = -5,   /* residual became NaN or Inf                                              */
@@ -56,7 +56,7 @@ enum {
  * active dimension while all stay even and >= 2 afterwards (256x128x128 -> ... -> 4x2x2); the coarsest grid
  * must have <= 512 cells (VMG_ERR_SIZE otherwise).  cuda_stream is a cudaStream_t (NULL = legacy default
  * stream); every kernel, copy and graph of this handle is enqueued on it.  All device memory the handle
- * needs (about 9.2 fp64 arrays of nx*ny*nz) is allocated here; vmg_solve allocates nothing on the device. */
+ * needs (about 9.3 fp64 arrays of (nx+2)*ny*nz) is allocated here; vmg_solve allocates nothing on the device. */
 int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream);
 
 /* Coefficients.  a: cell array or NULL (a == 0, alpha ignored).  bx, by, bz: face arrays, or all NULL for
@@ -88,9 +88,15 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
 
 /* Options (key is a HOST C string): "nu1", "nu2" (pre/post red-black sweeps, default 3, 0..8),
  * "bottom_sweeps" (default 32), "graph" (1: replay the V-cycle as a CUDA graph, default; 0: plain launches),
- * "blocked" (1: temporally blocked smoother passes with fused transfers, default; 0: one kernel per step),
- * "block_min_cells" (smallest level the blocked smoother is used on, default 4096),
  * "tail" (1: the coarsest levels run in one single-CTA launch, default; 0: one kernel per step),
+ * "snake" (1: consecutive whole-level kernels walk the level in opposite z-directions so that each starts on
+ *   what the previous one left in L2, default; 0: always ascending),
+ * "l2_persist" (MB of L2 set aside for the level-0 face weights through a stream access-policy window,
+ *   default 24, 0 = none; applied only when those weights exceed half the L2.  NOTE: this calls
+ *   cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize), a setting of the whole CUDA context),
+ * "blocked" (1: temporally blocked smoother passes with fused transfers (vmg_block2.cuh); 0: one kernel per
+ *   colour half-sweep, default -- the blocked passes are bitwise equal but measure slower on B200),
+ * "block_min_cells" (smallest level the blocked passes are used on when blocked = 1, default 4096),
  * "profile" (1: per-kernel-class event timing, see vmg_get_profile; implies plain launches; default 0). */
 int vmg_set_option(vmg_handle h, const char* key, double v);
 
