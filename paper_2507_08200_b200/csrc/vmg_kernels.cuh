@@ -238,20 +238,14 @@ struct LevelView {
 
 // c: the cell; xm: its low-x neighbour (the high-x neighbour is xm + 1: E_m sits between O_{m-1} and O_m, O_m between
 // E_m and E_{m+1}).  Same expression, same order, everywhere a relaxation or a residual is evaluated.
-// CG: load phi around L1 (ld.global.cg): the wavefront kernel (vmg_wave.cuh) reads values that other CTAs of the
-// same launch have written, and L1 is not coherent across SMs.
-template <bool CG = false>
-__device__ __forceinline__ double ld_phi(const double* p) { return CG ? __ldcg(p) : *p; }
-
-template <bool CG = false>
 __device__ __forceinline__ double nb_sum(const LevelView& L, const double* phi, long long c, long long xm)
 {
-    double s = L.wx[c] * ld_phi<CG>(phi + xm);
-    s = fma(L.wx[xm + 1], ld_phi<CG>(phi + xm + 1), s);
-    s = fma(L.wy[c], ld_phi<CG>(phi + c - L.G.pitch), s);
-    s = fma(L.wy[c + L.G.pitch], ld_phi<CG>(phi + c + L.G.pitch), s);
-    s = fma(L.wz[c], ld_phi<CG>(phi + c - L.G.plane), s);
-    s = fma(L.wz[c + L.G.plane], ld_phi<CG>(phi + c + L.G.plane), s);
+    double s = L.wx[c] * phi[xm];
+    s = fma(L.wx[xm + 1], phi[xm + 1], s);
+    s = fma(L.wy[c], phi[c - L.G.pitch], s);
+    s = fma(L.wy[c + L.G.pitch], phi[c + L.G.pitch], s);
+    s = fma(L.wz[c], phi[c - L.G.plane], s);
+    s = fma(L.wz[c + L.G.plane], phi[c + L.G.plane], s);
     return s;
 }
 
@@ -303,7 +297,6 @@ __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, cons
 // stored: the cells of the other colour keep their uncorrected values in memory until the next half-sweep
 // overwrites them.  Valid when at least one full sweep follows (nu2 >= 1).  phi_nb + e is the very addition
 // prolong_correct_kernel performs, so results are bitwise those of the two separate kernels.
-template <bool CGL = false>
 __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom& CG, double* phi,
                                                   const double* rhs, const double* e, int colour, int sz,
                                                   long long t)
@@ -318,8 +311,7 @@ __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom
     pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
     const int K = sz == 2 ? (k >> 1) : k;
     // out-of-domain neighbours carry a zero weight; their (zero-pad or foreign) value is used uncorrected
-    double vxm = ld_phi<CGL>(phi + xm), vxp = ld_phi<CGL>(phi + xm + 1), vym = ld_phi<CGL>(phi + c - G.pitch),
-           vyp = ld_phi<CGL>(phi + c + G.pitch), vzm = ld_phi<CGL>(phi + c - G.plane), vzp = ld_phi<CGL>(phi + c + G.plane);
+    double vxm = phi[xm], vxp = phi[xm + 1], vym = phi[c - G.pitch], vyp = phi[c + G.pitch], vzm = phi[c - G.plane], vzp = phi[c + G.plane];
     if (i > 0) vxm += e[cell_at(CG, (i - 1) >> 1, j >> 1, K)];
     if (i < G.nx - 1) vxp += e[cell_at(CG, (i + 1) >> 1, j >> 1, K)];
     if (j > 0) vym += e[cell_at(CG, i >> 1, (j - 1) >> 1, K)];
@@ -346,10 +338,9 @@ __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __res
 }
 
 // r = rhs - A phi, A phi = D phi - sum w phi_nb, D = 1/dinv.
-template <bool CG = false>
 __device__ __forceinline__ double residual_at(const LevelView& L, const double* phi, const double* rhs, long long c, long long xm)
 {
-    return rhs[c] + nb_sum<CG>(L, phi, c, xm) - ld_phi<CG>(phi + c) / L.dinv[c];
+    return rhs[c] + nb_sum(L, phi, c, xm) - phi[c] / L.dinv[c];
 }
 
 // r in the public layout (single-step entry point)
@@ -368,7 +359,6 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 // S3 (per-colour path). Fused residual + restriction: one thread per coarse cell; also zeroes the coarse phi.
 // (Four lanes per coarse cell with a shuffle gather was tried: 70 us instead of 49 us on 256x128x128, the 64-byte
 // runs per row coalesce worse than they gain in occupancy.)
-template <bool CGL = false>
 __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG, const double* phi,
                                              const double* rhs, double* crhs, double* cphi,
                                              int sz, long long t)
@@ -381,7 +371,7 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
             long long row = L.G.plane * (sz * K + r) + (long long)L.G.pitch * (2 * J + q), ce, xe, co, xo;
             pair_addr(L.G, row, I, 0, ce, xe);
             pair_addr(L.G, row, I, 1, co, xo);
-            s += residual_at<CGL>(L, phi, rhs, ce, xe) + residual_at<CGL>(L, phi, rhs, co, xo);
+            s += residual_at(L, phi, rhs, ce, xe) + residual_at(L, phi, rhs, co, xo);
         }
     const long long cc = cell_at(CG, I, J, K);
     crhs[cc] = s / (4.0 * sz);
