@@ -16,7 +16,7 @@ __host__ __device__ inline long long cdiv(long long a, long long b) { return (a 
 // touches every other cell of a row, so in the natural layout half of every 32-byte sector of rhs, 1/D and of the
 // phi being written is fetched for nothing.  Each row therefore stores its even-x cells first, then its odd-x
 // cells, each block followed by one zero element:   [E_0 .. E_{ne-1} 0 | O_0 .. O_{no-1} 0],  pitch = nx + 2.
-// A half-sweep then reads and writes unit-stride runs and moves 5 doubles per relaxation instead of 7.  The pad
+// A half-sweep then reads and writes unit-stride runs and moves 5 doubles per cell of the level (10 per relaxation) instead of 7 (14).  The pad
 // elements double as the zero weight / zero neighbour beyond the low and high x faces (the x-neighbours of E_m are
 // O_{m-1}, O_m, those of O_m are E_m, E_{m+1}); y- and z-neighbours are +-pitch, +-plane away, and beyond the domain
 // they land in another row / plane or in the zeroed pad before and after the array, always under a zero weight.
