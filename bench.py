@@ -34,6 +34,9 @@ B_PROLONG_CORRECT = 17.0
 B_FOLD = 16.0
 B_NORM = 8.0
 B_SETCOEFFS = 24.0
+# DRAM bytes of the six half-sweep launches of one 3-sweep pass over level 0 of config 3, from the ncu --set full
+# capture summarised in profiles/r1d_ncu_full.md (155.5 MB read + 16.8 MB written per launch, each launch cold)
+TRAFFIC_PASS_CONFIG3 = 6 * (155.5e6 + 16.8e6)
 
 
 def level_cells(nx, ny, nz):
@@ -310,7 +313,9 @@ def run_vmg(args):
         "hbm_frac_note": f"algorithmic bytes (203.4 B/cell/V-cycle model) / solve time / {peak} GB/s {peak_src}",
         "roofline": {"bound": "hbm", "kernel": "level-0 red-black smoother (all launches of a nu-sweep pass)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src,
+                     "traffic": TRAFFIC_PASS_CONFIG3 if args.config == 3 and not args.opt else None,
+                     "traffic_note": "DRAM bytes per pass, ncu, each launch cold (profiles/r1d_ncu_full.md); achieved and traffic are per pass = 6 launches",
+                     "achieved_bytes_per_pass": B_SMOOTH_PASS * n0, "peak_source": peak_src,
                      "launches_per_pass": sm_launches / max(2 * n_prof_cycles, 1)},
         "kernel_classes": klass,
         "e2e": {"value": e2e_value, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

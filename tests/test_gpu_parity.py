@@ -91,6 +91,26 @@ def test_single_steps_match_oracle(dims):
     s.destroy()
 
 
+def test_schedule_options_do_not_change_a_single_bit():
+    """Direction of traversal, L2 carve-out, graph replay and the single-CTA tail only reorder independent work:
+    the converged phi and the residual history are bitwise those of the plain in-order launches."""
+    b = _binding()
+    p = inputs.config4(32)
+    ref = None
+    for opts in (dict(snake=0, l2_persist=0, graph=0, tail=0), dict(), dict(snake=1, graph=0), dict(tail=0), dict(blocked=1)):
+        s, d = b.from_problem(p)
+        for k, v in opts.items():
+            s.set_option(k, v)
+        phi = torch.zeros_like(d["rhs"])
+        assert s.solve(d["rhs"], phi, rtol=p.rtol, max_vcycles=p.max_vcycles) == 0
+        out = (phi.clone(), list(s.get_info()[2]))
+        s.destroy()
+        if ref is None:
+            ref = out
+        else:
+            assert torch.equal(out[0], ref[0]) and out[1] == ref[1], opts
+
+
 @pytest.mark.parametrize("dims", [(40, 24, 16), (88, 56, 24), (144, 80, 48), (256, 128, 32)])
 def test_blocked_passes_equal_plain_launches_bitwise(dims):
     """The temporally blocked passes (with fused prolongation / restriction) relax in the same order with the
@@ -177,9 +197,29 @@ def test_config5_full_size_parity():
 @pytest.mark.parametrize("opts", [dict(nu1=2, nu2=2), dict(nu1=1, nu2=3, bottom_sweeps=8), dict(graph=0), dict(blocked=0),
                                   dict(tail=0), dict(blocked=0, tail=0, graph=0), dict(block_min_cells=0),
                                   dict(block_min_cells=0, graph=0, nu1=2, nu2=4), dict(block_min_cells=0, nu1=1, nu2=2),
-                                  dict(block_min_cells=0, nu1=4, nu2=1, tail=0)])
+                                  dict(block_min_cells=0, nu1=4, nu2=1, tail=0), dict(snake=0), dict(l2_persist=0, snake=0, graph=0),
+                                  dict(blocked=1, block_min_cells=0), dict(nu1=3, nu2=1)])
 def test_options_parity(opts):
     check_parity(inputs.random_problem(48, 24, 48, seed=3, bc_type=[D, D, N, N, N, D]), **opts)
+
+
+@pytest.mark.parametrize("nu", [(2, 0), (0, 2), (0, 0)])
+def test_one_sided_smoothing_matches_oracle_cycle_by_cycle(nu):
+    """nu2 = 0 takes the stand-alone prolongation kernel, nu1 = 0 restricts the unsmoothed residual: four fixed
+    cycles (these variants converge slowly or not at all), phi and history against the oracle."""
+    b = _binding()
+    p = inputs.random_problem(48, 24, 48, seed=3, bc_type=[D, D, N, N, N, D])
+    o = Oracle.from_problem(p)
+    s, d = b.from_problem(p)
+    for k, v in zip(("nu1", "nu2"), nu):
+        o.set_option(k, v)
+        s.set_option(k, v)
+    phi_o, st_o, cyc_o, rr_o, hist_o = o.solve(p.rhs, rtol=0.0, max_vcycles=4)
+    phi = torch.zeros_like(d["rhs"])
+    assert s.solve(d["rhs"], phi, rtol=0.0, max_vcycles=4) == st_o == 1
+    assert rel(phi.cpu().numpy(), phi_o) <= 1e-12
+    assert np.allclose(np.array(s.get_info()[2]), hist_o, rtol=1e-9)
+    s.destroy()
 
 
 def test_edge_cases_and_status_codes():
