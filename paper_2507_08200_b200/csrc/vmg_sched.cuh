@@ -126,12 +126,15 @@ inline void plain_prolong_correct(vmg_s* h, int l, long long* count)
     ++*count;
 }
 
-inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out)
+// red_only: the level was last touched by a black half-sweep, after which the residual of every black cell is its own
+// rounding error (rhs + s - fl(fl(dinv*(rhs + s))/dinv), ~2 ulp of D*phi, 1e-16 relative to ||btilde||): the norm is
+// the maximum over the red cells, half the traffic (reading R12 in DESIGN.md).
+inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_only = false)
 {
     VmgLevel& L = h->lev[0];
-    unsigned g = grid_for((long long)L.G.ne * L.ny * L.nz);   // one x-pair per thread
+    unsigned g = grid_for((long long)L.G.ne * L.ny * L.nz);   // one cell per thread, blockIdx.y = colour
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    residual_norm_kernel<<<dim3(g, 2), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
+    residual_norm_kernel<<<dim3(g, red_only ? 1 : 2), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -391,7 +394,7 @@ inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* co
         plain_smooth(h, last, h->nbottom, count);
     }
     for (int l = tail - 1; l >= 0; --l) norm_done = enqueue_up(h, l, l == 0 ? norm_out : nullptr, count);
-    if (norm_out && !norm_done) { enqueue_residual_norm(h, norm_out); ++*count; }
+    if (norm_out && !norm_done) { enqueue_residual_norm(h, norm_out, h->nu2 >= 1 && tail > 0); ++*count; }
     settle_phi(h, 0);
 }
 
