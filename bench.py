@@ -127,7 +127,8 @@ def make_problem(config: int):
 # reference arm: the CPU oracle, as it stands, on the box's host cores
 # ----------------------------------------------------------------------------------------------------
 def oracle_sample(p, cycles_per_step: int):
-    """A bounded sample of the workload: set_coeffs + set_bc + `cycles_per_step` V-cycles (rtol = 0)."""
+    """A bounded sample of the workload: set_coeffs + set_bc + `cycles_per_step` V-cycles (rtol = 0) -- for config 3
+    that is one whole step (the solve needs 10 cycles), ~25 core-seconds on the 16 host threads."""
     from oracle import Oracle
     t0 = time.perf_counter()
     o = Oracle.from_problem(p)
@@ -137,13 +138,18 @@ def oracle_sample(p, cycles_per_step: int):
     return dt
 
 
+def oracle_cycles(p):
+    """V-cycles per oracle sample: a whole solve where that stays within seconds, 2 cycles at 512^3."""
+    return 10 if p.ncells <= (1 << 23) else 2
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     p = make_problem(args.config)
     wm = work_model(p)
-    cyc = 2
+    cyc = oracle_cycles(p)
     for _ in range(args.warmup):
         oracle_sample(p, cyc)
     times = [oracle_sample(p, cyc) for _ in range(args.steps)]
@@ -289,6 +295,43 @@ def run_vmg(args):
     ncyc = float(np.mean(scycles))
     bytes_solve = ncyc * wm["bytes_per_cycle"] + wm["bytes_solve_fixed"]
 
+    # batched multi-component solves (the paper's own optimisation): K independent
+    # solves of the same workload, one handle and one stream each, advanced in lock-step by vmg_solve_batch
+    batched = None
+    if args.batch > 1:
+        K = args.batch
+        bstreams = [torch.cuda.Stream() for _ in range(K)]
+        bsolvers, bphis = [], []
+        for st_ in bstreams:
+            with torch.cuda.stream(st_):
+                sv = binding.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, stream=st_)
+                for kv in args.opt:
+                    key, val = kv.split("=")
+                    sv.set_option(key, float(val))
+                sv.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+                sv.set_bc(p.bc_type, d_bc)
+                bphis.append(torch.zeros(p.rhs.shape, dtype=torch.float64, device=dev))
+            bsolvers.append(sv)
+        torch.cuda.synchronize()
+        btimes = []
+        for it in range(1 + max(2, min(args.steps, 5))):
+            for ph in bphis:
+                ph.zero_()
+            flush.fill_(1.0)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            sts = binding.solve_batch(bsolvers, [d["rhs"]] * K, bphis, rtol=p.rtol, max_vcycles=p.max_vcycles)
+            torch.cuda.synchronize()
+            if it > 0:
+                btimes.append(time.perf_counter() - t0)
+        bcyc = float(np.mean([sv.get_info()[0] for sv in bsolvers]))
+        bt = float(np.mean(btimes))
+        batched = {"k": K, "solves_per_s": world * K / bt, "vcycles_per_s": world * K * bcyc / bt, "ms_per_batch": bt * 1e3,
+                   "hbm_frac": K * (bcyc * wm["bytes_per_cycle"] + wm["bytes_solve_fixed"]) / bt / 1e9 / peak,
+                   "timing": "host clock around vmg_solve_batch, device synchronised on both sides", "statuses": sorted(set(sts))}
+        for sv in bsolvers:
+            sv.destroy()
+
     # end to end through the C-ABI with host buffers
     etimes, ecycles, _ = timed(step_e2e, args.steps, max(1, min(args.warmup, 2)))
     etotal = float(etimes.sum())
@@ -318,13 +361,14 @@ def run_vmg(args):
                      "achieved_bytes_per_pass": B_SMOOTH_PASS * n0, "peak_source": peak_src,
                      "launches_per_pass": sm_launches / max(2 * n_prof_cycles, 1)},
         "kernel_classes": klass,
+        "batched": batched,
         "e2e": {"value": e2e_value, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": etotal / args.steps * 1e3},
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cyc = 2
+        cyc = oracle_cycles(p)
         oracle_sample(p, 1)
         t_or = [oracle_sample(p, cyc) for _ in range(2)]
         dt = float(np.mean(t_or))
@@ -346,6 +390,7 @@ def main():
     ap.add_argument("--impl", default="vmg", choices=["vmg", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch", type=int, default=8, help="K for the batched multi-component leg (0/1: skip)")
     ap.add_argument("--opt", action="append", default=[], help="vmg_set_option key=value (experiments)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "vmg" else args.warmup

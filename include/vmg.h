@@ -82,6 +82,19 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6]);
  * returning. */
 int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max_vcycles);
 
+/* Batched solve (the paper's "multi-component" optimisation: "simultaneously solving multiple scalar solution
+ * components with each multigrid solve results in more GPU work").  n independent
+ * problems, one handle each -- same or different grids, coefficients and boundary conditions -- advanced in
+ * lock-step: each round enqueues one V-cycle per unfinished handle on that handle's stream, then synchronises and
+ * applies the exit rules of vmg_solve to each.  Create the handles with DISTINCT streams (or cuda_stream = NULL,
+ * which gives each its own): the latency-bound coarse levels of one solve then overlap the bandwidth-bound fine
+ * level of another.  handles, rhs, phi: HOST arrays of n entries (rhs[i], phi[i]: DEVICE arrays as in vmg_solve);
+ * status: HOST array of n ints or NULL, receives what vmg_solve would have returned for problem i.  Every solve
+ * performs exactly the operations vmg_solve would: results are bitwise the same.  Returns the most severe status
+ * (the smallest negative code if any, else the largest positive, else VMG_OK). */
+int vmg_solve_batch(int n, const vmg_handle* handles, const double* const* rhs, double* const* phi, double rtol,
+                    int max_vcycles, int* status);
+
 /* Result of the last vmg_solve.  cycles, relres: HOST scalars (may be NULL).  history: HOST array of at
  * least cycles+1 doubles (relative residual before the first cycle and after each cycle) or NULL. */
 int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);

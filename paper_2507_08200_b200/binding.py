@@ -17,7 +17,7 @@ STATUS = {0: "OK", 1: "MAXCYCLES", 2: "STALLED", -1: "ERR_ARG", -2: "ERR_SIZE", 
           -4: "ERR_SINGULAR", -5: "ERR_DIVERGED", -6: "ERR_CUDA", -7: "ERR_ALLOC"}
 
 # every symbol include/vmg.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_solve", "vmg_get_info", "vmg_set_option",
+SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_solve", "vmg_solve_batch", "vmg_get_info", "vmg_set_option",
            "vmg_destroy", "vmg_strerror", "vmg_last_cuda_error", "vmg_num_levels", "vmg_level_dims",
            "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
            "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_down", "vmg_step_up", "vmg_step_vcycle", "vmg_step_norm_inf",
@@ -40,6 +40,8 @@ def load():
     lib.vmg_set_coeffs.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_double, C.c_double]
     lib.vmg_set_bc.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(_vp)]
     lib.vmg_solve.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int]
+    lib.vmg_solve_batch.argtypes = [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp), C.c_double, C.c_int,
+                                    C.POINTER(C.c_int)]
     lib.vmg_get_info.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.vmg_set_option.argtypes = [_vp, C.c_char_p, C.c_double]
     lib.vmg_destroy.argtypes = [_vp]
@@ -87,6 +89,24 @@ def _ptr(t) -> Optional[int]:
     torch = _torch()
     assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous(), "need contiguous fp64 CUDA tensors"
     return t.data_ptr()
+
+
+def solve_batch(solvers, rhs, phi, rtol: float = 1e-12, max_vcycles: int = 50) -> List[int]:
+    """vmg_solve_batch: n independent solves advanced in lock-step (give every Vmg its own torch stream so that they
+    overlap).  rhs, phi: lists of tensors; returns the list of status codes; raises on the first negative one."""
+    n = len(solvers)
+    assert len(rhs) == n and len(phi) == n
+    lib = load()
+    hs = (_vp * n)(*[s._h for s in solvers])
+    r = (_vp * n)(*[_ptr(t) for t in rhs])
+    p = (_vp * n)(*[_ptr(t) for t in phi])
+    st = (C.c_int * n)()
+    lib.vmg_solve_batch(n, hs, r, p, rtol, max_vcycles, st)
+    out = [int(v) for v in st]
+    for s, v in zip(solvers, out):
+        if v < 0:
+            raise VmgError(v, "vmg_solve_batch", lib.vmg_last_cuda_error(s._h))
+    return out
 
 
 class Vmg:

@@ -342,12 +342,20 @@ int vmg_get_profile(vmg_handle h, double ms[8], long long launches[8])
     return VMG_OK;
 }
 
-// C5 of DESIGN.md: relres = ||btilde - A phi||_inf / ||btilde||_inf; stall rule; status codes.
-static int solve_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int max_vcycles)
+}  // extern "C"
+
+// C5 of DESIGN.md: relres = ||btilde - A phi||_inf / ||btilde||_inf; stall rule; status codes.  The solve is cut
+// into phases that only enqueue work and phases that run after a stream synchronise, so that vmg_solve_batch can
+// advance several handles (one stream each) in lock-step and their kernels overlap on the GPU.
+namespace {
+
+// enqueue: fold_bc, phi -> internal layout, ||btilde||, the initial residual norm, read-back
+int solve_begin(vmg_s* h, const double* rhs, double* phi, double rtol, int max_vcycles)
 {
     VmgLevel& L0 = h->lev[0];
     unsigned long long* scal = (unsigned long long*)h->d_scal;
-
+    h->hist.clear(); h->cycles = 0; h->relres = 0.0; h->launches = 0;
+    h->sv_rtol = rtol; h->sv_max = max_vcycles; h->sv_phi = phi; h->sv_slow = 0; h->sv_status = VMG_MAXCYCLES; h->sv_active = false;
     int rc = enqueue_fold_bc(h, rhs, L0.rhs);
     if (rc != VMG_OK) return rc;
     {
@@ -363,45 +371,77 @@ static int solve_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int
     h->launches += 3;   // phi copy-in, ||btilde||, first residual norm
     CUDA_TRY(h, cudaGetLastError());
     CUDA_TRY(h, cudaMemcpyAsync(h->h_scal, scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    double nb = h->h_scal[0], r = h->h_scal[1];
-    int status = VMG_MAXCYCLES;
-    if (nb == 0.0) {
-        CUDA_TRY(h, cudaMemsetAsync(phi, 0, L0.n * sizeof(double), h->stream));
-        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return VMG_OK;
+}
+
+// after a synchronise: hist[0]; sets sv_active when V-cycles are needed.  Returns a negative code on failure.
+int solve_begin_finish(vmg_s* h)
+{
+    VmgLevel& L0 = h->lev[0];
+    h->sv_nb = h->h_scal[0];
+    if (h->sv_nb == 0.0) {   // zero right-hand side and homogeneous data: phi = 0
+        CUDA_TRY(h, cudaMemsetAsync(h->sv_phi, 0, L0.n * sizeof(double), h->stream));
         h->hist.push_back(0.0);
+        h->sv_status = VMG_OK;
+        h->sv_phi = nullptr;   // nothing to copy out
         return VMG_OK;
     }
-    h->relres = r / nb;
+    h->relres = h->h_scal[1] / h->sv_nb;
     h->hist.push_back(h->relres);
-    if (std::isnan(h->relres) || std::isinf(h->relres)) return VMG_ERR_DIVERGED;
-    if (rtol > 0.0 && h->relres <= rtol) status = VMG_OK;
-    else {
-        int slow = 0;
-        for (int c = 1; c <= max_vcycles; ++c) {
-            rc = run_vcycle_with_norm(h, scal + 1);       // graph replay or plain launches
-            if (rc != VMG_OK) return rc;
-            CUDA_TRY(h, cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-            CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-            h->relres = h->h_scal[1] / nb;
-            h->hist.push_back(h->relres);
-            h->cycles = c;
-            if (std::isnan(h->relres) || std::isinf(h->relres)) { status = VMG_ERR_DIVERGED; break; }
-            if (rtol > 0.0) {
-                if (h->relres <= rtol) { status = VMG_OK; break; }
-                slow = (h->hist[c] >= 0.9 * h->hist[c - 1]) ? slow + 1 : 0;
-                if (slow >= 3) { status = VMG_STALLED; break; }
-            }
-        }
-    }
-    {
-        ProfScope ps(h, VMG_PC_COPY, nullptr);
-        to_natural_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, L0.phi, phi);
-        h->launches += 1;
-    }
-    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    return status;
+    if (std::isnan(h->relres) || std::isinf(h->relres)) { h->sv_status = VMG_ERR_DIVERGED; h->sv_phi = nullptr; return VMG_OK; }
+    if (h->sv_rtol > 0.0 && h->relres <= h->sv_rtol) h->sv_status = VMG_OK;
+    else h->sv_active = h->sv_max > 0;
+    return VMG_OK;
 }
+
+// enqueue one V-cycle, its residual norm and the read-back
+int solve_cycle_launch(vmg_s* h)
+{
+    unsigned long long* scal = (unsigned long long*)h->d_scal;
+    int rc = run_vcycle_with_norm(h, scal + 1);       // graph replay or plain launches
+    if (rc != VMG_OK) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    return VMG_OK;
+}
+
+// after a synchronise: exit rules
+void solve_cycle_finish(vmg_s* h)
+{
+    const int c = ++h->cycles;
+    h->relres = h->h_scal[1] / h->sv_nb;
+    h->hist.push_back(h->relres);
+    if (std::isnan(h->relres) || std::isinf(h->relres)) { h->sv_status = VMG_ERR_DIVERGED; h->sv_active = false; h->sv_phi = nullptr; return; }
+    if (h->sv_rtol > 0.0) {
+        if (h->relres <= h->sv_rtol) { h->sv_status = VMG_OK; h->sv_active = false; return; }
+        h->sv_slow = (h->hist[c] >= 0.9 * h->hist[c - 1]) ? h->sv_slow + 1 : 0;
+        if (h->sv_slow >= 3) { h->sv_status = VMG_STALLED; h->sv_active = false; return; }
+    }
+    if (c >= h->sv_max) h->sv_active = false;
+}
+
+// enqueue: phi -> the caller's array
+int solve_end(vmg_s* h)
+{
+    VmgLevel& L0 = h->lev[0];
+    if (h->sv_phi) {
+        ProfScope ps(h, VMG_PC_COPY, nullptr);
+        to_natural_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, L0.phi, h->sv_phi);
+        h->launches += 1;
+        CUDA_TRY(h, cudaGetLastError());
+    }
+    return VMG_OK;
+}
+
+int solve_close(vmg_s* h, int rc)
+{
+    if (h->profile) { cudaStreamSynchronize(h->stream); prof_collect(h); }
+    h->total_launches += h->launches;
+    return rc != VMG_OK ? rc : h->sv_status;
+}
+
+}  // namespace
+
+extern "C" {
 
 int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max_vcycles)
 {
@@ -409,11 +449,67 @@ int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max
     int rc = ready(h);
     if (rc != VMG_OK) return rc;
     if (singular(h)) return VMG_ERR_SINGULAR;
-    h->hist.clear(); h->cycles = 0; h->relres = 0.0; h->launches = 0;
-    rc = solve_impl(h, rhs, phi, rtol, max_vcycles);
-    if (h->profile) { cudaStreamSynchronize(h->stream); prof_collect(h); }
-    h->total_launches += h->launches;
-    return rc;
+    rc = solve_begin(h, rhs, phi, rtol, max_vcycles);
+    if (rc == VMG_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = VMG_ERR_CUDA;
+    if (rc == VMG_OK) rc = solve_begin_finish(h);
+    while (rc == VMG_OK && h->sv_active) {
+        rc = solve_cycle_launch(h);
+        if (rc == VMG_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = VMG_ERR_CUDA;
+        if (rc == VMG_OK) solve_cycle_finish(h);
+    }
+    if (rc == VMG_OK) rc = solve_end(h);
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess && rc == VMG_OK) rc = VMG_ERR_CUDA;
+    if (rc == VMG_ERR_CUDA) { h->last_cuda_error = (int)cudaGetLastError(); }
+    return solve_close(h, rc);
+}
+
+// N independent problems (one handle and one stream each), advanced in lock-step: every round enqueues one V-cycle
+// per unfinished handle and then synchronises them, so the latency-bound coarse levels of one solve overlap the
+// bandwidth-bound fine level of another (the paper's "multi-component" optimisation).
+int vmg_solve_batch(int n, const vmg_handle* hs, const double* const* rhs, double* const* phi, double rtol, int max_vcycles,
+                    int* status)
+{
+    if (n < 0 || (n > 0 && (!hs || !rhs || !phi)) || max_vcycles < 0) return VMG_ERR_ARG;
+    std::vector<int> rc(n, VMG_OK);
+    for (int i = 0; i < n; ++i) {
+        vmg_s* h = hs[i];
+        if (!h || !rhs[i] || !phi[i]) { rc[i] = VMG_ERR_ARG; continue; }
+        for (int k = 0; k < i; ++k) if (hs[k] == h) rc[i] = VMG_ERR_ARG;   // a handle can run one solve at a time
+        if (rc[i] != VMG_OK) continue;
+        rc[i] = ready(h);
+        if (rc[i] == VMG_OK && singular(h)) rc[i] = VMG_ERR_SINGULAR;
+        if (rc[i] == VMG_OK) rc[i] = solve_begin(h, rhs[i], phi[i], rtol, max_vcycles);
+    }
+    auto sync_all = [&]() {
+        for (int i = 0; i < n; ++i)
+            if (rc[i] == VMG_OK && cudaStreamSynchronize(hs[i]->stream) != cudaSuccess) {
+                rc[i] = VMG_ERR_CUDA; hs[i]->last_cuda_error = (int)cudaGetLastError();
+            }
+    };
+    sync_all();
+    for (int i = 0; i < n; ++i) if (rc[i] == VMG_OK) rc[i] = solve_begin_finish(hs[i]);
+    for (;;) {
+        bool any = false;
+        for (int i = 0; i < n; ++i)
+            if (rc[i] == VMG_OK && hs[i]->sv_active) { rc[i] = solve_cycle_launch(hs[i]); any = true; }
+        if (!any) break;
+        for (int i = 0; i < n; ++i)
+            if (rc[i] == VMG_OK && hs[i]->sv_active) {
+                if (cudaStreamSynchronize(hs[i]->stream) != cudaSuccess) { rc[i] = VMG_ERR_CUDA; hs[i]->last_cuda_error = (int)cudaGetLastError(); }
+                else solve_cycle_finish(hs[i]);
+            }
+    }
+    for (int i = 0; i < n; ++i) if (rc[i] == VMG_OK) rc[i] = solve_end(hs[i]);
+    sync_all();
+    int worst = VMG_OK;
+    for (int i = 0; i < n; ++i) {
+        int st = rc[i];
+        if (hs && hs[i] && rc[i] != VMG_ERR_ARG && rc[i] != VMG_ERR_STATE && rc[i] != VMG_ERR_SINGULAR) st = solve_close(hs[i], rc[i]);
+        if (status) status[i] = st;
+        if (st < 0) worst = worst < 0 ? std::min(worst, st) : st;
+        else if (worst >= 0) worst = std::max(worst, st);
+    }
+    return worst;
 }
 
 }  // extern "C"

@@ -76,6 +76,11 @@ struct vmg_s {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t graph_exec = nullptr;
     bool graph_valid = false;
+    // state of the solve in progress (vmg_solve / vmg_solve_batch phases)
+    double sv_rtol = 0.0, sv_nb = 0.0;
+    int sv_max = 0, sv_slow = 0, sv_status = 0;
+    bool sv_active = false;
+    double* sv_phi = nullptr;
     // result of the last solve
     int cycles = 0;
     double relres = 0.0;

@@ -310,3 +310,38 @@ def test_user_stream_and_repeatability():
     st.synchronize()
     assert torch.equal(phi1, phi2)          # red-black updates are order independent: bitwise repeatable
     s.destroy()
+
+
+def test_batched_solves_are_bitwise_the_single_solves():
+    """vmg_solve_batch: different problems on different streams advanced in lock-step
+    give bit for bit what vmg_solve gives for each, with their own cycle counts and statuses."""
+    b = _binding()
+    probs = [inputs.config3(16), inputs.config4(16), inputs.config2(32), inputs.random_problem(40, 24, 16, seed=9, bc_type=MIXED)]
+    single = []
+    for p in probs:
+        s, d = b.from_problem(p)
+        phi = torch.zeros_like(d["rhs"])
+        st = s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=30)
+        single.append((st, s.get_info(), phi.clone()))
+        s.destroy()
+    streams = [torch.cuda.Stream() for _ in probs]
+    solvers, data = [], []
+    for p, stream in zip(probs, streams):
+        with torch.cuda.stream(stream):
+            s, d = b.from_problem(p, stream=stream)
+        solvers.append(s); data.append(d)
+    torch.cuda.synchronize()
+    phis = [torch.zeros_like(d["rhs"]) for d in data]
+    sts = b.solve_batch(solvers, [d["rhs"] for d in data], phis, rtol=1e-12, max_vcycles=30)
+    for s, st, phi, ref in zip(solvers, sts, phis, single):
+        cyc, rr, hist = s.get_info()
+        assert st == ref[0] and cyc == ref[1][0] and list(hist) == list(ref[1][2])
+        assert torch.equal(phi, ref[2])
+        s.destroy()
+    # a handle may appear once; an unready handle reports its own error without stopping the others
+    s1, d1 = b.from_problem(probs[0])
+    s2 = b.Vmg(16, 8, 8, 1.0, 1.0, 1.0)
+    with pytest.raises(b.VmgError) as e:
+        b.solve_batch([s1, s2], [d1["rhs"], d1["rhs"]], [torch.zeros_like(d1["rhs"]), torch.zeros_like(d1["rhs"])])
+    assert e.value.code == -3
+    s1.destroy(); s2.destroy()
