@@ -57,10 +57,46 @@ __device__ __forceinline__ double tail_nb_sum(const TailSmem& s, const TailLevel
     return v;
 }
 
+// nsweeps red-black sweeps.  Levels whose half-sweep fits the CTA (nt <= blockDim: all tail levels in practice) take
+// their cell indices once, not per half-sweep; levels whose half-sweep fits ONE WARP (the 32-sweep bottom solve on
+// 4x2x2 or 2x2x2: 8 or 4 relaxations per colour) are relaxed by warp 0 alone with __syncwarp() between the colours
+// instead of 64 block-wide barriers.  The caller's __syncthreads() semantics are kept: all threads leave in step.
 __device__ __forceinline__ void tail_smooth(const TailSmem& s, const TailLevel& L, int nsweeps)
 {
     const int hx = (L.nx + 1) >> 1;
     const int nt = hx * L.ny * L.nz;
+    if (nt <= (int)blockDim.x) {
+        const int t = threadIdx.x;
+        int c[2] = {-1, -1};
+        if (t < nt) {
+            const int m = t % hx, j = (t / hx) % L.ny, k = t / (hx * L.ny);
+#pragma unroll
+            for (int colour = 0; colour < 2; ++colour) {
+                const int i = 2 * m + ((colour + j + k) & 1);
+                if (i < L.nx) c[colour] = i + L.nx * j + L.nxy * k;
+            }
+        }
+        if (nt <= 32) {
+            if (threadIdx.x < 32)
+                for (int sw = 0; sw < nsweeps; ++sw) {
+#pragma unroll
+                    for (int colour = 0; colour < 2; ++colour) {
+                        if (c[colour] >= 0) s.phi[c[colour]] = s.dinv[c[colour]] * (s.rhs[c[colour]] + tail_nb_sum(s, L, c[colour]));
+                        __syncwarp();
+                    }
+                }
+            __syncthreads();
+            return;
+        }
+        for (int sw = 0; sw < nsweeps; ++sw) {
+#pragma unroll
+            for (int colour = 0; colour < 2; ++colour) {
+                if (c[colour] >= 0) s.phi[c[colour]] = s.dinv[c[colour]] * (s.rhs[c[colour]] + tail_nb_sum(s, L, c[colour]));
+                __syncthreads();
+            }
+        }
+        return;
+    }
     for (int sw = 0; sw < nsweeps; ++sw)
         for (int colour = 0; colour < 2; ++colour) {
             for (int t = threadIdx.x; t < nt; t += blockDim.x) {
