@@ -81,8 +81,7 @@ int finalize_dinv(vmg_s* h)
         finalize_dinv_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(g);
     }
     CUDA_TRY(h, cudaGetLastError());
-    h->dinv_dirty = false;
-    h->graph_valid = false;
+    h->dinv_dirty = false;   // (the captured V-cycle graph holds pointers and sizes only: new coefficients do not invalidate it)
     return VMG_OK;
 }
 
