@@ -70,6 +70,22 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def max_over_ranks(seconds: float, dist, device=None) -> float:
+    """Time of the slowest replica (the contract: barrier on both sides, MAX over ranks)."""
+    if dist is None:
+        return seconds
+    import torch
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_replicas(units_per_rank: float, seconds: float, world: int, dist, device=None) -> float:
+    """Whole-job throughput of `world` independent replicas: every rank processes
+    the same number of units, the job takes as long as its slowest rank; no collective touches the data path."""
+    return world * units_per_rank / max_over_ranks(seconds, dist, device)
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
 
@@ -266,13 +282,9 @@ def run_vmg(args):
 
     sampler = ClockSampler(local)
     times, cycles, launches = timed(step_resident, args.steps, args.warmup, sampler)
-    total = float(times.sum())
-    if dist is not None:
-        t = torch.tensor([total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total = float(t.item())
+    total = max_over_ranks(float(times.sum()), dist, dev)
     updates_per_step = float(np.mean(cycles)) * wm["updates_per_cycle"]
-    value = world * args.steps * updates_per_step / total
+    value = aggregate_replicas(args.steps * updates_per_step, float(times.sum()), world, dist, dev)
 
     # solve-only and per-kernel-class numbers (plain launches with event pairs; same workload)
     s.set_option("profile", 1)
@@ -334,11 +346,7 @@ def run_vmg(args):
 
     # end to end through the C-ABI with host buffers
     etimes, ecycles, _ = timed(step_e2e, args.steps, max(1, min(args.warmup, 2)))
-    etotal = float(etimes.sum())
-    if dist is not None:
-        t = torch.tensor([etotal], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        etotal = float(t.item())
+    etotal = max_over_ranks(float(etimes.sum()), dist, dev)
     e2e_value = world * args.steps * float(np.mean(ecycles)) * wm["updates_per_cycle"] / etotal
     clocks = sampler.finish()   # sampled over all timed regions of this run (headline, per-kernel, solve-only, end-to-end)
 
