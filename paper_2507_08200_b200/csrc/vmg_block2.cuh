@@ -24,7 +24,8 @@
 // Shared memory holds, for the S planes in flight, what OTHER threads read: phi (x- and y-neighbour outside the
 // patch) and rhs, 1/D, wx, wy, split by x-parity and by row parity so that a half-sweep (which touches one
 // x-parity per row) reads and writes unit-stride fp64 vectors without bank conflicts.  One relaxation = 8 LDS.64 +
-// 1 STS.64.  Global loads are register-staged one plane ahead (12 x 16-byte loads per thread per plane), so data
+// 1 STS.64.  Global loads are register-staged one plane ahead (24 x 8-byte loads per thread per plane: the level arrays
+// are stored x-parity split), so data
 // in flight costs no shared memory; a 2 x 2 patch per thread halves the thread count, which leaves each thread the
 // ~170 registers that the rings, the staged loads and the residual stage need without spilling.
 //
@@ -75,7 +76,6 @@ struct BlockCfg {
                       TX % 2 == 0 && TY % 2 == 0 && NYT % 2 == 0 && R >= S + 3 && R % 2 == 0, "tile");
 };
 
-__device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
 __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 constexpr int kBlkPrefetch = 2;   // planes ahead of the register-staged loads
 
@@ -150,21 +150,13 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
         for (int r = 0; r < 2; ++r) {
             r_phi[r] = r_wz[r] = r_rhs[r] = r_dinv[r] = r_wx[r] = r_wy[r] = zero;
             r_e[r] = 0.0;
-#ifdef VMG_ABL_NOLOAD
-            if (in_r[r] && zq == -12345) {
-#else
             if (in_r[r] && zq >= 0 && zq < g.G.nz) {
-#endif
                 const long long c = cbase + r * g.G.pitch + g.G.plane * zq;
                 r_phi[r] = ld2(g.phi_in, c);
                 r_wz[r] = ld2(g.wz, c);
                 if (PROLONG) r_e[r] = __ldg(g.e + cell_at(g.CG, gx >> 1, (gy0 + r) >> 1, zq >> 1));
             }
-#ifdef VMG_ABL_NOLOAD
-            if (in_r[r] && zq == -12345) {
-#else
             if (in_r[r] && zq - 1 >= 0 && zq - 1 < g.G.nz) {
-#endif
                 const long long c = cbase + r * g.G.pitch + g.G.plane * (zq - 1);
                 r_rhs[r] = ld2(g.rhs, c);
                 r_dinv[r] = ld2(g.dinv, c);
@@ -196,12 +188,8 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
 
             // ---- stages: half-sweep s on plane zl - s (ring slot (u-s) % R, shared slot sl[s-1]); rim threads compute
             // and discard.  Row r relaxes its cell of x-parity sg = (C0 + r + u + 1) & 1. ----
-#ifdef VMG_ABL_NOSTAGE
-            for (int s = 1; s <= 0; ++s) {
-#else
 #pragma unroll
             for (int s = 1; s <= S; ++s) {
-#endif
                 const int c = ((u - s) % R + R) % R, cu = ((u - s + 1) % R + R) % R, cd = ((u - s - 1) % R + R) % R;
                 double* P = blk_smem + sl[s - 1];
                 double nv[2];
@@ -284,9 +272,7 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
                         }
                     }
                 }
-#ifndef VMG_ABL_NOBAR
                 __syncthreads();
-#endif
             }
 
             // ---- plane zl - S is final: write it back from registers ----
@@ -308,12 +294,10 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
                 for (int r = 0; r < 2; ++r) {
                     const int o0 = r * NPH, o1 = XB + r * NPH;
                     F[A_PHI + o0] = pe[r][u];     F[A_PHI + o1] = po[r][u];
-#ifndef VMG_ABL_NOFILL
                     F[A_RHS + o0] = r_rhs[r].x;   F[A_RHS + o1] = r_rhs[r].y;
                     F[A_DINV + o0] = r_dinv[r].x; F[A_DINV + o1] = r_dinv[r].y;
                     F[A_WX + o0] = r_wx[r].x;     F[A_WX + o1] = r_wx[r].y;
                     F[A_WY + o0] = r_wy[r].x;     F[A_WY + o1] = r_wy[r].y;
-#endif
                 }
             }
             {
