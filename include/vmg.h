@@ -107,6 +107,8 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  * "l2_persist" (MB of L2 set aside for the level-0 face weights through a stream access-policy window,
  *   default 24, 0 = none; applied only when those weights exceed half the L2.  NOTE: this calls
  *   cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize), a setting of the whole CUDA context),
+ * "pdl" (1: the V-cycle kernels are launched with programmatic stream serialisation, so each kernel's launch overlaps
+ *   the tail of its predecessor, default; 0: plain serialisation),
  * "blocked" (1: temporally blocked smoother passes with fused transfers (vmg_block2.cuh); 0: one kernel per
  *   colour half-sweep, default -- the blocked passes are bitwise equal but measure slower on B200),
  * "block_min_cells" (smallest level the blocked passes are used on when blocked = 1, default 4096),

@@ -11,6 +11,18 @@ constexpr int kThreads = 256;
 
 __host__ __device__ inline long long cdiv(long long a, long long b) { return (a + b - 1) / b; }
 
+// Programmatic dependent launch: the V-cycle's kernels are launched with programmaticStreamSerialization, so a kernel's
+// launch (CTA scheduling, parameter fetch, index arithmetic) overlaps the tail of its predecessor; nothing of the
+// predecessor's output is touched, and nothing it still reads is overwritten, before this wait (which also flushes
+// the predecessor's writes).  A no-op when the kernel was launched without the attribute.
+// Right after it the kernel lets ITS dependents be scheduled (the trigger fires once every CTA of this grid has started
+// or exited): their CTAs fill the SM slots that this grid's last wave leaves free and sit in their own wait.
+__device__ __forceinline__ void grid_dependency_wait()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 // ------------------------------------------------------------------------------------------------
 // Internal layout of a level's cell arrays ("x-parity split").  A colour half-sweep
 // touches every other cell of a row, so in the natural layout half of every 32-byte sector of rhs, 1/D and of the
@@ -285,6 +297,7 @@ __device__ __forceinline__ void relax_one(const LevelView& L, double* phi, const
 // the phi just written are common to both colours).
 __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour, int reverse)
 {
+    grid_dependency_wait();
     const long long nt = (long long)L.G.ne * L.G.ny * L.G.nz;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
@@ -332,6 +345,7 @@ __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom
 __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __restrict__ phi, const double* __restrict__ rhs,
                                              const double* __restrict__ e, int colour, int sz, int reverse)
 {
+    grid_dependency_wait();
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
     if (t < (long long)L.G.ne * L.G.ny * L.G.nz) relax_prolong_one(L, CG, phi, rhs, e, colour, sz, t);
@@ -381,6 +395,7 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
 __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
                                          double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
 {
+    grid_dependency_wait();
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
     if (t < CG.n) restrict_one(L, CG, phi, rhs, crhs, cphi, sz, t);
@@ -398,6 +413,7 @@ __device__ __forceinline__ void prolong_one(const Geom& G, const Geom& CG, doubl
 
 __global__ void prolong_correct_kernel(Geom G, Geom CG, double* __restrict__ phi, const double* __restrict__ e, int sz)
 {
+    grid_dependency_wait();
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (t < G.n) prolong_one(G, CG, phi, e, sz, t);
 }
@@ -448,6 +464,7 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
                                      unsigned long long* out, int reverse)
 {
+    grid_dependency_wait();
     const Geom& G = L.G;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;

@@ -26,6 +26,20 @@ inline unsigned grid_for(long long n) { return (unsigned)cdiv(n, kThreads); }
 // direction of the next whole-level kernel: consecutive kernels walk the level in opposite directions (L2 reuse)
 inline int next_dir(vmg_s* h, VmgLevel& L) { int d = h->snake ? L.dir : 0; L.dir ^= 1; return d; }
 
+// launch with programmatic stream serialisation (see grid_dependency_wait in vmg_kernels.cuh)
+template <typename... KArgs, typename... Args>
+inline void launch_pdl(vmg_s* h, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = h->use_pdl ? 1 : 0;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 inline double* cur_phi(VmgLevel& L) { return L.cur ? L.phi2 : L.phi; }
 inline double* other_phi(VmgLevel& L) { return L.cur ? L.phi : L.phi2; }
 
@@ -103,7 +117,7 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
     for (int s = 0; s < nsweeps; ++s)
         for (int colour = 0; colour < 2; ++colour) {
             if (2 * s + colour < skip_first) continue;
-            smooth_colour_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(v, cur_phi(L), L.rhs, colour, next_dir(h, L));
+            launch_pdl(h, smooth_colour_kernel, grid_for(nt), kThreads, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
             ++*count;
         }
 }
@@ -113,16 +127,16 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
     VmgLevel& L = h->lev[l];
     VmgLevel& C = h->lev[l + 1];
     C.cur = 0;
-    residual_restrict_kernel<<<grid_for(C.n), kThreads, 0, h->stream>>>(view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
-                                                                       h->three_d ? 2 : 1, next_dir(h, L));
+    launch_pdl(h, residual_restrict_kernel, grid_for(C.n), kThreads, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
+               h->three_d ? 2 : 1, next_dir(h, L));
     ++*count;
 }
 
 inline void plain_prolong_correct(vmg_s* h, int l, long long* count)
 {
     VmgLevel& L = h->lev[l];
-    prolong_correct_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(L.G, h->lev[l + 1].G, cur_phi(L), cur_phi(h->lev[l + 1]),
-                                                                     h->three_d ? 2 : 1);
+    launch_pdl(h, prolong_correct_kernel, grid_for(L.n), kThreads, 0, L.G, h->lev[l + 1].G, cur_phi(L), cur_phi(h->lev[l + 1]),
+               h->three_d ? 2 : 1);
     ++*count;
 }
 
@@ -134,7 +148,7 @@ inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_on
     VmgLevel& L = h->lev[0];
     unsigned g = grid_for((long long)L.G.ne * L.ny * L.nz);   // one cell per thread, blockIdx.y = colour
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    residual_norm_kernel<<<dim3(g, red_only ? 1 : 2), kThreads, 0, h->stream>>>(view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
+    launch_pdl(h, residual_norm_kernel, dim3(g, red_only ? 1 : 2), kThreads, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -191,7 +205,7 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
     ProfScope ps(h, VMG_PC_COARSE, count);
     {
         int threads = (int)std::min<long long>(kTailThreads, std::max<long long>(64, (h->lev[first].n / 2 + 31) / 32 * 32));
-        coarse_tail_kernel<<<1, threads, h->tail_smem, h->stream>>>(g);
+        launch_pdl(h, coarse_tail_kernel, 1, threads, h->tail_smem, g);
     }
     ++*count;
 }
@@ -360,8 +374,8 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         VmgLevel& L = h->lev[l];
         long long nt = (long long)L.G.ne * L.ny * L.nz;
-        smooth_colour_prolong_kernel<<<grid_for(nt), kThreads, 0, h->stream>>>(view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
-                                                                              cur_phi(h->lev[l + 1]), 0, h->three_d ? 2 : 1, next_dir(h, L));
+        launch_pdl(h, smooth_colour_prolong_kernel, grid_for(nt), kThreads, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
+                   cur_phi(h->lev[l + 1]), 0, h->three_d ? 2 : 1, next_dir(h, L));
         ++*count;
         plain_smooth(h, l, h->nu2, count, 1);
         return false;

@@ -203,6 +203,10 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
 }
 
 
-__global__ void __launch_bounds__(kTailThreads, 1) coarse_tail_kernel(TailArgs g) { coarse_tail_body(g); }
+__global__ void __launch_bounds__(kTailThreads, 1) coarse_tail_kernel(TailArgs g)
+{
+    grid_dependency_wait();
+    coarse_tail_body(g);
+}
 
 }  // namespace vmg
