@@ -49,6 +49,7 @@ typedef struct ovmg {
     double *bcval[6];           /* level-0 value planes (owned copies; NULL = homogeneous) */
     int have_coeffs, have_bc;
     int nu1, nu2, nbottom;
+    int prolong;                /* 0: piecewise constant (R9 default), 1: trilinear (R9 option) */
     int cycles, status;
     double relres;
     double *hist;
@@ -169,15 +170,59 @@ static void restrict_level(const ovmg *h, int lev, const double *rfine, double *
             }
 }
 
-/* C3. Prolongation + correction: piecewise constant, phi_f[i,j,k] += e_c[i/2, j/2, k/2]. */
+/* C3. Prolongation + correction: piecewise constant, phi_f[i,j,k] += e_c[i/2, j/2, k/2] (R9, default).
+ *
+ * Option prolong = 1 (SURVEY.md sec. 8(c) R9 / DESIGN.md R9): cell-centred trilinear interpolation.  Per direction
+ * the fine cell i lies a quarter of a coarse cell from the centre of its parent I = i/2, towards I+1 if i is odd and
+ * towards I-1 if i is even: weights 3/4 (parent) and 1/4 (that neighbour); the 3-D weight is the product (8 coarse
+ * values; 4 in 2-D).  A neighbour beyond a domain face is a ghost: -e(parent) at a Dirichlet face (the error vanishes
+ * on the face, which lies half a coarse cell from the parent's centre), +e(parent) at a Neumann face. */
+static double coarse_or_ghost(const ovmg *h, const olevel *C, const double *e, const int idx[3], const int par[3])
+{
+    /* idx: requested coarse index per direction (may be -1 or n), par: the parent's index (always inside) */
+    int n[3], use[3], d;
+    double sign = 1.0;
+    n[0] = C->nx; n[1] = C->ny; n[2] = C->nz;
+    for (d = 0; d < 3; ++d) {
+        use[d] = idx[d];
+        if (idx[d] < 0)          { use[d] = par[d]; sign *= (h->bctype[2 * d] == BC_DIRICHLET) ? -1.0 : 1.0; }
+        else if (idx[d] >= n[d]) { use[d] = par[d]; sign *= (h->bctype[2 * d + 1] == BC_DIRICHLET) ? -1.0 : 1.0; }
+    }
+    return sign * e[CI(C, use[0], use[1], use[2])];
+}
+
 static void prolong_add_level(const ovmg *h, int lev, double *phifine, const double *ecoarse)
 {
     const olevel *F = &h->lev[lev], *C = &h->lev[lev + 1];
     int i, j, k;
+    if (!h->prolong) {
+        for (k = 0; k < F->nz; ++k)
+            for (j = 0; j < F->ny; ++j)
+                for (i = 0; i < F->nx; ++i)
+                    phifine[CI(F, i, j, k)] += ecoarse[CI(C, i / 2, j / 2, h->three_d ? k / 2 : k)];
+        return;
+    }
     for (k = 0; k < F->nz; ++k)
         for (j = 0; j < F->ny; ++j)
-            for (i = 0; i < F->nx; ++i)
-                phifine[CI(F, i, j, k)] += ecoarse[CI(C, i / 2, j / 2, h->three_d ? k / 2 : k)];
+            for (i = 0; i < F->nx; ++i) {
+                int par[3], far[3], sx, sy, sz, nzs = h->three_d ? 2 : 1;
+                double v = 0.0;
+                par[0] = i / 2; par[1] = j / 2; par[2] = h->three_d ? k / 2 : k;
+                far[0] = par[0] + ((i & 1) ? 1 : -1);
+                far[1] = par[1] + ((j & 1) ? 1 : -1);
+                far[2] = par[2] + ((k & 1) ? 1 : -1);
+                for (sz = 0; sz < nzs; ++sz)
+                    for (sy = 0; sy < 2; ++sy)
+                        for (sx = 0; sx < 2; ++sx) {
+                            int idx[3];
+                            double w = (sx ? 0.25 : 0.75) * (sy ? 0.25 : 0.75) * (h->three_d ? (sz ? 0.25 : 0.75) : 1.0);
+                            idx[0] = sx ? far[0] : par[0];
+                            idx[1] = sy ? far[1] : par[1];
+                            idx[2] = sz ? far[2] : par[2];
+                            v += w * coarse_or_ghost(h, C, ecoarse, idx, par);
+                        }
+                phifine[CI(F, i, j, k)] += v;
+            }
 }
 
 /* C3 / R10. Coarse coefficients: a = mean of the children; b on a coarse face = mean of the fine
@@ -314,6 +359,7 @@ int ovmg_create(ovmg **out, int nx, int ny, int nz, double dx, double dy, double
     h->lev = (olevel *)calloc(nlev, sizeof(olevel));
     h->nlev = nlev; h->three_d = three_d;
     h->nu1 = 3; h->nu2 = 3; h->nbottom = 32;                 /* R8, R11 */
+    h->prolong = 0;                                          /* R9 */
     for (l = 0; l < nlev; ++l) {
         olevel *L = &h->lev[l];
         size_t nc;
@@ -403,6 +449,7 @@ int ovmg_set_option(ovmg *h, const char *key, double v)
     if (!strcmp(key, "nu1")) { if (v < 0) return O_ERR_ARG; h->nu1 = (int)v; return O_OK; }
     if (!strcmp(key, "nu2")) { if (v < 0) return O_ERR_ARG; h->nu2 = (int)v; return O_OK; }
     if (!strcmp(key, "bottom_sweeps")) { if (v < 1) return O_ERR_ARG; h->nbottom = (int)v; return O_OK; }
+    if (!strcmp(key, "prolong")) { if (v != 0.0 && v != 1.0) return O_ERR_ARG; h->prolong = (int)v; return O_OK; }
     return O_ERR_ARG;
 }
 

@@ -122,3 +122,52 @@ def test_c5_solve_history_norm_and_exit_rules():
     o.set_bc(p.bc_type, None)
     phi5, status5, cycles5, *_ = o.solve(np.zeros_like(p.rhs), phi0=np.ones_like(p.rhs))
     assert status5 == 0 and cycles5 == 0 and not phi5.any()
+
+
+def test_r9_trilinear_prolongation_is_exact_for_linear_fields_and_honours_the_ghost_rules():
+    """R9 option prolong = 1 (cell-centred trilinear, weights 3/4 and 1/4 per direction): pinned by what interpolation
+    must do, not by its formula -- (i) a coarse field that is linear in the coarse cell centres comes out linear in the
+    fine cell centres wherever no ghost is involved; (ii) with the Neumann ghost (+e) a constant stays a constant
+    everywhere; (iii) with the Dirichlet ghost (-e) a field that is linear in the distance from the Dirichlet face and
+    vanishes ON the face (half a coarse cell from the first centre) is reproduced exactly in the cells next to it."""
+    nx, ny, nz = 16, 8, 8
+    p = inputs.random_problem(nx, ny, nz, seed=1, bc_type=[D, N, N, N, N, N], inhomogeneous=False, spacing=(1.0, 1.0, 1.0))
+    o = Oracle.from_problem(p)
+    o.set_option("prolong", 1)
+    H = 2.0                                                     # coarse spacing (fine spacing 1)
+    K, J, I = np.meshgrid(np.arange(nz // 2), np.arange(ny // 2), np.arange(nx // 2), indexing="ij")
+    xc, yc, zc = (I + 0.5) * H, (J + 0.5) * H, (K + 0.5) * H   # coarse centres
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    xf, yf, zf = i + 0.5, j + 0.5, k + 0.5                      # fine centres
+    # (i) linear field, interior cells (fine index 1 .. n-2 in every direction: no ghost in their stencil)
+    lin_c = 0.3 + 1.7 * xc - 0.9 * yc + 0.4 * zc
+    out = o.prolong_add(np.zeros((nz, ny, nx)), lin_c)
+    lin_f = 0.3 + 1.7 * xf - 0.9 * yf + 0.4 * zf
+    inner = (slice(1, -1),) * 3
+    assert np.abs(out[inner] - lin_f[inner]).max() < 1e-13
+    # (ii) constants: exact wherever only Neumann ghosts are involved (everywhere but the cells at the Dirichlet face)
+    out = o.prolong_add(np.zeros((nz, ny, nx)), np.full((nz // 2, ny // 2, nx // 2), 2.5))
+    assert np.abs(out[:, :, 1:] - 2.5).max() < 1e-14
+    # ... and next to the Dirichlet face the ghost -e pulls the value towards the face value 0: 3/4 e - 1/4 e
+    assert np.abs(out[:, :, 0] - 1.25).max() < 1e-14
+    # (iii) e = c * x (zero on the Dirichlet face x = 0): exact for ALL cells in x, including i = 0
+    out = o.prolong_add(np.zeros((nz, ny, nx)), 3.0 * xc)
+    assert np.abs(out[:, :, :-1] - 3.0 * xf[:, :, :-1]).max() < 1e-13   # (the far x face is Neumann: last cell not linear)
+    # the correction is ADDED
+    base = np.random.default_rng(0).standard_normal((nz, ny, nx))
+    assert np.allclose(o.prolong_add(base.copy(), lin_c), base + o.prolong_add(np.zeros_like(base), lin_c), atol=1e-14)
+    o.close()
+
+
+def test_r9_trilinear_v22_converges_to_the_same_discrete_solution():
+    """The option changes the iteration, not its fixed point: V(2,2) with trilinear prolongation reaches the solution
+    V(3,3) with piecewise-constant prolongation reaches (both to 1e-12), in no more cycles on a smooth problem."""
+    p = inputs.config3(16)
+    o = Oracle.from_problem(p)
+    phi_c, st_c, cyc_c, *_ = o.solve(p.rhs, rtol=1e-12)
+    for k, v in (("prolong", 1), ("nu1", 2), ("nu2", 2)):
+        o.set_option(k, v)
+    phi_l, st_l, cyc_l, rr_l, hist = o.solve(p.rhs, rtol=1e-12)
+    assert st_c == 0 and st_l == 0 and cyc_l <= cyc_c + 2
+    assert np.abs(phi_l - phi_c).max() <= 1e-10 * np.abs(phi_c).max()
+    o.close()
