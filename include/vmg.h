@@ -100,7 +100,8 @@ int vmg_solve_batch(int n, const vmg_handle* handles, const double* const* rhs, 
 int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
 
 /* Options (key is a HOST C string): "nu1", "nu2" (pre/post red-black sweeps, default 3, 0..8),
- * "bottom_sweeps" (default 32), "graph" (1: replay the V-cycle as a CUDA graph, default; 0: plain launches),
+ * "bottom_sweeps" (default 32), "prolong" (0: piecewise-constant prolongation, default; 1: cell-centred trilinear,
+ *   weights 3/4 and 1/4 per direction, ghost value -e at Dirichlet and +e at Neumann faces), "graph" (1: replay the V-cycle as a CUDA graph, default; 0: plain launches),
  * "tail" (1: the coarsest levels run in one single-CTA launch, default; 0: one kernel per step),
  * "snake" (1: consecutive whole-level kernels walk the level in opposite z-directions so that each starts on
  *   what the previous one left in L2, default; 0: always ascending),

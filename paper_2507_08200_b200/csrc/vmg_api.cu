@@ -283,6 +283,7 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
     for (int f = 0; f < 6; ++f)
         if (type[f] != VMG_BC_DIRICHLET && type[f] != VMG_BC_NEUMANN) return VMG_ERR_ARG;
     for (int f = 0; f < 6; ++f) {
+        if (h->bctype[f] != type[f]) h->graph_valid = false;   // the trilinear prolongation kernels carry the types by value
         h->bctype[f] = type[f];
         bool active = f < 4 || h->three_d;
         h->bc_has_value[f] = active && value && value[f];
@@ -303,6 +304,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     if (!strcmp(key, "nu1")) { if (iv < 0 || iv > 8) return VMG_ERR_ARG; h->nu1 = iv; }
     else if (!strcmp(key, "nu2")) { if (iv < 0 || iv > 8) return VMG_ERR_ARG; h->nu2 = iv; }
     else if (!strcmp(key, "bottom_sweeps")) { if (iv < 1) return VMG_ERR_ARG; h->nbottom = iv; }
+    else if (!strcmp(key, "prolong")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->prolong = iv; }
     else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
     else if (!strcmp(key, "blocked")) { h->use_blocked = iv != 0; }
     else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }

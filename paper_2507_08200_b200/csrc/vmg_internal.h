@@ -57,6 +57,7 @@ struct vmg_s {
     bool bc_has_value[6] = {false, false, false, false, false, false};
     bool have_coeffs = false, have_bc = false, dinv_dirty = true;
     int nu1 = 3, nu2 = 3, nbottom = 32;
+    int prolong = 0;              // 0: piecewise constant (R9 default), 1: trilinear
     int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200
     double l2_persist_mb = 24.0;  // L2 set aside for the level-0 face weights (0: none); see apply_l2_window
     bool l2_applied = false, l2_window_set = false;

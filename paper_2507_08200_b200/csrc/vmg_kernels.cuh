@@ -418,6 +418,55 @@ __global__ void prolong_correct_kernel(Geom G, Geom CG, double* __restrict__ phi
     if (t < G.n) prolong_one(G, CG, phi, e, sz, t);
 }
 
+// S4, option prolong = 1 (reading R9): cell-centred trilinear prolongation + correction.  Per direction the fine cell
+// lies a quarter of a coarse cell from its parent's centre, towards the next coarse cell if its index is odd, towards
+// the previous one if even: weights 3/4 (parent), 1/4 (that neighbour), products over the directions (8 coarse values,
+// 4 in 2-D).  A neighbour beyond a domain face is a ghost: -e(parent) at a Dirichlet face, +e(parent) at a Neumann
+// face.  Same loop order as the oracle's statement of R9 (z, y, x; parent first).
+struct ProlongBC { int dirichlet[6]; };
+
+__device__ __forceinline__ double trilinear_value(const int par[3], const int fine[3], const int n[3], int sz, const ProlongBC& bc,
+                                                  const double* e, long long (*at)(const void*, int, int, int), const void* geom)
+{
+    double v = 0.0;
+    const int nzs = sz == 2 ? 2 : 1;
+    for (int c = 0; c < nzs; ++c)
+        for (int b = 0; b < 2; ++b)
+            for (int a = 0; a < 2; ++a) {
+                const int s[3] = {a, b, c};
+                int use[3];
+                double sign = 1.0;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    int idx = s[d] ? par[d] + ((fine[d] & 1) ? 1 : -1) : par[d];
+                    if (idx < 0) { idx = par[d]; sign *= bc.dirichlet[2 * d] ? -1.0 : 1.0; }
+                    else if (idx >= n[d]) { idx = par[d]; sign *= bc.dirichlet[2 * d + 1] ? -1.0 : 1.0; }
+                    use[d] = idx;
+                }
+                const double w = (a ? 0.25 : 0.75) * (b ? 0.25 : 0.75) * (sz == 2 ? (c ? 0.25 : 0.75) : 1.0);
+                v += w * (sign * e[at(geom, use[0], use[1], use[2])]);
+            }
+    return v;
+}
+
+__device__ inline long long at_geom(const void* g, int i, int j, int k) { return cell_at(*(const Geom*)g, i, j, k); }
+
+__device__ __forceinline__ void prolong_trilinear_one(const Geom& G, const Geom& CG, double* phi, const double* e, int sz,
+                                                      const ProlongBC& bc, long long t)
+{
+    int i, j, k;
+    unflatten(G, t, i, j, k);
+    const int par[3] = {i >> 1, j >> 1, sz == 2 ? (k >> 1) : k}, fine[3] = {i, j, k}, n[3] = {CG.nx, CG.ny, CG.nz};
+    phi[cell_at(G, i, j, k)] += trilinear_value(par, fine, n, sz, bc, e, at_geom, &CG);
+}
+
+__global__ void prolong_trilinear_kernel(Geom G, Geom CG, double* __restrict__ phi, const double* __restrict__ e, int sz, ProlongBC bc)
+{
+    grid_dependency_wait();
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < G.n) prolong_trilinear_one(G, CG, phi, e, sz, bc, t);
+}
+
 // ------------------------------------------------------------------------------------------------
 // S6. Infinity norms: warp shuffle -> block reduce -> one atomicMax on the bit pattern (non-negative
 // doubles order like unsigned 64-bit integers; a NaN's pattern is larger than every finite value, so

@@ -132,11 +132,22 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
     ++*count;
 }
 
+inline ProlongBC prolong_bc(const vmg_s* h)
+{
+    ProlongBC bc;
+    for (int f = 0; f < 6; ++f) bc.dirichlet[f] = h->bctype[f] == VMG_BC_DIRICHLET;
+    return bc;
+}
+
 inline void plain_prolong_correct(vmg_s* h, int l, long long* count)
 {
     VmgLevel& L = h->lev[l];
-    launch_pdl(h, prolong_correct_kernel, grid_for(L.n), kThreads, 0, L.G, h->lev[l + 1].G, cur_phi(L), cur_phi(h->lev[l + 1]),
-               h->three_d ? 2 : 1);
+    if (h->prolong)
+        launch_pdl(h, prolong_trilinear_kernel, grid_for(L.n), kThreads, 0, L.G, h->lev[l + 1].G, cur_phi(L), cur_phi(h->lev[l + 1]),
+                   h->three_d ? 2 : 1, prolong_bc(h));
+    else
+        launch_pdl(h, prolong_correct_kernel, grid_for(L.n), kThreads, 0, L.G, h->lev[l + 1].G, cur_phi(L), cur_phi(h->lev[l + 1]),
+                   h->three_d ? 2 : 1);
     ++*count;
 }
 
@@ -200,6 +211,7 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
         if (l >= tail) off += tail_level_doubles(T.n, T.guard);
     }
     g.nu1 = h->nu1; g.nu2 = h->nu2; g.nbottom = h->nbottom; g.sz = h->three_d ? 2 : 1;
+    g.prolong = h->prolong; g.bc = prolong_bc(h);
     g.whole = first == 0;
     g.norm_out = first == 0 ? norm_out : nullptr;
     ProfScope ps(h, VMG_PC_COARSE, count);
@@ -365,12 +377,16 @@ inline void enqueue_down(vmg_s* h, int l, long long* count)
 inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long* count)
 {
     if (h->nu2 > 0 && blocked_ok(h, l)) {
+        if (h->prolong) {   // the blocked passes can only add a piecewise-constant correction while loading
+            ProfScope ps(h, l == 0 ? VMG_PC_PROLONG0 : VMG_PC_COARSE, count);
+            plain_prolong_correct(h, l, count);
+        }
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         bool fuse = l == 0 && norm_out != nullptr;
-        blocked_sweeps(h, l, 2 * h->nu2, 0, true, fuse ? BT_NORM : BT_NONE, norm_out, count);
+        blocked_sweeps(h, l, 2 * h->nu2, 0, !h->prolong, fuse ? BT_NORM : BT_NONE, norm_out, count);
         return fuse;
     }
-    if (h->nu2 >= 1) {   // the correction rides on the first half-sweep (smooth_colour_prolong_kernel)
+    if (h->nu2 >= 1 && !h->prolong) {   // the correction rides on the first half-sweep (smooth_colour_prolong_kernel)
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         VmgLevel& L = h->lev[l];
         long long nt = (long long)L.G.ne * L.ny * L.nz;
@@ -384,6 +400,8 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         ProfScope ps(h, l == 0 ? VMG_PC_PROLONG0 : VMG_PC_COARSE, count);
         plain_prolong_correct(h, l, count);
     }
+    ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
+    plain_smooth(h, l, h->nu2, count);
     return false;
 }
 

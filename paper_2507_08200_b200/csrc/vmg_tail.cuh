@@ -26,6 +26,8 @@ struct TailArgs {
     int ns;                    // 0 (levels lev[ns..nl-1] run in shared memory; a cluster-wide variant for larger levels,
                                // barrier.cluster between half-sweeps on global arrays, measured slower than graph launches)
     int nu1, nu2, nbottom, sz; // sz = 2 in 3-D, 1 in 2-D (children per coarse cell along z)
+    int prolong;               // 0: piecewise constant, 1: trilinear (R9 option)
+    ProlongBC bc;              // boundary types (trilinear ghosts)
     int whole;                 // 1: lev[0] is level 0 of the hierarchy (phi is an initial guess, not zero)
     unsigned long long* norm_out;   // whole == 1: ||rhs - A phi||_inf bits after the cycle (may be NULL)
 };
@@ -45,6 +47,13 @@ struct TailSmem {
         phi = p; rhs = p + st; dinv = p + 2 * st; wx = p + 3 * st; wy = p + 4 * st; wz = p + 5 * st;
     }
 };
+
+// natural-layout index of a shared-memory level (trilinear_value's accessor)
+__device__ inline long long at_tail(const void* l, int i, int j, int k)
+{
+    const TailLevel& L = *(const TailLevel*)l;
+    return i + L.nx * (j + L.ny * k);
+}
 
 __device__ __forceinline__ double tail_nb_sum(const TailSmem& s, const TailLevel& L, int c)
 {
@@ -174,9 +183,13 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         const TailLevel& L = g.lev[l];
         const TailLevel& C = g.lev[l + 1];
         TailSmem s(tail_smem, L), c(tail_smem, C);
-        for (int t = tid; t < L.n; t += nth) {     // prolongation + correction (piecewise constant, R9)
+        for (int t = tid; t < L.n; t += nth) {     // prolongation + correction (R9: piecewise constant, or trilinear)
             int i = t % L.nx, j = (t / L.nx) % L.ny, k = t / L.nxy;
-            s.phi[t] += c.phi[(i >> 1) + C.nx * ((j >> 1) + C.ny * (g.sz == 2 ? (k >> 1) : k))];
+            if (g.prolong) {
+                const int par[3] = {i >> 1, j >> 1, g.sz == 2 ? (k >> 1) : k}, fine[3] = {i, j, k}, n[3] = {C.nx, C.ny, C.nz};
+                s.phi[t] += trilinear_value(par, fine, n, g.sz, g.bc, c.phi, at_tail, &C);
+            } else
+                s.phi[t] += c.phi[(i >> 1) + C.nx * ((j >> 1) + C.ny * (g.sz == 2 ? (k >> 1) : k))];
         }
         __syncthreads();
         tail_smooth(s, L, g.nu2);

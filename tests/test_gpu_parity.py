@@ -147,7 +147,7 @@ def solve_both(p, **opts):
     o = Oracle.from_problem(p)
     s, d = b.from_problem(p)
     for k, v in opts.items():
-        o.set_option(k, v) if k in ("nu1", "nu2", "bottom_sweeps") else None
+        o.set_option(k, v) if k in ("nu1", "nu2", "bottom_sweeps", "prolong") else None
     for k, v in opts.items():
         s.set_option(k, v)
     phi_o, st_o, cyc_o, rr_o, hist_o = o.solve(p.rhs, rtol=p.rtol, max_vcycles=p.max_vcycles)
@@ -198,7 +198,8 @@ def test_config5_full_size_parity():
                                   dict(tail=0), dict(blocked=0, tail=0, graph=0), dict(block_min_cells=0),
                                   dict(block_min_cells=0, graph=0, nu1=2, nu2=4), dict(block_min_cells=0, nu1=1, nu2=2),
                                   dict(block_min_cells=0, nu1=4, nu2=1, tail=0), dict(snake=0), dict(l2_persist=0, snake=0, graph=0),
-                                  dict(blocked=1, block_min_cells=0), dict(nu1=3, nu2=1)])
+                                  dict(blocked=1, block_min_cells=0), dict(nu1=3, nu2=1), dict(prolong=1, nu1=2, nu2=2), dict(prolong=1),
+                                  dict(prolong=1, blocked=1, block_min_cells=0), dict(prolong=1, tail=0, graph=0)])
 def test_options_parity(opts):
     check_parity(inputs.random_problem(48, 24, 48, seed=3, bc_type=[D, D, N, N, N, D]), **opts)
 
@@ -404,4 +405,28 @@ def test_full_size_residual_property_without_the_oracle(make, rho):
     h = np.array(hist)
     live = h[1:] > 1e-11
     assert np.all(h[1:][live] < rho * h[:-1][live])
+    s.destroy()
+
+
+@pytest.mark.parametrize("dims", [(40, 24, 16), (48, 40, 1), (72, 40, 24), (5, 3, 4)])
+def test_trilinear_prolongation_matches_oracle(dims):
+    """Option prolong = 1 (reading R9): the stand-alone kernel on every level, all boundary kinds (MIXED has Dirichlet and
+    Neumann faces in every direction), 2-D and odd coarse sizes; then a whole V-cycle, which also runs the shared-memory
+    tail's version."""
+    b = _binding()
+    p = inputs.random_problem(*dims, seed=21, bc_type=MIXED)
+    o = Oracle.from_problem(p)
+    s, d = b.from_problem(p)
+    o.set_option("prolong", 1)
+    s.set_option("prolong", 1)
+    rng = np.random.default_rng(5)
+    for lev in range(o.num_levels - 1):
+        nx, ny, nz = o.level_dims(lev)
+        cnx, cny, cnz = o.level_dims(lev + 1)
+        phi, e = rng.standard_normal((nz, ny, nx)), rng.standard_normal((cnz, cny, cnx))
+        got = s.step_prolong_correct(lev, dev(phi), dev(e)).cpu().numpy()
+        assert rel(got, o.prolong_add(phi, e, lev)) <= STEP_TOL
+    bt = o.fold_bc(p.rhs)
+    phi0 = rng.standard_normal(p.rhs.shape)
+    assert rel(s.step_vcycle(dev(phi0), dev(bt)).cpu().numpy(), o.vcycle(phi0, bt)) <= 1e-12
     s.destroy()
