@@ -187,6 +187,55 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def timestep_leg(binding, torch, p, d, d_bc, dev, s, flush, nsteps: int = 3, rtol: float = 1e-10):
+    """20 elliptic solves per (single-corrector) time step on the 256x128x128 grid, all through the public calls:
+      Poisson        config 3 (a = 0, b = 1, electrode Dirichlet values),
+      15 species     alpha a phi - beta_k div(b grad phi) = f with config 4's a = n_e/dt, b = (5/3) D_e n_e and
+                     beta_k = 15 diffusivity ratios over two decades (same arrays, different operator per species),
+      energy         config 4 itself,
+      3 x photoion.  a = 1 (array), alpha = (lambda_j p)^2 for three absorption lengths, b = 1 (NULL), random source.
+    Right-hand sides grow by 1 % per step; every solve starts from its field of the previous step (PAPER.md:142-148:
+    the correctors re-solve with slowly changing data).  Step 0 (cold start) is the warm-up."""
+    from paper_2507_08200_b200 import inputs
+    p4 = inputs.config4(p.ny)
+    up = lambda x: torch.from_numpy(np.ascontiguousarray(x)).to(dev)
+    d4 = {k: up(getattr(p4, k)) for k in ("a", "bx", "by", "bz", "rhs")}
+    ones = torch.ones_like(d["rhs"])
+    gen = torch.Generator(device=dev).manual_seed(1234)
+    photo_rhs = torch.randn(d["rhs"].shape, generator=gen, device=dev, dtype=torch.float64)
+    betas = np.logspace(-1.0, 1.0, 15)
+    lambdas2 = [1.0e2, 1.0e3, 1.0e4]
+    eqs = [("poisson", lambda: (s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta), s.set_bc(p.bc_type, d_bc)), d["rhs"])]
+    for b_k in betas:
+        eqs.append(("species", lambda b_k=b_k: (s.set_coeffs(d4["a"], d4["bx"], d4["by"], d4["bz"], 1.0, float(b_k)), s.set_bc(p4.bc_type, None)), d4["rhs"]))
+    eqs.append(("energy", lambda: (s.set_coeffs(d4["a"], d4["bx"], d4["by"], d4["bz"], 1.0, 1.0), s.set_bc(p4.bc_type, None)), d4["rhs"]))
+    for l2 in lambdas2:
+        eqs.append(("photo", lambda l2=l2: (s.set_coeffs(ones, None, None, None, l2, 1.0), s.set_bc(p4.bc_type, None)), photo_rhs))
+    fields = [torch.zeros_like(d["rhs"]) for _ in eqs]
+    times, cycles = [], []
+    for step in range(nsteps + 1):
+        scale = 1.0 + 0.01 * step
+        flush.fill_(1.0)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ncyc = 0
+        for (name, setup, rhs), phi in zip(eqs, fields):
+            setup()
+            st = s.solve(rhs * scale, phi, rtol=rtol, max_vcycles=50)
+            assert st in (0, 2), (name, st)
+            ncyc += s.get_info()[0]
+        e1.record()
+        e1.synchronize()
+        if step > 0:
+            times.append(e0.elapsed_time(e1))
+            cycles.append(ncyc)
+    ms = float(np.mean(times))
+    return {"ms_per_time_step": ms, "time_steps_per_s": 1e3 / ms, "solves_per_time_step": len(eqs),
+            "vcycles_per_time_step": float(np.mean(cycles)), "rtol": rtol,
+            "sequence": "Poisson + 15 species + energy + 3 photoionisation; set_coeffs + set_bc + warm-started solve each; one handle"}
+
+
 # ----------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ----------------------------------------------------------------------------------------------------
@@ -344,6 +393,13 @@ def run_vmg(args):
         for sv in bsolvers:
             sv.destroy()
 
+    # one time step of the paper's scheme (Eq. 9-10): Poisson, 15
+    # species, electron energy and three photoionisation Helmholtz solves, each vmg_set_coeffs + vmg_set_bc +
+    # vmg_solve on ONE handle, warm-started from the previous step's field while the data drift by 1 % per step
+    timestep = None
+    if args.config == 3 and not args.no_timestep:
+        timestep = timestep_leg(binding, torch, p, d, d_bc, dev, s, flush)
+
     # end to end through the C-ABI with host buffers
     etimes, ecycles, _ = timed(step_e2e, args.steps, max(1, min(args.warmup, 2)))
     etotal = max_over_ranks(float(etimes.sum()), dist, dev)
@@ -370,6 +426,7 @@ def run_vmg(args):
                      "launches_per_pass": sm_launches / max(2 * n_prof_cycles, 1)},
         "kernel_classes": klass,
         "batched": batched,
+        "timestep": timestep,
         "e2e": {"value": e2e_value, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": etotal / args.steps * 1e3},
         "gpu_launches": int(launches),
@@ -398,6 +455,7 @@ def main():
     ap.add_argument("--impl", default="vmg", choices=["vmg", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-timestep", action="store_true", help="skip the per-time-step sequence leg")
     ap.add_argument("--batch", type=int, default=8, help="K for the batched multi-component leg (0/1: skip)")
     ap.add_argument("--opt", action="append", default=[], help="vmg_set_option key=value (experiments)")
     args = ap.parse_args()
