@@ -47,6 +47,7 @@ def lib():
         _lib.ovmg_set_bc.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(_dp)]
         _lib.ovmg_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_double]
         _lib.ovmg_solve.argtypes = [C.c_void_p, _dp, _dp, C.c_double, C.c_int]
+        _lib.ovmg_solve_pcg.argtypes = [C.c_void_p, _dp, _dp, C.c_double, C.c_int]
         _lib.ovmg_get_info.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_double), _dp]
         _lib.ovmg_num_levels.argtypes = [C.c_void_p]
         _lib.ovmg_level_dims.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int)]
@@ -122,11 +123,15 @@ class Oracle:
     def set_option(self, key: str, v: float):
         self._chk(lib().ovmg_set_option(self._h, key.encode(), float(v)), "set_option")
 
-    def solve(self, rhs, phi0=None, rtol: float = 1e-12, max_vcycles: int = 50):
+    def solve_pcg(self, rhs, phi0=None, rtol: float = 1e-12, max_iter: int = 50):
+        """MG-preconditioned conjugate gradients. Returns (phi, status, iterations, relres, history)."""
+        return self.solve(rhs, phi0, rtol, max_iter, _fn="ovmg_solve_pcg")
+
+    def solve(self, rhs, phi0=None, rtol: float = 1e-12, max_vcycles: int = 50, _fn: str = "ovmg_solve"):
         """Returns (phi, status, cycles, relres, history)."""
         rhs = _c(rhs)
         phi = np.zeros_like(rhs) if phi0 is None else np.array(phi0, dtype=np.float64, order="C")
-        status = lib().ovmg_solve(self._h, _p(rhs), _p(phi), rtol, max_vcycles)
+        status = getattr(lib(), _fn)(self._h, _p(rhs), _p(phi), rtol, max_vcycles)
         self._chk(status, "solve") if status not in (-5,) else None
         cyc, rr = C.c_int(), C.c_double()
         hist = np.zeros(max_vcycles + 1)

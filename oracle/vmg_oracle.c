@@ -50,6 +50,7 @@ typedef struct ovmg {
     int have_coeffs, have_bc;
     int nu1, nu2, nbottom;
     int prolong;                /* 0: piecewise constant (R9 default), 1: trilinear (R9 option) */
+    int symmetric;              /* 1: symmetric V-cycle (post-smoothing and second half of the bottom black->red) */
     int cycles, status;
     double relres;
     double *hist;
@@ -134,13 +135,16 @@ static void residual_level(const ovmg *h, int lev, const double *phi, const doub
             }
 }
 
-/* C2. One red-black Gauss-Seidel sweep: red = (i+j+k) even first, then black; no over-relaxation. */
-static void smooth_level(const ovmg *h, int lev, double *phi, const double *rhs, int nsweeps)
+/* C2. One red-black Gauss-Seidel sweep: red = (i+j+k) even first, then black; no over-relaxation.
+ * first = 1 runs every sweep black first, then red: the adjoint order, used by the post-smoothing of the symmetric
+ * V-cycle that preconditions conjugate gradients (ovmg_solve_pcg). */
+static void smooth_level_order(const ovmg *h, int lev, double *phi, const double *rhs, int nsweeps, int first)
 {
     const olevel *L = &h->lev[lev];
-    int s, colour, i, j, k;
+    int s, c2, colour, i, j, k;
     for (s = 0; s < nsweeps; ++s)
-        for (colour = 0; colour < 2; ++colour) {
+        for (c2 = 0; c2 < 2; ++c2) {
+            colour = (first + c2) & 1;
 #pragma omp parallel for collapse(2) private(i)
             for (k = 0; k < L->nz; ++k)
                 for (j = 0; j < L->ny; ++j)
@@ -151,6 +155,11 @@ static void smooth_level(const ovmg *h, int lev, double *phi, const double *rhs,
                         phi[CI(L, i, j, k)] = (rhs[CI(L, i, j, k)] + nbsum(L, phi, i, j, k, w)) / D;
                     }
         }
+}
+
+static void smooth_level(const ovmg *h, int lev, double *phi, const double *rhs, int nsweeps)
+{
+    smooth_level_order(h, lev, phi, rhs, nsweeps, 0);
 }
 
 /* C3. Restriction: coarse rhs = mean of the 8 (4 in 2-D) children of the fine residual. */
@@ -302,9 +311,14 @@ static void fold_bc(const ovmg *h, const double *rhs, double *bt)
 static void vcycle(ovmg *h, int lev, double *phi, const double *rhs)
 {
     olevel *L = &h->lev[lev];
+    const int back = h->symmetric ? 1 : 0;          /* colour order of the second half of the cycle */
     if (lev == h->nlev - 1) {                       /* bottom: fixed sweeps from zero (R11) */
         memset(phi, 0, ncell(L) * sizeof(double));
-        smooth_level(h, lev, phi, rhs, h->nbottom);
+        if (!h->symmetric) smooth_level(h, lev, phi, rhs, h->nbottom);
+        else {                                      /* half of them red->black, the other half black->red */
+            smooth_level_order(h, lev, phi, rhs, h->nbottom / 2, 0);
+            smooth_level_order(h, lev, phi, rhs, h->nbottom - h->nbottom / 2, 1);
+        }
         return;
     }
     smooth_level(h, lev, phi, rhs, h->nu1);
@@ -313,7 +327,7 @@ static void vcycle(ovmg *h, int lev, double *phi, const double *rhs)
     memset(h->lev[lev + 1].phi, 0, ncell(&h->lev[lev + 1]) * sizeof(double));
     vcycle(h, lev + 1, h->lev[lev + 1].phi, h->lev[lev + 1].rhs);
     prolong_add_level(h, lev, phi, h->lev[lev + 1].phi);
-    smooth_level(h, lev, phi, rhs, h->nu2);
+    smooth_level_order(h, lev, phi, rhs, h->nu2, back);
 }
 
 static double norm_inf(const double *v, size_t n)
@@ -360,6 +374,7 @@ int ovmg_create(ovmg **out, int nx, int ny, int nz, double dx, double dy, double
     h->nlev = nlev; h->three_d = three_d;
     h->nu1 = 3; h->nu2 = 3; h->nbottom = 32;                 /* R8, R11 */
     h->prolong = 0;                                          /* R9 */
+    h->symmetric = 0;
     for (l = 0; l < nlev; ++l) {
         olevel *L = &h->lev[l];
         size_t nc;
@@ -449,6 +464,7 @@ int ovmg_set_option(ovmg *h, const char *key, double v)
     if (!strcmp(key, "nu1")) { if (v < 0) return O_ERR_ARG; h->nu1 = (int)v; return O_OK; }
     if (!strcmp(key, "nu2")) { if (v < 0) return O_ERR_ARG; h->nu2 = (int)v; return O_OK; }
     if (!strcmp(key, "bottom_sweeps")) { if (v < 1) return O_ERR_ARG; h->nbottom = (int)v; return O_OK; }
+    if (!strcmp(key, "symmetric")) { if (v != 0.0 && v != 1.0) return O_ERR_ARG; h->symmetric = (int)v; return O_OK; }
     if (!strcmp(key, "prolong")) { if (v != 0.0 && v != 1.0) return O_ERR_ARG; h->prolong = (int)v; return O_OK; }
     return O_ERR_ARG;
 }
@@ -499,6 +515,85 @@ int ovmg_solve(ovmg *h, const double *rhs, double *phi, double rtol, int max_vcy
         }
     }
     return h->status = O_MAXCYCLES;
+}
+
+/* conjugate gradients on A phi = btilde, preconditioned by ONE symmetric V-cycle from a zero
+ * guess (pre-smoothing red->black, post-smoothing black->red, nu1 = nu2, the bottom's sweeps half and half; R = P^T/8)
+ * -- the remedy for the diffusion-dominated high-contrast regime in which plain V-cycles contract slowly (R17) and for
+ * which the paper falls back to HYPRE.  Textbook PCG (Hestenes-Stiefel with preconditioner):
+ *     r = b - A x;  z = M^-1 r;  p = z;  rho = <r, z>
+ *     repeat:  q = A p;  alpha = rho / <p, q>;  x += alpha p;  r -= alpha q;  relres = ||r||_inf / ||b||_inf;
+ *              z = M^-1 r;  rho' = <r, z>;  p = z + (rho'/rho) p;  rho = rho'
+ * hist[c] is the norm of the recurrence residual after c iterations; exit rules as in ovmg_solve. */
+static double dot(const double *u, const double *v, size_t n)
+{
+    double s = 0.0;
+    size_t i;
+    for (i = 0; i < n; ++i) s += u[i] * v[i];
+    return s;
+}
+
+int ovmg_solve_pcg(ovmg *h, const double *rhs, double *phi, double rtol, int max_iter)
+{
+    olevel *L;
+    double nb, rho, *r, *z, *p, *q;
+    size_t n, i;
+    int c, slow = 0, keep_sym, status = O_MAXCYCLES;
+    if (!h || !rhs || !phi || max_iter < 0) return O_ERR_ARG;
+    if (!h->have_coeffs || !h->have_bc) return O_ERR_STATE;
+    if (singular(h)) return O_ERR_SINGULAR;
+    if (h->nu1 != h->nu2) return O_ERR_ARG;          /* the preconditioner must be symmetric */
+    L = &h->lev[0];
+    n = ncell(L);
+    free(h->hist);
+    h->hist = (double *)calloc((size_t)max_iter + 1, sizeof(double));
+    h->hist_len = 0; h->cycles = 0; h->relres = 0.0;
+    r = (double *)malloc(4 * n * sizeof(double));
+    if (!r) return O_ERR_ARG;
+    z = r + n; p = z + n; q = p + n;
+    fold_bc(h, rhs, q);                               /* q = btilde for a moment */
+    nb = norm_inf(q, n);
+    if (nb == 0.0) {
+        memset(phi, 0, n * sizeof(double));
+        h->hist[0] = 0.0; h->hist_len = 1;
+        free(r);
+        return h->status = O_OK;
+    }
+    residual_level(h, 0, phi, q, r);                  /* r = btilde - A phi */
+    h->hist[0] = h->relres = norm_inf(r, n) / nb;
+    h->hist_len = 1;
+    if (!(h->relres == h->relres) || isinf(h->relres)) { free(r); return h->status = O_ERR_DIVERGED; }
+    if (rtol > 0.0 && h->relres <= rtol) { free(r); return h->status = O_OK; }
+    keep_sym = h->symmetric;
+    h->symmetric = 1;
+    memset(z, 0, n * sizeof(double));
+    vcycle(h, 0, z, r);
+    memcpy(p, z, n * sizeof(double));
+    rho = dot(r, z, n);
+    for (c = 1; c <= max_iter; ++c) {
+        double alpha, rho2, beta;
+        apply_level(h, 0, p, q);
+        alpha = rho / dot(p, q, n);
+        for (i = 0; i < n; ++i) { phi[i] += alpha * p[i]; r[i] -= alpha * q[i]; }
+        h->hist[c] = h->relres = norm_inf(r, n) / nb;
+        h->hist_len = c + 1; h->cycles = c;
+        if (!(h->relres == h->relres) || isinf(h->relres)) { status = O_ERR_DIVERGED; break; }
+        if (rtol > 0.0) {
+            if (h->relres <= rtol) { status = O_OK; break; }
+            slow = (h->hist[c] >= 0.9 * h->hist[c - 1]) ? slow + 1 : 0;
+            if (slow >= 3) { status = O_STALLED; break; }
+        }
+        if (c == max_iter) break;
+        memset(z, 0, n * sizeof(double));
+        vcycle(h, 0, z, r);
+        rho2 = dot(r, z, n);
+        beta = rho2 / rho;
+        rho = rho2;
+        for (i = 0; i < n; ++i) p[i] = z[i] + beta * p[i];
+    }
+    h->symmetric = keep_sym;
+    free(r);
+    return h->status = status;
 }
 
 int ovmg_get_info(const ovmg *h, int *cycles, double *relres, double *history)
