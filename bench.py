@@ -356,6 +356,14 @@ def run_vmg(args):
     ncyc = float(np.mean(scycles))
     bytes_solve = ncyc * wm["bytes_per_cycle"] + wm["bytes_solve_fixed"]
 
+    # MG-preconditioned conjugate gradients: the same solve through vmg_solve_pcg
+    def solve_pcg_only():
+        phi.zero_()
+        return s.solve_pcg(d["rhs"], phi, rtol=p.rtol if p.rtol > 0 else 1e-12, max_iter=max(p.max_vcycles, 60))
+    ptimes_, piters, _ = timed(solve_pcg_only, max(2, min(args.steps, 5)), 1)
+    pcg = {"solve_ms": float(np.mean(ptimes_)) * 1e3, "solves_per_s": world / float(np.mean(ptimes_)), "iterations": float(np.mean(piters)),
+           "relres": s.get_info()[1], "note": "one symmetric V-cycle, one operator application and two dot products per iteration"}
+
     # batched multi-component solves (the paper's own optimisation): K independent
     # solves of the same workload, one handle and one stream each, advanced in lock-step by vmg_solve_batch
     batched = None
@@ -425,6 +433,7 @@ def run_vmg(args):
                      "achieved_bytes_per_pass": B_SMOOTH_PASS * n0, "peak_source": peak_src,
                      "launches_per_pass": sm_launches / max(2 * n_prof_cycles, 1)},
         "kernel_classes": klass,
+        "pcg": pcg,
         "batched": batched,
         "timestep": timestep,
         "e2e": {"value": e2e_value, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

@@ -95,12 +95,22 @@ int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max
 int vmg_solve_batch(int n, const vmg_handle* handles, const double* const* rhs, double* const* phi, double rtol,
                     int max_vcycles, int* status);
 
+/* Conjugate gradients preconditioned by one symmetric V-cycle -- for the diffusion-dominated,
+ * high-contrast regime in which the plain V-cycle iteration of vmg_solve contracts slowly or not at all and for which
+ * the paper falls back to HYPRE.  Same arguments, layout, exit rules and status codes as vmg_solve;
+ * max_iter counts CG iterations (one V-cycle, one operator application and two dot products each); the history holds
+ * ||r||_inf / ||btilde||_inf of the recurrence residual.  The preconditioner is the V-cycle of vmg_solve with the
+ * post-smoothing sweeps (and the second half of the bottom sweeps) run black -> red, from a zero guess; it needs
+ * nu1 == nu2 (VMG_ERR_ARG otherwise).  Allocates three more level-0 arrays on first use (VMG_ERR_ALLOC). */
+int vmg_solve_pcg(vmg_handle h, const double* rhs, double* phi, double rtol, int max_iter);
+
 /* Result of the last vmg_solve.  cycles, relres: HOST scalars (may be NULL).  history: HOST array of at
  * least cycles+1 doubles (relative residual before the first cycle and after each cycle) or NULL. */
 int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
 
 /* Options (key is a HOST C string): "nu1", "nu2" (pre/post red-black sweeps, default 3, 0..8),
- * "bottom_sweeps" (default 32), "prolong" (0: piecewise-constant prolongation, default; 1: cell-centred trilinear,
+ * "bottom_sweeps" (default 32), "symmetric" (1: post-smoothing and the second half of the bottom sweeps run black -> red,
+ *   which makes one V-cycle from zero a symmetric operator; default 0; vmg_solve_pcg switches it on for itself), "prolong" (0: piecewise-constant prolongation, default; 1: cell-centred trilinear,
  *   weights 3/4 and 1/4 per direction, ghost value -e at Dirichlet and +e at Neumann faces), "graph" (1: replay the V-cycle as a CUDA graph, default; 0: plain launches),
  * "tail" (1: the coarsest levels run in one single-CTA launch, default; 0: one kernel per step),
  * "snake" (1: consecutive whole-level kernels walk the level in opposite z-directions so that each starts on

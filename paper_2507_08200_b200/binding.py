@@ -17,7 +17,7 @@ STATUS = {0: "OK", 1: "MAXCYCLES", 2: "STALLED", -1: "ERR_ARG", -2: "ERR_SIZE", 
           -4: "ERR_SINGULAR", -5: "ERR_DIVERGED", -6: "ERR_CUDA", -7: "ERR_ALLOC"}
 
 # every symbol include/vmg.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_solve", "vmg_solve_batch", "vmg_get_info", "vmg_set_option",
+SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_solve", "vmg_solve_batch", "vmg_solve_pcg", "vmg_get_info", "vmg_set_option",
            "vmg_destroy", "vmg_strerror", "vmg_last_cuda_error", "vmg_num_levels", "vmg_level_dims",
            "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
            "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_down", "vmg_step_up", "vmg_step_vcycle", "vmg_step_norm_inf",
@@ -40,6 +40,7 @@ def load():
     lib.vmg_set_coeffs.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_double, C.c_double]
     lib.vmg_set_bc.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(_vp)]
     lib.vmg_solve.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int]
+    lib.vmg_solve_pcg.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int]
     lib.vmg_solve_batch.argtypes = [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp), C.c_double, C.c_int,
                                     C.POINTER(C.c_int)]
     lib.vmg_get_info.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -153,6 +154,10 @@ class Vmg:
     def solve(self, rhs, phi, rtol: float = 1e-12, max_vcycles: int = 50) -> int:
         """phi: initial guess in, solution out (in place). Returns the status code (>= 0)."""
         return self._chk(self._lib.vmg_solve(self._h, _ptr(rhs), _ptr(phi), rtol, max_vcycles), "vmg_solve")
+
+    def solve_pcg(self, rhs, phi, rtol: float = 1e-12, max_iter: int = 50) -> int:
+        """MG-preconditioned conjugate gradients; phi: initial guess in, solution out. Returns the status code (>= 0)."""
+        return self._chk(self._lib.vmg_solve_pcg(self._h, _ptr(rhs), _ptr(phi), rtol, max_iter), "vmg_solve_pcg")
 
     def get_info(self):
         cyc, rr = C.c_int(), C.c_double()

@@ -3,6 +3,7 @@
 #include "vmg_internal.h"
 #include "vmg_kernels.cuh"
 #include "vmg_sched.cuh"
+#include "vmg_pcg.cuh"
 
 #include <cmath>
 #include <cstring>
@@ -120,7 +121,7 @@ int apply_l2_window(vmg_s* h)
     CUDA_TRY(h, cudaStreamSetAttribute(h->stream, cudaStreamAttributeAccessPolicyWindow, &a));
     if (!want) CUDA_TRY(h, cudaCtxResetPersistingL2Cache());
     h->l2_window_set = want != 0;
-    h->graph_valid = false;
+    { h->graph_valid = false; ++h->graph_epoch; }
     return VMG_OK;
 }
 
@@ -220,6 +221,11 @@ int vmg_destroy(vmg_handle h)
     cudaStreamSynchronize(h->stream);
     prof_collect(h);
     for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
+    for (int i = 0; i < 2; ++i) {
+        if (h->pcg_exec[i]) cudaGraphExecDestroy(h->pcg_exec[i]);
+        if (h->pcg_graph[i]) cudaGraphDestroy(h->pcg_graph[i]);
+    }
+    if (h->pcg_base) cudaFree(h->pcg_base);
     if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
     if (h->graph) cudaGraphDestroy(h->graph);
     if (h->h_scal) cudaFreeHost(h->h_scal);
@@ -283,7 +289,7 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
     for (int f = 0; f < 6; ++f)
         if (type[f] != VMG_BC_DIRICHLET && type[f] != VMG_BC_NEUMANN) return VMG_ERR_ARG;
     for (int f = 0; f < 6; ++f) {
-        if (h->bctype[f] != type[f]) h->graph_valid = false;   // the trilinear prolongation kernels carry the types by value
+        if (h->bctype[f] != type[f]) { h->graph_valid = false; ++h->graph_epoch; }   // the trilinear prolongation kernels carry the types by value
         h->bctype[f] = type[f];
         bool active = f < 4 || h->three_d;
         h->bc_has_value[f] = active && value && value[f];
@@ -305,6 +311,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "nu2")) { if (iv < 0 || iv > 8) return VMG_ERR_ARG; h->nu2 = iv; }
     else if (!strcmp(key, "bottom_sweeps")) { if (iv < 1) return VMG_ERR_ARG; h->nbottom = iv; }
     else if (!strcmp(key, "prolong")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->prolong = iv; }
+    else if (!strcmp(key, "symmetric")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->symmetric = iv; }
     else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
     else if (!strcmp(key, "blocked")) { h->use_blocked = iv != 0; }
     else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }
@@ -317,7 +324,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
         for (int c = 0; c < VMG_PC_COUNT; ++c) { h->prof_ms[c] = 0.0; h->prof_launches[c] = 0; }
     }
     else return VMG_ERR_ARG;
-    h->graph_valid = false;
+    { h->graph_valid = false; ++h->graph_epoch; }
     plan_schedule(h);
     return VMG_OK;
 }
@@ -463,6 +470,157 @@ int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max
     if (cudaStreamSynchronize(h->stream) != cudaSuccess && rc == VMG_OK) rc = VMG_ERR_CUDA;
     if (rc == VMG_ERR_CUDA) { h->last_cuda_error = (int)cudaGetLastError(); }
     return solve_close(h, rc);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// conjugate gradients preconditioned by one symmetric V-cycle (kernels: vmg_pcg.cuh)
+// ---------------------------------------------------------------------------------------------------------------
+}  // extern "C"
+
+namespace {
+
+int pcg_alloc(vmg_s* h)
+{
+    if (h->pcg_base) return VMG_OK;
+    VmgLevel& L = h->lev[0];
+    const size_t arr = round_up((size_t)L.nalloc + 2 * (size_t)L.pad, 32);
+    h->pcg_npartial = (int)std::max<long long>(grid_for((long long)L.G.ne * L.ny * L.nz), 8LL * h->num_sms);   // apply / dot grids
+    const size_t doubles = 3 * arr + round_up((size_t)h->pcg_npartial, 32) + 32;
+    if (cudaMalloc(&h->pcg_base, doubles * sizeof(double)) != cudaSuccess) { (void)cudaGetLastError(); h->pcg_base = nullptr; return VMG_ERR_ALLOC; }
+    CUDA_TRY(h, cudaMemsetAsync(h->pcg_base, 0, doubles * sizeof(double), h->stream));
+    double* b = (double*)h->pcg_base;
+    h->pcg_x = b + L.pad; h->pcg_p = b + arr + L.pad; h->pcg_q = b + 2 * arr + L.pad;
+    h->pcg_partial = b + 3 * arr; h->pcg_scal = h->pcg_partial + round_up((size_t)h->pcg_npartial, 32);
+    return VMG_OK;
+}
+
+// run `body` (which only enqueues on h->stream) as plain launches, or capture it once and replay it
+template <typename F>
+int pcg_run(vmg_s* h, int slot, F body)
+{
+    if (!h->use_graph || h->profile) { body(); return cudaGetLastError() == cudaSuccess ? VMG_OK : VMG_ERR_CUDA; }
+    if (h->pcg_epoch[slot] != h->graph_epoch) {
+        if (h->pcg_exec[slot]) { cudaGraphExecDestroy(h->pcg_exec[slot]); h->pcg_exec[slot] = nullptr; }
+        if (h->pcg_graph[slot]) { cudaGraphDestroy(h->pcg_graph[slot]); h->pcg_graph[slot] = nullptr; }
+        CUDA_TRY(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeRelaxed));
+        body();
+        cudaError_t e = cudaStreamEndCapture(h->stream, &h->pcg_graph[slot]);
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&h->pcg_exec[slot], h->pcg_graph[slot], 0);
+        if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
+        h->pcg_epoch[slot] = h->graph_epoch;
+    }
+    CUDA_TRY(h, cudaGraphLaunch(h->pcg_exec[slot], h->stream));
+    return VMG_OK;
+}
+
+int solve_pcg_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int max_iter)
+{
+    VmgLevel& L0 = h->lev[0];
+    unsigned long long* scal = (unsigned long long*)h->d_scal;
+    const long long n = L0.nalloc;                                   // element-wise kernels run over the whole allocation
+    const unsigned gpair = grid_for((long long)L0.G.ne * L0.ny * L0.nz), glin = 8u * (unsigned)h->num_sms;
+    double* r = L0.rhs;                                              // the CG residual lives where the V-cycle reads its rhs
+    double* z = L0.phi;                                              // ... and z = M^-1 r where it leaves its result
+    const LevelView v = view(L0);
+    long long count = 0;
+
+    int rc = enqueue_fold_bc(h, rhs, r);
+    if (rc != VMG_OK) return rc;
+    to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, h->pcg_x);
+    CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
+    norm_inf_kernel<<<glin, kThreads, 0, h->stream>>>(r, n, scal + 0);
+    pcg_residual_inplace_kernel<<<gpair, kPcgThreads, 0, h->stream>>>(v, h->pcg_x, r);
+    norm_inf_kernel<<<glin, kThreads, 0, h->stream>>>(r, n, scal + 1);
+    h->launches += 5;
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaMemcpyAsync(h->h_scal, scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    const double nb = h->h_scal[0];
+    if (nb == 0.0) {
+        CUDA_TRY(h, cudaMemsetAsync(phi, 0, L0.n * sizeof(double), h->stream));
+        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+        h->hist.push_back(0.0);
+        return VMG_OK;
+    }
+    h->relres = h->h_scal[1] / nb;
+    h->hist.push_back(h->relres);
+    if (std::isnan(h->relres) || std::isinf(h->relres)) return VMG_ERR_DIVERGED;
+    int status = VMG_MAXCYCLES;
+    if (rtol > 0.0 && h->relres <= rtol) status = VMG_OK;
+    else if (max_iter > 0) {
+        auto precondition = [&]() {                                   // z = M^-1 r: one symmetric V-cycle from zero
+            cudaMemsetAsync(z - L0.pad, 0, ((size_t)L0.nalloc + 2 * (size_t)L0.pad) * sizeof(double), h->stream);
+            enqueue_vcycle(h, nullptr, &count);
+        };
+        // p = z = M^-1 r, rho = <r, z>
+        precondition();
+        pcg_dot_kernel<<<glin, kPcgThreads, 0, h->stream>>>(r, z, n, h->pcg_partial);
+        pcg_reduce_kernel<<<1, 1024, 0, h->stream>>>(h->pcg_partial, (int)glin, PCG_MODE_RHO0, h->pcg_scal);
+        pcg_direction_kernel<<<glin, kPcgThreads, 0, h->stream>>>(h->pcg_p, z, n, h->pcg_scal, 1);
+        CUDA_TRY(h, cudaGetLastError());
+        h->launches += count + 3;
+        const long long per_cycle = count;
+        int slow = 0;
+        for (int c = 1; c <= max_iter; ++c) {
+            rc = pcg_run(h, 0, [&]() {                                // q = A p, alpha, x += alpha p, r -= alpha q, ||r||
+                pcg_apply_dot_kernel<<<gpair, kPcgThreads, 0, h->stream>>>(v, h->pcg_p, h->pcg_q, h->pcg_partial);
+                pcg_reduce_kernel<<<1, 1024, 0, h->stream>>>(h->pcg_partial, (int)gpair, PCG_MODE_ALPHA, h->pcg_scal);
+                cudaMemsetAsync(scal + 1, 0, sizeof(double), h->stream);
+                pcg_update_kernel<<<glin, kPcgThreads, 0, h->stream>>>(h->pcg_x, r, h->pcg_p, h->pcg_q, n, h->pcg_scal, scal + 1);
+            });
+            if (rc != VMG_OK) return rc;
+            h->launches += 3;
+            CUDA_TRY(h, cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+            CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+            h->relres = h->h_scal[1] / nb;
+            h->hist.push_back(h->relres);
+            h->cycles = c;
+            if (std::isnan(h->relres) || std::isinf(h->relres)) return VMG_ERR_DIVERGED;
+            if (rtol > 0.0) {
+                if (h->relres <= rtol) { status = VMG_OK; break; }
+                slow = (h->hist[c] >= 0.9 * h->hist[c - 1]) ? slow + 1 : 0;
+                if (slow >= 3) { status = VMG_STALLED; break; }
+            }
+            if (c == max_iter) break;
+            rc = pcg_run(h, 1, [&]() {                                // z = M^-1 r, beta, p = z + beta p
+                long long dummy = 0;
+                cudaMemsetAsync(z - L0.pad, 0, ((size_t)L0.nalloc + 2 * (size_t)L0.pad) * sizeof(double), h->stream);
+                enqueue_vcycle(h, nullptr, &dummy);
+                pcg_dot_kernel<<<glin, kPcgThreads, 0, h->stream>>>(r, z, n, h->pcg_partial);
+                pcg_reduce_kernel<<<1, 1024, 0, h->stream>>>(h->pcg_partial, (int)glin, PCG_MODE_BETA, h->pcg_scal);
+                pcg_direction_kernel<<<glin, kPcgThreads, 0, h->stream>>>(h->pcg_p, z, n, h->pcg_scal, 0);
+            });
+            if (rc != VMG_OK) return rc;
+            h->launches += per_cycle + 3;
+        }
+    }
+    to_natural_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, h->pcg_x, phi);
+    h->launches += 1;
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return status;
+}
+
+}  // namespace
+
+extern "C" {
+
+int vmg_solve_pcg(vmg_handle h, const double* rhs, double* phi, double rtol, int max_iter)
+{
+    if (!h || !rhs || !phi || max_iter < 0) return VMG_ERR_ARG;
+    int rc = ready(h);
+    if (rc != VMG_OK) return rc;
+    if (singular(h)) return VMG_ERR_SINGULAR;
+    if (h->nu1 != h->nu2) return VMG_ERR_ARG;          // the preconditioner must be symmetric
+    if ((rc = pcg_alloc(h)) != VMG_OK) return rc;
+    h->hist.clear(); h->cycles = 0; h->relres = 0.0; h->launches = 0;
+    const int keep = h->symmetric;
+    h->symmetric = 1;   // (vmg_solve's own graph is not used here and stays as captured)
+    rc = solve_pcg_impl(h, rhs, phi, rtol, max_iter);
+    h->symmetric = keep;
+    if (h->profile) { cudaStreamSynchronize(h->stream); prof_collect(h); }
+    h->total_launches += h->launches;
+    return rc;
 }
 
 // N independent problems (one handle and one stream each), advanced in lock-step: every round enqueues one V-cycle

@@ -58,6 +58,7 @@ struct vmg_s {
     bool have_coeffs = false, have_bc = false, dinv_dirty = true;
     int nu1 = 3, nu2 = 3, nbottom = 32;
     int prolong = 0;              // 0: piecewise constant (R9 default), 1: trilinear
+    int symmetric = 0;            // 1: symmetric V-cycle (post-smoothing / second half of the bottom black -> red): the PCG preconditioner
     int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200
     double l2_persist_mb = 24.0;  // L2 set aside for the level-0 face weights (0: none); see apply_l2_window
     bool l2_applied = false, l2_window_set = false;
@@ -83,6 +84,14 @@ struct vmg_s {
     int sv_max = 0, sv_slow = 0, sv_status = 0;
     bool sv_active = false;
     double* sv_phi = nullptr;
+    // MG-preconditioned CG (vmg_solve_pcg): x, p, q in the internal layout, partial sums, device scalars; allocated on first use
+    void* pcg_base = nullptr;
+    double *pcg_x = nullptr, *pcg_p = nullptr, *pcg_q = nullptr, *pcg_partial = nullptr, *pcg_scal = nullptr;
+    int pcg_npartial = 0;
+    cudaGraph_t pcg_graph[2] = {nullptr, nullptr};
+    cudaGraphExec_t pcg_exec[2] = {nullptr, nullptr};
+    unsigned pcg_epoch[2] = {0, 0};
+    unsigned graph_epoch = 1;          // bumped whenever captured graphs become stale
     // result of the last solve
     int cycles = 0;
     double relres = 0.0;

@@ -109,14 +109,16 @@ inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt, bool bt_natu
 // plain path: one launch per step, in place on the level's current phi buffer
 // ------------------------------------------------------------------------------------------------
 // skip_first: number of leading half-sweeps already done by the caller
-inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int skip_first = 0)
+// first: colour of the first half-sweep of every sweep (1: black -> red, the adjoint order of the symmetric V-cycle)
+inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int skip_first = 0, int first = 0)
 {
     VmgLevel& L = h->lev[l];
     LevelView v = view(L);
     long long nt = (long long)L.G.ne * L.ny * L.nz;
     for (int s = 0; s < nsweeps; ++s)
-        for (int colour = 0; colour < 2; ++colour) {
-            if (2 * s + colour < skip_first) continue;
+        for (int c2 = 0; c2 < 2; ++c2) {
+            const int colour = (first + c2) & 1;
+            if (2 * s + c2 < skip_first) continue;
             launch_pdl(h, smooth_colour_kernel, grid_for(nt), kThreads, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
             ++*count;
         }
@@ -211,7 +213,7 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
         if (l >= tail) off += tail_level_doubles(T.n, T.guard);
     }
     g.nu1 = h->nu1; g.nu2 = h->nu2; g.nbottom = h->nbottom; g.sz = h->three_d ? 2 : 1;
-    g.prolong = h->prolong; g.bc = prolong_bc(h);
+    g.prolong = h->prolong; g.bc = prolong_bc(h); g.sym = h->symmetric;
     g.whole = first == 0;
     g.norm_out = first == 0 ? norm_out : nullptr;
     ProfScope ps(h, VMG_PC_COARSE, count);
@@ -383,7 +385,7 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         }
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         bool fuse = l == 0 && norm_out != nullptr;
-        blocked_sweeps(h, l, 2 * h->nu2, 0, !h->prolong, fuse ? BT_NORM : BT_NONE, norm_out, count);
+        blocked_sweeps(h, l, 2 * h->nu2, h->symmetric, !h->prolong, fuse ? BT_NORM : BT_NONE, norm_out, count);
         return fuse;
     }
     if (h->nu2 >= 1 && !h->prolong) {   // the correction rides on the first half-sweep (smooth_colour_prolong_kernel)
@@ -391,9 +393,9 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         VmgLevel& L = h->lev[l];
         long long nt = (long long)L.G.ne * L.ny * L.nz;
         launch_pdl(h, smooth_colour_prolong_kernel, grid_for(nt), kThreads, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
-                   cur_phi(h->lev[l + 1]), 0, h->three_d ? 2 : 1, next_dir(h, L));
+                   cur_phi(h->lev[l + 1]), h->symmetric, h->three_d ? 2 : 1, next_dir(h, L));
         ++*count;
-        plain_smooth(h, l, h->nu2, count, 1);
+        plain_smooth(h, l, h->nu2, count, 1, h->symmetric);
         return false;
     }
     {
@@ -401,7 +403,7 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         plain_prolong_correct(h, l, count);
     }
     ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
-    plain_smooth(h, l, h->nu2, count);
+    plain_smooth(h, l, h->nu2, count, 0, h->symmetric);
     return false;
 }
 
@@ -423,10 +425,11 @@ inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* co
         VmgLevel& B = h->lev[last];
         if (last == 0) cudaMemsetAsync(B.phi, 0, B.nalloc * sizeof(double), h->stream);   // single level: bottom from zero
         ProfScope ps(h, VMG_PC_COARSE, count);
-        plain_smooth(h, last, h->nbottom, count);
+        if (!h->symmetric) plain_smooth(h, last, h->nbottom, count);
+        else { plain_smooth(h, last, h->nbottom / 2, count, 0, 0); plain_smooth(h, last, h->nbottom - h->nbottom / 2, count, 0, 1); }
     }
     for (int l = tail - 1; l >= 0; --l) norm_done = enqueue_up(h, l, l == 0 ? norm_out : nullptr, count);
-    if (norm_out && !norm_done) { enqueue_residual_norm(h, norm_out, h->nu2 >= 1 && tail > 0); ++*count; }
+    if (norm_out && !norm_done) { enqueue_residual_norm(h, norm_out, h->nu2 >= 1 && tail > 0 && !h->symmetric); ++*count; }
     settle_phi(h, 0);
 }
 

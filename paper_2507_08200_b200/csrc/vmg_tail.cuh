@@ -27,6 +27,7 @@ struct TailArgs {
                                // barrier.cluster between half-sweeps on global arrays, measured slower than graph launches)
     int nu1, nu2, nbottom, sz; // sz = 2 in 3-D, 1 in 2-D (children per coarse cell along z)
     int prolong;               // 0: piecewise constant, 1: trilinear (R9 option)
+    int sym;                   // 1: symmetric V-cycle: post-smoothing and the second half of the bottom sweeps black->red
     ProlongBC bc;              // boundary types (trilinear ghosts)
     int whole;                 // 1: lev[0] is level 0 of the hierarchy (phi is an initial guess, not zero)
     unsigned long long* norm_out;   // whole == 1: ||rhs - A phi||_inf bits after the cycle (may be NULL)
@@ -70,7 +71,7 @@ __device__ __forceinline__ double tail_nb_sum(const TailSmem& s, const TailLevel
 // their cell indices once, not per half-sweep; levels whose half-sweep fits ONE WARP (the 32-sweep bottom solve on
 // 4x2x2 or 2x2x2: 8 or 4 relaxations per colour) are relaxed by warp 0 alone with __syncwarp() between the colours
 // instead of 64 block-wide barriers.  The caller's __syncthreads() semantics are kept: all threads leave in step.
-__device__ __forceinline__ void tail_smooth(const TailSmem& s, const TailLevel& L, int nsweeps)
+__device__ __forceinline__ void tail_smooth(const TailSmem& s, const TailLevel& L, int nsweeps, int first = 0)
 {
     const int hx = (L.nx + 1) >> 1;
     const int nt = hx * L.ny * L.nz;
@@ -84,6 +85,7 @@ __device__ __forceinline__ void tail_smooth(const TailSmem& s, const TailLevel& 
                 const int i = 2 * m + ((colour + j + k) & 1);
                 if (i < L.nx) c[colour] = i + L.nx * j + L.nxy * k;
             }
+            if (first) { const int tmp = c[0]; c[0] = c[1]; c[1] = tmp; }   // c[0]: the colour relaxed first
         }
         if (nt <= 32) {
             if (threadIdx.x < 32)
@@ -107,7 +109,8 @@ __device__ __forceinline__ void tail_smooth(const TailSmem& s, const TailLevel& 
         return;
     }
     for (int sw = 0; sw < nsweeps; ++sw)
-        for (int colour = 0; colour < 2; ++colour) {
+        for (int c2 = 0; c2 < 2; ++c2) {
+            const int colour = (first + c2) & 1;
             for (int t = threadIdx.x; t < nt; t += blockDim.x) {
                 int m = t % hx, j = (t / hx) % L.ny, k = t / (hx * L.ny);
                 int i = 2 * m + ((colour + j + k) & 1);
@@ -176,7 +179,8 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
             for (int t = tid; t < B.n; t += nth) s.phi[t] = 0.0;
             __syncthreads();
         }
-        tail_smooth(s, B, g.nbottom);
+        if (!g.sym) tail_smooth(s, B, g.nbottom);
+        else { tail_smooth(s, B, g.nbottom / 2, 0); tail_smooth(s, B, g.nbottom - g.nbottom / 2, 1); }
     }
     // ---- up-stroke ----
     for (int l = g.nl - 2; l >= g.ns; --l) {
@@ -192,7 +196,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
                 s.phi[t] += c.phi[(i >> 1) + C.nx * ((j >> 1) + C.ny * (g.sz == 2 ? (k >> 1) : k))];
         }
         __syncthreads();
-        tail_smooth(s, L, g.nu2);
+        tail_smooth(s, L, g.nu2, g.sym);
     }
     // ---- stage out ----
     {

@@ -430,3 +430,53 @@ def test_trilinear_prolongation_matches_oracle(dims):
     phi0 = rng.standard_normal(p.rhs.shape)
     assert rel(s.step_vcycle(dev(phi0), dev(bt)).cpu().numpy(), o.vcycle(phi0, bt)) <= 1e-12
     s.destroy()
+
+
+def test_symmetric_vcycle_matches_oracle():
+    """Option symmetric = 1 (the PCG preconditioner): one V-cycle against the oracle's, per-colour path, blocked passes
+    and the shared-memory tail."""
+    b = _binding()
+    p = inputs.random_problem(48, 24, 48, seed=3, bc_type=[D, D, N, N, N, D])
+    o = Oracle.from_problem(p)
+    o.set_option("symmetric", 1)
+    bt = o.fold_bc(p.rhs)
+    phi0 = np.random.default_rng(2).standard_normal(p.rhs.shape)
+    ref = o.vcycle(phi0, bt)
+    for opts in (dict(), dict(blocked=1, block_min_cells=0), dict(tail=0, graph=0)):
+        s, d = b.from_problem(p)
+        s.set_option("symmetric", 1)
+        for k, v in opts.items():
+            s.set_option(k, v)
+        assert rel(s.step_vcycle(dev(phi0), dev(bt)).cpu().numpy(), ref) <= 1e-12, opts
+        s.destroy()
+
+
+@pytest.mark.parametrize("make", [lambda: inputs.config3(32), lambda: inputs.config4(32), lambda: inputs.config2(32),
+                                  lambda: inputs.config1(64),
+                                  lambda: inputs.random_problem(32, 32, 32, seed=3, bc_type=[D, N, N, N, N, N], ell=0.06, sigma=2.0,
+                                                                a_scale=1.0, inhomogeneous=False)],
+                         ids=["config3", "config4", "config2", "config1_2d", "contrast_where_vcycles_stall"])
+def test_pcg_parity(make):
+    """vmg_solve_pcg against ovmg_solve_pcg: same status, iteration counts within 1, phi within 1e-10
+    after both reach the tolerance, histories alike while above the floor.  The last case is the one on which the plain
+    V-cycle iteration stalls (tests/test_oracle_pins.py)."""
+    b = _binding()
+    p = make()
+    rtol = 1e-10 if "random" in p.name else 1e-12
+    o = Oracle.from_problem(p)
+    phi_o, st_o, it_o, rr_o, hist_o = o.solve_pcg(p.rhs, rtol=rtol, max_iter=80)
+    s, d = b.from_problem(p)
+    phi = torch.zeros_like(d["rhs"])
+    st = s.solve_pcg(d["rhs"], phi, rtol=rtol, max_iter=80)
+    it, rr, hist = s.get_info()
+    assert st == st_o == 0 and abs(it - it_o) <= 1 and rr <= rtol
+    assert rel(phi.cpu().numpy(), phi_o) <= PHI_TOL
+    m = min(len(hist), len(hist_o))
+    live = hist_o[:m] > 1e-9
+    assert np.all(np.abs(np.array(hist)[:m][live] / hist_o[:m][live] - 1.0) < 1e-2)
+    # the handle still does plain V-cycle solves afterwards, and PCG again
+    phi2 = torch.zeros_like(d["rhs"])
+    s.solve(d["rhs"], phi2, rtol=1e-6, max_vcycles=60) if "random" not in p.name else None
+    phi3 = torch.zeros_like(d["rhs"])
+    assert s.solve_pcg(d["rhs"], phi3, rtol=rtol, max_iter=80) == 0 and torch.equal(phi3, phi)
+    s.destroy()
