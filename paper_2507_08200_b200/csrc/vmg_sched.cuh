@@ -1,6 +1,8 @@
 // vmg_sched.cuh -- sequencing of one V-cycle (S7): which kernel runs each step on each level, plain
 // launches or one CUDA graph replay (north_star (4)).
-//   levels 0 .. tail_level-1 : blocked passes (vmg_block.cuh) where the level qualifies, else one launch per step
+//   levels 0 .. tail_level-1 : one launch per colour half-sweep / transfer, in an order that reuses L2 (next_dir), with
+//                              programmatic dependent launch; with option blocked = 1 the blocked passes of
+//                              vmg_block2.cuh where the level qualifies
 //   levels tail_level .. last: one single-CTA launch (vmg_tail.cuh)
 #pragma once
 #include "vmg_internal.h"
