@@ -480,3 +480,19 @@ def test_pcg_parity(make):
     phi3 = torch.zeros_like(d["rhs"])
     assert s.solve_pcg(d["rhs"], phi3, rtol=rtol, max_iter=80) == 0 and torch.equal(phi3, phi)
     s.destroy()
+
+
+@pytest.mark.parametrize("dims,spacing", [((96, 48, 80), (0.5, 0.6, 0.55)), ((512, 256, 1), (1.0, 1.0, 1.0)), ((36, 20, 12), (1.0, 1.2, 0.9)),
+                                          ((130, 66, 34), (1.0, 1.0, 1.0))],
+                         ids=["96x48x80_unequal_h", "512x256_2d", "36x20x12_odd_coarse", "130x66x34_single_coarsening"])
+def test_more_shapes_parity(dims, spacing):
+    """Unequal mesh widths, a large 2-D grid, hierarchies that stop at odd sizes (36x20x12 -> 9x5x3; 130x66x34 -> 65x33x17:
+    two levels, 36 465 coarsest cells would exceed the bottom limit -> VMG_ERR_SIZE, checked instead)."""
+    b = _binding()
+    if dims == (130, 66, 34):
+        with pytest.raises(b.VmgError) as e:
+            b.Vmg(*dims, *spacing)
+        assert e.value.code == -2
+        return
+    p = inputs.random_problem(*dims, seed=17, bc_type=[N, D, D, N, N, D], spacing=spacing)
+    check_parity(p)
