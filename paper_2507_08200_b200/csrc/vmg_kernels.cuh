@@ -323,15 +323,26 @@ __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom
     long long c, xm;
     pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
     const int K = sz == 2 ? (k >> 1) : k;
+    // In every direction one neighbour has this cell's own coarse parent and the other the adjacent coarse cell (on the
+    // low side for an even fine index, on the high side for an odd one): four coarse values, not six.
+    const int I = i >> 1;
+    long long cP, xP;
+    pair_addr(CG, CG.plane * K + (long long)CG.pitch * (j >> 1), I >> 1, I & 1, cP, xP);
+    const double eP = e[cP];
+    const double eX = (i & 1) ? e[xP + 1] : e[xP];                                  // zero pad beyond the x faces: not used there
+    const double eY = (j & 1) ? e[cP + CG.pitch] : e[cP - CG.pitch];
     // out-of-domain neighbours carry a zero weight; their (zero-pad or foreign) value is used uncorrected
     double vxm = phi[xm], vxp = phi[xm + 1], vym = phi[c - G.pitch], vyp = phi[c + G.pitch], vzm = phi[c - G.plane], vzp = phi[c + G.plane];
-    if (i > 0) vxm += e[cell_at(CG, (i - 1) >> 1, j >> 1, K)];
-    if (i < G.nx - 1) vxp += e[cell_at(CG, (i + 1) >> 1, j >> 1, K)];
-    if (j > 0) vym += e[cell_at(CG, i >> 1, (j - 1) >> 1, K)];
-    if (j < G.ny - 1) vyp += e[cell_at(CG, i >> 1, (j + 1) >> 1, K)];
+    if (i > 0) vxm += (i & 1) ? eP : eX;
+    if (i < G.nx - 1) vxp += (i & 1) ? eX : eP;
+    if (j > 0) vym += (j & 1) ? eP : eY;
+    if (j < G.ny - 1) vyp += (j & 1) ? eY : eP;
     if (sz == 2) {
-        if (k > 0) vzm += e[cell_at(CG, i >> 1, j >> 1, (k - 1) >> 1)];
-        if (k < G.nz - 1) vzp += e[cell_at(CG, i >> 1, j >> 1, (k + 1) >> 1)];
+        const double eZ = (k & 1) ? e[cP + CG.plane] : e[cP - CG.plane];
+        if (k > 0) vzm += (k & 1) ? eP : eZ;
+        if (k < G.nz - 1) vzp += (k & 1) ? eZ : eP;
+    } else {
+        // 2-D: no z coupling (wz = 0), the z-neighbours are pads
     }
     double s = L.wx[c] * vxm;
     s = fma(L.wx[xm + 1], vxp, s);
