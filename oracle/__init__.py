@@ -47,6 +47,7 @@ def lib():
         _lib.ovmg_set_bc.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(_dp)]
         _lib.ovmg_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_double]
         _lib.ovmg_solve.argtypes = [C.c_void_p, _dp, _dp, C.c_double, C.c_int]
+        _lib.ovmg_set_mask.argtypes = [C.c_void_p, C.c_void_p, C.c_int, _dp]
         _lib.ovmg_solve_pcg.argtypes = [C.c_void_p, _dp, _dp, C.c_double, C.c_int]
         _lib.ovmg_get_info.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_double), _dp]
         _lib.ovmg_num_levels.argtypes = [C.c_void_p]
@@ -119,6 +120,15 @@ class Oracle:
         keep = [_c(v) for v in (values or [None] * 6)]
         arr = (_dp * 6)(*[_p(v) for v in keep])
         self._chk(lib().ovmg_set_bc(self._h, t, arr), "set_bc")
+
+    def set_mask(self, mask, kind: int, cval=None):
+        """Cell mask (1 valid, 0 covered), BC kind at the covered-valid interfaces, Dirichlet values of covered cells.
+        Call set_coeffs afterwards (it applies the mask)."""
+        m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+        cv = None if cval is None else _c(cval)
+        self._keep_mask = (m, cv)
+        self._chk(lib().ovmg_set_mask(self._h, None if m is None else m.ctypes.data_as(C.c_void_p), int(kind),
+                                      None if cv is None else _p(cv)), "set_mask")
 
     def set_option(self, key: str, v: float):
         self._chk(lib().ovmg_set_option(self._h, key.encode(), float(v)), "set_option")

@@ -39,6 +39,7 @@ typedef struct {
     double hx, hy, hz;
     double *a, *bx, *by, *bz;   /* coefficients of this level (owned) */
     double *phi, *rhs, *res;    /* work arrays of this level (owned) */
+    double *adiag;              /* masking: extra diagonal (interface Dirichlet terms, 1 in covered cells); NULL without a mask */
 } olevel;
 
 typedef struct ovmg {
@@ -48,6 +49,10 @@ typedef struct ovmg {
     int bctype[6];
     double *bcval[6];           /* level-0 value planes (owned copies; NULL = homogeneous) */
     int have_coeffs, have_bc;
+    unsigned char *mask;        /* level 0: 1 = valid, 0 = covered (owned copy); NULL = no mask */
+    int mask_kind;              /* BC kind at every covered-valid interface */
+    double *cval;               /* Dirichlet value carried by the covered cells (owned copy; NULL = 0) */
+    double *mfold;              /* level 0: interface terms of btilde */
     int nu1, nu2, nbottom;
     int prolong;                /* 0: piecewise constant (R9 default), 1: trilinear (R9 option) */
     int symmetric;              /* 1: symmetric V-cycle (post-smoothing and second half of the bottom black->red) */
@@ -85,6 +90,7 @@ static void stencil(const ovmg *h, const olevel *L, int i, int j, int k, double 
         hh[ZLO] = hh[ZHI] = L->hz;
     }
     *D = h->alpha * (L->a ? L->a[CI(L, i, j, k)] : 0.0);
+    if (L->adiag) *D += L->adiag[CI(L, i, j, k)];
     for (f = 0; f < 6; ++f) w[f] = 0.0;
     for (f = 0; f < nd; ++f) {
         double wf = h->beta * b[f] / (hh[f] * hh[f]);
@@ -248,6 +254,12 @@ static void average_coeffs(const ovmg *h, int lev)
                 for (s = 0; s < sz; ++s) for (q = 0; q < 2; ++q) for (p = 0; p < 2; ++p)
                     sum += F->a[CI(F, 2 * I + p, 2 * J + q, sz * K + s)];
                 C->a[CI(C, I, J, K)] = sum / (4.0 * sz);
+                if (F->adiag) {   /* masking: the extra diagonal is averaged like a */
+                    double sd = 0.0;
+                    for (s = 0; s < sz; ++s) for (q = 0; q < 2; ++q) for (p = 0; p < 2; ++p)
+                        sd += F->adiag[CI(F, 2 * I + p, 2 * J + q, sz * K + s)];
+                    C->adiag[CI(C, I, J, K)] = sd / (4.0 * sz);
+                }
             }
     for (K = 0; K < C->nz; ++K)
         for (J = 0; J < C->ny; ++J)
@@ -303,6 +315,7 @@ static void fold_bc(const ovmg *h, const double *rhs, double *bt)
                     if (h->bctype[f] == BC_DIRICHLET) v += 2.0 * h->beta * b * g / (hd * hd);
                     else                              v += h->beta * b * g / hd;
                 }
+                if (h->mask) v = h->mask[CI(L, i, j, k)] ? v + h->mfold[CI(L, i, j, k)] : 0.0;
                 bt[CI(L, i, j, k)] = v;
             }
 }
@@ -348,7 +361,7 @@ static double norm_inf(const double *v, size_t n)
  * ============================================================================================= */
 static void free_level(olevel *L)
 {
-    free(L->a); free(L->bx); free(L->by); free(L->bz); free(L->phi); free(L->rhs); free(L->res);
+    free(L->a); free(L->bx); free(L->by); free(L->bz); free(L->phi); free(L->rhs); free(L->res); free(L->adiag);
 }
 
 int ovmg_create(ovmg **out, int nx, int ny, int nz, double dx, double dy, double dz)
@@ -400,11 +413,81 @@ int ovmg_destroy(ovmg *h)
     if (!h) return O_ERR_ARG;
     for (l = 0; l < h->nlev; ++l) free_level(&h->lev[l]);
     for (l = 0; l < 6; ++l) free(h->bcval[l]);
+    free(h->mask); free(h->cval); free(h->mfold);
     free(h->lev); free(h->hist); free(h);
     return O_OK;
 }
 
 /* a == NULL means a = 0; bx,by,bz all NULL means b = 1 (bz ignored in 2-D). */
+/* SURVEY.md sec. 8(f) N4 / PAPER.md:136 ("a mask field is set as 1 inside valid plasma regions while it is set as 0 in
+ * covered regions. The linear solvers are disabled in covered regions with one-sided numerical schemes enabled at
+ * covered-valid interfaces", "directly specifying flux as well as Dirichlet boundary conditions at interior
+ * interfaces").  Reading: every face between a valid and a covered cell is an interior boundary of ONE kind --
+ * Dirichlet with the value the covered cell carries (an electrode's potential), discretised like a domain face
+ * (two-point flux, 2 beta b/h^2 on the diagonal and 2 beta b g/h^2 on the right-hand side), or homogeneous Neumann
+ * (zero flux) -- and covered cells are identity rows holding phi = 0.  Realised on the level's coefficients, so that
+ * every other routine is unchanged: faces touching a covered cell get b = 0, a = 0 in covered cells, and the extra
+ * diagonal `adiag` carries the Dirichlet interface terms (valid cells) and 1 (covered cells); coarse levels average
+ * adiag like a (a coarse cell with any valid child stays in the solve, a fully covered one is an identity row). */
+static void apply_mask(ovmg *h)
+{
+    olevel *L = &h->lev[0];
+    int i, j, k, f, nd = h->three_d ? 6 : 4;
+    for (k = 0; k < L->nz; ++k)
+        for (j = 0; j < L->ny; ++j)
+            for (i = 0; i < L->nx; ++i) {
+                size_t c = CI(L, i, j, k);
+                double ad = 0.0, mf = 0.0;
+                if (!h->mask[c]) { L->adiag[c] = 1.0; h->mfold[c] = 0.0; continue; }
+                for (f = 0; f < nd; ++f) {
+                    int ii = i + (f == XHI) - (f == XLO), jj = j + (f == YHI) - (f == YLO), kk = k + (f == ZHI) - (f == ZLO);
+                    double b, hd;
+                    if (ii < 0 || ii >= L->nx || jj < 0 || jj >= L->ny || kk < 0 || kk >= L->nz) continue;   /* domain face */
+                    if (h->mask[CI(L, ii, jj, kk)]) continue;                                                /* valid neighbour */
+                    if (h->mask_kind != BC_DIRICHLET) continue;                                              /* zero flux */
+                    b = f < 2 ? L->bx[XI(L, i + (f == XHI), j, k)] : f < 4 ? L->by[YI(L, i, j + (f == YHI), k)]
+                                                                          : L->bz[ZI(L, i, j, k + (f == ZHI))];
+                    hd = f < 2 ? L->hx : f < 4 ? L->hy : L->hz;
+                    ad += 2.0 * h->beta * b / (hd * hd);
+                    mf += 2.0 * h->beta * b * (h->cval ? h->cval[CI(L, ii, jj, kk)] : 0.0) / (hd * hd);
+                }
+                L->adiag[c] = ad; h->mfold[c] = mf;
+            }
+    /* now cut the couplings: b = 0 on every face that touches a covered cell, a = 0 in covered cells */
+    for (k = 0; k < L->nz; ++k)
+        for (j = 0; j < L->ny; ++j)
+            for (i = 0; i < L->nx; ++i) {
+                if (h->mask[CI(L, i, j, k)]) continue;
+                L->a[CI(L, i, j, k)] = 0.0;
+                L->bx[XI(L, i, j, k)] = 0.0; L->bx[XI(L, i + 1, j, k)] = 0.0;
+                L->by[YI(L, i, j, k)] = 0.0; L->by[YI(L, i, j + 1, k)] = 0.0;
+                if (h->three_d) { L->bz[ZI(L, i, j, k)] = 0.0; L->bz[ZI(L, i, j, k + 1)] = 0.0; }
+            }
+}
+
+/* mask: nx*ny*nz bytes (1 valid, 0 covered) or NULL to remove the mask; kind: BC_DIRICHLET / BC_NEUMANN at all
+ * covered-valid interfaces; cval: cell array with the Dirichlet value of covered cells, or NULL (0).  The coefficients
+ * must be set (again) afterwards: ovmg_set_coeffs applies the mask. */
+int ovmg_set_mask(ovmg *h, const unsigned char *mask, int kind, const double *cval)
+{
+    olevel *L;
+    int l;
+    if (!h || (kind != BC_DIRICHLET && kind != BC_NEUMANN)) return O_ERR_ARG;
+    L = &h->lev[0];
+    free(h->mask); free(h->cval); free(h->mfold);
+    h->mask = NULL; h->cval = NULL; h->mfold = NULL;
+    for (l = 0; l < h->nlev; ++l) { free(h->lev[l].adiag); h->lev[l].adiag = NULL; }
+    h->have_coeffs = 0;
+    if (!mask) return O_OK;
+    h->mask = (unsigned char *)malloc(ncell(L));
+    memcpy(h->mask, mask, ncell(L));
+    h->mask_kind = kind;
+    if (cval) { h->cval = (double *)malloc(ncell(L) * sizeof(double)); memcpy(h->cval, cval, ncell(L) * sizeof(double)); }
+    h->mfold = (double *)calloc(ncell(L), sizeof(double));
+    for (l = 0; l < h->nlev; ++l) h->lev[l].adiag = (double *)calloc(ncell(&h->lev[l]), sizeof(double));
+    return O_OK;
+}
+
 int ovmg_set_coeffs(ovmg *h, const double *a, const double *bx, const double *by, const double *bz,
                     double alpha, double beta)
 {
@@ -429,6 +512,7 @@ int ovmg_set_coeffs(ovmg *h, const double *a, const double *bx, const double *by
     }
     h->alpha = a ? alpha : 0.0;
     h->beta = beta;
+    if (h->mask) apply_mask(h);
     for (l = 0; l + 1 < h->nlev; ++l) average_coeffs(h, l);
     h->have_coeffs = 1;
     return O_OK;
@@ -469,8 +553,18 @@ int ovmg_set_option(ovmg *h, const char *key, double v)
     return O_ERR_ARG;
 }
 
+static void zero_covered(const ovmg *h, double *phi)
+{
+    size_t c, n = ncell(&h->lev[0]);
+    if (h->mask) for (c = 0; c < n; ++c) if (!h->mask[c]) phi[c] = 0.0;
+}
+
 static int singular(const ovmg *h)
 {
+    if (h->mask && h->mask_kind == BC_DIRICHLET) {   /* a covered cell with a Dirichlet interface pins the solution */
+        size_t c, n = ncell(&h->lev[0]);
+        for (c = 0; c < n; ++c) if (!h->mask[c]) return 0;
+    }
     int f, nd = h->three_d ? 6 : 4;
     for (f = 0; f < nd; ++f) if (h->bctype[f] == BC_DIRICHLET) return 0;
     return h->alpha == 0.0;
@@ -490,6 +584,7 @@ int ovmg_solve(ovmg *h, const double *rhs, double *phi, double rtol, int max_vcy
     free(h->hist);
     h->hist = (double *)calloc((size_t)max_vcycles + 1, sizeof(double));
     h->hist_len = 0; h->cycles = 0; h->relres = 0.0;
+    zero_covered(h, phi);
     fold_bc(h, rhs, bt);
     nb = norm_inf(bt, ncell(L));
     if (nb == 0.0) {
@@ -551,6 +646,7 @@ int ovmg_solve_pcg(ovmg *h, const double *rhs, double *phi, double rtol, int max
     r = (double *)malloc(4 * n * sizeof(double));
     if (!r) return O_ERR_ARG;
     z = r + n; p = z + n; q = p + n;
+    zero_covered(h, phi);
     fold_bc(h, rhs, q);                               /* q = btilde for a moment */
     nb = norm_inf(q, n);
     if (nb == 0.0) {

@@ -390,3 +390,110 @@ def test_n2_pcg_converges_where_plain_vcycles_do_not():
     assert st_v != 0 and rr_v > 1e-3
     assert st_c == 0 and it_c <= 30 and rr_c <= 1e-10
     o.close()
+
+
+def _masked_system_by_faces(p, mask, kind, cval):
+    """(A, btilde) of the masked problem written face by face from the finite-volume statement:
+    a face between two valid cells couples them; a face between a valid and a covered cell is an interior boundary --
+    Dirichlet with the covered cell's value (two-point flux over half a cell) or zero flux; domain faces of valid cells
+    as usual; a covered cell is an identity row with zero right-hand side.  Per-cell form (divided by the volume)."""
+    nx, ny, nz = p.nx, p.ny, p.nz
+    h = (p.dx, p.dy, p.dz)
+    n = nx * ny * nz
+    idx = lambda i, j, k: i + nx * (j + ny * k)
+    A = np.zeros((n, n))
+    bt = p.rhs.ravel().copy()
+    a = p.a if p.a is not None else np.zeros((nz, ny, nx))
+    m = mask.astype(bool)
+    for k in range(nz):
+        for j in range(ny):
+            for i in range(nx):
+                c = idx(i, j, k)
+                if m[k, j, i]:
+                    A[c, c] += p.alpha * a[k, j, i]
+                else:
+                    A[c, c] = 1.0
+                    bt[c] = 0.0
+    barr = (p.bx, p.by, p.bz)
+    for d in range(3):
+        nd = (nx, ny, nz)[d]
+        for k in range(nz):
+            for j in range(ny):
+                for i in range(nx):
+                    pos = (i, j, k)[d]
+                    # the LOW face of cell (i,j,k) in direction d, and -- for the last cell -- its high face as well
+                    for side in ([0] if pos < nd - 1 else [0, 1]):
+                        fi = [i, j, k]; fi[d] += side
+                        b = barr[d][fi[2], fi[1], fi[0]]
+                        t = p.beta * b / h[d] ** 2
+                        c = idx(i, j, k)
+                        if side == 0 and pos > 0:                          # interior face between (pos-1) and pos
+                            lo = [i, j, k]; lo[d] -= 1
+                            l = idx(*lo)
+                            vl, vr = m[lo[2], lo[1], lo[0]], m[k, j, i]
+                            if vl and vr:
+                                A[l, l] += t; A[c, c] += t; A[l, c] -= t; A[c, l] -= t
+                            elif vl != vr and kind == D:
+                                v, cov = (l, (k, j, i)) if vl else (c, (lo[2], lo[1], lo[0]))
+                                A[v, v] += 2 * t
+                                bt[v] += 2 * t * (cval[cov] if cval is not None else 0.0)
+                        else:                                              # domain face
+                            if not m[k, j, i]:
+                                continue
+                            f = 2 * d + (0 if side == 0 and pos == 0 else 1)
+                            val = p.bc_value[f]
+                            pl = [(j, k), (i, k), (i, j)][d]
+                            g = 0.0 if val is None else val[pl[1], pl[0]]
+                            if p.bc_type[f] == D:
+                                A[c, c] += 2 * t; bt[c] += 2 * t * g
+                            else:
+                                bt[c] += t * h[d] * g
+    return A, bt
+
+
+@pytest.mark.parametrize("kind", [D, N], ids=["dirichlet_interfaces", "zero_flux_interfaces"])
+def test_n4_masked_operator_and_solution_match_facewise_assembly(kind):
+    """SURVEY 8(f) N4 / PAPER.md:136: the masked problem the oracle solves is the one assembled face by face above
+    (operator on every level-0 row, folded right-hand side), and multigrid / PCG reach its dense solution."""
+    p = inputs.random_problem(8, 8, 8, seed=12, bc_type=[D, N, N, D, N, N])
+    rng = np.random.default_rng(1)
+    mask = np.ones(p.rhs.shape, dtype=np.uint8)
+    mask[2:5, 3:6, 1:4] = 0                     # a covered block (k, j, i ranges) inside the box
+    mask[0, 0, :3] = 0                          # and covered cells touching the domain boundary
+    cval = np.where(mask == 0, 0.7 + 0.1 * rng.standard_normal(p.rhs.shape), 0.0)
+    o = Oracle.from_problem(p)
+    o.set_mask(mask, kind, cval if kind == D else None)
+    o.set_coeffs(p.a, p.bx, p.by, p.bz, p.alpha, p.beta)
+    A, bt = _masked_system_by_faces(p, mask, kind, cval if kind == D else None)
+    assert np.abs(dense_from_apply(o) - A).max() <= 1e-12 * np.abs(A).max()
+    assert np.abs(o.fold_bc(p.rhs).ravel() - bt).max() <= 1e-12 * np.abs(bt).max()
+    x = np.linalg.solve(A, bt).reshape(p.rhs.shape)
+    assert np.abs(x[mask == 0]).max() == 0.0
+    phi, st, cyc, rr, _ = o.solve(p.rhs, rtol=1e-13, max_vcycles=60)
+    assert st == 0 and np.abs(phi - x).max() <= 1e-10 * np.abs(x).max()
+    phi, st, it, rr, _ = o.solve_pcg(p.rhs, rtol=1e-13, max_iter=60)
+    assert st == 0 and np.abs(phi - x).max() <= 1e-10 * np.abs(x).max()
+    o.close()
+
+
+def test_n4_electrode_block_obeys_the_maximum_principle():
+    """A covered block at potential 1 inside a grounded box (Laplace, no source): 0 <= phi <= 1 in every valid cell, phi
+    decays away from the block, and the solution has the block's mirror symmetry."""
+    n = 16
+    h = 1.0 / n
+    ones = lambda shape: np.ones(shape)
+    p = inputs.Problem(name="electrode", nx=n, ny=n, nz=n, dx=h, dy=h, dz=h, alpha=0.0, beta=1.0, a=None,
+                       bx=ones((n, n, n + 1)), by=ones((n, n + 1, n)), bz=ones((n + 1, n, n)),
+                       bc_type=[D] * 6, bc_value=[None] * 6, rhs=np.zeros((n, n, n)))
+    mask = np.ones((n, n, n), dtype=np.uint8)
+    mask[6:10, 6:10, 6:10] = 0
+    o = Oracle.from_problem(p)
+    o.set_mask(mask, D, np.where(mask == 0, 1.0, 0.0))
+    o.set_coeffs(None, p.bx, p.by, p.bz, 0.0, 1.0)
+    phi, st, cyc, rr, _ = o.solve(p.rhs, rtol=1e-12, max_vcycles=60)
+    assert st == 0
+    v = phi[mask == 1]
+    assert v.min() > 0.0 and v.max() < 1.0
+    assert np.abs(phi - phi[::-1, :, :]).max() < 1e-10 and np.abs(phi - phi.transpose(2, 1, 0)).max() < 1e-10
+    assert phi[8, 8, 10] > phi[8, 8, 12] > phi[8, 8, 14] > 0.0
+    o.close()
