@@ -75,6 +75,17 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
  * vmg_set_coeffs, and again at any time. */
 int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6]);
 
+/* Cell masking ("cell masking for complex geometries").  mask: DEVICE array of
+ * nx*ny*nz bytes in the cell layout, 1 = valid cell, 0 = covered cell (inside a solid), or NULL to remove the
+ * mask.  kind: what every covered/valid interface face is: VMG_BC_DIRICHLET (phi = the covered cell's value at the
+ * face, e.g. an electrode; cval: DEVICE cell array that holds that value in covered cells, NULL = 0) or
+ * VMG_BC_NEUMANN (zero flux, e.g. an insulating body; cval ignored).  Covered cells are taken out of the solve: phi
+ * comes back 0 there and f is not read there.  Both arrays are copied.  vmg_set_coeffs must be called (again)
+ * afterwards -- it applies the mask to the coefficients of every level -- and VMG_ERR_STATE is returned by the
+ * solves until then.  A Dirichlet mask with at least one covered cell makes an all-Neumann alpha = 0 problem
+ * regular. */
+int vmg_set_mask(vmg_handle h, const unsigned char* mask, int kind, const double* cval);
+
 /* Solve.  rhs: f at cell centres (never written).  phi: initial guess in, solution out.
  * Iterates V(nu1,nu2) cycles until ||btilde - A phi||_inf <= rtol * ||btilde||_inf, where btilde is f with
  * the boundary data folded in, or until max_vcycles cycles (rtol <= 0: run exactly max_vcycles cycles).

@@ -17,7 +17,7 @@ STATUS = {0: "OK", 1: "MAXCYCLES", 2: "STALLED", -1: "ERR_ARG", -2: "ERR_SIZE", 
           -4: "ERR_SINGULAR", -5: "ERR_DIVERGED", -6: "ERR_CUDA", -7: "ERR_ALLOC"}
 
 # every symbol include/vmg.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_solve", "vmg_solve_batch", "vmg_solve_pcg", "vmg_get_info", "vmg_set_option",
+SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_set_mask", "vmg_solve", "vmg_solve_batch", "vmg_solve_pcg", "vmg_get_info", "vmg_set_option",
            "vmg_destroy", "vmg_strerror", "vmg_last_cuda_error", "vmg_num_levels", "vmg_level_dims",
            "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
            "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_down", "vmg_step_up", "vmg_step_vcycle", "vmg_step_norm_inf",
@@ -39,6 +39,7 @@ def load():
     lib.vmg_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _vp]
     lib.vmg_set_coeffs.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_double, C.c_double]
     lib.vmg_set_bc.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(_vp)]
+    lib.vmg_set_mask.argtypes = [_vp, _vp, C.c_int, _vp]
     lib.vmg_solve.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int]
     lib.vmg_solve_pcg.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int]
     lib.vmg_solve_batch.argtypes = [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp), C.c_double, C.c_int,
@@ -147,6 +148,16 @@ class Vmg:
         vals = list(values) if values is not None else [None] * 6
         arr = (_vp * 6)(*[_ptr(v) for v in vals])
         self._chk(self._lib.vmg_set_bc(self._h, t, arr), "vmg_set_bc")
+
+    def set_mask(self, mask, kind: int = 1, cval=None):
+        """mask: contiguous uint8 CUDA tensor (1 valid, 0 covered) or None; kind: BC type of the covered/valid interfaces;
+        cval: fp64 cell tensor with the Dirichlet value in covered cells.  Call set_coeffs afterwards."""
+        mp = None
+        if mask is not None:
+            torch = _torch()
+            assert mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous(), "need a contiguous uint8 CUDA mask"
+            mp = mask.data_ptr()
+        self._chk(self._lib.vmg_set_mask(self._h, mp, int(kind), _ptr(cval)), "vmg_set_mask")
 
     def set_option(self, key: str, v: float):
         self._chk(self._lib.vmg_set_option(self._h, key.encode(), float(v)), "vmg_set_option")

@@ -90,6 +90,7 @@ bool singular(const vmg_s* h)
 {
     int nd = h->three_d ? 6 : 4;
     for (int f = 0; f < nd; ++f) if (h->bctype[f] == VMG_BC_DIRICHLET) return false;
+    if (h->d_mask && h->mask_kind == VMG_BC_DIRICHLET && h->mask_covered > 0) return false;   // an interior electrode pins phi
     return h->alpha == 0.0;
 }
 
@@ -226,6 +227,7 @@ int vmg_destroy(vmg_handle h)
         if (h->pcg_graph[i]) cudaGraphDestroy(h->pcg_graph[i]);
     }
     if (h->pcg_base) cudaFree(h->pcg_base);
+    if (h->mask_base) cudaFree(h->mask_base);
     if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
     if (h->graph) cudaGraphDestroy(h->graph);
     if (h->h_scal) cudaFreeHost(h->h_scal);
@@ -251,6 +253,21 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
     const double *fa = a, *fbx = bx, *fby = by, *fbz = h->three_d ? bz : nullptr;
     long long setup_launches = 0;
     ProfScope* ps = new ProfScope(h, VMG_PC_SETUP, &setup_launches);
+    if (h->d_mask) {   // masking: level 0 is built from the effective coefficients (vmg_kernels.cuh "Cell masking")
+        VmgLevel& L = h->lev[0];
+        MaskArgs m;
+        m.mask = h->d_mask; m.cval = h->d_cval; m.a = a; m.bx = bx; m.by = by; m.bz = h->three_d ? bz : nullptr;
+        m.ea = h->m_a; m.ebx = h->m_bx; m.eby = h->m_by; m.ebz = h->m_bz; m.adiag = L.adiag; m.mfold = h->m_fold;
+        m.nx = L.nx; m.ny = L.ny; m.nz = L.nz; m.three_d = h->three_d; m.dirichlet = h->mask_kind == VMG_BC_DIRICHLET;
+        m.cx = beta / (L.hx * L.hx); m.cy = beta / (L.hy * L.hy); m.cz = h->three_d ? beta / (L.hz * L.hz) : 0.0;
+        mask_cells_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(m);
+        mask_faces_kernel<<<grid_for((long long)face_count(L, 0)), kThreads, 0, h->stream>>>(m, 0);
+        mask_faces_kernel<<<grid_for((long long)face_count(L, 1)), kThreads, 0, h->stream>>>(m, 1);
+        if (h->three_d) mask_faces_kernel<<<grid_for((long long)face_count(L, 2)), kThreads, 0, h->stream>>>(m, 2);
+        setup_launches += h->three_d ? 4 : 3;
+        fa = a ? h->m_a : nullptr; fbx = h->m_bx; fby = h->m_by; fbz = h->three_d ? h->m_bz : nullptr;
+    }
+    const double* fad = h->d_mask ? h->lev[0].adiag : nullptr;
     for (int l = 0; l < h->nlev; ++l) {
         VmgLevel& L = h->lev[l];
         if (l > 0) {   // S0: average the previous level's raw coefficients
@@ -259,11 +276,17 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
             coarsen_b_kernel<<<grid_for((long long)face_count(L, 1)), kThreads, 0, h->stream>>>(fby, L.by, L.nx, L.ny, L.nz, sz, 1);
             if (h->three_d)
                 coarsen_b_kernel<<<grid_for((long long)face_count(L, 2)), kThreads, 0, h->stream>>>(fbz, L.bz, L.nx, L.ny, L.nz, sz, 2);
+            if (fad) {   // the extra diagonal is averaged like a
+                coarsen_a_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(fad, L.adiag, L.nx, L.ny, L.nz, sz);
+                fad = L.adiag;
+                ++setup_launches;
+            }
             fa = L.a; fbx = L.bx; fby = L.by; fbz = h->three_d ? L.bz : nullptr;
             setup_launches += h->three_d ? 4 : 3;
         }
         StencilBuildArgs g;
         g.a = (l == 0 && !a) ? nullptr : fa;
+        g.adiag = fad;
         g.bx = fbx; g.by = fby; g.bz = fbz;
         g.wx = L.wx; g.wy = L.wy; g.wz = L.wz; g.dbase = L.dbase;
         for (int f = 0; f < 6; ++f) g.wb[f] = L.wb[f];
@@ -300,6 +323,44 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     h->have_bc = true;
     h->dinv_dirty = true;
+    return VMG_OK;
+}
+
+int vmg_set_mask(vmg_handle h, const unsigned char* mask, int kind, const double* cval)
+{
+    if (!h || (kind != VMG_BC_DIRICHLET && kind != VMG_BC_NEUMANN)) return VMG_ERR_ARG;
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (h->mask_base) { cudaFree(h->mask_base); h->mask_base = nullptr; }
+    h->d_mask = nullptr; h->d_cval = nullptr; h->m_fold = h->m_a = h->m_bx = h->m_by = h->m_bz = nullptr;
+    for (int l = 0; l < h->nlev; ++l) h->lev[l].adiag = nullptr;
+    h->mask_covered = 0;
+    h->have_coeffs = false;            // the stencil has to be rebuilt: vmg_set_coeffs applies the mask
+    h->graph_valid = false; ++h->graph_epoch;
+    if (!mask) return VMG_OK;
+    VmgLevel& L0 = h->lev[0];
+    // one allocation: [doubles: cval, m_fold, m_a, m_bx, m_by, m_bz, adiag of every level][bytes: mask]
+    ArenaPlan p;
+    size_t o_cval = p.take((size_t)L0.n), o_fold = p.take((size_t)L0.n), o_a = p.take((size_t)L0.n);
+    size_t o_bx = p.take(face_count(L0, 0)), o_by = p.take(face_count(L0, 1)), o_bz = p.take(face_count(L0, 2));
+    std::vector<size_t> o_ad((size_t)h->nlev);
+    for (int l = 0; l < h->nlev; ++l) o_ad[l] = p.take((size_t)h->lev[l].n);
+    size_t o_mask = p.off;
+    CUDA_TRY(h, cudaMalloc(&h->mask_base, o_mask * sizeof(double) + (size_t)L0.n));
+    double* base = (double*)h->mask_base;
+    h->m_fold = base + o_fold; h->m_a = base + o_a; h->m_bx = base + o_bx; h->m_by = base + o_by; h->m_bz = base + o_bz;
+    for (int l = 0; l < h->nlev; ++l) h->lev[l].adiag = base + o_ad[l];
+    h->d_mask = (unsigned char*)(base + o_mask);
+    h->mask_kind = kind;
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_mask, mask, (size_t)L0.n, cudaMemcpyDeviceToDevice, h->stream));
+    if (cval) {
+        h->d_cval = base + o_cval;
+        CUDA_TRY(h, cudaMemcpyAsync(h->d_cval, cval, (size_t)L0.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    }
+    // the number of covered cells decides whether a Dirichlet mask pins the solution (setup path: counted on the host)
+    std::vector<unsigned char> hm((size_t)L0.n);
+    CUDA_TRY(h, cudaMemcpyAsync(hm.data(), h->d_mask, (size_t)L0.n, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    for (unsigned char v : hm) h->mask_covered += v == 0;
     return VMG_OK;
 }
 
@@ -369,7 +430,7 @@ int solve_begin(vmg_s* h, const double* rhs, double* phi, double rtol, int max_v
     if (rc != VMG_OK) return rc;
     {
         ProfScope ps(h, VMG_PC_COPY, nullptr);
-        to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, L0.phi);
+        to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, L0.phi, h->d_mask);
     }
     CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
     {
@@ -526,7 +587,7 @@ int solve_pcg_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int ma
 
     int rc = enqueue_fold_bc(h, rhs, r);
     if (rc != VMG_OK) return rc;
-    to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, h->pcg_x);
+    to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, h->pcg_x, h->d_mask);
     CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
     norm_inf_kernel<<<glin, kThreads, 0, h->stream>>>(r, n, scal + 0);
     pcg_residual_inplace_kernel<<<gpair, kPcgThreads, 0, h->stream>>>(v, h->pcg_x, r);

@@ -41,6 +41,7 @@ struct VmgLevel {
     double* wb[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     // averaged raw coefficients in the public layout (levels >= 1 only; level 0 reads the caller's arrays)
     double *a = nullptr, *bx = nullptr, *by = nullptr, *bz = nullptr;
+    double* adiag = nullptr;  // masking: extra diagonal of this level, public layout (nullptr without a mask)
 };
 
 struct vmg_s {
@@ -84,6 +85,12 @@ struct vmg_s {
     int sv_max = 0, sv_slow = 0, sv_status = 0;
     bool sv_active = false;
     double* sv_phi = nullptr;
+    // cell masking (vmg_set_mask): device copies and the effective level-0 coefficients, one allocation
+    void* mask_base = nullptr;
+    unsigned char* d_mask = nullptr;
+    double *d_cval = nullptr, *m_fold = nullptr, *m_a = nullptr, *m_bx = nullptr, *m_by = nullptr, *m_bz = nullptr;
+    int mask_kind = 1;
+    long long mask_covered = 0;
     // MG-preconditioned CG (vmg_solve_pcg): x, p, q in the internal layout, partial sums, device scalars; allocated on first use
     void* pcg_base = nullptr;
     double *pcg_x = nullptr, *pcg_p = nullptr, *pcg_q = nullptr, *pcg_partial = nullptr, *pcg_scal = nullptr;

@@ -120,6 +120,7 @@ __global__ void coarsen_b_kernel(const double* __restrict__ fb, double* __restri
 // ------------------------------------------------------------------------------------------------
 struct StencilBuildArgs {
     const double *a, *bx, *by, *bz;      // raw, public layout (may be NULL)
+    const double* adiag;                 // masking: extra diagonal of this level, public layout (NULL without a mask)
     double *wx, *wy, *wz, *dbase;        // internal cell arrays
     double* wb[6];                       // boundary planes (natural plane layout)
     Geom G;
@@ -156,6 +157,7 @@ __global__ void build_stencil_kernel(StencilBuildArgs g)
     const long long c = cell_at(g.G, i, j, k);
     g.wx[c] = wxl; g.wy[c] = wyl; g.wz[c] = wzl;
     double d = g.a ? g.alpha * g.a[t] : 0.0;
+    if (g.adiag) d += g.adiag[t];
     d += wxl; d += wxh; d += wyl; d += wyh; d += wzl; d += wzh;
     g.dbase[c] = d;
 }
@@ -193,6 +195,7 @@ __global__ void finalize_dinv_kernel(DinvArgs g)
 // ------------------------------------------------------------------------------------------------
 struct FoldArgs {
     const double* rhs; double* bt; const double* wb[6]; const double* val[6];
+    const unsigned char* mask; const double* mfold;   // masking (NULL without a mask): interface terms, covered cells -> 0
     Geom G;
     int three_d, bt_natural; int dirichlet[6]; double h[3];
 };
@@ -218,17 +221,19 @@ __global__ void fold_bc_kernel(FoldArgs g)
         if (k == 0)      add(4, i + (long long)nx * j, g.h[2]);
         if (k == nz - 1) add(5, i + (long long)nx * j, g.h[2]);
     }
+    if (g.mask) v = g.mask[t] ? v + g.mfold[t] : 0.0;
     g.bt[g.bt_natural ? t : cell_at(g.G, i, j, k)] = v;
 }
 
 // public (natural) layout <-> internal layout of one cell array
-__global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in)
+// mask (may be NULL): covered cells enter as zero (they are identity rows of the masked operator)
+__global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in, const unsigned char* __restrict__ mask)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (t >= G.n) return;
     int i, j, k;
     unflatten(G, t, i, j, k);
-    in[cell_at(G, i, j, k)] = nat[t];
+    in[cell_at(G, i, j, k)] = (mask && !mask[t]) ? 0.0 : nat[t];
 }
 __global__ void to_natural_kernel(Geom G, const double* __restrict__ in, double* __restrict__ nat)
 {
@@ -237,6 +242,70 @@ __global__ void to_natural_kernel(Geom G, const double* __restrict__ in, double*
     int i, j, k;
     unflatten(G, t, i, j, k);
     nat[t] = in[cell_at(G, i, j, k)];
+}
+
+// ------------------------------------------------------------------------------------------------
+// Cell masking (reading N4 in DESIGN.md): covered cells are identity rows, a face
+// between a valid and a covered cell is an interior boundary of one kind -- Dirichlet with the value the covered cell
+// carries, or zero flux.  Realised on the level-0 raw coefficients, so that averaging, stencil build and every solver
+// kernel run unchanged: effective a (0 in covered cells), effective b (0 on every face that touches a covered cell),
+// an extra diagonal (2 beta b/h^2 per Dirichlet interface face of a valid cell, 1 in a covered cell; averaged to the
+// coarse levels like a) and the interface terms of btilde.  All arrays in the public layout.
+// ------------------------------------------------------------------------------------------------
+struct MaskArgs {
+    const unsigned char* mask; const double* cval;      // cval may be NULL (0)
+    const double *a, *bx, *by, *bz;                      // the caller's coefficients (may be NULL)
+    double *ea, *ebx, *eby, *ebz, *adiag, *mfold;        // effective coefficients, extra diagonal, interface terms
+    int nx, ny, nz, three_d, dirichlet;
+    double cx, cy, cz;                                   // beta / h^2
+};
+
+__global__ void mask_cells_kernel(MaskArgs g)
+{
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const long long n = (long long)g.nx * g.ny * g.nz, nxy = (long long)g.nx * g.ny;
+    if (t >= n) return;
+    int i = (int)(t % g.nx), j = (int)((t / g.nx) % g.ny), k = (int)(t / nxy);
+    if (!g.mask[t]) { g.ea[t] = 0.0; g.adiag[t] = 1.0; g.mfold[t] = 0.0; return; }
+    g.ea[t] = g.a ? g.a[t] : 0.0;
+    double ad = 0.0, mf = 0.0;
+    if (g.dirichlet) {
+        auto face = [&](bool inside, long long nb, double b, double c) {   // nb: the neighbour cell across the face
+            if (!inside || g.mask[nb]) return;
+            ad += 2.0 * c * b;
+            mf += 2.0 * c * b * (g.cval ? g.cval[nb] : 0.0);
+        };
+        const long long fx = i + (long long)(g.nx + 1) * (j + (long long)g.ny * k), fy = i + (long long)g.nx * (j + (long long)(g.ny + 1) * k);
+        face(i > 0, t - 1, g.bx ? g.bx[fx] : 1.0, g.cx);
+        face(i < g.nx - 1, t + 1, g.bx ? g.bx[fx + 1] : 1.0, g.cx);
+        face(j > 0, t - g.nx, g.by ? g.by[fy] : 1.0, g.cy);
+        face(j < g.ny - 1, t + g.nx, g.by ? g.by[fy + g.nx] : 1.0, g.cy);
+        if (g.three_d) {
+            face(k > 0, t - nxy, g.bz ? g.bz[t] : 1.0, g.cz);
+            face(k < g.nz - 1, t + nxy, g.bz ? g.bz[t + nxy] : 1.0, g.cz);
+        }
+    }
+    g.adiag[t] = ad; g.mfold[t] = mf;
+}
+
+// dir: 0 x faces, 1 y faces, 2 z faces: b = 0 on every face that touches a covered cell
+__global__ void mask_faces_kernel(MaskArgs g, int dir)
+{
+    const int ex = g.nx + (dir == 0), ey = g.ny + (dir == 1), ez = g.nz + (dir == 2);
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= (long long)ex * ey * ez) return;
+    int i = (int)(t % ex), j = (int)((t / ex) % ey), k = (int)(t / ((long long)ex * ey));
+    const double* b = dir == 0 ? g.bx : dir == 1 ? g.by : g.bz;
+    double* eb = dir == 0 ? g.ebx : dir == 1 ? g.eby : g.ebz;
+    const int lim = dir == 0 ? g.nx : dir == 1 ? g.ny : g.nz, pos = dir == 0 ? i : dir == 1 ? j : k;
+    auto cell = [&](int d) {                             // the cell on the low (d = -1) / high (d = 0) side of the face
+        int ci = i + (dir == 0 ? d : 0), cj = j + (dir == 1 ? d : 0), ck = k + (dir == 2 ? d : 0);
+        return (long long)ci + (long long)g.nx * (cj + (long long)g.ny * ck);
+    };
+    bool open = true;
+    if (pos > 0) open = open && g.mask[cell(-1)];
+    if (pos < lim) open = open && g.mask[cell(0)];
+    eb[t] = open ? (b ? b[t] : 1.0) : 0.0;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -98,6 +98,7 @@ inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt, bool bt_natu
         g.dirichlet[f] = h->bctype[f] == VMG_BC_DIRICHLET;
     }
     g.G = L.G; g.three_d = h->three_d; g.bt_natural = bt_natural;
+    g.mask = h->d_mask; g.mfold = h->m_fold;
     g.h[0] = L.hx; g.h[1] = L.hy; g.h[2] = L.hz;
     {
         ProfScope ps(h, VMG_PC_FOLD, nullptr);

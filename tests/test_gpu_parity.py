@@ -496,3 +496,163 @@ def test_more_shapes_parity(dims, spacing):
         return
     p = inputs.random_problem(*dims, seed=17, bc_type=[N, D, D, N, N, D], spacing=spacing)
     check_parity(p)
+
+
+def _mask_for(p, seed=5):
+    """Covered geometry of the paper's kind (electrodes / dielectric bodies inside the box): a ball, a slab that
+    touches two domain faces, and a few isolated covered cells, so that coarse cells end up fully, partly and not covered."""
+    nz, ny, nx = p.rhs.shape
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    mask = np.ones(p.rhs.shape, dtype=np.uint8)
+    r = max(2.0, 0.22 * min(nx, ny, nz if nz > 1 else nx))
+    mask[(i - 0.55 * nx) ** 2 + (j - 0.45 * ny) ** 2 + ((k - 0.5 * nz) ** 2 if nz > 1 else 0) < r * r] = 0
+    mask[: max(1, nz // 3), : max(1, ny // 5), nx // 8: nx // 8 + 3] = 0
+    rng = np.random.default_rng(seed)
+    mask[rng.random(p.rhs.shape) < 0.003] = 0
+    cval = np.where(mask == 0, 0.5 + 0.2 * rng.standard_normal(p.rhs.shape), 0.0)
+    return mask, cval
+
+
+@pytest.mark.parametrize("kind", [D, N], ids=["dirichlet_interface", "neumann_interface"])
+@pytest.mark.parametrize("dims", [(40, 24, 16), (48, 40, 1), (64, 64, 32)])
+def test_masked_solve_matches_oracle(dims, kind):
+    """vmg_set_mask against ovmg_set_mask: folded right-hand side, V-cycle solve and PCG on a
+    domain with covered cells, both interface kinds; covered cells come back exactly 0; removing the mask restores the
+    unmasked solve bit for bit."""
+    b = _binding()
+    p = inputs.random_problem(*dims, seed=23, bc_type=[D, N, N, D, N, N])
+    mask, cval = _mask_for(p)
+    cv = cval if kind == D else None
+    o = Oracle.from_problem(p)
+    o.set_mask(mask, kind, cv)
+    o.set_coeffs(p.a, p.bx, p.by, p.bz, p.alpha, p.beta)
+    s, d = b.from_problem(p)
+    phi_plain = torch.zeros_like(d["rhs"])
+    s.solve(d["rhs"], phi_plain, rtol=1e-12, max_vcycles=60)
+    s.set_mask(dev(mask), kind, None if cv is None else dev(cv))
+    with pytest.raises(b.VmgError) as e:                       # the coefficients have to be set again
+        s.solve(d["rhs"], torch.zeros_like(d["rhs"]))
+    assert e.value.code == -3
+    s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+    bt = s.step_fold_bc(d["rhs"])
+    bt_o = o.fold_bc(p.rhs)
+    assert np.abs(bt.cpu().numpy() - bt_o).max() <= 1e-13 * np.abs(bt_o).max()
+    phi_o, st_o, cyc_o, rr_o, hist_o = o.solve(p.rhs, rtol=1e-12, max_vcycles=60)
+    phi = torch.full_like(d["rhs"], 3.0)                       # a guess that is non-zero in covered cells
+    phi0 = np.full(p.rhs.shape, 3.0)
+    phi_o2, st_o2, cyc_o2, _, _ = o.solve(p.rhs, phi0, rtol=1e-12, max_vcycles=60)
+    st = s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=60)
+    cyc, rr, hist = s.get_info()
+    assert st == st_o2 == 0 and abs(cyc - cyc_o2) <= 1 and rr <= 1e-12
+    g = phi.cpu().numpy()
+    assert np.all(g[mask == 0] == 0.0)
+    assert rel(g, phi_o2) <= PHI_TOL
+    phi = torch.zeros_like(d["rhs"])
+    assert s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=60) == st_o
+    cyc, rr, hist = s.get_info()
+    assert abs(cyc - cyc_o) <= 1 and rel(phi.cpu().numpy(), phi_o) <= PHI_TOL
+    m = min(len(hist), len(hist_o))
+    live = hist_o[:m] > 1e-11
+    assert np.all(np.abs(np.array(hist)[:m][live] / hist_o[:m][live] - 1.0) < 1e-3)
+    phi_po, st_po, it_po, _, _ = o.solve_pcg(p.rhs, rtol=1e-12, max_iter=60)
+    phi = torch.zeros_like(d["rhs"])
+    assert s.solve_pcg(d["rhs"], phi, rtol=1e-12, max_iter=60) == st_po == 0
+    it, rr, _ = s.get_info()
+    assert abs(it - it_po) <= 1 and rel(phi.cpu().numpy(), phi_po) <= PHI_TOL
+    assert np.all(phi.cpu().numpy()[mask == 0] == 0.0)
+    s.set_mask(None)
+    s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+    phi = torch.zeros_like(d["rhs"])
+    s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=60)
+    assert torch.equal(phi, phi_plain)
+    s.destroy()
+    o.close()
+
+
+def test_masked_electrode_regularises_the_all_neumann_problem():
+    """All-Neumann Poisson is singular (VMG_ERR_SINGULAR) until a covered block with a Dirichlet interface pins phi; with a
+    zero-flux interface it stays singular; an all-valid Dirichlet mask changes nothing."""
+    b = _binding()
+    p = inputs.random_problem(32, 32, 16, seed=4, bc_type=[N] * 6, inhomogeneous=False)
+    s, d = b.from_problem(p)
+    s.set_coeffs(None, d["bx"], d["by"], d["bz"], 0.0, p.beta)
+    phi = torch.zeros_like(d["rhs"])
+    with pytest.raises(b.VmgError) as e:
+        s.solve(d["rhs"], phi)
+    assert e.value.code == -4
+    mask = np.ones(p.rhs.shape, dtype=np.uint8)
+    for kind, ok in ((D, False), (N, False)):                  # no covered cell: still singular
+        s.set_mask(dev(mask), kind)
+        s.set_coeffs(None, d["bx"], d["by"], d["bz"], 0.0, p.beta)
+        with pytest.raises(b.VmgError) as e:
+            s.solve(d["rhs"], phi)
+        assert e.value.code == -4
+    mask[6:10, 12:20, 12:20] = 0
+    s.set_mask(dev(mask), N)
+    s.set_coeffs(None, d["bx"], d["by"], d["bz"], 0.0, p.beta)
+    with pytest.raises(b.VmgError) as e:
+        s.solve(d["rhs"], phi)
+    assert e.value.code == -4
+    cval = np.where(mask == 0, 1.0, 0.0)
+    s.set_mask(dev(mask), D, dev(cval))
+    s.set_coeffs(None, d["bx"], d["by"], d["bz"], 0.0, p.beta)
+    o = Oracle.from_problem(p)
+    o.set_mask(mask, D, cval)
+    o.set_coeffs(None, p.bx, p.by, p.bz, 0.0, p.beta)
+    phi_o, st_o, cyc_o, _, _ = o.solve(p.rhs, rtol=1e-11, max_vcycles=80)
+    st = s.solve(d["rhs"], phi, rtol=1e-11, max_vcycles=80)
+    cyc, rr, _ = s.get_info()
+    assert st == st_o == 0 and abs(cyc - cyc_o) <= 1 and rel(phi.cpu().numpy(), phi_o) <= PHI_TOL
+    s.destroy()
+    o.close()
+
+
+@pytest.mark.parametrize("opts", [dict(prolong=1), dict(blocked=1, block_min_cells=0), dict(graph=0, tail=0), dict(snake=0, pdl=0, l2_persist=0),
+                                  dict(nu1=2, nu2=1, bottom_sweeps=8)],
+                         ids=["trilinear", "blocked", "no_graph_no_tail", "plain_schedule", "v21"])
+def test_masked_solve_under_options(opts):
+    """The mask lives in the stencil arrays, so every schedule / kernel variant has to solve the same masked problem."""
+    b = _binding()
+    p = inputs.random_problem(72, 40, 24, seed=31, bc_type=[N, D, D, N, D, N])
+    mask, cval = _mask_for(p, seed=9)
+    o = Oracle.from_problem(p)
+    o.set_mask(mask, D, cval)
+    o.set_coeffs(p.a, p.bx, p.by, p.bz, p.alpha, p.beta)
+    s, d = b.from_problem(p)
+    s.set_mask(dev(mask), D, dev(cval))
+    s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+    for k, v in opts.items():
+        if k in ("nu1", "nu2", "bottom_sweeps", "prolong"):
+            o.set_option(k, v)
+        s.set_option(k, v)
+    phi_o, st_o, cyc_o, _, hist_o = o.solve(p.rhs, rtol=1e-12, max_vcycles=60)
+    phi = torch.zeros_like(d["rhs"])
+    st = s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=60)
+    cyc, rr, hist = s.get_info()
+    assert st == st_o == 0 and abs(cyc - cyc_o) <= 1
+    assert rel(phi.cpu().numpy(), phi_o) <= PHI_TOL
+    assert np.all(phi.cpu().numpy()[mask == 0] == 0.0)
+    s.destroy()
+    o.close()
+
+
+def test_masked_full_size_parity():
+    """256x128x128 (config 3's grid and coefficients) with an electrode ball and a dielectric-like slab covered: the launch
+    configuration bench.py times, element by element against the oracle."""
+    b = _binding()
+    p = inputs.config3(128)
+    mask, cval = _mask_for(p, seed=2)
+    o = Oracle.from_problem(p)
+    o.set_mask(mask, D, cval)
+    o.set_coeffs(p.a, p.bx, p.by, p.bz, p.alpha, p.beta)
+    s, d = b.from_problem(p)
+    s.set_mask(dev(mask), D, dev(cval))
+    s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+    phi_o, st_o, cyc_o, _, _ = o.solve(p.rhs, rtol=1e-11, max_vcycles=40)
+    phi = torch.zeros_like(d["rhs"])
+    st = s.solve(d["rhs"], phi, rtol=1e-11, max_vcycles=40)
+    cyc, rr, _ = s.get_info()
+    assert st == st_o == 0 and abs(cyc - cyc_o) <= 1, (st, st_o, cyc, cyc_o)
+    assert rel(phi.cpu().numpy(), phi_o) <= PHI_TOL
+    s.destroy()
+    o.close()
