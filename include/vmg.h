@@ -60,7 +60,10 @@ enum {
 int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream);
 
 /* Coefficients.  a: cell array or NULL (a == 0, alpha ignored).  bx, by, bz: face arrays, or all NULL for
- * b == 1.  a must be >= 0 with alpha >= 0 and b > 0, beta > 0 (not checked; otherwise undefined behaviour).
+ * b == 1 (then, unless a mask is set, the sweeps, the residual + restriction and the residual norm run as kernels that form
+ * the face weights from beta/h^2 and the cell's position instead of loading three weight arrays: the same numbers in
+ * the same order, bitwise the results of explicit arrays of ones, at 2 instead of 5 doubles of traffic per cell and
+ * half-sweep -- the Poisson equation PAPER.md:54 Eq. 3 and Helmholtz equations with a variable a).  a must be >= 0 with alpha >= 0 and b > 0, beta > 0 (not checked; otherwise undefined behaviour).
  * The arrays are read during this call only (enqueued on the stream, then synchronised): the library
  * averages them to all coarse levels (a: mean of the 8 children, 4 in 2-D; b: mean of the fine faces lying
  * on the coarse face) and converts each level to its internal stencil form.  The caller may free or modify
@@ -134,6 +137,8 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  * "blocked" (1: temporally blocked smoother passes with fused transfers (vmg_block2.cuh); 0: one kernel per
  *   colour half-sweep, default -- the blocked passes are bitwise equal but measure slower on B200),
  * "block_min_cells" (smallest level the blocked passes are used on when blocked = 1, default 4096),
+ * "const_weights" (1: use the constant-weight kernels when b == NULL, default; 0: always load the weight arrays; takes
+ *   effect at the next vmg_set_coeffs, which must follow),
  * "profile" (1: per-kernel-class event timing, see vmg_get_profile; implies plain launches; default 0). */
 int vmg_set_option(vmg_handle h, const char* key, double v);
 

@@ -122,7 +122,7 @@ int apply_l2_window(vmg_s* h)
     CUDA_TRY(h, cudaStreamSetAttribute(h->stream, cudaStreamAttributeAccessPolicyWindow, &a));
     if (!want) CUDA_TRY(h, cudaCtxResetPersistingL2Cache());
     h->l2_window_set = want != 0;
-    { h->graph_valid = false; ++h->graph_epoch; }
+    { ++h->graph_epoch; }
     return VMG_OK;
 }
 
@@ -222,14 +222,16 @@ int vmg_destroy(vmg_handle h)
     cudaStreamSynchronize(h->stream);
     prof_collect(h);
     for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < 4; ++i) {
         if (h->pcg_exec[i]) cudaGraphExecDestroy(h->pcg_exec[i]);
         if (h->pcg_graph[i]) cudaGraphDestroy(h->pcg_graph[i]);
     }
     if (h->pcg_base) cudaFree(h->pcg_base);
     if (h->mask_base) cudaFree(h->mask_base);
-    if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
-    if (h->graph) cudaGraphDestroy(h->graph);
+    for (int i = 0; i < 2; ++i) {
+        if (h->graph_exec[i]) cudaGraphExecDestroy(h->graph_exec[i]);
+        if (h->graph[i]) cudaGraphDestroy(h->graph[i]);
+    }
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->arena) cudaFree(h->arena);
     if (h->own_stream) cudaStreamDestroy(h->stream);
@@ -268,6 +270,11 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
         fa = a ? h->m_a : nullptr; fbx = h->m_bx; fby = h->m_by; fbz = h->three_d ? h->m_bz : nullptr;
     }
     const double* fad = h->d_mask ? h->lev[0].adiag : nullptr;
+    const int cw = (!bx && !h->d_mask && h->const_weights) ? 1 : 0;   // b = 1 on every face of every level (LevelView::cw)
+    {   // the constant-weight kernels take beta/h^2 by value: graphs captured with another beta are stale
+        const VmgLevel& L = h->lev[0];
+        if (cw && (L.cx != beta / (L.hx * L.hx) || L.cy != beta / (L.hy * L.hy))) ++h->graph_epoch;
+    }
     for (int l = 0; l < h->nlev; ++l) {
         VmgLevel& L = h->lev[l];
         if (l > 0) {   // S0: average the previous level's raw coefficients
@@ -293,6 +300,7 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
         g.G = L.G; g.three_d = h->three_d;
         g.alpha = h->alpha; g.cx = beta / (L.hx * L.hx); g.cy = beta / (L.hy * L.hy);
         g.cz = h->three_d ? beta / (L.hz * L.hz) : 0.0;
+        L.cx = g.cx; L.cy = g.cy; L.cz = g.cz; L.cw = cw;
         build_stencil_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(g);
         ++setup_launches;
     }
@@ -312,7 +320,7 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
     for (int f = 0; f < 6; ++f)
         if (type[f] != VMG_BC_DIRICHLET && type[f] != VMG_BC_NEUMANN) return VMG_ERR_ARG;
     for (int f = 0; f < 6; ++f) {
-        if (h->bctype[f] != type[f]) { h->graph_valid = false; ++h->graph_epoch; }   // the trilinear prolongation kernels carry the types by value
+        if (h->bctype[f] != type[f]) { ++h->graph_epoch; }   // the trilinear prolongation kernels carry the types by value
         h->bctype[f] = type[f];
         bool active = f < 4 || h->three_d;
         h->bc_has_value[f] = active && value && value[f];
@@ -335,7 +343,7 @@ int vmg_set_mask(vmg_handle h, const unsigned char* mask, int kind, const double
     for (int l = 0; l < h->nlev; ++l) h->lev[l].adiag = nullptr;
     h->mask_covered = 0;
     h->have_coeffs = false;            // the stencil has to be rebuilt: vmg_set_coeffs applies the mask
-    h->graph_valid = false; ++h->graph_epoch;
+    ++h->graph_epoch;
     if (!mask) return VMG_OK;
     VmgLevel& L0 = h->lev[0];
     // one allocation: [doubles: cval, m_fold, m_a, m_bx, m_by, m_bz, adiag of every level][bytes: mask]
@@ -373,6 +381,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "bottom_sweeps")) { if (iv < 1) return VMG_ERR_ARG; h->nbottom = iv; }
     else if (!strcmp(key, "prolong")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->prolong = iv; }
     else if (!strcmp(key, "symmetric")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->symmetric = iv; }
+    else if (!strcmp(key, "const_weights")) { h->const_weights = iv != 0; h->have_coeffs = false; }   // takes effect in vmg_set_coeffs
     else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
     else if (!strcmp(key, "blocked")) { h->use_blocked = iv != 0; }
     else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }
@@ -385,7 +394,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
         for (int c = 0; c < VMG_PC_COUNT; ++c) { h->prof_ms[c] = 0.0; h->prof_launches[c] = 0; }
     }
     else return VMG_ERR_ARG;
-    { h->graph_valid = false; ++h->graph_epoch; }
+    { ++h->graph_epoch; }
     plan_schedule(h);
     return VMG_OK;
 }
@@ -559,6 +568,7 @@ int pcg_alloc(vmg_s* h)
 template <typename F>
 int pcg_run(vmg_s* h, int slot, F body)
 {
+    slot += h->lev[0].cw ? 2 : 0;
     if (!h->use_graph || h->profile) { body(); return cudaGetLastError() == cudaSuccess ? VMG_OK : VMG_ERR_CUDA; }
     if (h->pcg_epoch[slot] != h->graph_epoch) {
         if (h->pcg_exec[slot]) { cudaGraphExecDestroy(h->pcg_exec[slot]); h->pcg_exec[slot] = nullptr; }

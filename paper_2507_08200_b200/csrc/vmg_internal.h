@@ -41,6 +41,8 @@ struct VmgLevel {
     double* wb[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     // averaged raw coefficients in the public layout (levels >= 1 only; level 0 reads the caller's arrays)
     double *a = nullptr, *bx = nullptr, *by = nullptr, *bz = nullptr;
+    double cx = 0.0, cy = 0.0, cz = 0.0;   // beta / h^2 of this level
+    int cw = 0;                             // constant face weights (LevelView::cw)
     double* adiag = nullptr;  // masking: extra diagonal of this level, public layout (nullptr without a mask)
 };
 
@@ -58,6 +60,7 @@ struct vmg_s {
     bool bc_has_value[6] = {false, false, false, false, false, false};
     bool have_coeffs = false, have_bc = false, dinv_dirty = true;
     int nu1 = 3, nu2 = 3, nbottom = 32;
+    int const_weights = 1;                  // option "const_weights": use the constant-weight kernels when b == NULL
     int prolong = 0;              // 0: piecewise constant (R9 default), 1: trilinear
     int symmetric = 0;            // 1: symmetric V-cycle (post-smoothing / second half of the bottom black -> red): the PCG preconditioner
     int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200
@@ -77,9 +80,12 @@ struct vmg_s {
     void* arena = nullptr;
     size_t arena_bytes = 0;
     // graph of one V-cycle (+ residual norm)
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t graph_exec = nullptr;
-    bool graph_valid = false;
+    // two slots: [0] general kernels, [1] constant-weight kernels (LevelView::cw), so that a time step that alternates
+    // between the two kinds of equation re-instantiates nothing; a slot is current when its epoch equals graph_epoch
+    cudaGraph_t graph[2] = {nullptr, nullptr};
+    cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
+    unsigned graph_slot_epoch[2] = {0, 0};
+    long long graph_slot_launches[2] = {0, 0};
     // state of the solve in progress (vmg_solve / vmg_solve_batch phases)
     double sv_rtol = 0.0, sv_nb = 0.0;
     int sv_max = 0, sv_slow = 0, sv_status = 0;
@@ -95,9 +101,9 @@ struct vmg_s {
     void* pcg_base = nullptr;
     double *pcg_x = nullptr, *pcg_p = nullptr, *pcg_q = nullptr, *pcg_partial = nullptr, *pcg_scal = nullptr;
     int pcg_npartial = 0;
-    cudaGraph_t pcg_graph[2] = {nullptr, nullptr};
-    cudaGraphExec_t pcg_exec[2] = {nullptr, nullptr};
-    unsigned pcg_epoch[2] = {0, 0};
+    cudaGraph_t pcg_graph[4] = {nullptr, nullptr, nullptr, nullptr};       // [slot + 2 * cw]
+    cudaGraphExec_t pcg_exec[4] = {nullptr, nullptr, nullptr, nullptr};
+    unsigned pcg_epoch[4] = {0, 0, 0, 0};
     unsigned graph_epoch = 1;          // bumped whenever captured graphs become stale
     // result of the last solve
     int cycles = 0;

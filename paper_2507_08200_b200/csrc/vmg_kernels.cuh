@@ -315,7 +315,29 @@ __global__ void mask_faces_kernel(MaskArgs g, int dir)
 struct LevelView {
     const double *wx, *wy, *wz, *dinv;
     Geom G;
+    // constant face weights (b == NULL in vmg_set_coeffs, i.e. b = 1 on every face of every level, and no mask: the
+    // Poisson equation PAPER.md:54 Eq. 3 and the Helmholtz equations of photoionisation): the kernels instantiated
+    // with CW = true take the six weights from these three numbers and the cell's position instead of loading them,
+    // 2 doubles per cell and half-sweep instead of 5.  Same values, same order of operations: bitwise the results
+    // of the general kernels on arrays of ones.
+    double cx, cy, cz;
+    int cw;
 };
+
+// the six face weights of cell (i, j, k): low x, high x, low y, high y, low z, high z
+template <bool CW>
+__device__ __forceinline__ void face_weights(const LevelView& L, long long c, long long xm, int i, int j, int k, double (&w)[6])
+{
+    if (CW) {
+        w[0] = i > 0 ? L.cx : 0.0;  w[1] = i < L.G.nx - 1 ? L.cx : 0.0;
+        w[2] = j > 0 ? L.cy : 0.0;  w[3] = j < L.G.ny - 1 ? L.cy : 0.0;
+        w[4] = k > 0 ? L.cz : 0.0;  w[5] = k < L.G.nz - 1 ? L.cz : 0.0;
+    } else {
+        w[0] = L.wx[c];  w[1] = L.wx[xm + 1];
+        w[2] = L.wy[c];  w[3] = L.wy[c + L.G.pitch];
+        w[4] = L.wz[c];  w[5] = L.wz[c + L.G.plane];
+    }
+}
 
 // c: the cell; xm: its low-x neighbour (the high-x neighbour is xm + 1: E_m sits between O_{m-1} and O_m, O_m between
 // E_m and E_{m+1}).  Same expression, same order, everywhere a relaxation or a residual is evaluated.
@@ -343,6 +365,7 @@ __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, i
 // L2 residency: what the NEXT half-sweep (other colour, opposite direction) needs again are the face weights and the
 // phi written here; rhs, 1/D and the neighbours' phi are dead after this read, so they are loaded with the streaming
 // (evict-first) policy and do not push the weights out of the 126 MB L2.
+template <bool CW>
 __device__ __forceinline__ void relax_one(const LevelView& L, double* phi, const double* rhs, int colour, long long t)
 {
     const Geom& G = L.G;
@@ -352,25 +375,28 @@ __device__ __forceinline__ void relax_one(const LevelView& L, double* phi, const
     if (2 * m + par >= G.nx) return;
     long long c, xm;
     pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
-    double s = L.wx[c] * __ldcs(phi + xm);
-    s = fma(L.wx[xm + 1], __ldcs(phi + xm + 1), s);
-    s = fma(L.wy[c], __ldcs(phi + c - G.pitch), s);
-    s = fma(L.wy[c + G.pitch], __ldcs(phi + c + G.pitch), s);
-    s = fma(L.wz[c], __ldcs(phi + c - G.plane), s);
-    s = fma(L.wz[c + G.plane], __ldcs(phi + c + G.plane), s);
+    double w[6];
+    face_weights<CW>(L, c, xm, 2 * m + par, j, k, w);
+    double s = w[0] * __ldcs(phi + xm);
+    s = fma(w[1], __ldcs(phi + xm + 1), s);
+    s = fma(w[2], __ldcs(phi + c - G.pitch), s);
+    s = fma(w[3], __ldcs(phi + c + G.pitch), s);
+    s = fma(w[4], __ldcs(phi + c - G.plane), s);
+    s = fma(w[5], __ldcs(phi + c + G.plane), s);
     phi[c] = __ldcs(L.dinv + c) * (__ldcs(rhs + c) + s);
 }
 
 // reverse: walk the level from its last plane to its first.  Consecutive half-sweeps alternate direction, so that
 // each one starts on the planes the previous one touched last, which are still in the 126 MB L2 (face weights and
 // the phi just written are common to both colours).
+template <bool CW>
 __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour, int reverse)
 {
     grid_dependency_wait();
     const long long nt = (long long)L.G.ne * L.G.ny * L.G.nz;
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
-    if (t < nt) relax_one(L, phi, rhs, colour, t);
+    if (t < nt) relax_one<CW>(L, phi, rhs, colour, t);
 }
 
 // S4 + S2 fused (per-colour path).  The first colour half-sweep after a coarse-grid correction: a relaxation never
@@ -379,6 +405,7 @@ __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, cons
 // stored: the cells of the other colour keep their uncorrected values in memory until the next half-sweep
 // overwrites them.  Valid when at least one full sweep follows (nu2 >= 1).  phi_nb + e is the very addition
 // prolong_correct_kernel performs, so results are bitwise those of the two separate kernels.
+template <bool CW>
 __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom& CG, double* phi,
                                                   const double* rhs, const double* e, int colour, int sz,
                                                   long long t)
@@ -413,28 +440,48 @@ __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom
     } else {
         // 2-D: no z coupling (wz = 0), the z-neighbours are pads
     }
-    double s = L.wx[c] * vxm;
-    s = fma(L.wx[xm + 1], vxp, s);
-    s = fma(L.wy[c], vym, s);
-    s = fma(L.wy[c + G.pitch], vyp, s);
-    s = fma(L.wz[c], vzm, s);
-    s = fma(L.wz[c + G.plane], vzp, s);
+    double w[6];
+    face_weights<CW>(L, c, xm, i, j, k, w);
+    double s = w[0] * vxm;
+    s = fma(w[1], vxp, s);
+    s = fma(w[2], vym, s);
+    s = fma(w[3], vyp, s);
+    s = fma(w[4], vzm, s);
+    s = fma(w[5], vzp, s);
     phi[c] = L.dinv[c] * (rhs[c] + s);
 }
 
+template <bool CW>
 __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __restrict__ phi, const double* __restrict__ rhs,
                                              const double* __restrict__ e, int colour, int sz, int reverse)
 {
     grid_dependency_wait();
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
-    if (t < (long long)L.G.ne * L.G.ny * L.G.nz) relax_prolong_one(L, CG, phi, rhs, e, colour, sz, t);
+    if (t < (long long)L.G.ne * L.G.ny * L.G.nz) relax_prolong_one<CW>(L, CG, phi, rhs, e, colour, sz, t);
 }
 
 // r = rhs - A phi, A phi = D phi - sum w phi_nb, D = 1/dinv.
 __device__ __forceinline__ double residual_at(const LevelView& L, const double* phi, const double* rhs, long long c, long long xm)
 {
     return rhs[c] + nb_sum(L, phi, c, xm) - phi[c] / L.dinv[c];
+}
+
+// the same with the cell's position known (CW = true: constant face weights, see LevelView)
+template <bool CW>
+__device__ __forceinline__ double residual_at(const LevelView& L, const double* phi, const double* rhs, long long c, long long xm,
+                                              int i, int j, int k)
+{
+    if (!CW) return residual_at(L, phi, rhs, c, xm);
+    double w[6];
+    face_weights<true>(L, c, xm, i, j, k, w);
+    double s = w[0] * phi[xm];
+    s = fma(w[1], phi[xm + 1], s);
+    s = fma(w[2], phi[c - L.G.pitch], s);
+    s = fma(w[3], phi[c + L.G.pitch], s);
+    s = fma(w[4], phi[c - L.G.plane], s);
+    s = fma(w[5], phi[c + L.G.plane], s);
+    return rhs[c] + s - phi[c] / L.dinv[c];
 }
 
 // r in the public layout (single-step entry point)
@@ -453,6 +500,7 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 // S3 (per-colour path). Fused residual + restriction: one thread per coarse cell; also zeroes the coarse phi.
 // (Four lanes per coarse cell with a shuffle gather was tried: 70 us instead of 49 us on 256x128x128, the 64-byte
 // runs per row coalesce worse than they gain in occupancy.)
+template <bool CW>
 __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG, const double* phi,
                                              const double* rhs, double* crhs, double* cphi,
                                              int sz, long long t)
@@ -462,23 +510,25 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
     double s = 0.0;
     for (int r = 0; r < sz; ++r)
         for (int q = 0; q < 2; ++q) {   // the x-pair first, then accumulated (the blocked kernel sums in this order too)
-            long long row = L.G.plane * (sz * K + r) + (long long)L.G.pitch * (2 * J + q), ce, xe, co, xo;
+            const int j = 2 * J + q, k = sz * K + r;
+            long long row = L.G.plane * k + (long long)L.G.pitch * j, ce, xe, co, xo;
             pair_addr(L.G, row, I, 0, ce, xe);
             pair_addr(L.G, row, I, 1, co, xo);
-            s += residual_at(L, phi, rhs, ce, xe) + residual_at(L, phi, rhs, co, xo);
+            s += residual_at<CW>(L, phi, rhs, ce, xe, 2 * I, j, k) + residual_at<CW>(L, phi, rhs, co, xo, 2 * I + 1, j, k);
         }
     const long long cc = cell_at(CG, I, J, K);
     crhs[cc] = s / (4.0 * sz);
     if (cphi) cphi[cc] = 0.0;
 }
 
+template <bool CW>
 __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
                                          double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
 {
     grid_dependency_wait();
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
-    if (t < CG.n) restrict_one(L, CG, phi, rhs, crhs, cphi, sz, t);
+    if (t < CG.n) restrict_one<CW>(L, CG, phi, rhs, crhs, cphi, sz, t);
 }
 
 // S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise
@@ -590,6 +640,7 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
 
 // ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one cell per thread, blockIdx.y =
 // colour (like two colour half-sweeps in one launch: 13 loads and a division per thread at full occupancy)
+template <bool CW>
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
                                      unsigned long long* out, int reverse)
 {
@@ -606,7 +657,7 @@ __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi
         if (2 * m + par < G.nx) {
             long long c, xm;
             pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
-            mx = fabs(residual_at(L, phi, rhs, c, xm));
+            mx = fabs(residual_at<CW>(L, phi, rhs, c, xm, 2 * m + par, j, k));
             if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
         }
     }

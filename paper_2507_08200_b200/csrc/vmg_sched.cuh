@@ -20,8 +20,12 @@ inline LevelView view(const VmgLevel& L)
     LevelView v;
     v.wx = L.wx; v.wy = L.wy; v.wz = L.wz; v.dinv = L.dinv;
     v.G = L.G;
+    v.cx = L.cx; v.cy = L.cy; v.cz = L.cz; v.cw = L.cw;
     return v;
 }
+
+// picks the instantiation for the level's kind of weights (LevelView::cw)
+#define VMG_BY_WEIGHTS(L, KERNEL) ((L).cw ? KERNEL<true> : KERNEL<false>)
 
 inline unsigned grid_for(long long n) { return (unsigned)cdiv(n, kThreads); }
 
@@ -122,7 +126,7 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
         for (int c2 = 0; c2 < 2; ++c2) {
             const int colour = (first + c2) & 1;
             if (2 * s + c2 < skip_first) continue;
-            launch_pdl(h, smooth_colour_kernel, grid_for(nt), kThreads, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
+            launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_kernel), grid_for(nt), kThreads, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
             ++*count;
         }
 }
@@ -132,7 +136,7 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
     VmgLevel& L = h->lev[l];
     VmgLevel& C = h->lev[l + 1];
     C.cur = 0;
-    launch_pdl(h, residual_restrict_kernel, grid_for(C.n), kThreads, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
+    launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_kernel), grid_for(C.n), kThreads, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
                h->three_d ? 2 : 1, next_dir(h, L));
     ++*count;
 }
@@ -164,7 +168,7 @@ inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_on
     VmgLevel& L = h->lev[0];
     unsigned g = grid_for((long long)L.G.ne * L.ny * L.nz);   // one cell per thread, blockIdx.y = colour
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    launch_pdl(h, residual_norm_kernel, dim3(g, red_only ? 1 : 2), kThreads, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
+    launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), dim3(g, red_only ? 1 : 2), kThreads, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -395,7 +399,7 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         VmgLevel& L = h->lev[l];
         long long nt = (long long)L.G.ne * L.ny * L.nz;
-        launch_pdl(h, smooth_colour_prolong_kernel, grid_for(nt), kThreads, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
+        launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_prolong_kernel), grid_for(nt), kThreads, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
                    cur_phi(h->lev[l + 1]), h->symmetric, h->three_d ? 2 : 1, next_dir(h, L));
         ++*count;
         plain_smooth(h, l, h->nu2, count, 1, h->symmetric);
@@ -449,22 +453,24 @@ inline int run_vcycle_with_norm(vmg_s* h, unsigned long long* out)
         if (cudaGetLastError() != cudaSuccess) return VMG_ERR_CUDA;
         return VMG_OK;
     }
-    if (!h->graph_valid) {
-        if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
-        if (h->graph) { cudaGraphDestroy(h->graph); h->graph = nullptr; }
+    const int gi = h->lev[0].cw ? 1 : 0;
+    if (h->graph_slot_epoch[gi] != h->graph_epoch) {
+        if (h->graph_exec[gi]) { cudaGraphExecDestroy(h->graph_exec[gi]); h->graph_exec[gi] = nullptr; }
+        if (h->graph[gi]) { cudaGraphDestroy(h->graph[gi]); h->graph[gi] = nullptr; }
         long long count = 0;
         if (cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
             h->last_cuda_error = (int)cudaGetLastError();
             return VMG_ERR_CUDA;
         }
         body(&count);
-        cudaError_t e = cudaStreamEndCapture(h->stream, &h->graph);
-        if (e == cudaSuccess) e = cudaGraphInstantiate(&h->graph_exec, h->graph, 0);
+        cudaError_t e = cudaStreamEndCapture(h->stream, &h->graph[gi]);
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&h->graph_exec[gi], h->graph[gi], 0);
         if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
-        h->launches_per_cycle = count;
-        h->graph_valid = true;
+        h->graph_slot_launches[gi] = count;
+        h->graph_slot_epoch[gi] = h->graph_epoch;
     }
-    cudaError_t e = cudaGraphLaunch(h->graph_exec, h->stream);
+    h->launches_per_cycle = h->graph_slot_launches[gi];
+    cudaError_t e = cudaGraphLaunch(h->graph_exec[gi], h->stream);
     if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
     h->launches += h->launches_per_cycle;
     return VMG_OK;

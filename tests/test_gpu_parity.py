@@ -656,3 +656,74 @@ def test_masked_full_size_parity():
     assert rel(phi.cpu().numpy(), phi_o) <= PHI_TOL
     s.destroy()
     o.close()
+
+
+@pytest.mark.parametrize("make", [lambda: inputs.config3(32), lambda: inputs.config1(64),
+                                  lambda: inputs.random_problem(40, 24, 16, seed=8, bc_type=[N, D, D, N, N, D], inhomogeneous=True),
+                                  lambda: inputs.random_problem(36, 20, 12, seed=9, bc_type=[D, D, N, N, N, N], spacing=(1.0, 1.2, 0.9)),
+                                  lambda: inputs.config3(128)],
+                         ids=["config3_64x32x32", "config1_2d", "helmholtz_40x24x16", "unequal_h_odd_coarse", "config3_full"])
+@pytest.mark.parametrize("opts", [dict(), dict(prolong=1, symmetric=1)], ids=["default", "trilinear_symmetric"])
+def test_constant_weight_kernels_equal_the_general_ones_bitwise(make, opts):
+    """b == NULL (b = 1: the Poisson equation PAPER.md:54 Eq. 3, Helmholtz with a variable a) selects kernels that form the six
+    face weights from beta/h^2 and the cell's position instead of loading them.  Same numbers, same order: phi and the residual
+    history equal, bit for bit, those of the general kernels on explicit arrays of ones and those of the general kernels
+    with b == NULL (option const_weights=0); PCG likewise."""
+    b = _binding()
+    p = make()
+    d = b.upload(p)
+    nz1 = p.nz + 1 if p.nz > 1 else 1
+    ones = [torch.ones(sh, dtype=torch.float64, device="cuda") for sh in ((p.nz, p.ny, p.nx + 1), (p.nz, p.ny + 1, p.nx), (nz1, p.ny, p.nx))]
+    out = []
+    for variant in ("const", "ones", "null_general"):
+        s = b.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz)
+        for k, v in opts.items():
+            s.set_option(k, v)
+        if variant == "null_general":
+            s.set_option("const_weights", 0)
+        if variant == "ones":
+            s.set_coeffs(d["a"], ones[0], ones[1], ones[2] if p.nz > 1 else None, p.alpha, p.beta)
+        else:
+            s.set_coeffs(d["a"], None, None, None, p.alpha, p.beta)
+        s.set_bc(p.bc_type, d["bc_value"])
+        phi = torch.zeros_like(d["rhs"])
+        st = s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=12)
+        info = s.get_info()
+        phi2 = torch.zeros_like(d["rhs"])
+        st2 = s.solve_pcg(d["rhs"], phi2, rtol=1e-12, max_iter=12)
+        out.append((st, info, phi, st2, s.get_info(), phi2))
+        s.destroy()
+    for o in out[1:]:
+        assert o[0] == out[0][0] and o[1] == out[0][1] and torch.equal(o[2], out[0][2])
+        assert o[3] == out[0][3] and o[4] == out[0][4] and torch.equal(o[5], out[0][5])
+
+
+def test_alternating_equation_kinds_on_one_handle_keeps_results():
+    """One handle used like a time step does (bench.py timestep_leg): constant-weight and general equations in turn, a changed
+    beta on the constant-weight one (its kernels take beta/h^2 by value and the V-cycle is a replayed graph).  Every solve
+    must equal the solve of a fresh handle bit for bit."""
+    b = _binding()
+    p = inputs.random_problem(40, 24, 16, seed=14, bc_type=[D, N, N, D, N, N])
+    d = b.upload(p)
+    kinds = [("const", 1.0), ("general", 1.0), ("const", 1.0), ("const", 2.5), ("general", 0.5), ("const", 2.5), ("const", 1.0)]
+
+    def run(s, kind, beta, pcg):
+        if kind == "const":
+            s.set_coeffs(d["a"], None, None, None, p.alpha, beta)
+        else:
+            s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, beta)
+        phi = torch.zeros_like(d["rhs"])
+        (s.solve_pcg if pcg else s.solve)(d["rhs"], phi, 1e-12, 12)
+        return phi, s.get_info()
+
+    s = b.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz)
+    s.set_bc(p.bc_type, d["bc_value"])
+    for pcg in (False, True):
+        for kind, beta in kinds:
+            got = run(s, kind, beta, pcg)
+            f = b.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz)
+            f.set_bc(p.bc_type, d["bc_value"])
+            want = run(f, kind, beta, pcg)
+            f.destroy()
+            assert got[1] == want[1] and torch.equal(got[0], want[0]), (kind, beta, pcg)
+    s.destroy()
