@@ -366,11 +366,9 @@ __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, i
 // phi written here; rhs, 1/D and the neighbours' phi are dead after this read, so they are loaded with the streaming
 // (evict-first) policy and do not push the weights out of the 126 MB L2.
 template <bool CW>
-__device__ __forceinline__ void relax_one(const LevelView& L, double* phi, const double* rhs, int colour, long long t)
+__device__ __forceinline__ void relax_at(const LevelView& L, double* phi, const double* rhs, int colour, int m, int j, int k)
 {
     const Geom& G = L.G;
-    int m, j, k;
-    unflatten_pair(G, t, m, j, k);
     int par = (colour + j + k) & 1;
     if (2 * m + par >= G.nx) return;
     long long c, xm;
@@ -393,10 +391,10 @@ template <bool CW>
 __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour, int reverse)
 {
     grid_dependency_wait();
-    const long long nt = (long long)L.G.ne * L.G.ny * L.G.nz;
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
-    if (t < nt) relax_one<CW>(L, phi, rhs, colour, t);
+    // grid (x-pair blocks, row blocks, planes), block (x-pairs, rows): no division to find the cell (pair_launch_dims)
+    int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    if (reverse) { k = L.G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
+    if (m < L.G.ne && j < L.G.ny) relax_at<CW>(L, phi, rhs, colour, m, j, k);
 }
 
 // S4 + S2 fused (per-colour path).  The first colour half-sweep after a coarse-grid correction: a relaxation never
@@ -408,11 +406,9 @@ __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, cons
 template <bool CW>
 __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom& CG, double* phi,
                                                   const double* rhs, const double* e, int colour, int sz,
-                                                  long long t)
+                                                  int m, int j, int k)
 {
     const Geom& G = L.G;
-    int m, j, k;
-    unflatten_pair(G, t, m, j, k);
     int par = (colour + j + k) & 1;
     int i = 2 * m + par;
     if (i >= G.nx) return;
@@ -456,9 +452,9 @@ __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __res
                                              const double* __restrict__ e, int colour, int sz, int reverse)
 {
     grid_dependency_wait();
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
-    if (t < (long long)L.G.ne * L.G.ny * L.G.nz) relax_prolong_one<CW>(L, CG, phi, rhs, e, colour, sz, t);
+    int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;   // pair_launch_dims
+    if (reverse) { k = L.G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
+    if (m < L.G.ne && j < L.G.ny) relax_prolong_one<CW>(L, CG, phi, rhs, e, colour, sz, m, j, k);
 }
 
 // r = rhs - A phi, A phi = D phi - sum w phi_nb, D = 1/dinv.
@@ -503,10 +499,8 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 template <bool CW>
 __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG, const double* phi,
                                              const double* rhs, double* crhs, double* cphi,
-                                             int sz, long long t)
+                                             int sz, int I, int J, int K)
 {
-    int I, J, K;
-    unflatten(CG, t, I, J, K);
     double s = 0.0;
     for (int r = 0; r < sz; ++r)
         for (int q = 0; q < 2; ++q) {   // the x-pair first, then accumulated (the blocked kernel sums in this order too)
@@ -526,9 +520,10 @@ __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __r
                                          double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
 {
     grid_dependency_wait();
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
-    if (t < CG.n) restrict_one<CW>(L, CG, phi, rhs, crhs, cphi, sz, t);
+    // grid (coarse x blocks, coarse row blocks, coarse planes), block (coarse x, coarse rows): cell_launch_dims of the coarse level
+    int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
+    if (reverse) { K = CG.nz - 1 - K; J = gridDim.y * blockDim.y - 1 - J; }
+    if (I < CG.nx && J < CG.ny) restrict_one<CW>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K);
 }
 
 // S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise
@@ -610,11 +605,12 @@ __device__ __forceinline__ void block_max_to_global(double v, unsigned long long
         b = other > b ? other : b;
     }
     __shared__ unsigned long long warp_max[32];
-    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int tid = threadIdx.x + blockDim.x * threadIdx.y;   // blocks are (x, rows) with x a multiple of the warp, or 1-D
+    int lane = tid & 31, w = tid >> 5;
     if (lane == 0) warp_max[w] = b;
     __syncthreads();
     if (w == 0) {
-        int nw = (blockDim.x + 31) >> 5;
+        int nw = (blockDim.x * blockDim.y + 31) >> 5;
         b = lane < nw ? warp_max[lane] : 0ull;
         for (int o = 16; o > 0; o >>= 1) {
             unsigned long long other = __shfl_xor_sync(0xffffffffu, b, o);
@@ -638,22 +634,22 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
     block_max_to_global(m, out);
 }
 
-// ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one cell per thread, blockIdx.y =
-// colour (like two colour half-sweeps in one launch: 13 loads and a division per thread at full occupancy)
+// ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one cell per thread, both colours or red only
+// (as (like two colour half-sweeps in one launch: 13 loads and a division per thread at full occupancy)
 template <bool CW>
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
                                      unsigned long long* out, int reverse)
 {
     grid_dependency_wait();
     const Geom& G = L.G;
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (reverse) t = (long long)gridDim.x * blockDim.x - 1 - t;
-    long long nt = (long long)G.ne * G.ny * G.nz;
+    // grid (x-pair blocks, row blocks, planes * colours), block (x-pairs, rows): pair_launch_dims, z extended by the colour
+    int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+    int k = (int)blockIdx.z % G.nz;
+    const int colour = (int)blockIdx.z / G.nz;
+    if (reverse) { k = G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
     double mx = 0.0;
-    if (t < nt) {
-        int m, j, k;
-    unflatten_pair(G, t, m, j, k);
-        int par = ((int)blockIdx.y + j + k) & 1;
+    if (m < G.ne && j < G.ny) {
+        int par = (colour + j + k) & 1;
         if (2 * m + par < G.nx) {
             long long c, xm;
             pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);

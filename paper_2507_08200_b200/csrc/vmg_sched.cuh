@@ -29,6 +29,22 @@ inline LevelView view(const VmgLevel& L)
 
 inline unsigned grid_for(long long n) { return (unsigned)cdiv(n, kThreads); }
 
+// launch shape of the kernels that take one x-pair slot per thread: block (x-pairs, rows) of kThreads threads with as many
+// x-pairs as the row has (whole warps, at most 128), grid (x-pair blocks, row blocks, planes)
+inline void cell_launch_dims(const Geom& G, dim3& grid, dim3& block)
+{
+    const int bx = std::min(128, 32 * ((G.nx + 31) / 32)), by = kThreads / bx;
+    block = dim3(bx, by, 1);
+    grid = dim3((G.nx + bx - 1) / bx, (G.ny + by - 1) / by, G.nz);
+}
+
+inline void pair_launch_dims(const VmgLevel& L, dim3& grid, dim3& block)
+{
+    const int bx = std::min(128, 32 * ((L.G.ne + 31) / 32)), by = kThreads / bx;
+    block = dim3(bx, by, 1);
+    grid = dim3((L.G.ne + bx - 1) / bx, (L.ny + by - 1) / by, L.nz);
+}
+
 // direction of the next whole-level kernel: consecutive kernels walk the level in opposite directions (L2 reuse)
 inline int next_dir(vmg_s* h, VmgLevel& L) { int d = h->snake ? L.dir : 0; L.dir ^= 1; return d; }
 
@@ -126,7 +142,9 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
         for (int c2 = 0; c2 < 2; ++c2) {
             const int colour = (first + c2) & 1;
             if (2 * s + c2 < skip_first) continue;
-            launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_kernel), grid_for(nt), kThreads, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
+            dim3 grid, block;
+            pair_launch_dims(L, grid, block);
+            launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_kernel), grid, block, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
             ++*count;
         }
 }
@@ -136,7 +154,9 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
     VmgLevel& L = h->lev[l];
     VmgLevel& C = h->lev[l + 1];
     C.cur = 0;
-    launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_kernel), grid_for(C.n), kThreads, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
+    dim3 grid, block;
+    cell_launch_dims(C.G, grid, block);
+    launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_kernel), grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
                h->three_d ? 2 : 1, next_dir(h, L));
     ++*count;
 }
@@ -166,9 +186,11 @@ inline void plain_prolong_correct(vmg_s* h, int l, long long* count)
 inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_only = false)
 {
     VmgLevel& L = h->lev[0];
-    unsigned g = grid_for((long long)L.G.ne * L.ny * L.nz);   // one cell per thread, blockIdx.y = colour
+    dim3 grid, block;
+    pair_launch_dims(L, grid, block);
+    if (!red_only) grid.z *= 2;                               // one cell per thread: the planes once per colour
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), dim3(g, red_only ? 1 : 2), kThreads, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
+    launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -399,7 +421,9 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         VmgLevel& L = h->lev[l];
         long long nt = (long long)L.G.ne * L.ny * L.nz;
-        launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_prolong_kernel), grid_for(nt), kThreads, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
+        dim3 grid, block;
+        pair_launch_dims(L, grid, block);
+        launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_prolong_kernel), grid, block, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
                    cur_phi(h->lev[l + 1]), h->symmetric, h->three_d ? 2 : 1, next_dir(h, L));
         ++*count;
         plain_smooth(h, l, h->nu2, count, 1, h->symmetric);
