@@ -44,7 +44,7 @@ enum {
     VMG_MAXCYCLES = 1,       /* ran max_vcycles cycles without reaching rtol (always, when rtol <= 0)   */
     VMG_STALLED = 2,         /* residual reduced by less than 10 % in 3 consecutive cycles (fp64 floor) */
     VMG_ERR_ARG = -1,        /* NULL / out-of-range argument, unknown option key                        */
-    VMG_ERR_SIZE = -2,       /* grid cannot be coarsened to a bottom grid of <= 512 cells, or >= 2^31 cells */
+    VMG_ERR_SIZE = -2,       /* grid cannot be coarsened to a bottom grid of <= 512 cells, >= 2^31 cells, ny > 65535 or nz > 32767 */
     VMG_ERR_STATE = -3,      /* vmg_solve before both vmg_set_coeffs and vmg_set_bc                     */
     VMG_ERR_SINGULAR = -4,   /* all active faces Neumann and (a == NULL or alpha == 0)                  */
     VMG_ERR_DIVERGED = -5,   /* residual became NaN or Inf                                              */

@@ -163,6 +163,7 @@ int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, do
     bool three_d = nz > 1;
     if (nx < 2 || ny < 2 || nz < 1 || !(dx > 0) || !(dy > 0) || (three_d && !(dz > 0))) return VMG_ERR_SIZE;
     if ((long long)nx * ny * nz >= (1LL << 31)) return VMG_ERR_SIZE;   // kernels decompose cell numbers in 32 bits
+    if (nz > 32767 || ny > 65535) return VMG_ERR_SIZE;                 // rows and planes are grid dimensions y and z (pair_launch_dims)
     int n[3] = {nx, ny, nz}, nlev = 1;
     for (;;) {   // R11: halve while every active dimension is even and stays >= 2
         bool ok = n[0] % 2 == 0 && n[0] / 2 >= 2 && n[1] % 2 == 0 && n[1] / 2 >= 2;
