@@ -360,8 +360,7 @@ __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, i
 }
 
 // S2 (per-colour path). One colour half-sweep: phi_c <- (rhs_c + sum w phi_nb) / D_c for (i+j+k)%2 == colour.
-// t: index of the x-pair (m, j, k), t < ne*ny*nz.  The *_one functions take plain pointers: the cluster tail calls
-// them on arrays that other CTAs of the same launch have just written (no non-coherent loads there).
+// (m, j, k): the x-pair slot; the kernel derives it from a 3-D grid (pair_launch_dims in vmg_sched.cuh).
 // L2 residency: what the NEXT half-sweep (other colour, opposite direction) needs again are the face weights and the
 // phi written here; rhs, 1/D and the neighbours' phi are dead after this read, so they are loaded with the streaming
 // (evict-first) policy and do not push the weights out of the 126 MB L2.
