@@ -279,13 +279,13 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
     for (int l = 0; l < h->nlev; ++l) {
         VmgLevel& L = h->lev[l];
         if (l > 0) {   // S0: average the previous level's raw coefficients
-            coarsen_a_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(fa, L.a, L.nx, L.ny, L.nz, sz);
-            coarsen_b_kernel<<<grid_for((long long)face_count(L, 0)), kThreads, 0, h->stream>>>(fbx, L.bx, L.nx, L.ny, L.nz, sz, 0);
-            coarsen_b_kernel<<<grid_for((long long)face_count(L, 1)), kThreads, 0, h->stream>>>(fby, L.by, L.nx, L.ny, L.nz, sz, 1);
+            launch_pdl(h, coarsen_a_kernel, grid_for(L.n), kThreads, 0, fa, L.a, L.nx, L.ny, L.nz, sz);
+            launch_pdl(h, coarsen_b_kernel, grid_for((long long)face_count(L, 0)), kThreads, 0, fbx, L.bx, L.nx, L.ny, L.nz, sz, 0);
+            launch_pdl(h, coarsen_b_kernel, grid_for((long long)face_count(L, 1)), kThreads, 0, fby, L.by, L.nx, L.ny, L.nz, sz, 1);
             if (h->three_d)
-                coarsen_b_kernel<<<grid_for((long long)face_count(L, 2)), kThreads, 0, h->stream>>>(fbz, L.bz, L.nx, L.ny, L.nz, sz, 2);
+                launch_pdl(h, coarsen_b_kernel, grid_for((long long)face_count(L, 2)), kThreads, 0, fbz, L.bz, L.nx, L.ny, L.nz, sz, 2);
             if (fad) {   // the extra diagonal is averaged like a
-                coarsen_a_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(fad, L.adiag, L.nx, L.ny, L.nz, sz);
+                launch_pdl(h, coarsen_a_kernel, grid_for(L.n), kThreads, 0, fad, L.adiag, L.nx, L.ny, L.nz, sz);
                 fad = L.adiag;
                 ++setup_launches;
             }
@@ -297,12 +297,14 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
         g.adiag = fad;
         g.bx = fbx; g.by = fby; g.bz = fbz;
         g.wx = L.wx; g.wy = L.wy; g.wz = L.wz; g.dbase = L.dbase;
+        g.dinv = L.dinv; g.write_dinv = h->have_bc ? 1 : 0;   // boundary types known: 1/D in the same pass
+        for (int f = 0; f < 6; ++f) g.dirichlet[f] = h->bctype[f] == VMG_BC_DIRICHLET;
         for (int f = 0; f < 6; ++f) g.wb[f] = L.wb[f];
         g.G = L.G; g.three_d = h->three_d;
         g.alpha = h->alpha; g.cx = beta / (L.hx * L.hx); g.cy = beta / (L.hy * L.hy);
         g.cz = h->three_d ? beta / (L.hz * L.hz) : 0.0;
         L.cx = g.cx; L.cy = g.cy; L.cz = g.cz; L.cw = cw;
-        build_stencil_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(g);
+        launch_pdl(h, build_stencil_kernel, grid_for(L.n), kThreads, 0, g);
         ++setup_launches;
     }
     delete ps;
@@ -311,7 +313,7 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
     h->total_launches += setup_launches;
     if (h->profile) prof_collect(h);
     h->have_coeffs = true;
-    h->dinv_dirty = true;
+    h->dinv_dirty = !h->have_bc;
     return VMG_OK;
 }
 
@@ -320,8 +322,9 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
     if (!h || !type) return VMG_ERR_ARG;
     for (int f = 0; f < 6; ++f)
         if (type[f] != VMG_BC_DIRICHLET && type[f] != VMG_BC_NEUMANN) return VMG_ERR_ARG;
+    if (!h->have_bc) h->dinv_dirty = true;
     for (int f = 0; f < 6; ++f) {
-        if (h->bctype[f] != type[f]) { ++h->graph_epoch; }   // the trilinear prolongation kernels carry the types by value
+        if (h->bctype[f] != type[f]) { ++h->graph_epoch; h->dinv_dirty = true; }   // the trilinear prolongation kernels carry the types by value; 1/D depends on them
         h->bctype[f] = type[f];
         bool active = f < 4 || h->three_d;
         h->bc_has_value[f] = active && value && value[f];
@@ -331,7 +334,6 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
     }
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     h->have_bc = true;
-    h->dinv_dirty = true;
     return VMG_OK;
 }
 

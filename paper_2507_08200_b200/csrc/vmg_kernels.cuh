@@ -72,6 +72,7 @@ __device__ __forceinline__ void unflatten_pair(const Geom& G, long long t, int& 
 __global__ void coarsen_a_kernel(const double* __restrict__ fa, double* __restrict__ ca,
                                  int cnx, int cny, int cnz, int sz)
 {
+    grid_dependency_wait();   // vmg_set_coeffs launches its kernels with programmatic serialisation
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     long long n = (long long)cnx * cny * cnz;
     if (t >= n) return;
@@ -90,6 +91,7 @@ __global__ void coarsen_a_kernel(const double* __restrict__ fa, double* __restri
 __global__ void coarsen_b_kernel(const double* __restrict__ fb, double* __restrict__ cb,
                                  int cnx, int cny, int cnz, int sz, int dir)
 {
+    grid_dependency_wait();
     int ex = cnx + (dir == 0), ey = cny + (dir == 1), ez = cnz + (dir == 2);
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     long long n = (long long)ex * ey * ez;
@@ -122,6 +124,8 @@ struct StencilBuildArgs {
     const double *a, *bx, *by, *bz;      // raw, public layout (may be NULL)
     const double* adiag;                 // masking: extra diagonal of this level, public layout (NULL without a mask)
     double *wx, *wy, *wz, *dbase;        // internal cell arrays
+    double* dinv;                        // written as well when the boundary types are known (write_dinv): the same
+    int write_dinv, dirichlet[6];        // expression, in the same order, as finalize_dinv_kernel
     double* wb[6];                       // boundary planes (natural plane layout)
     Geom G;
     int three_d;
@@ -130,6 +134,7 @@ struct StencilBuildArgs {
 
 __global__ void build_stencil_kernel(StencilBuildArgs g)
 {
+    grid_dependency_wait();   // vmg_set_coeffs launches its kernels with programmatic serialisation
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (t >= g.G.n) return;
     const int nx = g.G.nx, ny = g.G.ny, nz = g.G.nz;
@@ -146,13 +151,14 @@ __global__ void build_stencil_kernel(StencilBuildArgs g)
         double bzh = g.bz ? g.bz[t + nxy] : 1.0;
         wzl = g.cz * bzl; wzh = g.cz * bzh;
     }
-    if (i == 0)      { g.wb[0][j + (long long)ny * k] = wxl; wxl = 0.0; }
-    if (i == nx - 1) { g.wb[1][j + (long long)ny * k] = wxh; wxh = 0.0; }
-    if (j == 0)      { g.wb[2][i + (long long)nx * k] = wyl; wyl = 0.0; }
-    if (j == ny - 1) { g.wb[3][i + (long long)nx * k] = wyh; wyh = 0.0; }
+    double bw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // this cell's boundary-face weights
+    if (i == 0)      { g.wb[0][j + (long long)ny * k] = bw[0] = wxl; wxl = 0.0; }
+    if (i == nx - 1) { g.wb[1][j + (long long)ny * k] = bw[1] = wxh; wxh = 0.0; }
+    if (j == 0)      { g.wb[2][i + (long long)nx * k] = bw[2] = wyl; wyl = 0.0; }
+    if (j == ny - 1) { g.wb[3][i + (long long)nx * k] = bw[3] = wyh; wyh = 0.0; }
     if (g.three_d) {
-        if (k == 0)      { g.wb[4][i + (long long)nx * j] = wzl; wzl = 0.0; }
-        if (k == nz - 1) { g.wb[5][i + (long long)nx * j] = wzh; wzh = 0.0; }
+        if (k == 0)      { g.wb[4][i + (long long)nx * j] = bw[4] = wzl; wzl = 0.0; }
+        if (k == nz - 1) { g.wb[5][i + (long long)nx * j] = bw[5] = wzh; wzh = 0.0; }
     }
     const long long c = cell_at(g.G, i, j, k);
     g.wx[c] = wxl; g.wy[c] = wyl; g.wz[c] = wzl;
@@ -160,6 +166,17 @@ __global__ void build_stencil_kernel(StencilBuildArgs g)
     if (g.adiag) d += g.adiag[t];
     d += wxl; d += wxh; d += wyl; d += wyh; d += wzl; d += wzh;
     g.dbase[c] = d;
+    if (g.write_dinv) {
+        if (i == 0 && g.dirichlet[0])      d += 2.0 * bw[0];
+        if (i == nx - 1 && g.dirichlet[1]) d += 2.0 * bw[1];
+        if (j == 0 && g.dirichlet[2])      d += 2.0 * bw[2];
+        if (j == ny - 1 && g.dirichlet[3]) d += 2.0 * bw[3];
+        if (g.three_d) {
+            if (k == 0 && g.dirichlet[4])      d += 2.0 * bw[4];
+            if (k == nz - 1 && g.dirichlet[5]) d += 2.0 * bw[5];
+        }
+        g.dinv[c] = 1.0 / d;
+    }
 }
 
 struct DinvArgs {
