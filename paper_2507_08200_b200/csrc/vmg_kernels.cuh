@@ -479,21 +479,24 @@ __device__ __forceinline__ double residual_at(const LevelView& L, const double* 
     return rhs[c] + nb_sum(L, phi, c, xm) - phi[c] / L.dinv[c];
 }
 
-// the same with the cell's position known (CW = true: constant face weights, see LevelView)
-template <bool CW>
+// the same with the cell's position known (CW = true: constant face weights, see LevelView).  STREAM: phi, rhs and 1/D
+// are read with the streaming (evict-first) policy, as in relax_at -- for the norm at the end of a cycle, after which
+// the next kernel needs the face weights again and nothing else that is read here.
+template <bool CW, bool STREAM = false>
 __device__ __forceinline__ double residual_at(const LevelView& L, const double* phi, const double* rhs, long long c, long long xm,
                                               int i, int j, int k)
 {
-    if (!CW) return residual_at(L, phi, rhs, c, xm);
+    if (!CW && !STREAM) return residual_at(L, phi, rhs, c, xm);
+    auto ld = [](const double* p) { return STREAM ? __ldcs(p) : *p; };
     double w[6];
-    face_weights<true>(L, c, xm, i, j, k, w);
-    double s = w[0] * phi[xm];
-    s = fma(w[1], phi[xm + 1], s);
-    s = fma(w[2], phi[c - L.G.pitch], s);
-    s = fma(w[3], phi[c + L.G.pitch], s);
-    s = fma(w[4], phi[c - L.G.plane], s);
-    s = fma(w[5], phi[c + L.G.plane], s);
-    return rhs[c] + s - phi[c] / L.dinv[c];
+    face_weights<CW>(L, c, xm, i, j, k, w);
+    double s = w[0] * ld(phi + xm);
+    s = fma(w[1], ld(phi + xm + 1), s);
+    s = fma(w[2], ld(phi + c - L.G.pitch), s);
+    s = fma(w[3], ld(phi + c + L.G.pitch), s);
+    s = fma(w[4], ld(phi + c - L.G.plane), s);
+    s = fma(w[5], ld(phi + c + L.G.plane), s);
+    return ld(rhs + c) + s - ld(phi + c) / ld(L.dinv + c);
 }
 
 // r in the public layout (single-step entry point)
@@ -669,7 +672,7 @@ __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi
         if (2 * m + par < G.nx) {
             long long c, xm;
             pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
-            mx = fabs(residual_at<CW>(L, phi, rhs, c, xm, 2 * m + par, j, k));
+            mx = fabs(residual_at<CW, !CW>(L, phi, rhs, c, xm, 2 * m + par, j, k));   // constant weights: the level fits L2, keep it there
             if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
         }
     }
