@@ -137,7 +137,6 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
 {
     VmgLevel& L = h->lev[l];
     LevelView v = view(L);
-    long long nt = (long long)L.G.ne * L.ny * L.nz;
     for (int s = 0; s < nsweeps; ++s)
         for (int c2 = 0; c2 < 2; ++c2) {
             const int colour = (first + c2) & 1;
@@ -420,7 +419,6 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
     if (h->nu2 >= 1 && !h->prolong) {   // the correction rides on the first half-sweep (smooth_colour_prolong_kernel)
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         VmgLevel& L = h->lev[l];
-        long long nt = (long long)L.G.ne * L.ny * L.nz;
         dim3 grid, block;
         pair_launch_dims(L, grid, block);
         launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_prolong_kernel), grid, block, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
