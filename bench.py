@@ -231,9 +231,56 @@ def timestep_leg(binding, torch, p, d, d_bc, dev, s, flush, nsteps: int = 3, rto
             times.append(e0.elapsed_time(e1))
             cycles.append(ncyc)
     ms = float(np.mean(times))
-    return {"ms_per_time_step": ms, "time_steps_per_s": 1e3 / ms, "solves_per_time_step": len(eqs),
-            "vcycles_per_time_step": float(np.mean(cycles)), "rtol": rtol,
-            "sequence": "Poisson + 15 species + energy + 3 photoionisation; set_coeffs + set_bc + warm-started solve each; one handle"}
+    out = {"ms_per_time_step": ms, "time_steps_per_s": 1e3 / ms, "solves_per_time_step": len(eqs),
+           "vcycles_per_time_step": float(np.mean(cycles)), "rtol": rtol,
+           "sequence": "Poisson + 15 species + energy + 3 photoionisation; set_coeffs + set_bc + warm-started solve each; one handle"}
+
+    # The same time step with the 16 transport solves (15 species + energy: independent of each other once the potential is
+    # known) advanced together by vmg_solve_batch, one handle and one stream each (SURVEY.md 8(f) N1 inside N3: the
+    # paper's "multi-component MG solves"); Poisson before them and the photoionisation solves after,
+    # on the first handle as above.
+    nb = 16
+    streams = [torch.cuda.Stream() for _ in range(nb)]
+    hs = [binding.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, stream=st) for st in streams]
+    for hb in hs:
+        hb.set_bc(p4.bc_type, None)
+    tb = list(betas) + [1.0]
+    bfields = [torch.zeros_like(d["rhs"]) for _ in range(nb)]
+    for f in fields:
+        f.zero_()
+    times_b, cycles_b = [], []
+    for step in range(nsteps + 1):
+        scale = 1.0 + 0.01 * step
+        flush.fill_(1.0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ncyc = 0
+        name, setup, rhs = eqs[0]
+        setup()
+        assert s.solve(rhs * scale, fields[0], rtol=rtol, max_vcycles=50) in (0, 2)
+        ncyc += s.get_info()[0]
+        torch.cuda.synchronize()
+        for hb, b_k in zip(hs, tb):
+            hb.set_coeffs(d4["a"], d4["bx"], d4["by"], d4["bz"], 1.0, float(b_k))
+        rb = d4["rhs"] * scale
+        torch.cuda.synchronize()
+        sts = binding.solve_batch(hs, [rb] * nb, bfields, rtol=rtol, max_vcycles=50)
+        assert all(v in (0, 2) for v in sts), sts
+        ncyc += sum(hb.get_info()[0] for hb in hs)
+        for (name, setup, rhs), phi in zip(eqs[17:], fields[17:]):
+            setup()
+            assert s.solve(rhs * scale, phi, rtol=rtol, max_vcycles=50) in (0, 2)
+            ncyc += s.get_info()[0]
+        torch.cuda.synchronize()
+        if step > 0:
+            times_b.append((time.perf_counter() - t0) * 1e3)
+            cycles_b.append(ncyc)
+    for hb in hs:
+        hb.destroy()
+    out["batched_transport"] = {"ms_per_time_step": float(np.mean(times_b)), "time_steps_per_s": 1e3 / float(np.mean(times_b)),
+                                "vcycles_per_time_step": float(np.mean(cycles_b)), "handles": nb,
+                                "timing": "host clock, device synchronised on both sides"}
+    return out
 
 
 # ----------------------------------------------------------------------------------------------------
