@@ -232,7 +232,12 @@ int vmg_destroy(vmg_handle h)
     for (int i = 0; i < 2; ++i) {
         if (h->graph_exec[i]) cudaGraphExecDestroy(h->graph_exec[i]);
         if (h->graph[i]) cudaGraphDestroy(h->graph[i]);
+        for (int sg = 0; sg < 3; ++sg) {
+            if (h->seg_exec[i][sg]) cudaGraphExecDestroy(h->seg_exec[i][sg]);
+            if (h->seg_graph[i][sg]) cudaGraphDestroy(h->seg_graph[i][sg]);
+        }
     }
+    if (h->token) cudaEventDestroy(h->token);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->arena) cudaFree(h->arena);
     if (h->own_stream) cudaStreamDestroy(h->stream);
@@ -724,6 +729,33 @@ int vmg_solve_batch(int n, const vmg_handle* hs, const double* const* rhs, doubl
     for (int i = 0; i < n; ++i) if (rc[i] == VMG_OK) rc[i] = solve_begin_finish(hs[i]);
     for (;;) {
         bool any = false;
+        // Staggered schedule: the level-0 strokes of the handles follow one another (a token event passed from stream to
+        // stream), so that one handle at a time streams its fine level through the L2 -- keeping the reuse between its
+        // consecutive half-sweeps -- while the latency-bound coarser levels of the others run beside it.
+        int nact = 0;
+        bool seg_ok = true;
+        for (int i = 0; i < n; ++i)
+            if (rc[i] == VMG_OK && hs[i]->sv_active) { ++nact; seg_ok = seg_ok && vcycle_segmentable(hs[i]); }
+        if (nact >= 2 && seg_ok) {
+            cudaEvent_t prev = nullptr;
+            for (int pass = 0; pass < 2; ++pass)
+                for (int i = 0; i < n; ++i) {
+                    vmg_s* h = hs[i];
+                    if (rc[i] != VMG_OK || !h->sv_active) continue;
+                    unsigned long long* scal = (unsigned long long*)h->d_scal;
+                    if (!h->token && cudaEventCreateWithFlags(&h->token, cudaEventDisableTiming) != cudaSuccess) { rc[i] = VMG_ERR_CUDA; continue; }
+                    // capture (first use) before the wait is enqueued: a capturing stream must not hold foreign work
+                    if (pass == 0 && h->seg_epoch[h->lev[0].cw ? 1 : 0] != h->graph_epoch) cudaStreamSynchronize(h->stream);
+                    if (prev) cudaStreamWaitEvent(h->stream, prev, 0);
+                    rc[i] = run_vcycle_segment(h, pass == 0 ? 0 : 2, scal + 1);
+                    if (rc[i] != VMG_OK) continue;
+                    cudaEventRecord(h->token, h->stream);
+                    prev = h->token;
+                    if (pass == 0) rc[i] = run_vcycle_segment(h, 1, scal + 1);
+                    else if (cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) rc[i] = VMG_ERR_CUDA;
+                    any = true;
+                }
+        } else
         for (int i = 0; i < n; ++i)
             if (rc[i] == VMG_OK && hs[i]->sv_active) { rc[i] = solve_cycle_launch(hs[i]); any = true; }
         if (!any) break;

@@ -86,6 +86,13 @@ struct vmg_s {
     cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
     unsigned graph_slot_epoch[2] = {0, 0};
     long long graph_slot_launches[2] = {0, 0};
+    // the same cycle cut in three graphs for the staggered batch schedule (vmg_solve_batch): [cw][segment], segment
+    // 0 = level-0 down-stroke, 1 = all coarser levels, 2 = level-0 up-stroke + residual norm
+    cudaGraph_t seg_graph[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+    cudaGraphExec_t seg_exec[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+    long long seg_launches[2][3] = {{0, 0, 0}, {0, 0, 0}};
+    unsigned seg_epoch[2] = {0, 0};
+    cudaEvent_t token = nullptr;       // "level 0 of the GPU is free again" (staggered batch schedule)
     // state of the solve in progress (vmg_solve / vmg_solve_batch phases)
     double sv_rtol = 0.0, sv_nb = 0.0;
     int sv_max = 0, sv_slow = 0, sv_status = 0;

@@ -462,6 +462,69 @@ inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* co
     settle_phi(h, 0);
 }
 
+// The same cycle in three pieces (staggered batch schedule of vmg_solve_batch): 0 = level-0 down-stroke, 1 = all coarser
+// levels (strokes of levels 1.., tail or bottom solve), 2 = level-0 up-stroke + residual norm.  Enqueued in this order they
+// are enqueue_vcycle, launch for launch.
+inline bool vcycle_segmentable(const vmg_s* h)
+{
+    const int last = h->nlev - 1;
+    const int tail = h->tail_level < 0 ? last : h->cluster_level >= 0 ? h->cluster_level : h->tail_level;
+    return tail >= 1 && h->use_graph && !h->profile;
+}
+
+inline void enqueue_vcycle_segment(vmg_s* h, int seg, unsigned long long* norm_out, long long* count)
+{
+    const int last = h->nlev - 1;
+    const int tail = h->tail_level < 0 ? last : h->cluster_level >= 0 ? h->cluster_level : h->tail_level;
+    if (seg == 0) {
+        cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
+        for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }
+        enqueue_down(h, 0, count);
+    } else if (seg == 1) {
+        for (int l = 1; l < tail; ++l) enqueue_down(h, l, count);
+        if (h->tail_level >= 0) enqueue_tail(h, nullptr, count);
+        else {
+            ProfScope ps(h, VMG_PC_COARSE, count);
+            if (!h->symmetric) plain_smooth(h, last, h->nbottom, count);
+            else { plain_smooth(h, last, h->nbottom / 2, count, 0, 0); plain_smooth(h, last, h->nbottom - h->nbottom / 2, count, 0, 1); }
+        }
+        for (int l = tail - 1; l >= 1; --l) enqueue_up(h, l, nullptr, count);
+    } else {
+        const bool norm_done = enqueue_up(h, 0, norm_out, count);
+        if (!norm_done) { enqueue_residual_norm(h, norm_out, h->nu2 >= 1 && !h->symmetric); ++*count; }
+        settle_phi(h, 0);
+    }
+}
+
+// captures the three segments (once per epoch and kind of weights), then launches segment `seg`
+inline int run_vcycle_segment(vmg_s* h, int seg, unsigned long long* out)
+{
+    const int gi = h->lev[0].cw ? 1 : 0;
+    if (h->seg_epoch[gi] != h->graph_epoch) {
+        prepare_blocked(h);
+        for (int sg = 0; sg < 3; ++sg) {
+            if (h->seg_exec[gi][sg]) { cudaGraphExecDestroy(h->seg_exec[gi][sg]); h->seg_exec[gi][sg] = nullptr; }
+            if (h->seg_graph[gi][sg]) { cudaGraphDestroy(h->seg_graph[gi][sg]); h->seg_graph[gi][sg] = nullptr; }
+            long long count = 0;
+            if (cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+                h->last_cuda_error = (int)cudaGetLastError();
+                return VMG_ERR_CUDA;
+            }
+            enqueue_vcycle_segment(h, sg, out, &count);
+            cudaError_t e = cudaStreamEndCapture(h->stream, &h->seg_graph[gi][sg]);
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&h->seg_exec[gi][sg], h->seg_graph[gi][sg], 0);
+            if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
+            h->seg_launches[gi][sg] = count;
+        }
+        h->seg_epoch[gi] = h->graph_epoch;
+    }
+    cudaError_t e = cudaGraphLaunch(h->seg_exec[gi][seg], h->stream);
+    if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
+    h->launches += h->seg_launches[gi][seg];
+    if (seg == 2) h->launches_per_cycle = h->seg_launches[gi][0] + h->seg_launches[gi][1] + h->seg_launches[gi][2];
+    return VMG_OK;
+}
+
 // V-cycle followed by the residual norm into *out (device), as a graph replay when enabled.
 inline int run_vcycle_with_norm(vmg_s* h, unsigned long long* out)
 {
