@@ -339,6 +339,30 @@ def test_batched_solves_are_bitwise_the_single_solves():
         assert st == ref[0] and cyc == ref[1][0] and list(hist) == list(ref[1][2])
         assert torch.equal(phi, ref[2])
         s.destroy()
+    # the staggered schedule (three graphs per handle, token events) keeps no state between calls: the same handles again,
+    # in another order, one of them switched to constant weights, then alone through vmg_solve
+    solvers, data, streams2 = [], [], [torch.cuda.Stream() for _ in probs]
+    for p, stream in zip(probs, streams2):
+        s, d = b.from_problem(p, stream=stream)
+        solvers.append(s); data.append(d)
+    torch.cuda.synchronize()
+    for rnd in range(3):
+        order = [0, 1, 2, 3] if rnd == 0 else [3, 1, 0, 2] if rnd == 1 else [2, 0]
+        want = list(single)
+        if rnd >= 1:   # problem 0 (b = 1) with b == NULL: bitwise the same solve through the constant-weight kernels
+            solvers[0].set_coeffs(data[0]["a"], None, None, None, probs[0].alpha, probs[0].beta)
+        phis = [torch.zeros_like(data[i]["rhs"]) for i in order]
+        sts = b.solve_batch([solvers[i] for i in order], [data[i]["rhs"] for i in order], phis, rtol=1e-12, max_vcycles=30)
+        for i, st, phi in zip(order, sts, phis):
+            cyc, rr, hist = solvers[i].get_info()
+            assert st == want[i][0] and cyc == want[i][1][0] and list(hist) == list(want[i][1][2]), (rnd, i)
+            assert torch.equal(phi, want[i][2]), (rnd, i)
+    for i, s in enumerate(solvers):
+        phi = torch.zeros_like(data[i]["rhs"])
+        with torch.cuda.stream(streams2[i]):
+            st = s.solve(data[i]["rhs"], phi, rtol=1e-12, max_vcycles=30)
+        assert st == single[i][0] and torch.equal(phi, single[i][2])
+        s.destroy()
     # a handle may appear once; an unready handle reports its own error without stopping the others
     s1, d1 = b.from_problem(probs[0])
     s2 = b.Vmg(16, 8, 8, 1.0, 1.0, 1.0)
