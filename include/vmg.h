@@ -100,7 +100,9 @@ int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max
  * components with each multigrid solve results in more GPU work").  n independent
  * problems, one handle each -- same or different grids, coefficients and boundary conditions -- advanced in
  * lock-step: each round enqueues one V-cycle per unfinished handle on that handle's stream, then synchronises and
- * applies the exit rules of vmg_solve to each.  Create the handles with DISTINCT streams (or cuda_stream = NULL,
+ * applies the exit rules of vmg_solve to each.  With two or more active handles the level-0 strokes of the handles are
+ * run one after the other (token event) and the coarser levels of each handle beside the others' fine levels on a
+ * highest-priority stream of its own: same kernels, same order per handle, bitwise the results of vmg_solve.  Create the handles with DISTINCT streams (or cuda_stream = NULL,
  * which gives each its own): the latency-bound coarse levels of one solve then overlap the bandwidth-bound fine
  * level of another.  handles, rhs, phi: HOST arrays of n entries (rhs[i], phi[i]: DEVICE arrays as in vmg_solve);
  * status: HOST array of n ints or NULL, receives what vmg_solve would have returned for problem i.  Every solve

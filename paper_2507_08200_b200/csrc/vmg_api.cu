@@ -238,6 +238,9 @@ int vmg_destroy(vmg_handle h)
         }
     }
     if (h->token) cudaEventDestroy(h->token);
+    if (h->coarse_go) cudaEventDestroy(h->coarse_go);
+    if (h->coarse_done) cudaEventDestroy(h->coarse_done);
+    if (h->coarse_stream) cudaStreamDestroy(h->coarse_stream);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->arena) cudaFree(h->arena);
     if (h->own_stream) cudaStreamDestroy(h->stream);
@@ -743,7 +746,16 @@ int vmg_solve_batch(int n, const vmg_handle* hs, const double* const* rhs, doubl
                     vmg_s* h = hs[i];
                     if (rc[i] != VMG_OK || !h->sv_active) continue;
                     unsigned long long* scal = (unsigned long long*)h->d_scal;
-                    if (!h->token && cudaEventCreateWithFlags(&h->token, cudaEventDisableTiming) != cudaSuccess) { rc[i] = VMG_ERR_CUDA; continue; }
+                    if (!h->token) {
+                        int lo = 0, hi = 0;
+                        cudaDeviceGetStreamPriorityRange(&lo, &hi);
+                        if (cudaEventCreateWithFlags(&h->token, cudaEventDisableTiming) != cudaSuccess ||
+                            cudaEventCreateWithFlags(&h->coarse_go, cudaEventDisableTiming) != cudaSuccess ||
+                            cudaEventCreateWithFlags(&h->coarse_done, cudaEventDisableTiming) != cudaSuccess ||
+                            cudaStreamCreateWithPriority(&h->coarse_stream, cudaStreamNonBlocking, hi) != cudaSuccess) {
+                            h->last_cuda_error = (int)cudaGetLastError(); rc[i] = VMG_ERR_CUDA; continue;
+                        }
+                    }
                     // capture (first use) before the wait is enqueued: a capturing stream must not hold foreign work
                     if (pass == 0 && h->seg_epoch[h->lev[0].cw ? 1 : 0] != h->graph_epoch) cudaStreamSynchronize(h->stream);
                     if (prev) cudaStreamWaitEvent(h->stream, prev, 0);
@@ -751,7 +763,12 @@ int vmg_solve_batch(int n, const vmg_handle* hs, const double* const* rhs, doubl
                     if (rc[i] != VMG_OK) continue;
                     cudaEventRecord(h->token, h->stream);
                     prev = h->token;
-                    if (pass == 0) rc[i] = run_vcycle_segment(h, 1, scal + 1);
+                    if (pass == 0) {   // the coarser levels on the high-priority stream, between the two level-0 strokes
+                        cudaStreamWaitEvent(h->coarse_stream, h->token, 0);
+                        rc[i] = run_vcycle_segment(h, 1, scal + 1, h->coarse_stream);
+                        cudaEventRecord(h->coarse_done, h->coarse_stream);
+                        cudaStreamWaitEvent(h->stream, h->coarse_done, 0);
+                    }
                     else if (cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) rc[i] = VMG_ERR_CUDA;
                     any = true;
                 }

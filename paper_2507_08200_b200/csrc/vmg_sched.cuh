@@ -496,8 +496,10 @@ inline void enqueue_vcycle_segment(vmg_s* h, int seg, unsigned long long* norm_o
     }
 }
 
-// captures the three segments (once per epoch and kind of weights), then launches segment `seg`
-inline int run_vcycle_segment(vmg_s* h, int seg, unsigned long long* out)
+// captures the three segments (once per epoch and kind of weights), then launches segment `seg` into `into`
+// (the handle's stream, or its high-priority stream for segment 1: a graph runs at the priority of the stream it is
+// launched into)
+inline int run_vcycle_segment(vmg_s* h, int seg, unsigned long long* out, cudaStream_t into = nullptr)
 {
     const int gi = h->lev[0].cw ? 1 : 0;
     if (h->seg_epoch[gi] != h->graph_epoch) {
@@ -518,7 +520,7 @@ inline int run_vcycle_segment(vmg_s* h, int seg, unsigned long long* out)
         }
         h->seg_epoch[gi] = h->graph_epoch;
     }
-    cudaError_t e = cudaGraphLaunch(h->seg_exec[gi][seg], h->stream);
+    cudaError_t e = cudaGraphLaunch(h->seg_exec[gi][seg], into ? into : h->stream);
     if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
     h->launches += h->seg_launches[gi][seg];
     if (seg == 2) h->launches_per_cycle = h->seg_launches[gi][0] + h->seg_launches[gi][1] + h->seg_launches[gi][2];
