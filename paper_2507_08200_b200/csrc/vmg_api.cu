@@ -238,7 +238,6 @@ int vmg_destroy(vmg_handle h)
         }
     }
     if (h->token) cudaEventDestroy(h->token);
-    if (h->coarse_go) cudaEventDestroy(h->coarse_go);
     if (h->coarse_done) cudaEventDestroy(h->coarse_done);
     if (h->coarse_stream) cudaStreamDestroy(h->coarse_stream);
     if (h->h_scal) cudaFreeHost(h->h_scal);
@@ -750,14 +749,11 @@ int vmg_solve_batch(int n, const vmg_handle* hs, const double* const* rhs, doubl
                         int lo = 0, hi = 0;
                         cudaDeviceGetStreamPriorityRange(&lo, &hi);
                         if (cudaEventCreateWithFlags(&h->token, cudaEventDisableTiming) != cudaSuccess ||
-                            cudaEventCreateWithFlags(&h->coarse_go, cudaEventDisableTiming) != cudaSuccess ||
                             cudaEventCreateWithFlags(&h->coarse_done, cudaEventDisableTiming) != cudaSuccess ||
                             cudaStreamCreateWithPriority(&h->coarse_stream, cudaStreamNonBlocking, hi) != cudaSuccess) {
                             h->last_cuda_error = (int)cudaGetLastError(); rc[i] = VMG_ERR_CUDA; continue;
                         }
                     }
-                    // capture (first use) before the wait is enqueued: a capturing stream must not hold foreign work
-                    if (pass == 0 && h->seg_epoch[h->lev[0].cw ? 1 : 0] != h->graph_epoch) cudaStreamSynchronize(h->stream);
                     if (prev) cudaStreamWaitEvent(h->stream, prev, 0);
                     rc[i] = run_vcycle_segment(h, pass == 0 ? 0 : 2, scal + 1);
                     if (rc[i] != VMG_OK) continue;

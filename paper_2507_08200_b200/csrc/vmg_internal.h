@@ -94,7 +94,7 @@ struct vmg_s {
     unsigned seg_epoch[2] = {0, 0};
     cudaEvent_t token = nullptr;       // "level 0 of the GPU is free again" (staggered batch schedule)
     cudaStream_t coarse_stream = nullptr;   // highest priority: the coarser levels of this handle beside another handle's fine level
-    cudaEvent_t coarse_go = nullptr, coarse_done = nullptr;
+    cudaEvent_t coarse_done = nullptr;
     // state of the solve in progress (vmg_solve / vmg_solve_batch phases)
     double sv_rtol = 0.0, sv_nb = 0.0;
     int sv_max = 0, sv_slow = 0, sv_status = 0;
