@@ -60,10 +60,12 @@ enum {
 int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream);
 
 /* Coefficients.  a: cell array or NULL (a == 0, alpha ignored).  bx, by, bz: face arrays, or all NULL for
- * b == 1 (then, unless a mask is set, the sweeps, the residual + restriction and the residual norm run as kernels that form
+ * b == 1 (then the sweeps, the residual + restriction and the residual norm run as kernels that form
  * the face weights from beta/h^2 and the cell's position instead of loading three weight arrays: the same numbers in
  * the same order, bitwise the results of explicit arrays of ones, at 2 instead of 5 doubles of traffic per cell and
- * half-sweep -- the Poisson equation PAPER.md:54 Eq. 3 and Helmholtz equations with a variable a).  a must be >= 0 with alpha >= 0 and b > 0, beta > 0 (not checked; otherwise undefined behaviour).
+ * half-sweep -- the Poisson equation PAPER.md:54 Eq. 3 and Helmholtz equations with a variable a; with a mask set
+ * this holds for level 0, whose kernels then read one byte of open-face flags per cell, the averaged coarser levels
+ * keep their arrays).  a must be >= 0 with alpha >= 0 and b > 0, beta > 0 (not checked; otherwise undefined behaviour).
  * The arrays are read during this call only (enqueued on the stream, then synchronised): the library
  * averages them to all coarse levels (a: mean of the 8 children, 4 in 2-D; b: mean of the fine faces lying
  * on the coarse face) and converts each level to its internal stencil form.  The caller may free or modify

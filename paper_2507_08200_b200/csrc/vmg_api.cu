@@ -223,13 +223,13 @@ int vmg_destroy(vmg_handle h)
     cudaStreamSynchronize(h->stream);
     prof_collect(h);
     for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < 6; ++i) {
         if (h->pcg_exec[i]) cudaGraphExecDestroy(h->pcg_exec[i]);
         if (h->pcg_graph[i]) cudaGraphDestroy(h->pcg_graph[i]);
     }
     if (h->pcg_base) cudaFree(h->pcg_base);
     if (h->mask_base) cudaFree(h->mask_base);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < 3; ++i) {
         if (h->graph_exec[i]) cudaGraphExecDestroy(h->graph_exec[i]);
         if (h->graph[i]) cudaGraphDestroy(h->graph[i]);
         for (int sg = 0; sg < 3; ++sg) {
@@ -278,7 +278,7 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
         fa = a ? h->m_a : nullptr; fbx = h->m_bx; fby = h->m_by; fbz = h->three_d ? h->m_bz : nullptr;
     }
     const double* fad = h->d_mask ? h->lev[0].adiag : nullptr;
-    const int cw = (!bx && !h->d_mask && h->const_weights) ? 1 : 0;   // b = 1 on every face of every level (LevelView::cw)
+    const int cw = (!bx && h->const_weights) ? (h->d_mask ? 2 : 1) : 0;   // b = 1 on every face (LevelView::cw); with a mask: level 0 only
     {   // the constant-weight kernels take beta/h^2 by value: graphs captured with another beta are stale
         const VmgLevel& L = h->lev[0];
         if (cw && (L.cx != beta / (L.hx * L.hx) || L.cy != beta / (L.hy * L.hy))) ++h->graph_epoch;
@@ -310,7 +310,7 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
         g.G = L.G; g.three_d = h->three_d;
         g.alpha = h->alpha; g.cx = beta / (L.hx * L.hx); g.cy = beta / (L.hy * L.hy);
         g.cz = h->three_d ? beta / (L.hz * L.hz) : 0.0;
-        L.cx = g.cx; L.cy = g.cy; L.cz = g.cz; L.cw = cw;
+        L.cx = g.cx; L.cy = g.cy; L.cz = g.cz; L.cw = cw == 2 ? (l == 0 ? 2 : 0) : cw; L.mk = l == 0 ? h->mk0 : nullptr;
         launch_pdl(h, build_stencil_kernel, grid_for(L.n), kThreads, 0, g);
         ++setup_launches;
     }
@@ -349,7 +349,7 @@ int vmg_set_mask(vmg_handle h, const unsigned char* mask, int kind, const double
     if (!h || (kind != VMG_BC_DIRICHLET && kind != VMG_BC_NEUMANN)) return VMG_ERR_ARG;
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     if (h->mask_base) { cudaFree(h->mask_base); h->mask_base = nullptr; }
-    h->d_mask = nullptr; h->d_cval = nullptr; h->m_fold = h->m_a = h->m_bx = h->m_by = h->m_bz = nullptr;
+    h->d_mask = nullptr; h->mk0 = nullptr; h->d_cval = nullptr; h->m_fold = h->m_a = h->m_bx = h->m_by = h->m_bz = nullptr;
     for (int l = 0; l < h->nlev; ++l) h->lev[l].adiag = nullptr;
     h->mask_covered = 0;
     h->have_coeffs = false;            // the stencil has to be rebuilt: vmg_set_coeffs applies the mask
@@ -363,13 +363,18 @@ int vmg_set_mask(vmg_handle h, const unsigned char* mask, int kind, const double
     std::vector<size_t> o_ad((size_t)h->nlev);
     for (int l = 0; l < h->nlev; ++l) o_ad[l] = p.take((size_t)h->lev[l].n);
     size_t o_mask = p.off;
-    CUDA_TRY(h, cudaMalloc(&h->mask_base, o_mask * sizeof(double) + (size_t)L0.n));
+    const size_t mk_bytes = (size_t)L0.nalloc + 2 * (size_t)L0.pad;   // internal layout, pads included
+    CUDA_TRY(h, cudaMalloc(&h->mask_base, o_mask * sizeof(double) + round_up((size_t)L0.n, 16) + mk_bytes));
     double* base = (double*)h->mask_base;
     h->m_fold = base + o_fold; h->m_a = base + o_a; h->m_bx = base + o_bx; h->m_by = base + o_by; h->m_bz = base + o_bz;
     for (int l = 0; l < h->nlev; ++l) h->lev[l].adiag = base + o_ad[l];
     h->d_mask = (unsigned char*)(base + o_mask);
     h->mask_kind = kind;
     CUDA_TRY(h, cudaMemcpyAsync(h->d_mask, mask, (size_t)L0.n, cudaMemcpyDeviceToDevice, h->stream));
+    unsigned char* mk_base = h->d_mask + round_up((size_t)L0.n, 16);
+    CUDA_TRY(h, cudaMemsetAsync(mk_base, 0, mk_bytes, h->stream));
+    h->mk0 = mk_base + L0.pad;
+    mask_face_bits_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, h->d_mask, h->mk0);
     if (cval) {
         h->d_cval = base + o_cval;
         CUDA_TRY(h, cudaMemcpyAsync(h->d_cval, cval, (size_t)L0.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
@@ -578,7 +583,7 @@ int pcg_alloc(vmg_s* h)
 template <typename F>
 int pcg_run(vmg_s* h, int slot, F body)
 {
-    slot += h->lev[0].cw ? 2 : 0;
+    slot += 2 * h->lev[0].cw;
     if (!h->use_graph || h->profile) { body(); return cudaGetLastError() == cudaSuccess ? VMG_OK : VMG_ERR_CUDA; }
     if (h->pcg_epoch[slot] != h->graph_epoch) {
         if (h->pcg_exec[slot]) { cudaGraphExecDestroy(h->pcg_exec[slot]); h->pcg_exec[slot] = nullptr; }

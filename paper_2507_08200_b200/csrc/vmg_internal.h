@@ -42,7 +42,8 @@ struct VmgLevel {
     // averaged raw coefficients in the public layout (levels >= 1 only; level 0 reads the caller's arrays)
     double *a = nullptr, *bx = nullptr, *by = nullptr, *bz = nullptr;
     double cx = 0.0, cy = 0.0, cz = 0.0;   // beta / h^2 of this level
-    int cw = 0;                             // constant face weights (LevelView::cw)
+    int cw = 0;                             // constant face weights (LevelView::cw: 0 arrays, 1 constant, 2 constant + mask)
+    const unsigned char* mk = nullptr;      // cw == 2: the open faces of every cell, one byte, internal layout
     double* adiag = nullptr;  // masking: extra diagonal of this level, public layout (nullptr without a mask)
 };
 
@@ -80,18 +81,18 @@ struct vmg_s {
     void* arena = nullptr;
     size_t arena_bytes = 0;
     // graph of one V-cycle (+ residual norm)
-    // two slots: [0] general kernels, [1] constant-weight kernels (LevelView::cw), so that a time step that alternates
+    // one slot per kind of level-0 kernels (LevelView::cw), so that a time step that alternates
     // between the two kinds of equation re-instantiates nothing; a slot is current when its epoch equals graph_epoch
-    cudaGraph_t graph[2] = {nullptr, nullptr};
-    cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
-    unsigned graph_slot_epoch[2] = {0, 0};
-    long long graph_slot_launches[2] = {0, 0};
+    cudaGraph_t graph[3] = {nullptr, nullptr, nullptr};
+    cudaGraphExec_t graph_exec[3] = {nullptr, nullptr, nullptr};
+    unsigned graph_slot_epoch[3] = {0, 0, 0};
+    long long graph_slot_launches[3] = {0, 0, 0};
     // the same cycle cut in three graphs for the staggered batch schedule (vmg_solve_batch): [cw][segment], segment
     // 0 = level-0 down-stroke, 1 = all coarser levels, 2 = level-0 up-stroke + residual norm
-    cudaGraph_t seg_graph[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
-    cudaGraphExec_t seg_exec[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
-    long long seg_launches[2][3] = {{0, 0, 0}, {0, 0, 0}};
-    unsigned seg_epoch[2] = {0, 0};
+    cudaGraph_t seg_graph[3][3] = {};
+    cudaGraphExec_t seg_exec[3][3] = {};
+    long long seg_launches[3][3] = {};
+    unsigned seg_epoch[3] = {0, 0, 0};
     cudaEvent_t token = nullptr;       // "level 0 of the GPU is free again" (staggered batch schedule)
     cudaStream_t coarse_stream = nullptr;   // highest priority: the coarser levels of this handle beside another handle's fine level
     cudaEvent_t coarse_done = nullptr;
@@ -103,6 +104,7 @@ struct vmg_s {
     // cell masking (vmg_set_mask): device copies and the effective level-0 coefficients, one allocation
     void* mask_base = nullptr;
     unsigned char* d_mask = nullptr;
+    unsigned char* mk0 = nullptr;      // open-face bits of level 0 in the internal layout (inside mask_base)
     double *d_cval = nullptr, *m_fold = nullptr, *m_a = nullptr, *m_bx = nullptr, *m_by = nullptr, *m_bz = nullptr;
     int mask_kind = 1;
     long long mask_covered = 0;
@@ -110,9 +112,9 @@ struct vmg_s {
     void* pcg_base = nullptr;
     double *pcg_x = nullptr, *pcg_p = nullptr, *pcg_q = nullptr, *pcg_partial = nullptr, *pcg_scal = nullptr;
     int pcg_npartial = 0;
-    cudaGraph_t pcg_graph[4] = {nullptr, nullptr, nullptr, nullptr};       // [slot + 2 * cw]
-    cudaGraphExec_t pcg_exec[4] = {nullptr, nullptr, nullptr, nullptr};
-    unsigned pcg_epoch[4] = {0, 0, 0, 0};
+    cudaGraph_t pcg_graph[6] = {};       // [slot + 2 * cw]
+    cudaGraphExec_t pcg_exec[6] = {};
+    unsigned pcg_epoch[6] = {0, 0, 0, 0, 0, 0};
     unsigned graph_epoch = 1;          // bumped whenever captured graphs become stale
     // result of the last solve
     int cycles = 0;

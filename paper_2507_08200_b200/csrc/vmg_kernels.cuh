@@ -242,6 +242,27 @@ __global__ void fold_bc_kernel(FoldArgs g)
     g.bt[g.bt_natural ? t : cell_at(g.G, i, j, k)] = v;
 }
 
+// the open faces of every cell as one byte in the internal layout (LevelView::mk): bit f (0..5 = low x, high x, low y,
+// high y, low z, high z) is set when the face is interior to the domain and the cells on both sides are valid
+__global__ void mask_face_bits_kernel(Geom G, const unsigned char* __restrict__ nat, unsigned char* __restrict__ in)
+{
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= G.n) return;
+    int i, j, k;
+    unflatten(G, t, i, j, k);
+    const long long nxy = (long long)G.nx * G.ny;
+    unsigned fb = 0;
+    if (nat[t]) {
+        if (i > 0 && nat[t - 1]) fb |= 1u;
+        if (i < G.nx - 1 && nat[t + 1]) fb |= 2u;
+        if (j > 0 && nat[t - G.nx]) fb |= 4u;
+        if (j < G.ny - 1 && nat[t + G.nx]) fb |= 8u;
+        if (k > 0 && nat[t - nxy]) fb |= 16u;
+        if (k < G.nz - 1 && nat[t + nxy]) fb |= 32u;
+    }
+    in[cell_at(G, i, j, k)] = (unsigned char)fb;
+}
+
 // public (natural) layout <-> internal layout of one cell array
 // mask (may be NULL): covered cells enter as zero (they are identity rows of the masked operator)
 __global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in, const unsigned char* __restrict__ mask)
@@ -337,15 +358,25 @@ struct LevelView {
     // with CW = true take the six weights from these three numbers and the cell's position instead of loading them,
     // 2 doubles per cell and half-sweep instead of 5.  Same values, same order of operations: bitwise the results
     // of the general kernels on arrays of ones.
+    // cw = 2: the same with a cell mask (vmg_set_mask): a face carries beta/h^2 if the cells on both sides are valid and 0
+    // otherwise -- exactly the effective coefficients of the masked operator on level 0 (coarser levels of a masked
+    // hierarchy have averaged, fractional b and use the arrays).  mk: one byte per cell in the internal layout, bit f =
+    // face f open (mask_face_bits_kernel): half a byte per cell and half-sweep instead of 24.
     double cx, cy, cz;
     int cw;
+    const unsigned char* mk;
 };
 
 // the six face weights of cell (i, j, k): low x, high x, low y, high y, low z, high z
-template <bool CW>
+template <int CW>
 __device__ __forceinline__ void face_weights(const LevelView& L, long long c, long long xm, int i, int j, int k, double (&w)[6])
 {
-    if (CW) {
+    if (CW == 2) {
+        const unsigned fb = L.mk[c];     // bit f: face f is open (both cells valid, not a domain face)
+        w[0] = (fb & 1u) ? L.cx : 0.0;   w[1] = (fb & 2u) ? L.cx : 0.0;
+        w[2] = (fb & 4u) ? L.cy : 0.0;   w[3] = (fb & 8u) ? L.cy : 0.0;
+        w[4] = (fb & 16u) ? L.cz : 0.0;  w[5] = (fb & 32u) ? L.cz : 0.0;
+    } else if (CW) {
         w[0] = i > 0 ? L.cx : 0.0;  w[1] = i < L.G.nx - 1 ? L.cx : 0.0;
         w[2] = j > 0 ? L.cy : 0.0;  w[3] = j < L.G.ny - 1 ? L.cy : 0.0;
         w[4] = k > 0 ? L.cz : 0.0;  w[5] = k < L.G.nz - 1 ? L.cz : 0.0;
@@ -381,7 +412,7 @@ __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, i
 // L2 residency: what the NEXT half-sweep (other colour, opposite direction) needs again are the face weights and the
 // phi written here; rhs, 1/D and the neighbours' phi are dead after this read, so they are loaded with the streaming
 // (evict-first) policy and do not push the weights out of the 126 MB L2.
-template <bool CW>
+template <int CW>
 __device__ __forceinline__ void relax_at(const LevelView& L, double* phi, const double* rhs, int colour, int m, int j, int k)
 {
     const Geom& G = L.G;
@@ -403,7 +434,7 @@ __device__ __forceinline__ void relax_at(const LevelView& L, double* phi, const 
 // reverse: walk the level from its last plane to its first.  Consecutive half-sweeps alternate direction, so that
 // each one starts on the planes the previous one touched last, which are still in the 126 MB L2 (face weights and
 // the phi just written are common to both colours).
-template <bool CW>
+template <int CW>
 __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour, int reverse)
 {
     grid_dependency_wait();
@@ -419,7 +450,7 @@ __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, cons
 // stored: the cells of the other colour keep their uncorrected values in memory until the next half-sweep
 // overwrites them.  Valid when at least one full sweep follows (nu2 >= 1).  phi_nb + e is the very addition
 // prolong_correct_kernel performs, so results are bitwise those of the two separate kernels.
-template <bool CW>
+template <int CW>
 __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom& CG, double* phi,
                                                   const double* rhs, const double* e, int colour, int sz,
                                                   int m, int j, int k)
@@ -463,7 +494,7 @@ __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom
     phi[c] = L.dinv[c] * (rhs[c] + s);
 }
 
-template <bool CW>
+template <int CW>
 __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __restrict__ phi, const double* __restrict__ rhs,
                                              const double* __restrict__ e, int colour, int sz, int reverse)
 {
@@ -482,7 +513,7 @@ __device__ __forceinline__ double residual_at(const LevelView& L, const double* 
 // the same with the cell's position known (CW = true: constant face weights, see LevelView).  STREAM: phi, rhs and 1/D
 // are read with the streaming (evict-first) policy, as in relax_at -- for the norm at the end of a cycle, after which
 // the next kernel needs the face weights again and nothing else that is read here.
-template <bool CW, bool STREAM = false>
+template <int CW, bool STREAM = false>
 __device__ __forceinline__ double residual_at(const LevelView& L, const double* phi, const double* rhs, long long c, long long xm,
                                               int i, int j, int k)
 {
@@ -515,7 +546,7 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 // S3 (per-colour path). Fused residual + restriction: one thread per coarse cell; also zeroes the coarse phi.
 // (Four lanes per coarse cell with a shuffle gather was tried: 70 us instead of 49 us on 256x128x128, the 64-byte
 // runs per row coalesce worse than they gain in occupancy.)
-template <bool CW>
+template <int CW>
 __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG, const double* phi,
                                              const double* rhs, double* crhs, double* cphi,
                                              int sz, int I, int J, int K)
@@ -534,7 +565,7 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
     if (cphi) cphi[cc] = 0.0;
 }
 
-template <bool CW>
+template <int CW>
 __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
                                          double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
 {
@@ -655,7 +686,7 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
 
 // ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one cell per thread, both colours or red only
 // (as (like two colour half-sweeps in one launch: 13 loads and a division per thread at full occupancy)
-template <bool CW>
+template <int CW>
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
                                      unsigned long long* out, int reverse)
 {

@@ -20,12 +20,12 @@ inline LevelView view(const VmgLevel& L)
     LevelView v;
     v.wx = L.wx; v.wy = L.wy; v.wz = L.wz; v.dinv = L.dinv;
     v.G = L.G;
-    v.cx = L.cx; v.cy = L.cy; v.cz = L.cz; v.cw = L.cw;
+    v.cx = L.cx; v.cy = L.cy; v.cz = L.cz; v.cw = L.cw; v.mk = L.mk;
     return v;
 }
 
 // picks the instantiation for the level's kind of weights (LevelView::cw)
-#define VMG_BY_WEIGHTS(L, KERNEL) ((L).cw ? KERNEL<true> : KERNEL<false>)
+#define VMG_BY_WEIGHTS(L, KERNEL) ((L).cw == 2 ? KERNEL<2> : (L).cw ? KERNEL<1> : KERNEL<0>)
 
 inline unsigned grid_for(long long n) { return (unsigned)cdiv(n, kThreads); }
 
@@ -501,7 +501,7 @@ inline void enqueue_vcycle_segment(vmg_s* h, int seg, unsigned long long* norm_o
 // launched into)
 inline int run_vcycle_segment(vmg_s* h, int seg, unsigned long long* out, cudaStream_t into = nullptr)
 {
-    const int gi = h->lev[0].cw ? 1 : 0;
+    const int gi = h->lev[0].cw;
     if (h->seg_epoch[gi] != h->graph_epoch) {
         prepare_blocked(h);
         for (int sg = 0; sg < 3; ++sg) {
@@ -540,7 +540,7 @@ inline int run_vcycle_with_norm(vmg_s* h, unsigned long long* out)
         if (cudaGetLastError() != cudaSuccess) return VMG_ERR_CUDA;
         return VMG_OK;
     }
-    const int gi = h->lev[0].cw ? 1 : 0;
+    const int gi = h->lev[0].cw;
     if (h->graph_slot_epoch[gi] != h->graph_epoch) {
         if (h->graph_exec[gi]) { cudaGraphExecDestroy(h->graph_exec[gi]); h->graph_exec[gi] = nullptr; }
         if (h->graph[gi]) { cudaGraphDestroy(h->graph[gi]); h->graph[gi] = nullptr; }

@@ -751,3 +751,39 @@ def test_alternating_equation_kinds_on_one_handle_keeps_results():
             f.destroy()
             assert got[1] == want[1] and torch.equal(got[0], want[0]), (kind, beta, pcg)
     s.destroy()
+
+
+@pytest.mark.parametrize("kind", [D, N], ids=["dirichlet_interface", "neumann_interface"])
+@pytest.mark.parametrize("dims", [(40, 24, 16), (48, 40, 1), (64, 64, 32), (256, 128, 32)])
+def test_masked_constant_weight_kernels_equal_the_general_ones_bitwise(dims, kind):
+    """b == NULL with a mask (the Poisson equation around electrodes): level 0 runs kernels that take a
+    face weight to be beta/h^2 when the cells on both sides are valid and 0 otherwise, read from the byte mask instead of
+    three weight arrays.  Bitwise the general kernels (const_weights=0) for V-cycles and PCG, and the oracle's solution."""
+    b = _binding()
+    p = inputs.random_problem(*dims, seed=27, bc_type=[D, N, N, D, N, N])
+    mask, cval = _mask_for(p, seed=3)
+    cv = cval if kind == D else None
+    d = b.upload(p)
+    out = []
+    for cwopt in (1, 0):
+        s = b.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz)
+        s.set_option("const_weights", cwopt)
+        s.set_mask(dev(mask), kind, None if cv is None else dev(cv))
+        s.set_coeffs(d["a"], None, None, None, p.alpha, p.beta)
+        s.set_bc(p.bc_type, d["bc_value"])
+        phi = torch.full_like(d["rhs"], 0.5)
+        st = s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=40)
+        info = s.get_info()
+        phi2 = torch.zeros_like(d["rhs"])
+        st2 = s.solve_pcg(d["rhs"], phi2, rtol=1e-12, max_iter=40)
+        out.append((st, info, phi, st2, s.get_info(), phi2))
+        s.destroy()
+    assert out[0][0] == out[1][0] == 0 and out[0][1] == out[1][1] and torch.equal(out[0][2], out[1][2])
+    assert out[0][3] == out[1][3] == 0 and out[0][4] == out[1][4] and torch.equal(out[0][5], out[1][5])
+    if p.nx * p.ny * p.nz <= 200000:
+        o = Oracle.from_problem(p)
+        o.set_mask(mask, kind, cv)
+        o.set_coeffs(p.a, None, None, None, p.alpha, p.beta)
+        phi_o, st_o, cyc_o, _, _ = o.solve(p.rhs, np.full(p.rhs.shape, 0.5), rtol=1e-12, max_vcycles=40)
+        assert st_o == 0 and abs(cyc_o - out[0][1][0]) <= 1 and rel(out[0][2].cpu().numpy(), phi_o) <= PHI_TOL
+        o.close()
