@@ -787,3 +787,32 @@ def test_masked_constant_weight_kernels_equal_the_general_ones_bitwise(dims, kin
         phi_o, st_o, cyc_o, _, _ = o.solve(p.rhs, np.full(p.rhs.shape, 0.5), rtol=1e-12, max_vcycles=40)
         assert st_o == 0 and abs(cyc_o - out[0][1][0]) <= 1 and rel(out[0][2].cpu().numpy(), phi_o) <= PHI_TOL
         o.close()
+
+
+def test_staggered_batch_at_full_size_is_bitwise_the_single_solves():
+    """vmg_solve_batch at 256x128x128, where the staggered schedule really overlaps one handle's coarse levels with another's
+    fine level (three handles: config 3, config 4, config 3 with b == NULL): bit for bit the single solves."""
+    b = _binding()
+    probs = [inputs.config3(128), inputs.config4(128), inputs.config3(128)]
+    streams = [torch.cuda.Stream() for _ in probs]
+    solvers, data = [], []
+    for n, (p, stream) in enumerate(zip(probs, streams)):
+        s, d = b.from_problem(p, stream=stream)
+        if n == 2:
+            s.set_coeffs(d["a"], None, None, None, p.alpha, p.beta)
+        solvers.append(s); data.append(d)
+    torch.cuda.synchronize()
+    single = []
+    for s, d, p, stream in zip(solvers, data, probs, streams):
+        phi = torch.zeros_like(d["rhs"])
+        with torch.cuda.stream(stream):
+            st = s.solve(d["rhs"], phi, rtol=p.rtol, max_vcycles=p.max_vcycles)
+        single.append((st, s.get_info(), phi))
+    for _ in range(2):
+        phis = [torch.zeros_like(d["rhs"]) for d in data]
+        sts = b.solve_batch(solvers, [d["rhs"] for d in data], phis, rtol=probs[0].rtol, max_vcycles=probs[0].max_vcycles)
+        for s, st, phi, ref in zip(solvers, sts, phis, single):
+            assert st == ref[0] and s.get_info() == ref[1] and torch.equal(phi, ref[2])
+    assert torch.equal(single[0][2], single[2][2])   # constant-weight kernels = arrays of ones
+    for s in solvers:
+        s.destroy()
