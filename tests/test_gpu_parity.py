@@ -816,3 +816,36 @@ def test_staggered_batch_at_full_size_is_bitwise_the_single_solves():
     assert torch.equal(single[0][2], single[2][2])   # constant-weight kernels = arrays of ones
     for s in solvers:
         s.destroy()
+
+
+def test_changing_the_mask_on_a_handle_equals_fresh_handles():
+    """vmg_set_mask twice with different geometry and kind, then removed, with and without explicit b: every solve equals the
+    solve of a fresh handle bit for bit (the handle re-allocates the mask arrays and drops its captured graphs)."""
+    b = _binding()
+    p = inputs.random_problem(40, 24, 16, seed=19, bc_type=[D, N, N, D, N, N])
+    d = b.upload(p)
+    m1, c1 = _mask_for(p, seed=1)
+    m2 = np.ones(p.rhs.shape, dtype=np.uint8)
+    m2[4:9, 5:15, 10:30] = 0
+    steps = [(m1, D, c1, True), (m2, N, None, True), (m2, D, None, False), (None, D, None, False), (m1, N, None, True), (None, D, None, True)]
+
+    def run(s, mask, kind, cval, explicit_b):
+        s.set_mask(None if mask is None else dev(mask), kind, None if cval is None else dev(cval))
+        if explicit_b:
+            s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+        else:
+            s.set_coeffs(d["a"], None, None, None, p.alpha, p.beta)
+        phi = torch.zeros_like(d["rhs"])
+        st = s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=60)
+        return st, s.get_info(), phi
+
+    s = b.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz)
+    s.set_bc(p.bc_type, d["bc_value"])
+    for step in steps:
+        got = run(s, *step)
+        f = b.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz)
+        f.set_bc(p.bc_type, d["bc_value"])
+        want = run(f, *step)
+        f.destroy()
+        assert got[0] == want[0] == 0 and got[1] == want[1] and torch.equal(got[2], want[2])
+    s.destroy()
