@@ -510,15 +510,17 @@ __device__ __forceinline__ double residual_at(const LevelView& L, const double* 
     return rhs[c] + nb_sum(L, phi, c, xm) - phi[c] / L.dinv[c];
 }
 
-// the same with the cell's position known (CW = true: constant face weights, see LevelView).  STREAM: phi, rhs and 1/D
+// the same with the cell's position known (CW: constant face weights, see LevelView).  STREAM = 1: phi, rhs and 1/D
 // are read with the streaming (evict-first) policy, as in relax_at -- for the norm at the end of a cycle, after which
-// the next kernel needs the face weights again and nothing else that is read here.
-template <int CW, bool STREAM = false>
+// the next kernel needs the face weights again and nothing else that is read here.  STREAM = 2: rhs and 1/D only (the
+// residual + restriction: phi and the weights are what the up-stroke should still find in L2).
+template <int CW, int STREAM = 0>
 __device__ __forceinline__ double residual_at(const LevelView& L, const double* phi, const double* rhs, long long c, long long xm,
                                               int i, int j, int k)
 {
     if (!CW && !STREAM) return residual_at(L, phi, rhs, c, xm);
-    auto ld = [](const double* p) { return STREAM ? __ldcs(p) : *p; };
+    auto ld = [](const double* p) { return STREAM == 1 ? __ldcs(p) : *p; };
+    auto ld2 = [](const double* p) { return STREAM ? __ldcs(p) : *p; };
     double w[6];
     face_weights<CW>(L, c, xm, i, j, k, w);
     double s = w[0] * ld(phi + xm);
@@ -527,7 +529,7 @@ __device__ __forceinline__ double residual_at(const LevelView& L, const double* 
     s = fma(w[3], ld(phi + c + L.G.pitch), s);
     s = fma(w[4], ld(phi + c - L.G.plane), s);
     s = fma(w[5], ld(phi + c + L.G.plane), s);
-    return ld(rhs + c) + s - ld(phi + c) / ld(L.dinv + c);
+    return ld2(rhs + c) + s - ld(phi + c) / ld2(L.dinv + c);
 }
 
 // r in the public layout (single-step entry point)
@@ -558,7 +560,7 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
             long long row = L.G.plane * k + (long long)L.G.pitch * j, ce, xe, co, xo;
             pair_addr(L.G, row, I, 0, ce, xe);
             pair_addr(L.G, row, I, 1, co, xo);
-            s += residual_at<CW>(L, phi, rhs, ce, xe, 2 * I, j, k) + residual_at<CW>(L, phi, rhs, co, xo, 2 * I + 1, j, k);
+            s += residual_at<CW, CW ? 0 : 2>(L, phi, rhs, ce, xe, 2 * I, j, k) + residual_at<CW, CW ? 0 : 2>(L, phi, rhs, co, xo, 2 * I + 1, j, k);   // rhs, 1/D streamed
         }
     const long long cc = cell_at(CG, I, J, K);
     crhs[cc] = s / (4.0 * sz);
@@ -703,7 +705,7 @@ __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi
         if (2 * m + par < G.nx) {
             long long c, xm;
             pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
-            mx = fabs(residual_at<CW, !CW>(L, phi, rhs, c, xm, 2 * m + par, j, k));   // constant weights: the level fits L2, keep it there
+            mx = fabs(residual_at<CW, CW ? 0 : 1>(L, phi, rhs, c, xm, 2 * m + par, j, k));   // constant weights: the level fits L2, keep it there
             if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
         }
     }
