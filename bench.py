@@ -37,6 +37,8 @@ B_SETCOEFFS = 24.0
 # DRAM bytes of the six half-sweep launches of one 3-sweep pass over level 0 of config 3, from the ncu --set full
 # capture summarised in profiles/r1d_ncu_full.md (155.5 MB read + 16.8 MB written per launch, each launch cold)
 TRAFFIC_PASS_CONFIG3 = 6 * (155.5e6 + 16.8e6)
+# the same pass with the L2 as the previous launch left it (single-pass ncu, --cache-control none: profiles/r1h_warm_dram.md)
+TRAFFIC_PASS_CONFIG3_WARM = 6 * (100.76e6 + 3.34e6)
 
 
 def level_cells(nx, ny, nz):
@@ -488,6 +490,8 @@ def run_vmg(args):
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": TRAFFIC_PASS_CONFIG3 if args.config == 3 and not args.opt else None,
                      "traffic_note": "DRAM bytes per pass, ncu, each launch cold (profiles/r1d_ncu_full.md); achieved and traffic are per pass = 6 launches",
+                     "traffic_warm": TRAFFIC_PASS_CONFIG3_WARM if args.config == 3 and not args.opt else None,
+                     "traffic_warm_note": "the same with the L2 left as the previous launch left it (profiles/r1h_warm_dram.md); whole V-cycle 1612 MB",
                      "achieved_bytes_per_pass": B_SMOOTH_PASS * n0, "peak_source": peak_src,
                      "launches_per_pass": sm_launches / max(2 * n_prof_cycles, 1)},
         "kernel_classes": klass,
