@@ -403,6 +403,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "snake")) { h->snake = iv != 0; }
     else if (!strcmp(key, "pdl")) { h->use_pdl = iv != 0; }
     else if (!strcmp(key, "block_min_cells")) { if (v < 0) return VMG_ERR_ARG; h->block_min_cells = (long long)v; }
+    else if (!strcmp(key, "phi_keep_cells")) { if (v < 0) return VMG_ERR_ARG; h->phi_keep_cells = (long long)v; }
     else if (!strcmp(key, "l2_persist")) { if (v < 0) return VMG_ERR_ARG; h->l2_persist_mb = v; h->l2_applied = false; }
     else if (!strcmp(key, "profile")) {
         h->profile = iv != 0;

@@ -68,6 +68,7 @@ struct vmg_s {
     double l2_persist_mb = 24.0;  // L2 set aside for the level-0 face weights (0: none); see apply_l2_window
     bool l2_applied = false, l2_window_set = false;
     int use_pdl = 1;              // programmatic dependent launch of the V-cycle kernels
+    long long phi_keep_cells = 1ll << 25;     // option "phi_keep_cells": levels with at least this many cells (default 32 Mi: phi = 2 x L2) load the neighbours' phi with the normal policy
     int snake = 1;                // consecutive half-sweeps walk the level in opposite directions (L2 reuse)
     int use_tail = 1;             // run the coarsest levels in one CTA (vmg_tail.cuh)
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)

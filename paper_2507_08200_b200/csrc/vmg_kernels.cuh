@@ -412,7 +412,9 @@ __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, i
 // L2 residency: what the NEXT half-sweep (other colour, opposite direction) needs again are the face weights and the
 // phi written here; rhs, 1/D and the neighbours' phi are dead after this read, so they are loaded with the streaming
 // (evict-first) policy and do not push the weights out of the 126 MB L2.
-template <int CW>
+// KEEP = 1 (option "phi_keep_cells"): the neighbours' phi with the normal policy -- on levels far larger than the L2 the
+// evict-first lines are gone before the next row and plane ask for them (512^3: 12 % more DRAM traffic than algorithmic).
+template <int CW, int KEEP = 0>
 __device__ __forceinline__ void relax_at(const LevelView& L, double* phi, const double* rhs, int colour, int m, int j, int k)
 {
     const Geom& G = L.G;
@@ -422,26 +424,27 @@ __device__ __forceinline__ void relax_at(const LevelView& L, double* phi, const 
     pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
     double w[6];
     face_weights<CW>(L, c, xm, 2 * m + par, j, k, w);
-    double s = w[0] * __ldcs(phi + xm);
-    s = fma(w[1], __ldcs(phi + xm + 1), s);
-    s = fma(w[2], __ldcs(phi + c - G.pitch), s);
-    s = fma(w[3], __ldcs(phi + c + G.pitch), s);
-    s = fma(w[4], __ldcs(phi + c - G.plane), s);
-    s = fma(w[5], __ldcs(phi + c + G.plane), s);
+    auto ld = [](const double* q) { return KEEP ? *q : __ldcs(q); };
+    double s = w[0] * ld(phi + xm);
+    s = fma(w[1], ld(phi + xm + 1), s);
+    s = fma(w[2], ld(phi + c - G.pitch), s);
+    s = fma(w[3], ld(phi + c + G.pitch), s);
+    s = fma(w[4], ld(phi + c - G.plane), s);
+    s = fma(w[5], ld(phi + c + G.plane), s);
     phi[c] = __ldcs(L.dinv + c) * (__ldcs(rhs + c) + s);
 }
 
 // reverse: walk the level from its last plane to its first.  Consecutive half-sweeps alternate direction, so that
 // each one starts on the planes the previous one touched last, which are still in the 126 MB L2 (face weights and
 // the phi just written are common to both colours).
-template <int CW>
+template <int CW, int KEEP = 0>
 __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, const double* __restrict__ rhs, int colour, int reverse)
 {
     grid_dependency_wait();
     // grid (x-pair blocks, row blocks, planes), block (x-pairs, rows): no division to find the cell (pair_launch_dims)
     int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
     if (reverse) { k = L.G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
-    if (m < L.G.ne && j < L.G.ny) relax_at<CW>(L, phi, rhs, colour, m, j, k);
+    if (m < L.G.ne && j < L.G.ny) relax_at<CW, KEEP>(L, phi, rhs, colour, m, j, k);
 }
 
 // S4 + S2 fused (per-colour path).  The first colour half-sweep after a coarse-grid correction: a relaxation never

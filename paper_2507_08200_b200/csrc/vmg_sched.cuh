@@ -143,7 +143,10 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
             if (2 * s + c2 < skip_first) continue;
             dim3 grid, block;
             pair_launch_dims(L, grid, block);
-            launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_kernel), grid, block, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
+            if (L.cw == 0 && L.n >= h->phi_keep_cells)
+                launch_pdl(h, smooth_colour_kernel<0, 1>, grid, block, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
+            else
+                launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_kernel), grid, block, 0, v, cur_phi(L), L.rhs, colour, next_dir(h, L));
             ++*count;
         }
 }
