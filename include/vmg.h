@@ -136,7 +136,7 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  * "l2_persist" (MB of L2 set aside for the level-0 face weights through a stream access-policy window,
  *   default 24, 0 = none; applied only when those weights exceed half the L2.  NOTE: this calls
  *   cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize), a setting of the whole CUDA context),
- * "phi_keep_cells" (levels with at least this many cells read the neighbours' phi in a colour half-sweep with the normal
+ * "phi_keep_cells" (levels with at least this many cells read phi in a colour half-sweep (the neighbours) and in the residual norm with the normal
  *   cache policy instead of the streaming one, default 33554432: on a level whose phi is more than twice the L2 the
  *   evict-first lines are gone before the next row and plane ask for them; results do not depend on it),
  * "pdl" (1: the V-cycle kernels are launched with programmatic stream serialisation, so each kernel's launch overlaps

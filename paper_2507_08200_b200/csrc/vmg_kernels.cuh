@@ -691,7 +691,7 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
 
 // ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one cell per thread, both colours or red only
 // (as (like two colour half-sweeps in one launch: 13 loads and a division per thread at full occupancy)
-template <int CW>
+template <int CW, int KEEP = 0>   // KEEP = 1: phi with the normal policy (levels far larger than the L2, see relax_at)
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
                                      unsigned long long* out, int reverse)
 {
@@ -708,7 +708,7 @@ __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi
         if (2 * m + par < G.nx) {
             long long c, xm;
             pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
-            mx = fabs(residual_at<CW, CW ? 0 : 1>(L, phi, rhs, c, xm, 2 * m + par, j, k));   // constant weights: the level fits L2, keep it there
+            mx = fabs(residual_at<CW, CW ? 0 : KEEP ? 2 : 1>(L, phi, rhs, c, xm, 2 * m + par, j, k));   // constant weights: the level fits L2, keep it there
             if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
         }
     }

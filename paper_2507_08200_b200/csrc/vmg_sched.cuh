@@ -192,7 +192,10 @@ inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_on
     pair_launch_dims(L, grid, block);
     if (!red_only) grid.z *= 2;                               // one cell per thread: the planes once per colour
     ProfScope ps(h, VMG_PC_NORM, nullptr);
-    launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
+    if (L.cw == 0 && L.n >= h->phi_keep_cells)
+        launch_pdl(h, residual_norm_kernel<0, 1>, grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
+    else
+        launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
 }
 
 // ------------------------------------------------------------------------------------------------
