@@ -92,12 +92,13 @@ def test_single_steps_match_oracle(dims):
 
 
 def test_schedule_options_do_not_change_a_single_bit():
-    """Direction of traversal, L2 carve-out, graph replay and the single-CTA tail only reorder independent work:
+    """Direction of traversal, L2 carve-out, cache policy of the loads, graph replay and the single-CTA tail only reorder independent work:
     the converged phi and the residual history are bitwise those of the plain in-order launches."""
     b = _binding()
     p = inputs.config4(32)
     ref = None
-    for opts in (dict(snake=0, l2_persist=0, graph=0, tail=0), dict(), dict(snake=1, graph=0), dict(tail=0), dict(blocked=1)):
+    for opts in (dict(snake=0, l2_persist=0, graph=0, tail=0), dict(), dict(snake=1, graph=0), dict(tail=0), dict(blocked=1),
+                 dict(phi_keep_cells=0), dict(phi_keep_cells=0, graph=0, tail=0)):   # cache policy of the largest levels on all levels
         s, d = b.from_problem(p)
         for k, v in opts.items():
             s.set_option(k, v)
