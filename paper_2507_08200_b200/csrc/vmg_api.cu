@@ -279,9 +279,10 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
     }
     const double* fad = h->d_mask ? h->lev[0].adiag : nullptr;
     const int cw = (!bx && h->const_weights) ? (h->d_mask ? 2 : 1) : 0;   // b = 1 on every face (LevelView::cw); with a mask: level 0 only
-    {   // the constant-weight kernels take beta/h^2 by value: graphs captured with another beta are stale
-        const VmgLevel& L = h->lev[0];
-        if (cw && (L.cx != beta / (L.hx * L.hx) || L.cy != beta / (L.hy * L.hy))) ++h->graph_epoch;
+    if (cw) {   // the constant-weight kernels take beta/h^2 by value: graphs captured with another beta are stale.  Compared
+                // with the beta of the last constant-weight call (a general call in between overwrites the levels' cx, cy, cz)
+        if (h->cw_beta != beta) ++h->graph_epoch;
+        h->cw_beta = beta;
     }
     for (int l = 0; l < h->nlev; ++l) {
         VmgLevel& L = h->lev[l];

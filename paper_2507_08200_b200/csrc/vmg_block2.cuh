@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(BlockCfg<S, TAIL, NXT, NYT>::NT, 1) smooth_blo
                            {live && jj <= NYT / 2 - 2 && m > 0, live && jj <= NYT / 2 - 2 && m < NXP - 1}};
     // the x-pair's even cell in row gy0 of plane 0 (internal layout); its odd cell is `odd` further on
     const long long cbase = (long long)g.G.pitch * gy0 + (gx >> 1);
-    const int odd = g.G.ne + 1;
+    const int odd = g.G.hp;
 
     // register rings [row][slot]: even-x / odd-x phi and wz of this thread's pair; plane z0 + n lives in slot n % R
     double pe[2][R], po[2][R], we[2][R], wo[2][R];

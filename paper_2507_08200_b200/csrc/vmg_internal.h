@@ -62,6 +62,7 @@ struct vmg_s {
     bool have_coeffs = false, have_bc = false, dinv_dirty = true;
     int nu1 = 3, nu2 = 3, nbottom = 32;
     int const_weights = 1;                  // option "const_weights": use the constant-weight kernels when b == NULL
+    double cw_beta = -1.0;                  // beta of the last vmg_set_coeffs with b == NULL (the captured constant-weight graphs carry beta/h^2 by value)
     int prolong = 0;              // 0: piecewise constant (R9 default), 1: trilinear
     int symmetric = 0;            // 1: symmetric V-cycle (post-smoothing / second half of the bottom black -> red): the PCG preconditioner
     int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200

@@ -27,28 +27,31 @@ __device__ __forceinline__ void grid_dependency_wait()
 // Internal layout of a level's cell arrays ("x-parity split").  A colour half-sweep
 // touches every other cell of a row, so in the natural layout half of every 32-byte sector of rhs, 1/D and of the
 // phi being written is fetched for nothing.  Each row therefore stores its even-x cells first, then its odd-x
-// cells, each block followed by one zero element:   [E_0 .. E_{ne-1} 0 | O_0 .. O_{no-1} 0],  pitch = nx + 2.
+// cells, each block followed by at least one zero element:   [E_0 .. E_{ne-1} 0.. | O_0 .. O_{no-1} 0..].  Each half is
+// hp = ne + 1 rounded up to a multiple of 4 doubles long (pitch = 2 hp), so both halves of every row start on a 32-byte
+// sector and every stride of the level is a multiple of 16 bytes: the array is then a legal TMA tensor
+// (m, row pair, row parity, x-parity, plane) for the blocked smoother (vmg_block3.cuh).
 // A half-sweep then reads and writes unit-stride runs and moves 5 doubles per cell of the level (10 per relaxation) instead of 7 (14).  The pad
 // elements double as the zero weight / zero neighbour beyond the low and high x faces (the x-neighbours of E_m are
 // O_{m-1}, O_m, those of O_m are E_m, E_{m+1}); y- and z-neighbours are +-pitch, +-plane away, and beyond the domain
 // they land in another row / plane or in the zeroed pad before and after the array, always under a zero weight.
 // ------------------------------------------------------------------------------------------------
 struct Geom {
-    int nx, ny, nz, ne, pitch;   // ne = even-x cells per row
-    long long plane, n;          // plane = pitch * ny (doubles per z-plane), n = nx*ny*nz (cells)
+    int nx, ny, nz, ne, hp, pitch;   // ne = even-x cells per row, hp = doubles per half row (>= ne + 1), pitch = 2 hp
+    long long plane, n;              // plane = pitch * ny (doubles per z-plane), n = nx*ny*nz (cells)
 };
 
 __host__ __device__ inline Geom make_geom(int nx, int ny, int nz)
 {
     Geom G;
-    G.nx = nx; G.ny = ny; G.nz = nz; G.ne = (nx + 1) / 2; G.pitch = nx + 2;
+    G.nx = nx; G.ny = ny; G.nz = nz; G.ne = (nx + 1) / 2; G.hp = (G.ne + 1 + 3) / 4 * 4; G.pitch = 2 * G.hp;
     G.plane = (long long)G.pitch * ny; G.n = (long long)nx * ny * nz;
     return G;
 }
 __host__ __device__ inline long long geom_alloc(const Geom& G) { return G.plane * G.nz; }
 __host__ __device__ __forceinline__ long long cell_at(const Geom& G, int i, int j, int k)
 {
-    return G.plane * k + (long long)G.pitch * j + (i & 1) * (G.ne + 1) + (i >> 1);
+    return G.plane * k + (long long)G.pitch * j + (i & 1) * G.hp + (i >> 1);
 }
 // natural cell number t = i + nx*(j + ny*k) -> (i, j, k).  32-bit arithmetic: vmg_create caps n below 2^31, and a
 // 64-bit division is ~100 dependent instructions, which the latency-bound coarse levels cannot hide.
@@ -403,8 +406,8 @@ __device__ __forceinline__ double nb_sum(const LevelView& L, const double* phi, 
 // cell and low-x neighbour of pair m, x-parity par, in the row starting at `row`
 __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, int par, long long& c, long long& xm)
 {
-    c = row + m + (par ? G.ne + 1 : 0);
-    xm = row + m + (par ? 0 : G.ne);
+    c = row + m + (par ? G.hp : 0);
+    xm = row + m + (par ? 0 : G.hp - 1);
 }
 
 // S2 (per-colour path). One colour half-sweep: phi_c <- (rhs_c + sum w phi_nb) / D_c for (i+j+k)%2 == colour.

@@ -730,7 +730,10 @@ def test_alternating_equation_kinds_on_one_handle_keeps_results():
     b = _binding()
     p = inputs.random_problem(40, 24, 16, seed=14, bc_type=[D, N, N, D, N, N])
     d = b.upload(p)
-    kinds = [("const", 1.0), ("general", 1.0), ("const", 1.0), ("const", 2.5), ("general", 0.5), ("const", 2.5), ("const", 1.0)]
+    # (const b1, general b2, const b2) with b1 != b2: the general call overwrites the levels' beta/h^2, which must not hide
+    # from the following constant-weight call that its captured graph still carries b1
+    kinds = [("const", 1.0), ("general", 1.0), ("const", 1.0), ("const", 2.5), ("general", 0.5), ("const", 2.5), ("const", 1.0),
+             ("general", 2.5), ("const", 2.5), ("general", 4.0), ("const", 4.0), ("const", 1.0)]
 
     def run(s, kind, beta, pcg):
         if kind == "const":
