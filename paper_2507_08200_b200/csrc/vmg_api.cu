@@ -130,6 +130,7 @@ int ready(vmg_s* h)
 {
     if (!h) return VMG_ERR_ARG;
     if (!h->have_coeffs || !h->have_bc) return VMG_ERR_STATE;
+    prepare_blocked(h);   // once per device, outside any stream capture (every solve / step entry point passes here)
     if (!h->l2_applied) { int rc = apply_l2_window(h); if (rc != VMG_OK) return rc; }
     if (h->dinv_dirty) return finalize_dinv(h);
     return VMG_OK;
@@ -399,7 +400,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "symmetric")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->symmetric = iv; }
     else if (!strcmp(key, "const_weights")) { h->const_weights = iv != 0; h->have_coeffs = false; }   // takes effect in vmg_set_coeffs
     else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
-    else if (!strcmp(key, "blocked")) { h->use_blocked = iv != 0; }
+    else if (!strcmp(key, "blocked")) { if (iv < 0 || iv > 2) return VMG_ERR_ARG; h->use_blocked = iv; }   // 1: vmg_block2.cuh, 2: vmg_block3.cuh (TMA)
     else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }
     else if (!strcmp(key, "snake")) { h->snake = iv != 0; }
     else if (!strcmp(key, "pdl")) { h->use_pdl = iv != 0; }

@@ -13,6 +13,7 @@
 // cell are always readable and every out-of-domain neighbour is multiplied by a zero weight:
 // the kernels carry no boundary branches (PAPER.md:230,266,284 boundary kinds live in the coefficients).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <vector>
@@ -23,6 +24,9 @@ enum { VMG_PC_SMOOTH0 = 0, VMG_PC_RESREST0 = 1, VMG_PC_PROLONG0 = 2, VMG_PC_COAR
        VMG_PC_FOLD = 5, VMG_PC_COPY = 6, VMG_PC_SETUP = 7, VMG_PC_COUNT = 8 };
 
 struct VmgProfEvent { int cls; long long launches; cudaEvent_t start, stop; };
+
+// a cached TMA descriptor of one level array for one box shape (vmg_sched.cuh level_map)
+struct VmgTensorMap { const double* base; int nxp, nyt; alignas(64) CUtensorMap map; };
 
 struct VmgLevel {
     int nx = 0, ny = 0, nz = 0;
@@ -45,6 +49,7 @@ struct VmgLevel {
     int cw = 0;                             // constant face weights (LevelView::cw: 0 arrays, 1 constant, 2 constant + mask)
     const unsigned char* mk = nullptr;      // cw == 2: the open faces of every cell, one byte, internal layout
     double* adiag = nullptr;  // masking: extra diagonal of this level, public layout (nullptr without a mask)
+    std::vector<VmgTensorMap> tmaps;   // TMA descriptors of this level's arrays (blocked smoother, vmg_block3.cuh)
 };
 
 struct vmg_s {

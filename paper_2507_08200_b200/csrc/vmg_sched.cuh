@@ -9,9 +9,11 @@
 #include "vmg_kernels.cuh"
 #include "vmg_tail.cuh"
 #include "vmg_block2.cuh"
+#include "vmg_block3.cuh"
 #include "../../include/vmg.h"
 #include <algorithm>
 #include <cstring>
+#include <mutex>
 
 namespace vmg {
 
@@ -323,15 +325,131 @@ inline void blk_run(vmg_s* h, const BlockArgs& g, int S, int tail, bool prolong,
 }
 #undef VMG_BLK_CASE
 
+// ------------------------------------------------------------------------------------------------
+// S2-S4, S6: blocked passes, third design (vmg_block3.cuh; option blocked = 2): TMA-fed ring, one split barrier per plane.
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point: the library does not link libcuda
+inline EncodeTiledFn tensor_map_encoder()
+{
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        (void)cudaGetLastError();
+    });
+    return fn;
+}
+
+// A level array (x-parity split rows, Geom) as the 5-D fp64 tensor (m, row pair, row parity, x-parity, plane); a box
+// {nxp, nyt/2, 2, 2, 1} lands in shared memory as [x-parity][row parity][row pair][m].  ny must be even.
+inline bool make_level_tensor_map(CUtensorMap* map, const Geom& G, const double* base, int nxp, int nyt)
+{
+    EncodeTiledFn enc = tensor_map_encoder();
+    if (!enc) return false;
+    const cuuint64_t dims[5] = {(cuuint64_t)G.hp, (cuuint64_t)(G.ny / 2), 2, 2, (cuuint64_t)G.nz};
+    const cuuint64_t strides[4] = {(cuuint64_t)2 * G.pitch * 8, (cuuint64_t)G.pitch * 8, (cuuint64_t)G.hp * 8, (cuuint64_t)G.plane * 8};
+    const cuuint32_t box[5] = {(cuuint32_t)nxp, (cuuint32_t)(nyt / 2), 2, 2, 1};
+    const cuuint32_t es[5] = {1, 1, 1, 1, 1};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// the level's tensor maps are encoded once per (array, box) and kept with the level
+inline bool level_map(VmgLevel& L, const double* base, int nxp, int nyt, CUtensorMap* out)
+{
+    for (auto& m : L.tmaps)
+        if (m.base == base && m.nxp == nxp && m.nyt == nyt) { *out = m.map; return true; }
+    VmgTensorMap m;
+    m.base = base; m.nxp = nxp; m.nyt = nyt;
+    if (!make_level_tensor_map(&m.map, L.G, base, nxp, nyt)) return false;
+    L.tmaps.push_back(m);
+    *out = m.map;
+    return true;
+}
+
+constexpr int kB3NXT = 40;
+constexpr int kB3PF = 1;
+constexpr int kB3MaxSmem = 232448;
+constexpr int kB3MaxThreads = 384;
+
+constexpr int b3_pick_nyt(int S, int T)
+{
+    int best = 0;
+    for (int nyt = 10; nyt <= 64; nyt += 2) {
+        const long long nph = (long long)(kB3NXT / 2) * (nyt / 2);
+        const int ns = S + T + 1 + kB3PF, np = S + T;
+        const long long smem = (long long)(3 * ns + 2 * np) * 4 * nph * 8 + (ns + 1) * 8 + 128;
+        if (nph <= kB3MaxThreads && smem <= kB3MaxSmem) best = nyt;
+    }
+    return best;
+}
+
+template <int S, int TAIL, bool PROLONG, int C0>
+struct B3Kernel {
+    static constexpr int NYT = b3_pick_nyt(S, TAIL ? 1 : 0);
+    using C = B3Cfg<S, TAIL, kB3NXT, NYT, kB3PF>;
+    static void prepare()
+    {
+        cudaFuncSetAttribute(smooth_block3_kernel<S, TAIL, PROLONG, C0, kB3NXT, NYT, kB3PF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)C::SMEM);
+    }
+    static bool launch(vmg_s* h, VmgLevel& L, Block3Args& g, const double* phi_in)
+    {
+        if (!level_map(L, phi_in, C::NXP, NYT, &g.tm_phi) || !level_map(L, L.wx, C::NXP, NYT, &g.tm_wx) ||
+            !level_map(L, L.wy, C::NXP, NYT, &g.tm_wy))
+            return false;
+        g.ntx = (int)cdiv(g.G.nx, C::TX); g.nty = (int)cdiv(g.G.ny, C::TY);
+        // z-segments per tile: minimise waves x (planes per CTA incl. the 2 ZH halo planes each segment pays)
+        const long long ntiles = (long long)g.ntx * g.nty;
+        int best = 1;
+        double best_cost = 1e300;
+        for (int ns = 1; ns <= std::max(1, g.G.nz / 4); ++ns) {
+            double waves = (double)cdiv(ntiles * ns, h->num_sms);
+            double cost = waves * ((double)cdiv(g.G.nz / 2, ns) * 2 + 2 * C::ZH + 2);
+            if (cost < best_cost) { best_cost = cost; best = ns; }
+        }
+        g.nzseg = best;
+        unsigned grid = (unsigned)(ntiles * g.nzseg);
+        smooth_block3_kernel<S, TAIL, PROLONG, C0, kB3NXT, NYT, kB3PF><<<grid, C::NT, C::SMEM, h->stream>>>(g);
+        return true;
+    }
+};
+
+#define VMG_B3_CASE(S_, T_, P_)                                                              \
+    if (prepare_all) { B3Kernel<S_, T_, P_, 0>::prepare(); B3Kernel<S_, T_, P_, 1>::prepare(); } \
+    else if (S == S_ && tail == T_ && prolong == P_)                                         \
+        return (g.colour0 & 1) ? B3Kernel<S_, T_, P_, 1>::launch(h, *L, g, phi_in) : B3Kernel<S_, T_, P_, 0>::launch(h, *L, g, phi_in);
+
+inline bool b3_run(vmg_s* h, VmgLevel* L, Block3Args& g, const double* phi_in, int S, int tail, bool prolong, bool prepare_all = false)
+{
+    VMG_B3_CASE(1, 0, false) VMG_B3_CASE(1, 0, true) VMG_B3_CASE(1, 1, false) VMG_B3_CASE(1, 1, true)
+    VMG_B3_CASE(1, 2, false) VMG_B3_CASE(1, 2, true)
+    VMG_B3_CASE(2, 0, false) VMG_B3_CASE(2, 0, true) VMG_B3_CASE(2, 1, false) VMG_B3_CASE(2, 1, true)
+    VMG_B3_CASE(2, 2, false) VMG_B3_CASE(2, 2, true)
+    VMG_B3_CASE(3, 0, false) VMG_B3_CASE(3, 0, true) VMG_B3_CASE(3, 1, false) VMG_B3_CASE(3, 1, true)
+    VMG_B3_CASE(3, 2, false) VMG_B3_CASE(3, 2, true)
+    return prepare_all;
+}
+#undef VMG_B3_CASE
+
 // once per process, outside any stream capture
 inline void prepare_blocked(vmg_s* h)
 {
-    static bool done = false;
-    if (done) return;
-    BlockArgs g{};
-    blk_run(h, g, 0, 0, false, true);
-    (void)cudaGetLastError();
-    done = true;
+    static std::once_flag once[64];   // per device: the attributes belong to the device's copy of the kernels
+    std::call_once(once[h->device & 63], [&] {
+        BlockArgs g{};
+        blk_run(h, g, 0, 0, false, true);
+        Block3Args g3{};
+        b3_run(h, nullptr, g3, nullptr, 0, 0, false, true);
+        (void)cudaGetLastError();
+    });
 }
 
 inline bool blocked_ok(const vmg_s* h, int l)
@@ -363,6 +481,12 @@ inline void blocked_sweeps(vmg_s* h, int l, int nhalf, int colour0, bool prolong
             if (T == BT_RESTRICT) { C.cur = 0; g.crhs = C.rhs; g.cphi = C.phi; }
         }
         g.norm_out = norm_out;
+        if (h->use_blocked == 2) {
+            Block3Args g3{};
+            g3.wz = L.wz; g3.dinv = L.dinv; g3.rhs = L.rhs; g3.phi_out = g.phi_out;
+            g3.G = g.G; g3.CG = g.CG; g3.colour0 = g.colour0; g3.e = g.e; g3.crhs = g.crhs; g3.cphi = g.cphi; g3.norm_out = norm_out;
+            if (!b3_run(h, &L, g3, g.phi_in, S, T, first && prolong)) h->last_cuda_error = (int)cudaErrorNotSupported;
+        } else
         blk_run(h, g, S, T, first && prolong);
         L.cur ^= 1;
         done += S;
