@@ -400,7 +400,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "symmetric")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->symmetric = iv; }
     else if (!strcmp(key, "const_weights")) { h->const_weights = iv != 0; h->have_coeffs = false; }   // takes effect in vmg_set_coeffs
     else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
-    else if (!strcmp(key, "blocked")) { if (iv < 0 || iv > 2) return VMG_ERR_ARG; h->use_blocked = iv; }   // 1: vmg_block2.cuh, 2: vmg_block3.cuh (TMA)
+    else if (!strcmp(key, "blocked")) { if (iv < 0 || iv > 3) return VMG_ERR_ARG; h->use_blocked = iv; }   // 1: vmg_block2.cuh, 2 / 3: vmg_block3.cuh (TMA; 2 x 2 patches / rows)
     else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }
     else if (!strcmp(key, "snake")) { h->snake = iv != 0; }
     else if (!strcmp(key, "pdl")) { h->use_pdl = iv != 0; }

@@ -110,8 +110,8 @@ __global__ void __launch_bounds__(B3Cfg<S, TAIL, NXT, NYT, PF>::NT, 1) smooth_bl
     constexpr int TSLOT = C::TSLOT, PSLOT = C::PSLOT;
     constexpr int A_PHI = 0, A_WX = ARR, A_WY = 2 * ARR, B_RHS = 0, B_DINV = ARR;
     constexpr int XB = 2 * NPH;                     // offset of the odd-x block inside an array
-    extern __shared__ unsigned char b3_raw[];
-    double* const ring = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(b3_raw) + 127) & ~(uintptr_t)127);
+    extern __shared__ __align__(128) double b3_smem[];   // (indexed as an array: the accesses must stay LDS / STS, not generic loads)
+    double* const ring = b3_smem;
     double* const priv = ring + NS * TSLOT;
     uint64_t* const full = reinterpret_cast<uint64_t*>(priv + NP * PSLOT);
     uint64_t* const stepbar = full + NS;
@@ -368,6 +368,304 @@ __global__ void __launch_bounds__(B3Cfg<S, TAIL, NXT, NYT, PF>::NT, 1) smooth_bl
         }
     }
 
+    if (TAIL == BT_NORM) {
+        if (nrm_nan) nrm = __longlong_as_double(0x7ff8000000000000ll);
+        block_max_to_global(nrm, g.norm_out);
+    }
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// Row variant: one thread per x-pair of ONE row (twice the threads of the 2 x 2 patch variant, half the registers each:
+// the ncu capture of the patch variant shows 11 warps per SM waiting on their own LDS -> DFMA chains, nothing saturated).
+// 9 LDS.64 + 1 STS.64 per relaxation instead of 8 + 1 (both y-neighbours come from shared memory).  The array is the 4-D
+// tensor (m, row, x-parity, plane), a box {NXP, NYT, 2, 1} lands as [x-parity][row][m]; the y halo is S + T rows, not
+// rounded up to even.  A thread calls its two cells by when they are relaxed, not by x-parity: cell L (0 / 1) is the one
+// relaxed in iterations of parity L, so every register index stays a compile-time constant although rows of both parities
+// share a warp; what depends on the row's parity are three shared-memory offsets per cell, computed once.
+// BT_RESTRICT: the two rows of a coarse cell belong to two threads; the odd row's x-pair sum goes through a small
+// shared-memory scratch and is consumed by the even row's thread one iteration later (after the step barrier), in the
+// order residual_restrict_kernel sums the children.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c3)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(0), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c3)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global [%0, {%1, %2, %3, %4}];"
+                 ::"l"(map), "r"(c0), "r"(c1), "r"(0), "r"(c3) : "memory");
+}
+
+template <int S, int TAIL, int NXT, int NYT, int PF>
+struct B3rCfg {
+    static constexpr int T = TAIL ? 1 : 0;
+    static constexpr int HX = 4, H = S + T;              // halo in x (tiles start on an x-pair, 32-byte aligned) and y
+    static constexpr int ZH = S + T;
+    static constexpr int TX = NXT - 2 * HX, TY = NYT - 2 * H;
+    static constexpr int NXP = NXT / 2, NPH = NXP * NYT; // x-pairs per row, x-pairs per plane (= live threads)
+    static constexpr int NT = (NPH + 31) / 32 * 32;
+    static constexpr int R = (S + T + 3) / 2 * 2;
+    static constexpr int NS = S + T + 1 + PF, NP = S + T;
+    static constexpr int ARR = 2 * NPH;                  // one array of one plane: [x-parity][NPH]
+    static constexpr int TSLOT = 3 * ARR, PSLOT = 2 * ARR;
+    static constexpr int SCRATCH = TAIL == BT_RESTRICT ? 2 * NPH : 0;
+    static constexpr size_t SMEM_DATA = (size_t)(NS * TSLOT + NP * PSLOT + SCRATCH) * sizeof(double);
+    static constexpr size_t SMEM = SMEM_DATA + 256;      // + front pad (mbarriers)
+    static constexpr uint32_t TX_BYTES = (uint32_t)(TSLOT * sizeof(double));
+    static_assert(S >= 1 && S + T <= 4 && TX > 0 && TY > 0 && TY % 2 == 0 && NXT % 4 == 0 && (ARR * 8) % 128 == 0 &&
+                      R >= S + 2 + T && R % 2 == 0 && PF >= 1, "tile");
+};
+
+template <int S, int TAIL, bool PROLONG, int C0, int NXT, int NYT, int PF>
+__global__ void __launch_bounds__(B3rCfg<S, TAIL, NXT, NYT, PF>::NT, 1) smooth_block3r_kernel(const __grid_constant__ Block3Args g)
+{
+    using C = B3rCfg<S, TAIL, NXT, NYT, PF>;
+    constexpr int NXP = C::NXP, NPH = C::NPH, R = C::R, NS = C::NS, NP = C::NP, ARR = C::ARR;
+    constexpr int TSLOT = C::TSLOT, PSLOT = C::PSLOT;
+    constexpr int A_PHI = 0, A_WX = ARR, A_WY = 2 * ARR, B_RHS = 0, B_DINV = ARR;
+    constexpr int XB = NPH;                         // offset of the odd-x block inside an array
+    extern __shared__ __align__(128) double b3_smem[];
+    // the first 256 bytes hold the mbarriers and keep the y-neighbour reads of the first row (rim: computed and
+    // discarded) inside the allocation
+    double* const ring = b3_smem + 32;
+    double* const priv = ring + NS * TSLOT;
+    double* const scratch = priv + NP * PSLOT;
+    uint64_t* const full = reinterpret_cast<uint64_t*>(b3_smem);
+    uint64_t* const stepbar = full + NS;
+    static_assert((NS + 1) * 8 + NXP * 8 <= 256, "front pad");
+
+    const bool live = threadIdx.x < NPH;
+    const int t = live ? threadIdx.x : 0;
+    const int m = t % NXP, j = t / NXP;
+    const int lane = threadIdx.x & 31;
+
+    for (int q = threadIdx.x; q < NS * TSLOT + NP * PSLOT + C::SCRATCH; q += C::NT) ring[q] = 0.0;
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < NS; ++k) mbar_init(full + k, 1);
+        mbar_init(stepbar, C::NT / 32);
+        fence_mbar_init();
+    }
+    fence_proxy_async();
+    __syncthreads();
+
+    const int ntiles = g.ntx * g.nty;
+    const int tile = (int)(blockIdx.x % ntiles), seg = (int)(blockIdx.x / ntiles);
+    const int za = (int)((long long)(g.G.nz / 2) * seg / g.nzseg) * 2;
+    const int zb = seg == g.nzseg - 1 ? g.G.nz : (int)((long long)(g.G.nz / 2) * (seg + 1) / g.nzseg) * 2;
+    const int tx = tile % g.ntx, ty = tile / g.ntx;
+    const int m0 = (tx * C::TX - C::HX) / 2, j0 = ty * C::TY - C::H;          // box origin: x-pair, row
+    const int gx = 2 * (m0 + m), gy = j0 + j;
+    const bool in_p = live && gx >= 0 && gx < g.G.nx && gy >= 0 && gy < g.G.ny;
+    const bool interior = in_p && m >= C::HX / 2 && m < C::HX / 2 + C::TX / 2 && j >= C::H && j < C::H + C::TY;
+    // cell L of this thread is relaxed in iterations n with n % 2 == L: its x-parity p0 ^ L, where
+    // p0 = (C0 + 1 + ZH + gy) & 1 (cell (x, y, z) has colour (x + y + z) & 1; stage s in iteration n relaxes colour
+    // C0 + s - 1 on plane z0 + n - s; za and gx are even)
+    const int p0 = (C0 + 1 + C::ZH + gy) & 1;
+    int oA[2], oX[2], oW[2];                        // per cell: itself, its x-neighbour outside the pair, its high-x weight
+    bool ok[2];                                     // rim cells (first / last row, first / last cell of a row) are never relaxed
+#pragma unroll
+    for (int L = 0; L < 2; ++L) {
+        const int sg = p0 ^ L;
+        oA[L] = sg * XB + t;
+        oX[L] = sg ? t + 1 : XB + t - 1;
+        oW[L] = sg ? t + 1 : XB + t;
+        ok[L] = live && j >= 1 && j <= NYT - 2 && (sg ? m < NXP - 1 : m > 0);
+    }
+    const long long cbase = (long long)g.G.pitch * gy + (gx >> 1);
+    const int odd = g.G.hp;
+
+    // register rings [cell L][slot]: phi and wz of this thread's pair; iteration n lives in slot n % R
+    double ph[2][R], wz[2][R];
+#pragma unroll
+    for (int L = 0; L < 2; ++L)
+#pragma unroll
+        for (int k = 0; k < R; ++k) ph[L][k] = wz[L][k] = 0.0;
+
+    double r_wz[2], r_rhs[2], r_dinv[2];            // [x-parity]
+    double r_e = 0.0;
+    auto issue_wz = [&](int zq) {
+        const bool z_in = in_p && zq >= 0 && zq < g.G.nz;
+        r_wz[0] = r_wz[1] = 0.0; r_e = 0.0;
+        if (z_in) {
+            const long long c = cbase + g.G.plane * zq;
+            r_wz[0] = __ldg(g.wz + c); r_wz[1] = __ldg(g.wz + c + odd);
+            if (PROLONG) r_e = __ldg(g.e + cell_at(g.CG, gx >> 1, gy >> 1, zq >> 1));
+        }
+    };
+    auto issue_rd = [&](int zq) {
+        const bool z_in = in_p && zq >= 0 && zq < g.G.nz;
+        r_rhs[0] = r_rhs[1] = r_dinv[0] = r_dinv[1] = 0.0;
+        if (z_in) {
+            const long long c = cbase + g.G.plane * zq;
+            r_rhs[0] = __ldg(g.rhs + c); r_rhs[1] = __ldg(g.rhs + c + odd);
+            r_dinv[0] = __ldg(g.dinv + c); r_dinv[1] = __ldg(g.dinv + c + odd);
+        }
+    };
+    auto tma_plane = [&](int slot, int z) {
+        double* dst = ring + slot * TSLOT;
+        mbar_expect_tx(full + slot, C::TX_BYTES);
+        tma_load_4d(dst + A_PHI, &g.tm_phi, full + slot, m0, j0, z);
+        tma_load_4d(dst + A_WX, &g.tm_wx, full + slot, m0, j0, z);
+        tma_load_4d(dst + A_WY, &g.tm_wy, full + slot, m0, j0, z);
+    };
+
+    const int z0 = za - C::ZH;
+    const int niter = (zb - za) + 2 * C::ZH;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 0; q < PF; ++q)
+            if (q < niter) tma_plane(q, z0 + q);
+    }
+    issue_wz(z0);
+
+    double nrm = 0.0;
+    bool nrm_nan = false;
+    double acc = 0.0, rsum_prev = 0.0;             // BT_RESTRICT (even rows): running sum of a coarse cell, this row's last x-pair sum
+    int slotn = 0, phasen = 0, pn = 0;
+
+    // BT_RESTRICT: the children of plane pr (tail of the previous iteration): even row (this thread), then odd row (scratch)
+    auto consume_restrict = [&](int pr, int par) {
+        if (pr >= za && pr < zb && interior && !(gy & 1)) {
+            acc += rsum_prev;
+            acc += scratch[par * NPH + t + NXP];
+            if (pr & 1) {
+                const long long cc = cell_at(g.CG, gx >> 1, gy >> 1, pr >> 1);
+                g.crhs[cc] = acc / 8.0;
+                g.cphi[cc] = 0.0;
+                acc = 0.0;
+            }
+        }
+    };
+
+    for (int nbase = 0; nbase < niter; nbase += R) {
+#pragma unroll
+        for (int u = 0; u < R; ++u) {
+            const int n = nbase + u;
+            if (n >= niter) break;
+            const int zl = z0 + n;
+
+            // ---- A: plane zl has landed: its own cells enter the register rings ----
+            mbar_wait(full + slotn, (uint32_t)phasen);
+            {
+                double* P0 = ring + slotn * TSLOT;
+#pragma unroll
+                for (int L = 0; L < 2; ++L) {
+                    double a = P0[A_PHI + oA[L]];
+                    if (PROLONG) { a += r_e; if (live) P0[A_PHI + oA[L]] = a; }
+                    ph[L][u] = a;
+                    wz[L][u] = (p0 ^ L) ? r_wz[1] : r_wz[0];
+                }
+            }
+            issue_wz(zl + 1);
+            issue_rd(zl);
+
+            // ---- B: every thread has finished iteration n-1 ----
+            if (n > 0) mbar_wait(stepbar, (uint32_t)((n - 1) & 1));
+            if (threadIdx.x == 0) {
+                if (n + PF < niter) {
+                    int sl = slotn + PF; if (sl >= NS) sl -= NS;
+                    tma_plane(sl, zl + PF);
+                }
+                if (n + PF + 2 < niter && zl + PF + 2 < g.G.nz) {
+                    tma_prefetch_4d(&g.tm_phi, m0, j0, zl + PF + 2);
+                    tma_prefetch_4d(&g.tm_wx, m0, j0, zl + PF + 2);
+                    tma_prefetch_4d(&g.tm_wy, m0, j0, zl + PF + 2);
+                }
+            }
+            if (TAIL == BT_RESTRICT) consume_restrict(zl - 1 - S - 1, (n - 1) & 1);
+
+            // ---- C: stage s relaxes cell L = u & 1 of plane zl - s (register slot (u-s) % R) ----
+            const int L = u & 1;
+#pragma unroll
+            for (int s = 1; s <= S; ++s) {
+                const int c = ((u - s) % R + R) % R, cu = ((u - s + 1) % R + R) % R, cd = ((u - s - 1) % R + R) % R;
+                int sl = slotn - s; if (sl < 0) sl += NS;
+                int ps = pn - s; if (ps < 0) ps += NP;
+                double* P = ring + sl * TSLOT;
+                const double* Q = priv + ps * PSLOT;
+                const double mate = ph[1 - L][c], xo = P[A_PHI + oX[L]];
+                const bool sg = (p0 ^ L) != 0;
+                const double xm = sg ? mate : xo, xp = sg ? xo : mate;
+                double v = P[A_WX + oA[L]] * xm;
+                v = fma(P[A_WX + oW[L]], xp, v);
+                v = fma(P[A_WY + oA[L]], P[A_PHI + oA[L] - NXP], v);
+                v = fma(P[A_WY + oA[L] + NXP], P[A_PHI + oA[L] + NXP], v);
+                v = fma(wz[L][c], ph[L][cd], v);
+                v = fma(wz[L][cu], ph[L][cu], v);
+                const double nv = Q[B_DINV + oA[L]] * (Q[B_RHS + oA[L]] + v);
+                if (ok[L]) { ph[L][c] = nv; P[A_PHI + oA[L]] = nv; }
+            }
+
+            // ---- residual stage on plane zl - S - 1 (all its neighbours are final) ----
+            if (TAIL != BT_NONE) {
+                const int pr = zl - S - 1;
+                if (pr >= za && pr < zb && interior) {
+                    const int k = ((u - S - 1) % R + R) % R, ku = ((u - S) % R + R) % R, kd = ((u - S - 2) % R + R) % R;
+                    int sl = slotn - (S + 1); if (sl < 0) sl += NS;
+                    int ps = pn - (S + 1); if (ps < 0) ps += NP;
+                    const double* P = ring + sl * TSLOT;
+                    const double* Q = priv + ps * PSLOT;
+                    double res[2];                       // [cell L]
+#pragma unroll
+                    for (int LL = 0; LL < 2; ++LL) {
+                        const double ce = ph[LL][k], mate = ph[1 - LL][k], xo = P[A_PHI + oX[LL]];
+                        const bool sg = (p0 ^ LL) != 0;
+                        const double xm = sg ? mate : xo, xp = sg ? xo : mate;
+                        double v = P[A_WX + oA[LL]] * xm;
+                        v = fma(P[A_WX + oW[LL]], xp, v);
+                        v = fma(P[A_WY + oA[LL]], P[A_PHI + oA[LL] - NXP], v);
+                        v = fma(P[A_WY + oA[LL] + NXP], P[A_PHI + oA[LL] + NXP], v);
+                        v = fma(wz[LL][k], ph[LL][kd], v);
+                        v = fma(wz[LL][ku], ph[LL][ku], v);
+                        res[LL] = Q[B_RHS + oA[LL]] + v - ce / Q[B_DINV + oA[LL]];
+                    }
+                    if (TAIL == BT_NORM) {
+#pragma unroll
+                        for (int LL = 0; LL < 2; ++LL) {
+                            const double a = fabs(res[LL]);
+                            nrm_nan |= (a != a);
+                            nrm = fmax(nrm, a);
+                        }
+                    }
+                    if (TAIL == BT_RESTRICT) {
+                        const double rs = p0 ? res[1] + res[0] : res[0] + res[1];   // even-x child first
+                        if (gy & 1) scratch[(n & 1) * NPH + t] = rs; else rsum_prev = rs;
+                    }
+                }
+            }
+
+            // ---- D: this thread's shared-memory writes of iteration n are done ----
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(stepbar);
+
+            // ---- E: plane zl - S is final: write it back from registers ----
+            {
+                const int p = zl - S, c = ((u - S) % R + R) % R;
+                if (p >= za && p < zb && interior) {
+                    double* q = g.phi_out + cbase + g.G.plane * p;
+                    q[0] = p0 ? ph[1][c] : ph[0][c];
+                    q[odd] = p0 ? ph[0][c] : ph[1][c];
+                }
+            }
+            // ---- F: rhs and 1/D of plane zl take the private slot that plane zl - S - T just vacated ----
+            if (live) {
+                double* F = priv + pn * PSLOT + t;
+                F[B_RHS] = r_rhs[0];   F[B_RHS + XB] = r_rhs[1];
+                F[B_DINV] = r_dinv[0]; F[B_DINV + XB] = r_dinv[1];
+            }
+            if (++slotn == NS) { slotn = 0; phasen ^= 1; }
+            if (++pn == NP) pn = 0;
+        }
+    }
+
+    if (TAIL == BT_RESTRICT) {                       // the last plane's children
+        mbar_wait(stepbar, (uint32_t)((niter - 1) & 1));
+        consume_restrict(z0 + niter - 1 - S - 1, (niter - 1) & 1);
+    }
     if (TAIL == BT_NORM) {
         if (nrm_nan) nrm = __longlong_as_double(0x7ff8000000000000ll);
         block_max_to_global(nrm, g.norm_out);

@@ -26,7 +26,7 @@ enum { VMG_PC_SMOOTH0 = 0, VMG_PC_RESREST0 = 1, VMG_PC_PROLONG0 = 2, VMG_PC_COAR
 struct VmgProfEvent { int cls; long long launches; cudaEvent_t start, stop; };
 
 // a cached TMA descriptor of one level array for one box shape (vmg_sched.cuh level_map)
-struct VmgTensorMap { const double* base; int nxp, nyt; alignas(64) CUtensorMap map; };
+struct VmgTensorMap { const double* base; int nxp, nyt, rank; alignas(64) CUtensorMap map; };
 
 struct VmgLevel {
     int nx = 0, ny = 0, nz = 0;

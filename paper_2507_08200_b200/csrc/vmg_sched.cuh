@@ -361,14 +361,27 @@ inline bool make_level_tensor_map(CUtensorMap* map, const Geom& G, const double*
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// the same array as the 4-D tensor (m, row, x-parity, plane): a box {nxp, nyt, 2, 1} lands as [x-parity][row][m] (row variant)
+inline bool make_level_tensor_map4(CUtensorMap* map, const Geom& G, const double* base, int nxp, int nyt)
+{
+    EncodeTiledFn enc = tensor_map_encoder();
+    if (!enc) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)G.hp, (cuuint64_t)G.ny, 2, (cuuint64_t)G.nz};
+    const cuuint64_t strides[3] = {(cuuint64_t)G.pitch * 8, (cuuint64_t)G.hp * 8, (cuuint64_t)G.plane * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)nxp, (cuuint32_t)nyt, 2, 1};
+    const cuuint32_t es[4] = {1, 1, 1, 1};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // the level's tensor maps are encoded once per (array, box) and kept with the level
-inline bool level_map(VmgLevel& L, const double* base, int nxp, int nyt, CUtensorMap* out)
+inline bool level_map(VmgLevel& L, const double* base, int nxp, int nyt, CUtensorMap* out, int rank = 5)
 {
     for (auto& m : L.tmaps)
-        if (m.base == base && m.nxp == nxp && m.nyt == nyt) { *out = m.map; return true; }
+        if (m.base == base && m.nxp == nxp && m.nyt == nyt && m.rank == rank) { *out = m.map; return true; }
     VmgTensorMap m;
-    m.base = base; m.nxp = nxp; m.nyt = nyt;
-    if (!make_level_tensor_map(&m.map, L.G, base, nxp, nyt)) return false;
+    m.base = base; m.nxp = nxp; m.nyt = nyt; m.rank = rank;
+    if (!(rank == 5 ? make_level_tensor_map(&m.map, L.G, base, nxp, nyt) : make_level_tensor_map4(&m.map, L.G, base, nxp, nyt))) return false;
     L.tmaps.push_back(m);
     *out = m.map;
     return true;
@@ -439,6 +452,68 @@ inline bool b3_run(vmg_s* h, VmgLevel* L, Block3Args& g, const double* phi_in, i
 }
 #undef VMG_B3_CASE
 
+// row variant (option blocked = 3): one thread per x-pair of one row, up to 704 threads
+constexpr int kB3rMaxThreads = 704;
+constexpr int b3r_pick_nyt(int S, int TAIL)
+{
+    const int T = TAIL ? 1 : 0;
+    int best = 0;
+    for (int nyt = 2 * (S + T) + 2; nyt <= 64; nyt += 2) {
+        const long long nph = (long long)(kB3NXT / 2) * nyt;
+        const int ns = S + T + 1 + kB3PF, np = S + T;
+        const long long smem = ((long long)(3 * ns + 2 * np) * 2 * nph + (TAIL == BT_RESTRICT ? 2 * nph : 0)) * 8 + 256;
+        if (nph <= kB3rMaxThreads && smem <= kB3MaxSmem) best = nyt;
+    }
+    return best;
+}
+
+template <int S, int TAIL, bool PROLONG, int C0>
+struct B3rKernel {
+    static constexpr int NYT = b3r_pick_nyt(S, TAIL);
+    using C = B3rCfg<S, TAIL, kB3NXT, NYT, kB3PF>;
+    static void prepare()
+    {
+        cudaFuncSetAttribute(smooth_block3r_kernel<S, TAIL, PROLONG, C0, kB3NXT, NYT, kB3PF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)C::SMEM);
+    }
+    static bool launch(vmg_s* h, VmgLevel& L, Block3Args& g, const double* phi_in)
+    {
+        if (!level_map(L, phi_in, C::NXP, NYT, &g.tm_phi, 4) || !level_map(L, L.wx, C::NXP, NYT, &g.tm_wx, 4) ||
+            !level_map(L, L.wy, C::NXP, NYT, &g.tm_wy, 4))
+            return false;
+        g.ntx = (int)cdiv(g.G.nx, C::TX); g.nty = (int)cdiv(g.G.ny, C::TY);
+        const long long ntiles = (long long)g.ntx * g.nty;
+        int best = 1;
+        double best_cost = 1e300;
+        for (int ns = 1; ns <= std::max(1, g.G.nz / 4); ++ns) {
+            double waves = (double)cdiv(ntiles * ns, h->num_sms);
+            double cost = waves * ((double)cdiv(g.G.nz / 2, ns) * 2 + 2 * C::ZH + 2);
+            if (cost < best_cost) { best_cost = cost; best = ns; }
+        }
+        g.nzseg = best;
+        unsigned grid = (unsigned)(ntiles * g.nzseg);
+        smooth_block3r_kernel<S, TAIL, PROLONG, C0, kB3NXT, NYT, kB3PF><<<grid, C::NT, C::SMEM, h->stream>>>(g);
+        return true;
+    }
+};
+
+#define VMG_B3R_CASE(S_, T_, P_)                                                             \
+    if (prepare_all) { B3rKernel<S_, T_, P_, 0>::prepare(); B3rKernel<S_, T_, P_, 1>::prepare(); } \
+    else if (S == S_ && tail == T_ && prolong == P_)                                         \
+        return (g.colour0 & 1) ? B3rKernel<S_, T_, P_, 1>::launch(h, *L, g, phi_in) : B3rKernel<S_, T_, P_, 0>::launch(h, *L, g, phi_in);
+
+inline bool b3r_run(vmg_s* h, VmgLevel* L, Block3Args& g, const double* phi_in, int S, int tail, bool prolong, bool prepare_all = false)
+{
+    VMG_B3R_CASE(1, 0, false) VMG_B3R_CASE(1, 0, true) VMG_B3R_CASE(1, 1, false) VMG_B3R_CASE(1, 1, true)
+    VMG_B3R_CASE(1, 2, false) VMG_B3R_CASE(1, 2, true)
+    VMG_B3R_CASE(2, 0, false) VMG_B3R_CASE(2, 0, true) VMG_B3R_CASE(2, 1, false) VMG_B3R_CASE(2, 1, true)
+    VMG_B3R_CASE(2, 2, false) VMG_B3R_CASE(2, 2, true)
+    VMG_B3R_CASE(3, 0, false) VMG_B3R_CASE(3, 0, true) VMG_B3R_CASE(3, 1, false) VMG_B3R_CASE(3, 1, true)
+    VMG_B3R_CASE(3, 2, false) VMG_B3R_CASE(3, 2, true)
+    return prepare_all;
+}
+#undef VMG_B3R_CASE
+
 // once per process, outside any stream capture
 inline void prepare_blocked(vmg_s* h)
 {
@@ -448,6 +523,7 @@ inline void prepare_blocked(vmg_s* h)
         blk_run(h, g, 0, 0, false, true);
         Block3Args g3{};
         b3_run(h, nullptr, g3, nullptr, 0, 0, false, true);
+        b3r_run(h, nullptr, g3, nullptr, 0, 0, false, true);
         (void)cudaGetLastError();
     });
 }
@@ -481,11 +557,13 @@ inline void blocked_sweeps(vmg_s* h, int l, int nhalf, int colour0, bool prolong
             if (T == BT_RESTRICT) { C.cur = 0; g.crhs = C.rhs; g.cphi = C.phi; }
         }
         g.norm_out = norm_out;
-        if (h->use_blocked == 2) {
+        if (h->use_blocked >= 2) {
             Block3Args g3{};
             g3.wz = L.wz; g3.dinv = L.dinv; g3.rhs = L.rhs; g3.phi_out = g.phi_out;
             g3.G = g.G; g3.CG = g.CG; g3.colour0 = g.colour0; g3.e = g.e; g3.crhs = g.crhs; g3.cphi = g.cphi; g3.norm_out = norm_out;
-            if (!b3_run(h, &L, g3, g.phi_in, S, T, first && prolong)) h->last_cuda_error = (int)cudaErrorNotSupported;
+            const bool okl = h->use_blocked == 3 ? b3r_run(h, &L, g3, g.phi_in, S, T, first && prolong)
+                                                 : b3_run(h, &L, g3, g.phi_in, S, T, first && prolong);
+            if (!okl) h->last_cuda_error = (int)cudaErrorNotSupported;
         } else
         blk_run(h, g, S, T, first && prolong);
         L.cur ^= 1;

@@ -98,6 +98,7 @@ def test_schedule_options_do_not_change_a_single_bit():
     p = inputs.config4(32)
     ref = None
     for opts in (dict(snake=0, l2_persist=0, graph=0, tail=0), dict(), dict(snake=1, graph=0), dict(tail=0), dict(blocked=1),
+                 dict(blocked=2), dict(blocked=3, block_min_cells=0),
                  dict(phi_keep_cells=0), dict(phi_keep_cells=0, graph=0, tail=0)):   # cache policy of the largest levels on all levels
         s, d = b.from_problem(p)
         for k, v in opts.items():
@@ -130,7 +131,7 @@ def test_blocked_passes_equal_plain_launches_bitwise(dims):
         phi, rhs = dev(rng.standard_normal((nz, ny, nx))), dev(rng.standard_normal((nz, ny, nx)) * 50.0)
         e = dev(rng.standard_normal((cnz, cny, cnx)))
         out = {}
-        for blocked in (1, 0):
+        for blocked in (1, 2, 3, 0):   # vmg_block2.cuh; vmg_block3.cuh (TMA-fed): 2 x 2 patches, rows; per-colour launches
             s.set_option("blocked", blocked)
             res = [s.step_smooth(lev, phi, rhs, ns) for ns in (1, 2, 3, 4)]
             for nu in (1, 2, 3):
@@ -138,8 +139,9 @@ def test_blocked_passes_equal_plain_launches_bitwise(dims):
                 s.set_option("nu2", nu)
                 res += list(s.step_down(lev, phi, rhs)) + [s.step_up(lev, phi, rhs, e)]
             out[blocked] = res
-        for x, y in zip(out[1], out[0]):
-            assert torch.equal(x, y), (lev, (x - y).abs().max().item())
+        for blocked in (1, 2, 3):
+            for x, y in zip(out[blocked], out[0]):
+                assert torch.equal(x, y), (blocked, lev, (x - y).abs().max().item())
     s.destroy()
 
 
