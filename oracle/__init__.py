@@ -53,6 +53,7 @@ def lib():
         _lib.ovmg_num_levels.argtypes = [C.c_void_p]
         _lib.ovmg_level_dims.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int)]
         _lib.ovmg_get_level_coeffs.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, _dp]
+        _lib.ovmg_get_level_adiag.argtypes = [C.c_void_p, C.c_int, _dp]
         _lib.ovmg_apply.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
         _lib.ovmg_fold_bc.argtypes = [C.c_void_p, _dp, _dp]
         _lib.ovmg_smooth.argtypes = [C.c_void_p, C.c_int, _dp, _dp, C.c_int]
@@ -168,6 +169,12 @@ class Oracle:
         by, bz = np.zeros((nz, ny + 1, nx)), np.zeros((nz + 1, ny, nx))
         self._chk(lib().ovmg_get_level_coeffs(self._h, lev, _p(a), _p(bx), _p(by), _p(bz)), "level_coeffs")
         return a, bx, by, bz
+
+    def level_adiag(self, lev: int):
+        """Masking: the extra diagonal of a level (reading N4)."""
+        out = self._zeros(lev)
+        self._chk(lib().ovmg_get_level_adiag(self._h, lev, _p(out)), "level_adiag")
+        return out
 
     def apply(self, phi, lev: int = 0):
         phi = _c(phi)

@@ -723,6 +723,18 @@ int ovmg_get_level_coeffs(const ovmg *h, int lev, double *a, double *bx, double 
     return O_OK;
 }
 
+/* masking: the extra diagonal of level `lev` (reading N4: Dirichlet interface terms of valid cells, 1 in covered cells on
+ * level 0; averaged like a on the coarse levels).  Accessor only, for the pins of the coarse average. */
+int ovmg_get_level_adiag(const ovmg *h, int lev, double *adiag)
+{
+    const olevel *L;
+    if (!h || lev < 0 || lev >= h->nlev || !adiag) return O_ERR_ARG;
+    L = &h->lev[lev];
+    if (!L->adiag) return O_ERR_ARG;
+    memcpy(adiag, L->adiag, ncell(L) * sizeof(double));
+    return O_OK;
+}
+
 int ovmg_apply(const ovmg *h, int lev, const double *phi, double *out)
 {
     if (!h || lev < 0 || lev >= h->nlev || !h->have_coeffs || !h->have_bc) return O_ERR_ARG;

@@ -476,6 +476,53 @@ def test_n4_masked_operator_and_solution_match_facewise_assembly(kind):
     o.close()
 
 
+@pytest.mark.parametrize("kind", [D, N], ids=["dirichlet_interfaces", "zero_flux_interfaces"])
+def test_n4_coarse_levels_of_a_masked_hierarchy(kind):
+    """Reading N4, coarse levels: the effective coefficients a_eff, b_eff are averaged as R10 and the extra diagonal like a.
+    Level-1 adiag = mean of the 8 children of the level-0 adiag written here from the mask and b; and the level-1
+    operator is the ordinary face-wise operator of the averaged coefficients plus that diagonal -- a wrong coarse average
+    (a dropped child, a wrong factor) fails one of the two."""
+    import dataclasses
+    p = inputs.random_problem(16, 8, 8, seed=15, bc_type=[D, N, N, D, N, N])
+    mask = np.ones(p.rhs.shape, dtype=np.uint8)
+    mask[2:5, 3:6, 5:11] = 0                    # a covered block that cuts through coarse cells (odd offsets)
+    mask[0, 0, :3] = 0
+    o = Oracle.from_problem(p)
+    o.set_mask(mask, kind, None)
+    o.set_coeffs(p.a, p.bx, p.by, p.bz, p.alpha, p.beta)
+    nz, ny, nx = p.rhs.shape
+    m = mask.astype(bool)
+    # level-0 extra diagonal from its definition: 2 beta b / h^2 per face to a covered neighbour (Dirichlet kind), 1 if covered
+    ad0 = np.zeros(p.rhs.shape)
+    h = (p.dx, p.dy, p.dz)
+    for k in range(nz):
+        for j in range(ny):
+            for i in range(nx):
+                if not m[k, j, i]:
+                    ad0[k, j, i] = 1.0
+                    continue
+                if kind != D:
+                    continue
+                for d, (di, dj, dk) in enumerate(((1, 0, 0), (0, 1, 0), (0, 0, 1))):
+                    for side in (0, 1):
+                        ii, jj, kk = i + (2 * side - 1) * di, j + (2 * side - 1) * dj, k + (2 * side - 1) * dk
+                        if 0 <= ii < nx and 0 <= jj < ny and 0 <= kk < nz and not m[kk, jj, ii]:
+                            b = (p.bx, p.by, p.bz)[d][k + side * dk, j + side * dj, i + side * di]
+                            ad0[k, j, i] += 2.0 * p.beta * b / h[d] ** 2
+    assert np.abs(o.level_adiag(0) - ad0).max() <= 1e-13 * np.abs(ad0).max()
+    ad1 = ad0.reshape(nz // 2, 2, ny // 2, 2, nx // 2, 2).mean(axis=(1, 3, 5))
+    assert np.abs(o.level_adiag(1) - ad1).max() <= 1e-13 * np.abs(ad1).max()
+    # level-1 operator = face-wise operator of the level's averaged coefficients (h doubled) + diag(adiag)
+    a1, bx1, by1, bz1 = o.level_coeffs(1)
+    p1 = dataclasses.replace(p, nx=nx // 2, ny=ny // 2, nz=nz // 2, dx=2 * p.dx, dy=2 * p.dy, dz=2 * p.dz, a=a1, bx=bx1, by=by1, bz=bz1)
+    A1 = brute_force_matrix(p1) + np.diag(o.level_adiag(1).ravel())
+    assert np.abs(dense_from_apply(o, 1) - A1).max() <= 1e-12 * np.abs(A1).max()
+    # the averaged effective coefficients themselves: a_eff = a in valid cells, 0 in covered ones
+    a_eff = np.where(m, p.a, 0.0)
+    assert np.abs(a1 - a_eff.reshape(nz // 2, 2, ny // 2, 2, nx // 2, 2).mean(axis=(1, 3, 5))).max() <= 1e-13 * np.abs(a_eff).max()
+    o.close()
+
+
 def test_n4_electrode_block_obeys_the_maximum_principle():
     """A covered block at potential 1 inside a grounded box (Laplace, no source): 0 <= phi <= 1 in every valid cell, phi
     decays away from the block, and the solution has the block's mirror symmetry."""
