@@ -54,8 +54,12 @@ enum {
 
 /* Create a solver for an nx x ny x nz box with cell sizes dx, dy, dz.  The level hierarchy halves every
  * active dimension while all stay even and >= 2 afterwards (256x128x128 -> ... -> 4x2x2); the coarsest grid
- * must have <= 512 cells (VMG_ERR_SIZE otherwise).  cuda_stream is a cudaStream_t (NULL = legacy default
- * stream); every kernel, copy and graph of this handle is enqueued on it.  All device memory the handle
+ * must have <= 512 cells (VMG_ERR_SIZE otherwise).  cuda_stream is a cudaStream_t; every kernel, copy and graph of this handle is
+ * enqueued on it.  NULL: the handle creates a blocking stream of its own (ordered with the legacy default stream, not with
+ * non-blocking or per-thread default streams: a caller that produces its inputs there must synchronise first) and
+ * vmg_set_coeffs / vmg_set_bc synchronise it before they return.  With a caller-supplied stream those two calls only
+ * ENQUEUE: the arrays passed to them must stay valid and unmodified until the stream has passed that point (stream-ordered
+ * allocators such as torch's guarantee this for work on the same stream; vmg_solve synchronises the stream anyway).  All device memory the handle
  * needs (about 9.3 fp64 arrays of (nx+2)*ny*nz) is allocated here; vmg_solve allocates nothing on the device. */
 int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream);
 
@@ -66,18 +70,20 @@ int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, do
  * half-sweep -- the Poisson equation PAPER.md:54 Eq. 3 and Helmholtz equations with a variable a; with a mask set
  * this holds for level 0, whose kernels then read one byte of open-face flags per cell, the averaged coarser levels
  * keep their arrays).  a must be >= 0 with alpha >= 0 and b > 0, beta > 0 (not checked; otherwise undefined behaviour).
- * The arrays are read during this call only (enqueued on the stream, then synchronised): the library
+ * The arrays are read by the kernels this call enqueues (see vmg_create for when they may be reused): the library
  * averages them to all coarse levels (a: mean of the 8 children, 4 in 2-D; b: mean of the fine faces lying
- * on the coarse face) and converts each level to its internal stencil form.  The caller may free or modify
- * them afterwards; call again when coefficients change. */
+ * on the coarse face) and converts each level to its internal stencil form.  They are not referenced after
+ * that; call again when coefficients change.  Passage: the Helmholtz form every governing equation is cast into,
+ * PAPER.md:159 (section 4); Poisson PAPER.md:54 (Eq. 3), implicit diffusion PAPER.md:129-134 (Eq. 17). */
 int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double* by, const double* bz,
                    double alpha, double beta);
 
 /* Boundary conditions.  type: HOST array of 6 entries (VMG_BC_DIRICHLET / VMG_BC_NEUMANN), order XLO..ZHI.
  * value: HOST array of 6 DEVICE pointers to value planes, or NULL; a NULL entry (or value == NULL) means
  * homogeneous.  Dirichlet value = phi on the face; Neumann value = outward-normal derivative d(phi)/dn on
- * the face (not the flux b*d(phi)/dn).  The planes are copied.  May be called before or after
- * vmg_set_coeffs, and again at any time. */
+ * the face (not the flux b*d(phi)/dn).  The planes are copied (enqueued, see vmg_create).  May be called before
+ * or after vmg_set_coeffs, and again at any time.  Passage: fixed-potential electrodes and homogeneous Neumann walls,
+ * PAPER.md:230, :266, :284; readings R3-R6 of DESIGN.md section 2 for the discrete form. */
 int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6]);
 
 /* Cell masking ("cell masking for complex geometries").  mask: DEVICE array of
@@ -95,7 +101,8 @@ int vmg_set_mask(vmg_handle h, const unsigned char* mask, int kind, const double
  * Iterates V(nu1,nu2) cycles until ||btilde - A phi||_inf <= rtol * ||btilde||_inf, where btilde is f with
  * the boundary data folded in, or until max_vcycles cycles (rtol <= 0: run exactly max_vcycles cycles).
  * Returns VMG_OK / VMG_MAXCYCLES / VMG_STALLED or a negative error.  Synchronises the stream before
- * returning. */
+ * returning.  Passage: "The composite multilevel multigrid solver ... is used for each of the governing equations"
+ * PAPER.md:159; cycle, smoother, transfers and exit rules are readings C1-C5 / R7-R13 of DESIGN.md section 2. */
 int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max_vcycles);
 
 /* Batched solve (the paper's "multi-component" optimisation: "simultaneously solving multiple scalar solution
@@ -134,15 +141,17 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  * "snake" (1: consecutive whole-level kernels walk the level in opposite z-directions so that each starts on
  *   what the previous one left in L2, default; 0: always ascending),
  * "l2_persist" (MB of L2 set aside for the level-0 face weights through a stream access-policy window,
- *   default 24, 0 = none; applied only when those weights exceed half the L2.  NOTE: this calls
- *   cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize), a setting of the whole CUDA context),
+ *   default 24, 0 = none; applied only when those weights exceed half the L2.  NOTE: this raises
+ *   cudaLimitPersistingL2CacheSize, a setting of the whole CUDA context, and sets the window on the handle's stream;
+ *   vmg_destroy clears the window and puts the limit back to what it was when this handle first changed it),
  * "phi_keep_cells" (levels with at least this many cells read phi in a colour half-sweep (the neighbours) and in the residual norm with the normal
  *   cache policy instead of the streaming one, default 33554432: on a level whose phi is more than twice the L2 the
  *   evict-first lines are gone before the next row and plane ask for them; results do not depend on it),
  * "pdl" (1: the V-cycle kernels are launched with programmatic stream serialisation, so each kernel's launch overlaps
  *   the tail of its predecessor, default; 0: plain serialisation),
- * "blocked" (1: temporally blocked smoother passes with fused transfers (vmg_block2.cuh); 0: one kernel per
- *   colour half-sweep, default -- the blocked passes are bitwise equal but measure slower on B200),
+ * "blocked" (temporally blocked smoother passes with fused transfers: 1 = register-staged (vmg_block2.cuh), 2 = TMA-fed
+ *   ring with one split mbarrier per plane, 2 x 2 patch per thread, 3 = the same with one row per thread (vmg_block3.cuh);
+ *   0: one kernel per colour half-sweep, default -- the blocked passes are bitwise equal but measure slower on B200),
  * "block_min_cells" (smallest level the blocked passes are used on when blocked = 1, default 4096),
  * "const_weights" (1: use the constant-weight kernels when b == NULL, default; 0: always load the weight arrays; takes
  *   effect at the next vmg_set_coeffs, which must follow),

@@ -110,7 +110,14 @@ int apply_l2_window(vmg_s* h)
     if (bytes < (size_t)prop.l2CacheSize / 2) want = 0;
     if (want > cap) want = cap;
     if (want == 0 && !h->l2_window_set) return VMG_OK;
-    if (want) CUDA_TRY(h, cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));
+    if (want) {
+        if (!h->l2_limit_saved) {   // put back by vmg_destroy
+            size_t prev = 0;
+            if (cudaDeviceGetLimit(&prev, cudaLimitPersistingL2CacheSize) == cudaSuccess) { h->l2_limit_prev = prev; h->l2_limit_saved = true; }
+            (void)cudaGetLastError();
+        }
+        CUDA_TRY(h, cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));
+    }
     cudaStreamAttrValue a;
     memset(&a, 0, sizeof(a));
     if (bytes > (size_t)prop.accessPolicyMaxWindowSize) bytes = (size_t)prop.accessPolicyMaxWindowSize;
@@ -222,6 +229,13 @@ int vmg_destroy(vmg_handle h)
 {
     if (!h) return VMG_ERR_ARG;
     cudaStreamSynchronize(h->stream);
+    if (h->l2_window_set) {   // the window covers this handle's arena: take it off the (possibly caller-owned) stream
+        cudaStreamAttrValue a;
+        memset(&a, 0, sizeof(a));
+        cudaStreamSetAttribute(h->stream, cudaStreamAttributeAccessPolicyWindow, &a);
+        cudaCtxResetPersistingL2Cache();
+    }
+    if (h->l2_limit_saved) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, h->l2_limit_prev);
     prof_collect(h);
     for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
     for (int i = 0; i < 6; ++i) {
@@ -318,7 +332,7 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
     }
     delete ps;
     CUDA_TRY(h, cudaGetLastError());
-    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (h->own_stream || h->profile) CUDA_TRY(h, cudaStreamSynchronize(h->stream));   // caller's stream: enqueue only (vmg.h, vmg_create)
     h->total_launches += setup_launches;
     if (h->profile) prof_collect(h);
     h->have_coeffs = true;
@@ -341,7 +355,7 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
             CUDA_TRY(h, cudaMemcpyAsync(h->bcval[f], value[f], plane_count(h->lev[0], f) * sizeof(double),
                                         cudaMemcpyDeviceToDevice, h->stream));
     }
-    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (h->own_stream) CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     h->have_bc = true;
     return VMG_OK;
 }
@@ -381,11 +395,13 @@ int vmg_set_mask(vmg_handle h, const unsigned char* mask, int kind, const double
         h->d_cval = base + o_cval;
         CUDA_TRY(h, cudaMemcpyAsync(h->d_cval, cval, (size_t)L0.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
     }
-    // the number of covered cells decides whether a Dirichlet mask pins the solution (setup path: counted on the host)
-    std::vector<unsigned char> hm((size_t)L0.n);
-    CUDA_TRY(h, cudaMemcpyAsync(hm.data(), h->d_mask, (size_t)L0.n, cudaMemcpyDeviceToHost, h->stream));
+    // the number of covered cells decides whether a Dirichlet mask pins the solution: counted on the device, 8 bytes come back
+    unsigned long long* cnt = (unsigned long long*)h->d_scal + 8;
+    CUDA_TRY(h, cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), h->stream));
+    mask_count_covered_kernel<<<std::min<unsigned>(grid_for(L0.n), 8u * h->num_sms), kThreads, 0, h->stream>>>(h->d_mask, L0.n, cnt);
+    CUDA_TRY(h, cudaMemcpyAsync(h->h_scal + 8, cnt, sizeof(unsigned long long), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    for (unsigned char v : hm) h->mask_covered += v == 0;
+    h->mask_covered = (long long)*(unsigned long long*)(h->h_scal + 8);
     return VMG_OK;
 }
 
@@ -556,7 +572,7 @@ int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max
     }
     if (rc == VMG_OK) rc = solve_end(h);
     if (cudaStreamSynchronize(h->stream) != cudaSuccess && rc == VMG_OK) rc = VMG_ERR_CUDA;
-    if (rc == VMG_ERR_CUDA) { h->last_cuda_error = (int)cudaGetLastError(); }
+    if (rc == VMG_ERR_CUDA) { const int e = (int)cudaGetLastError(); if (e != 0 || h->last_cuda_error == 0) h->last_cuda_error = e; }   // keep the first recorded error
     return solve_close(h, rc);
 }
 

@@ -73,12 +73,13 @@ struct vmg_s {
     int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200
     double l2_persist_mb = 24.0;  // L2 set aside for the level-0 face weights (0: none); see apply_l2_window
     bool l2_applied = false, l2_window_set = false;
+    bool l2_limit_saved = false;  // cudaLimitPersistingL2CacheSize as it was before this handle raised it (restored by vmg_destroy)
+    size_t l2_limit_prev = 0;
     int use_pdl = 1;              // programmatic dependent launch of the V-cycle kernels
     long long phi_keep_cells = 1ll << 25;     // option "phi_keep_cells": levels with at least this many cells (default 32 Mi: phi = 2 x L2) load the neighbours' phi with the normal policy
     int snake = 1;                // consecutive half-sweeps walk the level in opposite directions (L2 reuse)
     int use_tail = 1;             // run the coarsest levels in one CTA (vmg_tail.cuh)
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
-    int cluster_level = -1;       // unused (-1)
     size_t tail_smem = 0;         // dynamic shared memory of the tail kernel
     long long block_min_cells = 4096;   // smallest level the blocked smoother is used on
     // device scalars

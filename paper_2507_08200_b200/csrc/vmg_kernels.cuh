@@ -266,6 +266,15 @@ __global__ void mask_face_bits_kernel(Geom G, const unsigned char* __restrict__ 
     in[cell_at(G, i, j, k)] = (unsigned char)fb;
 }
 
+// covered cells (mask == 0) of a level-0 mask, accumulated into *out (the caller zeroes it)
+__global__ void mask_count_covered_kernel(const unsigned char* __restrict__ mask, long long n, unsigned long long* out)
+{
+    unsigned long long c = 0;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) c += mask[t] == 0;
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
+}
+
 // public (natural) layout <-> internal layout of one cell array
 // mask (may be NULL): covered cells enter as zero (they are identity rows of the masked operator)
 __global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in, const unsigned char* __restrict__ mask)

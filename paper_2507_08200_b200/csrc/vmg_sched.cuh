@@ -210,7 +210,6 @@ inline int tail_guard(const vmg_s* h, const VmgLevel& L) { return (h->three_d ? 
 inline void plan_schedule(vmg_s* h)
 {
     h->tail_level = -1;
-    h->cluster_level = -1;
     h->tail_smem = 0;
     if (!h->use_tail) return;
     size_t doubles = 0;
@@ -233,10 +232,9 @@ inline void plan_schedule(vmg_s* h)
 inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* count)
 {
     TailArgs g;
-    const int tail = h->tail_level, first = h->cluster_level >= 0 ? h->cluster_level : tail;
+    const int tail = h->tail_level, first = tail;
     int off = 0;
     g.nl = h->nlev - first;
-    g.ns = tail - first;
     for (int l = first; l < h->nlev; ++l) {
         VmgLevel& L = h->lev[l];
         TailLevel& T = g.lev[l - first];
@@ -650,7 +648,7 @@ inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* co
 {
     const int last = h->nlev - 1;
     // first level not handled stroke by stroke
-    const int tail = h->tail_level < 0 ? last : h->cluster_level >= 0 ? h->cluster_level : h->tail_level;
+    const int tail = h->tail_level < 0 ? last : h->tail_level;
     if (norm_out) cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
     for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }
     for (int l = 0; l < tail; ++l) enqueue_down(h, l, count);
@@ -676,14 +674,14 @@ inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* co
 inline bool vcycle_segmentable(const vmg_s* h)
 {
     const int last = h->nlev - 1;
-    const int tail = h->tail_level < 0 ? last : h->cluster_level >= 0 ? h->cluster_level : h->tail_level;
+    const int tail = h->tail_level < 0 ? last : h->tail_level;
     return tail >= 1 && h->use_graph && !h->profile;
 }
 
 inline void enqueue_vcycle_segment(vmg_s* h, int seg, unsigned long long* norm_out, long long* count)
 {
     const int last = h->nlev - 1;
-    const int tail = h->tail_level < 0 ? last : h->cluster_level >= 0 ? h->cluster_level : h->tail_level;
+    const int tail = h->tail_level < 0 ? last : h->tail_level;
     if (seg == 0) {
         cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
         for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }

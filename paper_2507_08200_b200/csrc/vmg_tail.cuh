@@ -23,8 +23,6 @@ struct TailLevel {
 struct TailArgs {
     TailLevel lev[kTailMaxLevels];
     int nl;                    // levels in the tail; lev[nl-1] is the bottom
-    int ns;                    // 0 (levels lev[ns..nl-1] run in shared memory; a cluster-wide variant for larger levels,
-                               // barrier.cluster between half-sweeps on global arrays, measured slower than graph launches)
     int nu1, nu2, nbottom, sz; // sz = 2 in 3-D, 1 in 2-D (children per coarse cell along z)
     int prolong;               // 0: piecewise constant, 1: trilinear (R9 option)
     int sym;                   // 1: symmetric V-cycle: post-smoothing and the second half of the bottom sweeps black->red
@@ -128,7 +126,7 @@ __device__ __forceinline__ double tail_residual_at(const TailSmem& s, const Tail
     return s.rhs[c] + tail_nb_sum(s, L, c) - s.phi[c] / s.dinv[c];
 }
 
-// levels lev[g.ns] .. lev[g.nl-1], by one CTA, in shared memory
+// levels lev[0] .. lev[g.nl-1], by one CTA, in shared memory
 __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
 {
     extern __shared__ __align__(16) double tail_smem[];
@@ -141,19 +139,19 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         for (int t = tid; t < total; t += nth) tail_smem[t] = 0.0;
     }
     __syncthreads();
-    for (int l = g.ns; l < g.nl; ++l) {
+    for (int l = 0; l < g.nl; ++l) {
         const TailLevel& L = g.lev[l];
         TailSmem s(tail_smem, L);
         for (int t = tid; t < L.n; t += nth) {
             const long long c = cell_at(L.G, t % L.nx, (t / L.nx) % L.ny, t / L.nxy);
             s.dinv[t] = L.dinv[c]; s.wx[t] = L.wx[c]; s.wy[t] = L.wy[c]; s.wz[t] = L.wz[c];
-            if (l == g.ns) { s.rhs[t] = L.rhs[c]; if (g.whole) s.phi[t] = L.phi[c]; }
+            if (l == 0) { s.rhs[t] = L.rhs[c]; if (g.whole) s.phi[t] = L.phi[c]; }
         }
     }
     __syncthreads();
 
     // ---- down-stroke ----
-    for (int l = g.ns; l + 1 < g.nl; ++l) {
+    for (int l = 0; l + 1 < g.nl; ++l) {
         const TailLevel& L = g.lev[l];
         const TailLevel& C = g.lev[l + 1];
         TailSmem s(tail_smem, L), c(tail_smem, C);
@@ -175,7 +173,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
     {
         const TailLevel& B = g.lev[g.nl - 1];
         TailSmem s(tail_smem, B);
-        if (g.nl - g.ns == 1 && g.whole) {                 // single-level hierarchy: the bottom solve is the cycle (C4)
+        if (g.nl == 1 && g.whole) {                 // single-level hierarchy: the bottom solve is the cycle (C4)
             for (int t = tid; t < B.n; t += nth) s.phi[t] = 0.0;
             __syncthreads();
         }
@@ -183,7 +181,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         else { tail_smooth(s, B, g.nbottom / 2, 0); tail_smooth(s, B, g.nbottom - g.nbottom / 2, 1); }
     }
     // ---- up-stroke ----
-    for (int l = g.nl - 2; l >= g.ns; --l) {
+    for (int l = g.nl - 2; l >= 0; --l) {
         const TailLevel& L = g.lev[l];
         const TailLevel& C = g.lev[l + 1];
         TailSmem s(tail_smem, L), c(tail_smem, C);
@@ -200,7 +198,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
     }
     // ---- stage out ----
     {
-        const TailLevel& L = g.lev[g.ns];
+        const TailLevel& L = g.lev[0];
         TailSmem s(tail_smem, L);
         double m = 0.0;
         bool nan = false;
