@@ -138,6 +138,11 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  *   which makes one V-cycle from zero a symmetric operator; default 0; vmg_solve_pcg switches it on for itself), "prolong" (0: piecewise-constant prolongation, default; 1: cell-centred trilinear,
  *   weights 3/4 and 1/4 per direction, ghost value -e at Dirichlet and +e at Neumann faces), "graph" (1: replay the V-cycle as a CUDA graph, default; 0: plain launches),
  * "tail" (1: the coarsest levels run in one single-CTA launch, default; 0: one kernel per step),
+ * "device_loop" (1, default: all V-cycles of a vmg_solve are ONE graph launch -- a conditional WHILE node whose condition
+ *   a one-thread kernel sets from the exit rules -- and the residual norm of cycle c is taken by the first half-sweep of
+ *   cycle c+1, which writes beside phi so that a converged iterate is returned untouched; bitwise the status, cycle count,
+ *   history and phi of the host-driven loop; used when graph = 1, nu1 >= 2, nu2 >= 1, symmetric = 0, blocked = 0,
+ *   max_vcycles <= 1000 and level 0 is not in the single-CTA tail; 0: one graph replay and one 8-byte read-back per cycle),
  * "snake" (1: consecutive whole-level kernels walk the level in opposite z-directions so that each starts on
  *   what the previous one left in L2, default; 0: always ascending),
  * "l2_persist" (MB of L2 set aside for the level-0 face weights through a stream access-policy window,

@@ -68,6 +68,8 @@ size_t layout(vmg_s* h, double* base)
     }
     size_t o = p.take(32);
     if (base) h->d_scal = base + o;
+    o = p.take(8 + kLoopMaxCycles + 1);
+    if (base) h->d_loop = base + o;
     return p.off;
 }
 
@@ -213,6 +215,7 @@ int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, do
     layout(h, (double*)h->arena);
     if (cudaMemsetAsync(h->arena, 0, h->arena_bytes, h->stream) != cudaSuccess ||
         cudaMallocHost((void**)&h->h_scal, 32 * sizeof(double)) != cudaSuccess ||
+        cudaMallocHost((void**)&h->h_loop, (8 + kLoopMaxCycles + 1) * sizeof(double)) != cudaSuccess ||
         cudaStreamSynchronize(h->stream) != cudaSuccess) {
         (void)cudaGetLastError();
         cudaFree(h->arena);
@@ -245,6 +248,8 @@ int vmg_destroy(vmg_handle h)
     if (h->pcg_base) cudaFree(h->pcg_base);
     if (h->mask_base) cudaFree(h->mask_base);
     for (int i = 0; i < 3; ++i) {
+        if (h->loop_exec[i]) cudaGraphExecDestroy(h->loop_exec[i]);
+        if (h->loop_graph[i]) cudaGraphDestroy(h->loop_graph[i]);
         if (h->graph_exec[i]) cudaGraphExecDestroy(h->graph_exec[i]);
         if (h->graph[i]) cudaGraphDestroy(h->graph[i]);
         for (int sg = 0; sg < 3; ++sg) {
@@ -256,6 +261,7 @@ int vmg_destroy(vmg_handle h)
     if (h->coarse_done) cudaEventDestroy(h->coarse_done);
     if (h->coarse_stream) cudaStreamDestroy(h->coarse_stream);
     if (h->h_scal) cudaFreeHost(h->h_scal);
+    if (h->h_loop) cudaFreeHost(h->h_loop);
     if (h->arena) cudaFree(h->arena);
     if (h->own_stream) cudaStreamDestroy(h->stream);
     (void)cudaGetLastError();
@@ -418,6 +424,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "graph")) { h->use_graph = iv != 0; }
     else if (!strcmp(key, "blocked")) { if (iv < 0 || iv > 3) return VMG_ERR_ARG; h->use_blocked = iv; }   // 1: vmg_block2.cuh, 2 / 3: vmg_block3.cuh (TMA; 2 x 2 patches / rows)
     else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }
+    else if (!strcmp(key, "device_loop")) { h->use_loop = iv != 0; }
     else if (!strcmp(key, "snake")) { h->snake = iv != 0; }
     else if (!strcmp(key, "pdl")) { h->use_pdl = iv != 0; }
     else if (!strcmp(key, "block_min_cells")) { if (v < 0) return VMG_ERR_ARG; h->block_min_cells = (long long)v; }
@@ -565,6 +572,24 @@ int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max
     rc = solve_begin(h, rhs, phi, rtol, max_vcycles);
     if (rc == VMG_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = VMG_ERR_CUDA;
     if (rc == VMG_OK) rc = solve_begin_finish(h);
+    if (rc == VMG_OK && h->sv_active && solve_loop_ok(h, max_vcycles)) {
+        // all cycles as one graph launch: WHILE node, exit rules on the device (run_solve_loop); then the same bookkeeping
+        h->h_loop[0] = h->sv_nb; h->h_loop[1] = rtol; h->h_loop[2] = (double)max_vcycles; h->h_loop[3] = 0.0; h->h_loop[4] = 0.0;
+        h->h_loop[5] = (double)VMG_MAXCYCLES; h->h_loop[6] = h->h_loop[7] = 0.0; h->h_loop[8] = h->hist[0];
+        rc = run_solve_loop(h, (unsigned long long*)h->d_scal + 1);
+        if (rc == VMG_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = VMG_ERR_CUDA;
+        if (rc == VMG_OK) {
+            const int cyc = (int)h->h_loop[3];
+            for (int c = 1; c <= cyc; ++c) h->hist.push_back(h->h_loop[8 + c]);
+            h->cycles = cyc;
+            h->relres = h->h_loop[8 + cyc];
+            h->sv_status = (int)h->h_loop[5];
+            h->sv_active = false;
+            if (h->sv_status == VMG_ERR_DIVERGED) h->sv_phi = nullptr;
+            h->launches += h->loop_launches_head[h->lev[0].cw] + (long long)cyc * h->loop_launches_body[h->lev[0].cw];
+            h->launches_per_cycle = h->loop_launches_body[h->lev[0].cw];
+        }
+    }
     while (rc == VMG_OK && h->sv_active) {
         rc = solve_cycle_launch(h);
         if (rc == VMG_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = VMG_ERR_CUDA;

@@ -28,6 +28,8 @@ struct VmgProfEvent { int cls; long long launches; cudaEvent_t start, stop; };
 // a cached TMA descriptor of one level array for one box shape (vmg_sched.cuh level_map)
 struct VmgTensorMap { const double* base; int nxp, nyt, rank; alignas(64) CUtensorMap map; };
 
+constexpr int kLoopMaxCycles = 1000;   // longest solve the device-side loop keeps a history for (longer ones: host loop)
+
 struct VmgLevel {
     int nx = 0, ny = 0, nz = 0;
     long long n = 0;          // cells
@@ -95,6 +97,15 @@ struct vmg_s {
     cudaGraphExec_t graph_exec[3] = {nullptr, nullptr, nullptr};
     unsigned graph_slot_epoch[3] = {0, 0, 0};
     long long graph_slot_launches[3] = {0, 0, 0};
+    // the whole cycle loop of vmg_solve as ONE graph with a conditional WHILE node (run_solve_loop in vmg_sched.cuh): the
+    // exit rules run on the device, the residual norm rides on the first half-sweep of the next cycle
+    int use_loop = 1;                  // option "device_loop"
+    cudaGraph_t loop_graph[3] = {nullptr, nullptr, nullptr};
+    cudaGraphExec_t loop_exec[3] = {nullptr, nullptr, nullptr};
+    unsigned loop_epoch[3] = {0, 0, 0};
+    long long loop_launches_head[3] = {0, 0, 0}, loop_launches_body[3] = {0, 0, 0};
+    double* d_loop = nullptr;          // device: nb, rtol, max, cycles, slow, status, -, -, hist[kLoopMaxCycles + 1]
+    double* h_loop = nullptr;          // pinned host mirror
     // the same cycle cut in three graphs for the staggered batch schedule (vmg_solve_batch): [cw][segment], segment
     // 0 = level-0 down-stroke, 1 = all coarser levels, 2 = level-0 up-stroke + residual norm
     cudaGraph_t seg_graph[3][3] = {};

@@ -459,6 +459,78 @@ __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, cons
     if (m < L.G.ne && j < L.G.ny) relax_at<CW, KEEP>(L, phi, rhs, colour, m, j, k);
 }
 
+__device__ __forceinline__ void block_max_to_global(double v, unsigned long long* out);
+
+// S2 + S6 fused (per-colour path): a colour half-sweep that reads the neighbours from phi_in and writes the relaxed cells
+// to phi_out (which may be another array), optionally also forming the residual of the cells it relaxes BEFORE relaxing
+// them.  A relaxation computes t = rhs_c + sum w phi_nb anyway; the residual of that cell is t - phi_c / (1/D_c): one more
+// half double per cell of traffic and a division instead of a kernel of its own over the whole level (S6 "0 (fused)",
+// SURVEY.md 8(a)).  Used by the device-side solve loop (vmg_sched.cuh run_solve_loop): the first (red) half-sweep of cycle
+// c+1 takes the norm of the iterate after cycle c -- red cells only, reading R12 -- and writes its red cells to the second
+// phi array, so that the iterate itself stays untouched if it turns out to be converged; the black half-sweep that follows
+// reads its (all red) neighbours from that array and writes into the first one, after which the cycle continues in place.
+// Same expressions, same order as relax_at / residual_at: phi and the norms are bitwise those of the separate kernels.
+template <int CW, int KEEP, int NORM>
+__global__ void smooth_colour_io_kernel(LevelView L, const double* __restrict__ phi_in, double* __restrict__ phi_out,
+                                        const double* __restrict__ rhs, int colour, int reverse, unsigned long long* norm_out)
+{
+    grid_dependency_wait();
+    const Geom& G = L.G;
+    int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    if (reverse) { k = G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
+    double mx = 0.0;
+    if (m < G.ne && j < G.ny) {
+        const int par = (colour + j + k) & 1;
+        if (2 * m + par < G.nx) {
+            long long c, xm;
+            pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
+            double w[6];
+            face_weights<CW>(L, c, xm, 2 * m + par, j, k, w);
+            auto ld = [](const double* q) { return KEEP ? *q : __ldcs(q); };
+            double s = w[0] * ld(phi_in + xm);
+            s = fma(w[1], ld(phi_in + xm + 1), s);
+            s = fma(w[2], ld(phi_in + c - G.pitch), s);
+            s = fma(w[3], ld(phi_in + c + G.pitch), s);
+            s = fma(w[4], ld(phi_in + c - G.plane), s);
+            s = fma(w[5], ld(phi_in + c + G.plane), s);
+            const double di = __ldcs(L.dinv + c), t = __ldcs(rhs + c) + s;
+            if (NORM) {
+                mx = fabs(t - ld(phi_in + c) / di);
+                if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
+            }
+            phi_out[c] = di * t;
+        }
+    }
+    if (NORM) block_max_to_global(mx, norm_out);
+}
+
+// S7: the exit rules of the solve (C5 of DESIGN.md), on the device, after cycle c's norm has been accumulated:
+// st[0] = ||btilde||, [1] = rtol, [2] = max cycles, [3] = cycles done, [4] = slow-cycle counter, [5] = status,
+// hist = st + 8.  Sets the WHILE condition of the solve graph and clears the norm accumulator for the next cycle.
+__global__ void solve_decide_kernel(cudaGraphConditionalHandle handle, double* st, unsigned long long* norm_bits)
+{
+    if (threadIdx.x != 0) return;
+    const double norm = __longlong_as_double((long long)*norm_bits);
+    *norm_bits = 0ull;
+    double* hist = st + 8;
+    const int c = (int)st[3] + 1;
+    const double rtol = st[1], relres = norm / st[0];
+    st[3] = (double)c;
+    hist[c] = relres;
+    unsigned cont = 1u;
+    if (relres != relres || relres > 1.7976931348623157e308) { st[5] = -5.0; cont = 0u; }           // VMG_ERR_DIVERGED
+    else if (rtol > 0.0) {
+        if (relres <= rtol) { st[5] = 0.0; cont = 0u; }                                           // VMG_OK
+        else {
+            const int slow = hist[c] >= 0.9 * hist[c - 1] ? (int)st[4] + 1 : 0;
+            st[4] = (double)slow;
+            if (slow >= 3) { st[5] = 2.0; cont = 0u; }                                            // VMG_STALLED
+        }
+    }
+    if (cont && c >= (int)st[2]) cont = 0u;                                                       // VMG_MAXCYCLES (status as initialised)
+    cudaGraphSetConditional(handle, cont);
+}
+
 // S4 + S2 fused (per-colour path).  The first colour half-sweep after a coarse-grid correction: a relaxation never
 // reads the old value of the cell it overwrites, and all six neighbours of a cell of one colour have the other
 // colour, so the correction phi += P e (piecewise constant, R9) is applied to the NEIGHBOURS on the fly and never

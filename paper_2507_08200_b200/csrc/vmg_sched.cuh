@@ -733,6 +733,121 @@ inline int run_vcycle_segment(vmg_s* h, int seg, unsigned long long* out, cudaSt
     return VMG_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// S7 with the convergence test on the device ("device-side WHILE conditional node") and the
+// residual norm fused into the next cycle (S6 "0 (fused)").  One graph per solve:
+//     head:   norm accumulator = 0;  H1 = red half-sweep of cycle 1: neighbours from phi, red cells -> phi2
+//     WHILE (continue) {
+//         black half-sweep: (red) neighbours from phi2, black cells -> phi;   rest of the cycle in place on phi
+//         H1 of the NEXT cycle, which also takes the red-cell residual norm of the iterate just completed (reading R12)
+//         solve_decide_kernel: history, exit rules C5, sets `continue`
+//     }
+// phi itself holds the completed iterate until the device has decided to go on, so a converged solve returns exactly
+// the iterate the host-driven loop returns (bitwise: same kernels' arithmetic, same norms); what it costs is one red
+// half-sweep after the last cycle (21 us on config 3) in place of a residual-norm kernel per cycle (30 us) and of the
+// host round trip between cycles.
+// ------------------------------------------------------------------------------------------------
+inline bool solve_loop_ok(vmg_s* h, int max_vcycles)
+{
+    const int last = h->nlev - 1;
+    const int tail = h->tail_level < 0 ? last : h->tail_level;
+    // nu1 >= 2: the red cells relaxed by H1 live in phi2 until the second red half-sweep of the down-stroke rewrites them in phi
+    return h->use_loop && h->use_graph && !h->profile && h->nu1 >= 2 && h->nu2 >= 1 && !h->symmetric && tail >= 1 &&
+           !blocked_ok(h, 0) && max_vcycles >= 1 && max_vcycles <= kLoopMaxCycles;
+}
+
+// a colour half-sweep of level 0 with separate input / output arrays, optionally with the norm of the cells it relaxes
+inline void loop_halfsweep_io(vmg_s* h, const double* in, double* out, int colour, bool norm, unsigned long long* norm_out, long long* count)
+{
+    VmgLevel& L = h->lev[0];
+    LevelView v = view(L);
+    dim3 grid, block;
+    pair_launch_dims(L, grid, block);
+    const int dir = next_dir(h, L);
+    const bool keep = L.cw == 0 && L.n >= h->phi_keep_cells;
+#define VMG_IO(CW_, KEEP_) (norm ? smooth_colour_io_kernel<CW_, KEEP_, 1> : smooth_colour_io_kernel<CW_, KEEP_, 0>)
+    auto kernel = L.cw == 2 ? VMG_IO(2, 0) : L.cw == 1 ? VMG_IO(1, 0) : keep ? VMG_IO(0, 1) : VMG_IO(0, 0);
+#undef VMG_IO
+    launch_pdl(h, kernel, grid, block, 0, v, in, out, L.rhs, colour, dir, norm_out);
+    ++*count;
+}
+
+// one WHILE iteration (see above); the levels' phi in their primary buffers
+inline void enqueue_loop_body(vmg_s* h, cudaGraphConditionalHandle handle, unsigned long long* norm_out, long long* count)
+{
+    const int last = h->nlev - 1;
+    const int tail = h->tail_level < 0 ? last : h->tail_level;
+    for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }
+    VmgLevel& L0 = h->lev[0];
+    L0.dir = 1;                                                   // the half-sweep before this one walked forward
+    loop_halfsweep_io(h, L0.phi2, L0.phi, 1, false, nullptr, count);
+    plain_smooth(h, 0, h->nu1, count, 2);
+    plain_residual_restrict(h, 0, count);
+    for (int l = 1; l < tail; ++l) enqueue_down(h, l, count);
+    if (h->tail_level >= 0) enqueue_tail(h, nullptr, count);
+    else {
+        if (!h->symmetric) plain_smooth(h, last, h->nbottom, count);
+        else { plain_smooth(h, last, h->nbottom / 2, count, 0, 0); plain_smooth(h, last, h->nbottom - h->nbottom / 2, count, 0, 1); }
+    }
+    for (int l = tail - 1; l >= 0; --l) enqueue_up(h, l, nullptr, count);
+    loop_halfsweep_io(h, L0.phi, L0.phi2, 0, true, norm_out, count);
+    solve_decide_kernel<<<1, 32, 0, h->stream>>>(handle, h->d_loop, norm_out);
+    ++*count;
+}
+
+// builds (once per epoch and kind of weights) and launches the solve graph; the caller has filled h->h_loop[0..8]
+inline int run_solve_loop(vmg_s* h, unsigned long long* norm_out)
+{
+    const int gi = h->lev[0].cw;
+    auto fail = [&](cudaError_t e) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; };
+    if (h->loop_epoch[gi] != h->graph_epoch) {
+        if (h->loop_exec[gi]) { cudaGraphExecDestroy(h->loop_exec[gi]); h->loop_exec[gi] = nullptr; }
+        if (h->loop_graph[gi]) { cudaGraphDestroy(h->loop_graph[gi]); h->loop_graph[gi] = nullptr; }
+        cudaGraph_t g = nullptr, dummy = nullptr;
+        cudaError_t e = cudaGraphCreate(&g, 0);
+        if (e != cudaSuccess) return fail(e);
+        h->loop_graph[gi] = g;
+        cudaGraphConditionalHandle handle;
+        if ((e = cudaGraphConditionalHandleCreate(&handle, g, 1, cudaGraphCondAssignDefault)) != cudaSuccess) return fail(e);
+        // head
+        long long count = 0;
+        if ((e = cudaStreamBeginCaptureToGraph(h->stream, g, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed)) != cudaSuccess) return fail(e);
+        cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
+        for (int l = 0; l < h->nlev; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }
+        loop_halfsweep_io(h, h->lev[0].phi, h->lev[0].phi2, 0, false, nullptr, &count);
+        cudaStreamCaptureStatus st;
+        const cudaGraphNode_t* deps = nullptr;
+        size_t ndeps = 0;
+        e = cudaStreamGetCaptureInfo(h->stream, &st, nullptr, nullptr, &deps, &ndeps);
+        std::vector<cudaGraphNode_t> tails(deps, deps + (e == cudaSuccess ? ndeps : 0));
+        cudaError_t e2 = cudaStreamEndCapture(h->stream, &dummy);
+        if (e != cudaSuccess || e2 != cudaSuccess) return fail(e != cudaSuccess ? e : e2);
+        h->loop_launches_head[gi] = count;
+        // WHILE node and its body
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = handle;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        cudaGraphNode_t wnode;
+        if ((e = cudaGraphAddNode(&wnode, g, tails.data(), tails.size(), &np)) != cudaSuccess) return fail(e);
+        cudaGraph_t body = np.conditional.phGraph_out[0];
+        count = 0;
+        if ((e = cudaStreamBeginCaptureToGraph(h->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed)) != cudaSuccess) return fail(e);
+        enqueue_loop_body(h, handle, norm_out, &count);
+        if ((e = cudaStreamEndCapture(h->stream, &dummy)) != cudaSuccess) return fail(e);
+        h->loop_launches_body[gi] = count;
+        if ((e = cudaGraphInstantiate(&h->loop_exec[gi], g, 0)) != cudaSuccess) return fail(e);
+        h->loop_epoch[gi] = h->graph_epoch;
+    }
+    const int max = (int)h->h_loop[2];
+    cudaError_t e = cudaMemcpyAsync(h->d_loop, h->h_loop, 9 * sizeof(double), cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaGraphLaunch(h->loop_exec[gi], h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h->h_loop, h->d_loop, (size_t)(8 + max + 1) * sizeof(double), cudaMemcpyDeviceToHost, h->stream);
+    if (e != cudaSuccess) return fail(e);
+    return VMG_OK;
+}
+
 // V-cycle followed by the residual norm into *out (device), as a graph replay when enabled.
 inline int run_vcycle_with_norm(vmg_s* h, unsigned long long* out)
 {

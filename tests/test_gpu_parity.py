@@ -98,7 +98,7 @@ def test_schedule_options_do_not_change_a_single_bit():
     p = inputs.config4(32)
     ref = None
     for opts in (dict(snake=0, l2_persist=0, graph=0, tail=0), dict(), dict(snake=1, graph=0), dict(tail=0), dict(blocked=1),
-                 dict(blocked=2), dict(blocked=3, block_min_cells=0),
+                 dict(blocked=2), dict(blocked=3, block_min_cells=0), dict(device_loop=0), dict(device_loop=0, graph=0),
                  dict(phi_keep_cells=0), dict(phi_keep_cells=0, graph=0, tail=0)):   # cache policy of the largest levels on all levels
         s, d = b.from_problem(p)
         for k, v in opts.items():
@@ -111,6 +111,33 @@ def test_schedule_options_do_not_change_a_single_bit():
             ref = out
         else:
             assert torch.equal(out[0], ref[0]) and out[1] == ref[1], opts
+
+
+@pytest.mark.parametrize("rtol,maxc", [(1e-12, 50), (0.0, 7), (1e-12, 3), (1e-17, 40), (1e-3, 50)],
+                         ids=["converges", "fixed_cycles", "maxcycles", "stalls_on_the_floor", "two_cycles"])
+def test_device_side_solve_loop_applies_the_exit_rules_of_the_host_loop(rtol, maxc):
+    """The solve as one graph with a conditional WHILE node (exit rules C5 on the device, the residual norm riding on the
+    first half-sweep of the next cycle, option device_loop = 1, default) returns the status, the cycle count, the history and
+    phi of the host-driven loop bit for bit -- for every exit rule, from a zero and from a warm start, and it leaves a
+    converged iterate untouched although the next cycle's first half-sweep has already run."""
+    b = _binding()
+    p = inputs.config4(32)
+    out = {}
+    for loop in (0, 1):
+        s, d = b.from_problem(p)
+        s.set_option("device_loop", loop)
+        res = []
+        phi = torch.zeros_like(d["rhs"])
+        for rep in range(2):                    # second solve: warm start from the first result (often 0 or 1 cycles)
+            st = s.solve(d["rhs"], phi, rtol=rtol, max_vcycles=maxc)
+            cyc, rr, hist = s.get_info()
+            res.append((st, cyc, list(hist), phi.clone()))
+        out[loop] = res
+        s.destroy()
+    for a, c in zip(out[0], out[1]):
+        assert a[0] == c[0] and a[1] == c[1] and a[2] == c[2] and torch.equal(a[3], c[3]), (a[:3], c[:3])
+    assert out[1][0][0] == {"converges": 0, "fixed_cycles": 1, "maxcycles": 1, "stalls_on_the_floor": 2, "two_cycles": 0}[
+        {(1e-12, 50): "converges", (0.0, 7): "fixed_cycles", (1e-12, 3): "maxcycles", (1e-17, 40): "stalls_on_the_floor", (1e-3, 50): "two_cycles"}[(rtol, maxc)]]
 
 
 @pytest.mark.parametrize("dims", [(40, 24, 16), (88, 56, 24), (144, 80, 48), (256, 128, 32)])
