@@ -843,3 +843,11 @@ int vmg_solve_batch(int n, const vmg_handle* hs, const double* const* rhs, doubl
 }  // extern "C"
 
 #include "vmg_steps.inl"
+
+#ifdef VMG_TAIL_TIMING
+// debug build only (-DVMG_TAIL_TIMING): clock64 stamps of the last coarse_tail_kernel launch (vmg_tail.cuh TAIL_MARK)
+extern "C" int vmg_debug_tail_clock(long long* out64)
+{
+    return cudaMemcpyFromSymbol(out64, vmg::vmg_tail_clock, 64 * sizeof(long long)) == cudaSuccess ? 0 : -6;
+}
+#endif

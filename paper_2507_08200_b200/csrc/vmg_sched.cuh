@@ -225,7 +225,8 @@ inline void plan_schedule(vmg_s* h)
     if (first == h->nlev) return;
     h->tail_level = first;
     h->tail_smem = doubles * sizeof(double);
-    cudaFuncSetAttribute(coarse_tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmemCap);
+    cudaFuncSetAttribute(coarse_tail_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmemCap);
+    cudaFuncSetAttribute(coarse_tail_kernel<kTailThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmemCap);
     (void)cudaGetLastError();
 }
 
@@ -253,7 +254,8 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
     ProfScope ps(h, VMG_PC_COARSE, count);
     {
         int threads = (int)std::min<long long>(kTailThreads, std::max<long long>(64, (h->lev[first].n / 2 + 31) / 32 * 32));
-        launch_pdl(h, coarse_tail_kernel, 1, threads, h->tail_smem, g);
+        if (threads <= 512) launch_pdl(h, coarse_tail_kernel<512>, 1, threads, h->tail_smem, g);
+        else launch_pdl(h, coarse_tail_kernel<kTailThreads>, 1, threads, h->tail_smem, g);
     }
     ++*count;
 }

@@ -85,12 +85,42 @@ __device__ __forceinline__ void tail_smooth(const TailSmem& s, const TailLevel& 
             }
             if (first) { const int tmp = c[0]; c[0] = c[1]; c[1] = tmp; }   // c[0]: the colour relaxed first
         }
+        // the thread relaxes the same two cells in every sweep: their weights, 1/D and rhs stay in registers (16 doubles),
+        // a relaxation reads the six neighbours from shared memory and nothing else (was 14 LDS.64 per relaxation: the
+        // half-sweeps of a 1024-cell level were bound by shared-memory wavefronts, not by the barrier)
+        double w[2][6], di[2], rh[2];
+        int cc[2];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            cc[q] = c[q] >= 0 ? c[q] : 0;
+            w[q][0] = s.wx[cc[q]]; w[q][1] = s.wx[cc[q] + 1];
+            w[q][2] = s.wy[cc[q]]; w[q][3] = s.wy[cc[q] + L.nx];
+            w[q][4] = s.wz[cc[q]]; w[q][5] = s.wz[cc[q] + L.zs];
+            di[q] = s.dinv[cc[q]]; rh[q] = s.rhs[cc[q]];
+        }
+        // level constants and the neighbours' addresses in registers; the six neighbours are loaded before the first FMA
+        // (the compiler otherwise re-reads nx and the z-stride from the kernel parameters -- indexed constant loads -- and
+        // chains load -> FMA -> load inside every half-sweep)
+        const int nx = L.nx, zs = L.zs;
+        double* const ph = s.phi;
+        auto relax = [&](int q) {
+            if (c[q] < 0) return;                  // warps without a cell of this level go straight to the barrier
+            double* const x = ph + cc[q];
+            const double a0 = x[-1], a1 = x[1], a2 = x[-nx], a3 = x[nx], a4 = x[-zs], a5 = x[zs];
+            double v = w[q][0] * a0;
+            v = fma(w[q][1], a1, v);
+            v = fma(w[q][2], a2, v);
+            v = fma(w[q][3], a3, v);
+            v = fma(w[q][4], a4, v);
+            v = fma(w[q][5], a5, v);
+            *x = di[q] * (rh[q] + v);
+        };
         if (nt <= 32) {
             if (threadIdx.x < 32)
                 for (int sw = 0; sw < nsweeps; ++sw) {
 #pragma unroll
-                    for (int colour = 0; colour < 2; ++colour) {
-                        if (c[colour] >= 0) s.phi[c[colour]] = s.dinv[c[colour]] * (s.rhs[c[colour]] + tail_nb_sum(s, L, c[colour]));
+                    for (int q = 0; q < 2; ++q) {
+                        relax(q);
                         __syncwarp();
                     }
                 }
@@ -99,8 +129,8 @@ __device__ __forceinline__ void tail_smooth(const TailSmem& s, const TailLevel& 
         }
         for (int sw = 0; sw < nsweeps; ++sw) {
 #pragma unroll
-            for (int colour = 0; colour < 2; ++colour) {
-                if (c[colour] >= 0) s.phi[c[colour]] = s.dinv[c[colour]] * (s.rhs[c[colour]] + tail_nb_sum(s, L, c[colour]));
+            for (int q = 0; q < 2; ++q) {
+                relax(q);
                 __syncthreads();
             }
         }
@@ -127,8 +157,16 @@ __device__ __forceinline__ double tail_residual_at(const TailSmem& s, const Tail
 }
 
 // levels lev[0] .. lev[g.nl-1], by one CTA, in shared memory
+#ifdef VMG_TAIL_TIMING
+__device__ long long vmg_tail_clock[64];
+#define TAIL_MARK(i) do { if (threadIdx.x == 0) vmg_tail_clock[i] = clock64(); } while (0)
+#else
+#define TAIL_MARK(i) do { } while (0)
+#endif
+
 __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
 {
+    TAIL_MARK(0);
     extern __shared__ __align__(16) double tail_smem[];
     const int tid = threadIdx.x, nth = blockDim.x;
 
@@ -149,6 +187,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         }
     }
     __syncthreads();
+    TAIL_MARK(1);
 
     // ---- down-stroke ----
     for (int l = 0; l + 1 < g.nl; ++l) {
@@ -156,6 +195,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         const TailLevel& C = g.lev[l + 1];
         TailSmem s(tail_smem, L), c(tail_smem, C);
         tail_smooth(s, L, g.nu1);
+        TAIL_MARK(2 + 2 * l);
         for (int t = tid; t < C.n; t += nth) {     // residual + restriction (same order as residual_restrict_kernel)
             int I = t % C.nx, J = (t / C.nx) % C.ny, K = t / (C.nx * C.ny);
             double acc = 0.0;
@@ -168,6 +208,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
             c.phi[t] = 0.0;
         }
         __syncthreads();
+        TAIL_MARK(3 + 2 * l);
     }
     // ---- bottom: fixed number of sweeps from zero (R11) ----
     {
@@ -180,6 +221,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         if (!g.sym) tail_smooth(s, B, g.nbottom);
         else { tail_smooth(s, B, g.nbottom / 2, 0); tail_smooth(s, B, g.nbottom - g.nbottom / 2, 1); }
     }
+    TAIL_MARK(20);
     // ---- up-stroke ----
     for (int l = g.nl - 2; l >= 0; --l) {
         const TailLevel& L = g.lev[l];
@@ -194,7 +236,9 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
                 s.phi[t] += c.phi[(i >> 1) + C.nx * ((j >> 1) + C.ny * (g.sz == 2 ? (k >> 1) : k))];
         }
         __syncthreads();
+        TAIL_MARK(21 + 2 * l);
         tail_smooth(s, L, g.nu2, g.sym);
+        TAIL_MARK(22 + 2 * l);
     }
     // ---- stage out ----
     {
@@ -215,10 +259,13 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
             block_max_to_global(m, g.norm_out);
         }
     }
+    TAIL_MARK(40);
 }
 
 
-__global__ void __launch_bounds__(kTailThreads, 1) coarse_tail_kernel(TailArgs g)
+// NT: the largest CTA this instantiation is launched with (512 leaves the compiler 128 registers per thread)
+template <int NT>
+__global__ void __launch_bounds__(NT, 1) coarse_tail_kernel(TailArgs g)
 {
     grid_dependency_wait();
     coarse_tail_body(g);
