@@ -168,6 +168,11 @@ int vmg_destroy(vmg_handle h);
 const char* vmg_strerror(int code);       /* static string */
 int vmg_last_cuda_error(vmg_handle h);    /* cudaError_t of the last failed runtime call, 0 if none */
 
+/* Self-check: counts the non-zero elements among all pad elements of the handle's internal arrays (the zero pads that
+ * stand for the neighbours beyond the domain; no kernel may write them).  compute-sanitizer is not available on every
+ * pool; the tests call this after exercising every kernel family (tests/test_gpu_parity.py).  Synchronises the stream. */
+int vmg_debug_pad_check(vmg_handle h, long long* nonzero);
+
 /* ---------------------------------------------------------------------------------------------------------
  * Introspection and single-step entry points.  They run the very kernels vmg_solve runs, one step at a
  * time, on caller-owned DEVICE arrays of the level's size, so that tests can compare each kernel with the

@@ -17,7 +17,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "vmg_oracle.c")
-_LIB = os.path.join(_HERE, "libvmg_oracle.so")
+# VMG_ORACLE_LIB: another build of the same source (e.g. with -fsanitize=address,undefined, profiles/r2_sanitizers.md)
+_LIB = os.environ.get("VMG_ORACLE_LIB") or os.path.join(_HERE, "libvmg_oracle.so")
 
 STATUS = {0: "OK", 1: "MAXCYCLES", 2: "STALLED", -1: "ERR_ARG", -2: "ERR_SIZE", -3: "ERR_STATE",
           -4: "ERR_SINGULAR", -5: "ERR_DIVERGED"}
@@ -25,6 +26,8 @@ STATUS = {0: "OK", 1: "MAXCYCLES", 2: "STALLED", -1: "ERR_ARG", -2: "ERR_SIZE", 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain flags, no contraction, OpenMP over k-planes)."""
+    if os.environ.get("VMG_ORACLE_LIB"):
+        return _LIB
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall",
                "-o", _LIB, _SRC, "-lm"]

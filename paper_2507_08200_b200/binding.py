@@ -21,7 +21,7 @@ SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_set_mask", "vmg_so
            "vmg_destroy", "vmg_strerror", "vmg_last_cuda_error", "vmg_num_levels", "vmg_level_dims",
            "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
            "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_down", "vmg_step_up", "vmg_step_vcycle", "vmg_step_norm_inf",
-           "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile"]
+           "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile", "vmg_debug_pad_check"]
 
 _lib = None
 _vp = C.c_void_p
@@ -67,6 +67,7 @@ def load():
     lib.vmg_total_launch_count.argtypes = [_vp]
     lib.vmg_total_launch_count.restype = C.c_longlong
     lib.vmg_get_profile.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    lib.vmg_debug_pad_check.argtypes = [_vp, C.POINTER(C.c_longlong)]
     _lib = lib
     return lib
 
@@ -191,6 +192,12 @@ class Vmg:
         ms, ln = (C.c_double * 8)(), (C.c_longlong * 8)()
         self._chk(self._lib.vmg_get_profile(self._h, ms, ln), "vmg_get_profile")
         return {k: (ms[i], ln[i]) for i, k in enumerate(self.PROFILE_CLASSES)}
+
+    def pad_check(self) -> int:
+        """Non-zero elements among the zero pads of the handle's internal arrays (must be 0)."""
+        n = C.c_longlong()
+        self._chk(self._lib.vmg_debug_pad_check(self._h, C.byref(n)), "vmg_debug_pad_check")
+        return n.value
 
     # ---- introspection / single steps ---------------------------------------------------------------------
     @property

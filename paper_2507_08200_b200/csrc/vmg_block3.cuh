@@ -402,7 +402,8 @@ __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, 
 template <int S, int TAIL, int NXT, int NYT, int PF>
 struct B3rCfg {
     static constexpr int T = TAIL ? 1 : 0;
-    static constexpr int HX = 4, H = S + T;              // halo in x (tiles start on an x-pair, 32-byte aligned) and y
+    static constexpr int H = S + T;                      // halo in y
+    static constexpr int HX = H <= 4 ? 4 : (H + 1) / 2 * 2;   // halo in x: even (tiles start on an x-pair), >= 4 (32-byte aligned)
     static constexpr int ZH = S + T;
     static constexpr int TX = NXT - 2 * HX, TY = NYT - 2 * H;
     static constexpr int NXP = NXT / 2, NPH = NXP * NYT; // x-pairs per row, x-pairs per plane (= live threads)
@@ -415,7 +416,7 @@ struct B3rCfg {
     static constexpr size_t SMEM_DATA = (size_t)(NS * TSLOT + NP * PSLOT + SCRATCH) * sizeof(double);
     static constexpr size_t SMEM = SMEM_DATA + 256;      // + front pad (mbarriers)
     static constexpr uint32_t TX_BYTES = (uint32_t)(TSLOT * sizeof(double));
-    static_assert(S >= 1 && S + T <= 4 && TX > 0 && TY > 0 && TY % 2 == 0 && NXT % 4 == 0 && (ARR * 8) % 128 == 0 &&
+    static_assert(S >= 1 && S + T <= 7 && TX > 0 && TY > 0 && TY % 2 == 0 && NXT % 4 == 0 && (ARR * 8) % 128 == 0 &&
                       R >= S + 2 + T && R % 2 == 0 && PF >= 1, "tile");
 };
 

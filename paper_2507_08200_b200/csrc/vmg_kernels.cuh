@@ -275,6 +275,27 @@ __global__ void mask_count_covered_kernel(const unsigned char* __restrict__ mask
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
 }
 
+// Self-check (vmg_debug_pad_check): counts the non-zero elements among everything of a padded internal array that is not a
+// cell -- the `pad` doubles before and after it and the pad elements of every half row.  The kernels rely on these being
+// zero (they stand for the neighbours beyond the domain) and never write them; a stray store shows up here.
+__global__ void pad_check_kernel(Geom G, const double* __restrict__ arr, long long pad, unsigned long long* out)
+{
+    const long long total = 2 * pad + G.plane * G.nz;
+    unsigned long long bad = 0;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long q = t - pad;                       // index relative to cell 0
+        bool is_cell = false;
+        if (q >= 0 && q < G.plane * G.nz) {
+            const int in_row = (int)(q % G.pitch);
+            const int half = in_row / G.hp, m = in_row - half * G.hp;
+            is_cell = half == 0 ? m < G.ne : m < G.nx / 2;
+        }
+        if (!is_cell && arr[q] != 0.0) ++bad;
+    }
+    for (int o = 16; o > 0; o >>= 1) bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(out, bad);
+}
+
 // public (natural) layout <-> internal layout of one cell array
 // mask (may be NULL): covered cells enter as zero (they are identity rows of the masked operator)
 __global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in, const unsigned char* __restrict__ mask)

@@ -31,6 +31,24 @@ bool bad_level(vmg_s* h, int level) { return !h || level < 0 || level >= h->nlev
 
 extern "C" {
 
+int vmg_debug_pad_check(vmg_handle h, long long* nonzero)
+{
+    if (!h || !nonzero) return VMG_ERR_ARG;
+    unsigned long long* cnt = (unsigned long long*)h->d_scal + 9;
+    CUDA_TRY(h, cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), h->stream));
+    for (int l = 0; l < h->nlev; ++l) {
+        VmgLevel& L = h->lev[l];
+        const double* arrs[8] = {L.wx, L.wy, L.wz, L.dinv, L.dbase, L.phi, L.rhs, L.phi2};
+        for (const double* a : arrs)
+            pad_check_kernel<<<std::min<unsigned>(grid_for(L.nalloc + 2 * L.pad), 4u * h->num_sms), kThreads, 0, h->stream>>>(L.G, a, L.pad, cnt);
+    }
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaMemcpyAsync(h->h_scal + 9, cnt, sizeof(unsigned long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    *nonzero = (long long)*(unsigned long long*)(h->h_scal + 9);
+    return VMG_OK;
+}
+
 int vmg_num_levels(vmg_handle h) { return h ? h->nlev : VMG_ERR_ARG; }
 
 int vmg_level_dims(vmg_handle h, int level, int dims[3])

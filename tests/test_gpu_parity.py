@@ -140,6 +140,46 @@ def test_device_side_solve_loop_applies_the_exit_rules_of_the_host_loop(rtol, ma
         {(1e-12, 50): "converges", (0.0, 7): "fixed_cycles", (1e-12, 3): "maxcycles", (1e-17, 40): "stalls_on_the_floor", (1e-3, 50): "two_cycles"}[(rtol, maxc)]]
 
 
+@pytest.mark.parametrize("dims", [(40, 24, 16), (72, 40, 24), (5, 3, 4), (48, 40, 1)])
+def test_no_kernel_writes_the_zero_pads(dims):
+    """Own memory check (compute-sanitizer is closed on this pool, profiles/r2_sanitizers.md): the zero pads around and inside
+    every internal array stand for the neighbours beyond the domain and must never be written.  After every kernel family has
+    run on a handle -- per-colour sweeps, the three blocked designs with fused transfers, the single-CTA tail, the device-side
+    loop, plain launches, PCG, a masked solve -- not one pad element is non-zero."""
+    b = _binding()
+    p = inputs.random_problem(*dims, seed=5, bc_type=MIXED, sigma=1.0)
+    s, d = b.from_problem(p)
+    assert s.pad_check() == 0
+    rng = np.random.default_rng(2)
+    three_d = p.nz > 1
+    for opts in (dict(), dict(device_loop=0), dict(graph=0, tail=0), dict(blocked=1, block_min_cells=0),
+                 dict(blocked=2, block_min_cells=0), dict(blocked=3, block_min_cells=0), dict(prolong=1)):
+        for k, v in opts.items():
+            s.set_option(k, v)
+        phi = torch.zeros_like(d["rhs"])
+        s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=30)
+        for lev in range(s.num_levels - 1):
+            nx, ny, nz = s.level_dims(lev)
+            cnx, cny, cnz = s.level_dims(lev + 1)
+            f, r = dev(rng.standard_normal((nz, ny, nx))), dev(rng.standard_normal((nz, ny, nx)))
+            s.step_smooth(lev, f, r, 3); s.step_down(lev, f, r); s.step_up(lev, f, r, dev(rng.standard_normal((cnz, cny, cnx))))
+        assert s.pad_check() == 0, opts
+        for k in opts:
+            s.set_option(k, dict(device_loop=1, graph=1, tail=1, blocked=0, block_min_cells=4096, prolong=0)[k])
+    phi = torch.zeros_like(d["rhs"])
+    s.solve_pcg(d["rhs"], phi, 1e-12, 30)
+    assert s.pad_check() == 0
+    if three_d and min(dims) >= 8:
+        mask = torch.ones(p.rhs.shape, dtype=torch.uint8, device="cuda")
+        mask[2:5, 3:6, 1:4] = 0
+        s.set_mask(mask, D, None)
+        s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+        phi = torch.zeros_like(d["rhs"])
+        s.solve(d["rhs"], phi, rtol=1e-10, max_vcycles=60)
+        assert s.pad_check() == 0
+    s.destroy()
+
+
 @pytest.mark.parametrize("dims", [(40, 24, 16), (88, 56, 24), (144, 80, 48), (256, 128, 32)])
 def test_blocked_passes_equal_plain_launches_bitwise(dims):
     """The temporally blocked passes (with fused prolongation / restriction) relax in the same order with the
