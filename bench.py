@@ -587,6 +587,50 @@ def run_vmg(args):
         dist.destroy_process_group()
 
 
+def write_traffic_json(args):
+    """profiles/traffic.json from two ncu launch lists of the default path (`--metrics dram__bytes_read.sum,
+    dram__bytes_write.sum,gpu__time_duration.sum`; cold = ncu's default cache control, warm = --cache-control none):
+    DRAM bytes of the level-0 half-sweep launches, per nu-sweep pass of 6 launches, stamped with the commit and the hash of
+    the kernel sources so that a later bench run can tell whether the entry still describes the code it times."""
+    import csv
+    import subprocess
+    p = make_problem(args.config)
+
+    def per_launch(path):
+        per = {}
+        with open(path) as f:
+            rows = [r for r in csv.reader(f) if len(r) > 10]
+        hdr = rows[0]
+        ik, im, iv, ig, iid = (hdr.index(k) for k in ("Kernel Name", "Metric Name", "Metric Value", "Grid Size", "ID"))
+        for r in rows[1:]:
+            if "smooth_colour_kernel" in r[ik] and r[ig].replace(" ", "") == f"(1,{p.ny // 2},{p.nz})":
+                per.setdefault(r[iid], {})[r[im]] = float(r[iv].replace(",", ""))
+        vals = [v["dram__bytes_read.sum"] + v["dram__bytes_write.sum"] for v in per.values()]
+        us = [v["gpu__time_duration.sum"] / 1e3 for v in per.values()]
+        return float(np.mean(vals)), float(np.mean(us)), len(vals)
+
+    cold, cold_us, n_c = per_launch(args.traffic_from[0])
+    warm, warm_us, n_w = per_launch(args.traffic_from[1])
+    head = subprocess.run(["git", "rev-parse", "--short=12", "HEAD"], cwd=ROOT, capture_output=True, text=True).stdout.strip()
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            t = json.load(f)
+    except Exception:
+        t = {}
+    t[f"config{args.config}"] = {
+        "workload": p.name, "commit": head, "sources_sha16": kernel_sources_sha(), "sources": list(KERNEL_SOURCES),
+        "traffic_pass_cold": 6 * cold, "traffic_pass_warm": 6 * warm,
+        "per_launch": {"cold_bytes": cold, "cold_us": cold_us, "cold_launches": n_c, "warm_bytes": warm, "warm_us": warm_us, "warm_launches": n_w},
+        "note": "DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum, ncu) of the six level-0 half-sweep launches of one nu = 3 pass; "
+                "cold = every launch alone with flushed caches, warm = the L2 as the previous launch left it (--cache-control none); "
+                "algorithmic 234.9 MB per pass; commands in profiles/r2_dram.md"}
+    with open(path, "w") as f:
+        json.dump(t, f, indent=1)
+        f.write("\n")
+    print(json.dumps(t[f"config{args.config}"]))
+
+
 def run_blocked_probe(args):
     """Profiling aid (not a bench line): the level-0 strokes of the configured workload through the temporally blocked
     smoother passes (vmg_set_option blocked = 1 | 2 | 3) as separate calls, so that `ncu -k regex:smooth_block` sees the
@@ -620,11 +664,15 @@ def main():
     ap.add_argument("--no-timestep", action="store_true", help="skip the per-time-step sequence leg")
     ap.add_argument("--batch", type=int, default=8, help="K for the batched multi-component leg (0/1: skip)")
     ap.add_argument("--opt", action="append", default=[], help="vmg_set_option key=value (experiments)")
+    ap.add_argument("--traffic-from", nargs=2, metavar=("COLD_CSV", "WARM_CSV"),
+                    help="write profiles/traffic.json from two ncu launch lists (no GPU needed) and exit")
     ap.add_argument("--blocked-probe", type=int, default=0, choices=[0, 1, 2, 3],
                     help="profiling aid: run the level-0 strokes through the blocked passes of this kind and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "vmg" else args.warmup
-    if args.blocked_probe:
+    if args.traffic_from:
+        write_traffic_json(args)
+    elif args.blocked_probe:
         run_blocked_probe(args)
     elif args.impl == "reference":
         run_reference(args)
