@@ -513,6 +513,33 @@ def run_vmg(args):
                    "timing": "host clock around vmg_solve_batch, device synchronised on both sides", "statuses": sorted(set(sts))}
         for sv in bsolvers:
             sv.destroy()
+        # the same K solves with KERNEL-LEVEL batching (vmg_create_batch: one allocation, one stream; the coarser levels of all
+        # K problems as single launches over planes x problems, K CTAs in the tail; level 0 one problem at a time at this size)
+        with torch.cuda.stream(stream):
+            gs = binding.create_batch(K, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, stream=stream)
+            for sv in gs:
+                for kv in args.opt:
+                    key, val = kv.split("=")
+                    sv.set_option(key, float(val))
+                sv.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+                sv.set_bc(p.bc_type, d_bc)
+            gtimes = []
+            for it in range(1 + max(2, min(args.steps, 5))):
+                for ph in bphis:
+                    ph.zero_()
+                flush.fill_(1.0)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                gsts = binding.solve_batch(gs, [d["rhs"]] * K, bphis, rtol=p.rtol, max_vcycles=p.max_vcycles)
+                torch.cuda.synchronize()
+                if it > 0:
+                    gtimes.append(time.perf_counter() - t0)
+            gt = float(np.mean(gtimes))
+            batched["kernel_level"] = {"solves_per_s": world * K / gt, "ms_per_batch": gt * 1e3, "statuses": sorted(set(gsts)),
+                                       "hbm_frac": K * (bcyc * wm["bytes_per_cycle"] + wm["bytes_solve_fixed"]) / gt / 1e9 / peak,
+                                       "note": "vmg_create_batch group; at this size level 0 runs one problem at a time (L2 reuse), levels 1.. problem-major"}
+            for sv in gs:
+                sv.destroy()
 
     # one time step of the paper's scheme (Eq. 9-10): Poisson, 15
     # species, electron energy and three photoionisation Helmholtz solves, each vmg_set_coeffs + vmg_set_bc +

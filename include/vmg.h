@@ -105,6 +105,18 @@ int vmg_set_mask(vmg_handle h, const unsigned char* mask, int kind, const double
  * PAPER.md:159; cycle, smoother, transfers and exit rules are readings C1-C5 / R7-R13 of DESIGN.md section 2. */
 int vmg_solve(vmg_handle h, const double* rhs, double* phi, double rtol, int max_vcycles);
 
+/* K handles for K problems on the same grid -- the paper's "multi-component" multigrid solves (section 7:
+ * solving several solution components with each multigrid solve "results in more GPU work" per launch).  Same arguments as
+ * vmg_create; out: HOST array of k handles.  The members share ONE device allocation (member i's arrays lie a constant
+ * stride after member 0's) and one stream (cuda_stream, or one the library creates).  Each member is an ordinary handle for
+ * every other call (own coefficients, boundary data, options, vmg_solve, vmg_destroy -- the allocation goes with the last
+ * member).  vmg_solve_batch on exactly these k handles advances them with KERNEL-LEVEL batching: level 0 one problem after
+ * the other (its consecutive half-sweeps reuse the L2), every coarser level of all k problems in single launches that run
+ * over planes x problems, k CTAs in the single-CTA tail, one graph; bitwise the results of k separate vmg_solve calls.
+ * That path needs equal smoothing options on all members, piecewise-constant prolongation, blocked = 0 and (for b == NULL)
+ * equal beta; otherwise vmg_solve_batch falls back to its stream-level schedule. */
+int vmg_create_batch(int k, vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream);
+
 /* Batched solve (the paper's "multi-component" optimisation: "simultaneously solving multiple scalar solution
  * components with each multigrid solve results in more GPU work").  n independent
  * problems, one handle each -- same or different grids, coefficients and boundary conditions -- advanced in
@@ -158,6 +170,11 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  *   ring with one split mbarrier per plane, 2 x 2 patch per thread, 3 = the same with one row per thread (vmg_block3.cuh);
  *   0: one kernel per colour half-sweep, default -- the blocked passes are bitwise equal but measure slower on B200),
  * "block_min_cells" (smallest level the blocked passes are used on when blocked = 1, default 4096),
+ * "batch_full_mb" (set on member 0 of a vmg_create_batch group: while all members still iterate and k x 56 B x cells stays
+ *   below this many MB, vmg_solve_batch runs ALL levels of the group problem-major in one graph, above it only the coarser
+ *   levels and level 0 one problem after the other; default 400: measured on B200, k = 8: 64x32x32 4449 solves/s (1292
+ *   sequential, 2579 stream-level), 128x64x64 1558 (921, 1636), 256x128x128 278 with level 0 sequential against 266 with
+ *   everything batched -- eight 235 MB working sets defeat the L2 reuse of the half-sweeps -- (270, 303)),
  * "const_weights" (1: use the constant-weight kernels when b == NULL, default; 0: always load the weight arrays; takes
  *   effect at the next vmg_set_coeffs, which must follow),
  * "profile" (1: per-kernel-class event timing, see vmg_get_profile; implies plain launches; default 0). */

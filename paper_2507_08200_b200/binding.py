@@ -17,7 +17,7 @@ STATUS = {0: "OK", 1: "MAXCYCLES", 2: "STALLED", -1: "ERR_ARG", -2: "ERR_SIZE", 
           -4: "ERR_SINGULAR", -5: "ERR_DIVERGED", -6: "ERR_CUDA", -7: "ERR_ALLOC"}
 
 # every symbol include/vmg.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["vmg_create", "vmg_set_coeffs", "vmg_set_bc", "vmg_set_mask", "vmg_solve", "vmg_solve_batch", "vmg_solve_pcg", "vmg_get_info", "vmg_set_option",
+SYMBOLS = ["vmg_create", "vmg_create_batch", "vmg_set_coeffs", "vmg_set_bc", "vmg_set_mask", "vmg_solve", "vmg_solve_batch", "vmg_solve_pcg", "vmg_get_info", "vmg_set_option",
            "vmg_destroy", "vmg_strerror", "vmg_last_cuda_error", "vmg_num_levels", "vmg_level_dims",
            "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
            "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_down", "vmg_step_up", "vmg_step_vcycle", "vmg_step_norm_inf",
@@ -37,6 +37,7 @@ def load():
                            "(there is no CPU fallback)")
     lib = C.CDLL(LIB_PATH)
     lib.vmg_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _vp]
+    lib.vmg_create_batch.argtypes = [C.c_int, C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _vp]
     lib.vmg_set_coeffs.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_double, C.c_double]
     lib.vmg_set_bc.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(_vp)]
     lib.vmg_set_mask.argtypes = [_vp, _vp, C.c_int, _vp]
@@ -112,19 +113,36 @@ def solve_batch(solvers, rhs, phi, rtol: float = 1e-12, max_vcycles: int = 50) -
     return out
 
 
+def create_batch(k: int, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, stream=None):
+    """vmg_create_batch: k handles in one allocation on one stream; solve_batch on exactly these runs the coarser levels of
+    all of them as single launches (kernel-level batching).  Returns a list of Vmg."""
+    torch = _torch()
+    lib = load()
+    stream = stream if stream is not None else torch.cuda.current_stream()
+    sptr = stream.cuda_stream
+    hs = (_vp * k)()
+    rc = lib.vmg_create_batch(k, hs, nx, ny, nz, dx, dy, dz, _vp(sptr) if sptr else None)
+    if rc != 0:
+        raise VmgError(rc, "vmg_create_batch")
+    return [Vmg(nx, ny, nz, dx, dy, dz, stream=stream, _handle=_vp(hs[i])) for i in range(k)]
+
+
 class Vmg:
     """One solver handle (vmg_create ... vmg_destroy). Method names follow include/vmg.h."""
 
-    def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, stream=None):
+    def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, stream=None, _handle=None):
         torch = _torch()
         self._lib = load()
         self._h = _vp()
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         sptr = self.stream.cuda_stream
-        rc = self._lib.vmg_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, _vp(sptr) if sptr else None)
-        if rc != 0:
-            self._h = None
-            raise VmgError(rc, "vmg_create")
+        if _handle is not None:          # a member of a vmg_create_batch group (create_batch below)
+            self._h = _handle
+        else:
+            rc = self._lib.vmg_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, _vp(sptr) if sptr else None)
+            if rc != 0:
+                self._h = None
+                raise VmgError(rc, "vmg_create")
         self.nx, self.ny, self.nz = nx, ny, nz
         self.device = torch.device("cuda", torch.cuda.current_device())
 

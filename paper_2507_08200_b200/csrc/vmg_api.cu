@@ -166,7 +166,14 @@ const char* vmg_strerror(int code)
     }
 }
 
-int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream)
+}  // extern "C"
+
+namespace {
+
+// slice: nullptr = allocate an arena of this handle's own; otherwise the handle lives in [slice, slice + slice_bytes)
+// (vmg_create_batch) and *need receives the bytes one handle needs when slice_bytes is too small (then nothing is created)
+int create_impl(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream,
+                void* slice, size_t slice_bytes, size_t* need)
 {
     if (!out) return VMG_ERR_ARG;
     *out = nullptr;
@@ -206,7 +213,14 @@ int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, do
         h->own_stream = true;
     }
     h->arena_bytes = layout(h, nullptr) * sizeof(double);
-    if (cudaMalloc(&h->arena, h->arena_bytes) != cudaSuccess) {
+    if (need) *need = h->arena_bytes;
+    if (slice && slice_bytes >= h->arena_bytes) { h->arena = slice; h->own_arena = false; }
+    else if (slice || need) {   // measuring pass of vmg_create_batch
+        if (h->own_stream) cudaStreamDestroy(h->stream);
+        delete h;
+        return slice ? VMG_ERR_ALLOC : VMG_OK;
+    }
+    else if (cudaMalloc(&h->arena, h->arena_bytes) != cudaSuccess) {
         (void)cudaGetLastError();
         if (h->own_stream) cudaStreamDestroy(h->stream);
         delete h;
@@ -218,13 +232,64 @@ int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, do
         cudaMallocHost((void**)&h->h_loop, (8 + kLoopMaxCycles + 1) * sizeof(double)) != cudaSuccess ||
         cudaStreamSynchronize(h->stream) != cudaSuccess) {
         (void)cudaGetLastError();
-        cudaFree(h->arena);
+        if (h->own_arena) cudaFree(h->arena);
         if (h->own_stream) cudaStreamDestroy(h->stream);
         delete h;
         return VMG_ERR_CUDA;
     }
     plan_schedule(h);
     *out = h;
+    return VMG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int vmg_create(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream)
+{
+    return create_impl(out, nx, ny, nz, dx, dy, dz, cuda_stream, nullptr, 0, nullptr);
+}
+
+// K handles for K problems on the same grid (the paper's multi-component solves), in ONE allocation with a
+// constant stride between the members' arenas and on one stream: vmg_solve_batch on exactly these handles then runs the
+// coarser levels of all of them as single launches (kernel-level batching); each handle is otherwise an ordinary handle.
+int vmg_create_batch(int k, vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream)
+{
+    if (k < 1 || !out) return VMG_ERR_ARG;
+    for (int i = 0; i < k; ++i) out[i] = nullptr;
+    size_t need = 0;
+    vmg_handle probe = nullptr;
+    int rc = create_impl(&probe, nx, ny, nz, dx, dy, dz, cuda_stream, nullptr, 0, &need);   // sizes only
+    if (rc != VMG_OK) return rc;
+    VmgBatchGroup* G = new (std::nothrow) VmgBatchGroup();
+    if (!G) return VMG_ERR_ALLOC;
+    G->stride_bytes = round_up(need, 256);
+    if (cudaMalloc(&G->base, G->stride_bytes * (size_t)k) != cudaSuccess) { (void)cudaGetLastError(); delete G; return VMG_ERR_ALLOC; }
+    cudaStream_t shared = (cudaStream_t)cuda_stream;
+    bool own = false;
+    if (!shared) {
+        if (cudaStreamCreate(&shared) != cudaSuccess) { (void)cudaGetLastError(); cudaFree(G->base); delete G; return VMG_ERR_CUDA; }
+        own = true;
+    }
+    for (int i = 0; i < k && rc == VMG_OK; ++i) {
+        rc = create_impl(&out[i], nx, ny, nz, dx, dy, dz, (void*)shared, (char*)G->base + (size_t)i * G->stride_bytes, G->stride_bytes, nullptr);
+        if (rc == VMG_OK) {
+            out[i]->group = G; out[i]->group_index = i;
+            out[i]->own_stream = own && i == 0;      // member 0 owns a stream the library created; it is destroyed with the group
+            G->members.push_back(out[i]);
+            ++G->refs;
+        }
+    }
+    if (rc != VMG_OK) {
+        for (int i = 0; i < k; ++i) if (out[i]) { out[i]->own_stream = false; out[i]->group = nullptr; vmg_destroy(out[i]); out[i] = nullptr; }
+        if (own) cudaStreamDestroy(shared);
+        cudaFree(G->base);
+        delete G;
+        return rc;
+    }
+    G->coarse_epochs.assign((size_t)k, 0u);
+    G->full_epochs.assign((size_t)k, 0u);
     return VMG_OK;
 }
 
@@ -262,8 +327,22 @@ int vmg_destroy(vmg_handle h)
     if (h->coarse_stream) cudaStreamDestroy(h->coarse_stream);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->h_loop) cudaFreeHost(h->h_loop);
-    if (h->arena) cudaFree(h->arena);
-    if (h->own_stream) cudaStreamDestroy(h->stream);
+    if (h->arena && h->own_arena) cudaFree(h->arena);
+    VmgBatchGroup* G = h->group;
+    if (G) {   // the group's allocation, graph and (if the library created it) stream go with the last member
+        for (auto& m : G->members) if (m == h) m = nullptr;
+        if (G->coarse_exec) { cudaGraphExecDestroy(G->coarse_exec); G->coarse_exec = nullptr; }
+        if (G->coarse_graph) { cudaGraphDestroy(G->coarse_graph); G->coarse_graph = nullptr; }
+        if (G->full_exec) { cudaGraphExecDestroy(G->full_exec); G->full_exec = nullptr; }
+        if (G->full_graph) { cudaGraphDestroy(G->full_graph); G->full_graph = nullptr; }
+        if (h->own_stream) G->owned_stream = h->stream;
+        if (--G->refs == 0) {
+            cudaFree(G->base);
+            if (G->owned_stream) cudaStreamDestroy(G->owned_stream);
+            delete G;
+        }
+    }
+    else if (h->own_stream) cudaStreamDestroy(h->stream);
     (void)cudaGetLastError();
     delete h;
     return VMG_OK;
@@ -427,6 +506,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "device_loop")) { h->use_loop = iv != 0; }
     else if (!strcmp(key, "snake")) { h->snake = iv != 0; }
     else if (!strcmp(key, "pdl")) { h->use_pdl = iv != 0; }
+    else if (!strcmp(key, "batch_full_mb")) { if (v < 0) return VMG_ERR_ARG; h->batch_full_mb = v; }
     else if (!strcmp(key, "block_min_cells")) { if (v < 0) return VMG_ERR_ARG; h->block_min_cells = (long long)v; }
     else if (!strcmp(key, "phi_keep_cells")) { if (v < 0) return VMG_ERR_ARG; h->phi_keep_cells = (long long)v; }
     else if (!strcmp(key, "l2_persist")) { if (v < 0) return VMG_ERR_ARG; h->l2_persist_mb = v; h->l2_applied = false; }
@@ -787,6 +867,45 @@ int vmg_solve_batch(int n, const vmg_handle* hs, const double* const* rhs, doubl
         bool seg_ok = true;
         for (int i = 0; i < n; ++i)
             if (rc[i] == VMG_OK && hs[i]->sv_active) { ++nact; seg_ok = seg_ok && vcycle_segmentable(hs[i]); }
+        // Kernel-level batching: the handles are exactly the members of one vmg_create_batch group (one allocation, one
+        // stream).  Level 0 one problem after the other (its half-sweeps keep their L2 reuse), the coarser levels of ALL
+        // members as single launches over planes x problems with K CTAs in the tail (run_group_coarse); problems that have
+        // finished are simply not given their level-0 strokes any more (their coarse levels are recomputed, unused).
+        VmgBatchGroup* G = n >= 2 && hs[0] ? hs[0]->group : nullptr;
+        bool fused = G && (int)G->members.size() == n && nact >= 2 && seg_ok;
+        for (int i = 0; fused && i < n; ++i) fused = rc[i] == VMG_OK && hs[i]->group == G;
+        fused = fused && group_coarse_ok(G) && (long long)G->members[0]->lev[1].nz * n <= 65535;
+        if (fused && nact == n && group_full_ok(G)) {
+            // every problem still iterates and the K fine levels together fit the L2: ALL levels problem-major, one graph
+            const int rcg = run_group_full(G);
+            for (int i = 0; i < n; ++i) {
+                vmg_s* h = hs[i];
+                unsigned long long* scal = (unsigned long long*)h->d_scal;
+                rc[i] = rcg;
+                h->launches += G->full_launches;
+                h->launches_per_cycle = G->full_launches;
+                if (rc[i] == VMG_OK && cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) rc[i] = VMG_ERR_CUDA;
+                any = true;
+            }
+        } else
+        if (fused) {
+            for (int i = 0; i < n; ++i) {
+                vmg_s* h = hs[i];
+                if (!h->sv_active) continue;
+                rc[i] = run_vcycle_segment(h, 0, (unsigned long long*)h->d_scal + 1);
+            }
+            const int rcg = run_group_coarse(G);
+            for (int i = 0; i < n; ++i) {
+                vmg_s* h = hs[i];
+                if (rc[i] != VMG_OK || !h->sv_active) continue;
+                if (rcg != VMG_OK) { rc[i] = rcg; continue; }
+                unsigned long long* scal = (unsigned long long*)h->d_scal;
+                rc[i] = run_vcycle_segment(h, 2, scal + 1);
+                h->launches += G->coarse_launches - h->seg_launches[h->lev[0].cw][1];   // the group's coarse launches in place of its own
+                if (rc[i] == VMG_OK && cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) rc[i] = VMG_ERR_CUDA;
+                any = true;
+            }
+        } else
         if (nact >= 2 && seg_ok) {
             cudaEvent_t prev = nullptr;
             for (int pass = 0; pass < 2; ++pass)

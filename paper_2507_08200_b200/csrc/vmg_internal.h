@@ -52,9 +52,35 @@ struct VmgLevel {
     const unsigned char* mk = nullptr;      // cw == 2: the open faces of every cell, one byte, internal layout
     double* adiag = nullptr;  // masking: extra diagonal of this level, public layout (nullptr without a mask)
     std::vector<VmgTensorMap> tmaps;   // TMA descriptors of this level's arrays (blocked smoother, vmg_block3.cuh)
+    // set only while the batched coarse segment of a vmg_create_batch group is being captured (vmg_sched.cuh): the launches of
+    // this level then run over nprob problems whose arrays lie pstride doubles apart
+    int nprob = 1;
+    long long pstride = 0;
+};
+
+struct vmg_s;
+
+// K handles created together (vmg_create_batch): one arena allocation, member k's arena k * stride bytes after member 0's,
+// one stream.  The coarser levels of all members run as single launches (kernel-level batching).
+struct VmgBatchGroup {
+    void* base = nullptr;
+    size_t stride_bytes = 0;
+    int refs = 0;
+    std::vector<vmg_s*> members;
+    cudaGraph_t coarse_graph = nullptr;          // levels 1.. of ALL members: strokes + tail, problem-major launches
+    cudaGraphExec_t coarse_exec = nullptr;
+    std::vector<unsigned> coarse_epochs;         // the members' graph epochs the graph was captured at
+    long long coarse_launches = 0;
+    cudaGraph_t full_graph = nullptr;            // all levels of ALL members + their residual norms (small grids: K working sets share the L2)
+    cudaGraphExec_t full_exec = nullptr;
+    std::vector<unsigned> full_epochs;
+    long long full_launches = 0;
+    cudaStream_t owned_stream = nullptr;         // a stream the library created for the group (destroyed with the last member)
 };
 
 struct vmg_s {
+    VmgBatchGroup* group = nullptr;
+    int group_index = 0;
     int nlev = 0;
     bool three_d = true;
     std::vector<VmgLevel> lev;
@@ -84,12 +110,14 @@ struct vmg_s {
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
     size_t tail_smem = 0;         // dynamic shared memory of the tail kernel
     long long block_min_cells = 4096;   // smallest level the blocked smoother is used on
+    double batch_full_mb = 400.0;  // option "batch_full_mb" (member 0 of a vmg_create_batch group): all levels batched while K fine levels (56 B/cell) stay below this
     // device scalars
     double* d_scal = nullptr;     // [0] = ||btilde||_inf bits, [1] = residual norm bits, ...
     double* h_scal = nullptr;     // pinned host mirror
     // arena
     void* arena = nullptr;
     size_t arena_bytes = 0;
+    bool own_arena = true;        // false: a slice of a vmg_create_batch allocation
     // graph of one V-cycle (+ residual norm)
     // one slot per kind of level-0 kernels (LevelView::cw), so that a time step that alternates
     // between the two kinds of equation re-instantiates nothing; a slot is current when its epoch equals graph_epoch

@@ -398,7 +398,21 @@ struct LevelView {
     double cx, cy, cz;
     int cw;
     const unsigned char* mk;
+    // batched multi-component launches: nprob problems with identical grids whose arenas lie
+    // pstride doubles apart (vmg_create_batch); the launch's blockIdx.z runs over planes x problems, problem-major, and every
+    // array of problem kb is the first problem's array shifted by kb * pstride.  0: a single problem.
+    long long pstride;
+    int nprob;
 };
+
+// plane and problem of a batched launch: k = blockIdx.z -> (k % nz, offset of the problem's arrays)
+__device__ __forceinline__ long long batch_split(const LevelView& L, int nz, int& k)
+{
+    if (!L.pstride) return 0;
+    const int kb = k / nz;
+    k -= kb * nz;
+    return (long long)kb * L.pstride;
+}
 
 // the six face weights of cell (i, j, k): low x, high x, low y, high y, low z, high z
 template <int CW>
@@ -448,13 +462,13 @@ __device__ __forceinline__ void pair_addr(const Geom& G, long long row, int m, i
 // KEEP = 1 (option "phi_keep_cells"): the neighbours' phi with the normal policy -- on levels far larger than the L2 the
 // evict-first lines are gone before the next row and plane ask for them (512^3: 12 % more DRAM traffic than algorithmic).
 template <int CW, int KEEP = 0>
-__device__ __forceinline__ void relax_at(const LevelView& L, double* phi, const double* rhs, int colour, int m, int j, int k)
+__device__ __forceinline__ void relax_at(const LevelView& L, double* phi, const double* rhs, int colour, int m, int j, int k, long long off = 0)
 {
     const Geom& G = L.G;
     int par = (colour + j + k) & 1;
     if (2 * m + par >= G.nx) return;
     long long c, xm;
-    pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
+    pair_addr(G, off + G.plane * k + (long long)G.pitch * j, m, par, c, xm);
     double w[6];
     face_weights<CW>(L, c, xm, 2 * m + par, j, k, w);
     auto ld = [](const double* q) { return KEEP ? *q : __ldcs(q); };
@@ -476,8 +490,9 @@ __global__ void smooth_colour_kernel(LevelView L, double* __restrict__ phi, cons
     grid_dependency_wait();
     // grid (x-pair blocks, row blocks, planes), block (x-pairs, rows): no division to find the cell (pair_launch_dims)
     int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    const long long off = batch_split(L, L.G.nz, k);
     if (reverse) { k = L.G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
-    if (m < L.G.ne && j < L.G.ny) relax_at<CW, KEEP>(L, phi, rhs, colour, m, j, k);
+    if (m < L.G.ne && j < L.G.ny) relax_at<CW, KEEP>(L, phi, rhs, colour, m, j, k, off);
 }
 
 __device__ __forceinline__ void block_max_to_global(double v, unsigned long long* out);
@@ -561,20 +576,20 @@ __global__ void solve_decide_kernel(cudaGraphConditionalHandle handle, double* s
 template <int CW>
 __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom& CG, double* phi,
                                                   const double* rhs, const double* e, int colour, int sz,
-                                                  int m, int j, int k)
+                                                  int m, int j, int k, long long off = 0)
 {
     const Geom& G = L.G;
     int par = (colour + j + k) & 1;
     int i = 2 * m + par;
     if (i >= G.nx) return;
     long long c, xm;
-    pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
+    pair_addr(G, off + G.plane * k + (long long)G.pitch * j, m, par, c, xm);
     const int K = sz == 2 ? (k >> 1) : k;
     // In every direction one neighbour has this cell's own coarse parent and the other the adjacent coarse cell (on the
     // low side for an even fine index, on the high side for an odd one): four coarse values, not six.
     const int I = i >> 1;
     long long cP, xP;
-    pair_addr(CG, CG.plane * K + (long long)CG.pitch * (j >> 1), I >> 1, I & 1, cP, xP);
+    pair_addr(CG, off + CG.plane * K + (long long)CG.pitch * (j >> 1), I >> 1, I & 1, cP, xP);
     const double eP = e[cP];
     const double eX = (i & 1) ? e[xP + 1] : e[xP];                                  // zero pad beyond the x faces: not used there
     const double eY = (j & 1) ? e[cP + CG.pitch] : e[cP - CG.pitch];
@@ -608,8 +623,9 @@ __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __res
 {
     grid_dependency_wait();
     int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;   // pair_launch_dims
+    const long long off = batch_split(L, L.G.nz, k);
     if (reverse) { k = L.G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
-    if (m < L.G.ne && j < L.G.ny) relax_prolong_one<CW>(L, CG, phi, rhs, e, colour, sz, m, j, k);
+    if (m < L.G.ne && j < L.G.ny) relax_prolong_one<CW>(L, CG, phi, rhs, e, colour, sz, m, j, k, off);
 }
 
 // r = rhs - A phi, A phi = D phi - sum w phi_nb, D = 1/dinv.
@@ -659,18 +675,18 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 template <int CW>
 __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG, const double* phi,
                                              const double* rhs, double* crhs, double* cphi,
-                                             int sz, int I, int J, int K)
+                                             int sz, int I, int J, int K, long long off = 0)
 {
     double s = 0.0;
     for (int r = 0; r < sz; ++r)
         for (int q = 0; q < 2; ++q) {   // the x-pair first, then accumulated (the blocked kernel sums in this order too)
             const int j = 2 * J + q, k = sz * K + r;
-            long long row = L.G.plane * k + (long long)L.G.pitch * j, ce, xe, co, xo;
+            long long row = off + L.G.plane * k + (long long)L.G.pitch * j, ce, xe, co, xo;
             pair_addr(L.G, row, I, 0, ce, xe);
             pair_addr(L.G, row, I, 1, co, xo);
             s += residual_at<CW, CW ? 0 : 2>(L, phi, rhs, ce, xe, 2 * I, j, k) + residual_at<CW, CW ? 0 : 2>(L, phi, rhs, co, xo, 2 * I + 1, j, k);   // rhs, 1/D streamed
         }
-    const long long cc = cell_at(CG, I, J, K);
+    const long long cc = off + cell_at(CG, I, J, K);
     crhs[cc] = s / (4.0 * sz);
     if (cphi) cphi[cc] = 0.0;
 }
@@ -682,8 +698,9 @@ __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __r
     grid_dependency_wait();
     // grid (coarse x blocks, coarse row blocks, coarse planes), block (coarse x, coarse rows): cell_launch_dims of the coarse level
     int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
+    const long long off = batch_split(L, CG.nz, K);
     if (reverse) { K = CG.nz - 1 - K; J = gridDim.y * blockDim.y - 1 - J; }
-    if (I < CG.nx && J < CG.ny) restrict_one<CW>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K);
+    if (I < CG.nx && J < CG.ny) restrict_one<CW>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off);
 }
 
 // S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise
@@ -804,15 +821,23 @@ __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi
     const Geom& G = L.G;
     // grid (x-pair blocks, row blocks, planes * colours), block (x-pairs, rows): pair_launch_dims, z extended by the colour
     int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
-    int k = (int)blockIdx.z % G.nz;
-    const int colour = (int)blockIdx.z / G.nz;
+    int z = (int)blockIdx.z;
+    long long off = 0;
+    if (L.pstride) {                                  // batched: blockIdx.z = (problem, colour, plane), problem-major
+        const int span = (int)gridDim.z / L.nprob, kb = z / span;
+        z -= kb * span;
+        off = (long long)kb * L.pstride;
+        out += off;                                   // the members' scalars lie the same stride apart (8-byte units)
+    }
+    int k = z % G.nz;
+    const int colour = z / G.nz;
     if (reverse) { k = G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
     double mx = 0.0;
     if (m < G.ne && j < G.ny) {
         int par = (colour + j + k) & 1;
         if (2 * m + par < G.nx) {
             long long c, xm;
-            pair_addr(G, G.plane * k + (long long)G.pitch * j, m, par, c, xm);
+            pair_addr(G, off + G.plane * k + (long long)G.pitch * j, m, par, c, xm);
             mx = fabs(residual_at<CW, CW ? 0 : KEEP ? 2 : 1>(L, phi, rhs, c, xm, 2 * m + par, j, k));   // constant weights: the level fits L2, keep it there
             if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
         }

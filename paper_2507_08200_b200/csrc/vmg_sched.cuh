@@ -23,6 +23,7 @@ inline LevelView view(const VmgLevel& L)
     v.wx = L.wx; v.wy = L.wy; v.wz = L.wz; v.dinv = L.dinv;
     v.G = L.G;
     v.cx = L.cx; v.cy = L.cy; v.cz = L.cz; v.cw = L.cw; v.mk = L.mk;
+    v.pstride = L.pstride; v.nprob = L.nprob;
     return v;
 }
 
@@ -44,7 +45,7 @@ inline void pair_launch_dims(const VmgLevel& L, dim3& grid, dim3& block)
 {
     const int bx = std::min(128, 32 * ((L.G.ne + 31) / 32)), by = kThreads / bx;
     block = dim3(bx, by, 1);
-    grid = dim3((L.G.ne + bx - 1) / bx, (L.ny + by - 1) / by, L.nz);
+    grid = dim3((L.G.ne + bx - 1) / bx, (L.ny + by - 1) / by, L.nz * L.nprob);   // batched capture: planes x problems
 }
 
 // direction of the next whole-level kernel: consecutive kernels walk the level in opposite directions (L2 reuse)
@@ -160,6 +161,7 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
     C.cur = 0;
     dim3 grid, block;
     cell_launch_dims(C.G, grid, block);
+    grid.z *= L.nprob;
     launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_kernel), grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
                h->three_d ? 2 : 1, next_dir(h, L));
     ++*count;
@@ -251,11 +253,13 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
     g.prolong = h->prolong; g.bc = prolong_bc(h); g.sym = h->symmetric;
     g.whole = first == 0;
     g.norm_out = first == 0 ? norm_out : nullptr;
+    g.pstride = h->lev[first].pstride;
+    const int ncta = h->lev[first].nprob;
     ProfScope ps(h, VMG_PC_COARSE, count);
     {
         int threads = (int)std::min<long long>(kTailThreads, std::max<long long>(64, (h->lev[first].n / 2 + 31) / 32 * 32));
-        if (threads <= 512) launch_pdl(h, coarse_tail_kernel<512>, 1, threads, h->tail_smem, g);
-        else launch_pdl(h, coarse_tail_kernel<kTailThreads>, 1, threads, h->tail_smem, g);
+        if (threads <= 512) launch_pdl(h, coarse_tail_kernel<512>, ncta, threads, h->tail_smem, g);
+        else launch_pdl(h, coarse_tail_kernel<kTailThreads>, ncta, threads, h->tail_smem, g);
     }
     ++*count;
 }
@@ -847,6 +851,101 @@ inline int run_solve_loop(vmg_s* h, unsigned long long* norm_out)
     if (e == cudaSuccess) e = cudaGraphLaunch(h->loop_exec[gi], h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h->h_loop, h->d_loop, (size_t)(8 + max + 1) * sizeof(double), cudaMemcpyDeviceToHost, h->stream);
     if (e != cudaSuccess) return fail(e);
+    return VMG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// N1, kernel level: the coarser levels (segment 1 of the cycle) of ALL members of a vmg_create_batch group as one graph
+// whose launches run over planes x problems (LevelView::pstride), K CTAs in the tail.  Level 0 stays one problem at a
+// time (segments 0 and 2 of each member), which keeps the L2 reuse between its consecutive half-sweeps.
+// ------------------------------------------------------------------------------------------------
+inline bool group_coarse_ok(const VmgBatchGroup* G)
+{
+    const vmg_s* a = G->members[0];
+    if (!vcycle_segmentable(a) || a->use_blocked || a->prolong || a->nu2 < 1) return false;
+    for (const vmg_s* h : G->members) {
+        if (!h->have_coeffs || !h->have_bc || !vcycle_segmentable(h)) return false;
+        if (h->nu1 != a->nu1 || h->nu2 != a->nu2 || h->nbottom != a->nbottom || h->prolong != a->prolong || h->symmetric != a->symmetric ||
+            h->use_tail != a->use_tail || h->tail_level != a->tail_level || h->use_pdl != a->use_pdl || h->snake != a->snake ||
+            h->use_blocked != a->use_blocked)
+            return false;
+        for (int l = 1; l < h->nlev; ++l) {
+            const VmgLevel &x = h->lev[l], &y = a->lev[l];
+            if (x.cw != y.cw || (x.cw && (x.cx != y.cx || x.cy != y.cy || x.cz != y.cz))) return false;   // constant weights go by value
+        }
+    }
+    return true;
+}
+
+// every level of ALL members in one graph (all problems still iterating and K level-0 working sets small enough to share
+// the L2): the whole V-cycle + the K residual norms as problem-major launches
+inline bool group_full_ok(const VmgBatchGroup* G)
+{
+    const vmg_s* a = G->members[0];
+    const long long K = (long long)G->members.size();
+    if ((double)K * a->lev[0].n * 56.0 > a->batch_full_mb * 1048576.0 || (long long)a->lev[0].nz * K * 2 > 65535) return false;
+    for (const vmg_s* h : G->members) {
+        const VmgLevel &x = h->lev[0], &y = a->lev[0];
+        if (h->d_mask || x.cw != y.cw || (x.cw && (x.cx != y.cx || x.cy != y.cy || x.cz != y.cz))) return false;
+    }
+    return true;
+}
+
+inline int run_group_full(VmgBatchGroup* G)
+{
+    vmg_s* h = G->members[0];
+    const int K = (int)G->members.size();
+    bool stale = G->full_exec == nullptr;
+    for (int i = 0; i < K; ++i) stale = stale || G->full_epochs[i] != G->members[i]->graph_epoch;
+    if (stale) {
+        if (G->full_exec) { cudaGraphExecDestroy(G->full_exec); G->full_exec = nullptr; }
+        if (G->full_graph) { cudaGraphDestroy(G->full_graph); G->full_graph = nullptr; }
+        const long long stride = (long long)(G->stride_bytes / sizeof(double));
+        for (int l = 0; l < h->nlev; ++l) { h->lev[l].nprob = K; h->lev[l].pstride = stride; }
+        long long count = 0;
+        unsigned long long* out0 = (unsigned long long*)h->d_scal + 1;
+        cudaError_t e = cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeRelaxed);
+        if (e == cudaSuccess) {
+            for (int i = 1; i < K; ++i) cudaMemsetAsync(out0 + (long long)i * stride, 0, sizeof(unsigned long long), h->stream);
+            enqueue_vcycle(h, out0, &count);
+            e = cudaStreamEndCapture(h->stream, &G->full_graph);
+        }
+        for (int l = 0; l < h->nlev; ++l) { h->lev[l].nprob = 1; h->lev[l].pstride = 0; }
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&G->full_exec, G->full_graph, 0);
+        if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
+        G->full_launches = count;
+        for (int i = 0; i < K; ++i) G->full_epochs[i] = G->members[i]->graph_epoch;
+    }
+    cudaError_t e = cudaGraphLaunch(G->full_exec, h->stream);
+    if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
+    return VMG_OK;
+}
+
+inline int run_group_coarse(VmgBatchGroup* G)
+{
+    vmg_s* h = G->members[0];
+    bool stale = G->coarse_exec == nullptr;
+    for (size_t i = 0; i < G->members.size(); ++i) stale = stale || G->coarse_epochs[i] != G->members[i]->graph_epoch;
+    if (stale) {
+        if (G->coarse_exec) { cudaGraphExecDestroy(G->coarse_exec); G->coarse_exec = nullptr; }
+        if (G->coarse_graph) { cudaGraphDestroy(G->coarse_graph); G->coarse_graph = nullptr; }
+        const int K = (int)G->members.size();
+        for (int l = 0; l < h->nlev; ++l) h->lev[l].cur = 0;
+        for (int l = 1; l < h->nlev; ++l) { h->lev[l].nprob = K; h->lev[l].pstride = (long long)(G->stride_bytes / sizeof(double)); }
+        long long count = 0;
+        cudaError_t e = cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeRelaxed);
+        if (e == cudaSuccess) {
+            enqueue_vcycle_segment(h, 1, nullptr, &count);
+            e = cudaStreamEndCapture(h->stream, &G->coarse_graph);
+        }
+        for (int l = 1; l < h->nlev; ++l) { h->lev[l].nprob = 1; h->lev[l].pstride = 0; }
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&G->coarse_exec, G->coarse_graph, 0);
+        if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
+        G->coarse_launches = count;
+        for (size_t i = 0; i < G->members.size(); ++i) G->coarse_epochs[i] = G->members[i]->graph_epoch;
+    }
+    cudaError_t e = cudaGraphLaunch(G->coarse_exec, h->stream);
+    if (e != cudaSuccess) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; }
     return VMG_OK;
 }
 

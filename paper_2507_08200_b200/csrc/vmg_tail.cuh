@@ -29,6 +29,7 @@ struct TailArgs {
     ProlongBC bc;              // boundary types (trilinear ghosts)
     int whole;                 // 1: lev[0] is level 0 of the hierarchy (phi is an initial guess, not zero)
     unsigned long long* norm_out;   // whole == 1: ||rhs - A phi||_inf bits after the cycle (may be NULL)
+    long long pstride;         // batched launch (one CTA per problem): the arrays of problem blockIdx.x lie blockIdx.x * pstride doubles on
 };
 
 // shared-memory block of a level: six arrays (phi, rhs, dinv, wx, wy, wz), each `guard` zeroed doubles, n cells,
@@ -169,6 +170,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
     TAIL_MARK(0);
     extern __shared__ __align__(16) double tail_smem[];
     const int tid = threadIdx.x, nth = blockDim.x;
+    const long long off = (long long)blockIdx.x * g.pstride;   // this CTA's problem (vmg_create_batch), 0 for a single solve
 
     // ---- stage in: zero everything (guards), then copy coefficients of every level, rhs (and phi) of the first ----
     {
@@ -181,7 +183,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         const TailLevel& L = g.lev[l];
         TailSmem s(tail_smem, L);
         for (int t = tid; t < L.n; t += nth) {
-            const long long c = cell_at(L.G, t % L.nx, (t / L.nx) % L.ny, t / L.nxy);
+            const long long c = off + cell_at(L.G, t % L.nx, (t / L.nx) % L.ny, t / L.nxy);
             s.dinv[t] = L.dinv[c]; s.wx[t] = L.wx[c]; s.wy[t] = L.wy[c]; s.wz[t] = L.wz[c];
             if (l == 0) { s.rhs[t] = L.rhs[c]; if (g.whole) s.phi[t] = L.phi[c]; }
         }
@@ -247,7 +249,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         double m = 0.0;
         bool nan = false;
         for (int t = tid; t < L.n; t += nth) {
-            L.phi[cell_at(L.G, t % L.nx, (t / L.nx) % L.ny, t / L.nxy)] = s.phi[t];
+            L.phi[off + cell_at(L.G, t % L.nx, (t / L.nx) % L.ny, t / L.nxy)] = s.phi[t];
             if (g.whole && g.norm_out) {
                 double x = fabs(tail_residual_at(s, L, t));
                 nan |= (x != x);
@@ -256,7 +258,7 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
         }
         if (g.whole && g.norm_out) {
             if (nan) m = __longlong_as_double(0x7ff8000000000000ll);
-            block_max_to_global(m, g.norm_out);
+            block_max_to_global(m, g.norm_out + off);   // (a batched launch: this problem's scalar)
         }
     }
     TAIL_MARK(40);

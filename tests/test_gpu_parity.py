@@ -456,6 +456,65 @@ def test_batched_solves_are_bitwise_the_single_solves():
     s1.destroy(); s2.destroy()
 
 
+@pytest.mark.parametrize("full_mb", [400.0, 0.0], ids=["all_levels_batched", "coarse_levels_batched"])
+def test_kernel_level_batch_matches_oracle_and_single_solves(full_mb):
+    """SURVEY.md 8(f) N1 as written: K problems on one grid INSIDE the kernels -- vmg_create_batch puts the
+    members' arenas a constant stride apart, vmg_solve_batch runs the levels problem-major (blockIdx.z = planes x problems,
+    K CTAs in the tail, one graph; all levels, or -- option batch_full_mb = 0 -- the coarser levels with level 0 one problem
+    at a time).  Four different problems (coefficients, boundary kinds and data, right-hand sides; they need 8-10 cycles, so
+    the last cycles run with some members finished): every phi against the ORACLE's solve, and status, cycle count,
+    history and phi bitwise against vmg_solve on an ordinary handle; a second call and a changed member afterwards."""
+    b = _binding()
+    probs = [inputs.config4(32), inputs.config3(32), inputs.random_problem(64, 32, 32, seed=3, bc_type=[D, N, N, D, N, N]),
+             inputs.random_problem(64, 32, 32, seed=4, bc_type=[D, D, N, N, N, D])]
+
+    def single(p, d):
+        s = b.Vmg(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz)
+        s.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+        s.set_bc(p.bc_type, d["bc_value"])
+        phi = torch.zeros_like(d["rhs"])
+        st = s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=30)
+        out = (st, s.get_info(), phi)
+        s.destroy()
+        return out
+
+    p0 = probs[0]
+    hs = b.create_batch(len(probs), p0.nx, p0.ny, p0.nz, p0.dx, p0.dy, p0.dz)
+    hs[0].set_option("batch_full_mb", full_mb)
+    ds = [b.upload(p) for p in probs]
+    for h, p, d in zip(hs, probs, ds):
+        h.set_coeffs(d["a"], d["bx"], d["by"], d["bz"], p.alpha, p.beta)
+        h.set_bc(p.bc_type, d["bc_value"])
+    refs = [single(p, d) for p, d in zip(probs, ds)]
+    assert len({r[1][0] for r in refs}) > 1          # the members do not all stop at the same cycle
+    for rep in range(2):
+        phis = [torch.zeros_like(d["rhs"]) for d in ds]
+        sts = b.solve_batch(hs, [d["rhs"] for d in ds], phis, rtol=1e-12, max_vcycles=30)
+        for p, h, st, phi, ref in zip(probs, hs, sts, phis, refs):
+            cyc, rr, hist = h.get_info()
+            assert st == ref[0] and cyc == ref[1][0] and list(hist) == list(ref[1][2]) and torch.equal(phi, ref[2]), (rep, p.name)
+            if rep == 0:
+                o = Oracle.from_problem(p)
+                phi_o, st_o, cyc_o, rr_o, hist_o = o.solve(p.rhs, rtol=1e-12, max_vcycles=30)
+                o.close()
+                assert st == st_o and abs(cyc - cyc_o) <= 1 and rel(phi.cpu().numpy(), phi_o) <= PHI_TOL, p.name
+    # one member gets other coefficients (its graph epoch moves: the group's graphs are recaptured); a member used alone
+    p2 = inputs.random_problem(64, 32, 32, seed=8, bc_type=[D, N, N, D, N, N])
+    d2 = b.upload(p2)
+    hs[2].set_coeffs(d2["a"], d2["bx"], d2["by"], d2["bz"], p2.alpha, p2.beta)
+    hs[2].set_bc(p2.bc_type, d2["bc_value"])
+    probs[2], ds[2], refs[2] = p2, d2, single(p2, d2)
+    phis = [torch.zeros_like(d["rhs"]) for d in ds]
+    sts = b.solve_batch(hs, [d["rhs"] for d in ds], phis, rtol=1e-12, max_vcycles=30)
+    for h, st, phi, ref in zip(hs, sts, phis, refs):
+        assert st == ref[0] and h.get_info()[0] == ref[1][0] and torch.equal(phi, ref[2])
+    phi = torch.zeros_like(ds[1]["rhs"])
+    assert hs[1].solve(ds[1]["rhs"], phi, rtol=1e-12, max_vcycles=30) == refs[1][0] and torch.equal(phi, refs[1][2])
+    assert all(h.pad_check() == 0 for h in hs)
+    for h in hs:
+        h.destroy()
+
+
 def _torch_residual_relres(p, d, phi):
     """||btilde - A phi||_inf / ||btilde||_inf written with plain torch slicing from the definition C1 of DESIGN.md
     (face fluxes, two-point Dirichlet flux, Neumann data) -- no libvmg kernel involved.  3-D problems."""
