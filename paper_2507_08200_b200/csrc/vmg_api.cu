@@ -129,6 +129,7 @@ int apply_l2_window(vmg_s* h)
     a.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
     a.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
     CUDA_TRY(h, cudaStreamSetAttribute(h->stream, cudaStreamAttributeAccessPolicyWindow, &a));
+    h->l2_attr = a;
     if (!want) CUDA_TRY(h, cudaCtxResetPersistingL2Cache());
     h->l2_window_set = want != 0;
     { ++h->graph_epoch; }

@@ -101,6 +101,7 @@ struct vmg_s {
     int use_graph = 1, use_blocked = 0;   // blocked passes: measured slower than per-colour launches on B200
     double l2_persist_mb = 24.0;  // L2 set aside for the level-0 face weights (0: none); see apply_l2_window
     bool l2_applied = false, l2_window_set = false;
+    cudaStreamAttrValue l2_attr = {};   // the window as set on the stream (members of a batch group share a stream and re-apply theirs before a capture)
     bool l2_limit_saved = false;  // cudaLimitPersistingL2CacheSize as it was before this handle raised it (restored by vmg_destroy)
     size_t l2_limit_prev = 0;
     int use_pdl = 1;              // programmatic dependent launch of the V-cycle kernels

@@ -708,6 +708,17 @@ inline void enqueue_vcycle_segment(vmg_s* h, int seg, unsigned long long* norm_o
     }
 }
 
+// Members of a vmg_create_batch group share one stream, and the access-policy window that keeps a handle's level-0 face
+// weights in L2 is a stream attribute which captured kernel nodes inherit: before a member captures, it puts ITS window
+// back on the stream (otherwise every member's graph would carry the window of whichever member was prepared last).
+inline void own_l2_window(vmg_s* h)
+{
+    if (h->group && h->l2_window_set) {
+        cudaStreamSetAttribute(h->stream, cudaStreamAttributeAccessPolicyWindow, &h->l2_attr);
+        (void)cudaGetLastError();
+    }
+}
+
 // captures the three segments (once per epoch and kind of weights), then launches segment `seg` into `into`
 // (the handle's stream, or its high-priority stream for segment 1: a graph runs at the priority of the stream it is
 // launched into)
@@ -716,6 +727,7 @@ inline int run_vcycle_segment(vmg_s* h, int seg, unsigned long long* out, cudaSt
     const int gi = h->lev[0].cw;
     if (h->seg_epoch[gi] != h->graph_epoch) {
         prepare_blocked(h);
+        own_l2_window(h);
         for (int sg = 0; sg < 3; ++sg) {
             if (h->seg_exec[gi][sg]) { cudaGraphExecDestroy(h->seg_exec[gi][sg]); h->seg_exec[gi][sg] = nullptr; }
             if (h->seg_graph[gi][sg]) { cudaGraphDestroy(h->seg_graph[gi][sg]); h->seg_graph[gi][sg] = nullptr; }
@@ -807,6 +819,7 @@ inline int run_solve_loop(vmg_s* h, unsigned long long* norm_out)
     const int gi = h->lev[0].cw;
     auto fail = [&](cudaError_t e) { h->last_cuda_error = (int)e; (void)cudaGetLastError(); return VMG_ERR_CUDA; };
     if (h->loop_epoch[gi] != h->graph_epoch) {
+        own_l2_window(h);
         if (h->loop_exec[gi]) { cudaGraphExecDestroy(h->loop_exec[gi]); h->loop_exec[gi] = nullptr; }
         if (h->loop_graph[gi]) { cudaGraphDestroy(h->loop_graph[gi]); h->loop_graph[gi] = nullptr; }
         cudaGraph_t g = nullptr, dummy = nullptr;
@@ -964,6 +977,7 @@ inline int run_vcycle_with_norm(vmg_s* h, unsigned long long* out)
     }
     const int gi = h->lev[0].cw;
     if (h->graph_slot_epoch[gi] != h->graph_epoch) {
+        own_l2_window(h);
         if (h->graph_exec[gi]) { cudaGraphExecDestroy(h->graph_exec[gi]); h->graph_exec[gi] = nullptr; }
         if (h->graph[gi]) { cudaGraphDestroy(h->graph[gi]); h->graph[gi] = nullptr; }
         long long count = 0;
