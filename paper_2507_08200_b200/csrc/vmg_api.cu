@@ -557,21 +557,19 @@ int solve_begin(vmg_s* h, const double* rhs, double* phi, double rtol, int max_v
     unsigned long long* scal = (unsigned long long*)h->d_scal;
     h->hist.clear(); h->cycles = 0; h->relres = 0.0; h->launches = 0;
     h->sv_rtol = rtol; h->sv_max = max_vcycles; h->sv_phi = phi; h->sv_slow = 0; h->sv_status = VMG_MAXCYCLES; h->sv_active = false;
-    int rc = enqueue_fold_bc(h, rhs, L0.rhs);
+    // ||btilde|| is taken by fold_bc itself and max |phi_0| by the layout conversion: for a zero initial guess (every
+    // cold start) the initial residual IS btilde, bit for bit (rhs + sum(w * 0) - 0 / (1/D)), and the 56 us all-cell
+    // residual norm is not launched at all; otherwise solve_begin_finish launches it after this read-back.
+    CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
+    int rc = enqueue_fold_bc(h, rhs, L0.rhs, false, scal + 0);
     if (rc != VMG_OK) return rc;
     {
         ProfScope ps(h, VMG_PC_COPY, nullptr);
-        to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, L0.phi, h->d_mask);
+        to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, L0.phi, h->d_mask, scal + 2);
     }
-    CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
-    {
-        ProfScope ps(h, VMG_PC_NORM, nullptr);
-        norm_inf_kernel<<<std::min<unsigned>(grid_for(L0.nalloc), 8u * h->num_sms), kThreads, 0, h->stream>>>(L0.rhs, L0.nalloc, scal + 0);
-    }
-    enqueue_residual_norm(h, scal + 1);
-    h->launches += 3;   // phi copy-in, ||btilde||, first residual norm
+    h->launches += 1;   // phi copy-in
     CUDA_TRY(h, cudaGetLastError());
-    CUDA_TRY(h, cudaMemcpyAsync(h->h_scal, scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(h->h_scal, scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     return VMG_OK;
 }
 
@@ -586,6 +584,15 @@ int solve_begin_finish(vmg_s* h)
         h->sv_status = VMG_OK;
         h->sv_phi = nullptr;   // nothing to copy out
         return VMG_OK;
+    }
+    if (h->h_scal[2] == 0.0) h->h_scal[1] = h->h_scal[0];   // zero initial guess: the residual is btilde
+    else {
+        unsigned long long* scal = (unsigned long long*)h->d_scal;
+        enqueue_residual_norm(h, scal + 1);
+        h->launches += 1;
+        CUDA_TRY(h, cudaGetLastError());
+        CUDA_TRY(h, cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     }
     h->relres = h->h_scal[1] / h->sv_nb;
     h->hist.push_back(h->relres);

@@ -213,17 +213,18 @@ __global__ void finalize_dinv_kernel(DinvArgs g)
 // (w_b = beta*b/h^2 of the boundary face; R3, R5).  Level 0, once per solve.  rhs: public layout; bt: internal
 // layout, or public layout when bt_natural (the single-step entry point).
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void block_max_to_global(double v, unsigned long long* out);
+
 struct FoldArgs {
+    unsigned long long* norm_out;                      // ||btilde||_inf accumulated here as well (S6; NULL: not wanted)
     const double* rhs; double* bt; const double* wb[6]; const double* val[6];
     const unsigned char* mask; const double* mfold;   // masking (NULL without a mask): interface terms, covered cells -> 0
     Geom G;
     int three_d, bt_natural; int dirichlet[6]; double h[3];
 };
 
-__global__ void fold_bc_kernel(FoldArgs g)
+__device__ __forceinline__ double fold_bc_one(const FoldArgs& g, long long t)
 {
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (t >= g.G.n) return;
     const int nx = g.G.nx, ny = g.G.ny, nz = g.G.nz;
     int i, j, k;
     unflatten(g.G, t, i, j, k);
@@ -243,6 +244,19 @@ __global__ void fold_bc_kernel(FoldArgs g)
     }
     if (g.mask) v = g.mask[t] ? v + g.mfold[t] : 0.0;
     g.bt[g.bt_natural ? t : cell_at(g.G, i, j, k)] = v;
+    return v;
+}
+
+__global__ void fold_bc_kernel(FoldArgs g)
+{
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    double v = 0.0;
+    if (t < g.G.n) v = fold_bc_one(g, t);
+    if (g.norm_out) {                                  // the same maximum norm_inf_kernel takes over the stored array
+        v = fabs(v);
+        if (v != v) v = __longlong_as_double(0x7ff8000000000000ll);
+        block_max_to_global(v, g.norm_out);
+    }
 }
 
 // the open faces of every cell as one byte in the internal layout (LevelView::mk): bit f (0..5 = low x, high x, low y,
@@ -298,13 +312,23 @@ __global__ void pad_check_kernel(Geom G, const double* __restrict__ arr, long lo
 
 // public (natural) layout <-> internal layout of one cell array
 // mask (may be NULL): covered cells enter as zero (they are identity rows of the masked operator)
-__global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in, const unsigned char* __restrict__ mask)
+// max_out (may be NULL): max |value| stored, so that the solve can tell a zero initial guess (whose residual is btilde itself)
+__global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in, const unsigned char* __restrict__ mask,
+                                   unsigned long long* max_out = nullptr)
 {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (t >= G.n) return;
-    int i, j, k;
-    unflatten(G, t, i, j, k);
-    in[cell_at(G, i, j, k)] = (mask && !mask[t]) ? 0.0 : nat[t];
+    double v = 0.0;
+    if (t < G.n) {
+        int i, j, k;
+        unflatten(G, t, i, j, k);
+        v = (mask && !mask[t]) ? 0.0 : nat[t];
+        in[cell_at(G, i, j, k)] = v;
+    }
+    if (max_out) {
+        v = fabs(v);
+        if (v != v) v = __longlong_as_double(0x7ff8000000000000ll);
+        block_max_to_global(v, max_out);
+    }
 }
 __global__ void to_natural_kernel(Geom G, const double* __restrict__ in, double* __restrict__ nat)
 {

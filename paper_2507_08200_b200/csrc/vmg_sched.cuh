@@ -110,10 +110,11 @@ inline void prof_collect(vmg_s* h)
 }
 
 // bt: the level-0 internal array, or (bt_natural) a caller array in the public layout
-inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt, bool bt_natural = false)
+inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt, bool bt_natural = false, unsigned long long* norm_out = nullptr)
 {
     VmgLevel& L = h->lev[0];
     FoldArgs g;
+    g.norm_out = norm_out;
     g.rhs = rhs; g.bt = bt;
     for (int f = 0; f < 6; ++f) {
         g.wb[f] = L.wb[f];
