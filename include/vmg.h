@@ -150,6 +150,10 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  *   which makes one V-cycle from zero a symmetric operator; default 0; vmg_solve_pcg switches it on for itself), "prolong" (0: piecewise-constant prolongation, default; 1: cell-centred trilinear,
  *   weights 3/4 and 1/4 per direction, ghost value -e at Dirichlet and +e at Neumann faces), "graph" (1: replay the V-cycle as a CUDA graph, default; 0: plain launches),
  * "tail" (1: the coarsest levels run in one single-CTA launch, default; 0: one kernel per step),
+ * "cluster" (1, default: the level above the single-CTA tail runs distributed over a thread-block cluster of up to 8 CTAs,
+ *   resident in their shared memory for its whole down- and up-stroke, halo planes exchanged through distributed shared
+ *   memory, barrier.cluster between half-sweeps -- 13 fewer launches per V-cycle, bitwise the same results; needs 3-D,
+ *   piecewise-constant prolongation and a level whose slabs fit (vmg_cluster.cuh); 0: one launch per step on that level),
  * "device_loop" (1, default: all V-cycles of a vmg_solve are ONE graph launch -- a conditional WHILE node whose condition
  *   a one-thread kernel sets from the exit rules -- and the residual norm of cycle c is taken by the first half-sweep of
  *   cycle c+1, which writes beside phi so that a converged iterate is returned untouched; bitwise the status, cycle count,

@@ -505,6 +505,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "blocked")) { if (iv < 0 || iv > 3) return VMG_ERR_ARG; h->use_blocked = iv; }   // 1: vmg_block2.cuh, 2 / 3: vmg_block3.cuh (TMA; 2 x 2 patches / rows)
     else if (!strcmp(key, "tail")) { h->use_tail = iv != 0; }
     else if (!strcmp(key, "device_loop")) { h->use_loop = iv != 0; }
+    else if (!strcmp(key, "cluster")) { h->use_cluster = iv != 0; }
     else if (!strcmp(key, "snake")) { h->snake = iv != 0; }
     else if (!strcmp(key, "pdl")) { h->use_pdl = iv != 0; }
     else if (!strcmp(key, "batch_full_mb")) { if (v < 0) return VMG_ERR_ARG; h->batch_full_mb = v; }

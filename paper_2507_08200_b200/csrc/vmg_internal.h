@@ -110,6 +110,9 @@ struct vmg_s {
     int use_tail = 1;             // run the coarsest levels in one CTA (vmg_tail.cuh)
     int tail_level = -1;          // first level handled by the single-CTA coarse tail (-1: none)
     size_t tail_smem = 0;         // dynamic shared memory of the tail kernel
+    int use_cluster = 1;          // option "cluster": the level above the tail distributed over a thread-block cluster (vmg_cluster.cuh)
+    int cl_nc = 0, cl_P = 0;      // cluster size (0: not used) and planes per CTA; tail_level is then the distributed level
+    size_t cl_smem = 0;
     long long block_min_cells = 4096;   // smallest level the blocked smoother is used on
     double batch_full_mb = 400.0;  // option "batch_full_mb" (member 0 of a vmg_create_batch group): all levels batched while K fine levels (56 B/cell) stay below this
     // device scalars

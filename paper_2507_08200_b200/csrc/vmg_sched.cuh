@@ -8,6 +8,7 @@
 #include "vmg_internal.h"
 #include "vmg_kernels.cuh"
 #include "vmg_tail.cuh"
+#include "vmg_cluster.cuh"
 #include "vmg_block2.cuh"
 #include "vmg_block3.cuh"
 #include "../../include/vmg.h"
@@ -230,13 +231,49 @@ inline void plan_schedule(vmg_s* h)
     h->tail_smem = doubles * sizeof(double);
     cudaFuncSetAttribute(coarse_tail_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmemCap);
     cudaFuncSetAttribute(coarse_tail_kernel<kTailThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmemCap);
+    // the level above the tail distributed over a thread-block cluster (vmg_cluster.cuh): z-slabs of P planes (P even), at
+    // most 8 CTAs (the portable cluster size), one x-pair slot per thread, the slab's block beside the tail's in every CTA
+    h->cl_nc = 0;
+    const int d = first - 1;
+    if (h->use_cluster && d >= 1 && h->three_d && !h->prolong) {
+        const VmgLevel& D = h->lev[d];
+        for (int nc = 8; nc >= 2; nc /= 2) {
+            if (D.nz % (2 * nc)) continue;
+            const int P = D.nz / nc;
+            const long long nt = (long long)((D.nx + 1) / 2) * D.ny * P;
+            const size_t bytes = (doubles + (size_t)tail_level_doubles(D.nx * D.ny * P, tail_guard(h, D))) * sizeof(double);
+            if (nt > kTailThreads || bytes > kTailSmemCap) continue;
+            h->cl_nc = nc; h->cl_P = P; h->cl_smem = bytes;
+            h->tail_level = d;                       // the strokes hand levels >= d to enqueue_tail
+            cudaFuncSetAttribute(coarse_cluster_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmemCap);
+            cudaFuncSetAttribute(coarse_cluster_kernel<kTailThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmemCap);
+            break;
+        }
+    }
     (void)cudaGetLastError();
+}
+
+// launch with a thread-block cluster of nc CTAs (and programmatic stream serialisation like launch_pdl)
+template <typename... KArgs, typename... Args>
+inline void launch_cluster(vmg_s* h, void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, unsigned nc, Args... args)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = h->stream;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = h->use_pdl ? 1 : 0;
+    at[1].id = cudaLaunchAttributeClusterDimension;
+    at[1].val.clusterDim.x = nc; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 2;
+    cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
 inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* count)
 {
     TailArgs g;
-    const int tail = h->tail_level, first = tail;
+    const bool clustered = h->cl_nc > 0;
+    const int tail = h->tail_level + (clustered ? 1 : 0), first = tail;   // clustered: tail_level is the distributed level
     int off = 0;
     g.nl = h->nlev - first;
     for (int l = first; l < h->nlev; ++l) {
@@ -257,6 +294,23 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
     g.pstride = h->lev[first].pstride;
     const int ncta = h->lev[first].nprob;
     ProfScope ps(h, VMG_PC_COARSE, count);
+    if (clustered) {
+        ClusterArgs c;
+        c.tail = g;
+        VmgLevel& L = h->lev[first - 1];
+        TailLevel& T = c.D;
+        L.cur = 0;
+        T.wx = L.wx; T.wy = L.wy; T.wz = L.wz; T.dinv = L.dinv; T.phi = L.phi; T.rhs = L.rhs;
+        T.nx = L.nx; T.ny = L.ny; T.nz = L.nz; T.n = (int)L.n; T.nxy = L.nx * L.ny; T.G = L.G;
+        T.zs = T.nxy;
+        T.guard = tail_guard(h, L);
+        T.off = off;                                  // behind the tail's levels
+        c.P = h->cl_P;
+        const long long nt = (long long)((L.nx + 1) / 2) * L.ny * h->cl_P;
+        int threads = (int)std::max<long long>((nt + 31) / 32 * 32, std::min<long long>(kTailThreads, std::max<long long>(64, (h->lev[first].n / 2 + 31) / 32 * 32)));
+        if (threads <= 512) launch_cluster(h, coarse_cluster_kernel<512>, (unsigned)(ncta * h->cl_nc), (unsigned)threads, h->cl_smem, (unsigned)h->cl_nc, c);
+        else launch_cluster(h, coarse_cluster_kernel<kTailThreads>, (unsigned)(ncta * h->cl_nc), (unsigned)threads, h->cl_smem, (unsigned)h->cl_nc, c);
+    } else
     {
         int threads = (int)std::min<long long>(kTailThreads, std::max<long long>(64, (h->lev[first].n / 2 + 31) / 32 * 32));
         if (threads <= 512) launch_pdl(h, coarse_tail_kernel<512>, ncta, threads, h->tail_smem, g);

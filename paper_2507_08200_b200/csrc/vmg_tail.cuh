@@ -165,12 +165,12 @@ __device__ long long vmg_tail_clock[64];
 #define TAIL_MARK(i) do { } while (0)
 #endif
 
-__device__ __forceinline__ void coarse_tail_body(const TailArgs& g)
+// off: offset of this CTA's problem in a batched launch (vmg_create_batch), 0 for a single solve
+__device__ __forceinline__ void coarse_tail_body(const TailArgs& g, const long long off)
 {
     TAIL_MARK(0);
     extern __shared__ __align__(16) double tail_smem[];
     const int tid = threadIdx.x, nth = blockDim.x;
-    const long long off = (long long)blockIdx.x * g.pstride;   // this CTA's problem (vmg_create_batch), 0 for a single solve
 
     // ---- stage in: zero everything (guards), then copy coefficients of every level, rhs (and phi) of the first ----
     {
@@ -270,7 +270,7 @@ template <int NT>
 __global__ void __launch_bounds__(NT, 1) coarse_tail_kernel(TailArgs g)
 {
     grid_dependency_wait();
-    coarse_tail_body(g);
+    coarse_tail_body(g, (long long)blockIdx.x * g.pstride);
 }
 
 }  // namespace vmg

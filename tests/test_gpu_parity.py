@@ -98,7 +98,7 @@ def test_schedule_options_do_not_change_a_single_bit():
     p = inputs.config4(32)
     ref = None
     for opts in (dict(snake=0, l2_persist=0, graph=0, tail=0), dict(), dict(snake=1, graph=0), dict(tail=0), dict(blocked=1),
-                 dict(blocked=2), dict(blocked=3, block_min_cells=0), dict(device_loop=0), dict(device_loop=0, graph=0),
+                 dict(blocked=2), dict(blocked=3, block_min_cells=0), dict(device_loop=0), dict(device_loop=0, graph=0), dict(cluster=0), dict(cluster=0, device_loop=0),
                  dict(phi_keep_cells=0), dict(phi_keep_cells=0, graph=0, tail=0)):   # cache policy of the largest levels on all levels
         s, d = b.from_problem(p)
         for k, v in opts.items():
