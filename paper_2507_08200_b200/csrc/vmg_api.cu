@@ -560,7 +560,7 @@ int solve_begin(vmg_s* h, const double* rhs, double* phi, double rtol, int max_v
     h->sv_rtol = rtol; h->sv_max = max_vcycles; h->sv_phi = phi; h->sv_slow = 0; h->sv_status = VMG_MAXCYCLES; h->sv_active = false;
     // ||btilde|| is taken by fold_bc itself and max |phi_0| by the layout conversion: for a zero initial guess (every
     // cold start) the initial residual IS btilde, bit for bit (rhs + sum(w * 0) - 0 / (1/D)), and the 56 us all-cell
-    // residual norm is not launched at all; otherwise solve_begin_finish launches it after this read-back.
+    // residual norm returns at once (it reads that maximum on the device: no host round trip for warm starts either).
     CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
     int rc = enqueue_fold_bc(h, rhs, L0.rhs, false, scal + 0);
     if (rc != VMG_OK) return rc;
@@ -568,7 +568,8 @@ int solve_begin(vmg_s* h, const double* rhs, double* phi, double rtol, int max_v
         ProfScope ps(h, VMG_PC_COPY, nullptr);
         to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, L0.phi, h->d_mask, scal + 2);
     }
-    h->launches += 1;   // phi copy-in
+    enqueue_residual_norm(h, scal + 1, false, scal + 2);
+    h->launches += 2;   // phi copy-in, first residual norm
     CUDA_TRY(h, cudaGetLastError());
     CUDA_TRY(h, cudaMemcpyAsync(h->h_scal, scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     return VMG_OK;
@@ -586,15 +587,7 @@ int solve_begin_finish(vmg_s* h)
         h->sv_phi = nullptr;   // nothing to copy out
         return VMG_OK;
     }
-    if (h->h_scal[2] == 0.0) h->h_scal[1] = h->h_scal[0];   // zero initial guess: the residual is btilde
-    else {
-        unsigned long long* scal = (unsigned long long*)h->d_scal;
-        enqueue_residual_norm(h, scal + 1);
-        h->launches += 1;
-        CUDA_TRY(h, cudaGetLastError());
-        CUDA_TRY(h, cudaMemcpyAsync(h->h_scal + 1, scal + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    }
+    if (h->h_scal[2] == 0.0) h->h_scal[1] = h->h_scal[0];   // zero initial guess: the residual is btilde (the norm kernel skipped itself)
     h->relres = h->h_scal[1] / h->sv_nb;
     h->hist.push_back(h->relres);
     if (std::isnan(h->relres) || std::isinf(h->relres)) { h->sv_status = VMG_ERR_DIVERGED; h->sv_phi = nullptr; return VMG_OK; }

@@ -838,10 +838,13 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
 // ||rhs - A phi||_inf accumulated into *out with atomicMax (the caller zeroes it); one cell per thread, both colours or red only
 // (as (like two colour half-sweeps in one launch: 13 loads and a division per thread at full occupancy)
 template <int CW, int KEEP = 0>   // KEEP = 1: phi with the normal policy (levels far larger than the L2, see relax_at)
+// skip_if_zero (may be NULL): a device scalar; when its bits are 0 the kernel does nothing (vmg_solve's initial residual:
+// max |phi_0| == 0 means the residual is btilde, which the host then takes from ||btilde||)
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                     unsigned long long* out, int reverse)
+                                     unsigned long long* out, int reverse, const unsigned long long* skip_if_zero = nullptr)
 {
     grid_dependency_wait();
+    if (skip_if_zero && *skip_if_zero == 0ull) return;   // uniform over the grid
     const Geom& G = L.G;
     // grid (x-pair blocks, row blocks, planes * colours), block (x-pairs, rows): pair_launch_dims, z extended by the colour
     int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;

@@ -191,7 +191,7 @@ inline void plain_prolong_correct(vmg_s* h, int l, long long* count)
 // red_only: the level was last touched by a black half-sweep, after which the residual of every black cell is its own
 // rounding error (rhs + s - fl(fl(dinv*(rhs + s))/dinv), ~2 ulp of D*phi, 1e-16 relative to ||btilde||): the norm is
 // the maximum over the red cells, half the traffic (reading R12 in DESIGN.md).
-inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_only = false)
+inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_only = false, const unsigned long long* skip_if_zero = nullptr)
 {
     VmgLevel& L = h->lev[0];
     dim3 grid, block;
@@ -199,9 +199,9 @@ inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_on
     if (!red_only) grid.z *= 2;                               // one cell per thread: the planes once per colour
     ProfScope ps(h, VMG_PC_NORM, nullptr);
     if (L.cw == 0 && L.n >= h->phi_keep_cells)
-        launch_pdl(h, residual_norm_kernel<0, 1>, grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
+        launch_pdl(h, residual_norm_kernel<0, 1>, grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L), skip_if_zero);
     else
-        launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L));
+        launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L), skip_if_zero);
 }
 
 // ------------------------------------------------------------------------------------------------
