@@ -841,35 +841,41 @@ template <int CW, int KEEP = 0>   // KEEP = 1: phi with the normal policy (level
 // skip_if_zero (may be NULL): a device scalar; when its bits are 0 the kernel does nothing (vmg_solve's initial residual:
 // max |phi_0| == 0 means the residual is btilde, which the host then takes from ||btilde||)
 __global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                     unsigned long long* out, int reverse, const unsigned long long* skip_if_zero = nullptr)
+                                     unsigned long long* out, int reverse, const unsigned long long* skip_if_zero = nullptr,
+                                     int zslots = 0)
 {
     grid_dependency_wait();
     if (skip_if_zero && *skip_if_zero == 0ull) return;   // uniform over the grid
     const Geom& G = L.G;
-    // grid (x-pair blocks, row blocks, planes * colours), block (x-pairs, rows): pair_launch_dims, z extended by the colour
-    int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
-    int z = (int)blockIdx.z;
-    long long off = 0;
-    if (L.pstride) {                                  // batched: blockIdx.z = (problem, colour, plane), problem-major
-        const int span = (int)gridDim.z / L.nprob, kb = z / span;
-        z -= kb * span;
-        off = (long long)kb * L.pstride;
-        out += off;                                   // the members' scalars lie the same stride apart (8-byte units)
-    }
-    int k = z % G.nz;
-    const int colour = z / G.nz;
-    if (reverse) { k = G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
+    // grid (x-pair blocks, row blocks, planes * colours), block (x-pairs, rows): pair_launch_dims, z extended by the colour.
+    // zslots > gridDim.z: the z slots are taken gridDim.z apart (the self-skipping launch keeps its grid small: an
+    // empty grid of 32768 CTAs still costs 20 us); batched levels are launched with one slot per blockIdx.z
+    const int m = blockIdx.x * blockDim.x + threadIdx.x, j0 = blockIdx.y * blockDim.y + threadIdx.y;
+    if (zslots <= 0) zslots = (int)gridDim.z;
     double mx = 0.0;
-    if (m < G.ne && j < G.ny) {
-        int par = (colour + j + k) & 1;
-        if (2 * m + par < G.nx) {
-            long long c, xm;
-            pair_addr(G, off + G.plane * k + (long long)G.pitch * j, m, par, c, xm);
-            mx = fabs(residual_at<CW, CW ? 0 : KEEP ? 2 : 1>(L, phi, rhs, c, xm, 2 * m + par, j, k));   // constant weights: the level fits L2, keep it there
-            if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
+    long long off = 0;
+    for (int z = (int)blockIdx.z; z < zslots; z += (int)gridDim.z) {
+        int zz = z, j = j0;
+        if (L.pstride) {                              // batched: z = (problem, colour, plane), problem-major
+            const int span = zslots / L.nprob, kb = zz / span;
+            zz -= kb * span;
+            off = (long long)kb * L.pstride;
+        }
+        int k = zz % G.nz;
+        const int colour = zz / G.nz;
+        if (reverse) { k = G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
+        if (m < G.ne && j < G.ny) {
+            int par = (colour + j + k) & 1;
+            if (2 * m + par < G.nx) {
+                long long c, xm;
+                pair_addr(G, off + G.plane * k + (long long)G.pitch * j, m, par, c, xm);
+                double r = fabs(residual_at<CW, CW ? 0 : KEEP ? 2 : 1>(L, phi, rhs, c, xm, 2 * m + par, j, k));   // constant weights: the level fits L2, keep it there
+                if (r != r) r = __longlong_as_double(0x7ff8000000000000ll);
+                mx = (r > mx || r != r) ? r : mx;
+            }
         }
     }
-    block_max_to_global(mx, out);
+    block_max_to_global(mx, out + off);               // the members' scalars lie the same stride apart (8-byte units)
 }
 
 }  // namespace vmg

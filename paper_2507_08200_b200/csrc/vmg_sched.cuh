@@ -197,11 +197,13 @@ inline void enqueue_residual_norm(vmg_s* h, unsigned long long* out, bool red_on
     dim3 grid, block;
     pair_launch_dims(L, grid, block);
     if (!red_only) grid.z *= 2;                               // one cell per thread: the planes once per colour
+    const int zslots = (int)grid.z;
+    if (skip_if_zero && L.nprob <= 1) grid.z = std::min(grid.z, 32u);   // vmg_solve's initial norm, which mostly skips itself
     ProfScope ps(h, VMG_PC_NORM, nullptr);
     if (L.cw == 0 && L.n >= h->phi_keep_cells)
-        launch_pdl(h, residual_norm_kernel<0, 1>, grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L), skip_if_zero);
+        launch_pdl(h, residual_norm_kernel<0, 1>, grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L), skip_if_zero, zslots);
     else
-        launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L), skip_if_zero);
+        launch_pdl(h, VMG_BY_WEIGHTS(L, residual_norm_kernel), grid, block, 0, view(L), cur_phi(L), L.rhs, out, next_dir(h, L), skip_if_zero, zslots);
 }
 
 // ------------------------------------------------------------------------------------------------
