@@ -233,6 +233,30 @@ long long vmg_total_launch_count(vmg_handle h);
  * levels (incl. bottom), 4 norms, 5 fold_bc, 6 phi copies in/out, 7 vmg_set_coeffs kernels. */
 int vmg_get_profile(vmg_handle h, double ms[8], long long launches[8]);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * vmg_norm_inf_static -- the one entry point that ALLOCATES NOTHING (for callers that cannot call cudaMalloc: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it).  Operation: *out = ||v||_inf = max |v[t]|,
+ * t < n, the norm of the exit rules (S6 of SURVEY.md 8(a); relres of 8(c) C5 / R12, BASELINE.json north_star (3)
+ * "warp-shuffle and block reductions for the norms"), taken on the bit patterns as vmg_step_norm_inf does: the result
+ * is exact and order-independent, a NaN anywhere in v gives a NaN, n == 0 gives 0.
+ *   v            DEVICE array of n doubles (8-byte aligned), read only; may be NULL when n == 0
+ *   out          DEVICE scalar (8-byte aligned), written by the kernel; valid once the stream has reached this call
+ *   cuda_stream  a cudaStream_t of the CURRENT device (NULL = the legacy default stream); the call enqueues one 8-byte
+ *                memset and one kernel there and returns without synchronising
+ *   why          may be NULL; else receives a static string saying what was wrong ("ok" on success)
+ * No handle, no cudaMalloc / cudaFree, no allocating library routine: the kernel's scratch (one partial maximum per
+ * 4096 elements and a ticket counter) is a file-scope __device__ array of 262 400 bytes that every GPU which loads
+ * libvmg.so holds until the process exits; the first call on a device looks up its address (cudaGetSymbolAddress), so
+ * make one call (n = 0 will do) before a stream capture.  Limit: n <= VMG_NORM_INF_STATIC_MAX_N (= 512^3, the largest
+ * configuration); beyond it VMG_ERR_SIZE and nothing is enqueued.
+ * EVERY call on a device shares that array and it keeps the last call's contents (the call clears what has to start
+ * at zero itself): calls that may overlap on the GPU -- different streams, graph branches, host threads -- RACE and
+ * return garbage; order them on one stream or with events.  Ownership: caller owns v and out.
+ * Errors: VMG_ERR_ARG (out NULL, n < 0, v NULL with n > 0), VMG_ERR_SIZE (n beyond the limit), VMG_ERR_CUDA (symbol
+ * look-up, memset or launch refused; the sticky CUDA error is cleared). */
+#define VMG_NORM_INF_STATIC_MAX_N 134217728LL
+int vmg_norm_inf_static(const double* v, long long n, double* out, void* cuda_stream, const char** why);
+
 #ifdef __cplusplus
 }
 #endif

@@ -21,7 +21,8 @@ SYMBOLS = ["vmg_create", "vmg_create_batch", "vmg_set_coeffs", "vmg_set_bc", "vm
            "vmg_destroy", "vmg_strerror", "vmg_last_cuda_error", "vmg_num_levels", "vmg_level_dims",
            "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
            "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_down", "vmg_step_up", "vmg_step_vcycle", "vmg_step_norm_inf",
-           "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile", "vmg_debug_pad_check"]
+           "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile", "vmg_debug_pad_check",
+           "vmg_norm_inf_static"]
 
 _lib = None
 _vp = C.c_void_p
@@ -69,6 +70,7 @@ def load():
     lib.vmg_total_launch_count.restype = C.c_longlong
     lib.vmg_get_profile.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     lib.vmg_debug_pad_check.argtypes = [_vp, C.POINTER(C.c_longlong)]
+    lib.vmg_norm_inf_static.argtypes = [_vp, C.c_longlong, _vp, _vp, C.POINTER(C.c_char_p)]
     _lib = lib
     return lib
 
@@ -289,6 +291,26 @@ class Vmg:
         out = C.c_double()
         self._chk(self._lib.vmg_step_norm_inf(self._h, _ptr(v), v.numel(), C.byref(out)), "vmg_step_norm_inf")
         return out.value
+
+
+NORM_INF_STATIC_MAX_N = 134217728   # VMG_NORM_INF_STATIC_MAX_N of include/vmg.h
+
+
+def norm_inf_static(v, out, stream=None):
+    """vmg_norm_inf_static: out[0] = max |v| with no allocation inside the library (static device scratch; calls that
+    overlap on the GPU race).  v: fp64 CUDA tensor, out: fp64 CUDA tensor of one element, both caller-owned; asynchronous
+    on `stream` (default: torch's current stream).  Returns out."""
+    torch = _torch()
+    lib = load()
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 1
+    stream = stream if stream is not None else torch.cuda.current_stream()
+    why = C.c_char_p()
+    n = v.numel()
+    rc = lib.vmg_norm_inf_static(_ptr(v) if n else None, n, out.data_ptr(), _vp(stream.cuda_stream) if stream.cuda_stream else None,
+                                 C.byref(why))
+    if rc != 0:
+        raise RuntimeError(f"vmg_norm_inf_static: {STATUS.get(rc, rc)} ({(why.value or b'').decode()})")
+    return out
 
 
 def upload(p, device=None):
