@@ -17,6 +17,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "vmg_oracle.c")
+_SRC_AMR = os.path.join(_HERE, "amr_oracle.c")     # the two-level composite solve (N4, second half), same library
 # VMG_ORACLE_LIB: another build of the same source (e.g. with -fsanitize=address,undefined, profiles/r2_sanitizers.md)
 _LIB = os.environ.get("VMG_ORACLE_LIB") or os.path.join(_HERE, "libvmg_oracle.so")
 
@@ -28,9 +29,9 @@ def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain flags, no contraction, OpenMP over k-planes)."""
     if os.environ.get("VMG_ORACLE_LIB"):
         return _LIB
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_AMR)):
         cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall",
-               "-o", _LIB, _SRC, "-lm"]
+               "-o", _LIB, _SRC, _SRC_AMR, "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
     return _LIB
 
@@ -64,6 +65,17 @@ def lib():
         _lib.ovmg_restrict.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
         _lib.ovmg_prolong_add.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
         _lib.ovmg_vcycle.argtypes = [C.c_void_p, _dp, _dp]
+        _ip = C.POINTER(C.c_int)
+        _lib.oamr_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, _ip]
+        _lib.oamr_destroy.argtypes = [C.c_void_p]
+        _lib.oamr_set_coeffs.argtypes = [C.c_void_p] + [_dp] * 8 + [C.c_double, C.c_double]
+        _lib.oamr_set_bc.argtypes = [C.c_void_p, _ip, C.POINTER(_dp)]
+        _lib.oamr_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_double]
+        _lib.oamr_fine_dims.argtypes = [C.c_void_p, _ip]
+        _lib.oamr_apply.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
+        _lib.oamr_average_down.argtypes = [C.c_void_p, _dp, _dp]
+        _lib.oamr_solve.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, C.c_double, C.c_int]
+        _lib.oamr_get_info.argtypes = [C.c_void_p, _ip, C.POINTER(C.c_double), _dp]
     return _lib
 
 
@@ -220,3 +232,69 @@ class Oracle:
         bt = _c(btilde)
         self._chk(lib().ovmg_vcycle(self._h, _p(phi), _p(bt)), "vcycle")
         return phi
+
+
+class AmrOracle:
+    """Two-level composite solve (amr_oracle.c): an nx x ny x nz coarse box with one patch of coarse cells [lo, hi)
+    refined by 2.  Coarse arrays [k, j, i] on the box, fine arrays [K, J, I] on the patch (2 (hi - lo) cells a side)."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, lo, hi):
+        self._h = C.c_void_p()
+        l3, h3 = (C.c_int * 3)(*[int(v) for v in lo]), (C.c_int * 3)(*[int(v) for v in hi])
+        rc = lib().oamr_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, l3, h3)
+        if rc != 0:
+            self._h = None
+            raise OracleError(rc, "amr create")
+        d = (C.c_int * 3)()
+        lib().oamr_fine_dims(self._h, d)
+        self.coarse_shape, self.fine_shape = (nz, ny, nx), (d[2], d[1], d[0])
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().oamr_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _chk(self, rc, where):
+        if rc < 0:
+            raise OracleError(rc, where)
+        return rc
+
+    def set_coeffs(self, coarse, fine, alpha: float, beta: float):
+        """coarse, fine: (a, bx, by, bz) tuples (entries may be None: a = 0, b = 1)."""
+        arrs = [_c(x) for x in list(coarse) + list(fine)]
+        self._chk(lib().oamr_set_coeffs(self._h, *[_p(x) for x in arrs], alpha, beta), "amr set_coeffs")
+
+    def set_bc(self, types, values=None):
+        t = (C.c_int * 6)(*[int(v) for v in types])
+        keep = [_c(v) for v in (values or [None] * 6)]
+        arr = (_dp * 6)(*[_p(v) for v in keep])
+        self._chk(lib().oamr_set_bc(self._h, t, arr), "amr set_bc")
+
+    def set_option(self, key: str, v: float):
+        self._chk(lib().oamr_set_option(self._h, key.encode(), float(v)), "amr set_option")
+
+    def apply(self, phic, phif):
+        phic, phif = _c(phic), _c(phif)
+        oc, of = np.zeros_like(phic), np.zeros_like(phif)
+        self._chk(lib().oamr_apply(self._h, _p(phic), _p(phif), _p(oc), _p(of)), "amr apply")
+        return oc, of
+
+    def average_down(self, phic, phif):
+        phic = np.array(phic, dtype=np.float64, order="C")
+        self._chk(lib().oamr_average_down(self._h, _p(phic), _p(_c(phif))), "amr average_down")
+        return phic
+
+    def solve(self, rhsc, rhsf, phic0=None, phif0=None, rtol: float = 1e-12, max_cycles: int = 50):
+        """Returns (phic, phif, status, cycles, relres, history)."""
+        rhsc, rhsf = _c(rhsc), _c(rhsf)
+        phic = np.zeros_like(rhsc) if phic0 is None else np.array(phic0, dtype=np.float64, order="C")
+        phif = np.zeros_like(rhsf) if phif0 is None else np.array(phif0, dtype=np.float64, order="C")
+        status = lib().oamr_solve(self._h, _p(rhsc), _p(rhsf), _p(phic), _p(phif), rtol, max_cycles)
+        if status != -5:
+            self._chk(status, "amr solve")
+        cyc, rr = C.c_int(), C.c_double()
+        hist = np.zeros(max_cycles + 1)
+        lib().oamr_get_info(self._h, C.byref(cyc), C.byref(rr), _p(hist))
+        return phic, phif, status, cyc.value, rr.value, hist[:cyc.value + 1].copy()
