@@ -257,6 +257,46 @@ int vmg_get_profile(vmg_handle h, double ms[8], long long launches[8]);
 #define VMG_NORM_INF_STATIC_MAX_N 134217728LL
 int vmg_norm_inf_static(const double* v, long long n, double* out, void* cuda_stream, const char** why);
 
+
+/* ---------------------------------------------------------------------------------------------------------------
+ * vmg_amr_* -- two-level COMPOSITE solve (second half).  The paper advances all AMR levels with one
+ * time step and solves every equation with "the composite multilevel multigrid solver from within AMReX";
+ * it gives no formula, so the interface discretisation and the cycle are readings A1-A5 of DESIGN.md (restated in
+ * oracle/amr_oracle.c, which this is tested against):
+ *   A1  one box patch of coarse cells [lo, hi) refined by 2, at least one coarse cell away from the box boundary and at
+ *       least two coarse cells wide in every active direction; the patch as a box of 2 (hi - lo) fine cells must itself be
+ *       a legal vmg grid with at least two levels (else VMG_ERR_SIZE);
+ *   A2  coarse-fine face: flux b_f (g - phi_f) / (1.5 hf) per unit area, g = the coarse field at the point of the adjacent
+ *       coarse cell opposite the fine cell centre, interpolated linearly in the tangential directions;
+ *   A3  the coarse cell takes the sum of the fine fluxes through its face (conservation);
+ *   A4  cycle: composite residual -> ONE V-cycle of the coarse box (options nu1, nu2, ... of the coarse handle) for it,
+ *       under the patch for the mean of the children's residuals -> correction added on both levels (piecewise constant)
+ *       -> nu_f = 6 red-black sweeps on the patch -> coarse cells under the patch = means of their children;
+ *   A5  relres = max(||r_c||_inf over uncovered coarse cells, ||r_f||_inf) / max(||btilde_c||_inf uncovered, ||f_f||_inf);
+ *       exit rules, status codes and history as vmg_solve (hist[c] = relres after c cycles).
+ * Arrays: DEVICE pointers.  Coarse arrays have the layouts of vmg_set_coeffs / vmg_solve on the nx x ny x nz box; fine
+ * arrays the same layouts on the patch as a box of fx x fy x fz = 2 (hi - lo) cells (fz = 1 when nz == 1; vmg_amr_fine_dims).
+ * Coefficients are BORROWED on both levels until the next vmg_amr_set_coeffs / vmg_amr_destroy; the coarse coefficients
+ * under the patch define the operator of the correction V-cycle there (keep them consistent with the fine ones, e.g.
+ * their averages); a_c and a_f are both given or both NULL.  rhs_c under the patch is ignored; phi_c, phi_f: initial guess
+ * in, solution out (phi_c under the patch: means of the children).  vmg_set_bc semantics for the box faces.
+ * Stream: as vmg_create (NULL: the library creates one); both levels run on it.  vmg_amr_solve synchronises it.
+ * Options: "nu_f" (1..64); every other key goes to the coarse handle (vmg_set_option).  No mask, no PCG on composite grids. */
+typedef struct vmg_amr_s* vmg_amr_handle;
+int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, double dy, double dz,
+                   const int lo[3], const int hi[3], void* cuda_stream);
+int vmg_amr_fine_dims(vmg_amr_handle h, int dims[3]);
+int vmg_amr_set_coeffs(vmg_amr_handle h, const double* a_c, const double* bx_c, const double* by_c, const double* bz_c,
+                       const double* a_f, const double* bx_f, const double* by_f, const double* bz_f, double alpha, double beta);
+int vmg_amr_set_bc(vmg_amr_handle h, const int type[6], const double* const value[6]);
+int vmg_amr_set_option(vmg_amr_handle h, const char* key, double v);
+int vmg_amr_solve(vmg_amr_handle h, const double* rhs_c, const double* rhs_f, double* phi_c, double* phi_f,
+                  double rtol, int max_cycles);
+int vmg_amr_get_info(vmg_amr_handle h, int* cycles, double* relres, double* history /* >= cycles + 1 or NULL */);
+long long vmg_amr_last_launch_count(vmg_amr_handle h);
+int vmg_amr_last_cuda_error(vmg_amr_handle h);
+int vmg_amr_destroy(vmg_amr_handle h);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,9 @@ SYMBOLS = ["vmg_create", "vmg_create_batch", "vmg_set_coeffs", "vmg_set_bc", "vm
            "vmg_get_level_coeffs", "vmg_step_fold_bc", "vmg_step_smooth", "vmg_step_residual",
            "vmg_step_residual_restrict", "vmg_step_prolong_correct", "vmg_step_down", "vmg_step_up", "vmg_step_vcycle", "vmg_step_norm_inf",
            "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile", "vmg_debug_pad_check",
-           "vmg_norm_inf_static"]
+           "vmg_norm_inf_static", "vmg_amr_create", "vmg_amr_fine_dims", "vmg_amr_set_coeffs", "vmg_amr_set_bc",
+           "vmg_amr_set_option", "vmg_amr_solve", "vmg_amr_get_info", "vmg_amr_last_launch_count",
+           "vmg_amr_last_cuda_error", "vmg_amr_destroy"]
 
 _lib = None
 _vp = C.c_void_p
@@ -71,6 +73,18 @@ def load():
     lib.vmg_get_profile.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     lib.vmg_debug_pad_check.argtypes = [_vp, C.POINTER(C.c_longlong)]
     lib.vmg_norm_inf_static.argtypes = [_vp, C.c_longlong, _vp, _vp, C.POINTER(C.c_char_p)]
+    _ip = C.POINTER(C.c_int)
+    lib.vmg_amr_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, _ip, _vp]
+    lib.vmg_amr_fine_dims.argtypes = [_vp, _ip]
+    lib.vmg_amr_set_coeffs.argtypes = [_vp] + [_vp] * 8 + [C.c_double, C.c_double]
+    lib.vmg_amr_set_bc.argtypes = [_vp, _ip, C.POINTER(_vp)]
+    lib.vmg_amr_set_option.argtypes = [_vp, C.c_char_p, C.c_double]
+    lib.vmg_amr_solve.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_double, C.c_int]
+    lib.vmg_amr_get_info.argtypes = [_vp, _ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.vmg_amr_last_launch_count.argtypes = [_vp]
+    lib.vmg_amr_last_launch_count.restype = C.c_longlong
+    lib.vmg_amr_last_cuda_error.argtypes = [_vp]
+    lib.vmg_amr_destroy.argtypes = [_vp]
     _lib = lib
     return lib
 
@@ -291,6 +305,70 @@ class Vmg:
         out = C.c_double()
         self._chk(self._lib.vmg_step_norm_inf(self._h, _ptr(v), v.numel(), C.byref(out)), "vmg_step_norm_inf")
         return out.value
+
+
+class VmgAmr:
+    """Two-level composite solve (vmg_amr_* of include/vmg.h): an nx x ny x nz box with one patch of coarse cells [lo, hi)
+    refined by 2.  Coarse tensors [k, j, i] on the box, fine tensors [K, J, I] on the patch."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, lo, hi, stream=None):
+        torch = _torch()
+        self._lib = load()
+        self._h = _vp()
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        sptr = self.stream.cuda_stream
+        l3, h3 = (C.c_int * 3)(*[int(v) for v in lo]), (C.c_int * 3)(*[int(v) for v in hi])
+        rc = self._lib.vmg_amr_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, l3, h3, _vp(sptr) if sptr else None)
+        if rc != 0:
+            self._h = None
+            raise VmgError(rc, "vmg_amr_create")
+        d = (C.c_int * 3)()
+        self._lib.vmg_amr_fine_dims(self._h, d)
+        self.coarse_shape, self.fine_shape = (nz, ny, nx), (d[2], d[1], d[0])
+        self._keep = None
+
+    def _chk(self, rc, where):
+        if rc < 0:
+            raise VmgError(rc, where, self._lib.vmg_amr_last_cuda_error(self._h))
+        return rc
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.vmg_amr_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    def set_coeffs(self, coarse, fine, alpha: float, beta: float):
+        """coarse, fine: (a, bx, by, bz) tuples of tensors (None: a = 0, b = 1); borrowed until the next call."""
+        self._keep = (tuple(coarse), tuple(fine))
+        ptrs = [_ptr(t) for t in list(coarse) + list(fine)]
+        self._chk(self._lib.vmg_amr_set_coeffs(self._h, *ptrs, alpha, beta), "vmg_amr_set_coeffs")
+
+    def set_bc(self, types, values=None):
+        t = (C.c_int * 6)(*[int(v) for v in types])
+        vals = list(values) if values is not None else [None] * 6
+        arr = (_vp * 6)(*[_ptr(v) for v in vals])
+        self._chk(self._lib.vmg_amr_set_bc(self._h, t, arr), "vmg_amr_set_bc")
+
+    def set_option(self, key: str, v: float):
+        self._chk(self._lib.vmg_amr_set_option(self._h, key.encode(), float(v)), "vmg_amr_set_option")
+
+    def solve(self, rhs_c, rhs_f, phi_c=None, phi_f=None, rtol: float = 1e-12, max_cycles: int = 50):
+        """Returns (phi_c, phi_f, status, cycles, relres, history); phi_c, phi_f are updated in place when given."""
+        torch = _torch()
+        phi_c = torch.zeros_like(rhs_c) if phi_c is None else phi_c
+        phi_f = torch.zeros_like(rhs_f) if phi_f is None else phi_f
+        status = self._lib.vmg_amr_solve(self._h, _ptr(rhs_c), _ptr(rhs_f), _ptr(phi_c), _ptr(phi_f), rtol, max_cycles)
+        if status != -5:
+            self._chk(status, "vmg_amr_solve")
+        cyc, rr = C.c_int(), C.c_double()
+        hist = (C.c_double * (max_cycles + 2))()
+        self._lib.vmg_amr_get_info(self._h, C.byref(cyc), C.byref(rr), hist)
+        return phi_c, phi_f, status, cyc.value, rr.value, [hist[i] for i in range(cyc.value + 1)]
+
+    def last_launch_count(self) -> int:
+        return int(self._lib.vmg_amr_last_launch_count(self._h))
 
 
 NORM_INF_STATIC_MAX_N = 134217728   # VMG_NORM_INF_STATIC_MAX_N of include/vmg.h

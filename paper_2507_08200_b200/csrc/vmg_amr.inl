@@ -1,0 +1,332 @@
+// vmg_amr.inl -- C-ABI of the two-level composite solve (include/vmg.h, "vmg_amr_*"; kernels and the design in
+// vmg_amr.cuh).  Included at the end of vmg_api.cu: it uses the single-level handles' internals.
+
+#include "vmg_amr.cuh"
+
+struct vmg_amr_s {
+    vmg_s* hc = nullptr;            // the coarse box (an ordinary handle: correction V-cycle, fold_bc)
+    vmg_s* hf = nullptr;            // the patch (an ordinary handle whose faces are coarse-fine faces)
+    AmrGeom A;
+    cudaStream_t stream = nullptr;
+    void* base = nullptr;           // one allocation: phi_c, btilde_c (padded like a level array), rhs_f copy, 4 scalars
+    double *phic = nullptr, *btc = nullptr, *rhsf = nullptr;
+    unsigned long long* d_norm = nullptr;   // ||btilde_c||, ||f_f||, ||r_c||, ||r_f|| (bit patterns)
+    double* h_norm = nullptr;       // pinned mirror
+    int nu_f = 6;                   // A4: fine sweeps per cycle
+    bool have_coeffs = false, have_bc = false;
+    cudaGraph_t graph[2] = {nullptr, nullptr};          // 0: composite residual + norms, 1: correction + fine sweeps
+    cudaGraphExec_t exec[2] = {nullptr, nullptr};
+    long long graph_launches[2] = {0, 0};
+    unsigned epoch_c = 0, epoch_f = 0;
+    int graph_nu_f = -1;
+    int cycles = 0, last_cuda_error = 0;
+    double relres = 0.0;
+    std::vector<double> hist;
+    long long launches = 0;
+};
+
+#define AMR_TRY(A_, expr)                                                      \
+    do {                                                                       \
+        cudaError_t e__ = (expr);                                              \
+        if (e__ != cudaSuccess) {                                              \
+            (A_)->last_cuda_error = (int)e__;                                  \
+            (void)cudaGetLastError();                                          \
+            return VMG_ERR_CUDA;                                               \
+        }                                                                      \
+    } while (0)
+
+namespace {
+
+void amr_drop_graphs(vmg_amr_s* a)
+{
+    for (int i = 0; i < 2; ++i) {
+        if (a->exec[i]) { cudaGraphExecDestroy(a->exec[i]); a->exec[i] = nullptr; }
+        if (a->graph[i]) { cudaGraphDestroy(a->graph[i]); a->graph[i] = nullptr; }
+    }
+}
+
+// value planes of the patch from the coarse field, then btilde_f = f_f + 2 wb g (the library's fold_bc)
+int amr_enqueue_ghost_fold(vmg_amr_s* a, long long* count)
+{
+    vmg_s* hf = a->hf;
+    AmrGhostArgs g;
+    g.A = a->A; g.phic = a->phic;
+    long long most = 0;
+    for (int f = 0; f < 6; ++f) {
+        g.plane[f] = hf->bcval[f];
+        if (f < 2 * a->A.nd) most = std::max<long long>(most, (long long)plane_count(hf->lev[0], f));
+    }
+    amr_ghost_kernel<<<dim3(grid_for(most), 2 * a->A.nd), kThreads, 0, a->stream>>>(g);
+    ++*count;
+    long long before = hf->launches;
+    int rc = enqueue_fold_bc(hf, a->rhsf, hf->lev[0].rhs);
+    *count += hf->launches - before;
+    return rc;
+}
+
+// graph 0: the composite residual (A3) -- the patch's residual + restriction and residual norm, then the coarse right-hand side
+void amr_enqueue_residual(vmg_amr_s* a, long long* count)
+{
+    vmg_s *hc = a->hc, *hf = a->hf;
+    cudaMemsetAsync(a->d_norm + 2, 0, 2 * sizeof(unsigned long long), a->stream);
+    hf->lev[0].cur = 0;
+    plain_residual_restrict(hf, 0, count);
+    enqueue_residual_norm(hf, a->d_norm + 3);
+    ++*count;
+    AmrResArgs g;
+    g.A = a->A; g.Lc = view(hc->lev[0]);
+    g.phic = a->phic; g.btc = a->btc; g.rs = hf->lev[1].rhs; g.phif = hf->lev[0].phi;
+    g.R = hc->lev[0].rhs;
+    for (int f = 0; f < 6; ++f) { g.gplane[f] = hf->bcval[f]; g.wbf[f] = hf->lev[0].wb[f]; }
+    g.wscale = 2.0 / (double)(1 << a->A.nd);
+    g.norm = a->d_norm + 2;
+    amr_coarse_residual_kernel<<<grid_for(a->A.C.n), kThreads, 0, a->stream>>>(g);
+    ++*count;
+}
+
+// graph 1: A4 after the exit test -- coarse V-cycle from zero, corrections, ghosts, fine sweeps, average down
+int amr_enqueue_correction(vmg_amr_s* a, long long* count)
+{
+    vmg_s *hc = a->hc, *hf = a->hf;
+    VmgLevel& C0 = hc->lev[0];
+    cudaMemsetAsync(C0.phi, 0, (size_t)C0.nalloc * sizeof(double), a->stream);
+    enqueue_vcycle(hc, nullptr, count);
+    amr_add_kernel<<<grid_for(C0.nalloc), kThreads, 0, a->stream>>>(a->phic, C0.phi, C0.nalloc);
+    amr_prolong_add_kernel<<<grid_for(a->A.F.n), kThreads, 0, a->stream>>>(a->A, hf->lev[0].phi, C0.phi);
+    *count += 2;
+    int rc = amr_enqueue_ghost_fold(a, count);
+    if (rc != VMG_OK) return rc;
+    hf->lev[0].cur = 0; hf->lev[0].dir = 0;
+    plain_smooth(hf, 0, a->nu_f, count);
+    amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, hf->lev[0].phi, a->phic);
+    ++*count;
+    return VMG_OK;
+}
+
+// runs part `which` (0 residual, 1 correction): a graph replay, or plain launches with option graph = 0 / profile on the coarse handle
+int amr_run(vmg_amr_s* a, int which)
+{
+    vmg_s *hc = a->hc, *hf = a->hf;
+    if (!hc->use_graph || hc->profile) {
+        long long count = 0;
+        int rc = VMG_OK;
+        if (which == 0) amr_enqueue_residual(a, &count); else rc = amr_enqueue_correction(a, &count);
+        a->launches += count;
+        if (rc != VMG_OK) return rc;
+        AMR_TRY(a, cudaGetLastError());
+        return VMG_OK;
+    }
+    if (!a->exec[0] || a->epoch_c != hc->graph_epoch || a->epoch_f != hf->graph_epoch || a->graph_nu_f != a->nu_f) {
+        amr_drop_graphs(a);
+        for (int i = 0; i < 2; ++i) {
+            long long count = 0;
+            AMR_TRY(a, cudaStreamBeginCapture(a->stream, cudaStreamCaptureModeRelaxed));
+            int rc = VMG_OK;
+            if (i == 0) amr_enqueue_residual(a, &count); else rc = amr_enqueue_correction(a, &count);
+            cudaError_t e = cudaStreamEndCapture(a->stream, &a->graph[i]);
+            if (rc != VMG_OK) return rc;
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&a->exec[i], a->graph[i], 0);
+            AMR_TRY(a, e);
+            a->graph_launches[i] = count;
+        }
+        a->epoch_c = hc->graph_epoch; a->epoch_f = hf->graph_epoch; a->graph_nu_f = a->nu_f;
+    }
+    AMR_TRY(a, cudaGraphLaunch(a->exec[which], a->stream));
+    a->launches += a->graph_launches[which];
+    return VMG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int vmg_amr_destroy(vmg_amr_handle a)
+{
+    if (!a) return VMG_ERR_ARG;
+    if (a->stream) cudaStreamSynchronize(a->stream);
+    amr_drop_graphs(a);
+    if (a->hf) vmg_destroy(a->hf);          // the patch first: the coarse handle may own the stream
+    if (a->hc) vmg_destroy(a->hc);
+    if (a->base) cudaFree(a->base);
+    if (a->h_norm) cudaFreeHost(a->h_norm);
+    (void)cudaGetLastError();
+    delete a;
+    return VMG_OK;
+}
+
+int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, double dy, double dz,
+                   const int lo[3], const int hi[3], void* cuda_stream)
+{
+    if (!out || !lo || !hi) return VMG_ERR_ARG;
+    *out = nullptr;
+    const int n[3] = {nx, ny, nz}, nd = nz > 1 ? 3 : 2;
+    int m[3] = {1, 1, 1};
+    for (int d = 0; d < nd; ++d) {
+        // A1: inside the box, one coarse cell away from its boundary, at least two coarse cells wide
+        if (lo[d] < 1 || hi[d] > n[d] - 1 || hi[d] - lo[d] < 2) return VMG_ERR_SIZE;
+        m[d] = 2 * (hi[d] - lo[d]);
+    }
+    vmg_amr_s* a = new (std::nothrow) vmg_amr_s();
+    if (!a) return VMG_ERR_ALLOC;
+    int rc = vmg_create(&a->hc, nx, ny, nz, dx, dy, dz, cuda_stream);
+    if (rc == VMG_OK) {
+        a->stream = a->hc->stream;
+        rc = vmg_create(&a->hf, m[0], m[1], m[2], 0.5 * dx, 0.5 * dy, nd == 3 ? 0.5 * dz : dz, (void*)a->stream);
+        if (rc == VMG_OK && a->hf->nlev < 2) rc = VMG_ERR_SIZE;
+    }
+    if (rc != VMG_OK) { vmg_amr_destroy(a); return rc; }
+    a->hf->l2_persist_mb = 0.0;             // one stream: the access-policy window belongs to the coarse box
+    a->A.C = a->hc->lev[0].G; a->A.F = a->hf->lev[0].G; a->A.S = a->hf->lev[1].G;
+    a->A.nd = nd;
+    for (int d = 0; d < 3; ++d) { a->A.lo[d] = d < nd ? lo[d] : 0; a->A.hi[d] = d < nd ? hi[d] : 1; }
+    const VmgLevel& C0 = a->hc->lev[0];
+    const size_t arr = (size_t)C0.nalloc + 2 * (size_t)C0.pad;
+    const size_t total = 2 * round_up(arr, 32) + round_up((size_t)a->hf->lev[0].n, 32) + 32;
+    if (cudaMalloc(&a->base, total * sizeof(double)) != cudaSuccess ||
+        cudaMallocHost((void**)&a->h_norm, 4 * sizeof(double)) != cudaSuccess ||
+        cudaMemsetAsync(a->base, 0, total * sizeof(double), a->stream) != cudaSuccess ||
+        cudaStreamSynchronize(a->stream) != cudaSuccess) {
+        (void)cudaGetLastError();
+        vmg_amr_destroy(a);
+        return VMG_ERR_ALLOC;
+    }
+    double* b = (double*)a->base;
+    a->phic = b + C0.pad;
+    a->btc = b + round_up(arr, 32) + C0.pad;
+    a->rhsf = b + 2 * round_up(arr, 32);
+    a->d_norm = (unsigned long long*)(a->rhsf + round_up((size_t)a->hf->lev[0].n, 32));
+    *out = a;
+    return VMG_OK;
+}
+
+int vmg_amr_fine_dims(vmg_amr_handle a, int dims[3])
+{
+    if (!a || !dims) return VMG_ERR_ARG;
+    dims[0] = a->A.F.nx; dims[1] = a->A.F.ny; dims[2] = a->A.F.nz;
+    return VMG_OK;
+}
+
+int vmg_amr_set_coeffs(vmg_amr_handle a, const double* a_c, const double* bx_c, const double* by_c, const double* bz_c,
+                       const double* a_f, const double* bx_f, const double* by_f, const double* bz_f, double alpha, double beta)
+{
+    if (!a) return VMG_ERR_ARG;
+    if (!a_c != !a_f) return VMG_ERR_ARG;                  // the absorption term exists on both levels or on neither
+    int rc = vmg_set_coeffs(a->hc, a_c, bx_c, by_c, bz_c, alpha, beta);
+    if (rc != VMG_OK) { a->last_cuda_error = a->hc->last_cuda_error; return rc; }
+    rc = vmg_set_coeffs(a->hf, a_f, bx_f, by_f, bz_f, alpha, beta);
+    if (rc != VMG_OK) { a->last_cuda_error = a->hf->last_cuda_error; return rc; }
+    // A2: the patch's faces carry beta b / (1.5 hf^2) = 2 * (beta b / hf^2) / 3: scale its boundary planes, then 1/D again
+    VmgLevel& F0 = a->hf->lev[0];
+    for (int f = 0; f < 2 * a->A.nd; ++f) {
+        const long long np = (long long)plane_count(F0, f);
+        amr_scale_kernel<<<grid_for(np), kThreads, 0, a->stream>>>(F0.wb[f], np, 1.0 / 3.0);
+    }
+    AMR_TRY(a, cudaGetLastError());
+    a->hf->dinv_dirty = true;
+    a->have_coeffs = true;
+    return VMG_OK;
+}
+
+int vmg_amr_set_bc(vmg_amr_handle a, const int type[6], const double* const value[6])
+{
+    if (!a || !type) return VMG_ERR_ARG;
+    int rc = vmg_set_bc(a->hc, type, value);
+    if (rc != VMG_OK) return rc;
+    const int all_dirichlet[6] = {VMG_BC_DIRICHLET, VMG_BC_DIRICHLET, VMG_BC_DIRICHLET, VMG_BC_DIRICHLET, VMG_BC_DIRICHLET, VMG_BC_DIRICHLET};
+    rc = vmg_set_bc(a->hf, all_dirichlet, nullptr);
+    if (rc != VMG_OK) return rc;
+    for (int f = 0; f < 2 * a->A.nd; ++f) a->hf->bc_has_value[f] = true;   // the planes are written by amr_ghost_kernel
+    a->have_bc = true;
+    return VMG_OK;
+}
+
+int vmg_amr_set_option(vmg_amr_handle a, const char* key, double v)
+{
+    if (!a || !key) return VMG_ERR_ARG;
+    if (!strcmp(key, "nu_f")) { if (v < 1 || v > 64) return VMG_ERR_ARG; a->nu_f = (int)v; return VMG_OK; }
+    return vmg_set_option(a->hc, key, v);
+}
+
+int vmg_amr_get_info(vmg_amr_handle a, int* cycles, double* relres, double* history)
+{
+    if (!a) return VMG_ERR_ARG;
+    if (cycles) *cycles = a->cycles;
+    if (relres) *relres = a->relres;
+    if (history) memcpy(history, a->hist.data(), a->hist.size() * sizeof(double));
+    return VMG_OK;
+}
+
+long long vmg_amr_last_launch_count(vmg_amr_handle a) { return a ? a->launches : 0; }
+int vmg_amr_last_cuda_error(vmg_amr_handle a) { return a ? a->last_cuda_error : 0; }
+
+int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, double* phi_c, double* phi_f,
+                  double rtol, int max_cycles)
+{
+    if (!a || !rhs_c || !rhs_f || !phi_c || !phi_f || max_cycles < 0) return VMG_ERR_ARG;
+    if (!a->have_coeffs || !a->have_bc) return VMG_ERR_STATE;
+    vmg_s *hc = a->hc, *hf = a->hf;
+    int rc = ready(hc);
+    if (rc == VMG_OK) rc = ready(hf);
+    if (rc != VMG_OK) return rc;
+    VmgLevel &C0 = hc->lev[0], &F0 = hf->lev[0];
+    a->hist.clear(); a->cycles = 0; a->relres = 0.0; a->launches = 0;
+    // begin: btilde_c (box boundary values folded, zero under the patch), the two norms of A5, phi into the internal layouts
+    AMR_TRY(a, cudaMemsetAsync(a->d_norm, 0, 4 * sizeof(unsigned long long), a->stream));
+    rc = enqueue_fold_bc(hc, rhs_c, a->btc);
+    if (rc != VMG_OK) return rc;
+    amr_mask_norm_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(a->A, a->btc, a->d_norm + 0);
+    norm_inf_kernel<<<std::min<unsigned>(grid_for(F0.n), 4u * hf->num_sms), kThreads, 0, a->stream>>>(rhs_f, F0.n, a->d_norm + 1);
+    AMR_TRY(a, cudaMemcpyAsync(a->rhsf, rhs_f, (size_t)F0.n * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
+    to_internal_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(C0.G, phi_c, a->phic, nullptr);
+    to_internal_kernel<<<grid_for(F0.n), kThreads, 0, a->stream>>>(F0.G, phi_f, F0.phi, nullptr);
+    amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, F0.phi, a->phic);
+    long long count = 6;
+    rc = amr_enqueue_ghost_fold(a, &count);
+    if (rc != VMG_OK) return rc;
+    a->launches += count;
+    AMR_TRY(a, cudaGetLastError());
+    int status = VMG_MAXCYCLES, slow = 0;
+    double nb = 0.0;
+    for (int c = 0;; ++c) {
+        rc = amr_run(a, 0);
+        if (rc != VMG_OK) return rc;
+        AMR_TRY(a, cudaMemcpyAsync(a->h_norm, a->d_norm, 4 * sizeof(double), cudaMemcpyDeviceToHost, a->stream));
+        AMR_TRY(a, cudaStreamSynchronize(a->stream));
+        if (c == 0) {
+            nb = std::max(a->h_norm[0], a->h_norm[1]);
+            if (std::isnan(a->h_norm[0]) || std::isnan(a->h_norm[1])) nb = a->h_norm[0] + a->h_norm[1];
+            if (nb == 0.0) {                               // zero data: phi = 0
+                AMR_TRY(a, cudaMemsetAsync(phi_c, 0, (size_t)C0.n * sizeof(double), a->stream));
+                AMR_TRY(a, cudaMemsetAsync(phi_f, 0, (size_t)F0.n * sizeof(double), a->stream));
+                AMR_TRY(a, cudaStreamSynchronize(a->stream));
+                a->hist.push_back(0.0);
+                return VMG_OK;
+            }
+        }
+        const double rcn = a->h_norm[2], rfn = a->h_norm[3];
+        a->relres = (std::isnan(rcn) || std::isnan(rfn)) ? rcn + rfn : std::max(rcn, rfn) / nb;
+        a->hist.push_back(a->relres);
+        a->cycles = c;
+        if (std::isnan(a->relres) || std::isinf(a->relres)) { status = VMG_ERR_DIVERGED; break; }
+        if (rtol > 0.0) {
+            if (a->relres <= rtol) { status = VMG_OK; break; }
+            if (c > 0) {
+                slow = (a->hist[c] >= 0.9 * a->hist[c - 1]) ? slow + 1 : 0;
+                if (slow >= 3) { status = VMG_STALLED; break; }
+            }
+        }
+        if (c == max_cycles) { status = VMG_MAXCYCLES; break; }
+        rc = amr_run(a, 1);
+        if (rc != VMG_OK) return rc;
+    }
+    if (status >= 0) {
+        to_natural_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(C0.G, a->phic, phi_c);
+        to_natural_kernel<<<grid_for(F0.n), kThreads, 0, a->stream>>>(F0.G, F0.phi, phi_f);
+        a->launches += 2;
+        AMR_TRY(a, cudaGetLastError());
+    }
+    AMR_TRY(a, cudaStreamSynchronize(a->stream));
+    return status;
+}
+
+}  // extern "C"

@@ -964,6 +964,7 @@ int vmg_solve_batch(int n, const vmg_handle* hs, const double* const* rhs, doubl
 }  // extern "C"
 
 #include "vmg_steps.inl"
+#include "vmg_amr.inl"
 
 #ifdef VMG_TAIL_TIMING
 // debug build only (-DVMG_TAIL_TIMING): clock64 stamps of the last coarse_tail_kernel launch (vmg_tail.cuh TAIL_MARK)

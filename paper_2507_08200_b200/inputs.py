@@ -304,3 +304,119 @@ def random_problem(nx: int, ny: int, nz: int, seed: int = 0, bc_type=None, alpha
 
 
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
+
+
+# --------------------------------------------------------------------------------------------------
+# Two-level composite (AMR) inputs, SURVEY.md 8(f) N4 second half: a coarse box and one patch of coarse cells [lo, hi)
+# refined by 2 (the paper refines where the reduced field and the electron density are large, i.e. around the streamer
+# heads).  Every field is an analytic function (or a seeded GRF) sampled on both levels, so the coarse
+# coefficients under the patch are consistent with the fine ones.  Fine arrays: the patch as a box of 2 (hi - lo) cells.
+# --------------------------------------------------------------------------------------------------
+@dataclass
+class AmrProblem:
+    name: str
+    coarse: Problem                 # the box: coefficients, BC types and value planes, rhs (entries under the patch unused)
+    lo: tuple
+    hi: tuple
+    a_f: Optional[np.ndarray]
+    bx_f: Optional[np.ndarray]
+    by_f: Optional[np.ndarray]
+    bz_f: Optional[np.ndarray]
+    rhs_f: np.ndarray
+    rtol: float = 1e-12
+    max_cycles: int = 50
+
+    @property
+    def fine_dims(self):
+        c = self.coarse
+        nd = 3 if c.nz > 1 else 2
+        return tuple(2 * (self.hi[d] - self.lo[d]) if d < nd else 1 for d in range(3))
+
+    def coarse_coeffs(self):
+        c = self.coarse
+        return (c.a, c.bx, c.by, c.bz)
+
+    def fine_coeffs(self):
+        return (self.a_f, self.bx_f, self.by_f, self.bz_f)
+
+
+def _patch_axes(p: Problem, lo, hi):
+    """cell-centre and face coordinates of the patch's fine cells along x, y, z"""
+    nd = 3 if p.nz > 1 else 2
+    h = (p.dx, p.dy, p.dz)
+    cen, fac = [], []
+    for d in range(3):
+        if d < nd:
+            m = 2 * (hi[d] - lo[d])
+            cen.append(lo[d] * h[d] + _centres(m, h[d] / 2))
+            fac.append(lo[d] * h[d] + _faces(m, h[d] / 2))
+        else:
+            cen.append(_centres(1, h[d]))
+            fac.append(_faces(1, h[d]))
+    return cen, fac
+
+
+def amr_random_problem(nx: int, ny: int, nz: int, lo, hi, seed: int = 0, bc_type=None, alpha: float = 1.0,
+                       a_scale: float = 10.0, ell: float = 0.4, sigma: float = 1.0, spacing=None) -> AmrProblem:
+    """random_problem on the box with the same coefficient fields (GRFs) sampled on the patch's fine cells and faces."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    if spacing is None:
+        h = 1.0 / max(ny, 2)
+        spacing = (h, h, h)
+    dx, dy, dz = spacing
+    xc, yc, zc = _centres(nx, dx), _centres(ny, dy), _centres(nz, dz)
+    xf, yf, zf = _faces(nx, dx), _faces(ny, dy), _faces(nz, dz)
+    gb = GRF.draw(int(rng.integers(1 << 30)), ell=ell, sigma=sigma, modes=16)
+    ga = GRF.draw(int(rng.integers(1 << 30)), ell=ell, sigma=0.5, modes=16)
+    if bc_type is None:
+        bc_type = [DIRICHLET, NEUMANN, NEUMANN, DIRICHLET, DIRICHLET, NEUMANN]
+    shapes = [(nz, ny), (nz, ny), (nz, nx), (nz, nx), (ny, nx), (ny, nx)]
+    val = [rng.standard_normal(s) for s in shapes]
+    coarse = Problem(
+        name=f"amr_box_{nx}x{ny}x{nz}_s{seed}", nx=nx, ny=ny, nz=nz, dx=dx, dy=dy, dz=dz, alpha=alpha, beta=1.0,
+        a=a_scale * np.exp(ga.evaluate(xc, yc, zc)) if alpha > 0.0 else None,
+        bx=np.exp(gb.evaluate(xf, yc, zc)), by=np.exp(gb.evaluate(xc, yf, zc)),
+        bz=np.exp(gb.evaluate(xc, yc, zf)) if nz > 1 else None,
+        bc_type=list(bc_type), bc_value=val, rhs=rng.standard_normal((nz, ny, nx)))
+    (cx, cy, cz), (fx, fy, fz) = _patch_axes(coarse, lo, hi)
+    m = tuple(len(v) for v in (cx, cy, cz))
+    return AmrProblem(
+        name=f"amr_random_{nx}x{ny}x{nz}_s{seed}", coarse=coarse, lo=tuple(lo), hi=tuple(hi),
+        a_f=a_scale * np.exp(ga.evaluate(cx, cy, cz)) if alpha > 0.0 else None,
+        bx_f=np.exp(gb.evaluate(fx, cy, cz)), by_f=np.exp(gb.evaluate(cx, fy, cz)),
+        bz_f=np.exp(gb.evaluate(cx, cy, fz)) if nz > 1 else None,
+        rhs_f=rng.standard_normal((m[2], m[1], m[0])))
+
+
+def amr_streamer(ny: int = 128, seed: int = 1013, explicit_b: bool = True) -> AmrProblem:
+    """Config 3 (Poisson, streamer-shaped space charge) with the region around the streamer head x_h = (1.2, 0.5, 0.5)
+    refined: patch [15/16, 23/16] x [3/8, 5/8]^2 in units of L_y, i.e. 64 x 32 x 32 coarse cells of the 256 x 128 x 128
+    box -> 128 x 64 x 64 fine cells."""
+    base = config3(ny)
+    lo = (15 * ny // 16, 3 * ny // 8, 3 * ny // 8)
+    hi = (23 * ny // 16, 5 * ny // 8, 5 * ny // 8)
+    (cx, cy, cz), _ = _patch_axes(base, lo, hi)
+    R, xh = 0.05, (1.2, 0.5, 0.5)
+    rng = np.random.Generator(np.random.PCG64(seed))
+
+    def charge(xs, ys, zs):                                  # n_ion - n_e of config 3, with this level's own noise
+        r2 = ((xs - xh[0]) ** 2)[None, None, :] + ((ys - xh[1]) ** 2)[None, :, None] + ((zs - xh[2]) ** 2)[:, None, None]
+        n_e = np.exp(-r2 / R ** 2) + 0.01 * rng.random((len(zs), len(ys), len(xs)))
+        rho2 = ((ys - 0.5) ** 2)[None, :, None] + ((zs - 0.5) ** 2)[:, None, None]
+        n_ion = 0.8 * np.exp(-rho2 / R ** 2) * (0.5 * (1.0 + np.tanh((1.2 - xs) / R)))[None, None, :]
+        return n_ion - n_e
+
+    nx, nz = base.nx, base.nz
+    raw_c = charge(_centres(nx, base.dx), _centres(ny, base.dy), _centres(nz, base.dz))
+    scale = np.abs(raw_c).max()                              # one normalisation for both levels
+    base.rhs = np.ascontiguousarray(raw_c / scale)
+    rhs_f = np.ascontiguousarray(charge(cx, cy, cz) / scale)
+    m = (len(cx), len(cy), len(cz))
+    ones = lambda shape: np.ones(shape) if explicit_b else None
+    if not explicit_b:
+        base.bx = base.by = base.bz = None
+    base.a = None
+    return AmrProblem(
+        name=f"amr_streamer_{nx}x{ny}x{nz}_patch{m[0]}x{m[1]}x{m[2]}", coarse=base, lo=lo, hi=hi, a_f=None,
+        bx_f=ones((m[2], m[1], m[0] + 1)), by_f=ones((m[2], m[1] + 1, m[0])), bz_f=ones((m[2] + 1, m[1], m[0])),
+        rhs_f=rhs_f)
