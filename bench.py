@@ -330,6 +330,57 @@ def timestep_leg(binding, torch, p, d, d_bc, dev, s, flush, nsteps: int = 3, rto
 # ----------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ----------------------------------------------------------------------------------------------------
+def amr_leg(binding, torch, dev, flush, ny: int, steps: int = 5, with_oracle: bool = True):
+    """Two-level composite solve (second half): config 3 with the streamer head
+    refined -- the 2 ny x ny x ny box plus a patch of ny x ny/2 x ny/2 fine cells -- through vmg_amr_*; explicit arrays of
+    ones on both levels as in the headline run.  Device-resident inputs, CUDA events on the solver's stream, L2 flushed
+    between solves.  The oracle (oracle/amr_oracle.c) is timed beside it on ONE solve."""
+    from paper_2507_08200_b200 import inputs
+    p = inputs.amr_streamer(ny)
+    c = p.coarse
+    up = lambda x: None if x is None else torch.from_numpy(np.ascontiguousarray(x)).to(dev)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        s = binding.VmgAmr(c.nx, c.ny, c.nz, c.dx, c.dy, c.dz, p.lo, p.hi, stream=stream)
+        coarse, fine = [up(x) for x in p.coarse_coeffs()], [up(x) for x in p.fine_coeffs()]
+        bc = [up(v) for v in c.bc_value]
+        rhs_c, rhs_f = up(c.rhs), up(p.rhs_f)
+        phi_c, phi_f = torch.zeros_like(rhs_c), torch.zeros_like(rhs_f)
+        s.set_coeffs(coarse, fine, c.alpha, c.beta)
+        s.set_bc(c.bc_type, bc)
+        times, cyc, st, rr = [], 0, 0, 0.0
+        for it in range(steps + 2):
+            phi_c.zero_(); phi_f.zero_()
+            flush.fill_(1.0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            _, _, st, cyc, rr, hist = s.solve(rhs_c, rhs_f, phi_c, phi_f, rtol=p.rtol, max_cycles=p.max_cycles)
+            e1.record(stream)
+            e1.synchronize()
+            assert st == 0, f"composite solve status {st}"
+            if it >= 2:
+                times.append(e0.elapsed_time(e1) * 1e-3)
+        launches = s.last_launch_count()
+    stream.synchronize()
+    nf = int(np.prod(p.fine_dims))
+    out = {"workload": p.name, "coarse_cells": c.ncells, "fine_cells": nf, "solve_ms": float(np.mean(times)) * 1e3,
+           "solves_per_s": 1.0 / float(np.mean(times)), "cycles": cyc, "ms_per_cycle": float(np.mean(times)) * 1e3 / max(cyc, 1),
+           "relres": rr, "launches_per_solve": int(launches), "nu_f": 6,
+           "cycle": "composite residual -> one V(3,3) cycle of the box -> correction -> 6 red-black sweeps on the patch"}
+    if with_oracle:
+        from oracle import AmrOracle
+        o = AmrOracle(c.nx, c.ny, c.nz, c.dx, c.dy, c.dz, p.lo, p.hi)
+        o.set_coeffs(p.coarse_coeffs(), p.fine_coeffs(), c.alpha, c.beta)
+        o.set_bc(c.bc_type, c.bc_value)
+        t0 = time.perf_counter()
+        r = o.solve(c.rhs, p.rhs_f, rtol=p.rtol, max_cycles=p.max_cycles)
+        dt = time.perf_counter() - t0
+        err = max(float(np.abs(phi_f.cpu().numpy() - r[1]).max()), float(np.abs(phi_c.cpu().numpy() - r[0]).max())) / float(np.abs(r[0]).max())
+        out["oracle"] = {"solve_s": dt, "cycles": r[3], "cores": os.cpu_count(), "rel_linf_gpu_vs_oracle": err}
+    s.destroy()
+    return out
+
+
 def run_vmg(args):
     import torch
     from paper_2507_08200_b200 import binding
@@ -547,6 +598,9 @@ def run_vmg(args):
     timestep = None
     if args.config == 3 and not args.no_timestep:
         timestep = timestep_leg(binding, torch, p, d, d_bc, dev, s, flush)
+    amr = None
+    if args.config == 3 and not args.no_amr and world == 1:
+        amr = amr_leg(binding, torch, dev, flush, p.ny, with_oracle=not args.no_cpu_baseline)
 
     # end to end through the C-ABI with host buffers
     etimes, ecycles, _ = timed(step_e2e, args.steps, max(1, min(args.warmup, 2)))
@@ -582,6 +636,7 @@ def run_vmg(args):
         "const_weights": const_w,
         "batched": batched,
         "timestep": timestep,
+        "amr": amr,
         "e2e": {"value": e2e_value, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": etotal / args.steps * 1e3},
         "gpu_launches": int(launches),
@@ -689,6 +744,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-timestep", action="store_true", help="skip the per-time-step sequence leg")
+    ap.add_argument("--no-amr", action="store_true", help="skip the two-level composite (AMR) leg")
     ap.add_argument("--batch", type=int, default=8, help="K for the batched multi-component leg (0/1: skip)")
     ap.add_argument("--opt", action="append", default=[], help="vmg_set_option key=value (experiments)")
     ap.add_argument("--traffic-from", nargs=2, metavar=("COLD_CSV", "WARM_CSV"),
