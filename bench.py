@@ -745,6 +745,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-timestep", action="store_true", help="skip the per-time-step sequence leg")
     ap.add_argument("--no-amr", action="store_true", help="skip the two-level composite (AMR) leg")
+    ap.add_argument("--amr-only", action="store_true",
+                    help="profiling aid: run only the composite (AMR) leg (--steps solves after 2 untimed ones), print its JSON and exit")
     ap.add_argument("--batch", type=int, default=8, help="K for the batched multi-component leg (0/1: skip)")
     ap.add_argument("--opt", action="append", default=[], help="vmg_set_option key=value (experiments)")
     ap.add_argument("--traffic-from", nargs=2, metavar=("COLD_CSV", "WARM_CSV"),
@@ -757,6 +759,13 @@ def main():
         write_traffic_json(args)
     elif args.blocked_probe:
         run_blocked_probe(args)
+    elif args.amr_only:
+        import torch
+        from paper_2507_08200_b200 import binding
+        torch.cuda.set_device(0)
+        dev = torch.device("cuda", 0)
+        flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)
+        print(json.dumps({"amr": amr_leg(binding, torch, dev, flush, 128, steps=args.steps, with_oracle=False)}))
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -8,8 +8,9 @@
 // "Dirichlet" faces with the boundary-face weight scaled by 1/3 -- 2 * (beta b / 3 hf^2) = beta b / (1.5 hf^2) is exactly
 // the coarse-fine weight -- and whose value planes are rewritten from the coarse field before every fold (amr_ghost_kernel).
 // Smoother, residual + restriction, norms and fold_bc of the patch are then the library's own kernels.  The COARSE BOX is
-// an ordinary handle too: its V-cycle is the correction solver; the composite residual of its uncovered cells is the
-// library's residual with the flux through a face of the patch replaced by the fine fluxes (amr_coarse_residual_kernel).
+// an ordinary handle too: its V-cycle, run in place on phi_c with a right-hand side that differs from btilde_c only in and
+// next to the patch, is the correction solver; the composite residual of its uncovered cells is the library's residual with
+// the flux through a face of the patch replaced by the fine fluxes (amr_coarse_residual_kernel).
 #pragma once
 #include "vmg_kernels.cuh"
 
@@ -56,8 +57,10 @@ __global__ void amr_ghost_kernel(AmrGhostArgs g)
     g.plane[f][t] = gv;
 }
 
-// the coarse cells under the patch become the means of their children (A4); one thread per shadow cell
-__global__ void amr_average_down_kernel(AmrGeom A, const double* __restrict__ phif, double* __restrict__ phic)
+// the coarse cells under the patch become the means of their children (A4); one thread per shadow cell.  The mean is
+// also kept in old[] (shadow order): the coarse V-cycle runs in place on phi_c, and the correction the patch receives
+// is the difference to this value (amr_prolong_add_kernel).
+__global__ void amr_average_down_kernel(AmrGeom A, const double* __restrict__ phif, double* __restrict__ phic, double* __restrict__ old)
 {
     const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (t >= A.S.n) return;
@@ -68,7 +71,9 @@ __global__ void amr_average_down_kernel(AmrGeom A, const double* __restrict__ ph
     for (int s = 0; s < ns; ++s)
         for (int q = 0; q < 2; ++q)
             for (int p = 0; p < 2; ++p) sum += phif[cell_at(A.F, 2 * i + p, 2 * j + q, A.nd == 3 ? 2 * k + s : 0)];
-    phic[cell_at(A.C, A.lo[0] + i, A.lo[1] + j, A.nd == 3 ? A.lo[2] + k : 0)] = sum / (A.nd == 3 ? 8.0 : 4.0);
+    const double mean = sum / (A.nd == 3 ? 8.0 : 4.0);
+    phic[cell_at(A.C, A.lo[0] + i, A.lo[1] + j, A.nd == 3 ? A.lo[2] + k : 0)] = mean;
+    old[t] = mean;
 }
 
 // A5: the folded coarse right-hand side does not count under the patch: zero it there, ||.||_inf of the rest -> *norm
@@ -87,11 +92,22 @@ __global__ void amr_mask_norm_kernel(AmrGeom A, double* __restrict__ btc, unsign
     block_max_to_global(v, norm);
 }
 
-// A3 + A4: the right-hand side of the coarse correction.  Uncovered cell: btilde - A phi of the composite operator = the
-// library's residual, with the flux through a face shared with a covered cell replaced by the fluxes of the fine faces on
-// it (weights: the patch handle's scaled boundary planes, 2 wb / 2^nd = beta b_f / (1.5 hf) * area_f / volume_C; g: the
-// patch's value planes).  Covered cell: the mean of its children's residuals (rs, written by residual_restrict_kernel of
-// the patch).  ||.||_inf over the uncovered cells -> *norm.
+// A3 + A4: the right-hand side of the coarse V-cycle, which runs IN PLACE on phi_c (solution form): one V-cycle maps
+// (phi, rhs) to phi + B (rhs - A phi), so with rhs' = R + A phi_c (R: the right-hand side of the correction equation of A4,
+// A: the plain coarse operator) it returns phi_c + B R, the corrected field -- and rhs' differs from btilde_c only where R
+// is not the plain residual: on the covered cells and on the cells that share a face with the patch.  This kernel rewrites
+// exactly those entries every cycle (one thread per cell of the patch's bounding box grown by one cell); every other
+// entry of rhs' is btilde_c, copied once per solve.
+//   uncovered cell next to the patch:  rhs' = btilde + (the coarse flux through the shared face taken out, the fluxes of the
+//                                      fine faces on it put in; weights: the patch handle's scaled boundary planes,
+//                                      2 wb / 2^nd = beta b_f / (1.5 hf) * area_f / volume_C; g: the patch's value planes)
+//   covered cell:                      rhs' = R + A phi_c,  R = mean of the children's residuals (rs, residual_restrict_kernel
+//                                      of the patch)
+// With this rhs' the library's own residual norm over the box (residual_norm_kernel on rhs') IS the composite norm of A5:
+// rhs' - A phi is the composite residual on every uncovered cell and R on the covered ones, where |mean of the children's
+// residuals| <= ||r_f||_inf, which A5 takes anyway.  That kernel skips the black cells after the first cycle (R12: the
+// V-cycle's last half-sweep has just relaxed them) -- but the black cells next to the patch changed their right-hand side
+// since, so this kernel adds the residual of EVERY cell next to the patch to *norm itself.
 struct AmrResArgs {
     AmrGeom A; LevelView Lc;
     const double *phic, *btc, *rs, *phif;
@@ -101,33 +117,39 @@ struct AmrResArgs {
     unsigned long long* norm;
 };
 
-__global__ void amr_coarse_residual_kernel(AmrResArgs g)
+__global__ void amr_patch_rhs_kernel(AmrResArgs g)
 {
     const AmrGeom& A = g.A;
     const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    int ext[3] = {1, 1, 1};
+    for (int a = 0; a < A.nd; ++a) ext[a] = A.hi[a] - A.lo[a] + 2;
     double mx = 0.0;
-    if (t < A.C.n) {
-        int ci[3];
-        unflatten(A.C, t, ci[0], ci[1], ci[2]);
+    if (t < (long long)ext[0] * ext[1] * ext[2]) {
+        int ci[3] = {0, 0, 0};
+        ci[0] = (int)(t % ext[0]) + A.lo[0] - 1;
+        ci[1] = (int)((t / ext[0]) % ext[1]) + A.lo[1] - 1;
+        if (A.nd == 3) ci[2] = (int)(t / ((long long)ext[0] * ext[1])) + A.lo[2] - 1;
         long long c, xm;
         pair_addr(A.C, A.C.plane * ci[2] + (long long)A.C.pitch * ci[1], ci[0] >> 1, ci[0] & 1, c, xm);
-        double r;
         if (amr_covered(A, ci[0], ci[1], ci[2])) {
-            r = g.rs[cell_at(A.S, ci[0] - A.lo[0], ci[1] - A.lo[1], A.nd == 3 ? ci[2] - A.lo[2] : 0)];
+            const double rs = g.rs[cell_at(A.S, ci[0] - A.lo[0], ci[1] - A.lo[1], A.nd == 3 ? ci[2] - A.lo[2] : 0)];
+            g.R[c] = rs + (g.phic[c] / g.Lc.dinv[c] - nb_sum(g.Lc, g.phic, c, xm));
         } else {
-            r = residual_at(g.Lc, g.phic, g.btc, c, xm);
             const int m[3] = {A.F.nx, A.F.ny, A.F.nz};
+            double corr = 0.0;
+            bool touched = false;
             for (int f = 0; f < 2 * A.nd; ++f) {
                 const int d = f >> 1, side = f & 1;
                 int q[3] = {ci[0], ci[1], ci[2]};
                 q[d] += side ? 1 : -1;
-                if (q[d] < 0 || q[d] >= (d == 0 ? A.C.nx : d == 1 ? A.C.ny : A.C.nz) || !amr_covered(A, q[0], q[1], q[2])) continue;
+                if (!amr_covered(A, q[0], q[1], q[2])) continue;
+                touched = true;
                 // the coarse face weight and the covered neighbour, as nb_sum addresses them
                 const long long nb = d == 0 ? (side ? xm + 1 : xm) : d == 1 ? (side ? c + A.C.pitch : c - A.C.pitch)
                                                                             : (side ? c + A.C.plane : c - A.C.plane);
                 const double* warr = d == 0 ? g.Lc.wx : d == 1 ? g.Lc.wy : g.Lc.wz;
                 const double wface = warr[side ? nb : c];
-                r += wface * (g.phic[c] - g.phic[nb]);                 // take the coarse flux out ...
+                corr += wface * (g.phic[c] - g.phic[nb]);              // take the coarse flux out ...
                 int ua, va;
                 amr_plane_axes(d, ua, va);
                 const int ff = 2 * d + (1 - side), nt = A.nd - 1;
@@ -138,32 +160,30 @@ __global__ void amr_coarse_residual_kernel(AmrResArgs g)
                     F[d] = side ? 0 : m[d] - 1;
                     for (int a = 0; a < nt; ++a) F[ta[a]] = 2 * (ci[ta[a]] - A.lo[ta[a]]) + ((u >> a) & 1);
                     const long long pi = F[ua] + (long long)m[ua] * F[va];
-                    r -= g.wbf[ff][pi] * g.wscale * (g.gplane[ff][pi] - g.phif[cell_at(A.F, F[0], F[1], F[2])]);
+                    corr -= g.wbf[ff][pi] * g.wscale * (g.gplane[ff][pi] - g.phif[cell_at(A.F, F[0], F[1], F[2])]);
                 }
             }
-            mx = fabs(r);
-            if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
+            if (touched) {
+                g.R[c] = g.btc[c] + corr;
+                mx = fabs(residual_at(g.Lc, g.phic, g.btc, c, xm) + corr);
+                if (mx != mx) mx = __longlong_as_double(0x7ff8000000000000ll);
+            }
         }
-        g.R[c] = r;
     }
     block_max_to_global(mx, g.norm);
 }
 
-// phi_c += e_c on the whole coarse array (the zero pads stay zero)
-__global__ void amr_add_kernel(double* __restrict__ dst, const double* __restrict__ src, long long n)
-{
-    const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (t < n) dst[t] += src[t];
-}
-
-// phi_f += e_c of the parent (piecewise constant, R9)
-__global__ void amr_prolong_add_kernel(AmrGeom A, double* __restrict__ phif, const double* __restrict__ ec)
+// phi_f += the correction of the parent (piecewise constant, R9) = its new value - the mean it held before the V-cycle
+__global__ void amr_prolong_add_kernel(AmrGeom A, double* __restrict__ phif, const double* __restrict__ phic, const double* __restrict__ old)
 {
     const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (t >= A.F.n) return;
     int i, j, k;
     unflatten(A.F, t, i, j, k);
-    phif[cell_at(A.F, i, j, k)] += ec[cell_at(A.C, A.lo[0] + i / 2, A.lo[1] + j / 2, A.nd == 3 ? A.lo[2] + k / 2 : 0)];
+    const int I = i / 2, J = j / 2, K = A.nd == 3 ? k / 2 : 0;
+    const double e = phic[cell_at(A.C, A.lo[0] + I, A.lo[1] + J, A.nd == 3 ? A.lo[2] + K : 0)]
+                   - old[I + (long long)A.S.nx * (J + (long long)A.S.ny * K)];
+    phif[cell_at(A.F, i, j, k)] += e;
 }
 
 __global__ void amr_scale_kernel(double* __restrict__ v, long long n, double s)

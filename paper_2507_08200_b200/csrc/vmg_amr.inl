@@ -8,15 +8,15 @@ struct vmg_amr_s {
     vmg_s* hf = nullptr;            // the patch (an ordinary handle whose faces are coarse-fine faces)
     AmrGeom A;
     cudaStream_t stream = nullptr;
-    void* base = nullptr;           // one allocation: phi_c, btilde_c (padded like a level array), rhs_f copy, 4 scalars
-    double *phic = nullptr, *btc = nullptr, *rhsf = nullptr;
-    unsigned long long* d_norm = nullptr;   // ||btilde_c||, ||f_f||, ||r_c||, ||r_f|| (bit patterns)
+    void* base = nullptr;           // one allocation: btilde_c (padded like a level array), rhs_f copy, shadow means, scalars
+    double *btc = nullptr, *rhsf = nullptr, *old = nullptr;
+    unsigned long long* d_norm = nullptr;   // ||btilde_c||, ||f_f||, ||r_c||, ||r_f|| (bit patterns), 
     double* h_norm = nullptr;       // pinned mirror
     int nu_f = 6;                   // A4: fine sweeps per cycle
     bool have_coeffs = false, have_bc = false;
-    cudaGraph_t graph[2] = {nullptr, nullptr};          // 0: composite residual + norms, 1: correction + fine sweeps
-    cudaGraphExec_t exec[2] = {nullptr, nullptr};
-    long long graph_launches[2] = {0, 0};
+    cudaGraph_t graph[3] = {nullptr, nullptr, nullptr};   // 0: composite residual + norms (every cell), 1: correction + fine sweeps,
+    cudaGraphExec_t exec[3] = {nullptr, nullptr, nullptr};   // 2: as 0 with the coarse norm over the red cells (after a V-cycle, R12)
+    long long graph_launches[3] = {0, 0, 0};
     unsigned epoch_c = 0, epoch_f = 0;
     int graph_nu_f = -1;
     int cycles = 0, last_cuda_error = 0;
@@ -39,7 +39,7 @@ namespace {
 
 void amr_drop_graphs(vmg_amr_s* a)
 {
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < 3; ++i) {
         if (a->exec[i]) { cudaGraphExecDestroy(a->exec[i]); a->exec[i] = nullptr; }
         if (a->graph[i]) { cudaGraphDestroy(a->graph[i]); a->graph[i] = nullptr; }
     }
@@ -50,7 +50,7 @@ int amr_enqueue_ghost_fold(vmg_amr_s* a, long long* count)
 {
     vmg_s* hf = a->hf;
     AmrGhostArgs g;
-    g.A = a->A; g.phic = a->phic;
+    g.A = a->A; g.phic = a->hc->lev[0].phi;
     long long most = 0;
     for (int f = 0; f < 6; ++f) {
         g.plane[f] = hf->bcval[f];
@@ -64,8 +64,9 @@ int amr_enqueue_ghost_fold(vmg_amr_s* a, long long* count)
     return rc;
 }
 
-// graph 0: the composite residual (A3) -- the patch's residual + restriction and residual norm, then the coarse right-hand side
-void amr_enqueue_residual(vmg_amr_s* a, long long* count)
+// graphs 0 / 2: the composite residual (A3) -- the patch's residual + restriction and residual norm, the coarse right-hand
+// side in and next to the patch, then the library's residual norm of the box on that right-hand side (amr_patch_rhs_kernel)
+void amr_enqueue_residual(vmg_amr_s* a, long long* count, bool red_only)
 {
     vmg_s *hc = a->hc, *hf = a->hf;
     cudaMemsetAsync(a->d_norm + 2, 0, 2 * sizeof(unsigned long long), a->stream);
@@ -75,42 +76,45 @@ void amr_enqueue_residual(vmg_amr_s* a, long long* count)
     ++*count;
     AmrResArgs g;
     g.A = a->A; g.Lc = view(hc->lev[0]);
-    g.phic = a->phic; g.btc = a->btc; g.rs = hf->lev[1].rhs; g.phif = hf->lev[0].phi;
+    g.phic = hc->lev[0].phi; g.btc = a->btc; g.rs = hf->lev[1].rhs; g.phif = hf->lev[0].phi;
     g.R = hc->lev[0].rhs;
     for (int f = 0; f < 6; ++f) { g.gplane[f] = hf->bcval[f]; g.wbf[f] = hf->lev[0].wb[f]; }
     g.wscale = 2.0 / (double)(1 << a->A.nd);
     g.norm = a->d_norm + 2;
-    amr_coarse_residual_kernel<<<grid_for(a->A.C.n), kThreads, 0, a->stream>>>(g);
-    ++*count;
+    long long region = 1;
+    for (int d = 0; d < a->A.nd; ++d) region *= a->A.hi[d] - a->A.lo[d] + 2;
+    amr_patch_rhs_kernel<<<grid_for(region), kThreads, 0, a->stream>>>(g);
+    hc->lev[0].cur = 0;
+    enqueue_residual_norm(hc, a->d_norm + 2, red_only);
+    *count += 2;
 }
 
-// graph 1: A4 after the exit test -- coarse V-cycle from zero, corrections, ghosts, fine sweeps, average down
+// graph 1: A4 after the exit test -- coarse V-cycle (in place on phi_c, right-hand side of amr_coarse_residual_kernel),
+// correction of the patch, ghosts, fine sweeps, average down
 int amr_enqueue_correction(vmg_amr_s* a, long long* count)
 {
     vmg_s *hc = a->hc, *hf = a->hf;
     VmgLevel& C0 = hc->lev[0];
-    cudaMemsetAsync(C0.phi, 0, (size_t)C0.nalloc * sizeof(double), a->stream);
     enqueue_vcycle(hc, nullptr, count);
-    amr_add_kernel<<<grid_for(C0.nalloc), kThreads, 0, a->stream>>>(a->phic, C0.phi, C0.nalloc);
-    amr_prolong_add_kernel<<<grid_for(a->A.F.n), kThreads, 0, a->stream>>>(a->A, hf->lev[0].phi, C0.phi);
-    *count += 2;
+    amr_prolong_add_kernel<<<grid_for(a->A.F.n), kThreads, 0, a->stream>>>(a->A, hf->lev[0].phi, C0.phi, a->old);
+    ++*count;
     int rc = amr_enqueue_ghost_fold(a, count);
     if (rc != VMG_OK) return rc;
     hf->lev[0].cur = 0; hf->lev[0].dir = 0;
     plain_smooth(hf, 0, a->nu_f, count);
-    amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, hf->lev[0].phi, a->phic);
+    amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, hf->lev[0].phi, C0.phi, a->old);
     ++*count;
     return VMG_OK;
 }
 
-// runs part `which` (0 residual, 1 correction): a graph replay, or plain launches with option graph = 0 / profile on the coarse handle
+// runs part `which` (0 residual over every cell, 1 correction, 2 residual with the coarse norm over the red cells): a graph replay, or plain launches with option graph = 0 / profile on the coarse handle
 int amr_run(vmg_amr_s* a, int which)
 {
     vmg_s *hc = a->hc, *hf = a->hf;
     if (!hc->use_graph || hc->profile) {
         long long count = 0;
         int rc = VMG_OK;
-        if (which == 0) amr_enqueue_residual(a, &count); else rc = amr_enqueue_correction(a, &count);
+        if (which != 1) amr_enqueue_residual(a, &count, which == 2); else rc = amr_enqueue_correction(a, &count);
         a->launches += count;
         if (rc != VMG_OK) return rc;
         AMR_TRY(a, cudaGetLastError());
@@ -118,11 +122,11 @@ int amr_run(vmg_amr_s* a, int which)
     }
     if (!a->exec[0] || a->epoch_c != hc->graph_epoch || a->epoch_f != hf->graph_epoch || a->graph_nu_f != a->nu_f) {
         amr_drop_graphs(a);
-        for (int i = 0; i < 2; ++i) {
+        for (int i = 0; i < 3; ++i) {
             long long count = 0;
             AMR_TRY(a, cudaStreamBeginCapture(a->stream, cudaStreamCaptureModeRelaxed));
             int rc = VMG_OK;
-            if (i == 0) amr_enqueue_residual(a, &count); else rc = amr_enqueue_correction(a, &count);
+            if (i != 1) amr_enqueue_residual(a, &count, i == 2); else rc = amr_enqueue_correction(a, &count);
             cudaError_t e = cudaStreamEndCapture(a->stream, &a->graph[i]);
             if (rc != VMG_OK) return rc;
             if (e == cudaSuccess) e = cudaGraphInstantiate(&a->exec[i], a->graph[i], 0);
@@ -181,7 +185,7 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
     for (int d = 0; d < 3; ++d) { a->A.lo[d] = d < nd ? lo[d] : 0; a->A.hi[d] = d < nd ? hi[d] : 1; }
     const VmgLevel& C0 = a->hc->lev[0];
     const size_t arr = (size_t)C0.nalloc + 2 * (size_t)C0.pad;
-    const size_t total = 2 * round_up(arr, 32) + round_up((size_t)a->hf->lev[0].n, 32) + 32;
+    const size_t total = round_up(arr, 32) + round_up((size_t)a->hf->lev[0].n, 32) + round_up((size_t)a->hf->lev[1].n, 32) + 32;
     if (cudaMalloc(&a->base, total * sizeof(double)) != cudaSuccess ||
         cudaMallocHost((void**)&a->h_norm, 4 * sizeof(double)) != cudaSuccess ||
         cudaMemsetAsync(a->base, 0, total * sizeof(double), a->stream) != cudaSuccess ||
@@ -191,10 +195,10 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
         return VMG_ERR_ALLOC;
     }
     double* b = (double*)a->base;
-    a->phic = b + C0.pad;
-    a->btc = b + round_up(arr, 32) + C0.pad;
-    a->rhsf = b + 2 * round_up(arr, 32);
-    a->d_norm = (unsigned long long*)(a->rhsf + round_up((size_t)a->hf->lev[0].n, 32));
+    a->btc = b + C0.pad;
+    a->rhsf = b + round_up(arr, 32);
+    a->old = a->rhsf + round_up((size_t)a->hf->lev[0].n, 32);
+    a->d_norm = (unsigned long long*)(a->old + round_up((size_t)a->hf->lev[1].n, 32));
     *out = a;
     return VMG_OK;
 }
@@ -277,9 +281,11 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, do
     amr_mask_norm_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(a->A, a->btc, a->d_norm + 0);
     norm_inf_kernel<<<std::min<unsigned>(grid_for(F0.n), 4u * hf->num_sms), kThreads, 0, a->stream>>>(rhs_f, F0.n, a->d_norm + 1);
     AMR_TRY(a, cudaMemcpyAsync(a->rhsf, rhs_f, (size_t)F0.n * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
-    to_internal_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(C0.G, phi_c, a->phic, nullptr);
+    // rhs' of the coarse V-cycle = btilde_c except in and next to the patch (rewritten every cycle)
+    AMR_TRY(a, cudaMemcpyAsync(C0.rhs, a->btc, (size_t)C0.nalloc * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
+    to_internal_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(C0.G, phi_c, C0.phi, nullptr);
     to_internal_kernel<<<grid_for(F0.n), kThreads, 0, a->stream>>>(F0.G, phi_f, F0.phi, nullptr);
-    amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, F0.phi, a->phic);
+    amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, F0.phi, C0.phi, a->old);
     long long count = 6;
     rc = amr_enqueue_ghost_fold(a, &count);
     if (rc != VMG_OK) return rc;
@@ -287,8 +293,10 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, do
     AMR_TRY(a, cudaGetLastError());
     int status = VMG_MAXCYCLES, slow = 0;
     double nb = 0.0;
+    const int tail = hc->tail_level < 0 ? hc->nlev - 1 : hc->tail_level;
+    const bool red_ok = hc->nu2 >= 1 && !hc->symmetric && tail > 0;   // after a V-cycle the box was last touched by a black half-sweep (R12)
     for (int c = 0;; ++c) {
-        rc = amr_run(a, 0);
+        rc = amr_run(a, c > 0 && red_ok ? 2 : 0);
         if (rc != VMG_OK) return rc;
         AMR_TRY(a, cudaMemcpyAsync(a->h_norm, a->d_norm, 4 * sizeof(double), cudaMemcpyDeviceToHost, a->stream));
         AMR_TRY(a, cudaStreamSynchronize(a->stream));
@@ -320,7 +328,7 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, do
         if (rc != VMG_OK) return rc;
     }
     if (status >= 0) {
-        to_natural_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(C0.G, a->phic, phi_c);
+        to_natural_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(C0.G, C0.phi, phi_c);
         to_natural_kernel<<<grid_for(F0.n), kThreads, 0, a->stream>>>(F0.G, F0.phi, phi_f);
         a->launches += 2;
         AMR_TRY(a, cudaGetLastError());

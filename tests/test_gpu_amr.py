@@ -57,9 +57,9 @@ def _compare(p, s, o, phic0=None, phif0=None, rtol=1e-12, max_cycles=40, same_cy
     if same_cycles:
         assert cyc == cyc_o, (cyc, cyc_o, hist, hist_o)
     n = min(len(hist), len(hist_o))
-    for i in range(n):
-        if hist_o[i] > 1e-10:
-            assert abs(hist[i] - hist_o[i]) <= 1e-6 * hist_o[i], (i, hist[i], hist_o[i])
+    for i in range(n):       # 2e-15: the rounding floor of a residual formed from O(1) fields (the GPU runs the coarse V-cycle in place
+        if hist_o[i] > 1e-10:    # on phi_c and differences the covered cells for the patch's correction; the oracle solves for the correction)
+            assert abs(hist[i] - hist_o[i]) <= 1e-6 * hist_o[i] + 2e-15, (i, hist[i], hist_o[i])
     assert rel(pf.cpu().numpy(), pf_o) <= PHI_TOL
     assert rel(pc.cpu().numpy(), pc_o) <= PHI_TOL          # covered cells included: means of the children on both sides
     return pc, pf, cyc, hist
