@@ -10,7 +10,7 @@
 // Smoother, residual + restriction, norms and fold_bc of the patch are then the library's own kernels.  The COARSE BOX is
 // an ordinary handle too: its V-cycle, run in place on phi_c with a right-hand side that differs from btilde_c only in and
 // next to the patch, is the correction solver; the composite residual of its uncovered cells is the library's residual with
-// the flux through a face of the patch replaced by the fine fluxes (amr_coarse_residual_kernel).
+// the flux through a face of the patch replaced by the fine fluxes (amr_patch_rhs_kernel).
 #pragma once
 #include "vmg_kernels.cuh"
 

@@ -89,7 +89,7 @@ void amr_enqueue_residual(vmg_amr_s* a, long long* count, bool red_only)
     *count += 2;
 }
 
-// graph 1: A4 after the exit test -- coarse V-cycle (in place on phi_c, right-hand side of amr_coarse_residual_kernel),
+// graph 1: A4 after the exit test -- coarse V-cycle (in place on phi_c, right-hand side of amr_patch_rhs_kernel),
 // correction of the patch, ghosts, fine sweeps, average down
 int amr_enqueue_correction(vmg_amr_s* a, long long* count)
 {
