@@ -511,6 +511,7 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     else if (!strcmp(key, "batch_full_mb")) { if (v < 0) return VMG_ERR_ARG; h->batch_full_mb = v; }
     else if (!strcmp(key, "block_min_cells")) { if (v < 0) return VMG_ERR_ARG; h->block_min_cells = (long long)v; }
     else if (!strcmp(key, "phi_keep_cells")) { if (v < 0) return VMG_ERR_ARG; h->phi_keep_cells = (long long)v; }
+    else if (!strcmp(key, "restrict_red_cells")) { if (v < 0) return VMG_ERR_ARG; h->restrict_red_cells = (long long)v; }
     else if (!strcmp(key, "l2_persist")) { if (v < 0) return VMG_ERR_ARG; h->l2_persist_mb = v; h->l2_applied = false; }
     else if (!strcmp(key, "profile")) {
         h->profile = iv != 0;

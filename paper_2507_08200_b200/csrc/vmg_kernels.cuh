@@ -696,7 +696,10 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 // S3 (per-colour path). Fused residual + restriction: one thread per coarse cell; also zeroes the coarse phi.
 // (Four lanes per coarse cell with a shuffle gather was tried: 70 us instead of 49 us on 256x128x128, the 64-byte
 // runs per row coalesce worse than they gain in occupancy.)
-template <int CW>
+// RED = 1: the level was last touched by a black half-sweep (the pre-smoothing of a down-stroke), so the residual of every
+// black child is its own rounding error (reading R12 in DESIGN.md: t - fl(fl(dinv t) / dinv), ~2 ulp of D phi) and only the
+// four red children are evaluated: 5 doubles per fine cell instead of 7 (all of phi and the weights, half of rhs and 1/D).
+template <int CW, int RED = 0>
 __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG, const double* phi,
                                              const double* rhs, double* crhs, double* cphi,
                                              int sz, int I, int J, int K, long long off = 0)
@@ -706,16 +709,22 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
         for (int q = 0; q < 2; ++q) {   // the x-pair first, then accumulated (the blocked kernel sums in this order too)
             const int j = 2 * J + q, k = sz * K + r;
             long long row = off + L.G.plane * k + (long long)L.G.pitch * j, ce, xe, co, xo;
-            pair_addr(L.G, row, I, 0, ce, xe);
-            pair_addr(L.G, row, I, 1, co, xo);
-            s += residual_at<CW, CW ? 0 : 2>(L, phi, rhs, ce, xe, 2 * I, j, k) + residual_at<CW, CW ? 0 : 2>(L, phi, rhs, co, xo, 2 * I + 1, j, k);   // rhs, 1/D streamed
+            if (RED) {
+                const int par = (j + k) & 1;                           // x-parity of the row's red child: (i + j + k) even
+                pair_addr(L.G, row, I, par, ce, xe);
+                s += residual_at<CW, CW ? 0 : 2>(L, phi, rhs, ce, xe, 2 * I + par, j, k);
+            } else {
+                pair_addr(L.G, row, I, 0, ce, xe);
+                pair_addr(L.G, row, I, 1, co, xo);
+                s += residual_at<CW, CW ? 0 : 2>(L, phi, rhs, ce, xe, 2 * I, j, k) + residual_at<CW, CW ? 0 : 2>(L, phi, rhs, co, xo, 2 * I + 1, j, k);   // rhs, 1/D streamed
+            }
         }
     const long long cc = off + cell_at(CG, I, J, K);
     crhs[cc] = s / (4.0 * sz);
     if (cphi) cphi[cc] = 0.0;
 }
 
-template <int CW>
+template <int CW, int RED = 0>
 __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
                                          double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
 {
@@ -724,7 +733,7 @@ __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __r
     int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
     const long long off = batch_split(L, CG.nz, K);
     if (reverse) { K = CG.nz - 1 - K; J = gridDim.y * blockDim.y - 1 - J; }
-    if (I < CG.nx && J < CG.ny) restrict_one<CW>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off);
+    if (I < CG.nx && J < CG.ny) restrict_one<CW, RED>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off);
 }
 
 // S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise

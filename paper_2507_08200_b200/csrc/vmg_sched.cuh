@@ -156,7 +156,9 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
         }
 }
 
-inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
+// after_black: the level's last kernel was a black half-sweep (pre-smoothing with nu1 >= 1): on levels of at least
+// restrict_red_cells cells only the red children's residuals are evaluated (restrict_one<CW, 1>; option "restrict_red_cells")
+inline void plain_residual_restrict(vmg_s* h, int l, long long* count, bool after_black = false)
 {
     VmgLevel& L = h->lev[l];
     VmgLevel& C = h->lev[l + 1];
@@ -164,8 +166,13 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count)
     dim3 grid, block;
     cell_launch_dims(C.G, grid, block);
     grid.z *= L.nprob;
-    launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_kernel), grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
-               h->three_d ? 2 : 1, next_dir(h, L));
+    if (after_black && L.n >= h->restrict_red_cells) {
+        auto k = L.cw == 2 ? residual_restrict_kernel<2, 1> : L.cw ? residual_restrict_kernel<1, 1> : residual_restrict_kernel<0, 1>;
+        launch_pdl(h, k, grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi, h->three_d ? 2 : 1, next_dir(h, L));
+    } else {
+        auto k = L.cw == 2 ? residual_restrict_kernel<2, 0> : L.cw ? residual_restrict_kernel<1, 0> : residual_restrict_kernel<0, 0>;
+        launch_pdl(h, k, grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi, h->three_d ? 2 : 1, next_dir(h, L));
+    }
     ++*count;
 }
 
@@ -668,7 +675,7 @@ inline void enqueue_down(vmg_s* h, int l, long long* count)
         plain_smooth(h, l, h->nu1, count);
     }
     ProfScope ps(h, l == 0 ? VMG_PC_RESREST0 : VMG_PC_COARSE, count);
-    plain_residual_restrict(h, l, count);
+    plain_residual_restrict(h, l, count, h->nu1 >= 1);
 }
 
 // up-stroke of level l: prolongation+correction from level l+1 then nu2 sweeps [then the residual norm (level 0)].
@@ -857,7 +864,7 @@ inline void enqueue_loop_body(vmg_s* h, cudaGraphConditionalHandle handle, unsig
     L0.dir = 1;                                                   // the half-sweep before this one walked forward
     loop_halfsweep_io(h, L0.phi2, L0.phi, 1, false, nullptr, count);
     plain_smooth(h, 0, h->nu1, count, 2);
-    plain_residual_restrict(h, 0, count);
+    plain_residual_restrict(h, 0, count, true);
     for (int l = 1; l < tail; ++l) enqueue_down(h, l, count);
     if (h->tail_level >= 0) enqueue_tail(h, nullptr, count);
     else {

@@ -189,6 +189,7 @@ def test_blocked_passes_equal_plain_launches_bitwise(dims):
     p = inputs.random_problem(*dims, seed=11, bc_type=MIXED, sigma=1.0)
     s, d = b.from_problem(p)
     s.set_option("block_min_cells", 0)
+    s.set_option("restrict_red_cells", 2.0 ** 40)   # the blocked passes restrict all eight children's residuals: compare like with like
     rng = np.random.default_rng(3)
     for lev in range(s.num_levels - 1):
         nx, ny, nz = s.level_dims(lev)
@@ -1076,3 +1077,28 @@ def test_changing_the_mask_on_a_handle_equals_fresh_handles():
         f.destroy()
         assert got[0] == want[0] == 0 and got[1] == want[1] and torch.equal(got[2], want[2])
     s.destroy()
+
+
+def test_red_only_restriction_after_presmoothing_is_the_full_restriction_to_rounding():
+    """Option restrict_red_cells (reading R12 applied to the transfer): after a black half-sweep the black children's residuals
+    are their own rounding error, so restricting the red children only changes the coarse right-hand side by rounding: same
+    cycle counts, histories equal to rounding, phi within 1e-13 -- and the oracle (which restricts all eight) within the bar."""
+    b = _binding()
+    p = inputs.config4(32)
+    out = {}
+    for thresh in (0.0, 2.0 ** 40):          # every level launched as a kernel of its own / no level
+        s, d = b.from_problem(p)
+        s.set_option("restrict_red_cells", thresh)
+        s.set_option("tail", 0)              # no single-CTA tail: every down-stroke goes through residual_restrict_kernel
+        phi = torch.zeros_like(d["rhs"])
+        assert s.solve(d["rhs"], phi, rtol=p.rtol, max_vcycles=p.max_vcycles) == 0
+        out[thresh] = (phi.cpu().numpy(), s.get_info())
+        s.destroy()
+    (phi_r, info_r), (phi_a, info_a) = out[0.0], out[2.0 ** 40]
+    assert info_r[0] == info_a[0]
+    assert not np.array_equal(phi_r, phi_a)                      # the option did take effect
+    assert rel(phi_r, phi_a) <= 1e-13
+    for x, y in zip(info_r[2], info_a[2]):
+        assert abs(x - y) <= 1e-9 * y + 2e-15
+    phi_o, st_o, cyc_o, rr_o, _ = Oracle.from_problem(p).solve(p.rhs, rtol=p.rtol, max_vcycles=p.max_vcycles)
+    assert cyc_o == info_r[0] and rel(phi_r, phi_o) <= PHI_TOL
