@@ -168,7 +168,7 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  * "phi_keep_cells" (levels with at least this many cells read phi in a colour half-sweep (the neighbours) and in the residual norm with the normal
  *   cache policy instead of the streaming one, default 33554432: on a level whose phi is more than twice the L2 the
  *   evict-first lines are gone before the next row and plane ask for them; results do not depend on it),
- * "restrict_red_cells" (levels with at least this many cells, default 1048576, restrict the residuals of the RED children only
+ * "restrict_red_cells" (levels with at least this many cells, default 262144, restrict the residuals of the RED children only
  *   in the down-stroke: pre-smoothing ends with a black half-sweep, after which a black cell's residual is its own rounding
  *   error (~2 ulp of D phi, reading R12 of DESIGN.md), so the pass moves 5 instead of 7 doubles per cell; a very large value
  *   restricts all eight children everywhere, as vmg_step_residual_restrict and the blocked passes always do),

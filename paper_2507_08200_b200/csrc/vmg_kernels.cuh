@@ -724,7 +724,7 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
     if (cphi) cphi[cc] = 0.0;
 }
 
-template <int CW, int RED = 0>
+template <int CW>
 __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
                                          double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
 {
@@ -733,7 +733,21 @@ __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __r
     int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
     const long long off = batch_split(L, CG.nz, K);
     if (reverse) { K = CG.nz - 1 - K; J = gridDim.y * blockDim.y - 1 - J; }
-    if (I < CG.nx && J < CG.ny) restrict_one<CW, RED>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off);
+    if (I < CG.nx && J < CG.ny) restrict_one<CW, 0>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off);
+}
+
+// the red children only (restrict_one<CW, 1>).  Latency-bound (ncu: long-scoreboard stalls, 61 % of the warp slots at 34
+// registers): with array weights the kernel is held to 32 registers so that 8 CTAs fit an SM.
+template <int CW>
+__global__ void __launch_bounds__(kThreads, CW == 0 ? 8 : 1)
+residual_restrict_red_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
+                             double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
+{
+    grid_dependency_wait();
+    int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
+    const long long off = batch_split(L, CG.nz, K);
+    if (reverse) { K = CG.nz - 1 - K; J = gridDim.y * blockDim.y - 1 - J; }
+    if (I < CG.nx && J < CG.ny) restrict_one<CW, 1>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off);
 }
 
 // S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise
@@ -849,7 +863,7 @@ __global__ void norm_inf_kernel(const double* __restrict__ v, long long n, unsig
 template <int CW, int KEEP = 0>   // KEEP = 1: phi with the normal policy (levels far larger than the L2, see relax_at)
 // skip_if_zero (may be NULL): a device scalar; when its bits are 0 the kernel does nothing (vmg_solve's initial residual:
 // max |phi_0| == 0 means the residual is btilde, which the host then takes from ||btilde||)
-__global__ void residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
+__global__ void __launch_bounds__(kThreads, 8) residual_norm_kernel(LevelView L, const double* __restrict__ phi, const double* __restrict__ rhs,
                                      unsigned long long* out, int reverse, const unsigned long long* skip_if_zero = nullptr,
                                      int zslots = 0)
 {

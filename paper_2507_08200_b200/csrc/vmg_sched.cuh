@@ -167,11 +167,11 @@ inline void plain_residual_restrict(vmg_s* h, int l, long long* count, bool afte
     cell_launch_dims(C.G, grid, block);
     grid.z *= L.nprob;
     if (after_black && L.n >= h->restrict_red_cells) {
-        auto k = L.cw == 2 ? residual_restrict_kernel<2, 1> : L.cw ? residual_restrict_kernel<1, 1> : residual_restrict_kernel<0, 1>;
-        launch_pdl(h, k, grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi, h->three_d ? 2 : 1, next_dir(h, L));
+        launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_red_kernel), grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
+                   h->three_d ? 2 : 1, next_dir(h, L));
     } else {
-        auto k = L.cw == 2 ? residual_restrict_kernel<2, 0> : L.cw ? residual_restrict_kernel<1, 0> : residual_restrict_kernel<0, 0>;
-        launch_pdl(h, k, grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi, h->three_d ? 2 : 1, next_dir(h, L));
+        launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_kernel), grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
+                   h->three_d ? 2 : 1, next_dir(h, L));
     }
     ++*count;
 }
