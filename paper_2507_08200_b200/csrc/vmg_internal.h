@@ -43,6 +43,7 @@ struct VmgLevel {
     double *phi2 = nullptr;   // second phi buffer: passes of the blocked smoother ping-pong (tiles overlap)
     int dir = 0;              // direction of the next whole-level kernel (see next_dir)
     int cur = 0;              // which buffer holds phi while a V-cycle is being enqueued (0: phi, 1: phi2)
+    bool first_red_done = false;   // while a V-cycle is being enqueued: the finer level's restriction has already stored this level's first red half-sweep
     // boundary-face weight planes, order XLO..ZHI (unpadded)
     double* wb[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     // averaged raw coefficients in the public layout (levels >= 1 only; level 0 reads the caller's arrays)

@@ -699,10 +699,13 @@ __global__ void residual_kernel(LevelView L, const double* __restrict__ phi, con
 // RED = 1: the level was last touched by a black half-sweep (the pre-smoothing of a down-stroke), so the residual of every
 // black child is its own rounding error (reading R12 in DESIGN.md: t - fl(fl(dinv t) / dinv), ~2 ulp of D phi) and only the
 // four red children are evaluated: 5 doubles per fine cell instead of 7 (all of phi and the weights, half of rhs and 1/D).
+// cdinv (may be NULL): 1/D of the coarse level.  The coarse level starts its down-stroke from phi = 0, so its first red
+// half-sweep is phi_red = (1/D) (rhs + 0) and touches nothing else: with cdinv the kernel stores that instead of the zero
+// (bitwise what smooth_colour_kernel computes from a zero field) and the coarse level skips the launch.
 template <int CW, int RED = 0>
 __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG, const double* phi,
                                              const double* rhs, double* crhs, double* cphi,
-                                             int sz, int I, int J, int K, long long off = 0)
+                                             int sz, int I, int J, int K, long long off = 0, const double* cdinv = nullptr)
 {
     double s = 0.0;
     for (int r = 0; r < sz; ++r)
@@ -720,20 +723,22 @@ __device__ __forceinline__ void restrict_one(const LevelView& L, const Geom& CG,
             }
         }
     const long long cc = off + cell_at(CG, I, J, K);
-    crhs[cc] = s / (4.0 * sz);
-    if (cphi) cphi[cc] = 0.0;
+    const double v = s / (4.0 * sz);
+    crhs[cc] = v;
+    if (cphi) cphi[cc] = (cdinv && ((I + J + K) & 1) == 0) ? cdinv[cc] * (v + 0.0) : 0.0;   // + 0.0: the sweep's rhs + sum(w * 0)
 }
 
 template <int CW>
 __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
-                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
+                                         double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse,
+                                         const double* __restrict__ cdinv = nullptr)
 {
     grid_dependency_wait();
     // grid (coarse x blocks, coarse row blocks, coarse planes), block (coarse x, coarse rows): cell_launch_dims of the coarse level
     int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
     const long long off = batch_split(L, CG.nz, K);
     if (reverse) { K = CG.nz - 1 - K; J = gridDim.y * blockDim.y - 1 - J; }
-    if (I < CG.nx && J < CG.ny) restrict_one<CW, 0>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off);
+    if (I < CG.nx && J < CG.ny) restrict_one<CW, 0>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off, cdinv);
 }
 
 // the red children only (restrict_one<CW, 1>).  Latency-bound (ncu: long-scoreboard stalls, 61 % of the warp slots at 34
@@ -741,13 +746,14 @@ __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __r
 template <int CW>
 __global__ void __launch_bounds__(kThreads, CW == 0 ? 8 : 1)
 residual_restrict_red_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
-                             double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse)
+                             double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse,
+                             const double* __restrict__ cdinv = nullptr)
 {
     grid_dependency_wait();
     int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
     const long long off = batch_split(L, CG.nz, K);
     if (reverse) { K = CG.nz - 1 - K; J = gridDim.y * blockDim.y - 1 - J; }
-    if (I < CG.nx && J < CG.ny) restrict_one<CW, 1>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off);
+    if (I < CG.nx && J < CG.ny) restrict_one<CW, 1>(L, CG, phi, rhs, crhs, cphi, sz, I, J, K, off, cdinv);
 }
 
 // S4 (per-colour path, nu2 = 0 and the single-step entry point). Fused prolongation + correction (piecewise

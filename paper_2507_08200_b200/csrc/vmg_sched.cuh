@@ -158,20 +158,23 @@ inline void plain_smooth(vmg_s* h, int l, int nsweeps, long long* count, int ski
 
 // after_black: the level's last kernel was a black half-sweep (pre-smoothing with nu1 >= 1): on levels of at least
 // restrict_red_cells cells only the red children's residuals are evaluated (restrict_one<CW, 1>; option "restrict_red_cells")
-inline void plain_residual_restrict(vmg_s* h, int l, long long* count, bool after_black = false)
+// fold_first: the coarse level's first red half-sweep is stored by this kernel (restrict_one, cdinv); its down-stroke skips it
+inline void plain_residual_restrict(vmg_s* h, int l, long long* count, bool after_black = false, bool fold_first = false)
 {
     VmgLevel& L = h->lev[l];
     VmgLevel& C = h->lev[l + 1];
     C.cur = 0;
+    C.first_red_done = fold_first;
+    const double* cdinv = fold_first ? C.dinv : nullptr;
     dim3 grid, block;
     cell_launch_dims(C.G, grid, block);
     grid.z *= L.nprob;
     if (after_black && L.n >= h->restrict_red_cells) {
         launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_red_kernel), grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
-                   h->three_d ? 2 : 1, next_dir(h, L));
+                   h->three_d ? 2 : 1, next_dir(h, L), cdinv);
     } else {
         launch_pdl(h, VMG_BY_WEIGHTS(L, residual_restrict_kernel), grid, block, 0, view(L), C.G, cur_phi(L), L.rhs, C.rhs, C.phi,
-                   h->three_d ? 2 : 1, next_dir(h, L));
+                   h->three_d ? 2 : 1, next_dir(h, L), cdinv);
     }
     ++*count;
 }
@@ -662,9 +665,23 @@ inline void enqueue_smooth(vmg_s* h, int l, int nsweeps, long long* count)
     }
 }
 
-// down-stroke of level l: nu1 sweeps then residual+restriction into level l+1 (which also zeroes its phi)
-inline void enqueue_down(vmg_s* h, int l, long long* count)
+// Can the restriction INTO level c store that level's first red half-sweep (plain_residual_restrict fold_first)?  Only when
+// level c runs an ordinary down-stroke of per-colour launches afterwards: not the tail / bottom level, not a blocked level.
+inline bool can_fold_first(const vmg_s* h, int c)
 {
+    const int last = h->nlev - 1;
+    const int tail = h->tail_level < 0 ? last : h->tail_level;
+    return h->nu1 >= 1 && c < tail && !blocked_ok(h, c);
+}
+
+// down-stroke of level l: nu1 sweeps then residual+restriction into level l+1 (which also zeroes its phi)
+// chain: part of a whole V-cycle (the next level's down-stroke follows): the restriction may store the next level's first
+// red half-sweep; a single stroke (vmg_step_down) never does
+inline void enqueue_down(vmg_s* h, int l, long long* count, bool chain = false)
+{
+    VmgLevel& L = h->lev[l];
+    const int skip = L.first_red_done ? 1 : 0;
+    L.first_red_done = false;
     if (h->nu1 > 0 && blocked_ok(h, l)) {
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
         blocked_sweeps(h, l, 2 * h->nu1, 0, false, BT_RESTRICT, nullptr, count);
@@ -672,10 +689,10 @@ inline void enqueue_down(vmg_s* h, int l, long long* count)
     }
     {
         ProfScope ps(h, l == 0 ? VMG_PC_SMOOTH0 : VMG_PC_COARSE, count);
-        plain_smooth(h, l, h->nu1, count);
+        plain_smooth(h, l, h->nu1, count, skip);
     }
     ProfScope ps(h, l == 0 ? VMG_PC_RESREST0 : VMG_PC_COARSE, count);
-    plain_residual_restrict(h, l, count, h->nu1 >= 1);
+    plain_residual_restrict(h, l, count, h->nu1 >= 1, chain && can_fold_first(h, l + 1));
 }
 
 // up-stroke of level l: prolongation+correction from level l+1 then nu2 sweeps [then the residual norm (level 0)].
@@ -720,8 +737,8 @@ inline void enqueue_vcycle(vmg_s* h, unsigned long long* norm_out, long long* co
     // first level not handled stroke by stroke
     const int tail = h->tail_level < 0 ? last : h->tail_level;
     if (norm_out) cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
-    for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }
-    for (int l = 0; l < tail; ++l) enqueue_down(h, l, count);
+    for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; h->lev[l].first_red_done = false; }
+    for (int l = 0; l < tail; ++l) enqueue_down(h, l, count, true);
     bool norm_done = false;
     if (h->tail_level >= 0) {
         enqueue_tail(h, norm_out, count);
@@ -754,10 +771,10 @@ inline void enqueue_vcycle_segment(vmg_s* h, int seg, unsigned long long* norm_o
     const int tail = h->tail_level < 0 ? last : h->tail_level;
     if (seg == 0) {
         cudaMemsetAsync(norm_out, 0, sizeof(unsigned long long), h->stream);
-        for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }
-        enqueue_down(h, 0, count);
+        for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; h->lev[l].first_red_done = false; }
+        enqueue_down(h, 0, count, true);
     } else if (seg == 1) {
-        for (int l = 1; l < tail; ++l) enqueue_down(h, l, count);
+        for (int l = 1; l < tail; ++l) enqueue_down(h, l, count, true);
         if (h->tail_level >= 0) enqueue_tail(h, nullptr, count);
         else {
             ProfScope ps(h, VMG_PC_COARSE, count);
@@ -859,13 +876,13 @@ inline void enqueue_loop_body(vmg_s* h, cudaGraphConditionalHandle handle, unsig
 {
     const int last = h->nlev - 1;
     const int tail = h->tail_level < 0 ? last : h->tail_level;
-    for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; }
+    for (int l = 0; l <= last; ++l) { h->lev[l].cur = 0; h->lev[l].dir = 0; h->lev[l].first_red_done = false; }
     VmgLevel& L0 = h->lev[0];
     L0.dir = 1;                                                   // the half-sweep before this one walked forward
     loop_halfsweep_io(h, L0.phi2, L0.phi, 1, false, nullptr, count);
     plain_smooth(h, 0, h->nu1, count, 2);
-    plain_residual_restrict(h, 0, count, true);
-    for (int l = 1; l < tail; ++l) enqueue_down(h, l, count);
+    plain_residual_restrict(h, 0, count, true, can_fold_first(h, 1));
+    for (int l = 1; l < tail; ++l) enqueue_down(h, l, count, true);
     if (h->tail_level >= 0) enqueue_tail(h, nullptr, count);
     else {
         if (!h->symmetric) plain_smooth(h, last, h->nbottom, count);
