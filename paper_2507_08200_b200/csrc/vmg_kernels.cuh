@@ -597,7 +597,9 @@ __global__ void solve_decide_kernel(cudaGraphConditionalHandle handle, double* s
 // stored: the cells of the other colour keep their uncorrected values in memory until the next half-sweep
 // overwrites them.  Valid when at least one full sweep follows (nu2 >= 1).  phi_nb + e is the very addition
 // prolong_correct_kernel performs, so results are bitwise those of the two separate kernels.
-template <int CW>
+// Cache policy as in relax_at: rhs, 1/D and the neighbours' phi are dead after this read (streaming loads; KEEP = 1: phi with
+// the normal policy on levels far larger than the L2); the coarse e is read by eight fine cells and stays cached.
+template <int CW, int KEEP = 0>
 __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom& CG, double* phi,
                                                   const double* rhs, const double* e, int colour, int sz,
                                                   int m, int j, int k, long long off = 0)
@@ -618,7 +620,9 @@ __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom
     const double eX = (i & 1) ? e[xP + 1] : e[xP];                                  // zero pad beyond the x faces: not used there
     const double eY = (j & 1) ? e[cP + CG.pitch] : e[cP - CG.pitch];
     // out-of-domain neighbours carry a zero weight; their (zero-pad or foreign) value is used uncorrected
-    double vxm = phi[xm], vxp = phi[xm + 1], vym = phi[c - G.pitch], vyp = phi[c + G.pitch], vzm = phi[c - G.plane], vzp = phi[c + G.plane];
+    auto ld = [](const double* q) { return KEEP ? *q : __ldcs(q); };
+    double vxm = ld(phi + xm), vxp = ld(phi + xm + 1), vym = ld(phi + c - G.pitch), vyp = ld(phi + c + G.pitch),
+           vzm = ld(phi + c - G.plane), vzp = ld(phi + c + G.plane);
     if (i > 0) vxm += (i & 1) ? eP : eX;
     if (i < G.nx - 1) vxp += (i & 1) ? eX : eP;
     if (j > 0) vym += (j & 1) ? eP : eY;
@@ -638,10 +642,10 @@ __device__ __forceinline__ void relax_prolong_one(const LevelView& L, const Geom
     s = fma(w[3], vyp, s);
     s = fma(w[4], vzm, s);
     s = fma(w[5], vzp, s);
-    phi[c] = L.dinv[c] * (rhs[c] + s);
+    phi[c] = __ldcs(L.dinv + c) * (__ldcs(rhs + c) + s);
 }
 
-template <int CW>
+template <int CW, int KEEP = 0>
 __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __restrict__ phi, const double* __restrict__ rhs,
                                              const double* __restrict__ e, int colour, int sz, int reverse)
 {
@@ -649,7 +653,7 @@ __global__ void smooth_colour_prolong_kernel(LevelView L, Geom CG, double* __res
     int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;   // pair_launch_dims
     const long long off = batch_split(L, L.G.nz, k);
     if (reverse) { k = L.G.nz - 1 - k; j = gridDim.y * blockDim.y - 1 - j; }
-    if (m < L.G.ne && j < L.G.ny) relax_prolong_one<CW>(L, CG, phi, rhs, e, colour, sz, m, j, k, off);
+    if (m < L.G.ne && j < L.G.ny) relax_prolong_one<CW, KEEP>(L, CG, phi, rhs, e, colour, sz, m, j, k, off);
 }
 
 // r = rhs - A phi, A phi = D phi - sum w phi_nb, D = 1/dinv.

@@ -714,8 +714,12 @@ inline bool enqueue_up(vmg_s* h, int l, unsigned long long* norm_out, long long*
         VmgLevel& L = h->lev[l];
         dim3 grid, block;
         pair_launch_dims(L, grid, block);
-        launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_prolong_kernel), grid, block, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
-                   cur_phi(h->lev[l + 1]), h->symmetric, h->three_d ? 2 : 1, next_dir(h, L));
+        if (L.cw == 0 && L.n >= h->phi_keep_cells)
+            launch_pdl(h, smooth_colour_prolong_kernel<0, 1>, grid, block, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
+                       cur_phi(h->lev[l + 1]), h->symmetric, h->three_d ? 2 : 1, next_dir(h, L));
+        else
+            launch_pdl(h, VMG_BY_WEIGHTS(L, smooth_colour_prolong_kernel), grid, block, 0, view(L), h->lev[l + 1].G, cur_phi(L), L.rhs,
+                       cur_phi(h->lev[l + 1]), h->symmetric, h->three_d ? 2 : 1, next_dir(h, L));
         ++*count;
         plain_smooth(h, l, h->nu2, count, 1, h->symmetric);
         return false;
