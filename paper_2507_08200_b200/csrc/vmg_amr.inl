@@ -283,8 +283,8 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, do
     AMR_TRY(a, cudaMemcpyAsync(a->rhsf, rhs_f, (size_t)F0.n * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
     // rhs' of the coarse V-cycle = btilde_c except in and next to the patch (rewritten every cycle)
     AMR_TRY(a, cudaMemcpyAsync(C0.rhs, a->btc, (size_t)C0.nalloc * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
-    to_internal_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(C0.G, phi_c, C0.phi, nullptr);
-    to_internal_kernel<<<grid_for(F0.n), kThreads, 0, a->stream>>>(F0.G, phi_f, F0.phi, nullptr);
+    to_internal_kernel<<<conv_grid(C0.n), kThreads, 0, a->stream>>>(C0.G, phi_c, C0.phi, nullptr);
+    to_internal_kernel<<<conv_grid(F0.n), kThreads, 0, a->stream>>>(F0.G, phi_f, F0.phi, nullptr);
     amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, F0.phi, C0.phi, a->old);
     long long count = 6;
     rc = amr_enqueue_ghost_fold(a, &count);
@@ -328,8 +328,8 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, do
         if (rc != VMG_OK) return rc;
     }
     if (status >= 0) {
-        to_natural_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(C0.G, C0.phi, phi_c);
-        to_natural_kernel<<<grid_for(F0.n), kThreads, 0, a->stream>>>(F0.G, F0.phi, phi_f);
+        to_natural_kernel<<<conv_grid(C0.n), kThreads, 0, a->stream>>>(C0.G, C0.phi, phi_c);
+        to_natural_kernel<<<conv_grid(F0.n), kThreads, 0, a->stream>>>(F0.G, F0.phi, phi_f);
         a->launches += 2;
         AMR_TRY(a, cudaGetLastError());
     }

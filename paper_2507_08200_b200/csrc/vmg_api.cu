@@ -567,7 +567,7 @@ int solve_begin(vmg_s* h, const double* rhs, double* phi, double rtol, int max_v
     if (rc != VMG_OK) return rc;
     {
         ProfScope ps(h, VMG_PC_COPY, nullptr);
-        to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, L0.phi, h->d_mask, scal + 2);
+        to_internal_kernel<<<conv_grid(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, L0.phi, h->d_mask, scal + 2);
     }
     enqueue_residual_norm(h, scal + 1, false, scal + 2);
     h->launches += 2;   // phi copy-in, first residual norm
@@ -628,7 +628,7 @@ int solve_end(vmg_s* h)
     VmgLevel& L0 = h->lev[0];
     if (h->sv_phi) {
         ProfScope ps(h, VMG_PC_COPY, nullptr);
-        to_natural_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, L0.phi, h->sv_phi);
+        to_natural_kernel<<<conv_grid(L0.n), kThreads, 0, h->stream>>>(L0.G, L0.phi, h->sv_phi);
         h->launches += 1;
         CUDA_TRY(h, cudaGetLastError());
     }
@@ -739,7 +739,7 @@ int solve_pcg_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int ma
 
     int rc = enqueue_fold_bc(h, rhs, r);
     if (rc != VMG_OK) return rc;
-    to_internal_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, h->pcg_x, h->d_mask);
+    to_internal_kernel<<<conv_grid(L0.n), kThreads, 0, h->stream>>>(L0.G, phi, h->pcg_x, h->d_mask);
     CUDA_TRY(h, cudaMemsetAsync(scal, 0, 4 * sizeof(double), h->stream));
     norm_inf_kernel<<<glin, kThreads, 0, h->stream>>>(r, n, scal + 0);
     pcg_residual_inplace_kernel<<<gpair, kPcgThreads, 0, h->stream>>>(v, h->pcg_x, r);
@@ -807,7 +807,7 @@ int solve_pcg_impl(vmg_s* h, const double* rhs, double* phi, double rtol, int ma
             h->launches += per_cycle + 3;
         }
     }
-    to_natural_kernel<<<grid_for(L0.n), kThreads, 0, h->stream>>>(L0.G, h->pcg_x, phi);
+    to_natural_kernel<<<conv_grid(L0.n), kThreads, 0, h->stream>>>(L0.G, h->pcg_x, phi);
     h->launches += 1;
     CUDA_TRY(h, cudaGetLastError());
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));

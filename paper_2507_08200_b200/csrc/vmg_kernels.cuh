@@ -223,12 +223,11 @@ struct FoldArgs {
     int three_d, bt_natural; int dirichlet[6]; double h[3];
 };
 
-__device__ __forceinline__ double fold_bc_one(const FoldArgs& g, long long t)
+__device__ __forceinline__ double fold_bc_one(const FoldArgs& g, long long t, double v /* = g.rhs[t] */)
 {
     const int nx = g.G.nx, ny = g.G.ny, nz = g.G.nz;
     int i, j, k;
     unflatten(g.G, t, i, j, k);
-    double v = g.rhs[t];
     auto add = [&](int f, long long pl, double hd) {
         if (!g.val[f]) return;
         double w = g.wb[f][pl], q = g.val[f][pl];
@@ -247,14 +246,29 @@ __device__ __forceinline__ double fold_bc_one(const FoldArgs& g, long long t)
     return v;
 }
 
+// The layout conversions (fold_bc, to_internal, to_natural) move 8 bytes per element and are bound by the bytes in flight
+// (one load per thread: 2.1-3.8 TB/s): every thread takes kConvElems elements a whole grid apart, all loads issued first.
+constexpr int kConvElems = 4;
+
 __global__ void fold_bc_kernel(FoldArgs g)
 {
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const long long T = (long long)gridDim.x * blockDim.x, t0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    double r[kConvElems];
+#pragma unroll
+    for (int u = 0; u < kConvElems; ++u) { const long long t = t0 + u * T; r[u] = t < g.G.n ? g.rhs[t] : 0.0; }
     double v = 0.0;
-    if (t < g.G.n) v = fold_bc_one(g, t);
+    bool nan = false;
+#pragma unroll
+    for (int u = 0; u < kConvElems; ++u) {
+        const long long t = t0 + u * T;
+        if (t < g.G.n) {
+            const double x = fabs(fold_bc_one(g, t, r[u]));
+            nan |= x != x;
+            v = fmax(v, x);
+        }
+    }
     if (g.norm_out) {                                  // the same maximum norm_inf_kernel takes over the stored array
-        v = fabs(v);
-        if (v != v) v = __longlong_as_double(0x7ff8000000000000ll);
+        if (nan) v = __longlong_as_double(0x7ff8000000000000ll);
         block_max_to_global(v, g.norm_out);
     }
 }
@@ -316,27 +330,47 @@ __global__ void pad_check_kernel(Geom G, const double* __restrict__ arr, long lo
 __global__ void to_internal_kernel(Geom G, const double* __restrict__ nat, double* __restrict__ in, const unsigned char* __restrict__ mask,
                                    unsigned long long* max_out = nullptr)
 {
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const long long T = (long long)gridDim.x * blockDim.x, t0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    double r[kConvElems];
+#pragma unroll
+    for (int u = 0; u < kConvElems; ++u) {
+        const long long t = t0 + u * T;
+        r[u] = (t < G.n && !(mask && !mask[t])) ? nat[t] : 0.0;
+    }
     double v = 0.0;
-    if (t < G.n) {
-        int i, j, k;
-        unflatten(G, t, i, j, k);
-        v = (mask && !mask[t]) ? 0.0 : nat[t];
-        in[cell_at(G, i, j, k)] = v;
+    bool nan = false;
+#pragma unroll
+    for (int u = 0; u < kConvElems; ++u) {
+        const long long t = t0 + u * T;
+        if (t < G.n) {
+            int i, j, k;
+            unflatten(G, t, i, j, k);
+            in[cell_at(G, i, j, k)] = r[u];
+            const double x = fabs(r[u]);
+            nan |= x != x;
+            v = fmax(v, x);
+        }
     }
     if (max_out) {
-        v = fabs(v);
-        if (v != v) v = __longlong_as_double(0x7ff8000000000000ll);
+        if (nan) v = __longlong_as_double(0x7ff8000000000000ll);
         block_max_to_global(v, max_out);
     }
 }
 __global__ void to_natural_kernel(Geom G, const double* __restrict__ in, double* __restrict__ nat)
 {
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (t >= G.n) return;
-    int i, j, k;
-    unflatten(G, t, i, j, k);
-    nat[t] = in[cell_at(G, i, j, k)];
+    const long long T = (long long)gridDim.x * blockDim.x, t0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    double r[kConvElems];
+#pragma unroll
+    for (int u = 0; u < kConvElems; ++u) {
+        const long long t = t0 + u * T;
+        int i, j, k;
+        if (t < G.n) { unflatten(G, t, i, j, k); r[u] = in[cell_at(G, i, j, k)]; }
+    }
+#pragma unroll
+    for (int u = 0; u < kConvElems; ++u) {
+        const long long t = t0 + u * T;
+        if (t < G.n) nat[t] = r[u];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -32,6 +32,7 @@ inline LevelView view(const VmgLevel& L)
 #define VMG_BY_WEIGHTS(L, KERNEL) ((L).cw == 2 ? KERNEL<2> : (L).cw ? KERNEL<1> : KERNEL<0>)
 
 inline unsigned grid_for(long long n) { return (unsigned)cdiv(n, kThreads); }
+inline unsigned conv_grid(long long n) { return (unsigned)cdiv(cdiv(n, kConvElems), kThreads); }   // fold_bc, to_internal, to_natural: kConvElems elements per thread
 
 // launch shape of the kernels that take one x-pair slot per thread: block (x-pairs, rows) of kThreads threads with as many
 // x-pairs as the row has (whole warps, at most 128), grid (x-pair blocks, row blocks, planes)
@@ -127,7 +128,7 @@ inline int enqueue_fold_bc(vmg_s* h, const double* rhs, double* bt, bool bt_natu
     g.h[0] = L.hx; g.h[1] = L.hy; g.h[2] = L.hz;
     {
         ProfScope ps(h, VMG_PC_FOLD, nullptr);
-        fold_bc_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(g);
+        fold_bc_kernel<<<conv_grid(L.n), kThreads, 0, h->stream>>>(g);
     }
     h->launches += 1;
     return cudaGetLastError() == cudaSuccess ? VMG_OK : VMG_ERR_CUDA;

@@ -6,14 +6,14 @@ namespace {
 // caller array (public layout) -> level array (internal layout) and back
 int stage_in(vmg_s* h, const VmgLevel& L, double* dst, const double* src)
 {
-    to_internal_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(L.G, src, dst, nullptr);
+    to_internal_kernel<<<conv_grid(L.n), kThreads, 0, h->stream>>>(L.G, src, dst, nullptr);
     CUDA_TRY(h, cudaGetLastError());
     return VMG_OK;
 }
 
 int stage_out(vmg_s* h, const VmgLevel& L, double* dst, const double* src)
 {
-    to_natural_kernel<<<grid_for(L.n), kThreads, 0, h->stream>>>(L.G, src, dst);
+    to_natural_kernel<<<conv_grid(L.n), kThreads, 0, h->stream>>>(L.G, src, dst);
     CUDA_TRY(h, cudaGetLastError());
     return VMG_OK;
 }
