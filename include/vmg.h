@@ -297,6 +297,8 @@ int vmg_amr_set_option(vmg_amr_handle h, const char* key, double v);
 int vmg_amr_solve(vmg_amr_handle h, const double* rhs_c, const double* rhs_f, double* phi_c, double* phi_f,
                   double rtol, int max_cycles);
 int vmg_amr_get_info(vmg_amr_handle h, int* cycles, double* relres, double* history /* >= cycles + 1 or NULL */);
+/* vmg_debug_pad_check over the box and the patch: number of non-zero pad entries (0 expected) */
+int vmg_amr_debug_pad_check(vmg_amr_handle h, long long* nonzero);
 long long vmg_amr_last_launch_count(vmg_amr_handle h);
 int vmg_amr_last_cuda_error(vmg_amr_handle h);
 int vmg_amr_destroy(vmg_amr_handle h);

@@ -24,7 +24,7 @@ SYMBOLS = ["vmg_create", "vmg_create_batch", "vmg_set_coeffs", "vmg_set_bc", "vm
            "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile", "vmg_debug_pad_check",
            "vmg_norm_inf_static", "vmg_amr_create", "vmg_amr_fine_dims", "vmg_amr_set_coeffs", "vmg_amr_set_bc",
            "vmg_amr_set_option", "vmg_amr_solve", "vmg_amr_get_info", "vmg_amr_last_launch_count",
-           "vmg_amr_last_cuda_error", "vmg_amr_destroy"]
+           "vmg_amr_last_cuda_error", "vmg_amr_destroy", "vmg_amr_debug_pad_check"]
 
 _lib = None
 _vp = C.c_void_p
@@ -85,6 +85,7 @@ def load():
     lib.vmg_amr_last_launch_count.restype = C.c_longlong
     lib.vmg_amr_last_cuda_error.argtypes = [_vp]
     lib.vmg_amr_destroy.argtypes = [_vp]
+    lib.vmg_amr_debug_pad_check.argtypes = [_vp, C.POINTER(C.c_longlong)]
     _lib = lib
     return lib
 
@@ -369,6 +370,11 @@ class VmgAmr:
 
     def last_launch_count(self) -> int:
         return int(self._lib.vmg_amr_last_launch_count(self._h))
+
+    def pad_check(self) -> int:
+        n = C.c_longlong()
+        self._chk(self._lib.vmg_amr_debug_pad_check(self._h, C.byref(n)), "vmg_amr_debug_pad_check")
+        return n.value
 
 
 NORM_INF_STATIC_MAX_N = 134217728   # VMG_NORM_INF_STATIC_MAX_N of include/vmg.h

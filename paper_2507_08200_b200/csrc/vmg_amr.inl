@@ -260,6 +260,17 @@ int vmg_amr_get_info(vmg_amr_handle a, int* cycles, double* relres, double* hist
     return VMG_OK;
 }
 
+// vmg_debug_pad_check over both handles (the zero pads and pad elements of every level array of the box and of the patch)
+int vmg_amr_debug_pad_check(vmg_amr_handle a, long long* nonzero)
+{
+    if (!a || !nonzero) return VMG_ERR_ARG;
+    long long nc = 0, nf = 0;
+    int rc = vmg_debug_pad_check(a->hc, &nc);
+    if (rc == VMG_OK) rc = vmg_debug_pad_check(a->hf, &nf);
+    *nonzero = nc + nf;
+    return rc;
+}
+
 long long vmg_amr_last_launch_count(vmg_amr_handle a) { return a ? a->launches : 0; }
 int vmg_amr_last_cuda_error(vmg_amr_handle a) { return a ? a->last_cuda_error : 0; }
 

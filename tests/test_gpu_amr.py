@@ -84,6 +84,7 @@ def test_composite_solve_matches_the_oracle(case):
     phic0, phif0 = rng.standard_normal(p.coarse.rhs.shape), rng.standard_normal(p.rhs_f.shape)
     pc, pf, cyc, hist = _compare(p, s, o, phic0, phif0)
     assert hist[-1] <= 1e-12 and cyc <= 20
+    assert s.pad_check() == 0                 # no kernel of the composite cycle wrote a zero pad of either handle
     ratios = [hist[i] / hist[i - 1] for i in range(2, len(hist)) if hist[i] > 1e-11]
     assert max(ratios) < 0.25, ratios
     # a second solve on the same handles from a zero guess, then with new coefficients (1/D of the patch is rebuilt)
