@@ -66,15 +66,16 @@ def lib():
         _lib.ovmg_prolong_add.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
         _lib.ovmg_vcycle.argtypes = [C.c_void_p, _dp, _dp]
         _ip = C.POINTER(C.c_int)
-        _lib.oamr_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, _ip]
+        _lib.oamr_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, _ip, _ip]
         _lib.oamr_destroy.argtypes = [C.c_void_p]
-        _lib.oamr_set_coeffs.argtypes = [C.c_void_p] + [_dp] * 8 + [C.c_double, C.c_double]
+        _pp = C.POINTER(_dp)
+        _lib.oamr_set_coeffs.argtypes = [C.c_void_p] + [_dp] * 4 + [_pp] * 4 + [C.c_double, C.c_double]
         _lib.oamr_set_bc.argtypes = [C.c_void_p, _ip, C.POINTER(_dp)]
         _lib.oamr_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_double]
-        _lib.oamr_fine_dims.argtypes = [C.c_void_p, _ip]
-        _lib.oamr_apply.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
-        _lib.oamr_average_down.argtypes = [C.c_void_p, _dp, _dp]
-        _lib.oamr_solve.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, C.c_double, C.c_int]
+        _lib.oamr_fine_dims.argtypes = [C.c_void_p, C.c_int, _ip]
+        _lib.oamr_apply.argtypes = [C.c_void_p, _dp, _pp, _dp, _pp]
+        _lib.oamr_average_down.argtypes = [C.c_void_p, _dp, _pp]
+        _lib.oamr_solve.argtypes = [C.c_void_p, _dp, _pp, _dp, _pp, C.c_double, C.c_int]
         _lib.oamr_get_info.argtypes = [C.c_void_p, _ip, C.POINTER(C.c_double), _dp]
     return _lib
 
@@ -235,19 +236,28 @@ class Oracle:
 
 
 class AmrOracle:
-    """Two-level composite solve (amr_oracle.c): an nx x ny x nz coarse box with one patch of coarse cells [lo, hi)
-    refined by 2.  Coarse arrays [k, j, i] on the box, fine arrays [K, J, I] on the patch (2 (hi - lo) cells a side)."""
+    """Two-level composite solve (amr_oracle.c): an nx x ny x nz coarse box with patches of coarse cells [lo, hi) refined
+    by 2.  lo, hi: one triple (a single patch: fine arrays are then passed and returned bare) or lists of triples (fine
+    arrays as lists, one entry per patch).  Coarse arrays [k, j, i] on the box, fine arrays [K, J, I] on a patch."""
 
     def __init__(self, nx, ny, nz, dx, dy, dz, lo, hi):
         self._h = C.c_void_p()
-        l3, h3 = (C.c_int * 3)(*[int(v) for v in lo]), (C.c_int * 3)(*[int(v) for v in hi])
-        rc = lib().oamr_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, l3, h3)
+        self._single = not isinstance(lo[0], (list, tuple, np.ndarray))
+        los = [lo] if self._single else list(lo)
+        his = [hi] if self._single else list(hi)
+        self.np = len(los)
+        flat = lambda v: (C.c_int * (3 * self.np))(*[int(x) for t in v for x in t])
+        rc = lib().oamr_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, self.np, flat(los), flat(his))
         if rc != 0:
             self._h = None
             raise OracleError(rc, "amr create")
-        d = (C.c_int * 3)()
-        lib().oamr_fine_dims(self._h, d)
-        self.coarse_shape, self.fine_shape = (nz, ny, nx), (d[2], d[1], d[0])
+        self.coarse_shape = (nz, ny, nx)
+        self.fine_shapes = []
+        for q in range(self.np):
+            d = (C.c_int * 3)()
+            lib().oamr_fine_dims(self._h, q, d)
+            self.fine_shapes.append((d[2], d[1], d[0]))
+        self.fine_shape = self.fine_shapes[0]
 
     def close(self):
         if getattr(self, "_h", None):
@@ -261,10 +271,20 @@ class AmrOracle:
             raise OracleError(rc, where)
         return rc
 
+    def _list(self, x):
+        return [x] if self._single else list(x)
+
+    def _ptrs(self, arrs):
+        """array of np pointers (NULL entries allowed) + the arrays kept alive"""
+        keep = [_c(x) for x in arrs]
+        return (_dp * self.np)(*[_p(x) for x in keep]), keep
+
     def set_coeffs(self, coarse, fine, alpha: float, beta: float):
-        """coarse, fine: (a, bx, by, bz) tuples (entries may be None: a = 0, b = 1)."""
-        arrs = [_c(x) for x in list(coarse) + list(fine)]
-        self._chk(lib().oamr_set_coeffs(self._h, *[_p(x) for x in arrs], alpha, beta), "amr set_coeffs")
+        """coarse: (a, bx, by, bz); fine: the same per patch (entries may be None: a = 0, b = 1)."""
+        cc = [_c(x) for x in coarse]
+        per = self._list(fine)
+        cols = [self._ptrs([f[i] for f in per]) for i in range(4)]
+        self._chk(lib().oamr_set_coeffs(self._h, *[_p(x) for x in cc], *[c[0] for c in cols], alpha, beta), "amr set_coeffs")
 
     def set_bc(self, types, values=None):
         t = (C.c_int * 6)(*[int(v) for v in types])
@@ -276,25 +296,32 @@ class AmrOracle:
         self._chk(lib().oamr_set_option(self._h, key.encode(), float(v)), "amr set_option")
 
     def apply(self, phic, phif):
-        phic, phif = _c(phic), _c(phif)
-        oc, of = np.zeros_like(phic), np.zeros_like(phif)
-        self._chk(lib().oamr_apply(self._h, _p(phic), _p(phif), _p(oc), _p(of)), "amr apply")
-        return oc, of
+        phic = _c(phic)
+        pf, keep = self._ptrs(self._list(phif))
+        oc = np.zeros_like(phic)
+        of = [np.zeros_like(x) for x in keep]
+        po, _ = self._ptrs(of)
+        self._chk(lib().oamr_apply(self._h, _p(phic), pf, _p(oc), po), "amr apply")
+        return oc, (of[0] if self._single else of)
 
     def average_down(self, phic, phif):
         phic = np.array(phic, dtype=np.float64, order="C")
-        self._chk(lib().oamr_average_down(self._h, _p(phic), _p(_c(phif))), "amr average_down")
+        pf, keep = self._ptrs(self._list(phif))
+        self._chk(lib().oamr_average_down(self._h, _p(phic), pf), "amr average_down")
         return phic
 
     def solve(self, rhsc, rhsf, phic0=None, phif0=None, rtol: float = 1e-12, max_cycles: int = 50):
         """Returns (phic, phif, status, cycles, relres, history)."""
-        rhsc, rhsf = _c(rhsc), _c(rhsf)
+        rhsc = _c(rhsc)
+        pr, rkeep = self._ptrs(self._list(rhsf))
         phic = np.zeros_like(rhsc) if phic0 is None else np.array(phic0, dtype=np.float64, order="C")
-        phif = np.zeros_like(rhsf) if phif0 is None else np.array(phif0, dtype=np.float64, order="C")
-        status = lib().oamr_solve(self._h, _p(rhsc), _p(rhsf), _p(phic), _p(phif), rtol, max_cycles)
+        phif = [np.zeros_like(x) for x in rkeep] if phif0 is None else \
+            [np.array(x, dtype=np.float64, order="C") for x in self._list(phif0)]
+        pp, _ = self._ptrs(phif)
+        status = lib().oamr_solve(self._h, _p(rhsc), pr, _p(phic), pp, rtol, max_cycles)
         if status != -5:
             self._chk(status, "amr solve")
         cyc, rr = C.c_int(), C.c_double()
         hist = np.zeros(max_cycles + 1)
         lib().oamr_get_info(self._h, C.byref(cyc), C.byref(rr), _p(hist))
-        return phic, phif, status, cyc.value, rr.value, hist[:cyc.value + 1].copy()
+        return phic, (phif[0] if self._single else phif), status, cyc.value, rr.value, hist[:cyc.value + 1].copy()

@@ -43,34 +43,43 @@ def _at(arr, idx):
     return arr[idx[2], idx[1], idx[0]]
 
 
+def _patches(lo, hi):
+    """lo, hi: one triple or lists of triples -> lists of triples"""
+    single = not isinstance(lo[0], (list, tuple))
+    return ([lo], [hi], True) if single else (list(lo), list(hi), False)
+
+
 def assemble(n, h, lo, hi, coarse, fine, alpha, beta, bctype):
     """The composite matrix in FLUX form: a loop over faces; a face with transmissibility T (flux = T * difference) adds
-    T / volume to the rows of the two cells it separates.  Unknowns: uncovered coarse cells (box order), then fine cells
-    (patch order).  Returns (A, cnum, fnum) with cnum[k, j, i] = -1 under the patch."""
-    m, nd = _fine_dims(n, lo, hi)
+    T / volume to the rows of the two cells it separates.  Unknowns: uncovered coarse cells (box order), then the fine
+    cells patch by patch (patch order).  lo, hi, fine: one patch or lists.  Returns (A, cnum, fnums) with cnum[k, j, i] = -1
+    under a patch and fnums a list of index arrays (a bare array for a single patch)."""
+    los, his, single = _patches(lo, hi)
+    fines = [fine] if single else list(fine)
+    nd = 3 if n[2] > 1 else 2
+    ms = [_fine_dims(n, l, u)[0] for l, u in zip(los, his)]
     cnum = -np.ones((n[2], n[1], n[0]), dtype=int)
     cnt = 0
     for k, j, i in itertools.product(range(n[2]), range(n[1]), range(n[0])):
-        inside = all(lo[d] <= (i, j, k)[d] < hi[d] for d in range(nd))
+        inside = any(all(l[d] <= (i, j, k)[d] < u[d] for d in range(nd)) for l, u in zip(los, his))
         if not inside:
             cnum[k, j, i] = cnt
             cnt += 1
-    fnum = cnt + np.arange(m[0] * m[1] * m[2]).reshape(m[2], m[1], m[0])
-    size = cnt + fnum.size
+    fnums = []
+    for m in ms:
+        fnums.append(cnt + np.arange(m[0] * m[1] * m[2]).reshape(m[2], m[1], m[0]))
+        cnt += m[0] * m[1] * m[2]
+    size = cnt
     A = np.zeros((size, size))
     volc = float(np.prod(h[:nd]))
     volf = volc / 2 ** nd
     ac, bc = coarse[0], coarse[1:]
-    af, bf = fine[0], fine[1:]
     one = lambda arr, idx: 1.0 if arr is None else _at(arr, idx)
     # absorption
     for k, j, i in itertools.product(range(n[2]), range(n[1]), range(n[0])):
         r = cnum[k, j, i]
         if r >= 0 and ac is not None:
             A[r, r] += alpha * ac[k, j, i]
-    for K, J, I in itertools.product(range(m[2]), range(m[1]), range(m[0])):
-        if af is not None:
-            A[fnum[K, J, I], fnum[K, J, I]] += alpha * af[K, J, I]
     # coarse faces
     for d in range(nd):
         ext = [n[0], n[1], n[2]]
@@ -93,51 +102,59 @@ def assemble(n, h, lo, hi, coarse, fine, alpha, beta, bctype):
                 A[l, l] += T / volc; A[l, r] -= T / volc
                 A[r, r] += T / volc; A[r, l] -= T / volc
             # both covered: no unknowns; one covered: a coarse-fine face, taken from the fine side below
-    # fine faces
-    for d in range(nd):
-        ext = [m[0], m[1], m[2]]
-        ext[d] += 1
-        hf = h[d] / 2
-        area = volf / hf
-        tang = [t for t in range(nd) if t != d]
-        for K, J, I in itertools.product(range(ext[2]), range(ext[1]), range(ext[0])):
-            face = (I, J, K)
-            left = list(face); left[d] -= 1
-            right = list(face)
-            b = one(bf[d], face)
-            if left[d] >= 0 and right[d] < m[d]:
-                T = beta * b / hf * area
-                l, r = _at(fnum, left), _at(fnum, right)
-                A[l, l] += T / volf; A[l, r] -= T / volf
-                A[r, r] += T / volf; A[r, l] -= T / volf
-                continue
-            low_side = left[d] < 0
-            fcell = right if low_side else left
-            F = _at(fnum, fcell)
-            ccell = [lo[t] + fcell[t] // 2 if t < nd else 0 for t in range(3)]
-            ccell[d] += -1 if low_side else 1
-            g = {_at(cnum, ccell): 1.0}                                # g = sum of coefficient * coarse unknown
-            for t in tang:
-                s = 1.0 if fcell[t] % 2 else -1.0
-                up = list(ccell); up[t] += 1
-                dn = list(ccell); dn[t] -= 1
-                g[_at(cnum, up)] = g.get(_at(cnum, up), 0.0) + s / 8
-                g[_at(cnum, dn)] = g.get(_at(cnum, dn), 0.0) - s / 8
-            assert all(c >= 0 for c in g)
-            T = beta * b / (1.5 * hf) * area                           # flux out of the fine cell = T (phi_F - g)
-            Cn = _at(cnum, ccell)
-            A[F, F] += T / volf
-            A[Cn, F] -= T / volc
-            for c, coef in g.items():
-                A[F, c] -= T * coef / volf
-                A[Cn, c] += T * coef / volc
-    return A, cnum, fnum
+    # fine cells and faces, patch by patch
+    for lo_, m, fnum, fcoef in zip(los, ms, fnums, fines):
+        af, bf = fcoef[0], fcoef[1:]
+        for K, J, I in itertools.product(range(m[2]), range(m[1]), range(m[0])):
+            if af is not None:
+                A[fnum[K, J, I], fnum[K, J, I]] += alpha * af[K, J, I]
+        for d in range(nd):
+            ext = [m[0], m[1], m[2]]
+            ext[d] += 1
+            hf = h[d] / 2
+            area = volf / hf
+            tang = [t for t in range(nd) if t != d]
+            for K, J, I in itertools.product(range(ext[2]), range(ext[1]), range(ext[0])):
+                face = (I, J, K)
+                left = list(face); left[d] -= 1
+                right = list(face)
+                b = one(bf[d], face)
+                if left[d] >= 0 and right[d] < m[d]:
+                    T = beta * b / hf * area
+                    l, r = _at(fnum, left), _at(fnum, right)
+                    A[l, l] += T / volf; A[l, r] -= T / volf
+                    A[r, r] += T / volf; A[r, l] -= T / volf
+                    continue
+                low_side = left[d] < 0
+                fcell = right if low_side else left
+                F = _at(fnum, fcell)
+                ccell = [lo_[t] + fcell[t] // 2 if t < nd else 0 for t in range(3)]
+                ccell[d] += -1 if low_side else 1
+                g = {_at(cnum, ccell): 1.0}                                # g = sum of coefficient * coarse unknown
+                for t in tang:
+                    s = 1.0 if fcell[t] % 2 else -1.0
+                    up = list(ccell); up[t] += 1
+                    dn = list(ccell); dn[t] -= 1
+                    g[_at(cnum, up)] = g.get(_at(cnum, up), 0.0) + s / 8
+                    g[_at(cnum, dn)] = g.get(_at(cnum, dn), 0.0) - s / 8
+                assert all(c >= 0 for c in g)
+                T = beta * b / (1.5 * hf) * area                           # flux out of the fine cell = T (phi_F - g)
+                Cn = _at(cnum, ccell)
+                A[F, F] += T / volf
+                A[Cn, F] -= T / volc
+                for c, coef in g.items():
+                    A[F, c] -= T * coef / volf
+                    A[Cn, c] += T * coef / volc
+    return A, cnum, (fnums[0] if single else fnums)
 
 
 def pack(cnum, fnum, vc, vf):
-    out = np.zeros(fnum.max() + 1)
+    fnums = fnum if isinstance(fnum, list) else [fnum]
+    vfs = vf if isinstance(vf, list) else [vf]
+    out = np.zeros(max(f.max() for f in fnums) + 1)
     out[cnum[cnum >= 0]] = vc[cnum >= 0]
-    out[fnum.ravel()] = vf.ravel()
+    for f, v in zip(fnums, vfs):
+        out[f.ravel()] = v.ravel()
     return out
 
 
@@ -313,3 +330,78 @@ def test_cycle_converges_to_the_dense_solution_and_contracts_below_0p2(n, lo, hi
     np.testing.assert_allclose(pc, o.average_down(pc, pf), rtol=0, atol=1e-15 * np.abs(pc).max())
     ratios = [hist[c] / hist[c - 1] for c in range(2, len(hist)) if hist[c] > 1e-11]
     assert max(ratios) < 0.2, ratios
+
+
+# ---- several patches (A1: at least two coarse cells apart in some direction) ----------------------------------------
+MULTI = [((16, 12, 8), (0.1, 0.07, 0.13), [(2, 2, 2), (9, 3, 2), (2, 8, 3)], [(6, 6, 6), (14, 10, 6), (7, 10, 6)]),
+         ((20, 16, 1), (0.1, 0.07, 1.0), [(2, 2, 0), (11, 3, 0), (3, 11, 0)], [(8, 7, 1), (18, 9, 1), (16, 14, 1)])]
+
+
+@pytest.mark.parametrize("n,h,los,his", MULTI)
+def test_several_patches_linear_exactness_conservation_and_dense_assembly(n, h, los, his):
+    rng = np.random.default_rng(21)
+    nd = 3 if n[2] > 1 else 2
+    ms = [_fine_dims(n, l, u)[0] for l, u in zip(los, his)]
+    # linear field, b = 1
+    o = AmrOracle(*n, *h, los, his)
+    o.set_coeffs((None,) * 4, [(None,) * 4] * len(los), 0.0, 1.0)
+    o.set_bc([N] * 6)
+    lin = lambda x, y, z: 0.3 + 1.7 * x - 2.2 * y + (0.9 * z if nd == 3 else 0.0)
+    oc, ofs = o.apply(lin(*_centres(n, h)), [lin(*_centres(n, h, l, u)) for l, u in zip(los, his)])
+    scale = 2.2 / min(h[:nd]) ** 2
+    inner = np.zeros(oc.shape, bool)
+    inner[(slice(1, -1) if nd == 3 else slice(None)), 1:-1, 1:-1] = True
+    assert max(np.abs(f).max() for f in ofs) <= 1e-13 * scale and np.abs(oc[inner]).max() <= 1e-13 * scale
+    # conservation with random b and phi
+    coarse = _random_coeffs(rng, n, with_a=False)
+    fines = [_random_coeffs(rng, m, with_a=False) for m in ms]
+    o.set_coeffs(coarse, fines, 0.0, 1.3)
+    phic, phifs = rng.standard_normal(o.coarse_shape), [rng.standard_normal(sh) for sh in o.fine_shapes]
+    oc, ofs = o.apply(phic, phifs)
+    volc = float(np.prod(h[:nd]))
+    total = oc.sum() * volc + sum(f.sum() for f in ofs) * volc / 2 ** nd
+    assert abs(total) <= 1e-12 * (np.abs(oc).sum() * volc + sum(np.abs(f).sum() for f in ofs) * volc / 2 ** nd)
+    # dense assembly, absorption and mixed box faces
+    bctype = [D, N, N, D, D, N]
+    coarse = _random_coeffs(rng, n)
+    fines = [_random_coeffs(rng, m) for m in ms]
+    o.set_coeffs(coarse, fines, 0.7, 1.3)
+    o.set_bc(bctype)
+    A, cnum, fnums = assemble(n, h, los, his, coarse, fines, 0.7, 1.3, bctype)
+    phic[cnum < 0] = 1e30
+    oc, ofs = o.apply(phic, phifs)
+    want = A @ pack(cnum, fnums, np.where(cnum >= 0, phic, 0.0), phifs)
+    got = pack(cnum, fnums, oc, ofs)
+    assert np.all(oc[cnum < 0] == 0.0) and np.abs(got - want).max() <= 1e-13 * np.abs(want).max()
+
+
+def test_several_patches_cycle_converges_to_the_dense_solution():
+    rng = np.random.default_rng(22)
+    n, los, his = (16, 8, 8), [(2, 2, 2), (9, 1, 2)], [(6, 6, 6), (14, 5, 7)]
+    h = (1.0 / n[1],) * 3
+    ms = [_fine_dims(n, l, u)[0] for l, u in zip(los, his)]
+    hf = tuple(v / 2 for v in h)
+    bfun = lambda x, y, z: np.exp(0.6 * np.sin(3.0 * x + 1.0) * np.cos(2.0 * y) + 0.3 * np.sin(4.0 * z))
+    coarse = (None,) + tuple(bfun(*_face_coords(n, h, d)) for d in range(3))
+    fines = [(None,) + tuple(bfun(*_face_coords(m, hf, d, tuple(l[t] * h[t] for t in range(3)))) for d in range(3))
+             for l, m in zip(los, ms)]
+    bctype = [D, D, N, N, N, N]
+    o = AmrOracle(*n, *h, los, his)
+    o.set_coeffs(coarse, fines, 0.0, 1.0)
+    o.set_bc(bctype)
+    rhsc, rhsfs = rng.standard_normal(o.coarse_shape), [rng.standard_normal(sh) for sh in o.fine_shapes]
+    pc, pfs, status, cycles, relres, hist = o.solve(rhsc, rhsfs, rtol=1e-12, max_cycles=40)
+    assert status == 0 and hist[0] == 1.0 and relres <= 1e-12
+    A, cnum, fnums = assemble(n, h, los, his, coarse, fines, 0.0, 1.0, bctype)
+    want = np.linalg.solve(A, pack(cnum, fnums, rhsc, rhsfs))
+    assert np.abs(pack(cnum, fnums, pc, pfs) - want).max() <= 1e-9 * np.abs(want).max()
+    ratios = [hist[c] / hist[c - 1] for c in range(2, len(hist)) if hist[c] > 1e-11]
+    assert max(ratios) < 0.2, ratios
+
+
+def test_patches_closer_than_two_coarse_cells_are_rejected():
+    from oracle import OracleError
+    with pytest.raises(OracleError) as e:
+        AmrOracle(16, 8, 8, 0.1, 0.1, 0.1, [(2, 2, 2), (7, 2, 2)], [(6, 6, 6), (12, 6, 6)])     # one cell apart
+    assert e.value.code == -2
+    AmrOracle(16, 8, 8, 0.1, 0.1, 0.1, [(2, 2, 2), (8, 2, 2)], [(6, 6, 6), (12, 6, 6)]).close()   # two cells apart
