@@ -267,9 +267,10 @@ int vmg_norm_inf_static(const double* v, long long n, double* out, void* cuda_st
  * time step and solves every equation with "the composite multilevel multigrid solver from within AMReX";
  * it gives no formula, so the interface discretisation and the cycle are readings A1-A5 of DESIGN.md (restated in
  * oracle/amr_oracle.c, which this is tested against):
- *   A1  one box patch of coarse cells [lo, hi) refined by 2, at least one coarse cell away from the box boundary and at
- *       least two coarse cells wide in every active direction; the patch as a box of 2 (hi - lo) fine cells must itself be
- *       a legal vmg grid with at least two levels (else VMG_ERR_SIZE);
+ *   A1  box patches of coarse cells [lo, hi) refined by 2, each at least one coarse cell away from the box boundary and at
+ *       least two coarse cells wide in every active direction, two patches at least two coarse cells apart in some
+ *       direction; a patch as a box of 2 (hi - lo) fine cells must itself be a legal vmg grid with at least two levels
+ *       (else VMG_ERR_SIZE);
  *   A2  coarse-fine face: flux b_f (g - phi_f) / (1.5 hf) per unit area, g = the coarse field at the point of the adjacent
  *       coarse cell opposite the fine cell centre, interpolated linearly in the tangential directions;
  *   A3  the coarse cell takes the sum of the fine fluxes through its face (conservation);
@@ -287,17 +288,23 @@ int vmg_norm_inf_static(const double* v, long long n, double* out, void* cuda_st
  * Stream: as vmg_create (NULL: the library creates one); both levels run on it.  vmg_amr_solve synchronises it.
  * Options: "nu_f" (1..64); every other key goes to the coarse handle (vmg_set_option).  No mask, no PCG on composite grids. */
 typedef struct vmg_amr_s* vmg_amr_handle;
+/* npatch >= 1 patches; lo, hi: npatch triples of coarse cell indices, flattened (lo[3 q + d]); HOST arrays */
 int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, double dy, double dz,
-                   const int lo[3], const int hi[3], void* cuda_stream);
-int vmg_amr_fine_dims(vmg_amr_handle h, int dims[3]);
+                   int npatch, const int* lo, const int* hi, void* cuda_stream);
+int vmg_amr_num_patches(vmg_amr_handle h);
+int vmg_amr_fine_dims(vmg_amr_handle h, int patch, int dims[3]);
+/* a_f, bx_f, by_f, bz_f: HOST arrays of npatch DEVICE pointers (one set of fine arrays per patch); an array may be NULL
+ * altogether or hold NULL entries (a = 0, b = 1 on that patch) */
 int vmg_amr_set_coeffs(vmg_amr_handle h, const double* a_c, const double* bx_c, const double* by_c, const double* bz_c,
-                       const double* a_f, const double* bx_f, const double* by_f, const double* bz_f, double alpha, double beta);
+                       const double* const* a_f, const double* const* bx_f, const double* const* by_f, const double* const* bz_f,
+                       double alpha, double beta);
 int vmg_amr_set_bc(vmg_amr_handle h, const int type[6], const double* const value[6]);
 int vmg_amr_set_option(vmg_amr_handle h, const char* key, double v);
-int vmg_amr_solve(vmg_amr_handle h, const double* rhs_c, const double* rhs_f, double* phi_c, double* phi_f,
+/* rhs_f, phi_f: HOST arrays of npatch DEVICE pointers */
+int vmg_amr_solve(vmg_amr_handle h, const double* rhs_c, const double* const* rhs_f, double* phi_c, double* const* phi_f,
                   double rtol, int max_cycles);
 int vmg_amr_get_info(vmg_amr_handle h, int* cycles, double* relres, double* history /* >= cycles + 1 or NULL */);
-/* vmg_debug_pad_check over the box and the patch: number of non-zero pad entries (0 expected) */
+/* vmg_debug_pad_check over the box and the patches: number of non-zero pad entries (0 expected) */
 int vmg_amr_debug_pad_check(vmg_amr_handle h, long long* nonzero);
 long long vmg_amr_last_launch_count(vmg_amr_handle h);
 int vmg_amr_last_cuda_error(vmg_amr_handle h);

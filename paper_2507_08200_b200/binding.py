@@ -24,7 +24,7 @@ SYMBOLS = ["vmg_create", "vmg_create_batch", "vmg_set_coeffs", "vmg_set_bc", "vm
            "vmg_last_launch_count", "vmg_total_launch_count", "vmg_get_profile", "vmg_debug_pad_check",
            "vmg_norm_inf_static", "vmg_amr_create", "vmg_amr_fine_dims", "vmg_amr_set_coeffs", "vmg_amr_set_bc",
            "vmg_amr_set_option", "vmg_amr_solve", "vmg_amr_get_info", "vmg_amr_last_launch_count",
-           "vmg_amr_last_cuda_error", "vmg_amr_destroy", "vmg_amr_debug_pad_check"]
+           "vmg_amr_last_cuda_error", "vmg_amr_destroy", "vmg_amr_debug_pad_check", "vmg_amr_num_patches"]
 
 _lib = None
 _vp = C.c_void_p
@@ -74,12 +74,14 @@ def load():
     lib.vmg_debug_pad_check.argtypes = [_vp, C.POINTER(C.c_longlong)]
     lib.vmg_norm_inf_static.argtypes = [_vp, C.c_longlong, _vp, _vp, C.POINTER(C.c_char_p)]
     _ip = C.POINTER(C.c_int)
-    lib.vmg_amr_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, _ip, _vp]
-    lib.vmg_amr_fine_dims.argtypes = [_vp, _ip]
-    lib.vmg_amr_set_coeffs.argtypes = [_vp] + [_vp] * 8 + [C.c_double, C.c_double]
+    lib.vmg_amr_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, _ip, _ip, _vp]
+    lib.vmg_amr_num_patches.argtypes = [_vp]
+    lib.vmg_amr_fine_dims.argtypes = [_vp, C.c_int, _ip]
+    _pv = C.POINTER(_vp)
+    lib.vmg_amr_set_coeffs.argtypes = [_vp] + [_vp] * 4 + [_pv] * 4 + [C.c_double, C.c_double]
     lib.vmg_amr_set_bc.argtypes = [_vp, _ip, C.POINTER(_vp)]
     lib.vmg_amr_set_option.argtypes = [_vp, C.c_char_p, C.c_double]
-    lib.vmg_amr_solve.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_double, C.c_int]
+    lib.vmg_amr_solve.argtypes = [_vp, _vp, _pv, _vp, _pv, C.c_double, C.c_int]
     lib.vmg_amr_get_info.argtypes = [_vp, _ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.vmg_amr_last_launch_count.argtypes = [_vp]
     lib.vmg_amr_last_launch_count.restype = C.c_longlong
@@ -309,8 +311,9 @@ class Vmg:
 
 
 class VmgAmr:
-    """Two-level composite solve (vmg_amr_* of include/vmg.h): an nx x ny x nz box with one patch of coarse cells [lo, hi)
-    refined by 2.  Coarse tensors [k, j, i] on the box, fine tensors [K, J, I] on the patch."""
+    """Two-level composite solve (vmg_amr_* of include/vmg.h): an nx x ny x nz box with patches of coarse cells [lo, hi)
+    refined by 2.  lo, hi: one triple (a single patch: fine tensors are then passed and returned bare) or lists of triples
+    (fine tensors as lists, one entry per patch).  Coarse tensors [k, j, i] on the box, fine tensors [K, J, I] on a patch."""
 
     def __init__(self, nx, ny, nz, dx, dy, dz, lo, hi, stream=None):
         torch = _torch()
@@ -318,14 +321,23 @@ class VmgAmr:
         self._h = _vp()
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         sptr = self.stream.cuda_stream
-        l3, h3 = (C.c_int * 3)(*[int(v) for v in lo]), (C.c_int * 3)(*[int(v) for v in hi])
-        rc = self._lib.vmg_amr_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, l3, h3, _vp(sptr) if sptr else None)
+        self._single = not isinstance(lo[0], (list, tuple))
+        los = [lo] if self._single else list(lo)
+        his = [hi] if self._single else list(hi)
+        self.np = len(los)
+        flat = lambda v: (C.c_int * (3 * self.np))(*[int(x) for t in v for x in t])
+        rc = self._lib.vmg_amr_create(C.byref(self._h), nx, ny, nz, dx, dy, dz, self.np, flat(los), flat(his),
+                                      _vp(sptr) if sptr else None)
         if rc != 0:
             self._h = None
             raise VmgError(rc, "vmg_amr_create")
-        d = (C.c_int * 3)()
-        self._lib.vmg_amr_fine_dims(self._h, d)
-        self.coarse_shape, self.fine_shape = (nz, ny, nx), (d[2], d[1], d[0])
+        self.coarse_shape = (nz, ny, nx)
+        self.fine_shapes = []
+        for q in range(self.np):
+            d = (C.c_int * 3)()
+            self._lib.vmg_amr_fine_dims(self._h, q, d)
+            self.fine_shapes.append((d[2], d[1], d[0]))
+        self.fine_shape = self.fine_shapes[0]
         self._keep = None
 
     def _chk(self, rc, where):
@@ -340,11 +352,18 @@ class VmgAmr:
 
     __del__ = destroy
 
+    def _list(self, x):
+        return [x] if self._single else list(x)
+
+    def _ptrs(self, tensors):
+        return (_vp * self.np)(*[_ptr(t) for t in tensors])
+
     def set_coeffs(self, coarse, fine, alpha: float, beta: float):
-        """coarse, fine: (a, bx, by, bz) tuples of tensors (None: a = 0, b = 1); borrowed until the next call."""
-        self._keep = (tuple(coarse), tuple(fine))
-        ptrs = [_ptr(t) for t in list(coarse) + list(fine)]
-        self._chk(self._lib.vmg_amr_set_coeffs(self._h, *ptrs, alpha, beta), "vmg_amr_set_coeffs")
+        """coarse: (a, bx, by, bz) tensors; fine: the same per patch (None: a = 0, b = 1); borrowed until the next call."""
+        per = [tuple(f) for f in self._list(fine)]
+        self._keep = (tuple(coarse), per)
+        cols = [self._ptrs([f[i] for f in per]) for i in range(4)]
+        self._chk(self._lib.vmg_amr_set_coeffs(self._h, *[_ptr(t) for t in coarse], *cols, alpha, beta), "vmg_amr_set_coeffs")
 
     def set_bc(self, types, values=None):
         t = (C.c_int * 6)(*[int(v) for v in types])
@@ -358,15 +377,16 @@ class VmgAmr:
     def solve(self, rhs_c, rhs_f, phi_c=None, phi_f=None, rtol: float = 1e-12, max_cycles: int = 50):
         """Returns (phi_c, phi_f, status, cycles, relres, history); phi_c, phi_f are updated in place when given."""
         torch = _torch()
+        rf = self._list(rhs_f)
         phi_c = torch.zeros_like(rhs_c) if phi_c is None else phi_c
-        phi_f = torch.zeros_like(rhs_f) if phi_f is None else phi_f
-        status = self._lib.vmg_amr_solve(self._h, _ptr(rhs_c), _ptr(rhs_f), _ptr(phi_c), _ptr(phi_f), rtol, max_cycles)
+        pf = [torch.zeros_like(r) for r in rf] if phi_f is None else self._list(phi_f)
+        status = self._lib.vmg_amr_solve(self._h, _ptr(rhs_c), self._ptrs(rf), _ptr(phi_c), self._ptrs(pf), rtol, max_cycles)
         if status != -5:
             self._chk(status, "vmg_amr_solve")
         cyc, rr = C.c_int(), C.c_double()
         hist = (C.c_double * (max_cycles + 2))()
         self._lib.vmg_amr_get_info(self._h, C.byref(cyc), C.byref(rr), hist)
-        return phi_c, phi_f, status, cyc.value, rr.value, [hist[i] for i in range(cyc.value + 1)]
+        return phi_c, (pf[0] if self._single else pf), status, cyc.value, rr.value, [hist[i] for i in range(cyc.value + 1)]
 
     def last_launch_count(self) -> int:
         return int(self._lib.vmg_amr_last_launch_count(self._h))

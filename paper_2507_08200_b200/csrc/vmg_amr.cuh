@@ -89,7 +89,7 @@ __global__ void amr_mask_norm_kernel(AmrGeom A, double* __restrict__ btc, unsign
         v = fabs(btc[c]);
         if (v != v) v = __longlong_as_double(0x7ff8000000000000ll);
     }
-    block_max_to_global(v, norm);
+    if (norm) block_max_to_global(v, norm);      // NULL: only zero under this patch (more patches follow)
 }
 
 // A3 + A4: the right-hand side of the coarse V-cycle, which runs IN PLACE on phi_c (solution form): one V-cycle maps

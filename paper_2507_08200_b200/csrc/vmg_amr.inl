@@ -5,24 +5,27 @@
 
 struct vmg_amr_s {
     vmg_s* hc = nullptr;            // the coarse box (an ordinary handle: correction V-cycle, fold_bc)
-    vmg_s* hf = nullptr;            // the patch (an ordinary handle whose faces are coarse-fine faces)
-    AmrGeom A;
+    std::vector<vmg_s*> hf;         // the patches (ordinary handles whose faces are coarse-fine faces)
+    std::vector<AmrGeom> A;         // per patch: box, patch and shadow geometry
     cudaStream_t stream = nullptr;
-    void* base = nullptr;           // one allocation: btilde_c (padded like a level array), rhs_f copy, shadow means, scalars
-    double *btc = nullptr, *rhsf = nullptr, *old = nullptr;
-    unsigned long long* d_norm = nullptr;   // ||btilde_c||, ||f_f||, ||r_c||, ||r_f|| (bit patterns), 
+    void* base = nullptr;           // one allocation: btilde_c (padded like a level array), per patch rhs_f copy and shadow means, scalars
+    double* btc = nullptr;
+    std::vector<double*> rhsf, old;
+    unsigned long long* d_norm = nullptr;   // ||btilde_c||, ||f_f||, ||r_c||, ||r_f|| (bit patterns; the fine ones over all patches)
     double* h_norm = nullptr;       // pinned mirror
     int nu_f = 6;                   // A4: fine sweeps per cycle
     bool have_coeffs = false, have_bc = false;
     cudaGraph_t graph[3] = {nullptr, nullptr, nullptr};   // 0: composite residual + norms (every cell), 1: correction + fine sweeps,
     cudaGraphExec_t exec[3] = {nullptr, nullptr, nullptr};   // 2: as 0 with the coarse norm over the red cells (after a V-cycle, R12)
     long long graph_launches[3] = {0, 0, 0};
-    unsigned epoch_c = 0, epoch_f = 0;
+    unsigned epoch_c = 0;
+    std::vector<unsigned> epoch_f;
     int graph_nu_f = -1;
     int cycles = 0, last_cuda_error = 0;
     double relres = 0.0;
     std::vector<double> hist;
     long long launches = 0;
+    int np() const { return (int)hf.size(); }
 };
 
 #define AMR_TRY(A_, expr)                                                      \
@@ -45,72 +48,91 @@ void amr_drop_graphs(vmg_amr_s* a)
     }
 }
 
-// value planes of the patch from the coarse field, then btilde_f = f_f + 2 wb g (the library's fold_bc)
-int amr_enqueue_ghost_fold(vmg_amr_s* a, long long* count)
+// value planes of patch q from the coarse field, then btilde_f = f_f + 2 wb g (the library's fold_bc)
+int amr_enqueue_ghost_fold(vmg_amr_s* a, int q, long long* count)
 {
-    vmg_s* hf = a->hf;
+    vmg_s* hf = a->hf[q];
     AmrGhostArgs g;
-    g.A = a->A; g.phic = a->hc->lev[0].phi;
+    g.A = a->A[q]; g.phic = a->hc->lev[0].phi;
     long long most = 0;
     for (int f = 0; f < 6; ++f) {
         g.plane[f] = hf->bcval[f];
-        if (f < 2 * a->A.nd) most = std::max<long long>(most, (long long)plane_count(hf->lev[0], f));
+        if (f < 2 * g.A.nd) most = std::max<long long>(most, (long long)plane_count(hf->lev[0], f));
     }
-    amr_ghost_kernel<<<dim3(grid_for(most), 2 * a->A.nd), kThreads, 0, a->stream>>>(g);
+    amr_ghost_kernel<<<dim3(grid_for(most), 2 * g.A.nd), kThreads, 0, a->stream>>>(g);
     ++*count;
     long long before = hf->launches;
-    int rc = enqueue_fold_bc(hf, a->rhsf, hf->lev[0].rhs);
+    int rc = enqueue_fold_bc(hf, a->rhsf[q], hf->lev[0].rhs);
     *count += hf->launches - before;
     return rc;
 }
 
-// graphs 0 / 2: the composite residual (A3) -- the patch's residual + restriction and residual norm, the coarse right-hand
-// side in and next to the patch, then the library's residual norm of the box on that right-hand side (amr_patch_rhs_kernel)
+// graphs 0 / 2: the composite residual (A3) -- every patch's residual + restriction and residual norm, the coarse right-hand
+// side in and next to every patch, then the library's residual norm of the box on that right-hand side (amr_patch_rhs_kernel)
 void amr_enqueue_residual(vmg_amr_s* a, long long* count, bool red_only)
 {
-    vmg_s *hc = a->hc, *hf = a->hf;
+    vmg_s* hc = a->hc;
     cudaMemsetAsync(a->d_norm + 2, 0, 2 * sizeof(unsigned long long), a->stream);
-    hf->lev[0].cur = 0;
-    plain_residual_restrict(hf, 0, count);
-    enqueue_residual_norm(hf, a->d_norm + 3);
-    ++*count;
-    AmrResArgs g;
-    g.A = a->A; g.Lc = view(hc->lev[0]);
-    g.phic = hc->lev[0].phi; g.btc = a->btc; g.rs = hf->lev[1].rhs; g.phif = hf->lev[0].phi;
-    g.R = hc->lev[0].rhs;
-    for (int f = 0; f < 6; ++f) { g.gplane[f] = hf->bcval[f]; g.wbf[f] = hf->lev[0].wb[f]; }
-    g.wscale = 2.0 / (double)(1 << a->A.nd);
-    g.norm = a->d_norm + 2;
-    long long region = 1;
-    for (int d = 0; d < a->A.nd; ++d) region *= a->A.hi[d] - a->A.lo[d] + 2;
-    amr_patch_rhs_kernel<<<grid_for(region), kThreads, 0, a->stream>>>(g);
+    for (int q = 0; q < a->np(); ++q) {
+        vmg_s* hf = a->hf[q];
+        hf->lev[0].cur = 0;
+        plain_residual_restrict(hf, 0, count);
+        enqueue_residual_norm(hf, a->d_norm + 3);
+        ++*count;
+    }
+    for (int q = 0; q < a->np(); ++q) {
+        vmg_s* hf = a->hf[q];
+        AmrResArgs g;
+        g.A = a->A[q]; g.Lc = view(hc->lev[0]);
+        g.phic = hc->lev[0].phi; g.btc = a->btc; g.rs = hf->lev[1].rhs; g.phif = hf->lev[0].phi;
+        g.R = hc->lev[0].rhs;
+        for (int f = 0; f < 6; ++f) { g.gplane[f] = hf->bcval[f]; g.wbf[f] = hf->lev[0].wb[f]; }
+        g.wscale = 2.0 / (double)(1 << g.A.nd);
+        g.norm = a->d_norm + 2;
+        long long region = 1;
+        for (int d = 0; d < g.A.nd; ++d) region *= g.A.hi[d] - g.A.lo[d] + 2;
+        amr_patch_rhs_kernel<<<grid_for(region), kThreads, 0, a->stream>>>(g);
+        ++*count;
+    }
     hc->lev[0].cur = 0;
     enqueue_residual_norm(hc, a->d_norm + 2, red_only);
-    *count += 2;
+    ++*count;
 }
 
-// graph 1: A4 after the exit test -- coarse V-cycle (in place on phi_c, right-hand side of amr_patch_rhs_kernel),
-// correction of the patch, ghosts, fine sweeps, average down
+// graph 1: A4 after the exit test -- coarse V-cycle (in place on phi_c, right-hand side of amr_patch_rhs_kernel), then per
+// patch: correction, ghosts, fine sweeps, average down
 int amr_enqueue_correction(vmg_amr_s* a, long long* count)
 {
-    vmg_s *hc = a->hc, *hf = a->hf;
+    vmg_s* hc = a->hc;
     VmgLevel& C0 = hc->lev[0];
     enqueue_vcycle(hc, nullptr, count);
-    amr_prolong_add_kernel<<<grid_for(a->A.F.n), kThreads, 0, a->stream>>>(a->A, hf->lev[0].phi, C0.phi, a->old);
-    ++*count;
-    int rc = amr_enqueue_ghost_fold(a, count);
-    if (rc != VMG_OK) return rc;
-    hf->lev[0].cur = 0; hf->lev[0].dir = 0;
-    plain_smooth(hf, 0, a->nu_f, count);
-    amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, hf->lev[0].phi, C0.phi, a->old);
-    ++*count;
+    for (int q = 0; q < a->np(); ++q) {
+        vmg_s* hf = a->hf[q];
+        const AmrGeom& A = a->A[q];
+        amr_prolong_add_kernel<<<grid_for(A.F.n), kThreads, 0, a->stream>>>(A, hf->lev[0].phi, C0.phi, a->old[q]);
+        ++*count;
+        int rc = amr_enqueue_ghost_fold(a, q, count);
+        if (rc != VMG_OK) return rc;
+        hf->lev[0].cur = 0; hf->lev[0].dir = 0;
+        plain_smooth(hf, 0, a->nu_f, count);
+        amr_average_down_kernel<<<grid_for(A.S.n), kThreads, 0, a->stream>>>(A, hf->lev[0].phi, C0.phi, a->old[q]);
+        ++*count;
+    }
     return VMG_OK;
 }
 
-// runs part `which` (0 residual over every cell, 1 correction, 2 residual with the coarse norm over the red cells): a graph replay, or plain launches with option graph = 0 / profile on the coarse handle
+bool amr_graphs_current(const vmg_amr_s* a)
+{
+    if (!a->exec[0] || a->epoch_c != a->hc->graph_epoch || a->graph_nu_f != a->nu_f) return false;
+    for (int q = 0; q < a->np(); ++q) if (a->epoch_f[q] != a->hf[q]->graph_epoch) return false;
+    return true;
+}
+
+// runs part `which` (0 residual over every cell, 1 correction, 2 residual with the coarse norm over the red cells): a graph
+// replay, or plain launches with option graph = 0 / profile on the coarse handle
 int amr_run(vmg_amr_s* a, int which)
 {
-    vmg_s *hc = a->hc, *hf = a->hf;
+    vmg_s* hc = a->hc;
     if (!hc->use_graph || hc->profile) {
         long long count = 0;
         int rc = VMG_OK;
@@ -120,7 +142,7 @@ int amr_run(vmg_amr_s* a, int which)
         AMR_TRY(a, cudaGetLastError());
         return VMG_OK;
     }
-    if (!a->exec[0] || a->epoch_c != hc->graph_epoch || a->epoch_f != hf->graph_epoch || a->graph_nu_f != a->nu_f) {
+    if (!amr_graphs_current(a)) {
         amr_drop_graphs(a);
         for (int i = 0; i < 3; ++i) {
             long long count = 0;
@@ -133,7 +155,8 @@ int amr_run(vmg_amr_s* a, int which)
             AMR_TRY(a, e);
             a->graph_launches[i] = count;
         }
-        a->epoch_c = hc->graph_epoch; a->epoch_f = hf->graph_epoch; a->graph_nu_f = a->nu_f;
+        a->epoch_c = hc->graph_epoch; a->graph_nu_f = a->nu_f;
+        for (int q = 0; q < a->np(); ++q) a->epoch_f[q] = a->hf[q]->graph_epoch;
     }
     AMR_TRY(a, cudaGraphLaunch(a->exec[which], a->stream));
     a->launches += a->graph_launches[which];
@@ -149,7 +172,7 @@ int vmg_amr_destroy(vmg_amr_handle a)
     if (!a) return VMG_ERR_ARG;
     if (a->stream) cudaStreamSynchronize(a->stream);
     amr_drop_graphs(a);
-    if (a->hf) vmg_destroy(a->hf);          // the patch first: the coarse handle may own the stream
+    for (vmg_s* h : a->hf) if (h) vmg_destroy(h);   // the patches first: the coarse handle may own the stream
     if (a->hc) vmg_destroy(a->hc);
     if (a->base) cudaFree(a->base);
     if (a->h_norm) cudaFreeHost(a->h_norm);
@@ -159,33 +182,45 @@ int vmg_amr_destroy(vmg_amr_handle a)
 }
 
 int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, double dy, double dz,
-                   const int lo[3], const int hi[3], void* cuda_stream)
+                   int npatch, const int* lo, const int* hi, void* cuda_stream)
 {
-    if (!out || !lo || !hi) return VMG_ERR_ARG;
+    if (!out || !lo || !hi || npatch < 1) return VMG_ERR_ARG;
     *out = nullptr;
     const int n[3] = {nx, ny, nz}, nd = nz > 1 ? 3 : 2;
-    int m[3] = {1, 1, 1};
-    for (int d = 0; d < nd; ++d) {
-        // A1: inside the box, one coarse cell away from its boundary, at least two coarse cells wide
-        if (lo[d] < 1 || hi[d] > n[d] - 1 || hi[d] - lo[d] < 2) return VMG_ERR_SIZE;
-        m[d] = 2 * (hi[d] - lo[d]);
-    }
+    for (int q = 0; q < npatch; ++q)
+        for (int d = 0; d < nd; ++d)   // A1: inside the box, one coarse cell away from its boundary, at least two coarse cells wide
+            if (lo[3 * q + d] < 1 || hi[3 * q + d] > n[d] - 1 || hi[3 * q + d] - lo[3 * q + d] < 2) return VMG_ERR_SIZE;
+    for (int q = 0; q < npatch; ++q)       // A1: two patches at least two coarse cells apart in some direction
+        for (int r = q + 1; r < npatch; ++r) {
+            bool apart = false;
+            for (int d = 0; d < nd; ++d)
+                apart = apart || lo[3 * r + d] - hi[3 * q + d] >= 2 || lo[3 * q + d] - hi[3 * r + d] >= 2;
+            if (!apart) return VMG_ERR_SIZE;
+        }
     vmg_amr_s* a = new (std::nothrow) vmg_amr_s();
     if (!a) return VMG_ERR_ALLOC;
     int rc = vmg_create(&a->hc, nx, ny, nz, dx, dy, dz, cuda_stream);
-    if (rc == VMG_OK) {
-        a->stream = a->hc->stream;
-        rc = vmg_create(&a->hf, m[0], m[1], m[2], 0.5 * dx, 0.5 * dy, nd == 3 ? 0.5 * dz : dz, (void*)a->stream);
-        if (rc == VMG_OK && a->hf->nlev < 2) rc = VMG_ERR_SIZE;
-    }
     if (rc != VMG_OK) { vmg_amr_destroy(a); return rc; }
-    a->hf->l2_persist_mb = 0.0;             // one stream: the access-policy window belongs to the coarse box
-    a->A.C = a->hc->lev[0].G; a->A.F = a->hf->lev[0].G; a->A.S = a->hf->lev[1].G;
-    a->A.nd = nd;
-    for (int d = 0; d < 3; ++d) { a->A.lo[d] = d < nd ? lo[d] : 0; a->A.hi[d] = d < nd ? hi[d] : 1; }
+    a->stream = a->hc->stream;
     const VmgLevel& C0 = a->hc->lev[0];
     const size_t arr = (size_t)C0.nalloc + 2 * (size_t)C0.pad;
-    const size_t total = round_up(arr, 32) + round_up((size_t)a->hf->lev[0].n, 32) + round_up((size_t)a->hf->lev[1].n, 32) + 32;
+    size_t total = round_up(arr, 32) + 32;
+    for (int q = 0; q < npatch; ++q) {
+        int m[3] = {1, 1, 1};
+        for (int d = 0; d < nd; ++d) m[d] = 2 * (hi[3 * q + d] - lo[3 * q + d]);
+        vmg_s* hf = nullptr;
+        rc = vmg_create(&hf, m[0], m[1], m[2], 0.5 * dx, 0.5 * dy, nd == 3 ? 0.5 * dz : dz, (void*)a->stream);
+        if (rc == VMG_OK) a->hf.push_back(hf);
+        if (rc == VMG_OK && hf->nlev < 2) rc = VMG_ERR_SIZE;
+        if (rc != VMG_OK) { vmg_amr_destroy(a); return rc; }
+        hf->l2_persist_mb = 0.0;            // one stream: the access-policy window belongs to the coarse box
+        AmrGeom A;
+        A.C = C0.G; A.F = hf->lev[0].G; A.S = hf->lev[1].G; A.nd = nd;
+        for (int d = 0; d < 3; ++d) { A.lo[d] = d < nd ? lo[3 * q + d] : 0; A.hi[d] = d < nd ? hi[3 * q + d] : 1; }
+        a->A.push_back(A);
+        total += round_up((size_t)hf->lev[0].n, 32) + round_up((size_t)hf->lev[1].n, 32);
+    }
+    a->epoch_f.assign((size_t)npatch, 0u);
     if (cudaMalloc(&a->base, total * sizeof(double)) != cudaSuccess ||
         cudaMallocHost((void**)&a->h_norm, 4 * sizeof(double)) != cudaSuccess ||
         cudaMemsetAsync(a->base, 0, total * sizeof(double), a->stream) != cudaSuccess ||
@@ -196,37 +231,47 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
     }
     double* b = (double*)a->base;
     a->btc = b + C0.pad;
-    a->rhsf = b + round_up(arr, 32);
-    a->old = a->rhsf + round_up((size_t)a->hf->lev[0].n, 32);
-    a->d_norm = (unsigned long long*)(a->old + round_up((size_t)a->hf->lev[1].n, 32));
+    double* p = b + round_up(arr, 32);
+    for (int q = 0; q < npatch; ++q) {
+        a->rhsf.push_back(p); p += round_up((size_t)a->hf[q]->lev[0].n, 32);
+        a->old.push_back(p);  p += round_up((size_t)a->hf[q]->lev[1].n, 32);
+    }
+    a->d_norm = (unsigned long long*)p;
     *out = a;
     return VMG_OK;
 }
 
-int vmg_amr_fine_dims(vmg_amr_handle a, int dims[3])
+int vmg_amr_num_patches(vmg_amr_handle a) { return a ? a->np() : VMG_ERR_ARG; }
+
+int vmg_amr_fine_dims(vmg_amr_handle a, int patch, int dims[3])
 {
-    if (!a || !dims) return VMG_ERR_ARG;
-    dims[0] = a->A.F.nx; dims[1] = a->A.F.ny; dims[2] = a->A.F.nz;
+    if (!a || !dims || patch < 0 || patch >= a->np()) return VMG_ERR_ARG;
+    dims[0] = a->A[patch].F.nx; dims[1] = a->A[patch].F.ny; dims[2] = a->A[patch].F.nz;
     return VMG_OK;
 }
 
 int vmg_amr_set_coeffs(vmg_amr_handle a, const double* a_c, const double* bx_c, const double* by_c, const double* bz_c,
-                       const double* a_f, const double* bx_f, const double* by_f, const double* bz_f, double alpha, double beta)
+                       const double* const* a_f, const double* const* bx_f, const double* const* by_f, const double* const* bz_f,
+                       double alpha, double beta)
 {
     if (!a) return VMG_ERR_ARG;
-    if (!a_c != !a_f) return VMG_ERR_ARG;                  // the absorption term exists on both levels or on neither
+    for (int q = 0; q < a->np(); ++q)                      // the absorption term exists on both levels or on neither
+        if (!a_c != !(a_f && a_f[q])) return VMG_ERR_ARG;
     int rc = vmg_set_coeffs(a->hc, a_c, bx_c, by_c, bz_c, alpha, beta);
     if (rc != VMG_OK) { a->last_cuda_error = a->hc->last_cuda_error; return rc; }
-    rc = vmg_set_coeffs(a->hf, a_f, bx_f, by_f, bz_f, alpha, beta);
-    if (rc != VMG_OK) { a->last_cuda_error = a->hf->last_cuda_error; return rc; }
-    // A2: the patch's faces carry beta b / (1.5 hf^2) = 2 * (beta b / hf^2) / 3: scale its boundary planes, then 1/D again
-    VmgLevel& F0 = a->hf->lev[0];
-    for (int f = 0; f < 2 * a->A.nd; ++f) {
-        const long long np = (long long)plane_count(F0, f);
-        amr_scale_kernel<<<grid_for(np), kThreads, 0, a->stream>>>(F0.wb[f], np, 1.0 / 3.0);
+    for (int q = 0; q < a->np(); ++q) {
+        vmg_s* hf = a->hf[q];
+        rc = vmg_set_coeffs(hf, a_f ? a_f[q] : nullptr, bx_f ? bx_f[q] : nullptr, by_f ? by_f[q] : nullptr, bz_f ? bz_f[q] : nullptr, alpha, beta);
+        if (rc != VMG_OK) { a->last_cuda_error = hf->last_cuda_error; return rc; }
+        // A2: the patch's faces carry beta b / (1.5 hf^2) = 2 * (beta b / hf^2) / 3: scale its boundary planes, then 1/D again
+        VmgLevel& F0 = hf->lev[0];
+        for (int f = 0; f < 2 * a->A[q].nd; ++f) {
+            const long long npl = (long long)plane_count(F0, f);
+            amr_scale_kernel<<<grid_for(npl), kThreads, 0, a->stream>>>(F0.wb[f], npl, 1.0 / 3.0);
+        }
+        hf->dinv_dirty = true;
     }
     AMR_TRY(a, cudaGetLastError());
-    a->hf->dinv_dirty = true;
     a->have_coeffs = true;
     return VMG_OK;
 }
@@ -237,9 +282,11 @@ int vmg_amr_set_bc(vmg_amr_handle a, const int type[6], const double* const valu
     int rc = vmg_set_bc(a->hc, type, value);
     if (rc != VMG_OK) return rc;
     const int all_dirichlet[6] = {VMG_BC_DIRICHLET, VMG_BC_DIRICHLET, VMG_BC_DIRICHLET, VMG_BC_DIRICHLET, VMG_BC_DIRICHLET, VMG_BC_DIRICHLET};
-    rc = vmg_set_bc(a->hf, all_dirichlet, nullptr);
-    if (rc != VMG_OK) return rc;
-    for (int f = 0; f < 2 * a->A.nd; ++f) a->hf->bc_has_value[f] = true;   // the planes are written by amr_ghost_kernel
+    for (int q = 0; q < a->np(); ++q) {
+        rc = vmg_set_bc(a->hf[q], all_dirichlet, nullptr);
+        if (rc != VMG_OK) return rc;
+        for (int f = 0; f < 2 * a->A[q].nd; ++f) a->hf[q]->bc_has_value[f] = true;   // the planes are written by amr_ghost_kernel
+    }
     a->have_bc = true;
     return VMG_OK;
 }
@@ -260,46 +307,56 @@ int vmg_amr_get_info(vmg_amr_handle a, int* cycles, double* relres, double* hist
     return VMG_OK;
 }
 
-// vmg_debug_pad_check over both handles (the zero pads and pad elements of every level array of the box and of the patch)
+// vmg_debug_pad_check over all handles (the zero pads and pad elements of every level array of the box and of the patches)
 int vmg_amr_debug_pad_check(vmg_amr_handle a, long long* nonzero)
 {
     if (!a || !nonzero) return VMG_ERR_ARG;
-    long long nc = 0, nf = 0;
-    int rc = vmg_debug_pad_check(a->hc, &nc);
-    if (rc == VMG_OK) rc = vmg_debug_pad_check(a->hf, &nf);
-    *nonzero = nc + nf;
+    long long total = 0, one = 0;
+    int rc = vmg_debug_pad_check(a->hc, &total);
+    for (int q = 0; q < a->np() && rc == VMG_OK; ++q) { rc = vmg_debug_pad_check(a->hf[q], &one); total += one; }
+    *nonzero = total;
     return rc;
 }
 
 long long vmg_amr_last_launch_count(vmg_amr_handle a) { return a ? a->launches : 0; }
 int vmg_amr_last_cuda_error(vmg_amr_handle a) { return a ? a->last_cuda_error : 0; }
 
-int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, double* phi_c, double* phi_f,
+int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* const* rhs_f, double* phi_c, double* const* phi_f,
                   double rtol, int max_cycles)
 {
     if (!a || !rhs_c || !rhs_f || !phi_c || !phi_f || max_cycles < 0) return VMG_ERR_ARG;
+    for (int q = 0; q < a->np(); ++q) if (!rhs_f[q] || !phi_f[q]) return VMG_ERR_ARG;
     if (!a->have_coeffs || !a->have_bc) return VMG_ERR_STATE;
-    vmg_s *hc = a->hc, *hf = a->hf;
+    vmg_s* hc = a->hc;
     int rc = ready(hc);
-    if (rc == VMG_OK) rc = ready(hf);
+    for (int q = 0; q < a->np() && rc == VMG_OK; ++q) rc = ready(a->hf[q]);
     if (rc != VMG_OK) return rc;
-    VmgLevel &C0 = hc->lev[0], &F0 = hf->lev[0];
+    VmgLevel& C0 = hc->lev[0];
     a->hist.clear(); a->cycles = 0; a->relres = 0.0; a->launches = 0;
-    // begin: btilde_c (box boundary values folded, zero under the patch), the two norms of A5, phi into the internal layouts
+    // begin: btilde_c (box boundary values folded, zero under the patches), the two norms of A5, phi into the internal layouts
     AMR_TRY(a, cudaMemsetAsync(a->d_norm, 0, 4 * sizeof(unsigned long long), a->stream));
     rc = enqueue_fold_bc(hc, rhs_c, a->btc);
     if (rc != VMG_OK) return rc;
-    amr_mask_norm_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(a->A, a->btc, a->d_norm + 0);
-    norm_inf_kernel<<<std::min<unsigned>(grid_for(F0.n), 4u * hf->num_sms), kThreads, 0, a->stream>>>(rhs_f, F0.n, a->d_norm + 1);
-    AMR_TRY(a, cudaMemcpyAsync(a->rhsf, rhs_f, (size_t)F0.n * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
-    // rhs' of the coarse V-cycle = btilde_c except in and next to the patch (rewritten every cycle)
+    long long count = 2;
+    for (int q = 0; q < a->np(); ++q)
+        amr_mask_norm_kernel<<<grid_for(C0.n), kThreads, 0, a->stream>>>(a->A[q], a->btc, q == a->np() - 1 ? a->d_norm + 0 : nullptr);
+    count += a->np();
+    // rhs' of the coarse V-cycle = btilde_c except in and next to the patches (rewritten every cycle)
     AMR_TRY(a, cudaMemcpyAsync(C0.rhs, a->btc, (size_t)C0.nalloc * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
     to_internal_kernel<<<conv_grid(C0.n), kThreads, 0, a->stream>>>(C0.G, phi_c, C0.phi, nullptr);
-    to_internal_kernel<<<conv_grid(F0.n), kThreads, 0, a->stream>>>(F0.G, phi_f, F0.phi, nullptr);
-    amr_average_down_kernel<<<grid_for(a->A.S.n), kThreads, 0, a->stream>>>(a->A, F0.phi, C0.phi, a->old);
-    long long count = 6;
-    rc = amr_enqueue_ghost_fold(a, &count);
-    if (rc != VMG_OK) return rc;
+    for (int q = 0; q < a->np(); ++q) {
+        vmg_s* hf = a->hf[q];
+        VmgLevel& F0 = hf->lev[0];
+        norm_inf_kernel<<<std::min<unsigned>(grid_for(F0.n), 4u * hf->num_sms), kThreads, 0, a->stream>>>(rhs_f[q], F0.n, a->d_norm + 1);
+        AMR_TRY(a, cudaMemcpyAsync(a->rhsf[q], rhs_f[q], (size_t)F0.n * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
+        to_internal_kernel<<<conv_grid(F0.n), kThreads, 0, a->stream>>>(F0.G, phi_f[q], F0.phi, nullptr);
+        amr_average_down_kernel<<<grid_for(a->A[q].S.n), kThreads, 0, a->stream>>>(a->A[q], F0.phi, C0.phi, a->old[q]);
+        count += 3;
+    }
+    for (int q = 0; q < a->np(); ++q) {      // after every patch has averaged down (ghosts read uncovered cells only; kept in this order for clarity)
+        rc = amr_enqueue_ghost_fold(a, q, &count);
+        if (rc != VMG_OK) return rc;
+    }
     a->launches += count;
     AMR_TRY(a, cudaGetLastError());
     int status = VMG_MAXCYCLES, slow = 0;
@@ -316,7 +373,8 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, do
             if (std::isnan(a->h_norm[0]) || std::isnan(a->h_norm[1])) nb = a->h_norm[0] + a->h_norm[1];
             if (nb == 0.0) {                               // zero data: phi = 0
                 AMR_TRY(a, cudaMemsetAsync(phi_c, 0, (size_t)C0.n * sizeof(double), a->stream));
-                AMR_TRY(a, cudaMemsetAsync(phi_f, 0, (size_t)F0.n * sizeof(double), a->stream));
+                for (int q = 0; q < a->np(); ++q)
+                    AMR_TRY(a, cudaMemsetAsync(phi_f[q], 0, (size_t)a->hf[q]->lev[0].n * sizeof(double), a->stream));
                 AMR_TRY(a, cudaStreamSynchronize(a->stream));
                 a->hist.push_back(0.0);
                 return VMG_OK;
@@ -340,8 +398,11 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* rhs_f, do
     }
     if (status >= 0) {
         to_natural_kernel<<<conv_grid(C0.n), kThreads, 0, a->stream>>>(C0.G, C0.phi, phi_c);
-        to_natural_kernel<<<conv_grid(F0.n), kThreads, 0, a->stream>>>(F0.G, F0.phi, phi_f);
-        a->launches += 2;
+        for (int q = 0; q < a->np(); ++q) {
+            VmgLevel& F0 = a->hf[q]->lev[0];
+            to_natural_kernel<<<conv_grid(F0.n), kThreads, 0, a->stream>>>(F0.G, F0.phi, phi_f[q]);
+        }
+        a->launches += 1 + a->np();
         AMR_TRY(a, cudaGetLastError());
     }
     AMR_TRY(a, cudaStreamSynchronize(a->stream));

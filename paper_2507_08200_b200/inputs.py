@@ -326,17 +326,25 @@ class AmrProblem:
     rtol: float = 1e-12
     max_cycles: int = 50
 
+    # several patches: lo, hi are lists of triples and a_f, bx_f, by_f, bz_f, rhs_f lists with one entry per patch
+    @property
+    def multi(self) -> bool:
+        return isinstance(self.lo[0], (list, tuple))
+
     @property
     def fine_dims(self):
         c = self.coarse
         nd = 3 if c.nz > 1 else 2
-        return tuple(2 * (self.hi[d] - self.lo[d]) if d < nd else 1 for d in range(3))
+        one = lambda lo, hi: tuple(2 * (hi[d] - lo[d]) if d < nd else 1 for d in range(3))
+        return [one(l, u) for l, u in zip(self.lo, self.hi)] if self.multi else one(self.lo, self.hi)
 
     def coarse_coeffs(self):
         c = self.coarse
         return (c.a, c.bx, c.by, c.bz)
 
     def fine_coeffs(self):
+        if self.multi:
+            return [tuple(x) for x in zip(self.a_f, self.bx_f, self.by_f, self.bz_f)]
         return (self.a_f, self.bx_f, self.by_f, self.bz_f)
 
 
@@ -378,14 +386,23 @@ def amr_random_problem(nx: int, ny: int, nz: int, lo, hi, seed: int = 0, bc_type
         bx=np.exp(gb.evaluate(xf, yc, zc)), by=np.exp(gb.evaluate(xc, yf, zc)),
         bz=np.exp(gb.evaluate(xc, yc, zf)) if nz > 1 else None,
         bc_type=list(bc_type), bc_value=val, rhs=rng.standard_normal((nz, ny, nx)))
-    (cx, cy, cz), (fx, fy, fz) = _patch_axes(coarse, lo, hi)
-    m = tuple(len(v) for v in (cx, cy, cz))
-    return AmrProblem(
-        name=f"amr_random_{nx}x{ny}x{nz}_s{seed}", coarse=coarse, lo=tuple(lo), hi=tuple(hi),
-        a_f=a_scale * np.exp(ga.evaluate(cx, cy, cz)) if alpha > 0.0 else None,
-        bx_f=np.exp(gb.evaluate(fx, cy, cz)), by_f=np.exp(gb.evaluate(cx, fy, cz)),
-        bz_f=np.exp(gb.evaluate(cx, cy, fz)) if nz > 1 else None,
-        rhs_f=rng.standard_normal((m[2], m[1], m[0])))
+    def patch(lo_, hi_):
+        (cx, cy, cz), (fx, fy, fz) = _patch_axes(coarse, lo_, hi_)
+        m = tuple(len(v) for v in (cx, cy, cz))
+        return (a_scale * np.exp(ga.evaluate(cx, cy, cz)) if alpha > 0.0 else None,
+                np.exp(gb.evaluate(fx, cy, cz)), np.exp(gb.evaluate(cx, fy, cz)),
+                np.exp(gb.evaluate(cx, cy, fz)) if nz > 1 else None,
+                rng.standard_normal((m[2], m[1], m[0])))
+
+    if isinstance(lo[0], (list, tuple)):       # several patches: lists, one entry per patch
+        parts = [patch(l, u) for l, u in zip(lo, hi)]
+        cols = [list(c) for c in zip(*parts)]
+        return AmrProblem(name=f"amr_random_{nx}x{ny}x{nz}_s{seed}_{len(parts)}patches", coarse=coarse,
+                          lo=[tuple(l) for l in lo], hi=[tuple(u) for u in hi],
+                          a_f=cols[0], bx_f=cols[1], by_f=cols[2], bz_f=cols[3], rhs_f=cols[4])
+    a_f, bx_f, by_f, bz_f, rhs_f = patch(lo, hi)
+    return AmrProblem(name=f"amr_random_{nx}x{ny}x{nz}_s{seed}", coarse=coarse, lo=tuple(lo), hi=tuple(hi),
+                      a_f=a_f, bx_f=bx_f, by_f=by_f, bz_f=bz_f, rhs_f=rhs_f)
 
 
 def amr_streamer(ny: int = 128, seed: int = 1013, explicit_b: bool = True) -> AmrProblem:

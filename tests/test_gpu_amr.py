@@ -36,13 +36,18 @@ def _oracle(p):
     return o
 
 
+def _dev_fine(p, fine):
+    """fine coefficient tuple(s) of an AmrProblem -> tensors (a list of lists for several patches)"""
+    return [[dev(x) for x in f] for f in fine] if p.multi else [dev(x) for x in fine]
+
+
 def _gpu(p, **options):
     b = _binding()
     c = p.coarse
     s = b.VmgAmr(c.nx, c.ny, c.nz, c.dx, c.dy, c.dz, p.lo, p.hi)
     for k, v in options.items():
         s.set_option(k, v)
-    s.set_coeffs([dev(x) for x in p.coarse_coeffs()], [dev(x) for x in p.fine_coeffs()], c.alpha, c.beta)
+    s.set_coeffs([dev(x) for x in p.coarse_coeffs()], _dev_fine(p, p.fine_coeffs()), c.alpha, c.beta)
     s.set_bc(c.bc_type, [dev(v) for v in c.bc_value])
     return s
 
@@ -51,8 +56,13 @@ def _compare(p, s, o, phic0=None, phif0=None, rtol=1e-12, max_cycles=40, same_cy
     c = p.coarse
     pc_o, pf_o, st_o, cyc_o, rr_o, hist_o = o.solve(c.rhs, p.rhs_f, phic0, phif0, rtol=rtol, max_cycles=max_cycles)
     gc = dev(np.zeros_like(c.rhs) if phic0 is None else phic0)
-    gf = dev(np.zeros_like(p.rhs_f) if phif0 is None else phif0)
-    pc, pf, st, cyc, rr, hist = s.solve(dev(c.rhs), dev(p.rhs_f), gc, gf, rtol=rtol, max_cycles=max_cycles)
+    if p.multi:
+        gf = [dev(np.zeros_like(r) if phif0 is None else phif0[q]) for q, r in enumerate(p.rhs_f)]
+        rf = [dev(r) for r in p.rhs_f]
+    else:
+        gf = dev(np.zeros_like(p.rhs_f) if phif0 is None else phif0)
+        rf = dev(p.rhs_f)
+    pc, pf, st, cyc, rr, hist = s.solve(dev(c.rhs), rf, gc, gf, rtol=rtol, max_cycles=max_cycles)
     assert st == st_o, (st, st_o, hist, hist_o)
     if same_cycles:
         assert cyc == cyc_o, (cyc, cyc_o, hist, hist_o)
@@ -60,7 +70,8 @@ def _compare(p, s, o, phic0=None, phif0=None, rtol=1e-12, max_cycles=40, same_cy
     for i in range(n):       # 2e-15: the rounding floor of a residual formed from O(1) fields (the GPU runs the coarse V-cycle in place
         if hist_o[i] > 1e-10:    # on phi_c and differences the covered cells for the patch's correction; the oracle solves for the correction)
             assert abs(hist[i] - hist_o[i]) <= 1e-6 * hist_o[i] + 2e-15, (i, hist[i], hist_o[i])
-    assert rel(pf.cpu().numpy(), pf_o) <= PHI_TOL
+    for g, w in zip(pf if p.multi else [pf], pf_o if p.multi else [pf_o]):
+        assert rel(g.cpu().numpy(), w) <= PHI_TOL
     assert rel(pc.cpu().numpy(), pc_o) <= PHI_TOL          # covered cells included: means of the children on both sides
     return pc, pf, cyc, hist
 
@@ -94,9 +105,34 @@ def test_composite_solve_matches_the_oracle(case):
     c = q.coarse
     o.set_coeffs(q.coarse_coeffs(), q.fine_coeffs(), c.alpha, c.beta)
     o.set_bc(c.bc_type, c.bc_value)
-    s.set_coeffs([dev(x) for x in q.coarse_coeffs()], [dev(x) for x in q.fine_coeffs()], c.alpha, c.beta)
+    s.set_coeffs([dev(x) for x in q.coarse_coeffs()], _dev_fine(q, q.fine_coeffs()), c.alpha, c.beta)
     s.set_bc(c.bc_type, [dev(v) for v in c.bc_value])
     _compare(q, s, o)
+
+
+MULTI = [
+    dict(n=(48, 32, 16), lo=[(4, 4, 2), (28, 6, 4)], hi=[(20, 20, 10), (44, 26, 12)], alpha=1.0),                    # two patches
+    dict(n=(64, 48, 1), lo=[(4, 4, 0), (30, 6, 0), (8, 30, 0)], hi=[(24, 24, 1), (60, 26, 1), (56, 44, 1)], alpha=0.0),   # 2-D, three
+    dict(n=(32, 32, 32), lo=[(1, 1, 1), (19, 1, 1), (1, 19, 19)], hi=[(17, 17, 17), (31, 29, 17), (29, 31, 31)], alpha=0.0),  # two cells apart, next to the faces
+]
+
+
+@pytest.mark.parametrize("case", MULTI)
+def test_composite_solve_with_several_patches_matches_the_oracle(case):
+    n = case["n"]
+    p = inputs.amr_random_problem(*n, case["lo"], case["hi"], seed=sum(n) + 3, alpha=case["alpha"], sigma=0.7)
+    assert p.multi
+    o, s = _oracle(p), _gpu(p)
+    rng = np.random.default_rng(6)
+    phic0 = rng.standard_normal(p.coarse.rhs.shape)
+    phif0 = [rng.standard_normal(r.shape) for r in p.rhs_f]
+    pc, pf, cyc, hist = _compare(p, s, o, phic0, phif0)
+    assert hist[-1] <= 1e-12 and cyc <= 20 and s.pad_check() == 0
+    _compare(p, s, o)                                            # again from a zero guess on the same handles
+    s2 = _gpu(p, graph=0)                                        # plain launches: bitwise the graphs' result
+    pc0, pf0, *_ = s.solve(dev(p.coarse.rhs), [dev(r) for r in p.rhs_f], rtol=1e-12, max_cycles=40)
+    pc2, pf2, st2, cyc2, rr2, hist2 = s2.solve(dev(p.coarse.rhs), [dev(r) for r in p.rhs_f], rtol=1e-12, max_cycles=40)
+    assert torch.equal(pc0, pc2) and all(torch.equal(x, y) for x, y in zip(pf0, pf2))
 
 
 def test_plain_launches_fixed_cycle_counts_and_options():
@@ -135,6 +171,9 @@ def test_argument_and_state_errors():
     assert e.value.code == -2
     with pytest.raises(b.VmgError) as e:
         b.VmgAmr(16, 16, 16, 0.1, 0.1, 0.1, (4, 4, 4), (5, 12, 12))          # one coarse cell wide
+    assert e.value.code == -2
+    with pytest.raises(b.VmgError) as e:
+        b.VmgAmr(32, 16, 16, 0.1, 0.1, 0.1, [(2, 2, 2), (11, 2, 2)], [(10, 10, 10), (20, 10, 10)])   # one coarse cell apart
     assert e.value.code == -2
     s = b.VmgAmr(16, 16, 16, 0.1, 0.1, 0.1, (4, 4, 4), (12, 12, 12))
     with pytest.raises(b.VmgError) as e:
