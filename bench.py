@@ -330,27 +330,33 @@ def timestep_leg(binding, torch, p, d, d_bc, dev, s, flush, nsteps: int = 3, rto
 # ----------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ----------------------------------------------------------------------------------------------------
-def amr_leg(binding, torch, dev, flush, ny: int, steps: int = 5, with_oracle: bool = True):
+def amr_leg(binding, torch, dev, flush, ny: int, steps: int = 5, with_oracle: bool = True, patches: int = 1):
     """Two-level composite solve (second half): config 3 with the streamer head
     refined -- the 2 ny x ny x ny box plus a patch of ny x ny/2 x ny/2 fine cells -- through vmg_amr_*; explicit arrays of
-    ones on both levels as in the headline run.  Device-resident inputs, CUDA events on the solver's stream, L2 flushed
-    between solves.  The oracle (oracle/amr_oracle.c) is timed beside it on ONE solve."""
+    ones on both levels as in the headline run.  patches = 3: three heads side by side, a patch around each.  Device-resident
+    inputs, CUDA events on the solver's stream, L2 flushed between solves.  The oracle (oracle/amr_oracle.c) is timed beside
+    it on ONE solve."""
     from paper_2507_08200_b200 import inputs
-    p = inputs.amr_streamer(ny)
+    p = inputs.amr_streamer(ny) if patches == 1 else inputs.amr_streamers(ny)
     c = p.coarse
     up = lambda x: None if x is None else torch.from_numpy(np.ascontiguousarray(x)).to(dev)
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         s = binding.VmgAmr(c.nx, c.ny, c.nz, c.dx, c.dy, c.dz, p.lo, p.hi, stream=stream)
-        coarse, fine = [up(x) for x in p.coarse_coeffs()], [up(x) for x in p.fine_coeffs()]
+        coarse = [up(x) for x in p.coarse_coeffs()]
+        fine = [[up(x) for x in f] for f in p.fine_coeffs()] if p.multi else [up(x) for x in p.fine_coeffs()]
         bc = [up(v) for v in c.bc_value]
-        rhs_c, rhs_f = up(c.rhs), up(p.rhs_f)
-        phi_c, phi_f = torch.zeros_like(rhs_c), torch.zeros_like(rhs_f)
+        rhs_c = up(c.rhs)
+        rhs_f = [up(r) for r in p.rhs_f] if p.multi else up(p.rhs_f)
+        phi_c = torch.zeros_like(rhs_c)
+        phi_f = [torch.zeros_like(r) for r in rhs_f] if p.multi else torch.zeros_like(rhs_f)
         s.set_coeffs(coarse, fine, c.alpha, c.beta)
         s.set_bc(c.bc_type, bc)
         times, cyc, st, rr = [], 0, 0, 0.0
         for it in range(steps + 2):
-            phi_c.zero_(); phi_f.zero_()
+            phi_c.zero_()
+            for t in (phi_f if p.multi else [phi_f]):
+                t.zero_()
             flush.fill_(1.0)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(stream)
@@ -362,11 +368,13 @@ def amr_leg(binding, torch, dev, flush, ny: int, steps: int = 5, with_oracle: bo
                 times.append(e0.elapsed_time(e1) * 1e-3)
         launches = s.last_launch_count()
     stream.synchronize()
-    nf = int(np.prod(p.fine_dims))
-    out = {"workload": p.name, "coarse_cells": c.ncells, "fine_cells": nf, "solve_ms": float(np.mean(times)) * 1e3,
+    dims = p.fine_dims if p.multi else [p.fine_dims]
+    nf = int(sum(np.prod(d) for d in dims))
+    out = {"workload": p.name, "coarse_cells": c.ncells, "fine_cells": nf, "patches": len(dims),
+           "solve_ms": float(np.mean(times)) * 1e3,
            "solves_per_s": 1.0 / float(np.mean(times)), "cycles": cyc, "ms_per_cycle": float(np.mean(times)) * 1e3 / max(cyc, 1),
            "relres": rr, "launches_per_solve": int(launches), "nu_f": 6,
-           "cycle": "composite residual -> one V(3,3) cycle of the box -> correction -> 6 red-black sweeps on the patch"}
+           "cycle": "composite residual -> one V(3,3) cycle of the box -> correction -> 6 red-black sweeps on every patch"}
     if with_oracle:
         from oracle import AmrOracle
         o = AmrOracle(c.nx, c.ny, c.nz, c.dx, c.dy, c.dz, p.lo, p.hi)
@@ -375,8 +383,9 @@ def amr_leg(binding, torch, dev, flush, ny: int, steps: int = 5, with_oracle: bo
         t0 = time.perf_counter()
         r = o.solve(c.rhs, p.rhs_f, rtol=p.rtol, max_cycles=p.max_cycles)
         dt = time.perf_counter() - t0
-        err = max(float(np.abs(phi_f.cpu().numpy() - r[1]).max()), float(np.abs(phi_c.cpu().numpy() - r[0]).max())) / float(np.abs(r[0]).max())
-        out["oracle"] = {"solve_s": dt, "cycles": r[3], "cores": os.cpu_count(), "rel_linf_gpu_vs_oracle": err}
+        gf, of = (phi_f if p.multi else [phi_f]), (r[1] if p.multi else [r[1]])
+        err = max([float(np.abs(phi_c.cpu().numpy() - r[0]).max())] + [float(np.abs(g.cpu().numpy() - w).max()) for g, w in zip(gf, of)])
+        out["oracle"] = {"solve_s": dt, "cycles": r[3], "cores": os.cpu_count(), "rel_linf_gpu_vs_oracle": err / float(np.abs(r[0]).max())}
     s.destroy()
     return out
 
@@ -601,6 +610,7 @@ def run_vmg(args):
     amr = None
     if args.config == 3 and not args.no_amr and world == 1:
         amr = amr_leg(binding, torch, dev, flush, p.ny, with_oracle=not args.no_cpu_baseline)
+        amr["three_patches"] = amr_leg(binding, torch, dev, flush, p.ny, steps=3, with_oracle=not args.no_cpu_baseline, patches=3)
 
     # end to end through the C-ABI with host buffers
     etimes, ecycles, _ = timed(step_e2e, args.steps, max(1, min(args.warmup, 2)))
@@ -765,7 +775,9 @@ def main():
         torch.cuda.set_device(0)
         dev = torch.device("cuda", 0)
         flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)
-        print(json.dumps({"amr": amr_leg(binding, torch, dev, flush, 128, steps=args.steps, with_oracle=False)}))
+        out = amr_leg(binding, torch, dev, flush, 128, steps=args.steps, with_oracle=False)
+        out["three_patches"] = amr_leg(binding, torch, dev, flush, 128, steps=args.steps, with_oracle=False, patches=3)
+        print(json.dumps({"amr": out}))
     elif args.impl == "reference":
         run_reference(args)
     else:

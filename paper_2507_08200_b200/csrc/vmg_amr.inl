@@ -8,6 +8,12 @@ struct vmg_amr_s {
     std::vector<vmg_s*> hf;         // the patches (ordinary handles whose faces are coarse-fine faces)
     std::vector<AmrGeom> A;         // per patch: box, patch and shadow geometry
     cudaStream_t stream = nullptr;
+    // several patches: every patch handle runs on a stream of its own, forked from and joined to `stream` around each per-patch
+    // section (amr_fork / amr_join) -- inside the captured graphs the patches are parallel branches (their kernels are small
+    // and latency-bound: one patch of 128 x 64 x 64 cells fills the GPU once).  One patch: it shares `stream`.
+    std::vector<cudaStream_t> ps;
+    cudaEvent_t ev_fork = nullptr;
+    std::vector<cudaEvent_t> ev_join;
     void* base = nullptr;           // one allocation: btilde_c (padded like a level array), per patch rhs_f copy and shadow means, scalars
     double* btc = nullptr;
     std::vector<double*> rhsf, old;
@@ -40,6 +46,23 @@ struct vmg_amr_s {
 
 namespace {
 
+cudaStream_t amr_pstream(const vmg_amr_s* a, int q) { return a->ps.empty() ? a->stream : a->ps[q]; }
+
+void amr_fork(vmg_amr_s* a)
+{
+    if (a->ps.empty()) return;
+    cudaEventRecord(a->ev_fork, a->stream);
+    for (cudaStream_t s : a->ps) cudaStreamWaitEvent(s, a->ev_fork, 0);
+}
+
+void amr_join(vmg_amr_s* a)
+{
+    for (size_t q = 0; q < a->ps.size(); ++q) {
+        cudaEventRecord(a->ev_join[q], a->ps[q]);
+        cudaStreamWaitEvent(a->stream, a->ev_join[q], 0);
+    }
+}
+
 void amr_drop_graphs(vmg_amr_s* a)
 {
     for (int i = 0; i < 3; ++i) {
@@ -59,7 +82,7 @@ int amr_enqueue_ghost_fold(vmg_amr_s* a, int q, long long* count)
         g.plane[f] = hf->bcval[f];
         if (f < 2 * g.A.nd) most = std::max<long long>(most, (long long)plane_count(hf->lev[0], f));
     }
-    amr_ghost_kernel<<<dim3(grid_for(most), 2 * g.A.nd), kThreads, 0, a->stream>>>(g);
+    amr_ghost_kernel<<<dim3(grid_for(most), 2 * g.A.nd), kThreads, 0, amr_pstream(a, q)>>>(g);
     ++*count;
     long long before = hf->launches;
     int rc = enqueue_fold_bc(hf, a->rhsf[q], hf->lev[0].rhs);
@@ -73,15 +96,13 @@ void amr_enqueue_residual(vmg_amr_s* a, long long* count, bool red_only)
 {
     vmg_s* hc = a->hc;
     cudaMemsetAsync(a->d_norm + 2, 0, 2 * sizeof(unsigned long long), a->stream);
+    amr_fork(a);
     for (int q = 0; q < a->np(); ++q) {
         vmg_s* hf = a->hf[q];
         hf->lev[0].cur = 0;
         plain_residual_restrict(hf, 0, count);
         enqueue_residual_norm(hf, a->d_norm + 3);
         ++*count;
-    }
-    for (int q = 0; q < a->np(); ++q) {
-        vmg_s* hf = a->hf[q];
         AmrResArgs g;
         g.A = a->A[q]; g.Lc = view(hc->lev[0]);
         g.phic = hc->lev[0].phi; g.btc = a->btc; g.rs = hf->lev[1].rhs; g.phif = hf->lev[0].phi;
@@ -91,9 +112,10 @@ void amr_enqueue_residual(vmg_amr_s* a, long long* count, bool red_only)
         g.norm = a->d_norm + 2;
         long long region = 1;
         for (int d = 0; d < g.A.nd; ++d) region *= g.A.hi[d] - g.A.lo[d] + 2;
-        amr_patch_rhs_kernel<<<grid_for(region), kThreads, 0, a->stream>>>(g);
+        amr_patch_rhs_kernel<<<grid_for(region), kThreads, 0, amr_pstream(a, q)>>>(g);
         ++*count;
     }
+    amr_join(a);
     hc->lev[0].cur = 0;
     enqueue_residual_norm(hc, a->d_norm + 2, red_only);
     ++*count;
@@ -106,19 +128,23 @@ int amr_enqueue_correction(vmg_amr_s* a, long long* count)
     vmg_s* hc = a->hc;
     VmgLevel& C0 = hc->lev[0];
     enqueue_vcycle(hc, nullptr, count);
+    amr_fork(a);
+    int rc_all = VMG_OK;
     for (int q = 0; q < a->np(); ++q) {
         vmg_s* hf = a->hf[q];
         const AmrGeom& A = a->A[q];
-        amr_prolong_add_kernel<<<grid_for(A.F.n), kThreads, 0, a->stream>>>(A, hf->lev[0].phi, C0.phi, a->old[q]);
+        cudaStream_t sq = amr_pstream(a, q);
+        amr_prolong_add_kernel<<<grid_for(A.F.n), kThreads, 0, sq>>>(A, hf->lev[0].phi, C0.phi, a->old[q]);
         ++*count;
         int rc = amr_enqueue_ghost_fold(a, q, count);
-        if (rc != VMG_OK) return rc;
+        if (rc != VMG_OK) rc_all = rc;           // keep going: the forked streams have to be joined before a capture can end
         hf->lev[0].cur = 0; hf->lev[0].dir = 0;
         plain_smooth(hf, 0, a->nu_f, count);
-        amr_average_down_kernel<<<grid_for(A.S.n), kThreads, 0, a->stream>>>(A, hf->lev[0].phi, C0.phi, a->old[q]);
+        amr_average_down_kernel<<<grid_for(A.S.n), kThreads, 0, sq>>>(A, hf->lev[0].phi, C0.phi, a->old[q]);
         ++*count;
     }
-    return VMG_OK;
+    amr_join(a);
+    return rc_all;
 }
 
 bool amr_graphs_current(const vmg_amr_s* a)
@@ -174,6 +200,9 @@ int vmg_amr_destroy(vmg_amr_handle a)
     amr_drop_graphs(a);
     for (vmg_s* h : a->hf) if (h) vmg_destroy(h);   // the patches first: the coarse handle may own the stream
     if (a->hc) vmg_destroy(a->hc);
+    for (cudaStream_t s : a->ps) cudaStreamDestroy(s);
+    for (cudaEvent_t e : a->ev_join) cudaEventDestroy(e);
+    if (a->ev_fork) cudaEventDestroy(a->ev_fork);
     if (a->base) cudaFree(a->base);
     if (a->h_norm) cudaFreeHost(a->h_norm);
     (void)cudaGetLastError();
@@ -209,7 +238,18 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
         int m[3] = {1, 1, 1};
         for (int d = 0; d < nd; ++d) m[d] = 2 * (hi[3 * q + d] - lo[3 * q + d]);
         vmg_s* hf = nullptr;
-        rc = vmg_create(&hf, m[0], m[1], m[2], 0.5 * dx, 0.5 * dy, nd == 3 ? 0.5 * dz : dz, (void*)a->stream);
+        cudaStream_t sq = a->stream;
+        if (npatch > 1) {
+            cudaEvent_t ev = nullptr;
+            if (cudaStreamCreateWithFlags(&sq, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) {
+                (void)cudaGetLastError();
+                vmg_amr_destroy(a);
+                return VMG_ERR_CUDA;
+            }
+            a->ps.push_back(sq); a->ev_join.push_back(ev);
+        }
+        rc = vmg_create(&hf, m[0], m[1], m[2], 0.5 * dx, 0.5 * dy, nd == 3 ? 0.5 * dz : dz, (void*)sq);
         if (rc == VMG_OK) a->hf.push_back(hf);
         if (rc == VMG_OK && hf->nlev < 2) rc = VMG_ERR_SIZE;
         if (rc != VMG_OK) { vmg_amr_destroy(a); return rc; }
@@ -221,6 +261,11 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
         total += round_up((size_t)hf->lev[0].n, 32) + round_up((size_t)hf->lev[1].n, 32);
     }
     a->epoch_f.assign((size_t)npatch, 0u);
+    if (npatch > 1 && cudaEventCreateWithFlags(&a->ev_fork, cudaEventDisableTiming) != cudaSuccess) {
+        (void)cudaGetLastError();
+        vmg_amr_destroy(a);
+        return VMG_ERR_CUDA;
+    }
     if (cudaMalloc(&a->base, total * sizeof(double)) != cudaSuccess ||
         cudaMallocHost((void**)&a->h_norm, 4 * sizeof(double)) != cudaSuccess ||
         cudaMemsetAsync(a->base, 0, total * sizeof(double), a->stream) != cudaSuccess ||
@@ -267,7 +312,7 @@ int vmg_amr_set_coeffs(vmg_amr_handle a, const double* a_c, const double* bx_c, 
         VmgLevel& F0 = hf->lev[0];
         for (int f = 0; f < 2 * a->A[q].nd; ++f) {
             const long long npl = (long long)plane_count(F0, f);
-            amr_scale_kernel<<<grid_for(npl), kThreads, 0, a->stream>>>(F0.wb[f], npl, 1.0 / 3.0);
+            amr_scale_kernel<<<grid_for(npl), kThreads, 0, hf->stream>>>(F0.wb[f], npl, 1.0 / 3.0);
         }
         hf->dinv_dirty = true;
     }
@@ -344,19 +389,21 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* const* rh
     // rhs' of the coarse V-cycle = btilde_c except in and next to the patches (rewritten every cycle)
     AMR_TRY(a, cudaMemcpyAsync(C0.rhs, a->btc, (size_t)C0.nalloc * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
     to_internal_kernel<<<conv_grid(C0.n), kThreads, 0, a->stream>>>(C0.G, phi_c, C0.phi, nullptr);
-    for (int q = 0; q < a->np(); ++q) {
+    amr_fork(a);
+    for (int q = 0; q < a->np(); ++q) {      // per patch, on its stream (ghosts read uncovered coarse cells only)
         vmg_s* hf = a->hf[q];
         VmgLevel& F0 = hf->lev[0];
-        norm_inf_kernel<<<std::min<unsigned>(grid_for(F0.n), 4u * hf->num_sms), kThreads, 0, a->stream>>>(rhs_f[q], F0.n, a->d_norm + 1);
-        AMR_TRY(a, cudaMemcpyAsync(a->rhsf[q], rhs_f[q], (size_t)F0.n * sizeof(double), cudaMemcpyDeviceToDevice, a->stream));
-        to_internal_kernel<<<conv_grid(F0.n), kThreads, 0, a->stream>>>(F0.G, phi_f[q], F0.phi, nullptr);
-        amr_average_down_kernel<<<grid_for(a->A[q].S.n), kThreads, 0, a->stream>>>(a->A[q], F0.phi, C0.phi, a->old[q]);
+        cudaStream_t sq = amr_pstream(a, q);
+        norm_inf_kernel<<<std::min<unsigned>(grid_for(F0.n), 4u * hf->num_sms), kThreads, 0, sq>>>(rhs_f[q], F0.n, a->d_norm + 1);
+        cudaMemcpyAsync(a->rhsf[q], rhs_f[q], (size_t)F0.n * sizeof(double), cudaMemcpyDeviceToDevice, sq);
+        to_internal_kernel<<<conv_grid(F0.n), kThreads, 0, sq>>>(F0.G, phi_f[q], F0.phi, nullptr);
+        amr_average_down_kernel<<<grid_for(a->A[q].S.n), kThreads, 0, sq>>>(a->A[q], F0.phi, C0.phi, a->old[q]);
         count += 3;
+        int r1 = amr_enqueue_ghost_fold(a, q, &count);
+        if (r1 != VMG_OK) rc = r1;
     }
-    for (int q = 0; q < a->np(); ++q) {      // after every patch has averaged down (ghosts read uncovered cells only; kept in this order for clarity)
-        rc = amr_enqueue_ghost_fold(a, q, &count);
-        if (rc != VMG_OK) return rc;
-    }
+    amr_join(a);
+    if (rc != VMG_OK) return rc;
     a->launches += count;
     AMR_TRY(a, cudaGetLastError());
     int status = VMG_MAXCYCLES, slow = 0;
@@ -373,7 +420,7 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* const* rh
             if (std::isnan(a->h_norm[0]) || std::isnan(a->h_norm[1])) nb = a->h_norm[0] + a->h_norm[1];
             if (nb == 0.0) {                               // zero data: phi = 0
                 AMR_TRY(a, cudaMemsetAsync(phi_c, 0, (size_t)C0.n * sizeof(double), a->stream));
-                for (int q = 0; q < a->np(); ++q)
+                for (int q = 0; q < a->np(); ++q)          // (on the main stream: nothing is in flight on the patch streams)
                     AMR_TRY(a, cudaMemsetAsync(phi_f[q], 0, (size_t)a->hf[q]->lev[0].n * sizeof(double), a->stream));
                 AMR_TRY(a, cudaStreamSynchronize(a->stream));
                 a->hist.push_back(0.0);
@@ -398,10 +445,12 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* const* rh
     }
     if (status >= 0) {
         to_natural_kernel<<<conv_grid(C0.n), kThreads, 0, a->stream>>>(C0.G, C0.phi, phi_c);
+        amr_fork(a);
         for (int q = 0; q < a->np(); ++q) {
             VmgLevel& F0 = a->hf[q]->lev[0];
-            to_natural_kernel<<<conv_grid(F0.n), kThreads, 0, a->stream>>>(F0.G, F0.phi, phi_f[q]);
+            to_natural_kernel<<<conv_grid(F0.n), kThreads, 0, amr_pstream(a, q)>>>(F0.G, F0.phi, phi_f[q]);
         }
+        amr_join(a);
         a->launches += 1 + a->np();
         AMR_TRY(a, cudaGetLastError());
     }

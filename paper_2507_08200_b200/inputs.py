@@ -437,3 +437,37 @@ def amr_streamer(ny: int = 128, seed: int = 1013, explicit_b: bool = True) -> Am
         name=f"amr_streamer_{nx}x{ny}x{nz}_patch{m[0]}x{m[1]}x{m[2]}", coarse=base, lo=lo, hi=hi, a_f=None,
         bx_f=ones((m[2], m[1], m[0] + 1)), by_f=ones((m[2], m[1] + 1, m[0])), bz_f=ones((m[2] + 1, m[1], m[0])),
         rhs_f=rhs_f)
+
+
+def amr_streamers(ny: int = 128, seed: int = 1014) -> AmrProblem:
+    """Three streamer heads side by side (the paper's 3-D case has fourteen): config 3's box and boundary data,
+    the space charge of config 3 repeated at y = 3/16, 1/2, 13/16 and a patch of ny/2 x ny/4 x ny/4 coarse cells around every
+    head (64 x 32 x 32 at ny = 128 -> 128 x 64 x 64 fine cells each), eight coarse cells apart in y."""
+    base = config3(ny)
+    yh = (3.0 / 16.0, 0.5, 13.0 / 16.0)
+    los = [(15 * ny // 16, int(round(y * ny)) - ny // 8, 3 * ny // 8) for y in yh]
+    his = [(23 * ny // 16, int(round(y * ny)) + ny // 8, 5 * ny // 8) for y in yh]
+    R, xh, zh = 0.05, 1.2, 0.5
+    rng = np.random.Generator(np.random.PCG64(seed))
+
+    def charge(xs, ys, zs):
+        out = -0.01 * rng.random((len(zs), len(ys), len(xs)))
+        for y0 in yh:
+            r2 = ((xs - xh) ** 2)[None, None, :] + ((ys - y0) ** 2)[None, :, None] + ((zs - zh) ** 2)[:, None, None]
+            rho2 = ((ys - y0) ** 2)[None, :, None] + ((zs - zh) ** 2)[:, None, None]
+            out += 0.8 * np.exp(-rho2 / R ** 2) * (0.5 * (1.0 + np.tanh((xh - xs) / R)))[None, None, :] - np.exp(-r2 / R ** 2)
+        return out
+
+    nx, nz = base.nx, base.nz
+    raw_c = charge(_centres(nx, base.dx), _centres(ny, base.dy), _centres(nz, base.dz))
+    scale = np.abs(raw_c).max()
+    base.rhs = np.ascontiguousarray(raw_c / scale)
+    base.a = None
+    rhs_f, bxs, bys, bzs = [], [], [], []
+    for lo, hi in zip(los, his):
+        (cx, cy, cz), _ = _patch_axes(base, lo, hi)
+        rhs_f.append(np.ascontiguousarray(charge(cx, cy, cz) / scale))
+        m = (len(cx), len(cy), len(cz))
+        bxs.append(np.ones((m[2], m[1], m[0] + 1))); bys.append(np.ones((m[2], m[1] + 1, m[0]))); bzs.append(np.ones((m[2] + 1, m[1], m[0])))
+    return AmrProblem(name=f"amr_streamers_{nx}x{ny}x{nz}_3patches", coarse=base, lo=los, hi=his,
+                      a_f=[None] * 3, bx_f=bxs, by_f=bys, bz_f=bzs, rhs_f=rhs_f)
