@@ -285,7 +285,8 @@ int vmg_norm_inf_static(const double* v, long long n, double* out, void* cuda_st
  * under the patch define the operator of the correction V-cycle there (keep them consistent with the fine ones, e.g.
  * their averages); a_c and a_f are both given or both NULL.  rhs_c under the patch is ignored; phi_c, phi_f: initial guess
  * in, solution out (phi_c under the patch: means of the children).  vmg_set_bc semantics for the box faces.
- * Stream: as vmg_create (NULL: the library creates one); both levels run on it.  vmg_amr_solve synchronises it.
+ * Stream: as vmg_create (NULL: the library creates one).  With one patch both levels run on it; with several, every patch runs
+ * on an internal stream forked from and joined to it around each per-patch section.  vmg_amr_solve synchronises it.
  * Options: "nu_f" (1..64); every other key goes to the coarse handle (vmg_set_option).  No mask, no PCG on composite grids. */
 typedef struct vmg_amr_s* vmg_amr_handle;
 /* npatch >= 1 patches; lo, hi: npatch triples of coarse cell indices, flattened (lo[3 q + d]); HOST arrays */
