@@ -1,6 +1,6 @@
 // vmg_amr.cuh -- kernels of the two-level composite solve (vmg_amr_* in include/vmg.h, second half;
 // PAPER.md:157-159 "composite multilevel multigrid solver", non-subcycled AMR levels).  Readings A1-A5 of DESIGN.md:
-// refinement ratio 2, one box patch away from the boundary; across a coarse-fine face a two-point flux over 1.5 hf
+// refinement ratio 2, one or several separated box patches away from the boundary; across a coarse-fine face a two-point flux over 1.5 hf
 // between the fine cell and the coarse field interpolated linearly in the tangential directions; the coarse cell takes
 // the sum of the fine fluxes.
 //
