@@ -330,7 +330,7 @@ def timestep_leg(binding, torch, p, d, d_bc, dev, s, flush, nsteps: int = 3, rto
 # ----------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ----------------------------------------------------------------------------------------------------
-def amr_leg(binding, torch, dev, flush, ny: int, steps: int = 5, with_oracle: bool = True, patches: int = 1):
+def amr_leg(binding, torch, dev, flush, ny: int, steps: int = 5, with_oracle: bool = True, patches: int = 1, opts=()):
     """Two-level composite solve (second half): config 3 with the streamer head
     refined -- the 2 ny x ny x ny box plus a patch of ny x ny/2 x ny/2 fine cells -- through vmg_amr_*; explicit arrays of
     ones on both levels as in the headline run.  patches = 3: three heads side by side, a patch around each.  Device-resident
@@ -343,6 +343,9 @@ def amr_leg(binding, torch, dev, flush, ny: int, steps: int = 5, with_oracle: bo
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         s = binding.VmgAmr(c.nx, c.ny, c.nz, c.dx, c.dy, c.dz, p.lo, p.hi, stream=stream)
+        for kv in opts:
+            key, val = kv.split("=")
+            s.set_option(key, float(val))
         coarse = [up(x) for x in p.coarse_coeffs()]
         fine = [[up(x) for x in f] for f in p.fine_coeffs()] if p.multi else [up(x) for x in p.fine_coeffs()]
         bc = [up(v) for v in c.bc_value]
@@ -775,8 +778,8 @@ def main():
         torch.cuda.set_device(0)
         dev = torch.device("cuda", 0)
         flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)
-        out = amr_leg(binding, torch, dev, flush, 128, steps=args.steps, with_oracle=False)
-        out["three_patches"] = amr_leg(binding, torch, dev, flush, 128, steps=args.steps, with_oracle=False, patches=3)
+        out = amr_leg(binding, torch, dev, flush, 128, steps=args.steps, with_oracle=False, opts=args.opt)
+        out["three_patches"] = amr_leg(binding, torch, dev, flush, 128, steps=args.steps, with_oracle=False, patches=3, opts=args.opt)
         print(json.dumps({"amr": out}))
     elif args.impl == "reference":
         run_reference(args)

@@ -24,6 +24,12 @@ struct vmg_amr_s {
     cudaGraph_t graph[3] = {nullptr, nullptr, nullptr};   // 0: composite residual + norms (every cell), 1: correction + fine sweeps,
     cudaGraphExec_t exec[3] = {nullptr, nullptr, nullptr};   // 2: as 0 with the coarse norm over the red cells (after a V-cycle, R12)
     long long graph_launches[3] = {0, 0, 0};
+    // the cycle loop as ONE graph with a conditional WHILE node (as vmg_solve): body = correction + composite
+    // residual + solve_decide_kernel; used when the coarse handle's options allow it (device_loop, graph, no profile)
+    cudaGraph_t loop_graph = nullptr;
+    cudaGraphExec_t loop_exec = nullptr;
+    long long loop_launches = 0;
+    double *d_loop = nullptr, *h_loop = nullptr;   // nb, rtol, max, cycles, slow, status, -, -, hist[kLoopMaxCycles + 1] (device / pinned)
     unsigned epoch_c = 0;
     std::vector<unsigned> epoch_f;
     int graph_nu_f = -1;
@@ -69,6 +75,8 @@ void amr_drop_graphs(vmg_amr_s* a)
         if (a->exec[i]) { cudaGraphExecDestroy(a->exec[i]); a->exec[i] = nullptr; }
         if (a->graph[i]) { cudaGraphDestroy(a->graph[i]); a->graph[i] = nullptr; }
     }
+    if (a->loop_exec) { cudaGraphExecDestroy(a->loop_exec); a->loop_exec = nullptr; }
+    if (a->loop_graph) { cudaGraphDestroy(a->loop_graph); a->loop_graph = nullptr; }
 }
 
 // value planes of patch q from the coarse field, then btilde_f = f_f + 2 wb g (the library's fold_bc)
@@ -95,13 +103,13 @@ int amr_enqueue_ghost_fold(vmg_amr_s* a, int q, long long* count)
 void amr_enqueue_residual(vmg_amr_s* a, long long* count, bool red_only)
 {
     vmg_s* hc = a->hc;
-    cudaMemsetAsync(a->d_norm + 2, 0, 2 * sizeof(unsigned long long), a->stream);
+    cudaMemsetAsync(a->d_norm + 2, 0, sizeof(unsigned long long), a->stream);   // the maximum of A5 over both levels: one scalar
     amr_fork(a);
     for (int q = 0; q < a->np(); ++q) {
         vmg_s* hf = a->hf[q];
         hf->lev[0].cur = 0;
         plain_residual_restrict(hf, 0, count);
-        enqueue_residual_norm(hf, a->d_norm + 3);
+        enqueue_residual_norm(hf, a->d_norm + 2);
         ++*count;
         AmrResArgs g;
         g.A = a->A[q]; g.Lc = view(hc->lev[0]);
@@ -184,8 +192,49 @@ int amr_run(vmg_amr_s* a, int which)
         a->epoch_c = hc->graph_epoch; a->graph_nu_f = a->nu_f;
         for (int q = 0; q < a->np(); ++q) a->epoch_f[q] = a->hf[q]->graph_epoch;
     }
+    if (which < 0) return VMG_OK;            // only (re)capture
     AMR_TRY(a, cudaGraphLaunch(a->exec[which], a->stream));
     a->launches += a->graph_launches[which];
+    return VMG_OK;
+}
+
+// The cycles after the first residual as one graph launch: WHILE (continue) { correction; composite residual (coarse norm over
+// the red cells); solve_decide_kernel: history, exit rules C5, sets `continue` }.  The caller has filled h_loop[0..8] and hist[0].
+int amr_run_loop(vmg_amr_s* a)
+{
+    if (!a->loop_exec || !amr_graphs_current(a)) {
+        if (a->loop_exec) { cudaGraphExecDestroy(a->loop_exec); a->loop_exec = nullptr; }
+        if (a->loop_graph) { cudaGraphDestroy(a->loop_graph); a->loop_graph = nullptr; }
+        cudaGraph_t g = nullptr, dummy = nullptr;
+        AMR_TRY(a, cudaGraphCreate(&g, 0));
+        a->loop_graph = g;
+        cudaGraphConditionalHandle handle;
+        AMR_TRY(a, cudaGraphConditionalHandleCreate(&handle, g, 1, cudaGraphCondAssignDefault));
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = handle;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        cudaGraphNode_t wnode;
+        AMR_TRY(a, cudaGraphAddNode(&wnode, g, nullptr, 0, &np));
+        cudaGraph_t body = np.conditional.phGraph_out[0];
+        long long count = 0;
+        AMR_TRY(a, cudaStreamBeginCaptureToGraph(a->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+        int rc = amr_enqueue_correction(a, &count);
+        amr_enqueue_residual(a, &count, true);
+        solve_decide_kernel<<<1, 32, 0, a->stream>>>(handle, a->d_loop, a->d_norm + 2);
+        ++count;
+        cudaError_t e = cudaStreamEndCapture(a->stream, &dummy);
+        if (rc != VMG_OK) return rc;
+        AMR_TRY(a, e);
+        AMR_TRY(a, cudaGraphInstantiate(&a->loop_exec, g, 0));
+        a->loop_launches = count;
+    }
+    const int max = (int)a->h_loop[2];
+    AMR_TRY(a, cudaMemcpyAsync(a->d_loop, a->h_loop, 9 * sizeof(double), cudaMemcpyHostToDevice, a->stream));
+    AMR_TRY(a, cudaGraphLaunch(a->loop_exec, a->stream));
+    AMR_TRY(a, cudaMemcpyAsync(a->h_loop, a->d_loop, (size_t)(8 + max + 1) * sizeof(double), cudaMemcpyDeviceToHost, a->stream));
+    AMR_TRY(a, cudaStreamSynchronize(a->stream));
     return VMG_OK;
 }
 
@@ -205,6 +254,7 @@ int vmg_amr_destroy(vmg_amr_handle a)
     if (a->ev_fork) cudaEventDestroy(a->ev_fork);
     if (a->base) cudaFree(a->base);
     if (a->h_norm) cudaFreeHost(a->h_norm);
+    if (a->h_loop) cudaFreeHost(a->h_loop);
     (void)cudaGetLastError();
     delete a;
     return VMG_OK;
@@ -233,7 +283,7 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
     a->stream = a->hc->stream;
     const VmgLevel& C0 = a->hc->lev[0];
     const size_t arr = (size_t)C0.nalloc + 2 * (size_t)C0.pad;
-    size_t total = round_up(arr, 32) + 32;
+    size_t total = round_up(arr, 32) + 32 + round_up(8 + kLoopMaxCycles + 1, 32);
     for (int q = 0; q < npatch; ++q) {
         int m[3] = {1, 1, 1};
         for (int d = 0; d < nd; ++d) m[d] = 2 * (hi[3 * q + d] - lo[3 * q + d]);
@@ -268,6 +318,7 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
     }
     if (cudaMalloc(&a->base, total * sizeof(double)) != cudaSuccess ||
         cudaMallocHost((void**)&a->h_norm, 4 * sizeof(double)) != cudaSuccess ||
+        cudaMallocHost((void**)&a->h_loop, (8 + kLoopMaxCycles + 1) * sizeof(double)) != cudaSuccess ||
         cudaMemsetAsync(a->base, 0, total * sizeof(double), a->stream) != cudaSuccess ||
         cudaStreamSynchronize(a->stream) != cudaSuccess) {
         (void)cudaGetLastError();
@@ -282,6 +333,7 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
         a->old.push_back(p);  p += round_up((size_t)a->hf[q]->lev[1].n, 32);
     }
     a->d_norm = (unsigned long long*)p;
+    a->d_loop = p + 8;
     *out = a;
     return VMG_OK;
 }
@@ -427,8 +479,7 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* const* rh
                 return VMG_OK;
             }
         }
-        const double rcn = a->h_norm[2], rfn = a->h_norm[3];
-        a->relres = (std::isnan(rcn) || std::isnan(rfn)) ? rcn + rfn : std::max(rcn, rfn) / nb;
+        a->relres = a->h_norm[2] / nb;
         a->hist.push_back(a->relres);
         a->cycles = c;
         if (std::isnan(a->relres) || std::isinf(a->relres)) { status = VMG_ERR_DIVERGED; break; }
@@ -440,6 +491,21 @@ int vmg_amr_solve(vmg_amr_handle a, const double* rhs_c, const double* const* rh
             }
         }
         if (c == max_cycles) { status = VMG_MAXCYCLES; break; }
+        if (c == 0 && red_ok && hc->use_loop && hc->use_graph && !hc->profile && max_cycles <= kLoopMaxCycles) {
+            // the remaining cycles in one graph launch with the exit rules on the device
+            if (!amr_graphs_current(a)) { rc = amr_run(a, -1); if (rc != VMG_OK) return rc; }   // (re)capture the three plain graphs first: they carry the epochs
+            double* st = a->h_loop;
+            st[0] = nb; st[1] = rtol; st[2] = (double)max_cycles; st[3] = 0.0; st[4] = 0.0; st[5] = (double)VMG_MAXCYCLES;
+            st[6] = st[7] = 0.0; st[8] = a->relres;
+            rc = amr_run_loop(a);
+            if (rc != VMG_OK) return rc;
+            const int done = (int)st[3];
+            for (int i = 1; i <= done; ++i) a->hist.push_back(st[8 + i]);
+            a->cycles = done; a->relres = a->hist.back();
+            a->launches += (long long)done * a->loop_launches;
+            status = (int)st[5];
+            break;
+        }
         rc = amr_run(a, 1);
         if (rc != VMG_OK) return rc;
     }

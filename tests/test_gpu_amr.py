@@ -147,6 +147,15 @@ def test_plain_launches_fixed_cycle_counts_and_options():
     pc2, pf2, st2, cyc2, rr2, hist2 = s2.solve(dev(p.coarse.rhs), dev(p.rhs_f), rtol=1e-12, max_cycles=40)
     assert cyc2 == cyc and hist2 == hist
     assert torch.equal(pc2, pc) and torch.equal(pf2, pf)
+    # device_loop = 0: one graph replay and one read-back per cycle instead of the conditional-WHILE graph: bitwise the same
+    s3 = _gpu(p, device_loop=0)
+    pc3, pf3, st3, cyc3, rr3, hist3 = s3.solve(dev(p.coarse.rhs), dev(p.rhs_f), rtol=1e-12, max_cycles=40)
+    assert cyc3 == cyc and hist3 == hist and torch.equal(pc3, pc) and torch.equal(pf3, pf)
+    # every exit rule through the device-side loop against the host loop: MAXCYCLES short of convergence, unreachable rtol -> STALLED
+    for rtol, maxc in ((1e-12, 3), (1e-17, 40), (1e-3, 40)):
+        g = s.solve(dev(p.coarse.rhs), dev(p.rhs_f), rtol=rtol, max_cycles=maxc)
+        w = s3.solve(dev(p.coarse.rhs), dev(p.rhs_f), rtol=rtol, max_cycles=maxc)
+        assert g[2] == w[2] and g[3] == w[3] and g[5] == w[5] and torch.equal(g[0], w[0]) and torch.equal(g[1], w[1]), (rtol, maxc, g[2:4], w[2:4])
     # rtol = 0: exactly max_cycles cycles, status MAXCYCLES, history of max_cycles + 1 entries
     o5 = o.solve(p.coarse.rhs, p.rhs_f, rtol=0.0, max_cycles=5)
     g5 = s.solve(dev(p.coarse.rhs), dev(p.rhs_f), rtol=0.0, max_cycles=5)
