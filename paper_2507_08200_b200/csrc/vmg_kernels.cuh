@@ -782,7 +782,7 @@ __global__ void residual_restrict_kernel(LevelView L, Geom CG, const double* __r
 // the red children only (restrict_one<CW, 1>).  Latency-bound (ncu: long-scoreboard stalls, 61 % of the warp slots at 34
 // registers): with array weights the kernel is held to 32 registers so that 8 CTAs fit an SM.
 template <int CW>
-__global__ void __launch_bounds__(kThreads, CW == 0 ? 8 : 1)
+__global__ void __launch_bounds__(kThreads, CW == 0 ? 8 : 5)
 residual_restrict_red_kernel(LevelView L, Geom CG, const double* __restrict__ phi, const double* __restrict__ rhs,
                              double* __restrict__ crhs, double* __restrict__ cphi, int sz, int reverse,
                              const double* __restrict__ cdinv = nullptr)
