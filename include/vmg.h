@@ -269,8 +269,7 @@ int vmg_norm_inf_static(const double* v, long long n, double* out, void* cuda_st
  * oracle/amr_oracle.c, which this is tested against):
  *   A1  box patches of coarse cells [lo, hi) refined by 2, each at least one coarse cell away from the box boundary and at
  *       least two coarse cells wide in every active direction, two patches at least two coarse cells apart in some
- *       direction; a patch as a box of 2 (hi - lo) fine cells must itself be a legal vmg grid with at least two levels
- *       (else VMG_ERR_SIZE);
+ *       direction (else VMG_ERR_SIZE); the box itself must be a legal vmg grid, a patch may have any such size;
  *   A2  coarse-fine face: flux b_f (g - phi_f) / (1.5 hf) per unit area, g = the coarse field at the point of the adjacent
  *       coarse cell opposite the fine cell centre, interpolated linearly in the tangential directions;
  *   A3  the coarse cell takes the sum of the fine fluxes through its face (conservation);

@@ -299,7 +299,8 @@ int vmg_amr_create(vmg_amr_handle* out, int nx, int ny, int nz, double dx, doubl
             }
             a->ps.push_back(sq); a->ev_join.push_back(ev);
         }
-        rc = vmg_create(&hf, m[0], m[1], m[2], 0.5 * dx, 0.5 * dy, nd == 3 ? 0.5 * dz : dz, (void*)sq);
+        // two levels only (the patch itself and its shadow): any even patch size is legal, whatever its coarser grids would be
+        rc = create_impl(&hf, m[0], m[1], m[2], 0.5 * dx, 0.5 * dy, nd == 3 ? 0.5 * dz : dz, (void*)sq, nullptr, 0, nullptr, 2);
         if (rc == VMG_OK) a->hf.push_back(hf);
         if (rc == VMG_OK && hf->nlev < 2) rc = VMG_ERR_SIZE;
         if (rc != VMG_OK) { vmg_amr_destroy(a); return rc; }

@@ -173,8 +173,10 @@ namespace {
 
 // slice: nullptr = allocate an arena of this handle's own; otherwise the handle lives in [slice, slice + slice_bytes)
 // (vmg_create_batch) and *need receives the bytes one handle needs when slice_bytes is too small (then nothing is created)
+// max_levels > 0 (the patches of the composite solve, vmg_amr.inl): at most that many levels, and no limit on the size of the
+// last one -- such a handle is only smoothed, restricted and prolonged on its first two levels, never solved
 int create_impl(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, double dz, void* cuda_stream,
-                void* slice, size_t slice_bytes, size_t* need)
+                void* slice, size_t slice_bytes, size_t* need, int max_levels = 0)
 {
     if (!out) return VMG_ERR_ARG;
     *out = nullptr;
@@ -186,11 +188,11 @@ int create_impl(vmg_handle* out, int nx, int ny, int nz, double dx, double dy, d
     for (;;) {   // R11: halve while every active dimension is even and stays >= 2
         bool ok = n[0] % 2 == 0 && n[0] / 2 >= 2 && n[1] % 2 == 0 && n[1] / 2 >= 2;
         if (three_d) ok = ok && n[2] % 2 == 0 && n[2] / 2 >= 2;
-        if (!ok) break;
+        if (!ok || (max_levels > 0 && nlev >= max_levels)) break;
         n[0] /= 2; n[1] /= 2; if (three_d) n[2] /= 2;
         ++nlev;
     }
-    if ((long long)n[0] * n[1] * n[2] > 512) return VMG_ERR_SIZE;
+    if (max_levels == 0 && (long long)n[0] * n[1] * n[2] > 512) return VMG_ERR_SIZE;
     vmg_s* h = new (std::nothrow) vmg_s();
     if (!h) return VMG_ERR_ALLOC;
     h->nlev = nlev; h->three_d = three_d;

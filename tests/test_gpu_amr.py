@@ -82,6 +82,7 @@ CASES = [
     dict(n=(48, 40, 1), lo=(8, 6, 0), hi=(32, 26, 1), spacing=None, alpha=1.0),                    # 2-D
     dict(n=(24, 24, 24), lo=(1, 3, 1), hi=(17, 23, 21), spacing=None, alpha=0.0),                  # one cell from the x-low, y-high and z-low faces
     dict(n=(64, 32, 32), lo=(30, 2, 14), hi=(34, 30, 18), spacing=None, alpha=0.0),                # a thin slab of a patch
+    dict(n=(48, 32, 32), lo=(5, 3, 9), hi=(28, 25, 20), spacing=None, alpha=1.0),                  # 23 x 22 x 11 coarse cells: no hierarchy of its own
 ]
 
 
