@@ -168,6 +168,10 @@ int vmg_get_info(vmg_handle h, int* cycles, double* relres, double* history);
  * "phi_keep_cells" (levels with at least this many cells read phi in a colour half-sweep (the neighbours) and in the residual norm with the normal
  *   cache policy instead of the streaming one, default 33554432: on a level whose phi is more than twice the L2 the
  *   evict-first lines are gone before the next row and plane ask for them; results do not depend on it),
+ * "bottom_matrix" (1, default: the single-CTA tail applies the bottom solve -- bottom_sweeps red-black sweeps from a zero field,
+ *   a fixed linear map of the right-hand side -- as that map's matrix, built once per coefficient change by running the sweeps
+ *   on the unit vectors, when the bottom grid has at most 64 cells and the cycle is not the symmetric one; 0: run the sweeps.
+ *   Same map, another rounding order),
  * "restrict_red_cells" (levels with at least this many cells, default 262144, restrict the residuals of the RED children only
  *   in the down-stroke: pre-smoothing ends with a black half-sweep, after which a black cell's residual is its own rounding
  *   error (~2 ulp of D phi, reading R12 of DESIGN.md), so the pass moves 5 instead of 7 doubles per cell; a very large value

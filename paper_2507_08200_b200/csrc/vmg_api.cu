@@ -70,6 +70,8 @@ size_t layout(vmg_s* h, double* base)
     if (base) h->d_scal = base + o;
     o = p.take(8 + kLoopMaxCycles + 1);
     if (base) h->d_loop = base + o;
+    o = p.take((size_t)kBottomMatrixMax * kBottomMatrixMax);
+    if (base) h->bottom_S = base + o;
     return p.off;
 }
 
@@ -136,13 +138,26 @@ int apply_l2_window(vmg_s* h)
     return VMG_OK;
 }
 
+// the bottom grid is small enough for its solve to be kept as a matrix, and there is a bottom to speak of
+bool bottom_matrix_ok(const vmg_s* h)
+{
+    return h->use_bottom_matrix && h->nlev >= 2 && h->lev[h->nlev - 1].n <= kBottomMatrixMax;
+}
+
 int ready(vmg_s* h)
 {
     if (!h) return VMG_ERR_ARG;
     if (!h->have_coeffs || !h->have_bc) return VMG_ERR_STATE;
     prepare_blocked(h);   // once per device, outside any stream capture (every solve / step entry point passes here)
     if (!h->l2_applied) { int rc = apply_l2_window(h); if (rc != VMG_OK) return rc; }
-    if (h->dinv_dirty) return finalize_dinv(h);
+    if (h->dinv_dirty) { int rc = finalize_dinv(h); if (rc != VMG_OK) return rc; }
+    if (h->bottom_dirty && bottom_matrix_ok(h)) {   // the bottom solve as a matrix (vmg_tail.cuh), after 1/D is final
+        const VmgLevel& B = h->lev[h->nlev - 1];
+        bottom_matrix_kernel<<<(unsigned)B.n, kBottomMatrixMax, 0, h->stream>>>(B.wx, B.wy, B.wz, B.dinv, B.G, h->three_d ? 1 : 0, h->nbottom, h->bottom_S);
+        CUDA_TRY(h, cudaGetLastError());
+        h->bottom_dirty = false;
+        ++h->total_launches;
+    }
     return VMG_OK;
 }
 
@@ -425,6 +440,7 @@ int vmg_set_coeffs(vmg_handle h, const double* a, const double* bx, const double
     if (h->profile) prof_collect(h);
     h->have_coeffs = true;
     h->dinv_dirty = !h->have_bc;
+    h->bottom_dirty = true;
     return VMG_OK;
 }
 
@@ -435,7 +451,7 @@ int vmg_set_bc(vmg_handle h, const int type[6], const double* const value[6])
         if (type[f] != VMG_BC_DIRICHLET && type[f] != VMG_BC_NEUMANN) return VMG_ERR_ARG;
     if (!h->have_bc) h->dinv_dirty = true;
     for (int f = 0; f < 6; ++f) {
-        if (h->bctype[f] != type[f]) { ++h->graph_epoch; h->dinv_dirty = true; }   // the trilinear prolongation kernels carry the types by value; 1/D depends on them
+        if (h->bctype[f] != type[f]) { ++h->graph_epoch; h->dinv_dirty = true; h->bottom_dirty = true; }   // the trilinear prolongation kernels carry the types by value; 1/D depends on them
         h->bctype[f] = type[f];
         bool active = f < 4 || h->three_d;
         h->bc_has_value[f] = active && value && value[f];
@@ -499,7 +515,8 @@ int vmg_set_option(vmg_handle h, const char* key, double v)
     int iv = (int)v;
     if (!strcmp(key, "nu1")) { if (iv < 0 || iv > 8) return VMG_ERR_ARG; h->nu1 = iv; }
     else if (!strcmp(key, "nu2")) { if (iv < 0 || iv > 8) return VMG_ERR_ARG; h->nu2 = iv; }
-    else if (!strcmp(key, "bottom_sweeps")) { if (iv < 1) return VMG_ERR_ARG; h->nbottom = iv; }
+    else if (!strcmp(key, "bottom_sweeps")) { if (iv < 1) return VMG_ERR_ARG; h->nbottom = iv; h->bottom_dirty = true; }
+    else if (!strcmp(key, "bottom_matrix")) { h->use_bottom_matrix = iv != 0; h->bottom_dirty = true; }
     else if (!strcmp(key, "prolong")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->prolong = iv; }
     else if (!strcmp(key, "symmetric")) { if (v != 0.0 && v != 1.0) return VMG_ERR_ARG; h->symmetric = iv; }
     else if (!strcmp(key, "const_weights")) { h->const_weights = iv != 0; h->have_coeffs = false; }   // takes effect in vmg_set_coeffs

@@ -115,6 +115,9 @@ struct vmg_s {
     int cl_nc = 0, cl_P = 0;      // cluster size (0: not used) and planes per CTA; tail_level is then the distributed level
     size_t cl_smem = 0;
     long long block_min_cells = 4096;   // smallest level the blocked smoother is used on
+    int use_bottom_matrix = 1;    // option "bottom_matrix": the single-CTA tail applies the bottom solve as a matrix (vmg_tail.cuh bottom_matrix_kernel)
+    double* bottom_S = nullptr;   // that matrix (arena; kBottomMatrixMax squared doubles)
+    bool bottom_dirty = true;     // coefficients, boundary types or bottom_sweeps changed since it was built
     long long restrict_red_cells = 1ll << 18;   // option "restrict_red_cells": levels with at least this many cells restrict the red children's residuals only after a pre-smoothing (vmg_kernels.cuh restrict_one)
     double batch_full_mb = 400.0;  // option "batch_full_mb" (member 0 of a vmg_create_batch group): all levels batched while K fine levels (56 B/cell) stay below this
     // device scalars

@@ -305,6 +305,7 @@ inline void enqueue_tail(vmg_s* h, unsigned long long* norm_out, long long* coun
     g.whole = first == 0;
     g.norm_out = first == 0 ? norm_out : nullptr;
     g.pstride = h->lev[first].pstride;
+    g.S = (h->use_bottom_matrix && h->lev[h->nlev - 1].n <= kBottomMatrixMax && h->nlev >= 2) ? h->bottom_S : nullptr;
     const int ncta = h->lev[first].nprob;
     ProfScope ps(h, VMG_PC_COARSE, count);
     if (clustered) {

@@ -30,7 +30,57 @@ struct TailArgs {
     int whole;                 // 1: lev[0] is level 0 of the hierarchy (phi is an initial guess, not zero)
     unsigned long long* norm_out;   // whole == 1: ||rhs - A phi||_inf bits after the cycle (may be NULL)
     long long pstride;         // batched launch (one CTA per problem): the arrays of problem blockIdx.x lie blockIdx.x * pstride doubles on
+    const double* S;           // the bottom solve as a matrix (bottom_matrix_kernel; NULL: run the sweeps), row-major lev[nl-1].n squared
 };
+
+constexpr int kBottomMatrixMax = 64;   // largest bottom grid (cells) whose solve is kept as a matrix
+
+// R11 says "nbottom red-black sweeps from a zero field": a fixed linear map of the right-hand side.  Column `blockIdx.x` of
+// its matrix = the sweeps run on the unit vector e_col, one thread per cell of the bottom grid (<= 64 cells), the field in
+// shared memory.  Built once per coefficient change (ready() in vmg_api.cu); the tail then replaces 2 nbottom dependent
+// half-sweeps (16 k clk of the single-CTA kernel for the 4 x 2 x 2 bottom of config 3) by n fused multiply-adds per cell.
+// Same map, different rounding order than the sweeps (the oracle runs the sweeps): covered by the 1e-10 / 1e-6 bars.
+__global__ void bottom_matrix_kernel(const double* __restrict__ wx, const double* __restrict__ wy, const double* __restrict__ wz,
+                                     const double* __restrict__ dinv, Geom G, int three_d, int nbottom, double* __restrict__ S)
+{
+    __shared__ double phi[kBottomMatrixMax];
+    const int n = (int)G.n, t = threadIdx.x, col = blockIdx.x;
+    int i = 0, j = 0, k = 0;
+    double w[6] = {0, 0, 0, 0, 0, 0}, di = 0.0;
+    int nb[6] = {0, 0, 0, 0, 0, 0};
+    if (t < n) {
+        i = t % G.nx; j = (t / G.nx) % G.ny; k = t / (G.nx * G.ny);
+        const long long c = cell_at(G, i, j, k);
+        di = dinv[c];
+        // a face on the domain boundary carries a zero weight in the internal arrays (vmg_internal.h); the high faces are the
+        // low faces of the neighbours
+        if (i > 0)        { w[0] = wx[c];                        nb[0] = t - 1; }
+        if (i < G.nx - 1) { w[1] = wx[cell_at(G, i + 1, j, k)];  nb[1] = t + 1; }
+        if (j > 0)        { w[2] = wy[c];                        nb[2] = t - G.nx; }
+        if (j < G.ny - 1) { w[3] = wy[cell_at(G, i, j + 1, k)];  nb[3] = t + G.nx; }
+        if (three_d) {
+            if (k > 0)        { w[4] = wz[c];                       nb[4] = t - G.nx * G.ny; }
+            if (k < G.nz - 1) { w[5] = wz[cell_at(G, i, j, k + 1)]; nb[5] = t + G.nx * G.ny; }
+        }
+        phi[t] = 0.0;
+    }
+    const double rhs = t == col ? 1.0 : 0.0;
+    __syncthreads();
+    for (int s = 0; s < nbottom; ++s)
+        for (int colour = 0; colour < 2; ++colour) {
+            if (t < n && ((i + j + k) & 1) == colour) {
+                double v = w[0] * phi[nb[0]];
+                v = fma(w[1], phi[nb[1]], v);
+                v = fma(w[2], phi[nb[2]], v);
+                v = fma(w[3], phi[nb[3]], v);
+                v = fma(w[4], phi[nb[4]], v);
+                v = fma(w[5], phi[nb[5]], v);
+                phi[t] = di * (rhs + v);
+            }
+            __syncthreads();
+        }
+    if (t < n) S[(long long)t * n + col] = phi[t];
+}
 
 // shared-memory block of a level: six arrays (phi, rhs, dinv, wx, wy, wz), each `guard` zeroed doubles, n cells,
 // `guard` zeroed doubles; guard >= zs + nx + 2 so that every stencil neighbour of every cell is addressable
@@ -220,7 +270,15 @@ __device__ __forceinline__ void coarse_tail_body(const TailArgs& g, const long l
             for (int t = tid; t < B.n; t += nth) s.phi[t] = 0.0;
             __syncthreads();
         }
-        if (!g.sym) tail_smooth(s, B, g.nbottom);
+        if (g.S && !g.sym && !(g.nl == 1 && g.whole)) {   // the sweeps from zero as a matrix (bottom_matrix_kernel)
+            const double* S = g.S + off;
+            double acc = 0.0;
+            if (tid < B.n)
+                for (int j = 0; j < B.n; ++j) acc = fma(S[tid * B.n + j], s.rhs[j], acc);
+            if (tid < B.n) s.phi[tid] = acc;
+            __syncthreads();
+        }
+        else if (!g.sym) tail_smooth(s, B, g.nbottom);
         else { tail_smooth(s, B, g.nbottom / 2, 0); tail_smooth(s, B, g.nbottom - g.nbottom / 2, 1); }
     }
     TAIL_MARK(20);

@@ -1102,3 +1102,39 @@ def test_red_only_restriction_after_presmoothing_is_the_full_restriction_to_roun
         assert abs(x - y) <= 1e-9 * y + 2e-15
     phi_o, st_o, cyc_o, rr_o, _ = Oracle.from_problem(p).solve(p.rhs, rtol=p.rtol, max_vcycles=p.max_vcycles)
     assert cyc_o == info_r[0] and rel(phi_r, phi_o) <= PHI_TOL
+
+
+@pytest.mark.parametrize("dims", [(64, 32, 32), (48, 40, 1), (40, 24, 16)])
+def test_bottom_solve_as_a_matrix_is_the_sweeps_to_rounding(dims):
+    """Option bottom_matrix (default on): the single-CTA tail applies the nbottom sweeps from zero as the matrix of that linear
+    map (built once per coefficient change by running the sweeps on the unit vectors).  Same map, another rounding order:
+    cycle counts equal, histories and phi equal to rounding -- against the sweeps and against the oracle (which sweeps)."""
+    b = _binding()
+    p = inputs.random_problem(*dims, seed=17, bc_type=MIXED, sigma=1.5)
+    out = {}
+    for bm in (1, 0):
+        s, d = b.from_problem(p)
+        s.set_option("bottom_matrix", bm)
+        phi = torch.zeros_like(d["rhs"])
+        assert s.solve(d["rhs"], phi, rtol=1e-12, max_vcycles=50) == 0
+        out[bm] = (phi.cpu().numpy(), s.get_info())
+        # new coefficients on the same handle: the matrix is rebuilt
+        q = inputs.random_problem(*dims, seed=18, bc_type=MIXED, sigma=1.5)
+        dq = b.upload(q)
+        s.set_coeffs(dq["a"], dq["bx"], dq["by"], dq["bz"], q.alpha, q.beta)
+        s.set_bc(q.bc_type, dq["bc_value"])
+        phi2 = torch.zeros_like(dq["rhs"])
+        assert s.solve(dq["rhs"], phi2, rtol=1e-12, max_vcycles=50) == 0
+        out[(bm, 2)] = (phi2.cpu().numpy(), s.get_info(), q)
+        s.destroy()
+    for key in (1, (1, 2)):
+        ref = out[0] if key == 1 else out[(0, 2)]
+        got = out[key]
+        assert got[1][0] == ref[1][0] and rel(got[0], ref[0]) <= 1e-12
+        for x, y in zip(got[1][2], ref[1][2]):
+            assert abs(x - y) <= 1e-9 * y + 2e-15
+    phi_o, st_o, cyc_o, rr_o, _ = Oracle.from_problem(p).solve(p.rhs, rtol=1e-12, max_vcycles=50)
+    assert cyc_o == out[1][1][0] and rel(out[1][0], phi_o) <= PHI_TOL
+    q = out[(1, 2)][2]
+    phi_o, st_o, cyc_o, rr_o, _ = Oracle.from_problem(q).solve(q.rhs, rtol=1e-12, max_vcycles=50)
+    assert cyc_o == out[(1, 2)][1][0] and rel(out[(1, 2)][0], phi_o) <= PHI_TOL
