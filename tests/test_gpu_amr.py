@@ -199,3 +199,11 @@ def test_streamer_patch_at_full_size_against_the_oracle():
     o, s = _oracle(p), _gpu(p)
     pc, pf, cyc, hist = _compare(p, s, o, max_cycles=30)
     assert hist[-1] <= 1e-12 and cyc <= 14
+
+
+def test_three_streamer_patches_at_full_size_against_the_oracle():
+    """bench.py's amr.three_patches workload: the 256 x 128 x 128 box + three 128 x 64 x 64 patches (parallel graph branches)."""
+    p = inputs.amr_streamers(128)
+    o, s = _oracle(p), _gpu(p)
+    pc, pf, cyc, hist = _compare(p, s, o, max_cycles=30)
+    assert hist[-1] <= 1e-12 and cyc <= 14 and s.pad_check() == 0
